@@ -1,0 +1,88 @@
+"""Pins for the oracle's Re w(x+iy) (oracle/hk_oracle.c: hko_voigt_K) against
+things other than itself: numerical quadrature of the Gauss-Lorentz convolution
+(Eq. 1-2, L65-77 define the Voigt profile as that convolution),
+erfcx on the imaginary axis, the Gaussian and Lorentzian limits, the asymptotic
+series, symmetry, and scipy's wofz (the routine the paper itself compares with,
+L146) as a third opinion."""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate, special
+
+from oracle import hk_oracle as O
+
+
+def _quad_K(x, y):
+    f = lambda t: math.exp(-t * t) / ((x - t) ** 2 + y * y)
+    pts = sorted({x, x - y, x + y, x - 5 * y, x + 5 * y, 0.0, -3.0, 3.0})
+    pts = [p for p in pts if -12.0 < p < max(12.0, x + 40 * y)]
+    lo, hi = -12.0, 12.0
+    val, _ = integrate.quad(f, lo, hi, points=pts, epsabs=0.0, epsrel=1e-12, limit=2000)
+    return y / math.pi * val
+
+
+@pytest.mark.parametrize("x", [0.0, 0.3, 1.0, 2.5, 5.0, 8.25, 11.0])
+@pytest.mark.parametrize("y", [0.05, 0.3, 1.0, 3.0, 10.0])
+def test_against_quadrature(x, y):
+    ref = _quad_K(x, y)
+    got = float(O.voigt_K(x, y))
+    assert got == pytest.approx(ref, rel=2e-10)
+
+
+def test_imaginary_axis_erfcx():
+    y = np.array([1e-3, 0.01, 0.1, 0.5, 1.0, 2.0, 5.0, 20.0, 300.0])
+    got = O.voigt_K(np.zeros_like(y), y)
+    np.testing.assert_allclose(got, special.erfcx(y), rtol=2e-13)
+    # the value quoted in SURVEY.md 8(c): K(0,1) = e * erfc(1)
+    assert float(O.voigt_K(0.0, 1.0)) == pytest.approx(math.e * math.erfc(1.0), rel=1e-14)
+    assert float(O.voigt_K(0.0, 1.0)) == pytest.approx(0.427583576155807, rel=1e-14)
+
+
+def test_gaussian_limit():
+    x = np.array([0.0, 0.2, 0.77, 1.3, 2.6, 3.9])          # off the h=1/2 nodes and on them
+    np.testing.assert_allclose(O.voigt_K(x, np.zeros_like(x)), np.exp(-x * x), rtol=1e-15)
+    # y -> 0+: K -> exp(-x^2) + O(y); first-order term is -(2y/sqrt(pi)) (1 - 2 x D(x))
+    y = 1e-7
+    lin = -2.0 * y / math.sqrt(math.pi) * (1.0 - 2.0 * x * special.dawsn(x))
+    np.testing.assert_allclose(O.voigt_K(x, np.full_like(x, y)), np.exp(-x * x) + lin, rtol=2e-9)
+
+
+def test_lorentzian_limit_and_asymptotic_series():
+    # |z| -> inf: K -> y/(sqrt(pi)|z|^2) (1 + (3x^2-y^2)/(2|z|^4))
+    for x, y in [(300.0, 0.5), (1e4, 2.0), (50.0, 400.0), (0.0, 1e3), (1e6, 1e-2), (2e3, 2e3)]:
+        r2 = x * x + y * y
+        lead = y / (math.sqrt(math.pi) * r2)
+        two = lead * (1.0 + (3 * x * x - y * y) / (2 * r2 * r2))
+        got = float(O.voigt_K(x, y))
+        assert abs(got / lead - 1.0) < 1.6 / r2
+        assert abs(got / two - 1.0) < 4.0 / r2 ** 2 + 1e-13
+
+
+def test_symmetry_and_positivity():
+    rng = np.random.default_rng(1)
+    x = rng.uniform(0, 30, 2000)
+    y = 10.0 ** rng.uniform(-3, 2, 2000)
+    a = O.voigt_K(x, y)
+    b = O.voigt_K(-x, y)
+    np.testing.assert_allclose(a, b, rtol=1e-13)       # summation order differs, value does not
+    assert np.all(a > 0) and np.all(a <= 1.0)
+
+
+def test_third_opinion_wofz_lattice():
+    x = np.concatenate([[0.0], 10.0 ** np.linspace(-3, 7, 161)])
+    y = 10.0 ** np.linspace(-3, 7, 121)
+    X, Y = np.meshgrid(x, y)
+    ref = special.wofz(X + 1j * Y).real
+    got = O.voigt_K(X, Y)
+    rel = np.abs(got / ref - 1.0)
+    assert rel.max() < 5e-12, (rel.max(), X.flat[rel.argmax()], Y.flat[rel.argmax()])
+
+
+def test_small_y_on_nodes_documented_limit():
+    # header of hk_oracle.c: relative accuracy ~1e-16 * h/(pi y) when x sits on a node
+    x = np.array([0.5, 1.0, 2.0, 3.5])
+    for y in (1e-2, 1e-4, 1e-6):
+        ref = special.wofz(x + 1j * y).real
+        got = O.voigt_K(x, np.full_like(x, y))
+        np.testing.assert_allclose(got, ref, rtol=4e-16 / y + 1e-13)
