@@ -1,0 +1,133 @@
+/*
+ * hk.h -- C ABI of the B200-native line-by-line opacity library
+ * (hot path of HELIOS-K 2.0, arxiv 2101.02005; citations are PAPER.md lines).
+ *
+ * What the library computes:
+ *
+ *   k(nu_i) = sum over lines l with i_lo(l) <= i <= i_hi(l) of S_l * V_l(nu_i)
+ *
+ *   nu_i    = numin + i*dnu, i = 0..N-1, N = floor((numax-numin)/dnu + 0.5)   (Eq. 14)
+ *   V_l     = Re w(x + i y) / (alpha_D sqrt(pi)),  x = (nu_i-nu0)/alpha_D, y = Gamma_L/alpha_D
+ *                                                              (Eq. 1-2, Eq. 11-12)
+ *   alpha_D = (nu0/c) sqrt(2 k_B T / m)                                      (Eq. 3, Eq. 13)
+ *   Gamma_L = A/(4 pi c) + gamma_ref (T_ref/T)^n_exp (P/P_ref)               (Eq. 5)
+ *   S_l     = A g'/(8 pi c m nu0^2 Q) exp(-c2 E''/T) (1 - exp(-c2 nu0/T))    (Eq. 9)
+ *   cut     : fixed cutting length from the line centre (L239, L262), or none (atoms, L7)
+ *
+ * Units: cm^-1, K, atm, amu, s^-1; gamma_ref in cm^-1/atm at T_ref = 296 K,
+ * P_ref = 1 atm; output cm^2 g^-1.  Constants: CODATA 2018 (c as printed at L129).
+ *
+ * All line arrays, the output and the workspace are DEVICE pointers owned by
+ * the caller (PyTorch tensors in the Python binding).  The library owns only
+ * the small host handle.  Inputs are never modified.  Every entry point returns
+ * 0 on success or a negative hk_status; nothing throws, aborts or prints.
+ * A context is not thread-safe.  There is no CPU fallback.
+ */
+#ifndef HK_H
+#define HK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hk_ctx hk_ctx; /* opaque; one per grid */
+
+typedef enum {
+    HK_OK = 0,
+    HK_EINVAL = -1, /* bad scalar, null pointer, n_lines < 0, N >= 2^31 - 2^12 */
+    HK_ESTATE = -2, /* compute before conditions / workspace; get_* before a compute */
+    HK_ENOSPC = -3, /* workspace smaller than hk_workspace_bytes() */
+    HK_ECUDA = -4,  /* a CUDA call failed; raw code from hk_last_cuda_error() */
+    HK_ENOMEM = -5  /* host allocation of the handle failed */
+} hk_status;
+
+/* Six SoA fp64 DEVICE arrays of n_lines elements each, read-only.
+ * g_up holds integer values stored as fp64 (R18). */
+typedef struct {
+    const double* nu0;       /* line centre, cm^-1 */
+    const double* A;         /* Einstein A, s^-1 */
+    const double* g_up;      /* upper-state degeneracy g' */
+    const double* E_low;     /* lower-state energy E'', cm^-1 */
+    const double* gamma_ref; /* pressure-broadening coefficient at T_ref, cm^-1/atm */
+    const double* n_exp;     /* temperature exponent n */
+} hk_lines;
+
+/* Exact integer work counts of the last hk_compute plus bookkeeping. */
+typedef struct {
+    int64_t n_lines;       /* as passed */
+    int64_t n_skipped;     /* nu0 <= 0, A < 0 or a non-finite field: contribute nothing (R14) */
+    int64_t n_off_grid;    /* valid lines whose extent misses the grid (or > 2^30 bins away) */
+    int64_t n_evals;       /* sum over lines of (i_hi - i_lo + 1): Voigt evaluations */
+    int64_t n_evals_far;   /* of those, |z|^2 >= HK_Z1 (1-term asymptotic = Lorentzian) */
+    int64_t n_evals_mid;   /* HK_Z2 <= |z|^2 < HK_Z1 (2-term asymptotic) */
+    int64_t n_evals_core;  /* |z|^2 < HK_Z2 (trapezoid + pole term) */
+    int64_t n_units_far;   /* (tile, line-chunk) work units run by the far kernel */
+    int64_t n_units_near;  /* ... by the near/edge kernel */
+    int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
+    int32_t sort_bits;     /* radix-sort key width used */
+} hk_stats;
+
+/* Region thresholds on |z|^2 = x^2 + y^2 used by the fp32 evaluator. */
+#define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */
+#define HK_Z2 625.0f   /* |z| >= 25 : two asymptotic terms, relative error <= 1.0e-5 */
+
+/* Grid: bin i is the POINT nu_i = numin + i*dnu (R8, R9).  HK_EINVAL if dnu <= 0,
+ * numax <= numin, a non-finite argument, N < 1 or N too large. */
+int hk_create(double numin, double numax, double dnu, hk_ctx** out);
+int hk_destroy(hk_ctx* ctx);
+int64_t hk_grid_size(const hk_ctx* ctx);
+
+/* T in K, P in atm, molecular/atomic mass in amu, partition function Q(T) as a
+ * scalar (Eq. 10 is evaluated by the caller, L234).  HK_EINVAL unless T, mass, Q > 0,
+ * P >= 0, all finite. */
+int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, double Q);
+
+/* Device scratch the caller must provide for hk_compute with up to n_lines lines. */
+size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines);
+int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
+
+/* Enqueue the whole hot path on `stream` (a cudaStream_t passed as void*; NULL is
+ * the legacy default stream): preprocess -> bucket/sort -> tile ranges -> far and
+ * near accumulation kernels -> k in out_k_dev.  out_k_dev (N doubles) is
+ * OVERWRITTEN.  cut_cm > 0 and finite: fixed cutting length from the centre,
+ * inclusive integer extent (R7); cut_cm <= 0 or +inf: uncut.  Lines need not be
+ * sorted.  n_lines == 0 is valid (k = 0).  Returns after enqueueing, without
+ * synchronising; every buffer must stay alive until the stream drains. */
+int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
+               double* out_k_dev, void* stream);
+
+/* Integer extents of the lines of the LAST hk_compute, in the caller's line order
+ * (int32 DEVICE arrays of n_lines; skipped / off-grid lines get ilo = 0, ihi = -1,
+ * jc as computed (0 for skipped)).  Any pointer may be NULL.  Synchronises. */
+int hk_get_extents(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, int32_t* ilo_dev,
+                   int32_t* ihi_dev, int32_t* jc_dev, void* stream);
+
+/* Per-line fp64 parameters as the preprocess kernel computes them (S, Gamma_L,
+ * alpha_D; zeros for skipped lines): parity of step a1.  DEVICE arrays, may be NULL. */
+int hk_get_line_params(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double* S_dev,
+                       double* gammaL_dev, double* alphaD_dev, void* stream);
+
+/* Counts of the last hk_compute.  Synchronises the stream it ran on. */
+int hk_get_stats(hk_ctx* ctx, hk_stats* host_out);
+
+/* Accuracy probe for the shipped fp32 evaluator (the counterpart of the paper's
+ * Fig. 4): out[i] = Re w(x[i] + i y[i]) exactly as the accumulation
+ * kernels evaluate it (region chosen by |z|^2 with alpha_D = 1 bin).  DEVICE fp32
+ * arrays of n.  region_out (optional, int32): 0 far, 1 mid, 2 core. */
+int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev,
+                      int32_t* region_out_dev, void* stream);
+
+/* Tuning knob for tests and sweeps: force every (tile, line) pair through the
+ * near/edge kernel (mode 1) or restore the default split (mode 0). */
+int hk_set_debug_mode(hk_ctx* ctx, int mode);
+
+int hk_last_cuda_error(const hk_ctx* ctx);
+const char* hk_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HK_H */

@@ -1,0 +1,176 @@
+"""Thin ctypes binding of include/hk.h: argument marshalling only.
+
+Every step of the hot path runs in the CUDA library (csrc/); PyTorch is used for
+device memory and streams.  There is no CPU fallback: if libhk.so is missing or
+cannot be loaded, importing this module raises.
+"""
+import ctypes as C
+import math
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhk.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} not found: build the CUDA library first "
+        "(python -m paper_2101_02005_b200.build, or __graft_entry__.build()); there is no CPU fallback")
+_lib = C.CDLL(LIB_PATH)
+
+HK_OK, HK_EINVAL, HK_ESTATE, HK_ENOSPC, HK_ECUDA, HK_ENOMEM = 0, -1, -2, -3, -4, -5
+HK_Z1, HK_Z2 = 90000.0, 625.0
+FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
+
+EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
+           "hk_set_workspace", "hk_compute", "hk_get_extents", "hk_get_line_params", "hk_get_stats",
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_last_cuda_error", "hk_strerror")
+
+
+class hk_lines(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in FIELDS]
+
+
+class hk_stats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("n_lines", "n_skipped", "n_off_grid", "n_evals", "n_evals_far",
+                                         "n_evals_mid", "n_evals_core", "n_units_far", "n_units_near")] + \
+               [("scale_exp", C.c_int32), ("sort_bits", C.c_int32)]
+
+
+_vp, _d, _i64 = C.c_void_p, C.c_double, C.c_int64
+_lib.hk_create.argtypes = [_d, _d, _d, C.POINTER(_vp)]
+_lib.hk_destroy.argtypes = [_vp]
+_lib.hk_grid_size.argtypes = [_vp]
+_lib.hk_grid_size.restype = _i64
+_lib.hk_set_conditions.argtypes = [_vp, _d, _d, _d, _d]
+_lib.hk_workspace_bytes.argtypes = [_vp, _i64]
+_lib.hk_workspace_bytes.restype = C.c_size_t
+_lib.hk_set_workspace.argtypes = [_vp, _vp, C.c_size_t]
+_lib.hk_compute.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
+_lib.hk_get_extents.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _vp, _vp]
+_lib.hk_get_line_params.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _vp, _vp]
+_lib.hk_get_stats.argtypes = [_vp, C.POINTER(hk_stats)]
+_lib.hk_eval_voigt_f32.argtypes = [_vp, _vp, _i64, _vp, _vp, _vp]
+_lib.hk_set_debug_mode.argtypes = [_vp, C.c_int]
+_lib.hk_last_cuda_error.argtypes = [_vp]
+_lib.hk_strerror.argtypes = [C.c_int]
+_lib.hk_strerror.restype = C.c_char_p
+for _name in ("hk_create", "hk_destroy", "hk_set_conditions", "hk_set_workspace", "hk_compute", "hk_get_extents",
+              "hk_get_line_params", "hk_get_stats", "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_last_cuda_error"):
+    getattr(_lib, _name).restype = C.c_int
+
+
+class HKError(RuntimeError):
+    def __init__(self, status, where, cuda_err=0):
+        self.status = status
+        msg = _lib.hk_strerror(status).decode()
+        super().__init__(f"{where}: {msg} (status {status}, cuda error {cuda_err})")
+
+
+def hk_strerror(status: int) -> str:
+    return _lib.hk_strerror(status).decode()
+
+
+def _stream_ptr(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _lines_struct(lines):
+    ls = hk_lines()
+    n = None
+    for k in FIELDS:
+        t = lines[k]
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError(f"lines[{k!r}] must be a contiguous CUDA float64 tensor")
+        if n is None:
+            n = t.numel()
+        elif t.numel() != n:
+            raise ValueError("line arrays differ in length")
+        setattr(ls, k, t.data_ptr())
+    return ls, n
+
+
+class Opacity:
+    """One grid (hk_create) + conditions + a torch-owned workspace; call compute()."""
+
+    def __init__(self, numin: float, numax: float, dnu: float):
+        self._ctx = _vp()
+        st = _lib.hk_create(numin, numax, dnu, C.byref(self._ctx))
+        if st != HK_OK:
+            self._ctx = None
+            raise HKError(st, "hk_create")
+        self.N = int(_lib.hk_grid_size(self._ctx))
+        self._ws = None
+
+    def _check(self, st, where):
+        if st != HK_OK:
+            raise HKError(st, where, _lib.hk_last_cuda_error(self._ctx))
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            _lib.hk_destroy(self._ctx)
+            self._ctx = None
+
+    __del__ = close
+
+    def set_conditions(self, T, P_atm, mass_amu, Q):
+        self._check(_lib.hk_set_conditions(self._ctx, T, P_atm, mass_amu, Q), "hk_set_conditions")
+
+    def set_debug_mode(self, mode: int):
+        self._check(_lib.hk_set_debug_mode(self._ctx, mode), "hk_set_debug_mode")
+
+    def workspace_bytes(self, n_lines: int) -> int:
+        return int(_lib.hk_workspace_bytes(self._ctx, n_lines))
+
+    def ensure_workspace(self, n_lines: int):
+        need = self.workspace_bytes(n_lines)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+            self._check(_lib.hk_set_workspace(self._ctx, self._ws.data_ptr(), self._ws.numel()), "hk_set_workspace")
+
+    def compute(self, lines, cut, out=None, stream=None):
+        """Enqueue lines -> k(nu) on the current (or given) torch stream; returns the fp64 CUDA tensor."""
+        ls, n = _lines_struct(lines)
+        self.ensure_workspace(n)
+        if out is None:
+            out = torch.empty(self.N, dtype=torch.float64, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.N
+        cut = float(cut) if cut is not None else 0.0
+        self._check(_lib.hk_compute(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)), "hk_compute")
+        return out
+
+    def extents(self, lines, stream=None):
+        ls, n = _lines_struct(lines)
+        ilo, ihi, jc = (torch.empty(n, dtype=torch.int32, device="cuda") for _ in range(3))
+        self._check(_lib.hk_get_extents(self._ctx, C.byref(ls), n, ilo.data_ptr(), ihi.data_ptr(), jc.data_ptr(),
+                                        _stream_ptr(stream)), "hk_get_extents")
+        return ilo, ihi, jc
+
+    def line_params(self, lines, stream=None):
+        ls, n = _lines_struct(lines)
+        S, gL, aD = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+        self._check(_lib.hk_get_line_params(self._ctx, C.byref(ls), n, S.data_ptr(), gL.data_ptr(), aD.data_ptr(),
+                                            _stream_ptr(stream)), "hk_get_line_params")
+        return S, gL, aD
+
+    def stats(self) -> dict:
+        s = hk_stats()
+        self._check(_lib.hk_get_stats(self._ctx, C.byref(s)), "hk_get_stats")
+        return {k: int(getattr(s, k)) for k, _ in hk_stats._fields_}
+
+
+def eval_voigt_f32(x: torch.Tensor, y: torch.Tensor, with_region=False, stream=None):
+    """Re w(x + i y) through the shipped fp32 evaluator (accuracy probe, hk_eval_voigt_f32)."""
+    assert x.is_cuda and y.is_cuda and x.dtype == torch.float32 and y.dtype == torch.float32
+    x = x.contiguous()
+    y = y.contiguous()
+    out = torch.empty_like(x)
+    reg = torch.empty(x.shape, dtype=torch.int32, device=x.device) if with_region else None
+    st = _lib.hk_eval_voigt_f32(x.data_ptr(), y.data_ptr(), x.numel(), out.data_ptr(),
+                                reg.data_ptr() if with_region else None, _stream_ptr(stream))
+    if st != HK_OK:
+        raise HKError(st, "hk_eval_voigt_f32")
+    return (out, reg) if with_region else out

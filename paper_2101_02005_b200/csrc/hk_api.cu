@@ -1,0 +1,395 @@
+// hk_api.cu -- host side of the C ABI in include/hk.h: argument checks, workspace
+// layout, and the enqueue of the whole hot path on the caller's stream.  No host
+// synchronisation inside hk_compute: launch shapes do not depend on device results
+// (persistent grids pull work units from a device-computed list).
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "hk_accumulate.cuh"
+
+using namespace hk;
+
+struct hk_ctx {
+    double numin, numax, dnu;
+    int64_t N;
+    bool have_cond;
+    double T, P_atm, mass_amu, Q;
+    void* ws;
+    size_t ws_bytes;
+    int cuda_err;
+    int debug_mode;
+    int n_sm, occ_far, occ_near;
+    // last compute
+    bool have_run;
+    int64_t last_n;
+    double last_cut;
+    cudaStream_t last_stream;
+    int32_t last_sort_bits;
+    DevStats* d_stats;
+};
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, tr, counts, prefix, cub;
+    size_t cub_bytes, total;
+    int32_t n_wt, n_ct;
+};
+
+bool is_uncut(double cut) { return !(cut > 0.0 && std::isfinite(cut)); }
+
+size_t cub_temp_bytes(int64_t n, int32_t n_ct)
+{
+    size_t b1 = 0, b2 = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, b1, (const int32_t*)nullptr, (int32_t*)nullptr, (const int32_t*)nullptr,
+                                    (int32_t*)nullptr, (int)n, 0, 32, (cudaStream_t)0);
+    cub::DeviceScan::ExclusiveSum(nullptr, b2, (const int32_t*)nullptr, (int32_t*)nullptr, (int)(n_ct + 1),
+                                  (cudaStream_t)0);
+    return b1 > b2 ? b1 : b2;
+}
+
+Layout make_layout(const hk_ctx* c, int64_t n)
+{
+    Layout L;
+    L.n_wt = (int32_t)((c->N + kWarpBins - 1) / kWarpBins);
+    L.n_ct = (int32_t)((c->N + kTileBins - 1) / kTileBins);
+    size_t nn = (size_t)(n > 0 ? n : 1);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+    L.stats = take(sizeof(DevStats));
+    L.keys_in = take(nn * 4);
+    L.keys_out = take(nn * 4);
+    L.idx_in = take(nn * 4);
+    L.idx_out = take(nn * 4);
+    L.recU = take(nn * sizeof(RecU));
+    L.recA = take(nn * 16);
+    L.recB = take(nn * 16);
+    L.tr = take((size_t)L.n_wt * sizeof(TileRange));
+    L.counts = take(((size_t)L.n_ct + 1) * 4);
+    L.prefix = take(((size_t)L.n_ct + 1) * 4);
+    L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_ct);
+    L.cub = take(L.cub_bytes);
+    L.total = off;
+    return L;
+}
+
+int fail_cuda(hk_ctx* c, cudaError_t e)
+{
+    if (c) c->cuda_err = (int)e;
+    return HK_ECUDA;
+}
+
+#define HK_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e__ = (call);                       \
+        if (e__ != cudaSuccess) return fail_cuda(ctx, e__); \
+    } while (0)
+
+// Fill the per-launch constants (step a0).
+Params make_params(const hk_ctx* c, double cut, int32_t chunk)
+{
+    Params p;
+    std::memset(&p, 0, sizeof(p));
+    p.numin = c->numin;
+    p.dnu = c->dnu;
+    p.N = c->N;
+    const double m = c->mass_amu / kNA;                        // grams (L83)
+    p.c2_over_T = kH * kC / kKB / c->T;
+    p.tfac = kTref / c->T;
+    p.P_atm = c->P_atm;
+    p.beta = std::sqrt(2.0 * kKB * c->T / m) / kC;
+    p.sfac = 1.0 / (8.0 * kPi * kC * m * c->Q);
+    p.inv4pic = 1.0 / (4.0 * kPi * kC);
+    p.uncut = is_uncut(cut) ? 1 : 0;
+    p.cut = p.uncut ? 0.0 : cut;
+    double cb = p.uncut ? 0.0 : cut / c->dnu;
+    bool compact = !p.uncut && cb < 268435456.0 && (double)c->N + 2.0 * std::ceil(cb) + 8.0 < 2147483647.0;
+    p.cb_floor = p.uncut ? 0 : (int64_t)std::fmin(std::floor(cb), 4.0e18);
+    p.cb_ceil = p.uncut ? 0 : (int64_t)std::fmin(std::ceil(cb), 4.0e18);
+    if (compact) {
+        p.kmin = -(p.cb_ceil + 2);
+        p.ksent = (int32_t)(c->N + 2 * p.cb_ceil + 6);
+    } else {
+        p.kmin = -(1LL << 30);
+        p.ksent = INT32_MAX;
+    }
+    p.kappa = std::sqrt((double)HK_Z1) * p.beta * 1.001;
+    p.numin_bins = c->numin / c->dnu;
+    p.n_wt = (int32_t)((c->N + kWarpBins - 1) / kWarpBins);
+    p.n_ct = (int32_t)((c->N + kTileBins - 1) / kTileBins);
+    p.chunk = chunk;
+    p.force_near = c->debug_mode == 1;
+    return p;
+}
+
+int32_t pick_chunk(const hk_ctx* c, int64_t n, double cut)
+{
+    double tiles_per_line = is_uncut(cut) ? (double)((c->N + kTileBins - 1) / kTileBins)
+                                          : std::fmin(2.0 * cut / c->dnu / kTileBins + 1.0,
+                                                      (double)((c->N + kTileBins - 1) / kTileBins));
+    double pairs = (double)n * tiles_per_line;
+    double want = pairs / ((double)c->n_sm * 32.0);
+    int64_t ch = (int64_t)std::ceil(want / 256.0) * 256;
+    if (ch < 512) ch = 512;
+    if (ch > 32768) ch = 32768;
+    return (int32_t)ch;
+}
+
+int bits_for(uint32_t v)
+{
+    int b = 1;
+    while (b < 32 && (v >> b) != 0) ++b;
+    return b;
+}
+
+__global__ void __launch_bounds__(256) extents_kernel(Params p, const double* __restrict__ nu0, const double* __restrict__ A,
+                                                      const double* __restrict__ g, const double* __restrict__ E,
+                                                      const double* __restrict__ gam, const double* __restrict__ nx,
+                                                      int64_t n, int32_t* ilo, int32_t* ihi, int32_t* jc, double* S,
+                                                      double* gL, double* aD)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        LineOut o = line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
+        bool live = o.valid && o.ilo <= o.ihi;
+        if (ilo) ilo[i] = live ? (int32_t)o.ilo : 0;
+        if (ihi) ihi[i] = live ? (int32_t)o.ihi : -1;
+        if (jc) jc[i] = o.valid ? (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN) : 0;
+        if (S) S[i] = o.S;
+        if (gL) gL[i] = o.gammaL;
+        if (aD) aD[i] = o.alphaD;
+    }
+}
+
+bool lines_ok(const hk_lines* l)
+{
+    return l && l->nu0 && l->A && l->g_up && l->E_low && l->gamma_ref && l->n_exp;
+}
+
+int grid_for(const hk_ctx* c, int64_t n)
+{
+    int64_t blocks = (n + 255) / 256;
+    int64_t cap = (int64_t)c->n_sm * 16;
+    return (int)(blocks < 1 ? 1 : (blocks > cap ? cap : blocks));
+}
+
+}  // namespace
+
+extern "C" {
+
+int hk_create(double numin, double numax, double dnu, hk_ctx** out)
+{
+    if (!out) return HK_EINVAL;
+    *out = nullptr;
+    if (!std::isfinite(numin) || !std::isfinite(numax) || !std::isfinite(dnu)) return HK_EINVAL;
+    if (!(dnu > 0.0) || !(numax > numin)) return HK_EINVAL;
+    double Nd = std::floor((numax - numin) / dnu + 0.5);
+    if (!(Nd >= 1.0) || Nd >= 2147483648.0 - 4096.0) return HK_EINVAL;
+    hk_ctx* c = new (std::nothrow) hk_ctx;
+    if (!c) return HK_ENOMEM;
+    std::memset(c, 0, sizeof(*c));
+    c->numin = numin; c->numax = numax; c->dnu = dnu; c->N = (int64_t)Nd;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_far, far_kernel, kThreads, 0);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_near, near_kernel, kThreads, 0);
+    if (e != cudaSuccess) { delete c; return HK_ECUDA; }
+    if (c->occ_far < 1) c->occ_far = 1;
+    if (c->occ_near < 1) c->occ_near = 1;
+    *out = c;
+    return HK_OK;
+}
+
+int hk_destroy(hk_ctx* ctx)
+{
+    delete ctx;
+    return HK_OK;
+}
+
+int64_t hk_grid_size(const hk_ctx* ctx) { return ctx ? ctx->N : (int64_t)HK_EINVAL; }
+
+int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, double Q)
+{
+    if (!ctx) return HK_EINVAL;
+    if (!std::isfinite(T_K) || !std::isfinite(P_atm) || !std::isfinite(mass_amu) || !std::isfinite(Q)) return HK_EINVAL;
+    if (!(T_K > 0.0) || !(P_atm >= 0.0) || !(mass_amu > 0.0) || !(Q > 0.0)) return HK_EINVAL;
+    ctx->T = T_K; ctx->P_atm = P_atm; ctx->mass_amu = mass_amu; ctx->Q = Q;
+    ctx->have_cond = true;
+    return HK_OK;
+}
+
+size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines)
+{
+    if (!ctx || n_lines < 0 || n_lines >= 2147483647LL) return 0;
+    return make_layout(ctx, n_lines).total;
+}
+
+int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes)
+{
+    if (!ctx || (!dev_ptr && bytes)) return HK_EINVAL;
+    if (((uintptr_t)dev_ptr & 255u) != 0) return HK_EINVAL;
+    ctx->ws = dev_ptr;
+    ctx->ws_bytes = bytes;
+    ctx->have_run = false;
+    return HK_OK;
+}
+
+int hk_set_debug_mode(hk_ctx* ctx, int mode)
+{
+    if (!ctx || mode < 0 || mode > 1) return HK_EINVAL;
+    ctx->debug_mode = mode;
+    return HK_OK;
+}
+
+int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
+{
+    if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL) return HK_EINVAL;
+    if (std::isnan(cut_cm)) return HK_EINVAL;
+    if (n_lines > 0 && !lines_ok(lines)) return HK_EINVAL;
+    if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
+    const Layout L = make_layout(ctx, n_lines);
+    if (ctx->ws_bytes < L.total) return HK_ENOSPC;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    char* ws = (char*)ctx->ws;
+    DevStats* st = (DevStats*)(ws + L.stats);
+    const int n = (int)n_lines;
+    const Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm));
+
+    HK_CUDA(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
+    HK_CUDA(cudaMemsetAsync(out_k_dev, 0, (size_t)ctx->N * sizeof(double), stream));
+    ctx->have_run = true;
+    ctx->last_n = n_lines;
+    ctx->last_cut = cut_cm;
+    ctx->last_stream = stream;
+    ctx->d_stats = st;
+    ctx->last_sort_bits = 0;
+    if (n == 0) return HK_OK;
+
+    int32_t* keys_in = (int32_t*)(ws + L.keys_in);
+    int32_t* keys_out = (int32_t*)(ws + L.keys_out);
+    int32_t* idx_in = (int32_t*)(ws + L.idx_in);
+    int32_t* idx_out = (int32_t*)(ws + L.idx_out);
+    RecU* recU = (RecU*)(ws + L.recU);
+    float4* recA = (float4*)(ws + L.recA);
+    float4* recB = (float4*)(ws + L.recB);
+    TileRange* tr = (TileRange*)(ws + L.tr);
+    int32_t* counts = (int32_t*)(ws + L.counts);
+    int32_t* prefix = (int32_t*)(ws + L.prefix);
+
+    // a1: per-line parameters, keys
+    line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
+                                                      lines->n_exp, n, recU, keys_in, idx_in, st);
+    scale_kernel<<<1, 1, 0, stream>>>(st);
+    // a2: order by centre bin
+    const int bits = bits_for((uint32_t)p.ksent);
+    ctx->last_sort_bits = bits;
+    size_t cub_bytes = L.cub_bytes;
+    HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
+                                            (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
+    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB);
+    // a3: tile ranges and work units
+    range_kernel<<<(p.n_wt + 255) / 256, 256, 0, stream>>>(p, keys_out, n, tr);
+    HK_CUDA(cudaMemsetAsync(counts, 0, ((size_t)p.n_ct + 1) * 4, stream));
+    unit_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, tr, counts);
+    cub_bytes = L.cub_bytes;
+    HK_CUDA(cub::DeviceScan::ExclusiveSum(ws + L.cub, cub_bytes, (const int32_t*)counts, prefix, p.n_ct + 1, stream));
+    // a4-a7: accumulate
+    AccArgs a;
+    a.recA = recA; a.recB = recB; a.tr = tr; a.unit_prefix = prefix; a.st = st; a.out_k = out_k_dev;
+    a.N = ctx->N; a.n_wt = p.n_wt; a.n_ct = p.n_ct; a.chunk = p.chunk;
+    if (!p.force_near) far_kernel<<<ctx->n_sm * ctx->occ_far, kThreads, 0, stream>>>(a);
+    near_kernel<<<ctx->n_sm * ctx->occ_near, kThreads, 0, stream>>>(a);
+    HK_CUDA(cudaGetLastError());
+    return HK_OK;
+}
+
+int hk_get_extents(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, int32_t* ilo_dev, int32_t* ihi_dev,
+                   int32_t* jc_dev, void* stream_v)
+{
+    if (!ctx || n_lines < 0 || (n_lines > 0 && !lines_ok(lines))) return HK_EINVAL;
+    if (!ctx->have_cond || !ctx->have_run) return HK_ESTATE;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    if (n_lines > 0) {
+        const Params p = make_params(ctx, ctx->last_cut, 512);
+        extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
+                                                                   lines->gamma_ref, lines->n_exp, n_lines, ilo_dev,
+                                                                   ihi_dev, jc_dev, nullptr, nullptr, nullptr);
+        HK_CUDA(cudaGetLastError());
+    }
+    HK_CUDA(cudaStreamSynchronize(stream));
+    return HK_OK;
+}
+
+int hk_get_line_params(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double* S_dev, double* gammaL_dev,
+                       double* alphaD_dev, void* stream_v)
+{
+    if (!ctx || n_lines < 0 || (n_lines > 0 && !lines_ok(lines))) return HK_EINVAL;
+    if (!ctx->have_cond) return HK_ESTATE;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    if (n_lines > 0) {
+        const Params p = make_params(ctx, 0.0, 512);
+        extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
+                                                                   lines->gamma_ref, lines->n_exp, n_lines, nullptr,
+                                                                   nullptr, nullptr, S_dev, gammaL_dev, alphaD_dev);
+        HK_CUDA(cudaGetLastError());
+    }
+    HK_CUDA(cudaStreamSynchronize(stream));
+    return HK_OK;
+}
+
+int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
+{
+    if (!ctx || !host_out) return HK_EINVAL;
+    if (!ctx->have_run) return HK_ESTATE;
+    DevStats d;
+    HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
+    HK_CUDA(cudaMemcpy(&d, ctx->d_stats, sizeof(d), cudaMemcpyDeviceToHost));
+    std::memset(host_out, 0, sizeof(*host_out));
+    host_out->n_lines = ctx->last_n;
+    host_out->n_skipped = (int64_t)d.n_skipped;
+    host_out->n_off_grid = (int64_t)d.n_off_grid;
+    host_out->n_evals = (int64_t)d.n_evals;
+    host_out->n_evals_far = (int64_t)(d.n_evals - d.n_cnt_mid);
+    host_out->n_evals_mid = (int64_t)(d.n_cnt_mid - d.n_cnt_core);
+    host_out->n_evals_core = (int64_t)d.n_cnt_core;
+    host_out->n_units_far = (int64_t)d.units_far;
+    host_out->n_units_near = (int64_t)d.units_near;
+    host_out->scale_exp = d.scale_exp;
+    host_out->sort_bits = ctx->last_sort_bits;
+    return HK_OK;
+}
+
+int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev, int32_t* region_out_dev,
+                      void* stream_v)
+{
+    if (n < 0 || (n > 0 && (!x_dev || !y_dev || !out_dev))) return HK_EINVAL;
+    if (n == 0) return HK_OK;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > 65535) blocks = 65535;
+    probe_kernel<<<(int)blocks, 256, 0, (cudaStream_t)stream_v>>>(x_dev, y_dev, n, out_dev, region_out_dev);
+    return cudaGetLastError() == cudaSuccess ? HK_OK : HK_ECUDA;
+}
+
+int hk_last_cuda_error(const hk_ctx* ctx) { return ctx ? ctx->cuda_err : 0; }
+
+const char* hk_strerror(int status)
+{
+    switch (status) {
+        case HK_OK: return "ok";
+        case HK_EINVAL: return "invalid argument";
+        case HK_ESTATE: return "call out of order (conditions / workspace / compute missing)";
+        case HK_ENOSPC: return "workspace too small";
+        case HK_ECUDA: return "CUDA call failed (see hk_last_cuda_error)";
+        case HK_ENOMEM: return "host allocation failed";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"

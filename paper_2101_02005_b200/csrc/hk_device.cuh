@@ -1,0 +1,126 @@
+// hk_device.cuh -- constants, record layouts and the fp32 Voigt evaluator shared by the
+// CUDA kernels of the line-by-line opacity path (HELIOS-K 2.0, arxiv 2101.02005).
+// Nothing here is shared with oracle/ (separate constants, separate formulas).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hk.h"
+
+namespace hk {
+
+// ---- physical constants, cgs (CODATA 2018; c as printed in PAPER.md L129; R2/R3)
+constexpr double kC = 2.99792458e10;     // cm/s
+constexpr double kKB = 1.380649e-16;     // erg/K
+constexpr double kH = 6.62607015e-27;    // erg s
+constexpr double kNA = 6.02214076e23;    // 1/mol
+constexpr double kTref = 296.0;          // K (Eq. 5; BASELINE.json config 1)
+constexpr double kPi = 3.141592653589793238462643383279502884;
+
+// ---- geometry of the accumulation kernels
+constexpr int kB = 8;                    // bins per lane (registers)
+constexpr int kWarpBins = 32 * kB;       // bins per warp tile
+constexpr int kWarps = 8;                // warps per CTA
+constexpr int kThreads = 32 * kWarps;
+constexpr int kTileBins = kWarpBins * kWarps;  // bins per CTA tile
+constexpr int kSub = 512;                // line records staged in shared memory at a time
+constexpr int kFlush = 128;              // fp32 partial sums hold at most this many lines
+constexpr int kFarMinDist = 128;         // far kernel only sees |t| >= this many bins
+
+constexpr int32_t kKeySentinelBias = 1;  // sentinel key = kmax + 1
+
+// ---- unsorted per-line record written by the preprocess kernel (32 B)
+struct __align__(16) RecU {
+    int32_t jc;      // centre bin floor((nu0-numin)/dnu)
+    float f;         // sub-bin offset in [0,1)
+    float G2;        // (Gamma_L/dnu)^2
+    float a2;        // (alpha_D/dnu)^2
+    int32_t ilo;     // inclusive integer extent
+    int32_t ihi;
+    double cK;       // S/(alpha_D sqrt(pi)) in cm^2/g per unit K (unscaled)
+};
+
+// sorted records consumed by the accumulation kernels: two float4 streams
+//   A = { jc (int bits), f, G2, c }        c  = scale * S * Gamma_L/(pi dnu^2)   (Lorentz amplitude, bin units)
+//   B = { a2, ilo (int bits), ihi (int bits), cK }   cK = scale * S/(alpha_D sqrt(pi))
+
+// per warp tile: candidate range [A0,A1) and the two far-interior ranges inside it
+struct TileRange {
+    int32_t A0, FL0, FL1, FR0, FR1, A1;
+};
+
+// ---- small helpers
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// ---- fp32 evaluator, by region of |z|^2 = x^2 + y^2 ----------------
+// All three work in "bin units": t = (nu_i - nu0)/dnu, G = Gamma_L/dnu, a = alpha_D/dnu,
+// q = t^2 + G^2 = a^2 |z|^2.
+//
+// far  (|z|^2 >= HK_Z1): first term of the asymptotic series of w(z) = i/(sqrt(pi) z) (1 + 1/(2z^2) + ...)
+//        S V = c / q                      -- the Lorentzian, what the paper's region A evaluates
+//        with a first-order Gauss-Hermite rule (Table 1).
+// mid  (HK_Z2 <= |z|^2 < HK_Z1): two terms,
+//        S V = c r (1 + r (1.5 a^2 - 2 a^2 G^2 r)),  r = 1/q
+//        since Re{ i/z (1 + 1/(2 z^2)) } = y/|z|^2 (1 + (3x^2 - y^2)/(2|z|^4)).
+// core (|z|^2 < HK_Z2): trapezoid rule on the convolution integral with the pole term,
+//        nodes shifted per evaluation so that x is never within h/4 of a node.
+__device__ __forceinline__ float term_far(float c, float q) { return c * rcp_approx(q); }
+
+__device__ __forceinline__ float shape_mid(float r, float A1, float A2)
+{
+    // r (1 + r (A1 - A2 r))
+    float u = fmaf(-A2, r, A1);
+    float v = fmaf(u, r, 1.0f);
+    return r * v;
+}
+
+// Re w(x + i y), x >= 0, y >= 0, intended for x^2 + y^2 < ~700.
+__device__ __noinline__ float core_K(float x, float y)
+{
+    constexpr float h = 0.8f;
+    constexpr float inv_h = 1.25f;
+    // weights exp(-((n+s)h)^2), n = -5..5, for s = 0 and s = 1/2
+    constexpr float wA[11] = {1.12535175e-07f, 3.57128496e-05f, 3.15111160e-03f, 7.73047404e-02f,
+                              5.27292424e-01f, 1.0f,            5.27292424e-01f, 7.73047404e-02f,
+                              3.15111160e-03f, 3.57128496e-05f, 1.12535175e-07f};
+    constexpr float wB[11] = {2.35257520e-06f, 3.93669041e-04f, 1.83156389e-02f, 2.36927759e-01f,
+                              8.52143789e-01f, 8.52143789e-01f, 2.36927759e-01f, 1.83156389e-02f,
+                              3.93669041e-04f, 2.35257520e-06f, 3.90893843e-09f};
+    float u = x * inv_h;
+    float fr = u - floorf(u);
+    bool on = (fr >= 0.25f) && (fr < 0.75f);        // integer nodes are >= h/4 away
+    float s = on ? 0.0f : 0.5f;
+    float us = u - s;
+    float frs = us - floorf(us);                    // in [1/4, 3/4]
+    float y2 = y * y;
+    float sum = 0.0f;
+#pragma unroll
+    for (int n = -5; n <= 5; ++n) {
+        float tn = fmaf(s, h, (float)n * h);
+        float d = x - tn;
+        float w = on ? wA[n + 5] : wB[n + 5];
+        sum = fmaf(w, rcp_approx(fmaf(d, d, y2)), sum);
+    }
+    float K = sum * (y * (h / 3.14159265358979f));
+    float re2 = fmaf(x, x, -y2);
+    if (y < 3.92699082f /* pi/h */ && re2 < 80.0f) {
+        // + Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) }
+        float amp = 2.0f * __expf(-re2);
+        float sp, cp;
+        sincosf(2.0f * x * y, &sp, &cp);
+        float nr = amp * cp, ni = -amp * sp;
+        float e = __expf(7.85398163f /* 2 pi/h */ * y);
+        float st, ct;
+        sincospif(2.0f * frs, &st, &ct);            // theta = 2 pi frac(x/h - s), cos(theta) <= 0
+        float dr = fmaf(-e, ct, 1.0f), di = e * st;
+        K += (nr * dr + ni * di) / fmaf(dr, dr, di * di);
+    }
+    return K;
+}
+
+}  // namespace hk
