@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- lines/s of the line-by-line opacity hot path on N B200s (replicas).
+
+A "step" is one hk_compute over the whole synthetic line list of the workload
+(default: BASELINE.json configs[3], BT2-shaped water, 5.0e8 lines, grid 0-30000 cm^-1
+at 0.01 cm^-1, cut 100 cm^-1 -- the configuration the metric is quoted on): preprocess
+-> sort -> tile ranges -> far / near accumulation -> k(nu) in fp64.  Inputs are resident
+in HBM when the timed region starts.  One JSON line on stdout (rank 0).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                  [--config 1..5] [--n-lines n] [--no-e2e] [--no-cpu-baseline]
+
+--impl reference times the fp64 CPU oracle (oracle/, as it stands) on a bounded sample
+of the same workload on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from workload import linelists as W
+
+METRIC = "lines_per_s"
+UNIT = "lines/s"
+FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM (4 SMSPs x 32), DESIGN.md section 7
+FLOP_PER_EVAL = {"far": 6.0, "mid": 12.0}   # algorithmic FLOPs per Voigt evaluation
+
+
+def _workload_name(cfg, n):
+    c = W.CONFIGS[cfg]
+    g = c["grid"]
+    cut = f"cut {c['cut']:g} cm^-1" if c["cut"] > 0 else "no cut"
+    return (f"config {cfg} ({c['name']}): {n:.3g} lines, grid {g[0]:g}-{g[1]:g} cm^-1 at {g[2]:g} cm^-1, {cut}, "
+            f"T={c['T']:g} K, P={c['P_atm']:.5g} atm")
+
+
+# ---------------------------------------------------------------------------------------
+# clocks
+# ---------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=float(max(pw)))
+        return out
+
+
+# ---------------------------------------------------------------------------------------
+# oracle legs (cpu_baseline and --impl reference): a bounded sample of the workload
+# ---------------------------------------------------------------------------------------
+def _window_lines(dl, grid, cut, b0, b1):
+    """Lines that can reach bins [b0, b1) (all lines when uncut), as numpy on the host."""
+    nu0 = dl["nu0"]
+    if not cut > 0:
+        return {f: v.cpu().numpy() for f, v in dl.items()}
+    lo = grid[0] + b0 * grid[2] - cut - 2 * grid[2]
+    hi = grid[0] + (b1 - 1) * grid[2] + cut + 2 * grid[2]
+    sel = (nu0 >= lo) & (nu0 <= hi)
+    return {f: v[sel].cpu().numpy() for f, v in dl.items()}
+
+
+class OracleSample:
+    """Stratified windows of contiguous bins; every bin summed over ALL lines within its cut."""
+
+    def __init__(self, dl, cfg, n_windows=8):
+        from oracle import hk_oracle as O
+        self.O = O
+        c = W.CONFIGS[cfg]
+        self.cond, self.grid, self.cut = W.conditions(cfg), c["grid"], c["cut"]
+        self.N = O.grid_size(*self.grid)
+        self.dl = dl
+        self.n_windows = n_windows
+        self.starts = [int(x) for x in np.linspace(0, max(0, self.N - 1), n_windows + 2)[1:-1]]
+        self.subs = None
+        self.width = None
+
+    def prepare(self, width):
+        self.width = int(max(1, min(width, self.N)))
+        self.subs = []
+        for s in self.starts:
+            b0 = min(s, self.N - self.width)
+            self.subs.append((b0, _window_lines(self.dl, self.grid, self.cut, b0, b0 + self.width)))
+
+    def run(self):
+        """-> (seconds, evaluations)"""
+        t0 = time.perf_counter()
+        evals = 0
+        for b0, sub in self.subs:
+            bins = np.arange(b0, b0 + self.width, dtype=np.int64)
+            _, ev = self.O.opacity_bins(sub, self.cond, self.grid, self.cut, bins)
+            evals += ev
+        return time.perf_counter() - t0, evals
+
+    def size_for(self, seconds):
+        """Pilot with 2-bin windows, then pick the width that gives about `seconds` of CPU work."""
+        self.prepare(2)
+        t, ev = self.run()
+        t, ev = self.run()
+        rate = ev / max(t, 1e-9)
+        per_bin = ev / (2.0 * len(self.subs))
+        width = int(np.clip(seconds * rate / max(per_bin * len(self.subs), 1.0), 2, 4096))
+        self.prepare(width)
+        return width
+
+
+def _evals_per_line(dl, cfg):
+    """Exact mean extent (bins per line) of the workload, from the integer extent formula (fp64, torch)."""
+    c = W.CONFIGS[cfg]
+    numin, numax, dnu = c["grid"]
+    N = int(np.floor((numax - numin) / dnu + 0.5))
+    if not c["cut"] > 0:
+        return float(N)
+    nu0 = dl["nu0"]
+    lo = torch.ceil((nu0 - c["cut"] - numin) / dnu).clamp_(min=0)
+    hi = torch.floor((nu0 + c["cut"] - numin) / dnu).clamp_(max=N - 1)
+    return float((hi - lo + 1).clamp_(min=0).sum() / nu0.numel())
+
+
+def cpu_baseline(dl, cfg, n_lines, seconds=15.0):
+    samp = OracleSample(dl, cfg)
+    width = samp.size_for(seconds)
+    t, ev = samp.run()
+    epl = _evals_per_line(dl, cfg)
+    rate = ev / t
+    return {"value": rate / epl, "unit": UNIT, "cores": samp.O.num_threads(), "kind": "oracle",
+            "evals_per_s": rate, "seconds": t,
+            "sample": (f"{len(samp.subs)} stratified windows x {width} bins, every bin summed over all lines within its cut "
+                       f"({ev:.3e} Voigt evaluations); lines/s extrapolated = evals/s / ({epl:.1f} evals per line)")}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.config
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    n = args.n_lines or (W.CONFIGS[cfg]["n"] if dev == "cuda" else min(W.CONFIGS[cfg]["n"], 2_000_000))
+    dl = W.make_lines(cfg, n=n, seed=0, device=dev)            # input generation only; the oracle runs on the host
+    samp = OracleSample(dl, cfg)
+    width = samp.size_for(8.0)
+    epl = _evals_per_line(dl, cfg)
+    for _ in range(args.warmup):
+        samp.run()
+    tt, ee = 0.0, 0
+    for _ in range(args.steps):
+        t, ev = samp.run()
+        tt += t
+        ee += ev
+    rate = ee / tt
+    val = rate / epl
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * tt / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": _workload_name(cfg, n), "generator_device": dev},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": samp.O.num_threads(), "kind": "oracle",
+                            "evals_per_s": rate,
+                            "sample": (f"each step: {len(samp.subs)} stratified windows x {width} bins, all lines within the cut "
+                                       f"({ee // args.steps:.3e} Voigt evaluations); lines/s = evals/s / ({epl:.1f} evals per line)")},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ---------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def run_ours(args):
+    from paper_2101_02005_b200 import binding as B       # raises if libhk.so is missing: no CPU fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = args.config
+    c = W.CONFIGS[cfg]
+    n = args.n_lines or c["n"]
+    cond, grid, cut = W.conditions(cfg), c["grid"], c["cut"]
+    dl = W.make_lines(cfg, n=n, seed=0, device="cuda")      # replicas: every rank holds the whole workload
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    k = torch.empty(op.N, dtype=torch.float64, device="cuda")
+    input_bytes = 6 * 8 * n
+    flush = None
+    if input_bytes < 256e6:                                  # inputs smaller than ~2x L2: flush L2 between iterations
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    def step():
+        if flush is not None:
+            flush.fill_(1)
+        op.compute(dl, cut, out=k)
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    torch.cuda.synchronize()
+    st = op.stats()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    try:
+        gpu_id = str(torch.cuda.get_device_properties(local).uuid)
+        gpu_id = gpu_id if gpu_id.startswith("GPU-") else "GPU-" + gpu_id
+    except Exception:
+        gpu_id = str(local)
+    sampler = ClockSampler(gpu_id) if rank == 0 else None
+    phases = {p: 0.0 for p in B.PHASES}
+    step_ms = []
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
+    for i in range(args.steps):
+        if flush is not None:
+            flush.fill_(1)
+        ev[2 * i].record()
+        op.compute(dl, cut, out=k)
+        ev[2 * i + 1].record()
+        for p, v in op.phase_ms().items():                   # CUDA events recorded by the library on this stream
+            phases[p] += v
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    step_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
+    total_ms = float(sum(step_ms))
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * n * args.steps / (total_ms * 1e-3)
+    for p in phases:
+        phases[p] /= args.steps
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    peaks, peaks_kind = _peaks()
+    props = torch.cuda.get_device_properties(local)
+    n_sm = props.multi_processor_count
+    sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0)
+    peak_nominal = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12     # TFLOP/s
+    probe_flops, _ = B.probe_fp32_peak(packed=True, iters=20000)
+    # dominant kernel: the far-wing accumulation kernel
+    far_ms = phases["far"]
+    far_flops = FLOP_PER_EVAL["far"] * st["n_pairs_far"]
+    achieved = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "far_kernel", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                "frac": achieved / peak_nominal if peak_nominal else None, "traffic": None,
+                "peak_kind": f"nominal FP32: {n_sm} SMs x {FP32_LANES_PER_SM} lanes x 2 FLOP x {sm_max:g} MHz (DESIGN.md 7)",
+                "peak_probe_ffma2": probe_flops / 1e12, "frac_of_probe": achieved / (probe_flops / 1e12),
+                "flop_per_eval": FLOP_PER_EVAL["far"], "evals_per_launch": st["n_pairs_far"], "ms_per_launch": far_ms,
+                "evals_per_s": st["n_pairs_far"] / (far_ms * 1e-3) if far_ms > 0 else 0.0,
+                "evals_per_clk_per_sm": (st["n_pairs_far"] / (far_ms * 1e-3) / n_sm / ((clocks or {}).get("sm_mhz") or sm_max) / 1e6)
+                if far_ms > 0 else 0.0,
+                "hbm_preprocess_gbs": (input_bytes + 40.0 * n) / (phases["preprocess"] * 1e-3) / 1e9 if phases["preprocess"] > 0 else None,
+                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_kind": peaks_kind}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic",
+           "config": {"workload": _workload_name(cfg, n), "parallelism": f"replicas x{world}",
+                      "l2": "inputs larger than L2" if flush is None else "L2 flushed between iterations (256 MiB write)",
+                      "accumulate": "fp32 evaluation, fp32 partial sums of <=128 terms flushed to fp64; fp64 preprocessing and output"},
+           "voigt_evals_per_s": world * st["n_evals"] * args.steps / (total_ms * 1e-3),
+           "evals_per_step": st["n_evals"],
+           "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"]},
+           "pairs_by_kernel": {"far": st["n_pairs_far"], "near": st["n_pairs_near"]},
+           "phase_ms": phases, "step_ms": step_ms, "roofline": roofline, "clocks": clocks,
+           "gpu_launches": int(st["n_launches"]) * args.steps,
+           "paper_context": "paper: ~1e7 lines/s (BT2, 0.01 cm^-1, cut 25, RTX 2080 Ti, incl. read; PAPER.md L7, Table 8 L778) -- other hardware and cut"}
+
+    # ---- end to end through the host-buffer entry of the C ABI --------------------------
+    if not args.no_e2e and world == 1:
+        try:
+            import psutil
+            avail = psutil.virtual_memory().available
+        except Exception:
+            avail = 0
+        n_host = n
+        note = "whole workload"
+        if avail < 1.5 * input_bytes + 8e9:
+            n_host = int(max(1, min(n, (avail - 8e9) / 1.5 / 48)))
+            note = f"host RAM allows {n_host} of {n} lines (first {n_host} lines in list order)"
+        hl = {}
+        for f, v in dl.items():
+            h = torch.empty(n_host, dtype=torch.float64, pin_memory=True)
+            h.copy_(v[:n_host])
+            hl[f] = h
+        k_host = torch.empty(op.N, dtype=torch.float64, pin_memory=True)
+        del dl
+        torch.cuda.empty_cache()
+        op.compute_host(hl, cut, out=k_host)                # warm-up (allocates the workspace)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 2
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            op.compute_host(hl, cut, out=k_host)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        out["e2e"] = {"value": n_host / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 48 * n_host,
+                      "d2h_bytes_per_step": 8 * op.N, "ms_per_step": ms, "n_lines": n_host, "note": note,
+                      "api": "hk_compute_host (pinned host line arrays -> pinned host k; blocks of 2^25 lines, copy overlapped with compute)"}
+        dl = None
+        del hl
+
+    if not args.no_cpu_baseline and world == 1:
+        if dl is None:
+            dl = W.make_lines(cfg, n=n, seed=0, device="cuda")
+        out["cpu_baseline"] = cpu_baseline(dl, cfg, n)
+
+    print(json.dumps(out))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--n-lines", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

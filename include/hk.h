@@ -66,9 +66,15 @@ typedef struct {
     int64_t n_evals_core;  /* |z|^2 < HK_Z2 (trapezoid + pole term) */
     int64_t n_units_far;   /* (tile, line-chunk) work units run by the far kernel */
     int64_t n_units_near;  /* ... by the near/edge kernel */
+    int64_t n_pairs_far;   /* (line, bin) pairs the far kernel evaluated (mask-free Lorentzian) */
+    int64_t n_pairs_near;  /* (line, bin) slots the near kernel walked (masked; includes bins outside extents) */
+    int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
     int32_t sort_bits;     /* radix-sort key width used */
 } hk_stats;
+
+/* Phases of one hk_compute, timed with CUDA events on the caller's stream. */
+enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_FAR = 3, HK_PH_NEAR = 4, HK_PH_COUNT = 5 };
 
 /* Region thresholds on |z|^2 = x^2 + y^2 used by the fp32 evaluator. */
 #define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */
@@ -99,6 +105,24 @@ int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
 int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
                double* out_k_dev, void* stream);
 
+/* Same as hk_compute but ADDS into out_k_dev instead of overwriting it (line lists that
+ * arrive in blocks, L187: the sum over lines is order-independent, R16). */
+int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
+                  double* out_k_dev, void* stream);
+
+/* Host-buffer entry (the paper's block pipeline, L183-189, Fig. 6): the six line
+ * arrays and out_k are HOST pointers (pinned memory gives asynchronous copies; pageable
+ * works, slower).  The list is cut into blocks of block_lines lines (<= 0: default 2^25);
+ * block b+1 is copied host->device on an internal copy stream while block b runs
+ * hk_accumulate on `stream`; k is copied back once at the end.  Device scratch comes
+ * from the workspace set with hk_set_workspace, which must hold
+ * hk_workspace_bytes_host(ctx, n_lines, block_lines).  SYNCHRONOUS: returns when
+ * out_k_host holds the result.  hk_get_stats afterwards reports the LAST block only,
+ * except n_lines / n_evals / n_skipped, which are totals. */
+size_t hk_workspace_bytes_host(const hk_ctx* ctx, int64_t n_lines, int64_t block_lines);
+int hk_compute_host(hk_ctx* ctx, const hk_lines* host_lines, int64_t n_lines, double cut_cm,
+                    double* out_k_host, int64_t block_lines, void* stream);
+
 /* Integer extents of the lines of the LAST hk_compute, in the caller's line order
  * (int32 DEVICE arrays of n_lines; skipped / off-grid lines get ilo = 0, ihi = -1,
  * jc as computed (0 for skipped)).  Any pointer may be NULL.  Synchronises. */
@@ -112,6 +136,17 @@ int hk_get_line_params(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, doub
 
 /* Counts of the last hk_compute.  Synchronises the stream it ran on. */
 int hk_get_stats(hk_ctx* ctx, hk_stats* host_out);
+
+/* Milliseconds per phase (HK_PH_*) of the last hk_compute / hk_accumulate, from CUDA
+ * events recorded on its stream between the phases.  out_ms: HOST array of
+ * HK_PH_COUNT floats.  Synchronises. */
+int hk_get_phase_ms(hk_ctx* ctx, float* out_ms);
+
+/* FP32 issue-rate probe for the roofline denominator ("measure an FFMA
+ * peak"): runs a register-resident chain of independent packed FMAs on every SM and
+ * returns the achieved FLOP/s (2 per FMA) in *flops_out (HOST) and the kernel time.
+ * packed != 0 uses fma.rn.f32x2 (FFMA2), else scalar FFMA. */
+int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, void* stream);
 
 /* Accuracy probe for the shipped fp32 evaluator (the counterpart of the paper's
  * Fig. 4): out[i] = Re w(x[i] + i y[i]) exactly as the accumulation

@@ -24,8 +24,10 @@ HK_Z1, HK_Z2 = 90000.0, 625.0
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
-           "hk_set_workspace", "hk_compute", "hk_get_extents", "hk_get_line_params", "hk_get_stats",
+           "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_workspace_bytes_host", "hk_compute_host",
+           "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_last_cuda_error", "hk_strerror")
+PHASES = ("preprocess", "sort", "ranges", "far", "near")
 
 
 class hk_lines(C.Structure):
@@ -34,7 +36,8 @@ class hk_lines(C.Structure):
 
 class hk_stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n_lines", "n_skipped", "n_off_grid", "n_evals", "n_evals_far",
-                                         "n_evals_mid", "n_evals_core", "n_units_far", "n_units_near")] + \
+                                         "n_evals_mid", "n_evals_core", "n_units_far", "n_units_near",
+                                         "n_pairs_far", "n_pairs_near", "n_launches")] + \
                [("scale_exp", C.c_int32), ("sort_bits", C.c_int32)]
 
 
@@ -48,6 +51,12 @@ _lib.hk_workspace_bytes.argtypes = [_vp, _i64]
 _lib.hk_workspace_bytes.restype = C.c_size_t
 _lib.hk_set_workspace.argtypes = [_vp, _vp, C.c_size_t]
 _lib.hk_compute.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
+_lib.hk_accumulate.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
+_lib.hk_workspace_bytes_host.argtypes = [_vp, _i64, _i64]
+_lib.hk_workspace_bytes_host.restype = C.c_size_t
+_lib.hk_compute_host.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _i64, _vp]
+_lib.hk_get_phase_ms.argtypes = [_vp, C.POINTER(C.c_float)]
+_lib.hk_probe_fp32_peak.argtypes = [C.c_int, C.c_int, C.POINTER(_d), C.POINTER(C.c_float), _vp]
 _lib.hk_get_extents.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _vp, _vp]
 _lib.hk_get_line_params.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _vp, _vp]
 _lib.hk_get_stats.argtypes = [_vp, C.POINTER(hk_stats)]
@@ -57,6 +66,7 @@ _lib.hk_last_cuda_error.argtypes = [_vp]
 _lib.hk_strerror.argtypes = [C.c_int]
 _lib.hk_strerror.restype = C.c_char_p
 for _name in ("hk_create", "hk_destroy", "hk_set_conditions", "hk_set_workspace", "hk_compute", "hk_get_extents",
+              "hk_accumulate", "hk_compute_host", "hk_get_phase_ms", "hk_probe_fp32_peak",
               "hk_get_line_params", "hk_get_stats", "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_last_cuda_error"):
     getattr(_lib, _name).restype = C.c_int
 
@@ -77,13 +87,13 @@ def _stream_ptr(stream=None):
     return C.c_void_p(s.cuda_stream)
 
 
-def _lines_struct(lines):
+def _lines_struct(lines, host=False):
     ls = hk_lines()
     n = None
     for k in FIELDS:
         t = lines[k]
-        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
-            raise ValueError(f"lines[{k!r}] must be a contiguous CUDA float64 tensor")
+        if not (t.is_cuda != host and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError(f"lines[{k!r}] must be a contiguous {'CPU' if host else 'CUDA'} float64 tensor")
         if n is None:
             n = t.numel()
         elif t.numel() != n:
@@ -124,23 +134,45 @@ class Opacity:
     def workspace_bytes(self, n_lines: int) -> int:
         return int(_lib.hk_workspace_bytes(self._ctx, n_lines))
 
-    def ensure_workspace(self, n_lines: int):
-        need = self.workspace_bytes(n_lines)
+    def ensure_workspace(self, n_lines: int, need: int = None):
+        if need is None:
+            need = self.workspace_bytes(n_lines)
         if self._ws is None or self._ws.numel() < need:
             self._ws = None
             self._ws = torch.empty(need, dtype=torch.uint8, device="cuda")
             self._check(_lib.hk_set_workspace(self._ctx, self._ws.data_ptr(), self._ws.numel()), "hk_set_workspace")
 
-    def compute(self, lines, cut, out=None, stream=None):
-        """Enqueue lines -> k(nu) on the current (or given) torch stream; returns the fp64 CUDA tensor."""
+    def compute(self, lines, cut, out=None, stream=None, accumulate=False):
+        """Enqueue lines -> k(nu) on the current (or given) torch stream; returns the fp64 CUDA tensor.
+        accumulate=True adds into `out` (hk_accumulate) instead of overwriting it."""
         ls, n = _lines_struct(lines)
         self.ensure_workspace(n)
         if out is None:
+            assert not accumulate
             out = torch.empty(self.N, dtype=torch.float64, device="cuda")
         assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.N
         cut = float(cut) if cut is not None else 0.0
-        self._check(_lib.hk_compute(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)), "hk_compute")
+        fn = _lib.hk_accumulate if accumulate else _lib.hk_compute
+        self._check(fn(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)), "hk_compute")
         return out
+
+    def compute_host(self, host_lines, cut, out=None, block_lines=0, stream=None):
+        """Host-buffer entry (hk_compute_host): CPU fp64 tensors in (pinned for async copies), CPU fp64
+        tensor out; blocks are copied host->device while the previous block computes.  Synchronous."""
+        ls, n = _lines_struct(host_lines, host=True)
+        self.ensure_workspace(n, int(_lib.hk_workspace_bytes_host(self._ctx, n, block_lines)))
+        if out is None:
+            out = torch.empty(self.N, dtype=torch.float64, pin_memory=True)
+        assert (not out.is_cuda) and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.N
+        cut = float(cut) if cut is not None else 0.0
+        self._check(_lib.hk_compute_host(self._ctx, C.byref(ls), n, cut, out.data_ptr(), block_lines,
+                                         _stream_ptr(stream)), "hk_compute_host")
+        return out
+
+    def phase_ms(self) -> dict:
+        arr = (C.c_float * len(PHASES))()
+        self._check(_lib.hk_get_phase_ms(self._ctx, arr), "hk_get_phase_ms")
+        return {k: float(arr[i]) for i, k in enumerate(PHASES)}
 
     def extents(self, lines, stream=None):
         ls, n = _lines_struct(lines)
@@ -160,6 +192,15 @@ class Opacity:
         s = hk_stats()
         self._check(_lib.hk_get_stats(self._ctx, C.byref(s)), "hk_get_stats")
         return {k: int(getattr(s, k)) for k, _ in hk_stats._fields_}
+
+
+def probe_fp32_peak(packed=True, iters=4096, stream=None):
+    """Achieved FLOP/s of a register-resident FMA chain (hk_probe_fp32_peak) -> (flops, ms)."""
+    f, ms = _d(0.0), C.c_float(0.0)
+    st = _lib.hk_probe_fp32_peak(1 if packed else 0, iters, C.byref(f), C.byref(ms), _stream_ptr(stream))
+    if st != HK_OK:
+        raise HKError(st, "hk_probe_fp32_peak")
+    return f.value, ms.value
 
 
 def eval_voigt_f32(x: torch.Tensor, y: torch.Tensor, with_region=False, stream=None):

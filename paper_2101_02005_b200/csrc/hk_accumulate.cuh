@@ -308,4 +308,28 @@ __global__ void __launch_bounds__(256) probe_kernel(const float* __restrict__ x,
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// FP32 issue-rate probe (roofline denominator): 32 independent FMA chains per thread
+// ---------------------------------------------------------------------------------------
+template <bool kPacked>
+__global__ void __launch_bounds__(512) fp32_peak_kernel(int iters, float* __restrict__ sink)
+{
+    float2 acc[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) acc[j] = make_float2(1.0f + j + threadIdx.x * 1e-3f, 0.5f + j);
+    const float2 a = make_float2(0.999999f, 1.000001f), b = make_float2(1e-7f, -1e-7f);
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            if (kPacked) acc[j] = __ffma2_rn(acc[j], a, b);
+            else { acc[j].x = fmaf(acc[j].x, a.x, b.x); acc[j].y = fmaf(acc[j].y, a.y, b.y); }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) s += acc[j].x + acc[j].y;
+    if (s == 123.456f) *sink = s;
+}
+
 }  // namespace hk

@@ -30,7 +30,15 @@ struct hk_ctx {
     double last_cut;
     cudaStream_t last_stream;
     int32_t last_sort_bits;
+    int64_t last_launches;
     DevStats* d_stats;
+    // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
+    bool host_totals;
+    int64_t tot_lines, tot_skipped, tot_off_grid, tot_evals;
+    // phase events (recorded on the caller's stream) and the host-pipeline resources
+    cudaEvent_t ev[HK_PH_COUNT + 1];
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_h2d[2], ev_done[2];
 };
 
 namespace {
@@ -203,12 +211,26 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     if (e != cudaSuccess) { delete c; return HK_ECUDA; }
     if (c->occ_far < 1) c->occ_far = 1;
     if (c->occ_near < 1) c->occ_near = 1;
+    for (int i = 0; i <= HK_PH_COUNT && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&c->ev_h2d[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { hk_destroy(c); return HK_ECUDA; }
     *out = c;
     return HK_OK;
 }
 
 int hk_destroy(hk_ctx* ctx)
 {
+    if (!ctx) return HK_OK;
+    for (int i = 0; i <= HK_PH_COUNT; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->ev_h2d[i]) cudaEventDestroy(ctx->ev_h2d[i]);
+        if (ctx->ev_done[i]) cudaEventDestroy(ctx->ev_done[i]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     delete ctx;
     return HK_OK;
 }
@@ -248,7 +270,8 @@ int hk_set_debug_mode(hk_ctx* ctx, int mode)
     return HK_OK;
 }
 
-int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
+static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
+                        cudaStream_t stream, bool zero_out)
 {
     if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL) return HK_EINVAL;
     if (std::isnan(cut_cm)) return HK_EINVAL;
@@ -256,21 +279,26 @@ int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_c
     if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
     const Layout L = make_layout(ctx, n_lines);
     if (ctx->ws_bytes < L.total) return HK_ENOSPC;
-    cudaStream_t stream = (cudaStream_t)stream_v;
     char* ws = (char*)ctx->ws;
     DevStats* st = (DevStats*)(ws + L.stats);
     const int n = (int)n_lines;
     const Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm));
 
+    HK_CUDA(cudaEventRecord(ctx->ev[0], stream));
     HK_CUDA(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
-    HK_CUDA(cudaMemsetAsync(out_k_dev, 0, (size_t)ctx->N * sizeof(double), stream));
+    if (zero_out) HK_CUDA(cudaMemsetAsync(out_k_dev, 0, (size_t)ctx->N * sizeof(double), stream));
     ctx->have_run = true;
+    ctx->host_totals = false;
     ctx->last_n = n_lines;
     ctx->last_cut = cut_cm;
     ctx->last_stream = stream;
     ctx->d_stats = st;
     ctx->last_sort_bits = 0;
-    if (n == 0) return HK_OK;
+    ctx->last_launches = 0;
+    if (n == 0) {
+        for (int i = 1; i <= HK_PH_COUNT; ++i) HK_CUDA(cudaEventRecord(ctx->ev[i], stream));
+        return HK_OK;
+    }
 
     int32_t* keys_in = (int32_t*)(ws + L.keys_in);
     int32_t* keys_out = (int32_t*)(ws + L.keys_out);
@@ -287,6 +315,7 @@ int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_c
     line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
                                                       lines->n_exp, n, recU, keys_in, idx_in, st);
     scale_kernel<<<1, 1, 0, stream>>>(st);
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
     // a2: order by centre bin
     const int bits = bits_for((uint32_t)p.ksent);
     ctx->last_sort_bits = bits;
@@ -294,19 +323,146 @@ int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_c
     HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                             (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
     gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB);
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges and work units
-    range_kernel<<<(p.n_wt + 255) / 256, 256, 0, stream>>>(p, keys_out, n, tr);
+    range_kernel<<<(p.n_wt + 255) / 256, 256, 0, stream>>>(p, keys_out, n, tr, st);
     HK_CUDA(cudaMemsetAsync(counts, 0, ((size_t)p.n_ct + 1) * 4, stream));
     unit_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, tr, counts);
     cub_bytes = L.cub_bytes;
     HK_CUDA(cub::DeviceScan::ExclusiveSum(ws + L.cub, cub_bytes, (const int32_t*)counts, prefix, p.n_ct + 1, stream));
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_RANGES + 1], stream));
     // a4-a7: accumulate
     AccArgs a;
     a.recA = recA; a.recB = recB; a.tr = tr; a.unit_prefix = prefix; a.st = st; a.out_k = out_k_dev;
     a.N = ctx->N; a.n_wt = p.n_wt; a.n_ct = p.n_ct; a.chunk = p.chunk;
-    if (!p.force_near) far_kernel<<<ctx->n_sm * ctx->occ_far, kThreads, 0, stream>>>(a);
+    ctx->last_launches = 6;
+    if (!p.force_near) {
+        far_kernel<<<ctx->n_sm * ctx->occ_far, kThreads, 0, stream>>>(a);
+        ++ctx->last_launches;
+    }
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream));
     near_kernel<<<ctx->n_sm * ctx->occ_near, kThreads, 0, stream>>>(a);
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream));
     HK_CUDA(cudaGetLastError());
+    return HK_OK;
+}
+
+int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
+{
+    return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true);
+}
+
+int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
+{
+    return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, false);
+}
+
+// ---- host-buffer pipeline ---------------------------------------------------------------
+namespace {
+constexpr int64_t kDefaultBlock = 1LL << 25;
+
+int64_t host_block(int64_t n_lines, int64_t block_lines)
+{
+    int64_t b = block_lines > 0 ? block_lines : kDefaultBlock;
+    if (b > n_lines) b = n_lines;
+    if (b < 1) b = 1;
+    if (b > 2147483646LL) b = 2147483646LL;
+    return b;
+}
+
+struct HostLayout {
+    size_t dev_ws, stage[2], k, total;
+};
+
+HostLayout make_host_layout(const hk_ctx* c, int64_t n_lines, int64_t block_lines)
+{
+    const int64_t b = host_block(n_lines, block_lines);
+    HostLayout H;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+    H.dev_ws = take(make_layout(c, b).total);
+    H.stage[0] = take((size_t)b * 6 * sizeof(double));
+    H.stage[1] = take((size_t)b * 6 * sizeof(double));
+    H.k = take((size_t)c->N * sizeof(double));
+    H.total = off;
+    return H;
+}
+}  // namespace
+
+size_t hk_workspace_bytes_host(const hk_ctx* ctx, int64_t n_lines, int64_t block_lines)
+{
+    if (!ctx || n_lines < 0) return 0;
+    return make_host_layout(ctx, n_lines, block_lines).total;
+}
+
+int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut_cm, double* out_k_host,
+                    int64_t block_lines, void* stream_v)
+{
+    if (!ctx || !out_k_host || n_lines < 0 || std::isnan(cut_cm)) return HK_EINVAL;
+    if (n_lines > 0 && !lines_ok(hl)) return HK_EINVAL;
+    if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
+    const HostLayout H = make_host_layout(ctx, n_lines, block_lines);
+    if (ctx->ws_bytes < H.total) return HK_ENOSPC;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    const int64_t B = host_block(n_lines, block_lines);
+    char* base = (char*)ctx->ws;
+    const size_t full_bytes = ctx->ws_bytes;
+    double* k_dev = (double*)(base + H.k);
+    const double* src[6] = {hl ? hl->nu0 : nullptr, hl ? hl->A : nullptr, hl ? hl->g_up : nullptr,
+                            hl ? hl->E_low : nullptr, hl ? hl->gamma_ref : nullptr, hl ? hl->n_exp : nullptr};
+    int64_t tot_skipped = 0, tot_off = 0, tot_evals = 0;
+    int rc = HK_OK;
+    // the per-block device scratch is the front of the caller's workspace
+    ctx->ws = base + H.dev_ws;
+    ctx->ws_bytes = H.stage[0] - H.dev_ws;
+    cudaError_t e = cudaMemsetAsync(k_dev, 0, (size_t)ctx->N * sizeof(double), stream);
+    const int64_t n_blocks = n_lines > 0 ? (n_lines + B - 1) / B : 0;
+    auto enqueue_copy = [&](int64_t b) -> cudaError_t {
+        const int s = (int)(b & 1);
+        const int64_t l0 = b * B, nb = (l0 + B <= n_lines) ? B : n_lines - l0;
+        double* dst = (double*)(base + H.stage[s]);
+        cudaError_t ee = cudaSuccess;
+        if (b >= 2) ee = cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_done[s], 0);   // staging buffer free again
+        for (int f = 0; f < 6 && ee == cudaSuccess; ++f)
+            ee = cudaMemcpyAsync(dst + (size_t)f * B, src[f] + l0, (size_t)nb * sizeof(double), cudaMemcpyHostToDevice,
+                                 ctx->copy_stream);
+        if (ee == cudaSuccess) ee = cudaEventRecord(ctx->ev_h2d[s], ctx->copy_stream);
+        return ee;
+    };
+    if (e == cudaSuccess && n_blocks > 0) e = enqueue_copy(0);
+    for (int64_t b = 0; b < n_blocks && e == cudaSuccess && rc == HK_OK; ++b) {
+        const int s = (int)(b & 1);
+        const int64_t l0 = b * B, nb = (l0 + B <= n_lines) ? B : n_lines - l0;
+        if (b + 1 < n_blocks) e = enqueue_copy(b + 1);
+        if (e != cudaSuccess) break;
+        e = cudaStreamWaitEvent(stream, ctx->ev_h2d[s], 0);
+        if (e != cudaSuccess) break;
+        double* d = (double*)(base + H.stage[s]);
+        hk_lines dl = {d, d + B, d + 2 * B, d + 3 * B, d + 4 * B, d + 5 * B};
+        rc = compute_impl(ctx, &dl, nb, cut_cm, k_dev, stream, false);
+        if (rc != HK_OK) break;
+        e = cudaEventRecord(ctx->ev_done[s], stream);
+        if (e != cudaSuccess) break;
+        // per-block counters: read back after the block (the stats buffer is reused by the next one)
+        DevStats ds;
+        e = cudaMemcpyAsync(&ds, ctx->d_stats, sizeof(ds), cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) break;
+        tot_skipped += (int64_t)ds.n_skipped;
+        tot_off += (int64_t)ds.n_off_grid;
+        tot_evals += (int64_t)ds.n_evals;
+    }
+    if (e == cudaSuccess && rc == HK_OK)
+        e = cudaMemcpyAsync(out_k_host, k_dev, (size_t)ctx->N * sizeof(double), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess && rc == HK_OK) e = cudaStreamSynchronize(stream);
+    cudaStreamSynchronize(ctx->copy_stream);
+    ctx->ws = base;
+    ctx->ws_bytes = full_bytes;
+    if (rc != HK_OK) return rc;
+    if (e != cudaSuccess) return fail_cuda(ctx, e);
+    if (n_blocks == 0) { ctx->have_run = true; ctx->last_n = 0; ctx->last_stream = stream; ctx->d_stats = nullptr; }
+    ctx->host_totals = true;
+    ctx->tot_lines = n_lines; ctx->tot_skipped = tot_skipped; ctx->tot_off_grid = tot_off; ctx->tot_evals = tot_evals;
     return HK_OK;
 }
 
@@ -349,8 +505,9 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     if (!ctx || !host_out) return HK_EINVAL;
     if (!ctx->have_run) return HK_ESTATE;
     DevStats d;
+    std::memset(&d, 0, sizeof(d));
     HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
-    HK_CUDA(cudaMemcpy(&d, ctx->d_stats, sizeof(d), cudaMemcpyDeviceToHost));
+    if (ctx->d_stats) HK_CUDA(cudaMemcpy(&d, ctx->d_stats, sizeof(d), cudaMemcpyDeviceToHost));
     std::memset(host_out, 0, sizeof(*host_out));
     host_out->n_lines = ctx->last_n;
     host_out->n_skipped = (int64_t)d.n_skipped;
@@ -361,8 +518,60 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_evals_core = (int64_t)d.n_cnt_core;
     host_out->n_units_far = (int64_t)d.units_far;
     host_out->n_units_near = (int64_t)d.units_near;
+    host_out->n_pairs_far = (int64_t)d.pairs_far;
+    host_out->n_pairs_near = (int64_t)d.pairs_near;
+    host_out->n_launches = ctx->last_launches;
     host_out->scale_exp = d.scale_exp;
     host_out->sort_bits = ctx->last_sort_bits;
+    if (ctx->host_totals) {
+        host_out->n_lines = ctx->tot_lines;
+        host_out->n_skipped = ctx->tot_skipped;
+        host_out->n_off_grid = ctx->tot_off_grid;
+        host_out->n_evals = ctx->tot_evals;
+    }
+    return HK_OK;
+}
+
+int hk_get_phase_ms(hk_ctx* ctx, float* out_ms)
+{
+    if (!ctx || !out_ms) return HK_EINVAL;
+    if (!ctx->have_run) return HK_ESTATE;
+    HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
+    for (int i = 0; i < HK_PH_COUNT; ++i) {
+        out_ms[i] = 0.f;
+        if (ctx->last_n > 0 || !ctx->host_totals) HK_CUDA(cudaEventElapsedTime(&out_ms[i], ctx->ev[i], ctx->ev[i + 1]));
+    }
+    return HK_OK;
+}
+
+int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, void* stream_v)
+{
+    if (iters < 1 || !flops_out) return HK_EINVAL;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HK_ECUDA;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HK_ECUDA;
+    float* sink = nullptr;
+    if (cudaMalloc(&sink, sizeof(float)) != cudaSuccess) return HK_ECUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = n_sm * 4, threads = 512;
+    for (int rep = 0; rep < 2; ++rep) {      // first launch warms up
+        cudaEventRecord(e0, stream);
+        if (packed) fp32_peak_kernel<true><<<blocks, threads, 0, stream>>>(iters, sink);
+        else fp32_peak_kernel<false><<<blocks, threads, 0, stream>>>(iters, sink);
+        cudaEventRecord(e1, stream);
+    }
+    cudaError_t e = cudaStreamSynchronize(stream);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (e != cudaSuccess) return HK_ECUDA;
+    // 16 independent accumulators x 2 floats (packed) or 32 scalars; 2 FLOP per FMA
+    const double fmas = (double)blocks * threads * (double)iters * 32.0;
+    *flops_out = 2.0 * fmas / ((double)ms * 1e-3);
+    if (ms_out) *ms_out = ms;
     return HK_OK;
 }
 

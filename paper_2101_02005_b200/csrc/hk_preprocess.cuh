@@ -41,6 +41,7 @@ struct DevStats {
     int32_t pad;
     unsigned int unit_counter_far, unit_counter_near;
     unsigned long long units_far, units_near;
+    unsigned long long pairs_far, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
 };
 
 __device__ __forceinline__ bool finite6(double a, double b, double c, double d, double e, double f)
@@ -214,7 +215,7 @@ __device__ __forceinline__ int32_t lower_bound_key(const int32_t* __restrict__ k
 // |t| >= max(kFarMinDist, sqrt(Z1) a): then |z|^2 >= Z1 for every (line, bin) pair and the
 // far kernel may run mask-free.  All bounds are conservative.
 __global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __restrict__ keys, int32_t n,
-                                                    TileRange* __restrict__ tr)
+                                                    TileRange* __restrict__ tr, DevStats* __restrict__ st)
 {
     int wt = blockIdx.x * blockDim.x + threadIdx.x;
     if (wt >= p.n_wt) return;
@@ -247,6 +248,11 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __r
     if (fr0 < fl1) fr0 = fr1 = fl1;
     r.FL0 = fl0; r.FL1 = fl1; r.FR0 = fr0; r.FR1 = fr1;
     tr[wt] = r;
+    const unsigned long long nb = (unsigned long long)(w1 - w0);
+    const unsigned long long nfar = (unsigned long long)(fl1 - fl0) + (unsigned long long)(fr1 - fr0);
+    const unsigned long long nall = (unsigned long long)(r.A1 - r.A0);
+    if (nfar) atomicAdd(&st->pairs_far, nfar * nb);
+    if (nall > nfar) atomicAdd(&st->pairs_near, (nall - nfar) * nb);
 }
 
 // Per CTA tile: number of line chunks over the union of its warp tiles' candidates.

@@ -1,0 +1,38 @@
+"""Shared helpers of the GPU parity tests: the north_star tolerance and the
+oracle-side reference on the same seeded inputs.  No arithmetic of the method
+lives here (the oracle is oracle/, the product is the C-ABI library)."""
+import numpy as np
+
+REL_TOL = 1e-4      # per bin where oracle >= FLOOR * max(k)      (BASELINE.json north_star)
+FLOOR = 1e-8        # absolute tolerance FLOOR * max(k) elsewhere
+
+
+def check_parity(k_gpu, k_ref, kmax=None, rel=REL_TOL, floor=FLOOR, what=""):
+    """Assert the north_star tolerance; returns (max rel err in the relative regime,
+    max abs err / kmax in the absolute regime, fraction of bins in the relative regime)."""
+    k_gpu = np.asarray(k_gpu, dtype=np.float64)
+    k_ref = np.asarray(k_ref, dtype=np.float64)
+    assert k_gpu.shape == k_ref.shape
+    assert np.all(np.isfinite(k_gpu)), f"{what}: non-finite GPU output"
+    if kmax is None:
+        kmax = float(k_ref.max()) if k_ref.size else 0.0
+    if k_ref.size == 0:
+        return 0.0, 0.0, 0.0
+    big = k_ref >= floor * kmax
+    err = np.abs(k_gpu - k_ref)
+    relerr = float((err[big] / k_ref[big]).max()) if big.any() else 0.0
+    abserr = float(err[~big].max() / kmax) if (~big).any() and kmax > 0 else 0.0
+    assert relerr <= rel, f"{what}: relative error {relerr:.3e} > {rel:g} (bin {np.argmax(np.where(big, err / np.maximum(k_ref, 1e-300), 0))})"
+    assert abserr <= floor, f"{what}: absolute error {abserr:.3e} x max(k) > {floor:g}"
+    return relerr, abserr, float(big.mean())
+
+
+def sample_windows(N, n_windows, width, rng):
+    """Stratified windows of `width` contiguous bins incl. the first and last."""
+    if N <= n_windows * width:
+        return [(0, N)]
+    starts = {0, N - width}
+    strata = np.linspace(0, N - width, n_windows - 1).astype(np.int64)
+    for a, b in zip(strata[:-1], strata[1:]):
+        starts.add(int(rng.integers(a, max(a + 1, b))))
+    return [(s, s + width) for s in sorted(starts)]

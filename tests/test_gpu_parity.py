@@ -1,0 +1,349 @@
+"""GPU parity: the CUDA path through the C ABI (include/hk.h) against the fp64 CPU
+oracle on the same seeded inputs.  Tolerance (BASELINE.json north_star): relative
+error <= 1e-4 per bin where oracle >= 1e-8 max(k), absolute <= 1e-8 max(k) elsewhere;
+integer extents and centre bins exact."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import hk_oracle as O
+from workload import linelists as W
+
+from parity_util import check_parity, sample_windows
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2101_02005_b200 import binding
+    return binding
+
+
+def _to_cuda(lines_np):
+    return {k: torch.as_tensor(np.ascontiguousarray(v), dtype=torch.float64).cuda() for k, v in lines_np.items()}
+
+
+def _gpu_k(B, lines_np, cond, grid, cut, debug_mode=0):
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_debug_mode(debug_mode)
+    dl = _to_cuda(lines_np)
+    k = op.compute(dl, cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    ext = tuple(t.cpu().numpy() for t in op.extents(dl))
+    op.close()
+    return k.cpu().numpy(), st, ext
+
+
+def _check_extents(ext, lines_np, cond, grid, cut):
+    numin, numax, dnu = grid
+    N = O.grid_size(*grid)
+    _, _, _, valid = O.line_params(lines_np, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    ilo, ihi, jc = O.extents(lines_np["nu0"], valid, numin, dnu, N, cut)
+    empty = ilo > ihi
+    ilo = np.where(empty, 0, ilo)
+    ihi = np.where(empty, -1, ihi)
+    g_ilo, g_ihi, g_jc = ext
+    assert np.array_equal(g_ilo.astype(np.int64), ilo)
+    assert np.array_equal(g_ihi.astype(np.int64), ihi)
+    in32 = (jc > -(1 << 31)) & (jc < (1 << 31) - 1)
+    assert np.array_equal(g_jc.astype(np.int64)[in32], jc[in32])
+    return int((ihi - ilo + 1).sum())
+
+
+def _mini(cfg, n):
+    lines = W.to_numpy(W.make_lines(cfg, n=n, seed=0))
+    c = W.CONFIGS[cfg]
+    return lines, W.conditions(cfg), c["grid"], c["cut"]
+
+
+# ---- full-grid parity on configs the oracle finishes in seconds -----------------------
+
+@pytest.mark.parametrize("cfg,n", [(1, None), (2, 20_000), (3, 200_000), (4, 6_000)])
+def test_full_grid_parity(B, cfg, n):
+    """Config 1 at full size; mini twins (same generator, fewer lines, full grid) of 2-4."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    k_gpu, st, ext = _gpu_k(B, lines, cond, grid, cut)
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    n_ev = _check_extents(ext, lines, cond, grid, cut)
+    assert st["n_evals"] == evals == n_ev
+    assert st["n_evals_far"] + st["n_evals_mid"] + st["n_evals_core"] == st["n_evals"]
+    rel, ab, frac = check_parity(k_gpu, k_ref, what=f"config {cfg}")
+    print(f"config {cfg}: n={len(lines['nu0'])} rel={rel:.2e} abs={ab:.2e} frac_rel={frac:.3f} evals={evals}")
+
+
+def test_uncut_atom_like_sampled_bins(B):
+    """Config 5 mini twin (2000 lines, all 5e6 bins on the GPU); the oracle sums every
+    line on 4096 sampled bins + windows around the strongest lines."""
+    lines, cond, grid, cut = _mini(5, 2000)
+    k_gpu, st, ext = _gpu_k(B, lines, cond, grid, cut)
+    N = O.grid_size(*grid)
+    assert st["n_evals"] == 2000 * N
+    rng = np.random.default_rng(5)
+    bins = set(rng.integers(0, N, 3000).tolist()) | {0, 1, N - 2, N - 1}
+    S, _, _, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    for l in np.argsort(S)[-8:]:
+        jc = int((lines["nu0"][l] - grid[0]) / grid[2])
+        bins |= set(range(max(0, jc - 40), min(N, jc + 40)))
+    bins = np.array(sorted(bins), dtype=np.int64)
+    k_ref, _ = O.opacity_bins(lines, cond, grid, cut, bins)
+    kmax = max(float(k_ref.max()), float(k_gpu.max()))
+    check_parity(k_gpu[bins], k_ref, kmax=kmax, what="config 5 mini")
+    _check_extents(ext, lines, cond, grid, cut)
+
+
+def test_cross_path_near_vs_default(B):
+    """force every (tile, line) pair through the masked near kernel and
+    compare with the default far/mid/near split on all bins."""
+    for cfg, n in [(2, 20_000), (4, 6_000)]:
+        lines, cond, grid, cut = _mini(cfg, n)
+        k0, _, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=0)
+        k1, _, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=1)
+        big = k0 >= 1e-8 * k0.max()
+        assert np.abs(k1[big] / k0[big] - 1.0).max() <= 4e-5
+
+
+# ---- per-line parameters (step a1) ----------------------------------------------------
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_line_params_and_extents(B, cfg):
+    lines, cond, grid, cut = _mini(cfg, 100_000 if cfg != 1 else None)
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    dl = _to_cuda(lines)
+    S, gL, aD = (t.cpu().numpy() for t in op.line_params(dl))
+    S0, gL0, aD0, valid = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    assert valid.all()
+    assert np.abs(S / S0 - 1).max() <= 1e-12
+    assert np.abs(gL / gL0 - 1).max() <= 1e-12
+    assert np.abs(aD / aD0 - 1).max() <= 1e-13
+    op.compute(dl, cut)
+    ext = tuple(t.cpu().numpy() for t in op.extents(dl))
+    _check_extents(ext, lines, cond, grid, cut)
+    op.close()
+
+
+# ---- edge cases -------------------------------------------------------------------------
+
+def _simple_lines(nu0, **kw):
+    n = len(nu0)
+    d = dict(nu0=np.asarray(nu0, dtype=np.float64), A=np.full(n, 1.0), g_up=np.full(n, 3.0),
+             E_low=np.full(n, 100.0), gamma_ref=np.full(n, 0.05), n_exp=np.full(n, 0.6))
+    d.update({k: np.asarray(v, dtype=np.float64) for k, v in kw.items()})
+    return d
+
+
+COND = dict(T=1200.0, P_atm=0.7, mass_amu=28.0, Q=300.0)
+
+
+def test_empty_input(B):
+    op = B.Opacity(0.0, 100.0, 0.1)
+    op.set_conditions(1000.0, 1.0, 18.0, 100.0)
+    lines = {k: torch.empty(0, dtype=torch.float64, device="cuda") for k in B.FIELDS}
+    k = op.compute(lines, 25.0, out=torch.full((op.N,), 7.0, dtype=torch.float64, device="cuda"))
+    torch.cuda.synchronize()
+    assert float(k.abs().max()) == 0.0
+    assert op.stats()["n_evals"] == 0
+
+
+@pytest.mark.parametrize("grid,cut", [
+    ((0.0, 0.1, 0.1), 25.0),            # N = 1
+    ((100.0, 437.3, 0.1), 25.0),        # ragged tail (N = 3373), numin != 0
+    ((100.0, 437.3, 0.1), 0.05),        # cut smaller than dnu: most extents empty or one bin
+    ((100.0, 437.3, 0.1), 1.0e4),       # cut larger than the grid
+    ((100.0, 437.3, 0.1), 0.0),         # uncut
+    ((1000.0, 1020.5, 0.001), 3.0),     # fine grid, resolved lines (20500 bins)
+    ((5.0, 3000.0, 1.0), 25.0),         # dnu >> widths
+])
+def test_edge_grids(B, grid, cut):
+    rng = np.random.default_rng(11)
+    numin, numax, dnu = grid
+    span = numax - numin
+    nu0 = np.concatenate([
+        rng.uniform(numin - 30.0, numax + 30.0, 3000),          # includes off-grid centres whose wings reach in
+        [numin, numax, numin + dnu * 7, numin + 0.5 * dnu, numax - dnu, numin - 25.0, numax + 25.0],
+        numin + dnu * rng.integers(0, max(1, int(span / dnu)), 50),   # centres exactly on grid points
+    ])
+    nu0 = np.abs(nu0) + 1e-3
+    n = nu0.size
+    lines = _simple_lines(nu0, A=10 ** rng.uniform(-4, 3, n), g_up=rng.integers(1, 20, n).astype(float),
+                          E_low=rng.uniform(0, 5000, n), gamma_ref=rng.uniform(0.01, 0.2, n),
+                          n_exp=rng.uniform(0.5, 0.75, n))
+    k_gpu, st, ext = _gpu_k(B, lines, COND, grid, cut)
+    k_ref, evals = O.opacity_grid(lines, COND, grid, cut)
+    assert _check_extents(ext, lines, COND, grid, cut) == evals == st["n_evals"]
+    check_parity(k_gpu, k_ref, what=f"grid {grid} cut {cut}")
+
+
+def test_bad_lines_are_skipped(B):
+    rng = np.random.default_rng(3)
+    n = 500
+    lines = _simple_lines(rng.uniform(1.0, 200.0, n))
+    bad = {0: ("nu0", 0.0), 1: ("nu0", -5.0), 2: ("nu0", np.nan), 3: ("A", -1.0), 4: ("A", np.inf),
+           5: ("g_up", np.nan), 6: ("E_low", np.inf), 7: ("gamma_ref", np.nan), 8: ("n_exp", -np.inf)}
+    for i, (f, v) in bad.items():
+        lines[f][i] = v
+    grid, cut = (0.0, 200.0, 0.05), 10.0
+    k_gpu, st, ext = _gpu_k(B, lines, COND, grid, cut)
+    assert st["n_skipped"] == len(bad)
+    good = {k: np.delete(v, list(bad)) for k, v in lines.items()}
+    k_ref, evals = O.opacity_grid(good, COND, grid, cut)
+    assert st["n_evals"] == evals
+    check_parity(k_gpu, k_ref, what="bad lines")
+    k_all, _ = O.opacity_grid(lines, COND, grid, cut)          # the oracle applies the same rule (R14)
+    assert np.array_equal(k_all, k_ref)
+    _check_extents(ext, lines, COND, grid, cut)
+
+
+def test_order_independence_and_linearity(B):
+    lines, cond, grid, cut = _mini(2, 8000)
+    k0, _, _ = _gpu_k(B, lines, cond, grid, cut)
+    perm = np.random.default_rng(1).permutation(8000)
+    k1, _, _ = _gpu_k(B, {k: v[perm] for k, v in lines.items()}, cond, grid, cut)
+    big = k0 >= 1e-8 * k0.max()
+    assert np.abs(k1[big] / k0[big] - 1).max() <= 1e-6                      # R16: order changes rounding only
+    ka, _, _ = _gpu_k(B, {k: v[:3000] for k, v in lines.items()}, cond, grid, cut)
+    kb, _, _ = _gpu_k(B, {k: v[3000:] for k, v in lines.items()}, cond, grid, cut)
+    assert np.abs((ka + kb)[big] / k0[big] - 1).max() <= 1e-6
+
+
+def test_strong_and_weak_lines_dynamic_range(B):
+    """35 decades of line strength in one launch: the weak lines' bins fall in
+    the absolute regime, but a launch of the weak lines alone must still be right."""
+    rng = np.random.default_rng(9)
+    n = 2000
+    nu0 = np.sort(rng.uniform(50.0, 950.0, n))
+    A = 10 ** rng.uniform(-10, 3, n)
+    E = rng.uniform(0, 40000, n)
+    lines = _simple_lines(nu0, A=A, E_low=E)
+    grid, cut = (0.0, 1000.0, 0.01), 25.0
+    cond = dict(T=700.0, P_atm=1.0, mass_amu=18.0, Q=1000.0)
+    k_gpu, _, _ = _gpu_k(B, lines, cond, grid, cut)
+    k_ref, _ = O.opacity_grid(lines, cond, grid, cut)
+    check_parity(k_gpu, k_ref, what="35 decades")
+    S, _, _, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    weak = S < np.quantile(S, 0.2)
+    lw = {k: v[weak] for k, v in lines.items()}
+    k_gpu, _, _ = _gpu_k(B, lw, cond, grid, cut)
+    k_ref, _ = O.opacity_grid(lw, cond, grid, cut)
+    check_parity(k_gpu, k_ref, what="weak lines alone")
+
+
+def test_error_codes_on_device_box(B):
+    op = B.Opacity(0.0, 10.0, 0.1)
+    lines = _to_cuda(_simple_lines([1.0, 2.0]))
+    with pytest.raises(B.HKError) as e:
+        op.compute(lines, 1.0)                       # no conditions yet
+    assert e.value.status == B.HK_ESTATE
+    with pytest.raises(B.HKError) as e:
+        op.set_conditions(-1.0, 1.0, 18.0, 1.0)
+    assert e.value.status == B.HK_EINVAL
+    op.set_conditions(300.0, 1.0, 18.0, 1.0)
+    ws = torch.empty(256, dtype=torch.uint8, device="cuda")
+    assert B._lib.hk_set_workspace(op._ctx, ws.data_ptr(), 256) == 0
+    ls, n = B._lines_struct(lines)
+    out = torch.empty(op.N, dtype=torch.float64, device="cuda")
+    import ctypes as C
+    assert B._lib.hk_compute(op._ctx, C.byref(ls), n, 1.0, out.data_ptr(), None) == B.HK_ENOSPC
+
+
+# ---- the fp32 evaluator: measured accuracy map (our counterpart of Fig. 4) ------
+
+def test_evaluator_accuracy_map(B):
+    """Re w(x+iy) through the shipped fp32 device functions on a log lattice and at the
+    region boundaries, against the oracle's w.  Budget per region: 3e-5."""
+    xs = np.concatenate([[0.0], np.logspace(-3, 7, 640)])
+    ys = np.logspace(-2, 7, 576)
+    X, Y = np.meshgrid(xs, ys, indexing="ij")
+    # region boundaries +- a few ulp
+    for z2 in (B.HK_Z1, B.HK_Z2):
+        for yv in np.logspace(-2, math.log10(math.sqrt(z2)) - 1e-3, 64):
+            xb = math.sqrt(z2 - yv * yv)
+            xe = xb * (1 + np.array([-4, -2, -1, 0, 1, 2, 4]) * 6e-8)
+            X = np.concatenate([X.ravel(), xe])
+            Y = np.concatenate([Y.ravel(), np.full(xe.size, yv)])
+    x32 = X.ravel().astype(np.float32)
+    y32 = Y.ravel().astype(np.float32)
+    out, reg = B.eval_voigt_f32(torch.from_numpy(x32).cuda(), torch.from_numpy(y32).cuda(), with_region=True)
+    got = out.cpu().numpy().astype(np.float64)
+    reg = reg.cpu().numpy()
+    ref = O.voigt_K(x32.astype(np.float64), y32.astype(np.float64))
+    ok = ref > 1e-30                     # below that the term is far under any bin's tolerance
+    rel = np.abs(got - ref) / np.maximum(ref, 1e-300)
+    for r, name in enumerate(("far", "mid", "core")):
+        m = ok & (reg == r)
+        assert m.any()
+        worst = rel[m].max()
+        p999 = np.quantile(rel[m], 0.999)
+        print(f"evaluator region {name}: n={m.sum()} max rel={worst:.2e} p99.9={p999:.2e}")
+        assert worst <= 3e-5, (name, worst, x32[m][rel[m].argmax()], y32[m][rel[m].argmax()])
+
+
+# ---- bench-size parity on sampled outputs ----------------------------------------------
+
+def _full_size_sampled(B, cfg, n_windows, width, n=None):
+    c = W.CONFIGS[cfg]
+    cond, grid, cut = W.conditions(cfg), c["grid"], c["cut"]
+    dl = W.make_lines(cfg, n=n, seed=0, device="cuda")
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    k = op.compute(dl, cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    kmax = float(k.max())
+    N = op.N
+    rng = np.random.default_rng(cfg)
+    wins = sample_windows(N, n_windows, width, rng)
+    jmax = int(k.argmax())
+    wins.append((max(0, jmax - width // 2), min(N, jmax + width // 2)))
+    nu0 = dl["nu0"]
+    sorted_in = bool((nu0[1:] >= nu0[:-1]).all())
+    worst = 0.0
+    for b0, b1 in wins:
+        if cut > 0:
+            lo, hi = grid[0] + b0 * grid[2] - cut - 2 * grid[2], grid[0] + (b1 - 1) * grid[2] + cut + 2 * grid[2]
+            if sorted_in:
+                i0 = int(torch.searchsorted(nu0, torch.tensor([lo], dtype=torch.float64, device="cuda")))
+                i1 = int(torch.searchsorted(nu0, torch.tensor([hi], dtype=torch.float64, device="cuda"), right=True))
+                sub = {f: v[i0:i1].cpu().numpy() for f, v in dl.items()}
+            else:
+                sel = (nu0 >= lo) & (nu0 <= hi)
+                sub = {f: v[sel].cpu().numpy() for f, v in dl.items()}
+        else:
+            sub = {f: v.cpu().numpy() for f, v in dl.items()}
+        bins = np.arange(b0, b1, dtype=np.int64)
+        k_ref, _ = O.opacity_bins(sub, cond, grid, cut, bins)
+        rel, _, _ = check_parity(k[b0:b1].cpu().numpy(), k_ref, kmax=kmax, what=f"config {cfg} window {b0}")
+        worst = max(worst, rel)
+    # exact integer work count from the extents, all lines (O(n))
+    ilo, ihi, _ = op.extents(dl)
+    assert int((ihi.long() - ilo.long() + 1).sum()) == st["n_evals"]
+    op.close()
+    return worst, st
+
+
+def test_config2_full_size_sampled(B):
+    worst, st = _full_size_sampled(B, 2, 24, 64)
+    print(f"config 2 full: worst rel {worst:.2e}, evals {st['n_evals']:.3e}")
+
+
+def test_config5_full_size_sampled(B):
+    worst, st = _full_size_sampled(B, 5, 12, 32)
+    assert st["n_evals"] == 200_000 * 5_000_000
+    print(f"config 5 full: worst rel {worst:.2e}")
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_bt2_shaped_full_size_sampled(B, cfg):
+    """The bench workload (config 4) and its coarse twin (config 3) at 5e8 lines, in the launch
+    configuration bench.py times; the oracle sums every line within the cut on sampled bins."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs ~110 GB of device memory")
+    worst, st = _full_size_sampled(B, cfg, 6 if cfg == 4 else 10, 8 if cfg == 4 else 32)
+    print(f"config {cfg} full: worst rel {worst:.2e}, evals {st['n_evals']:.3e}")
