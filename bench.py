@@ -313,7 +313,7 @@ def run_ours(args):
     far_ms = phases["far"]
     far_flops = FLOP_PER_EVAL["far"] * st["n_pairs_far"]
     achieved = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
-    roofline = {"bound": "alu", "kernel": "far_kernel", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+    roofline = {"bound": "alu", "kernel": f"interior_kernel<{st['bins_per_lane']},false> (far wing)", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                 "frac": achieved / peak_nominal if peak_nominal else None, "traffic": None,
                 "peak_kind": f"nominal FP32: {n_sm} SMs x {FP32_LANES_PER_SM} lanes x 2 FLOP x {sm_max:g} MHz (DESIGN.md 7)",
                 "peak_probe_ffma2": probe_flops / 1e12, "frac_of_probe": achieved / (probe_flops / 1e12),
@@ -333,7 +333,8 @@ def run_ours(args):
            "voigt_evals_per_s": world * st["n_evals"] * args.steps / (total_ms * 1e-3),
            "evals_per_step": st["n_evals"],
            "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"]},
-           "pairs_by_kernel": {"far": st["n_pairs_far"], "near": st["n_pairs_near"]},
+           "pairs_by_kernel": {"far": st["n_pairs_far"], "mid": st["n_pairs_mid"], "near": st["n_pairs_near"]},
+           "bins_per_lane": st["bins_per_lane"],
            "phase_ms": phases, "step_ms": step_ms, "roofline": roofline, "clocks": clocks,
            "gpu_launches": int(st["n_launches"]) * args.steps,
            "paper_context": "paper: ~1e7 lines/s (BT2, 0.01 cm^-1, cut 25, RTX 2080 Ti, incl. read; PAPER.md L7, Table 8 L778) -- other hardware and cut"}

@@ -65,16 +65,20 @@ typedef struct {
     int64_t n_evals_mid;   /* HK_Z2 <= |z|^2 < HK_Z1 (2-term asymptotic) */
     int64_t n_evals_core;  /* |z|^2 < HK_Z2 (trapezoid + pole term) */
     int64_t n_units_far;   /* (tile, line-chunk) work units run by the far kernel */
+    int64_t n_units_mid;   /* ... by the mid kernel */
     int64_t n_units_near;  /* ... by the near/edge kernel */
     int64_t n_pairs_far;   /* (line, bin) pairs the far kernel evaluated (mask-free Lorentzian) */
+    int64_t n_pairs_mid;   /* (line, bin) pairs the mid kernel evaluated (mask-free two-term asymptotic) */
     int64_t n_pairs_near;  /* (line, bin) slots the near kernel walked (masked; includes bins outside extents) */
     int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
     int32_t sort_bits;     /* radix-sort key width used */
+    int32_t bins_per_lane; /* tile geometry used: a warp owns 32 x this many bins, a CTA 256 x */
+    int32_t reserved;
 } hk_stats;
 
 /* Phases of one hk_compute, timed with CUDA events on the caller's stream. */
-enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_FAR = 3, HK_PH_NEAR = 4, HK_PH_COUNT = 5 };
+enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_FAR = 3, HK_PH_MID = 4, HK_PH_NEAR = 5, HK_PH_COUNT = 6 };
 
 /* Region thresholds on |z|^2 = x^2 + y^2 used by the fp32 evaluator. */
 #define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */
@@ -155,9 +159,12 @@ int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, 
 int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev,
                       int32_t* region_out_dev, void* stream);
 
-/* Tuning knob for tests and sweeps: force every (tile, line) pair through the
- * near/edge kernel (mode 1) or restore the default split (mode 0). */
+/* Knobs for tests and sweeps.  mode 1: every (tile, line) pair goes through the near/edge
+ * kernel; mode 2: far pairs go through the mid (two-term) kernel; mode 0: the default split.
+ * hk_set_tile_bins: bins per lane 2, 4 or 8 (a warp owns 32x, a CTA 256x); 0 = chosen from
+ * the cut (include/hk.h hk_stats.bins_per_lane reports the choice). */
 int hk_set_debug_mode(hk_ctx* ctx, int mode);
+int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane);
 
 int hk_last_cuda_error(const hk_ctx* ctx);
 const char* hk_strerror(int status);

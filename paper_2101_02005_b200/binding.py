@@ -26,8 +26,8 @@ FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
-           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_last_cuda_error", "hk_strerror")
-PHASES = ("preprocess", "sort", "ranges", "far", "near")
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_last_cuda_error", "hk_strerror")
+PHASES = ("preprocess", "sort", "ranges", "far", "mid", "near")
 
 
 class hk_lines(C.Structure):
@@ -36,9 +36,9 @@ class hk_lines(C.Structure):
 
 class hk_stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n_lines", "n_skipped", "n_off_grid", "n_evals", "n_evals_far",
-                                         "n_evals_mid", "n_evals_core", "n_units_far", "n_units_near",
-                                         "n_pairs_far", "n_pairs_near", "n_launches")] + \
-               [("scale_exp", C.c_int32), ("sort_bits", C.c_int32)]
+                                         "n_evals_mid", "n_evals_core", "n_units_far", "n_units_mid", "n_units_near",
+                                         "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_launches")] + \
+               [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("reserved", C.c_int32)]
 
 
 _vp, _d, _i64 = C.c_void_p, C.c_double, C.c_int64
@@ -62,12 +62,13 @@ _lib.hk_get_line_params.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _v
 _lib.hk_get_stats.argtypes = [_vp, C.POINTER(hk_stats)]
 _lib.hk_eval_voigt_f32.argtypes = [_vp, _vp, _i64, _vp, _vp, _vp]
 _lib.hk_set_debug_mode.argtypes = [_vp, C.c_int]
+_lib.hk_set_tile_bins.argtypes = [_vp, C.c_int]
 _lib.hk_last_cuda_error.argtypes = [_vp]
 _lib.hk_strerror.argtypes = [C.c_int]
 _lib.hk_strerror.restype = C.c_char_p
 for _name in ("hk_create", "hk_destroy", "hk_set_conditions", "hk_set_workspace", "hk_compute", "hk_get_extents",
-              "hk_accumulate", "hk_compute_host", "hk_get_phase_ms", "hk_probe_fp32_peak",
-              "hk_get_line_params", "hk_get_stats", "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_last_cuda_error"):
+              "hk_accumulate", "hk_compute_host", "hk_get_phase_ms", "hk_probe_fp32_peak", "hk_set_tile_bins",
+              "hk_get_line_params", "hk_get_stats", "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_last_cuda_error"):
     getattr(_lib, _name).restype = C.c_int
 
 
@@ -130,6 +131,9 @@ class Opacity:
 
     def set_debug_mode(self, mode: int):
         self._check(_lib.hk_set_debug_mode(self._ctx, mode), "hk_set_debug_mode")
+
+    def set_tile_bins(self, bins_per_lane: int):
+        self._check(_lib.hk_set_tile_bins(self._ctx, bins_per_lane), "hk_set_tile_bins")
 
     def workspace_bytes(self, n_lines: int) -> int:
         return int(_lib.hk_workspace_bytes(self._ctx, n_lines))

@@ -1,19 +1,28 @@
-// hk_accumulate.cuh -- steps a4-a7 of the hot path: the two accumulation
-// kernels.  Both are output-stationary: a CTA owns kTileBins consecutive bins, a warp owns
-// kWarpBins of them, a lane owns kB bins (lane + 32 j) in registers.  Lines arrive sorted by
-// centre bin, so the lines that can reach a tile are one contiguous index range; a work unit
-// is (CTA tile, chunk of that range) and units are handed out by an atomic counter to a
-// persistent grid (one wave, multiples of the SM count).  fp32 partial sums are flushed into
-// fp64 registers every kFlush lines and reach k(nu) with one fp64 atomic per bin per unit.
+// hk_accumulate.cuh -- steps a4-a7 of the hot path: the accumulation kernels.
 //
-//   far_kernel  : pairs whose whole warp tile is inside the extent and has |z|^2 >= Z1:
-//                 branch-free Lorentzian, two lines share one reciprocal, packed fp32 (FFMA2).
-//   near_kernel : everything else (extent edges, |z|^2 < Z1): exact integer extent mask,
-//                 two-term asymptotic, and the core evaluator where |z|^2 < Z2.
+// All are output-stationary: a CTA owns a tile of 32*KB consecutive bins, every warp of the CTA
+// holds the SAME bins (a lane owns bins lane + 32 j, j < KB, in registers) and the warps split the
+// LINES of each staged batch between them; their partial sums are combined through shared memory
+// at the end of a work unit and reach k(nu) with one fp64 atomic per bin per unit.
+// Lines arrive sorted by centre bin, so the lines that can reach a tile are one contiguous index
+// range, split by range_kernel into
+//   [A0,FL0) left-edge | [FL0,FL1) far | [FL1,ML1) mid | [ML1,MR0) centre | [MR0,FR0) mid | [FR0,FR1) far | [FR1,A1) right-edge
+// A work unit is (tile, chunk of that range); units are handed out by an atomic counter to a
+// persistent grid (a multiple of the SM count).  fp32 partial sums are flushed into fp64 registers
+// every kFlush lines.
+//
+//   interior_kernel<KB,false> (a5, "far") : pairs whose whole tile is inside the extent and has
+//        |z|^2 >= Z1: branch-free Lorentzian, two lines share one reciprocal, packed fp32 (FFMA2).
+//   interior_kernel<KB,true>  (a5, "mid") : same shape, |z|^2 >= Z2: two-term asymptotic, mask-free.
+//   near_kernel<KB>           (a4)        : extent edges and line centres.  Row pass: exact integer
+//        extent mask + two-term asymptotic where |z|^2 >= Z2, and the trapezoid evaluator in place
+//        for lines whose core (|z|^2 < Z2) spans >= 16 bins.  Lane pass, for narrower cores: lanes
+//        walk lines, each lane evaluates its own line's core bins; equal bins are combined in the
+//        warp and added to a bin tile staged in shared memory.
 //
 // The paper's kernel (L243-330) walks lines in threads and nu-points serially with a
 // shared-memory K_s and four launches per block (AL/AR/B/C, L354); what is kept is the idea
-// of formula-uniform launches.
+// of formula-uniform launches and of partial arrays merged at the end (L254-258, L268).
 #pragma once
 #include "hk_preprocess.cuh"
 
@@ -27,10 +36,10 @@ struct AccArgs {
     DevStats* st;
     double* __restrict__ out_k;
     int64_t N;
-    int32_t n_wt, n_ct, chunk;
+    int32_t n_ct, chunk;
 };
 
-// Which CTA tile does unit u belong to?  Largest ct with prefix[ct] <= u.
+// Which tile does unit u belong to?  Largest ct with prefix[ct] <= u.
 __device__ __forceinline__ int find_tile(const int32_t* __restrict__ prefix, int n_ct, int u)
 {
     int lo = 0, hi = n_ct;   // invariant: prefix[lo] <= u < prefix[hi]
@@ -49,242 +58,429 @@ __device__ __forceinline__ int next_unit(unsigned int* counter, int* s_unit)
     return *s_unit;
 }
 
-// ---------------------------------------------------------------------------------------
-// far kernel
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads, 2) far_kernel(AccArgs a)
+__device__ __forceinline__ float2 bcast2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ float2 rcp2(float2 q) { return make_float2(rcp_approx(q.x), rcp_approx(q.y)); }
+
+// this warp's share [w0, w1) of the lines [0, n): contiguous, even-sized (pairs stay together)
+__device__ __forceinline__ void warp_share(int n, int warp, int& w0, int& w1)
 {
-    __shared__ float4 sm[kSub];       // { -tl, G2, c, - } with tl = centre position relative to the CTA tile
+    const int per = ((n + 2 * kWarps - 1) / (2 * kWarps)) * 2;
+    w0 = min(warp * per, n);
+    w1 = min(w0 + per, n);
+}
+
+// combine the warps' partial sums (red aliases the staging buffers: call after a __syncthreads that
+// follows the last read of them) and add the tile to k(nu)
+template <int KB>
+__device__ __forceinline__ void flush_tile(double* red, const double (&v)[KB], int64_t ct0, const AccArgs& a)
+{
+    constexpr int kTB = 32 * KB;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int j = 0; j < KB; ++j) red[warp * kTB + lane + 32 * j] = v[j];
+    __syncthreads();
+    if (threadIdx.x < kTB) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) s += red[w * kTB + threadIdx.x];
+        const int64_t b = ct0 + threadIdx.x;
+        s *= scalbn(1.0, -a.st->scale_exp);
+        if (b < a.N && s != 0.0) atomicAdd(a.out_k + b, s);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// interior kernels (far: kMid = false, mid: kMid = true)
+// ---------------------------------------------------------------------------------------
+constexpr int kSubI = 1024;            // lines per staged batch (double-buffered)
+constexpr int kLPT = kSubI / kThreads; // lines each thread stages per batch
+
+template <int KB, bool kMid>
+__global__ void __launch_bounds__(kThreads, 2) interior_kernel(AccArgs a)
+{
+    constexpr int kTB = 32 * KB;          // bins per tile
+    constexpr int M = KB / 2;             // float2 accumulators per lane
+    static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubI, "red must fit in the staging buffers");
+    __shared__ float4 sm[2][kSubI];       // { -tl, G2, c, 1.5 a2 }, tl = centre position relative to the tile
     __shared__ int s_unit;
+    double* red = reinterpret_cast<double*>(&sm[0][0]);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int total = a.unit_prefix[a.n_ct];
+    unsigned int* counter = kMid ? &a.st->unit_counter_mid : &a.st->unit_counter_far;
 
-    float2 tb[kB / 2];
+    float2 tb[M];
 #pragma unroll
-    for (int m = 0; m < kB / 2; ++m) {
-        float b0 = (float)(warp * kWarpBins + lane + 64 * m);
+    for (int m = 0; m < M; ++m) {
+        float b0 = (float)(lane + 64 * m);
         tb[m] = make_float2(b0, b0 + 32.0f);
     }
 
     for (;;) {
-        const int u = next_unit(&a.st->unit_counter_far, &s_unit);
+        const int u = next_unit(counter, &s_unit);
         if (u >= total) break;
         const int ct = find_tile(a.unit_prefix, a.n_ct, u);
-        const int wt_first = ct * kWarps, wt_last = min(a.n_wt, wt_first + kWarps) - 1;
-        const int64_t ct0 = (int64_t)ct * kTileBins;
-        const int cA0 = a.tr[wt_first].A0, cA1 = a.tr[wt_last].A1;
-        const int c0 = cA0 + (u - a.unit_prefix[ct]) * a.chunk;
-        const int c1 = min(c0 + a.chunk, cA1);
-        const int wt = wt_first + warp;
-        int fl0 = 0, fl1 = 0, fr0 = 0, fr1 = 0;
-        if (wt <= wt_last) {
-            TileRange r = a.tr[wt];
-            fl0 = max(r.FL0, c0); fl1 = min(r.FL1, c1);
-            fr0 = max(r.FR0, c0); fr1 = min(r.FR1, c1);
-        }
-        if (!__syncthreads_or((fl0 < fl1) || (fr0 < fr1))) continue;
-        if (threadIdx.x == 0) atomicAdd(&a.st->units_far, 1ULL);
+        const int64_t ct0 = (int64_t)ct * kTB;
+        const TileRange r = a.tr[ct];
+        const int c0 = r.A0 + (u - a.unit_prefix[ct]) * a.chunk;
+        const int c1 = min(c0 + a.chunk, r.A1);
+        // left and right segments of this class, clipped to the chunk, walked as one list of nt lines
+        const int l0 = max(kMid ? r.FL1 : r.FL0, c0), l1 = min(kMid ? r.ML1 : r.FL1, c1);
+        const int r0 = max(kMid ? r.MR0 : r.FR0, c0), r1 = min(kMid ? r.FR0 : r.FR1, c1);
+        const int nl = max(l1 - l0, 0), nt = nl + max(r1 - r0, 0);
+        if (nt == 0) continue;
+        if (threadIdx.x == 0) atomicAdd(kMid ? &a.st->units_mid : &a.st->units_far, 1ULL);
 
-        float2 acc[kB / 2];
-        double acc64[kB];
+        float2 acc[M];
+        double acc64[KB];
 #pragma unroll
-        for (int m = 0; m < kB / 2; ++m) acc[m] = make_float2(0.f, 0.f);
+        for (int m = 0; m < M; ++m) acc[m] = make_float2(0.f, 0.f);
 #pragma unroll
-        for (int j = 0; j < kB; ++j) acc64[j] = 0.0;
+        for (int j = 0; j < KB; ++j) acc64[j] = 0.0;
         int since_flush = 0;
 
-        for (int s0 = c0; s0 < c1; s0 += kSub) {
-            const int s1 = min(s0 + kSub, c1);
-            const int p0 = max(fl0, s0), p1 = min(fl1, s1);
-            const int q0 = max(fr0, s0), q1 = min(fr1, s1);
-            if (!__syncthreads_or((p0 < p1) || (q0 < q1))) continue;   // also fences reuse of sm
-            for (int i = threadIdx.x; i < s1 - s0; i += kThreads) {
-                float4 r = a.recA[s0 + i];
-                float tl = (float)((int64_t)__float_as_int(r.x) - ct0) + r.y;
-                sm[i] = make_float4(-tl, r.z, r.w, 0.f);
-            }
-            __syncthreads();
-#pragma unroll 1
-            for (int seg = 0; seg < 2; ++seg) {
-                int l = (seg == 0 ? p0 : q0) - s0;
-                const int le = (seg == 0 ? p1 : q1) - s0;
-                while (l < le) {
-                    const int stop = min(le, l + (kFlush - since_flush));
-                    since_flush += stop - l;
-                    for (; l + 1 < stop; l += 2) {
-                        const float4 r1 = sm[l], r2 = sm[l + 1];
-                        const float2 n1 = make_float2(r1.x, r1.x), g1 = make_float2(r1.y, r1.y), c1 = make_float2(r1.z, r1.z);
-                        const float2 n2 = make_float2(r2.x, r2.x), g2 = make_float2(r2.y, r2.y), c2 = make_float2(r2.z, r2.z);
+        float4 pre[kLPT];
+        float prea[kLPT];
+        auto fetch = [&](int v0) {            // global loads of batch [v0, v0 + kSubI) into registers
 #pragma unroll
-                        for (int m = 0; m < kB / 2; ++m) {
+            for (int k = 0; k < kLPT; ++k) {
+                const int v = v0 + threadIdx.x + k * kThreads;
+                if (v < nt) {
+                    const int li = v < nl ? l0 + v : r0 + (v - nl);
+                    pre[k] = a.recA[li];
+                    if (kMid) prea[k] = a.recB[li].x;
+                }
+            }
+        };
+        auto stash = [&](int v0, int buf) {   // convert to tile-relative records in shared memory
+#pragma unroll
+            for (int k = 0; k < kLPT; ++k) {
+                const int i = threadIdx.x + k * kThreads;
+                if (v0 + i < nt) {
+                    const float tl = (float)((int64_t)__float_as_int(pre[k].x) - ct0) + pre[k].y;
+                    sm[buf][i] = make_float4(-tl, pre[k].z, pre[k].w, kMid ? 1.5f * prea[k] : 0.f);
+                }
+            }
+        };
+        fetch(0);
+        stash(0, 0);
+        __syncthreads();
+        int buf = 0;
+        for (int v0 = 0; v0 < nt; v0 += kSubI, buf ^= 1) {
+            const bool more = v0 + kSubI < nt;
+            if (more) fetch(v0 + kSubI);
+            const float4* __restrict__ smb = sm[buf];
+            int l, le;
+            warp_share(min(kSubI, nt - v0), warp, l, le);
+            while (l < le) {
+                const int stop = min(le, l + (kFlush - since_flush));
+                since_flush += stop - l;
+                if (!kMid) {
+                    for (; l + 1 < stop; l += 2) {
+                        const float4 r1 = smb[l], r2 = smb[l + 1];
+                        const float2 n1 = bcast2(r1.x), g1 = bcast2(r1.y), c1 = bcast2(r1.z);
+                        const float2 n2 = bcast2(r2.x), g2 = bcast2(r2.y), c2 = bcast2(r2.z);
+#pragma unroll
+                        for (int m = 0; m < M; ++m) {
                             // c1/q1 + c2/q2 = (c1 q2 + c2 q1) / (q1 q2): one reciprocal for two lines
-                            float2 t1 = __fadd2_rn(tb[m], n1);
-                            float2 t2 = __fadd2_rn(tb[m], n2);
-                            float2 q1 = __ffma2_rn(t1, t1, g1);
-                            float2 q2 = __ffma2_rn(t2, t2, g2);
-                            float2 pp = __fmul2_rn(q1, q2);
+                            const float2 t1 = __fadd2_rn(tb[m], n1);
+                            const float2 t2 = __fadd2_rn(tb[m], n2);
+                            const float2 q1 = __ffma2_rn(t1, t1, g1);
+                            const float2 q2 = __ffma2_rn(t2, t2, g2);
+                            const float2 pp = __fmul2_rn(q1, q2);
                             float2 nn = __fmul2_rn(c1, q2);
                             nn = __ffma2_rn(c2, q1, nn);
-                            float2 rr = make_float2(rcp_approx(pp.x), rcp_approx(pp.y));
-                            acc[m] = __ffma2_rn(nn, rr, acc[m]);
+                            acc[m] = __ffma2_rn(nn, rcp2(pp), acc[m]);
                         }
                     }
                     if (l < stop) {       // odd line out
-                        const float4 r1 = sm[l];
-                        const float2 n1 = make_float2(r1.x, r1.x), g1 = make_float2(r1.y, r1.y), c1 = make_float2(r1.z, r1.z);
+                        const float4 r1 = smb[l];
+                        const float2 n1 = bcast2(r1.x), g1 = bcast2(r1.y), c1 = bcast2(r1.z);
 #pragma unroll
-                        for (int m = 0; m < kB / 2; ++m) {
-                            float2 t1 = __fadd2_rn(tb[m], n1);
-                            float2 q1 = __ffma2_rn(t1, t1, g1);
-                            float2 rr = make_float2(rcp_approx(q1.x), rcp_approx(q1.y));
-                            acc[m] = __ffma2_rn(c1, rr, acc[m]);
+                        for (int m = 0; m < M; ++m) {
+                            const float2 t1 = __fadd2_rn(tb[m], n1);
+                            const float2 q1 = __ffma2_rn(t1, t1, g1);
+                            acc[m] = __ffma2_rn(c1, rcp2(q1), acc[m]);
                         }
                         ++l;
                     }
-                    if (since_flush >= kFlush) {
+                } else {
+                    for (; l < stop; ++l) {
+                        // c r (1 + r (A1 - A2 r)),  A1 = 1.5 a^2, A2 = 2 a^2 G^2 = (4/3) A1 G^2
+                        const float4 r1 = smb[l];
+                        const float2 n1 = bcast2(r1.x), g1 = bcast2(r1.y), c1 = bcast2(r1.z);
+                        const float2 A1 = bcast2(r1.w), one = bcast2(1.0f);
+                        const float2 nA2 = bcast2(-1.33333333f * r1.w * r1.y);
 #pragma unroll
-                        for (int m = 0; m < kB / 2; ++m) {
-                            acc64[2 * m] += (double)acc[m].x;
-                            acc64[2 * m + 1] += (double)acc[m].y;
-                            acc[m] = make_float2(0.f, 0.f);
+                        for (int m = 0; m < M; ++m) {
+                            const float2 t1 = __fadd2_rn(tb[m], n1);
+                            const float2 q1 = __ffma2_rn(t1, t1, g1);
+                            const float2 rr = rcp2(q1);
+                            const float2 uu = __ffma2_rn(nA2, rr, A1);
+                            const float2 vv = __ffma2_rn(uu, rr, one);
+                            const float2 ww = __fmul2_rn(rr, vv);
+                            acc[m] = __ffma2_rn(c1, ww, acc[m]);
                         }
-                        since_flush = 0;
                     }
                 }
-            }
-        }
-        const double inv_scale = scalbn(1.0, -a.st->scale_exp);
+                if (since_flush >= kFlush) {
 #pragma unroll
-        for (int m = 0; m < kB / 2; ++m) {
-            const int64_t b = ct0 + warp * kWarpBins + lane + 64 * m;
-            double v0 = (acc64[2 * m] + (double)acc[m].x) * inv_scale;
-            double v1 = (acc64[2 * m + 1] + (double)acc[m].y) * inv_scale;
-            if (b < a.N && v0 != 0.0) atomicAdd(a.out_k + b, v0);
-            if (b + 32 < a.N && v1 != 0.0) atomicAdd(a.out_k + b + 32, v1);
+                    for (int m = 0; m < M; ++m) {
+                        acc64[2 * m] += (double)acc[m].x;
+                        acc64[2 * m + 1] += (double)acc[m].y;
+                        acc[m] = make_float2(0.f, 0.f);
+                    }
+                    since_flush = 0;
+                }
+            }
+            if (more) stash(v0 + kSubI, buf ^ 1);
+            __syncthreads();
         }
+        double v[KB];
+#pragma unroll
+        for (int m = 0; m < M; ++m) {            // acc[m] holds bins lane + 64 m and lane + 64 m + 32: rows 2m and 2m+1
+            v[2 * m] = acc64[2 * m] + (double)acc[m].x;
+            v[2 * m + 1] = acc64[2 * m + 1] + (double)acc[m].y;
+        }
+        flush_tile<KB>(red, v, ct0, a);
     }
 }
 
 // ---------------------------------------------------------------------------------------
 // near / edge kernel
 // ---------------------------------------------------------------------------------------
-template <bool kCore>
-__device__ __forceinline__ void near_line(const float4 ra, const float4 rb, const float (&tb)[kB], float (&acc)[kB])
+constexpr int kSubN = 512;             // lines per staged batch
+constexpr int kLPTN = kSubN / kThreads;
+constexpr float kWideCore = 64.0f;     // (core half-width in bins)^2 from which the core is evaluated in the row pass
+// per-line flags, decided once per (line, tile) when the line is staged
+constexpr int kFlagFull = 1;           // the whole tile is inside the extent: no mask
+constexpr int kFlagNoCore = 2;         // |z|^2 >= Z2 on every bin of the tile
+constexpr int kFlagFar = 4;            // |z|^2 >= Z1 on every bin of the tile: one term is enough
+constexpr int kFlagWide = 8;           // core spans >= 16 bins: evaluated in the row pass
+
+// One line against the warp's KB rows of 32 bins.  A = { jc - ct0, f, G2, c }, B = { A1, -A2, qc, cK },
+// C = { ilo - ct0, ihi - ct0, y, flags }.
+template <int KB, bool kTwoTerm, bool kMask, bool kCore>
+__device__ __forceinline__ void near_rows(float2 (&acc)[KB / 2], const float2 (&tb)[KB / 2], const float4 A,
+                                          const float4 B, const float4 C, const bool wide)
 {
-    const float dlt = ra.x, f = ra.y, G2 = ra.z, c = ra.w;
-    const float a2 = rb.x, lo = rb.y, hi = rb.z, cK = rb.w;
-    const float A1 = 1.5f * a2, A2 = 2.0f * a2 * G2;
-    const float qc = HK_Z2 * a2;
-    float inv_a = 0.f, y = 0.f;
-    if (kCore) {
-        inv_a = rsqrtf(a2);
-        y = sqrtf(G2) * inv_a;
-    }
+    const float2 ndl = bcast2(-A.x), nf = bcast2(-A.y), g = bcast2(A.z);
+    const float2 A1 = bcast2(B.x), nA2 = bcast2(B.y), one = bcast2(1.0f);
+    const float c = A.w, qc = B.z, lo = C.x, hi = C.y;
+    float inv_a = 0.f;
+    if (kCore && wide) inv_a = rsqrtf(qc * (1.0f / HK_Z2));
 #pragma unroll
-    for (int j = 0; j < kB; ++j) {
-        const float d = tb[j] - dlt;            // exact: both are small integers
-        const float t = d - f;
-        const float q = fmaf(t, t, G2);
-        const bool in = (tb[j] >= lo) && (tb[j] <= hi);       // exact integer extent (R7)
-        const float r = rcp_approx(q);
-        const float term = c * shape_mid(r, A1, A2);
-        if (kCore) {
-            const bool core = in && (q < qc);
-            if (in && !core) acc[j] += term;
-            if (__any_sync(0xffffffffu, core)) {
-                if (core) acc[j] = fmaf(cK, core_K(fabsf(t) * inv_a, y), acc[j]);
+    for (int m = 0; m < KB / 2; ++m) {
+        const float2 d = __fadd2_rn(tb[m], ndl);            // exact: both are small integers
+        const float2 t = __fadd2_rn(d, nf);
+        const float2 q = __ffma2_rn(t, t, g);
+        const float2 rr = rcp2(q);
+        float2 ww = rr;
+        if (kTwoTerm) {
+            const float2 uu = __ffma2_rn(nA2, rr, A1);
+            const float2 vv = __ffma2_rn(uu, rr, one);
+            ww = __fmul2_rn(rr, vv);
+        }
+        bool in0 = true, in1 = true, co0 = false, co1 = false;
+        if (kMask) {                                         // exact integer extent (R7)
+            in0 = (tb[m].x >= lo) && (tb[m].x <= hi);
+            in1 = (tb[m].y >= lo) && (tb[m].y <= hi);
+        }
+        if (kCore) { co0 = q.x < qc; co1 = q.y < qc; }
+        const float2 cm = make_float2((in0 && !co0) ? c : 0.f, (in1 && !co1) ? c : 0.f);
+        acc[m] = __ffma2_rn(cm, ww, acc[m]);
+        if (kCore && wide) {
+            if (__any_sync(0xffffffffu, in0 && co0)) {
+                if (in0 && co0) acc[m].x = fmaf(B.w, core_K(fabsf(t.x) * inv_a, C.z), acc[m].x);
             }
-        } else {
-            if (in) acc[j] += term;
+            if (__any_sync(0xffffffffu, in1 && co1)) {
+                if (in1 && co1) acc[m].y = fmaf(B.w, core_K(fabsf(t.y) * inv_a, C.z), acc[m].y);
+            }
         }
     }
 }
 
+template <int KB>
 __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
 {
-    __shared__ float4 smA[kSub];   // { jc - ct0, f, G2, c }
-    __shared__ float4 smB[kSub];   // { a2, ilo - ct0, ihi - ct0, cK }   (as floats, exact integers)
+    constexpr int kTB = 32 * KB;
+    constexpr int M = KB / 2;
+    static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubN, "red must fit in smA + smB");
+    __shared__ float4 smem[3][kSubN];          // A, B, C records (see near_rows)
+    __shared__ float sacc[kWarps][kTB];        // per-warp bin tile of the lane pass
     __shared__ int s_unit;
+    float4* smA = smem[0];
+    float4* smB = smem[1];
+    float4* smC = smem[2];
+    double* red = reinterpret_cast<double*>(&smem[0][0]);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int total = a.unit_prefix[a.n_ct];
-    const float wlo = (float)(warp * kWarpBins), whi = wlo + (float)(kWarpBins - 1);
+    const float whi = (float)(kTB - 1);
 
-    float tb[kB];
+    float2 tb[M];
 #pragma unroll
-    for (int j = 0; j < kB; ++j) tb[j] = (float)(warp * kWarpBins + lane + 32 * j);
+    for (int m = 0; m < M; ++m) {
+        float b0 = (float)(lane + 64 * m);
+        tb[m] = make_float2(b0, b0 + 32.0f);
+    }
+#pragma unroll
+    for (int j = 0; j < KB; ++j) sacc[warp][lane + 32 * j] = 0.f;
 
     for (;;) {
         const int u = next_unit(&a.st->unit_counter_near, &s_unit);
         if (u >= total) break;
         const int ct = find_tile(a.unit_prefix, a.n_ct, u);
-        const int wt_first = ct * kWarps, wt_last = min(a.n_wt, wt_first + kWarps) - 1;
-        const int64_t ct0 = (int64_t)ct * kTileBins;
-        const int cA0 = a.tr[wt_first].A0, cA1 = a.tr[wt_last].A1;
-        const int c0 = cA0 + (u - a.unit_prefix[ct]) * a.chunk;
-        const int c1 = min(c0 + a.chunk, cA1);
-        const int wt = wt_first + warp;
-        int g0[3] = {0, 0, 0}, g1[3] = {0, 0, 0};
-        if (wt <= wt_last) {
-            TileRange r = a.tr[wt];
-            g0[0] = max(r.A0, c0);  g1[0] = min(r.FL0, c1);
-            g0[1] = max(r.FL1, c0); g1[1] = min(r.FR0, c1);
-            g0[2] = max(r.FR1, c0); g1[2] = min(r.A1, c1);
-        }
-        if (!__syncthreads_or((g0[0] < g1[0]) || (g0[1] < g1[1]) || (g0[2] < g1[2]))) continue;
+        const int64_t ct0 = (int64_t)ct * kTB;
+        const TileRange r = a.tr[ct];
+        const int c0 = r.A0 + (u - a.unit_prefix[ct]) * a.chunk;
+        const int c1 = min(c0 + a.chunk, r.A1);
+        // left-edge, centre and right-edge segments clipped to the chunk, walked as one list of nt lines
+        const int g0 = max(r.A0, c0), g1 = max(r.ML1, c0), g2 = max(r.FR1, c0);
+        const int n0 = max(min(r.FL0, c1) - g0, 0), n1 = max(min(r.MR0, c1) - g1, 0), n2 = max(min(r.A1, c1) - g2, 0);
+        const int nt = n0 + n1 + n2;
+        if (nt == 0) continue;
         if (threadIdx.x == 0) atomicAdd(&a.st->units_near, 1ULL);
 
-        float acc[kB];
-        double acc64[kB];
+        float2 acc[M];
+        double acc64[KB];
 #pragma unroll
-        for (int j = 0; j < kB; ++j) { acc[j] = 0.f; acc64[j] = 0.0; }
+        for (int m = 0; m < M; ++m) acc[m] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < KB; ++j) acc64[j] = 0.0;
         int since_flush = 0;
+        auto flush = [&]() {
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                acc64[2 * m] += (double)acc[m].x + (double)sacc[warp][lane + 64 * m];
+                acc64[2 * m + 1] += (double)acc[m].y + (double)sacc[warp][lane + 64 * m + 32];
+                acc[m] = make_float2(0.f, 0.f);
+                sacc[warp][lane + 64 * m] = 0.f;
+                sacc[warp][lane + 64 * m + 32] = 0.f;
+            }
+            since_flush = 0;
+            __syncwarp();
+        };
 
-        for (int s0 = c0; s0 < c1; s0 += kSub) {
-            const int s1 = min(s0 + kSub, c1);
-            int p0[3], p1[3];
-            bool mine = false;
+        float4 preA[kLPTN], preB[kLPTN];
+        auto fetch = [&](int v0) {
 #pragma unroll
-            for (int s = 0; s < 3; ++s) {
-                p0[s] = max(g0[s], s0); p1[s] = min(g1[s], s1);
-                mine |= p0[s] < p1[s];
-            }
-            if (!__syncthreads_or(mine)) continue;
-            for (int i = threadIdx.x; i < s1 - s0; i += kThreads) {
-                float4 ra = a.recA[s0 + i], rb = a.recB[s0 + i];
-                const int64_t lim = 1 << 24;
-                int64_t dj = (int64_t)__float_as_int(ra.x) - ct0;
-                int64_t dlo = (int64_t)__float_as_int(rb.y) - ct0, dhi = (int64_t)__float_as_int(rb.z) - ct0;
-                dlo = max(-lim, min(lim, dlo));
-                dhi = max(-lim, min(lim, dhi));
-                smA[i] = make_float4((float)dj, ra.y, ra.z, ra.w);
-                smB[i] = make_float4(rb.x, (float)dlo, (float)dhi, rb.w);
-            }
-            __syncthreads();
-#pragma unroll 1
-            for (int s = 0; s < 3; ++s) {
-#pragma unroll 1
-                for (int l = p0[s] - s0; l < p1[s] - s0; ++l) {
-                    const float4 ra = smA[l], rb = smB[l];
-                    // can |z|^2 < Z2 occur anywhere in this warp's bins?  (warp-uniform)
-                    const float pos = ra.x + ra.y;
-                    const float dist = fmaxf(0.f, fmaxf(wlo - pos, pos - whi));
-                    if (fmaf(dist, dist, ra.z) < HK_Z2 * rb.x) near_line<true>(ra, rb, tb, acc);
-                    else near_line<false>(ra, rb, tb, acc);
-                    if (++since_flush >= kFlush) {
-#pragma unroll
-                        for (int j = 0; j < kB; ++j) { acc64[j] += (double)acc[j]; acc[j] = 0.f; }
-                        since_flush = 0;
-                    }
+            for (int k = 0; k < kLPTN; ++k) {
+                const int v = v0 + threadIdx.x + k * kThreads;
+                if (v < nt) {
+                    const int li = v < n0 ? g0 + v : (v < n0 + n1 ? g1 + (v - n0) : g2 + (v - n0 - n1));
+                    preA[k] = a.recA[li];
+                    preB[k] = a.recB[li];
                 }
             }
-        }
-        const double inv_scale = scalbn(1.0, -a.st->scale_exp);
+        };
+        auto stash = [&](int v0) {
 #pragma unroll
-        for (int j = 0; j < kB; ++j) {
-            const int64_t b = ct0 + warp * kWarpBins + lane + 32 * j;
-            double v = (acc64[j] + (double)acc[j]) * inv_scale;
-            if (b < a.N && v != 0.0) atomicAdd(a.out_k + b, v);
+            for (int k = 0; k < kLPTN; ++k) {
+                const int i = threadIdx.x + k * kThreads;
+                if (v0 + i < nt) {
+                    const float4 ra = preA[k], rb = preB[k];
+                    const int64_t lim = 1 << 24;
+                    const int64_t dj = (int64_t)__float_as_int(ra.x) - ct0;
+                    int64_t dlo = (int64_t)__float_as_int(rb.y) - ct0, dhi = (int64_t)__float_as_int(rb.z) - ct0;
+                    dlo = max(-lim, min(lim, dlo));
+                    dhi = max(-lim, min(lim, dhi));
+                    const float fdj = (float)dj, flo = (float)dlo, fhi = (float)dhi;
+                    const float G2 = ra.z, a2 = rb.x;
+                    const float qc = HK_Z2 * a2;
+                    // smallest q = t^2 + G2 over the tile's bins, from below
+                    const float pos = fdj + ra.y;
+                    const float dist = fmaxf(fmaxf(-pos, pos - whi), 0.f) * 0.999f;
+                    const float qmin = fmaf(dist, dist, G2) * 0.9999f;
+                    int flags = 0;
+                    if (flo <= 0.f && fhi >= whi) flags |= kFlagFull;
+                    if (qmin >= qc) flags |= kFlagNoCore;
+                    if (qmin >= HK_Z1 * a2) flags |= kFlagFar;
+                    if ((qc - G2) >= kWideCore) flags |= kFlagWide;
+                    smA[i] = make_float4(fdj, ra.y, G2, ra.w);
+                    smB[i] = make_float4(1.5f * a2, -2.0f * a2 * G2, qc, rb.w);
+                    smC[i] = make_float4(flo, fhi, sqrtf(G2) * rsqrtf(a2), __int_as_float(flags));
+                }
+            }
+        };
+        fetch(0);
+        for (int v0 = 0; v0 < nt; v0 += kSubN) {
+            __syncthreads();                        // previous batch fully consumed
+            stash(v0);
+            __syncthreads();
+            if (v0 + kSubN < nt) fetch(v0 + kSubN);
+            int wl0, wl1;
+            warp_share(min(kSubN, nt - v0), warp, wl0, wl1);
+            // ---- row pass: lanes own bins, the warp walks its lines
+#pragma unroll 1
+            for (int l = wl0; l < wl1; ++l) {
+                const float4 A = smA[l], B = smB[l], C = smC[l];
+                const int flags = __float_as_int(C.w);
+                if (flags & kFlagFar) {
+                    if (flags & kFlagFull) near_rows<KB, false, false, false>(acc, tb, A, B, C, false);
+                    else near_rows<KB, false, true, false>(acc, tb, A, B, C, false);
+                } else if (flags & kFlagNoCore) {
+                    if (flags & kFlagFull) near_rows<KB, true, false, false>(acc, tb, A, B, C, false);
+                    else near_rows<KB, true, true, false>(acc, tb, A, B, C, false);
+                } else {
+                    near_rows<KB, true, true, true>(acc, tb, A, B, C, (flags & kFlagWide) != 0);
+                }
+                if (++since_flush >= kFlush) flush();
+            }
+            // ---- lane pass: lane <-> line, each lane walks its line's narrow core (|z|^2 < Z2) inside this tile
+#pragma unroll 1
+            for (int lb = wl0; lb < wl1; lb += 32) {
+                const int l = lb + lane;
+                float dlt = 0.f, f = 0.f, G2 = 0.f, cK = 0.f, qc = 0.f, y = 0.f;
+                int cnt = 0;
+                float clo = 0.f;
+                if (l < wl1) {
+                    const float4 A = smA[l], B = smB[l], C = smC[l];
+                    const int flags = __float_as_int(C.w);
+                    if (!(flags & (kFlagNoCore | kFlagWide))) {
+                        dlt = A.x; f = A.y; G2 = A.z; cK = B.w; qc = B.z; y = C.z;
+                        const float h2 = qc - G2;
+                        const float hw = sqrtf(fmaxf(h2, 0.f)) + 1.0f;           // |t| < hw covers every q < qc
+                        const float pos = dlt + f;
+                        clo = fmaxf(fmaxf(ceilf(pos - hw), C.x), 0.f);
+                        const float chi = fminf(fminf(floorf(pos + hw), C.y), whi);
+                        if (h2 > 0.f && chi >= clo) cnt = (int)(chi - clo) + 1;
+                    }
+                }
+                int maxcnt = cnt;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) maxcnt = max(maxcnt, __shfl_xor_sync(0xffffffffu, maxcnt, o));
+                if (maxcnt == 0) continue;
+                const float inv_a = rsqrtf(fmaxf(qc, 1e-30f) * (1.0f / HK_Z2));
+                for (int o = 0; o < maxcnt; ++o) {
+                    float val = 0.f;
+                    int bin = -1;
+                    if (o < cnt) {
+                        const float fb = clo + (float)o;
+                        const float d = fb - dlt;
+                        const float t = d - f;
+                        const float q = fmaf(t, t, G2);
+                        if (q < qc) { val = cK * core_K(fabsf(t) * inv_a, y); bin = (int)fb; }
+                    }
+                    // combine equal bins in the warp (sorted lines: neighbours share bins), one add per distinct bin
+                    unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
+                    while (todo) {
+                        const int leader = __ffs(todo) - 1;
+                        const int b = __shfl_sync(0xffffffffu, bin, leader);
+                        const bool mine = (bin == b);
+                        float sum = mine ? val : 0.f;
+#pragma unroll
+                        for (int x = 16; x > 0; x >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, x);
+                        if (lane == leader) sacc[warp][b] += sum;
+                        todo &= ~__ballot_sync(0xffffffffu, mine);
+                    }
+                }
+                since_flush += 32;     // the tile holds at most 32 lines' terms per bin per pass
+                if (since_flush >= kFlush) flush();
+            }
         }
+        flush();
+        __syncthreads();               // every warp is done with the staging buffers: red may overwrite them
+        flush_tile<KB>(red, acc64, ct0, a);
     }
 }
 

@@ -9,6 +9,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <type_traits>
 
 #include "hk_accumulate.cuh"
 
@@ -23,13 +24,14 @@ struct hk_ctx {
     size_t ws_bytes;
     int cuda_err;
     int debug_mode;
-    int n_sm, occ_far, occ_near;
+    int force_kb;
+    int n_sm;
     // last compute
     bool have_run;
     int64_t last_n;
     double last_cut;
     cudaStream_t last_stream;
-    int32_t last_sort_bits;
+    int32_t last_sort_bits, last_kb;
     int64_t last_launches;
     DevStats* d_stats;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
@@ -48,7 +50,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 struct Layout {
     size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, tr, counts, prefix, cub;
     size_t cub_bytes, total;
-    int32_t n_wt, n_ct;
+    int32_t n_ct;
 };
 
 bool is_uncut(double cut) { return !(cut > 0.0 && std::isfinite(cut)); }
@@ -63,11 +65,24 @@ size_t cub_temp_bytes(int64_t n, int32_t n_ct)
     return b1 > b2 ? b1 : b2;
 }
 
+constexpr int kMinKB = 2;     // smallest tile geometry: the workspace is sized for it
+
+// bins per lane from the half-extent in bins: wide extents amortise the per-line work over more
+// bins; narrow ones need small warp tiles so that most (line, tile) pairs are interior.
+int pick_kb(const hk_ctx* c, double cut)
+{
+    if (c->force_kb) return c->force_kb;
+    if (is_uncut(cut)) return 8;
+    const double cb = cut / c->dnu;
+    if (cb >= 4096.0) return 8;
+    if (cb >= 1024.0) return 4;
+    return 2;
+}
+
 Layout make_layout(const hk_ctx* c, int64_t n)
 {
     Layout L;
-    L.n_wt = (int32_t)((c->N + kWarpBins - 1) / kWarpBins);
-    L.n_ct = (int32_t)((c->N + kTileBins - 1) / kTileBins);
+    L.n_ct = (int32_t)((c->N + 32 * kMinKB - 1) / (32 * kMinKB));
     size_t nn = (size_t)(n > 0 ? n : 1);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -79,7 +94,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     L.recU = take(nn * sizeof(RecU));
     L.recA = take(nn * 16);
     L.recB = take(nn * 16);
-    L.tr = take((size_t)L.n_wt * sizeof(TileRange));
+    L.tr = take((size_t)L.n_ct * sizeof(TileRange));
     L.counts = take(((size_t)L.n_ct + 1) * 4);
     L.prefix = take(((size_t)L.n_ct + 1) * 4);
     L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_ct);
@@ -128,20 +143,21 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
         p.kmin = -(1LL << 30);
         p.ksent = INT32_MAX;
     }
-    p.kappa = std::sqrt((double)HK_Z1) * p.beta * 1.001;
+    p.kappa1 = std::sqrt((double)HK_Z1) * p.beta * 1.001;
+    p.kappa2 = std::sqrt((double)HK_Z2) * p.beta * 1.001;
     p.numin_bins = c->numin / c->dnu;
-    p.n_wt = (int32_t)((c->N + kWarpBins - 1) / kWarpBins);
-    p.n_ct = (int32_t)((c->N + kTileBins - 1) / kTileBins);
+    p.kb = pick_kb(c, cut);
+    p.n_ct = (int32_t)((c->N + 32 * p.kb - 1) / (32 * p.kb));
     p.chunk = chunk;
-    p.force_near = c->debug_mode == 1;
+    p.mode = c->debug_mode;
     return p;
 }
 
 int32_t pick_chunk(const hk_ctx* c, int64_t n, double cut)
 {
-    double tiles_per_line = is_uncut(cut) ? (double)((c->N + kTileBins - 1) / kTileBins)
-                                          : std::fmin(2.0 * cut / c->dnu / kTileBins + 1.0,
-                                                      (double)((c->N + kTileBins - 1) / kTileBins));
+    const double tile = 32.0 * pick_kb(c, cut);
+    const double n_ct = std::ceil((double)c->N / tile);
+    double tiles_per_line = is_uncut(cut) ? n_ct : std::fmin(2.0 * cut / c->dnu / tile + 1.0, n_ct);
     double pairs = (double)n * tiles_per_line;
     double want = pairs / ((double)c->n_sm * 32.0);
     int64_t ch = (int64_t)std::ceil(want / 256.0) * 256;
@@ -206,11 +222,7 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_far, far_kernel, kThreads, 0);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ_near, near_kernel, kThreads, 0);
     if (e != cudaSuccess) { delete c; return HK_ECUDA; }
-    if (c->occ_far < 1) c->occ_far = 1;
-    if (c->occ_near < 1) c->occ_near = 1;
     for (int i = 0; i <= HK_PH_COUNT && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
     for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
         e = cudaEventCreateWithFlags(&c->ev_h2d[i], cudaEventDisableTiming);
@@ -265,8 +277,15 @@ int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes)
 
 int hk_set_debug_mode(hk_ctx* ctx, int mode)
 {
-    if (!ctx || mode < 0 || mode > 1) return HK_EINVAL;
+    if (!ctx || mode < 0 || mode > 2) return HK_EINVAL;
     ctx->debug_mode = mode;
+    return HK_OK;
+}
+
+int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane)
+{
+    if (!ctx || !(bins_per_lane == 0 || bins_per_lane == 2 || bins_per_lane == 4 || bins_per_lane == 8)) return HK_EINVAL;
+    ctx->force_kb = bins_per_lane;
     return HK_OK;
 }
 
@@ -295,6 +314,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     ctx->d_stats = st;
     ctx->last_sort_bits = 0;
     ctx->last_launches = 0;
+    ctx->last_kb = p.kb;
     if (n == 0) {
         for (int i = 1; i <= HK_PH_COUNT; ++i) HK_CUDA(cudaEventRecord(ctx->ev[i], stream));
         return HK_OK;
@@ -325,7 +345,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges and work units
-    range_kernel<<<(p.n_wt + 255) / 256, 256, 0, stream>>>(p, keys_out, n, tr, st);
+    range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, keys_out, n, tr, st);
     HK_CUDA(cudaMemsetAsync(counts, 0, ((size_t)p.n_ct + 1) * 4, stream));
     unit_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, tr, counts);
     cub_bytes = L.cub_bytes;
@@ -334,15 +354,22 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     // a4-a7: accumulate
     AccArgs a;
     a.recA = recA; a.recB = recB; a.tr = tr; a.unit_prefix = prefix; a.st = st; a.out_k = out_k_dev;
-    a.N = ctx->N; a.n_wt = p.n_wt; a.n_ct = p.n_ct; a.chunk = p.chunk;
+    a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk;
     ctx->last_launches = 6;
-    if (!p.force_near) {
-        far_kernel<<<ctx->n_sm * ctx->occ_far, kThreads, 0, stream>>>(a);
+    const int grid = ctx->n_sm * 2;
+    auto launch = [&](auto kb_tag) {
+        constexpr int KB = decltype(kb_tag)::value;
+        if (p.mode == 0) { interior_kernel<KB, false><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream);
+        if (p.mode != 1) { interior_kernel<KB, true><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
+        near_kernel<KB><<<grid, kThreads, 0, stream>>>(a);
         ++ctx->last_launches;
-    }
-    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream));
-    near_kernel<<<ctx->n_sm * ctx->occ_near, kThreads, 0, stream>>>(a);
-    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream));
+        cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream);
+    };
+    if (p.kb == 8) launch(std::integral_constant<int, 8>());
+    else if (p.kb == 4) launch(std::integral_constant<int, 4>());
+    else launch(std::integral_constant<int, 2>());
     HK_CUDA(cudaGetLastError());
     return HK_OK;
 }
@@ -517,7 +544,10 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_evals_mid = (int64_t)(d.n_cnt_mid - d.n_cnt_core);
     host_out->n_evals_core = (int64_t)d.n_cnt_core;
     host_out->n_units_far = (int64_t)d.units_far;
+    host_out->n_units_mid = (int64_t)d.units_mid;
     host_out->n_units_near = (int64_t)d.units_near;
+    host_out->n_pairs_mid = (int64_t)d.pairs_mid;
+    host_out->bins_per_lane = ctx->last_kb;
     host_out->n_pairs_far = (int64_t)d.pairs_far;
     host_out->n_pairs_near = (int64_t)d.pairs_near;
     host_out->n_launches = ctx->last_launches;

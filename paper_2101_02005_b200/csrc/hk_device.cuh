@@ -17,15 +17,14 @@ constexpr double kNA = 6.02214076e23;    // 1/mol
 constexpr double kTref = 296.0;          // K (Eq. 5; BASELINE.json config 1)
 constexpr double kPi = 3.141592653589793238462643383279502884;
 
-// ---- geometry of the accumulation kernels
-constexpr int kB = 8;                    // bins per lane (registers)
-constexpr int kWarpBins = 32 * kB;       // bins per warp tile
+// ---- geometry of the accumulation kernels (KB = bins per lane is a template parameter: 2, 4 or 8)
 constexpr int kWarps = 8;                // warps per CTA
 constexpr int kThreads = 32 * kWarps;
-constexpr int kTileBins = kWarpBins * kWarps;  // bins per CTA tile
 constexpr int kSub = 512;                // line records staged in shared memory at a time
 constexpr int kFlush = 128;              // fp32 partial sums hold at most this many lines
-constexpr int kFarMinDist = 128;         // far kernel only sees |t| >= this many bins
+// interior (mask-free) kernels only see |t| >= 2*KB bins: with the centre position held as ONE fp32
+// relative to the tile (|tl| <= 32 KB + |t|) the rounding of t stays below 2^-24 (1 + 16) |t| = 1.0e-6 |t|
+constexpr int kMinDistPerKB = 2;
 
 constexpr int32_t kKeySentinelBias = 1;  // sentinel key = kmax + 1
 
@@ -44,9 +43,9 @@ struct __align__(16) RecU {
 //   A = { jc (int bits), f, G2, c }        c  = scale * S * Gamma_L/(pi dnu^2)   (Lorentz amplitude, bin units)
 //   B = { a2, ilo (int bits), ihi (int bits), cK }   cK = scale * S/(alpha_D sqrt(pi))
 
-// per warp tile: candidate range [A0,A1) and the two far-interior ranges inside it
-struct TileRange {
-    int32_t A0, FL0, FL1, FR0, FR1, A1;
+// per warp tile: the candidate range [A0,A1) of sorted line indices and its split (hk_accumulate.cuh)
+struct __align__(16) TileRange {
+    int32_t A0, FL0, FL1, ML1, MR0, FR0, FR1, A1;
 };
 
 // ---- small helpers
@@ -79,7 +78,11 @@ __device__ __forceinline__ float shape_mid(float r, float A1, float A2)
     return r * v;
 }
 
-// Re w(x + i y), x >= 0, y >= 0, intended for x^2 + y^2 < ~700.
+// Re w(x + i y), x >= 0, y > 0, intended for x^2 + y^2 < ~700.
+// K = (h y/pi) sum_n exp(-t_n^2)/((x-t_n)^2 + y^2) + pole term, t_n = (n + s) h, h = 0.8, n = -5..5
+// (Matta & Reichel 1971 / Hunter & Regan 1972: the family Algorithm 916, which the paper uses in region C
+// (L156), belongs to).  Two node sets (s = 0, 1/2), chosen per evaluation so that x is never within h/4
+// of a node; two nodes share one reciprocal.  The oracle uses h = 1/2, 29 nodes, fp64 and no node shift.
 __device__ __noinline__ float core_K(float x, float y)
 {
     constexpr float h = 0.8f;
@@ -91,34 +94,47 @@ __device__ __noinline__ float core_K(float x, float y)
     constexpr float wB[11] = {2.35257520e-06f, 3.93669041e-04f, 1.83156389e-02f, 2.36927759e-01f,
                               8.52143789e-01f, 8.52143789e-01f, 2.36927759e-01f, 1.83156389e-02f,
                               3.93669041e-04f, 2.35257520e-06f, 3.90893843e-09f};
-    float u = x * inv_h;
-    float fr = u - floorf(u);
-    bool on = (fr >= 0.25f) && (fr < 0.75f);        // integer nodes are >= h/4 away
-    float s = on ? 0.0f : 0.5f;
-    float us = u - s;
-    float frs = us - floorf(us);                    // in [1/4, 3/4]
-    float y2 = y * y;
+    const float u = x * inv_h;
+    const float fr = u - floorf(u);
+    const bool on = (fr >= 0.25f) && (fr < 0.75f);        // integer nodes are >= h/4 away
+    const float s = on ? 0.0f : 0.5f;
+    const float us = u - s;
+    const float frs = us - floorf(us);                    // in [1/4, 3/4]
+    const float y2 = y * y;
+    const float xs = fmaf(-s, h, x);                      // x - s h
+    float q[11];
+#pragma unroll
+    for (int n = 0; n < 11; ++n) {
+        const float d = xs - (float)(n - 5) * h;
+        q[n] = fmaf(d, d, y2);                            // >= (h/4)^2
+    }
     float sum = 0.0f;
 #pragma unroll
-    for (int n = -5; n <= 5; ++n) {
-        float tn = fmaf(s, h, (float)n * h);
-        float d = x - tn;
-        float w = on ? wA[n + 5] : wB[n + 5];
-        sum = fmaf(w, rcp_approx(fmaf(d, d, y2)), sum);
+    for (int n = 0; n < 10; n += 2) {
+        // w1/q1 + w2/q2 = (w1 q2 + w2 q1)/(q1 q2)
+        const float w1 = on ? wA[n] : wB[n], w2 = on ? wA[n + 1] : wB[n + 1];
+        const float num = fmaf(w2, q[n], w1 * q[n + 1]);
+        sum = fmaf(num, rcp_approx(q[n] * q[n + 1]), sum);
     }
+    sum = fmaf(on ? wA[10] : wB[10], rcp_approx(q[10]), sum);
     float K = sum * (y * (h / 3.14159265358979f));
-    float re2 = fmaf(x, x, -y2);
-    if (y < 3.92699082f /* pi/h */ && re2 < 80.0f) {
-        // + Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) }
-        float amp = 2.0f * __expf(-re2);
+    const float re2 = fmaf(x, x, -y2);
+    if (y < 3.92699082f /* pi/h */ && re2 < 40.0f) {
+        // + Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) };  below exp(-40) the term is < 1e-10 of K
+        const float amp = 2.0f * __expf(-re2);
+        // exp(-z^2) = exp(-re2) (cos phi - i sin phi), phi = 2 x y reduced to [-pi, pi] first
+        const float phi = 2.0f * x * y;
+        const float kk = rintf(phi * 0.159154943f);
+        float ph = fmaf(-kk, 6.28318548f, phi);
+        ph = fmaf(-kk, -1.74845553e-07f, ph);             // 2 pi = 6.28318548 - 1.74845553e-07
         float sp, cp;
-        sincosf(2.0f * x * y, &sp, &cp);
-        float nr = amp * cp, ni = -amp * sp;
-        float e = __expf(7.85398163f /* 2 pi/h */ * y);
+        __sincosf(ph, &sp, &cp);
+        const float nr = amp * cp, ni = -amp * sp;
+        const float e = __expf(7.85398163f /* 2 pi/h */ * y);
         float st, ct;
-        sincospif(2.0f * frs, &st, &ct);            // theta = 2 pi frac(x/h - s), cos(theta) <= 0
-        float dr = fmaf(-e, ct, 1.0f), di = e * st;
-        K += (nr * dr + ni * di) / fmaf(dr, dr, di * di);
+        sincospif(2.0f * frs, &st, &ct);                  // theta = 2 pi frac(x/h - s), cos(theta) <= 0
+        const float dr = fmaf(-e, ct, 1.0f), di = e * st;
+        K = fmaf(fmaf(nr, dr, ni * di), rcp_approx(fmaf(dr, dr, di * di)), K);
     }
     return K;
 }

@@ -27,11 +27,12 @@ struct Params {
     int32_t ksent;
     // tile ranges
     int64_t cb_floor, cb_ceil;  // floor/ceil of cut/dnu (bins)
-    double kappa;               // sqrt(Z1) * beta, slightly inflated
+    double kappa1, kappa2;      // sqrt(Z1) * beta and sqrt(Z2) * beta, slightly inflated
     double numin_bins;          // numin / dnu
-    int32_t n_wt, n_ct;         // warp tiles, CTA tiles
+    int32_t kb;                 // bins per lane (2, 4, 8)
+    int32_t n_ct;               // tiles of 32 kb bins
     int32_t chunk;              // lines per work unit
-    int force_near;             // debug: no far-interior ranges
+    int mode;                   // debug: 0 default, 1 everything through the near kernel, 2 far pairs through the mid kernel
 };
 
 struct DevStats {
@@ -39,9 +40,9 @@ struct DevStats {
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
     int32_t pad;
-    unsigned int unit_counter_far, unit_counter_near;
-    unsigned long long units_far, units_near;
-    unsigned long long pairs_far, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
+    unsigned int unit_counter_far, unit_counter_mid, unit_counter_near, pad2;
+    unsigned long long units_far, units_mid, units_near;
+    unsigned long long pairs_far, pairs_mid, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
 };
 
 __device__ __forceinline__ bool finite6(double a, double b, double c, double d, double e, double f)
@@ -210,17 +211,32 @@ __device__ __forceinline__ int32_t lower_bound_key(const int32_t* __restrict__ k
     return lo;
 }
 
-// Per warp tile [w0, w1): candidate lines and the far-interior sub-ranges.  A line is
-// "far interior" for the tile when every bin of the tile lies inside its extent and at
-// |t| >= max(kFarMinDist, sqrt(Z1) a): then |z|^2 >= Z1 for every (line, bin) pair and the
-// far kernel may run mask-free.  All bounds are conservative.
+// Per tile [w0, w1): candidate lines and their split into edge / far / mid / centre ranges.
+// A line is "interior" for the tile when every bin of the tile lies inside its extent and at
+// |t| >= max(16 KB, sqrt(Z) a): then |z|^2 >= Z for every (line, bin) pair (Z = Z1: far, Z = Z2: mid)
+// and the interior kernels may run mask-free.  alpha_D = beta nu0 is a function of the centre, so the
+// condition is a bound on the centre bin alone; all bounds are conservative.
+__device__ __forceinline__ int64_t left_bound(double w0, double kap, double numin_bins)
+{
+    // pos + 1 <= (w0 - kap numin_bins) / (1 + kap)   =>   w0 - pos >= kap (numin_bins + pos)
+    return (int64_t)floor((w0 - kap * (numin_bins + 1.0)) / (1.0 + kap)) - 3;
+}
+__device__ __forceinline__ int64_t right_bound(double w1m1, double kap, double numin_bins)
+{
+    // pos >= (w1 - 1 + kap numin_bins) / (1 - kap)   =>   pos - (w1 - 1) >= kap (numin_bins + pos)
+    if (!(kap < 0.9)) return INT64_MAX / 2;
+    return (int64_t)ceil((w1m1 + kap * (numin_bins + 1.0)) / (1.0 - kap)) + 3;
+}
+
 __global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __restrict__ keys, int32_t n,
                                                     TileRange* __restrict__ tr, DevStats* __restrict__ st)
 {
     int wt = blockIdx.x * blockDim.x + threadIdx.x;
-    if (wt >= p.n_wt) return;
-    const int64_t w0 = (int64_t)wt * kWarpBins;
-    const int64_t w1 = min(p.N, w0 + kWarpBins);
+    if (wt >= p.n_ct) return;
+    const int wb = 32 * p.kb;
+    const int64_t mind = (int64_t)kMinDistPerKB * p.kb;
+    const int64_t w0 = (int64_t)wt * wb;
+    const int64_t w1 = min(p.N, w0 + wb);
     const int32_t n_act = lower_bound_key(keys, n, (int64_t)p.ksent);
     int64_t jlo, jhi;                       // candidate centre bins
     if (p.uncut) { jlo = INT64_MIN / 2; jhi = INT64_MAX / 2; }
@@ -228,31 +244,38 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __r
     TileRange r;
     r.A0 = p.uncut ? 0 : lower_bound_key(keys, n_act, jlo - p.kmin);
     r.A1 = p.uncut ? n_act : lower_bound_key(keys, n_act, jhi + 1 - p.kmin);
-    // far-left: jc <= jL
-    double kap = p.kappa;
-    int64_t jL = (int64_t)floor(((double)(w0 - 1) - kap * (p.numin_bins + 1.0)) / (1.0 + kap)) - 2;
-    jL = min(jL, w0 - 1 - kFarMinDist);
-    int64_t jLmin = p.uncut ? INT64_MIN / 2 : w1 - p.cb_floor;       // extent must reach the tile's last bin
-    // far-right: jc >= jR
-    int64_t jR = INT64_MAX / 2;
-    if (kap < 0.9) jR = (int64_t)ceil(((double)(w1 - 1) + kap * (p.numin_bins + 1.0)) / (1.0 - kap)) + 2;
-    jR = max(jR, w1 - 1 + kFarMinDist);
-    int64_t jRmax = p.uncut ? INT64_MAX / 2 : w0 + p.cb_floor - 2;   // extent must reach the tile's first bin
-    if (p.force_near) { jL = INT64_MIN / 2; jR = INT64_MAX / 2; }
+    // left of the tile: the extent must reach the tile's last bin (jc >= jLmin)
+    const int64_t jLmin = p.uncut ? INT64_MIN / 2 : w1 - p.cb_floor;
+    int64_t jLfar = min(left_bound((double)w0, p.kappa1, p.numin_bins), w0 - 1 - mind);
+    int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.numin_bins), w0 - 1 - mind);
+    // right of the tile: the extent must reach the tile's first bin (jc <= jRmax)
+    const int64_t jRmax = p.uncut ? INT64_MAX / 2 : w0 + p.cb_floor - 2;
+    int64_t jRfar = max(right_bound((double)(w1 - 1), p.kappa1, p.numin_bins), w1 - 1 + mind);
+    int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.numin_bins), w1 - 1 + mind);
+    if (p.mode == 1) { jLfar = jLmid = INT64_MIN / 2; jRfar = jRmid = INT64_MAX / 2; }
+    if (p.mode == 2) { jLfar = INT64_MIN / 2; jRfar = INT64_MAX / 2; }
     int32_t fl0 = lower_bound_key(keys, n_act, jLmin - p.kmin);
-    int32_t fl1 = lower_bound_key(keys, n_act, jL + 1 - p.kmin);
-    int32_t fr0 = lower_bound_key(keys, n_act, jR - p.kmin);
+    int32_t fl1 = lower_bound_key(keys, n_act, jLfar + 1 - p.kmin);
+    int32_t ml1 = lower_bound_key(keys, n_act, jLmid + 1 - p.kmin);
+    int32_t mr0 = lower_bound_key(keys, n_act, jRmid - p.kmin);
+    int32_t fr0 = lower_bound_key(keys, n_act, jRfar - p.kmin);
     int32_t fr1 = lower_bound_key(keys, n_act, jRmax + 1 - p.kmin);
-    fl0 = max(fl0, r.A0); fl1 = min(fl1, r.A1); if (fl1 < fl0) fl1 = fl0;
-    fr0 = max(fr0, fl1);  fr1 = min(fr1, r.A1); if (fr1 < fr0) fr0 = fr1;
-    if (fr0 < fl1) fr0 = fr1 = fl1;
-    r.FL0 = fl0; r.FL1 = fl1; r.FR0 = fr0; r.FR1 = fr1;
+    // make the sequence monotone inside [A0, A1]; every adjustment only shrinks an interior class
+    fl0 = min(max(fl0, r.A0), r.A1);
+    fl1 = min(max(fl1, fl0), r.A1);
+    ml1 = min(max(ml1, fl1), r.A1);
+    fr1 = max(min(fr1, r.A1), ml1);
+    fr0 = max(min(fr0, fr1), ml1);
+    mr0 = max(min(mr0, fr0), ml1);
+    r.FL0 = fl0; r.FL1 = fl1; r.ML1 = ml1; r.MR0 = mr0; r.FR0 = fr0; r.FR1 = fr1;
     tr[wt] = r;
     const unsigned long long nb = (unsigned long long)(w1 - w0);
     const unsigned long long nfar = (unsigned long long)(fl1 - fl0) + (unsigned long long)(fr1 - fr0);
+    const unsigned long long nmid = (unsigned long long)(ml1 - fl1) + (unsigned long long)(fr0 - mr0);
     const unsigned long long nall = (unsigned long long)(r.A1 - r.A0);
     if (nfar) atomicAdd(&st->pairs_far, nfar * nb);
-    if (nall > nfar) atomicAdd(&st->pairs_near, (nall - nfar) * nb);
+    if (nmid) atomicAdd(&st->pairs_mid, nmid * nb);
+    if (nall > nfar + nmid) atomicAdd(&st->pairs_near, (nall - nfar - nmid) * nb);
 }
 
 // Per CTA tile: number of line chunks over the union of its warp tiles' candidates.
@@ -260,8 +283,7 @@ __global__ void __launch_bounds__(256) unit_kernel(Params p, const TileRange* __
 {
     int ct = blockIdx.x * blockDim.x + threadIdx.x;
     if (ct >= p.n_ct) return;
-    int wt0 = ct * kWarps, wt1 = min(p.n_wt, wt0 + kWarps) - 1;
-    int64_t len = (int64_t)tr[wt1].A1 - tr[wt0].A0;
+    int64_t len = (int64_t)tr[ct].A1 - tr[ct].A0;
     counts[ct] = len > 0 ? (int32_t)((len + p.chunk - 1) / p.chunk) : 0;
 }
 

@@ -27,10 +27,11 @@ def _to_cuda(lines_np):
     return {k: torch.as_tensor(np.ascontiguousarray(v), dtype=torch.float64).cuda() for k, v in lines_np.items()}
 
 
-def _gpu_k(B, lines_np, cond, grid, cut, debug_mode=0):
+def _gpu_k(B, lines_np, cond, grid, cut, debug_mode=0, tile_bins=0):
     op = B.Opacity(*grid)
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
     op.set_debug_mode(debug_mode)
+    op.set_tile_bins(tile_bins)
     dl = _to_cuda(lines_np)
     k = op.compute(dl, cut)
     torch.cuda.synchronize()
@@ -98,14 +99,54 @@ def test_uncut_atom_like_sampled_bins(B):
 
 
 def test_cross_path_near_vs_default(B):
-    """force every (tile, line) pair through the masked near kernel and
-    compare with the default far/mid/near split on all bins."""
+    """force every (tile, line) pair through the masked near kernel (mode 1), or the far
+    pairs through the mid kernel (mode 2), and compare with the default far/mid/near split on all bins."""
     for cfg, n in [(2, 20_000), (4, 6_000)]:
         lines, cond, grid, cut = _mini(cfg, n)
-        k0, _, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=0)
-        k1, _, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=1)
+        k0, st0, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=0)
+        assert st0["n_pairs_far"] > 0 and st0["n_pairs_mid"] > 0 and st0["n_pairs_near"] > 0
         big = k0 >= 1e-8 * k0.max()
-        assert np.abs(k1[big] / k0[big] - 1.0).max() <= 4e-5
+        for mode in (1, 2):
+            k1, st1, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=mode)
+            assert st1["n_pairs_far"] == 0
+            assert np.abs(k1[big] / k0[big] - 1.0).max() <= 4e-5
+
+
+@pytest.mark.parametrize("tile_bins", [2, 4, 8])
+@pytest.mark.parametrize("cfg,n", [(1, None), (2, 20_000), (3, 200_000)])
+def test_every_tile_geometry(B, cfg, n, tile_bins):
+    """Each tile geometry (bins per lane 2/4/8) on each workload shape against the oracle."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    k_gpu, st, _ = _gpu_k(B, lines, cond, grid, cut, tile_bins=tile_bins)
+    assert st["bins_per_lane"] == tile_bins
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    assert st["n_evals"] == evals
+    check_parity(k_gpu, k_ref, what=f"config {cfg} tile_bins {tile_bins}")
+
+
+def test_host_pipeline_and_accumulate(B):
+    """hk_compute_host (blocks copied host->device while the previous block computes) and
+    hk_accumulate (block-wise sum) against the one-shot device result and the oracle."""
+    lines, cond, grid, cut = _mini(2, 30_000)
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    hl = {k: torch.as_tensor(v).pin_memory() for k, v in lines.items()}
+    for block in (0, 7_000, 30_000, 100_000):
+        k_host = op.compute_host(hl, cut, block_lines=block)
+        st = op.stats()
+        assert st["n_evals"] == evals and st["n_lines"] == 30_000
+        check_parity(k_host.numpy(), k_ref, what=f"host pipeline block {block}")
+    k_page = op.compute_host({k: torch.as_tensor(v) for k, v in lines.items()}, cut,
+                             out=torch.empty(op.N, dtype=torch.float64), block_lines=9_000)   # pageable memory
+    check_parity(k_page.numpy(), k_ref, what="host pipeline, pageable")
+    dl = _to_cuda(lines)
+    k = torch.zeros(op.N, dtype=torch.float64, device="cuda")
+    for a, b in ((0, 11_000), (11_000, 11_000), (11_000, 30_000)):          # includes an empty block
+        op.compute({f: v[a:b].contiguous() for f, v in dl.items()}, cut, out=k, accumulate=True)
+    torch.cuda.synchronize()
+    check_parity(k.cpu().numpy(), k_ref, what="hk_accumulate")
+    op.close()
 
 
 # ---- per-line parameters (step a1) ----------------------------------------------------
