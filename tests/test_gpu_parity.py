@@ -383,6 +383,9 @@ def test_config5_full_size_sampled(B):
 def test_bt2_shaped_full_size_sampled(B, cfg):
     """The bench workload (config 4) and its coarse twin (config 3) at 5e8 lines, in the launch
     configuration bench.py times; the oracle sums every line within the cut on sampled bins."""
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 120e9:
         pytest.skip("needs ~110 GB of device memory")

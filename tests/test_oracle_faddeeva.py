@@ -86,3 +86,16 @@ def test_small_y_on_nodes_documented_limit():
         ref = special.wofz(x + 1j * y).real
         got = O.voigt_K(x, np.full_like(x, y))
         np.testing.assert_allclose(got, ref, rtol=4e-16 / y + 1e-13)
+
+
+def test_golden_mpmath_table():
+    """tests/golden/faddeeva_mpmath.txt: Re[exp(-z^2) erfc(-iz)] at 60 digits (mpmath), the definition of the
+    Faddeeva function the Voigt profile is built on; independent of the oracle's trapezoid rule."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "faddeeva_mpmath.txt")
+    tab = np.loadtxt(path)
+    assert tab.shape[0] >= 150
+    got = O.voigt_K(tab[:, 0], tab[:, 1])
+    rel = np.abs(got / tab[:, 2] - 1.0)
+    # documented limit of the oracle: ~1e-16 h/(pi y) on a node; the table has y >= 1e-3
+    assert rel.max() < 2e-12, (rel.max(), tab[rel.argmax()])
