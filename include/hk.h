@@ -70,19 +70,24 @@ typedef struct {
     int64_t n_pairs_far;   /* (line, bin) pairs the far kernel evaluated (mask-free Lorentzian) */
     int64_t n_pairs_mid;   /* (line, bin) pairs the mid kernel evaluated (mask-free two-term asymptotic) */
     int64_t n_pairs_near;  /* (line, bin) slots the near kernel walked (masked; includes bins outside extents) */
+    int64_t n_units_node;  /* ... by the node kernel */
+    int64_t n_pairs_node;  /* (line, tile) pairs evaluated at the tile's HK_NODES Chebyshev nodes (two-term asymptotic) */
+    int64_t n_bins_node;   /* (line, bin) pairs those node evaluations stand for */
     int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
     int32_t sort_bits;     /* radix-sort key width used */
-    int32_t bins_per_lane; /* tile geometry used: a warp owns 32 x this many bins, a CTA 256 x */
-    int32_t reserved;
+    int32_t bins_per_lane; /* tile geometry used: a level-0 tile is 32 x this many bins */
+    int32_t n_levels;      /* levels of the node hierarchy used (0: direct evaluation only) */
 } hk_stats;
 
 /* Phases of one hk_compute, timed with CUDA events on the caller's stream. */
-enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_FAR = 3, HK_PH_MID = 4, HK_PH_NEAR = 5, HK_PH_COUNT = 6 };
+enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, HK_PH_FAR = 4, HK_PH_MID = 5, HK_PH_NEAR = 6,
+       HK_PH_DOWN = 7, HK_PH_COUNT = 8 };
 
 /* Region thresholds on |z|^2 = x^2 + y^2 used by the fp32 evaluator. */
 #define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */
 #define HK_Z2 625.0f   /* |z| >= 25 : two asymptotic terms, relative error <= 1.0e-5 */
+#define HK_NODES 8     /* Chebyshev nodes per tile of the separated-tile evaluation */
 
 /* Grid: bin i is the POINT nu_i = numin + i*dnu (R8, R9).  HK_EINVAL if dnu <= 0,
  * numax <= numin, a non-finite argument, N < 1 or N too large. */
@@ -100,8 +105,8 @@ size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines);
 int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
 
 /* Enqueue the whole hot path on `stream` (a cudaStream_t passed as void*; NULL is
- * the legacy default stream): preprocess -> bucket/sort -> tile ranges -> far and
- * near accumulation kernels -> k in out_k_dev.  out_k_dev (N doubles) is
+ * the legacy default stream): preprocess -> bucket/sort -> tile ranges -> node, far, mid and
+ * near accumulation kernels -> interpolation of the node sums -> k in out_k_dev.  out_k_dev (N doubles) is
  * OVERWRITTEN.  cut_cm > 0 and finite: fixed cutting length from the centre,
  * inclusive integer extent (R7); cut_cm <= 0 or +inf: uncut.  Lines need not be
  * sorted.  n_lines == 0 is valid (k = 0).  Returns after enqueueing, without
@@ -159,12 +164,17 @@ int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, 
 int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev,
                       int32_t* region_out_dev, void* stream);
 
-/* Knobs for tests and sweeps.  mode 1: every (tile, line) pair goes through the near/edge
- * kernel; mode 2: far pairs go through the mid (two-term) kernel; mode 0: the default split.
+/* Knobs for tests and sweeps.  mode 0: the default split (separated tiles at Chebyshev nodes, the rest
+ * directly); mode 3: direct evaluation of every (line, bin) pair with the far / mid / near split;
+ * mode 1: every pair through the near/edge kernel; mode 2: far pairs through the mid (two-term) kernel
+ * (modes 1-3 do not use the node hierarchy).
+ * hk_set_node_separation: a (line, tile) pair is evaluated at nodes when the line centre is at least
+ * `sep` tile half-widths from the tile centre (default 4; < 1.5 disables the hierarchy).
  * hk_set_tile_bins: bins per lane 2, 4 or 8 (a warp owns 32x, a CTA 256x); 0 = chosen from
  * the cut (include/hk.h hk_stats.bins_per_lane reports the choice). */
 int hk_set_debug_mode(hk_ctx* ctx, int mode);
 int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane);
+int hk_set_node_separation(hk_ctx* ctx, double sep);
 
 int hk_last_cuda_error(const hk_ctx* ctx);
 const char* hk_strerror(int status);

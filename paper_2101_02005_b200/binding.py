@@ -26,8 +26,9 @@ FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
-           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_last_cuda_error", "hk_strerror")
-PHASES = ("preprocess", "sort", "ranges", "far", "mid", "near")
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation",
+           "hk_last_cuda_error", "hk_strerror")
+PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "near", "down")
 
 
 class hk_lines(C.Structure):
@@ -37,8 +38,9 @@ class hk_lines(C.Structure):
 class hk_stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n_lines", "n_skipped", "n_off_grid", "n_evals", "n_evals_far",
                                          "n_evals_mid", "n_evals_core", "n_units_far", "n_units_mid", "n_units_near",
-                                         "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_launches")] + \
-               [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("reserved", C.c_int32)]
+                                         "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_pairs_node",
+                                         "n_bins_node", "n_launches")] + \
+               [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("n_levels", C.c_int32)]
 
 
 _vp, _d, _i64 = C.c_void_p, C.c_double, C.c_int64
@@ -63,6 +65,8 @@ _lib.hk_get_stats.argtypes = [_vp, C.POINTER(hk_stats)]
 _lib.hk_eval_voigt_f32.argtypes = [_vp, _vp, _i64, _vp, _vp, _vp]
 _lib.hk_set_debug_mode.argtypes = [_vp, C.c_int]
 _lib.hk_set_tile_bins.argtypes = [_vp, C.c_int]
+_lib.hk_set_node_separation.argtypes = [_vp, _d]
+_lib.hk_set_node_separation.restype = C.c_int
 _lib.hk_last_cuda_error.argtypes = [_vp]
 _lib.hk_strerror.argtypes = [C.c_int]
 _lib.hk_strerror.restype = C.c_char_p
@@ -134,6 +138,9 @@ class Opacity:
 
     def set_tile_bins(self, bins_per_lane: int):
         self._check(_lib.hk_set_tile_bins(self._ctx, bins_per_lane), "hk_set_tile_bins")
+
+    def set_node_separation(self, sep: float):
+        self._check(_lib.hk_set_node_separation(self._ctx, sep), "hk_set_node_separation")
 
     def workspace_bytes(self, n_lines: int) -> int:
         return int(_lib.hk_workspace_bytes(self._ctx, n_lines))

@@ -6,8 +6,11 @@
 // at the end of a work unit and reach k(nu) with one fp64 atomic per bin per unit.
 // Lines arrive sorted by centre bin, so the lines that can reach a tile are one contiguous index
 // range, split by range_kernel into
-//   [A0,FL0) left-edge | [FL0,FL1) far | [FL1,ML1) mid | [ML1,MR0) centre | [MR0,FR0) mid | [FR0,FR1) far | [FR1,A1) right-edge
-// A work unit is (tile, chunk of that range); units are handed out by an atomic counter to a
+//   [A0,FL0) left-edge | [FL0,NL) node-handled | [NL,FL1) far | [FL1,ML1) mid | [ML1,MR0) centre |
+//   [MR0,FR0) mid | [FR0,NR) far | [NR,FR1) node-handled | [FR1,A1) right-edge
+// Node-handled pairs (tile separated from the line) are evaluated at Chebyshev nodes
+// by node_kernel on a binary hierarchy of tiles and interpolated onto the bins at the end.
+// A work unit is (tile, chunk of a kernel's own classes); units are handed out by an atomic counter to a
 // persistent grid (a multiple of the SM count).  fp32 partial sums are flushed into fp64 registers
 // every kFlush lines.
 //
@@ -31,15 +34,24 @@ namespace hk {
 struct AccArgs {
     const float4* __restrict__ recA;
     const float4* __restrict__ recB;
+    const float4* __restrict__ recN;
     const TileRange* __restrict__ tr;
-    const int32_t* __restrict__ unit_prefix;   // n_ct + 1 entries (exclusive scan of counts)
+    const NodeRange* __restrict__ nr;
+    // exclusive scans of the work-unit counts (one concatenated scan; each kernel reads its own slice, whose first
+    // element is the slice's base): n_ct + 1 entries for the direct kernels, n_entries + 1 for the node kernel
+    const int32_t* __restrict__ prefix_far;
+    const int32_t* __restrict__ prefix_mid;
+    const int32_t* __restrict__ prefix_near;
+    const int32_t* __restrict__ prefix_node;
     DevStats* st;
     double* __restrict__ out_k;
+    double* __restrict__ node_acc;             // n_entries x kP node sums (scaled), fp64
     int64_t N;
-    int32_t n_ct, chunk;
+    int32_t n_ct, chunk, chunk_node;
+    Levels lv;
 };
 
-// Which tile does unit u belong to?  Largest ct with prefix[ct] <= u.
+// Which tile does unit u belong to?  Largest ct with prefix[ct] <= u (u already includes the slice base prefix[0]).
 __device__ __forceinline__ int find_tile(const int32_t* __restrict__ prefix, int n_ct, int u)
 {
     int lo = 0, hi = n_ct;   // invariant: prefix[lo] <= u < prefix[hi]
@@ -105,7 +117,8 @@ __global__ void __launch_bounds__(kThreads, 2) interior_kernel(AccArgs a)
     __shared__ int s_unit;
     double* red = reinterpret_cast<double*>(&sm[0][0]);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int total = a.unit_prefix[a.n_ct];
+    const int32_t* __restrict__ prefix = kMid ? a.prefix_mid : a.prefix_far;
+    const int base = prefix[0], total = prefix[a.n_ct];
     unsigned int* counter = kMid ? &a.st->unit_counter_mid : &a.st->unit_counter_far;
 
     float2 tb[M];
@@ -116,18 +129,20 @@ __global__ void __launch_bounds__(kThreads, 2) interior_kernel(AccArgs a)
     }
 
     for (;;) {
-        const int u = next_unit(counter, &s_unit);
+        const int u = next_unit(counter, &s_unit) + base;
         if (u >= total) break;
-        const int ct = find_tile(a.unit_prefix, a.n_ct, u);
+        const int ct = find_tile(prefix, a.n_ct, u);
         const int64_t ct0 = (int64_t)ct * kTB;
         const TileRange r = a.tr[ct];
-        const int c0 = r.A0 + (u - a.unit_prefix[ct]) * a.chunk;
-        const int c1 = min(c0 + a.chunk, r.A1);
-        // left and right segments of this class, clipped to the chunk, walked as one list of nt lines
-        const int l0 = max(kMid ? r.FL1 : r.FL0, c0), l1 = min(kMid ? r.ML1 : r.FL1, c1);
-        const int r0 = max(kMid ? r.MR0 : r.FR0, c0), r1 = min(kMid ? r.FR0 : r.FR1, c1);
-        const int nl = max(l1 - l0, 0), nt = nl + max(r1 - r0, 0);
-        if (nt == 0) continue;
+        // left and right segments of this class walked as one list; this unit takes lines [v_lo, v_hi) of it
+        const int sl0 = kMid ? r.FL1 : r.NL, sl1 = kMid ? r.ML1 : r.FL1;
+        const int sr0 = kMid ? r.MR0 : r.FR0, sr1 = kMid ? r.FR0 : r.NR;
+        const int v_lo = (u - prefix[ct]) * a.chunk;
+        const int v_hi = min(v_lo + a.chunk, (sl1 - sl0) + (sr1 - sr0));
+        const int l0 = min(sl0 + v_lo, sl1), l1 = min(sl0 + v_hi, sl1);
+        const int r0 = sr0 + max(v_lo - (sl1 - sl0), 0), r1 = sr0 + max(v_hi - (sl1 - sl0), 0);
+        const int nl = l1 - l0, nt = nl + (r1 - r0);
+        if (nt <= 0) continue;
         if (threadIdx.x == 0) atomicAdd(kMid ? &a.st->units_mid : &a.st->units_far, 1ULL);
 
         float2 acc[M];
@@ -313,7 +328,8 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
     float4* smC = smem[2];
     double* red = reinterpret_cast<double*>(&smem[0][0]);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int total = a.unit_prefix[a.n_ct];
+    const int32_t* __restrict__ prefix = a.prefix_near;
+    const int base = prefix[0], total = prefix[a.n_ct];
     const float whi = (float)(kTB - 1);
 
     float2 tb[M];
@@ -326,18 +342,21 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
     for (int j = 0; j < KB; ++j) sacc[warp][lane + 32 * j] = 0.f;
 
     for (;;) {
-        const int u = next_unit(&a.st->unit_counter_near, &s_unit);
+        const int u = next_unit(&a.st->unit_counter_near, &s_unit) + base;
         if (u >= total) break;
-        const int ct = find_tile(a.unit_prefix, a.n_ct, u);
+        const int ct = find_tile(prefix, a.n_ct, u);
         const int64_t ct0 = (int64_t)ct * kTB;
         const TileRange r = a.tr[ct];
-        const int c0 = r.A0 + (u - a.unit_prefix[ct]) * a.chunk;
-        const int c1 = min(c0 + a.chunk, r.A1);
-        // left-edge, centre and right-edge segments clipped to the chunk, walked as one list of nt lines
-        const int g0 = max(r.A0, c0), g1 = max(r.ML1, c0), g2 = max(r.FR1, c0);
-        const int n0 = max(min(r.FL0, c1) - g0, 0), n1 = max(min(r.MR0, c1) - g1, 0), n2 = max(min(r.A1, c1) - g2, 0);
+        // left-edge, centre and right-edge segments walked as one list; this unit takes lines [v_lo, v_hi) of it
+        const int s0 = r.FL0 - r.A0, s1 = r.MR0 - r.ML1, s2 = r.A1 - r.FR1;
+        const int v_lo = (u - prefix[ct]) * a.chunk;
+        const int v_hi = min(v_lo + a.chunk, s0 + s1 + s2);
+        auto clip = [](int v, int n) { return max(0, min(v, n)); };
+        const int g0 = r.A0 + clip(v_lo, s0), n0 = clip(v_hi, s0) - clip(v_lo, s0);
+        const int g1 = r.ML1 + clip(v_lo - s0, s1), n1 = clip(v_hi - s0, s1) - clip(v_lo - s0, s1);
+        const int g2 = r.FR1 + clip(v_lo - s0 - s1, s2), n2 = clip(v_hi - s0 - s1, s2) - clip(v_lo - s0 - s1, s2);
         const int nt = n0 + n1 + n2;
-        if (nt == 0) continue;
+        if (nt <= 0) continue;
         if (threadIdx.x == 0) atomicAdd(&a.st->units_near, 1ULL);
 
         float2 acc[M];
@@ -482,6 +501,126 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
         __syncthreads();               // every warp is done with the staging buffers: red may overwrite them
         flush_tile<KB>(red, acc64, ct0, a);
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// node kernel: separated (line, tile) pairs evaluated at the tile's kP Chebyshev nodes
+// ---------------------------------------------------------------------------------------
+// Lanes walk LINES (one line per lane, coalesced 16 B records), every lane holds the tile's kP node
+// positions and kP partial sums in registers; two nodes share one reciprocal.  The partial sums are
+// combined with warp shuffles, then across warps, and reach the (level, tile) node sums with one
+// fp64 atomic per node per work unit.  Formula: two asymptotic terms (valid: |z|^2 >= Z2 on the tile).
+__global__ void __launch_bounds__(kThreads, 2) node_kernel(AccArgs a)
+{
+    constexpr int M = kP / 2;
+    __shared__ float red[kWarps][kP];
+    __shared__ int s_unit;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int32_t* __restrict__ prefix = a.prefix_node;
+    const int n_e = a.lv.n_entries;
+    const int base = prefix[0], total = prefix[n_e];
+    for (;;) {
+        const int u = next_unit(&a.st->unit_counter_node, &s_unit) + base;
+        if (u >= total) break;
+        const int e = find_tile(prefix, n_e, u);
+        int l = 0;
+        while (l + 1 < a.lv.n_levels && e >= a.lv.off[l + 1]) ++l;
+        const int64_t W = (int64_t)a.lv.w0 << l;
+        const int64_t tile0 = (int64_t)(e - a.lv.off[l]) * W;
+        const NodeRange r = a.nr[e];
+        const int s0 = r.a1 - r.a0, s1 = r.b1 - r.b0, s2 = r.c1 - r.c0, s3 = r.d1 - r.d0;
+        const int v_lo = (u - prefix[e]) * a.chunk_node;
+        const int v_hi = min(v_lo + a.chunk_node, s0 + s1 + s2 + s3);
+        if (v_hi <= v_lo) continue;
+        if (threadIdx.x == 0) atomicAdd(&a.st->units_node, 1ULL);
+        float2 xk[M], acc[M];
+        const double hc = 0.5 * (double)(W - 1), hw = 0.5 * (double)W;
+#pragma unroll
+        for (int m = 0; m < M; ++m) {
+            xk[m] = make_float2((float)(hc + hw * kChebX[2 * m]), (float)(hc + hw * kChebX[2 * m + 1]));
+            acc[m] = make_float2(0.f, 0.f);
+        }
+        for (int v = v_lo + (int)threadIdx.x; v < v_hi; v += kThreads) {
+            const int li = v < s0 ? r.a0 + v
+                         : v < s0 + s1 ? r.b0 + (v - s0)
+                         : v < s0 + s1 + s2 ? r.c0 + (v - s0 - s1) : r.d0 + (v - s0 - s1 - s2);
+            const float4 rec = a.recN[li];
+            const uint32_t pk = (uint32_t)__float_as_int(rec.y);
+            const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
+            const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
+            const float npos = -((float)((int64_t)__float_as_int(rec.x) - tile0) + f);
+            const float2 np2 = bcast2(npos), g2 = bcast2(rec.z), c2 = bcast2(rec.w), one = bcast2(1.0f);
+            const float2 A1 = bcast2(1.5f * a2), nA2 = bcast2(-2.0f * a2 * rec.z);
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const float2 t = __fadd2_rn(xk[m], np2);
+                const float2 q = __ffma2_rn(t, t, g2);
+                const float R = rcp_approx(q.x * q.y);             // 1/q.x = R q.y, 1/q.y = R q.x
+                const float2 rr = make_float2(R * q.y, R * q.x);
+                const float2 uu = __ffma2_rn(nA2, rr, A1);
+                const float2 vv = __ffma2_rn(uu, rr, one);
+                const float2 ww = __fmul2_rn(rr, vv);
+                acc[m] = __ffma2_rn(c2, ww, acc[m]);
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < M; ++m) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                acc[m].x += __shfl_xor_sync(0xffffffffu, acc[m].x, o);
+                acc[m].y += __shfl_xor_sync(0xffffffffu, acc[m].y, o);
+            }
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int m = 0; m < M; ++m) { red[warp][2 * m] = acc[m].x; red[warp][2 * m + 1] = acc[m].y; }
+        }
+        __syncthreads();
+        if (threadIdx.x < kP) {
+            double sum = 0.0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) sum += (double)red[w][threadIdx.x];
+            if (sum != 0.0) atomicAdd(a.node_acc + (size_t)e * kP + threadIdx.x, sum);
+        }
+    }
+}
+
+// value at xi (tile-normalised coordinate in [-1, 1]) of the degree-(kP-1) interpolant through the node sums
+__device__ __forceinline__ double cheb_interp(const double* __restrict__ nodes, double xi)
+{
+    double num = 0.0, den = 0.0;
+#pragma unroll
+    for (int k = 0; k < kP; ++k) {
+        const double d = xi - kChebX[k];
+        if (d == 0.0) return nodes[k];
+        const double w = kChebW[k] / d;
+        num = fma(w, nodes[k], num);
+        den += w;
+    }
+    return num / den;
+}
+
+// level l -> l - 1: restriction of the parent's polynomial to each child's nodes (exact for polynomials)
+__global__ void __launch_bounds__(256) node_down_kernel(AccArgs a, int l)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n_child = a.lv.off[l] - a.lv.off[l - 1];
+    if (idx >= n_child * kP) return;
+    const int jc = idx / kP, kk = idx - jc * kP;
+    const double xi = ((jc & 1) ? 0.5 : -0.5) + 0.5 * kChebX[kk];
+    const double v = cheb_interp(a.node_acc + (size_t)(a.lv.off[l] + (jc >> 1)) * kP, xi);
+    if (v != 0.0) a.node_acc[(size_t)(a.lv.off[l - 1] + jc) * kP + kk] += v;
+}
+
+// level-0 node sums -> bins of k(nu)
+__global__ void __launch_bounds__(256) node_bins_kernel(AccArgs a)
+{
+    const int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (b >= a.N) return;
+    const int64_t j = b / a.lv.w0;
+    const double xi = ((double)(b - j * a.lv.w0) - 0.5 * (double)(a.lv.w0 - 1)) / (0.5 * (double)a.lv.w0);
+    const double v = cheb_interp(a.node_acc + (size_t)j * kP, xi);
+    if (v != 0.0) a.out_k[b] += v * scalbn(1.0, -a.st->scale_exp);
 }
 
 // ---------------------------------------------------------------------------------------

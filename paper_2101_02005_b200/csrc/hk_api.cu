@@ -25,13 +25,14 @@ struct hk_ctx {
     int cuda_err;
     int debug_mode;
     int force_kb;
+    double node_sep;
     int n_sm;
     // last compute
     bool have_run;
     int64_t last_n;
     double last_cut;
     cudaStream_t last_stream;
-    int32_t last_sort_bits, last_kb;
+    int32_t last_sort_bits, last_kb, last_levels;
     int64_t last_launches;
     DevStats* d_stats;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
@@ -48,9 +49,11 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, tr, counts, prefix, cub;
+    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, recN, tr, nr, node_acc, counts, prefix, cub;
     size_t cub_bytes, total;
-    int32_t n_ct;
+    int32_t n_ct;        // level-0 tiles of the smallest geometry
+    int32_t n_entries;   // upper bound on (level, tile) entries of the node hierarchy
+    int32_t n_counts;    // work-unit counts: 3 n_ct (far, mid, near) + n_entries (node) + 1
 };
 
 bool is_uncut(double cut) { return !(cut > 0.0 && std::isfinite(cut)); }
@@ -60,7 +63,7 @@ size_t cub_temp_bytes(int64_t n, int32_t n_ct)
     size_t b1 = 0, b2 = 0;
     cub::DeviceRadixSort::SortPairs(nullptr, b1, (const int32_t*)nullptr, (int32_t*)nullptr, (const int32_t*)nullptr,
                                     (int32_t*)nullptr, (int)n, 0, 32, (cudaStream_t)0);
-    cub::DeviceScan::ExclusiveSum(nullptr, b2, (const int32_t*)nullptr, (int32_t*)nullptr, (int)(n_ct + 1),
+    cub::DeviceScan::ExclusiveSum(nullptr, b2, (const int32_t*)nullptr, (int32_t*)nullptr, (int)n_ct,
                                   (cudaStream_t)0);
     return b1 > b2 ? b1 : b2;
 }
@@ -83,6 +86,8 @@ Layout make_layout(const hk_ctx* c, int64_t n)
 {
     Layout L;
     L.n_ct = (int32_t)((c->N + 32 * kMinKB - 1) / (32 * kMinKB));
+    L.n_entries = 2 * L.n_ct + kMaxLevels;
+    L.n_counts = 3 * L.n_ct + L.n_entries + 1;
     size_t nn = (size_t)(n > 0 ? n : 1);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -94,10 +99,13 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     L.recU = take(nn * sizeof(RecU));
     L.recA = take(nn * 16);
     L.recB = take(nn * 16);
+    L.recN = take(nn * 16);
     L.tr = take((size_t)L.n_ct * sizeof(TileRange));
-    L.counts = take(((size_t)L.n_ct + 1) * 4);
-    L.prefix = take(((size_t)L.n_ct + 1) * 4);
-    L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_ct);
+    L.nr = take((size_t)L.n_entries * sizeof(NodeRange));
+    L.node_acc = take((size_t)L.n_entries * kP * sizeof(double));
+    L.counts = take((size_t)L.n_counts * 4);
+    L.prefix = take((size_t)L.n_counts * 4);
+    L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_counts);
     L.cub = take(L.cub_bytes);
     L.total = off;
     return L;
@@ -149,8 +157,34 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
     p.kb = pick_kb(c, cut);
     p.n_ct = (int32_t)((c->N + 32 * p.kb - 1) / (32 * p.kb));
     p.chunk = chunk;
+    p.chunk_node = 16384;
+    p.sep = c->node_sep;
     p.mode = c->debug_mode;
     return p;
+}
+
+// Node hierarchy of this launch: level l has tiles of 32 kb 2^l bins; a level is kept while some line can be both
+// separated from one of its tiles (centre >= sep half-widths away) and cover it (centre + cut beyond its far edge).
+Levels make_levels(const hk_ctx* c, const Params& p)
+{
+    Levels lv;
+    std::memset(&lv, 0, sizeof(lv));
+    lv.w0 = 32 * p.kb;
+    if (p.mode != 0 || !(p.sep >= 1.5)) return lv;
+    const double reach = p.uncut ? (double)c->N * 2.0 : (double)p.cb_floor;
+    int32_t off = 0;
+    for (int l = 0; l < kMaxLevels; ++l) {
+        const double W = (double)lv.w0 * (double)(1LL << l);
+        if (0.5 * W * (p.sep + 1.0) > reach) break;
+        const int64_t nt = (c->N + (int64_t)W - 1) / (int64_t)W;
+        lv.off[l] = off;
+        off += (int32_t)nt;
+        lv.n_levels = l + 1;
+        if (nt <= 1) break;
+    }
+    lv.off[lv.n_levels] = off;
+    lv.n_entries = off;
+    return lv;
 }
 
 int32_t pick_chunk(const hk_ctx* c, int64_t n, double cut)
@@ -219,6 +253,7 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     if (!c) return HK_ENOMEM;
     std::memset(c, 0, sizeof(*c));
     c->numin = numin; c->numax = numax; c->dnu = dnu; c->N = (int64_t)Nd;
+    c->node_sep = 4.0;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -277,8 +312,15 @@ int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes)
 
 int hk_set_debug_mode(hk_ctx* ctx, int mode)
 {
-    if (!ctx || mode < 0 || mode > 2) return HK_EINVAL;
+    if (!ctx || mode < 0 || mode > 3) return HK_EINVAL;
     ctx->debug_mode = mode;
+    return HK_OK;
+}
+
+int hk_set_node_separation(hk_ctx* ctx, double sep)
+{
+    if (!ctx || !std::isfinite(sep) || sep < 0.0 || sep > 64.0) return HK_EINVAL;
+    ctx->node_sep = sep;
     return HK_OK;
 }
 
@@ -327,9 +369,14 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     RecU* recU = (RecU*)(ws + L.recU);
     float4* recA = (float4*)(ws + L.recA);
     float4* recB = (float4*)(ws + L.recB);
+    float4* recN = (float4*)(ws + L.recN);
     TileRange* tr = (TileRange*)(ws + L.tr);
+    NodeRange* nr = (NodeRange*)(ws + L.nr);
+    double* node_acc = (double*)(ws + L.node_acc);
     int32_t* counts = (int32_t*)(ws + L.counts);
     int32_t* prefix = (int32_t*)(ws + L.prefix);
+    const Levels lv = make_levels(ctx, p);
+    ctx->last_levels = lv.n_levels;
 
     // a1: per-line parameters, keys
     line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
@@ -342,24 +389,38 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     size_t cub_bytes = L.cub_bytes;
     HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                             (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
-    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB);
+    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB, recN);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
-    // a3: tile ranges and work units
-    range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, keys_out, n, tr, st);
-    HK_CUDA(cudaMemsetAsync(counts, 0, ((size_t)p.n_ct + 1) * 4, stream));
-    unit_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, tr, counts);
+    // a3: tile ranges, node ranges and work units.  counts = [far | mid | near | node | 0], one scan.
+    const int n_counts = 3 * p.n_ct + lv.n_entries + 1;
+    int32_t* cnt_far = counts;
+    int32_t* cnt_mid = counts + p.n_ct;
+    int32_t* cnt_near = counts + 2 * p.n_ct;
+    int32_t* cnt_node = counts + 3 * p.n_ct;
+    HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
+    range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_near, st);
+    ctx->last_launches = 5;
+    if (lv.n_entries > 0) {
+        HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
+        node_range_kernel<<<(lv.n_entries + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, nr, cnt_node, st);
+        ++ctx->last_launches;
+    }
     cub_bytes = L.cub_bytes;
-    HK_CUDA(cub::DeviceScan::ExclusiveSum(ws + L.cub, cub_bytes, (const int32_t*)counts, prefix, p.n_ct + 1, stream));
+    HK_CUDA(cub::DeviceScan::ExclusiveSum(ws + L.cub, cub_bytes, (const int32_t*)counts, prefix, n_counts, stream));
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_RANGES + 1], stream));
     // a4-a7: accumulate
     AccArgs a;
-    a.recA = recA; a.recB = recB; a.tr = tr; a.unit_prefix = prefix; a.st = st; a.out_k = out_k_dev;
-    a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk;
-    ctx->last_launches = 6;
+    a.recA = recA; a.recB = recB; a.recN = recN; a.tr = tr; a.nr = nr;
+    a.prefix_far = prefix; a.prefix_mid = prefix + p.n_ct; a.prefix_near = prefix + 2 * p.n_ct;
+    a.prefix_node = prefix + 3 * p.n_ct;
+    a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc;
+    a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.lv = lv;
     const int grid = ctx->n_sm * 2;
+    if (lv.n_entries > 0) { node_kernel<<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NODE + 1], stream));
     auto launch = [&](auto kb_tag) {
         constexpr int KB = decltype(kb_tag)::value;
-        if (p.mode == 0) { interior_kernel<KB, false><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        if (p.mode != 1 && p.mode != 2) { interior_kernel<KB, false><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream);
         if (p.mode != 1) { interior_kernel<KB, true><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
@@ -370,6 +431,17 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     if (p.kb == 8) launch(std::integral_constant<int, 8>());
     else if (p.kb == 4) launch(std::integral_constant<int, 4>());
     else launch(std::integral_constant<int, 2>());
+    // downward pass: parents' polynomials onto the children's nodes, level-0 nodes onto the bins
+    if (lv.n_entries > 0) {
+        for (int l = lv.n_levels - 1; l >= 1; --l) {
+            const int nth = (lv.off[l] - lv.off[l - 1]) * kP;
+            node_down_kernel<<<(nth + 255) / 256, 256, 0, stream>>>(a, l);
+            ++ctx->last_launches;
+        }
+        node_bins_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
+        ++ctx->last_launches;
+    }
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_DOWN + 1], stream));
     HK_CUDA(cudaGetLastError());
     return HK_OK;
 }
@@ -551,6 +623,10 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_pairs_far = (int64_t)d.pairs_far;
     host_out->n_pairs_near = (int64_t)d.pairs_near;
     host_out->n_launches = ctx->last_launches;
+    host_out->n_units_node = (int64_t)d.units_node;
+    host_out->n_pairs_node = (int64_t)d.pairs_node;
+    host_out->n_bins_node = (int64_t)d.bins_node;
+    host_out->n_levels = ctx->last_levels;
     host_out->scale_exp = d.scale_exp;
     host_out->sort_bits = ctx->last_sort_bits;
     if (ctx->host_totals) {

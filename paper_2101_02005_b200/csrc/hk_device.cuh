@@ -43,9 +43,37 @@ struct __align__(16) RecU {
 //   A = { jc (int bits), f, G2, c }        c  = scale * S * Gamma_L/(pi dnu^2)   (Lorentz amplitude, bin units)
 //   B = { a2, ilo (int bits), ihi (int bits), cK }   cK = scale * S/(alpha_D sqrt(pi))
 
-// per warp tile: the candidate range [A0,A1) of sorted line indices and its split (hk_accumulate.cuh)
-struct __align__(16) TileRange {
-    int32_t A0, FL0, FL1, ML1, MR0, FR0, FR1, A1;
+//   N = { jc (int bits), (f13 << 19) | a2_19, G2, c }   compact record of the node kernel: f13 = sub-bin offset in
+//       1/8192 bins, a2_19 = top 19 bits below the sign of the fp32 pattern of a2 (8 exponent + 11 mantissa bits)
+
+// per level-0 tile: the candidate range [A0,A1) of sorted line indices and its split (hk_accumulate.cuh):
+//   [A0,FL0) left edge | [FL0,NL) node-handled | [NL,FL1) far | [FL1,ML1) mid | [ML1,MR0) centre |
+//   [MR0,FR0) mid | [FR0,NR) far | [NR,FR1) node-handled | [FR1,A1) right edge
+struct __align__(8) TileRange {
+    int32_t A0, FL0, NL, FL1, ML1, MR0, FR0, NR, FR1, A1;
+};
+
+// per (level, tile) entry of the node hierarchy: four index ranges of sorted lines evaluated at the tile's nodes
+struct __align__(16) NodeRange {
+    int32_t a0, a1, b0, b1, c0, c1, d0, d1;
+};
+
+// ---- Chebyshev nodes of the separated-tile evaluation ----------------
+constexpr int kP = 8;                    // nodes per tile: degree-7 interpolant
+constexpr int kMaxLevels = 24;
+// xi_k = cos((2k+1) pi/16); barycentric weights (-1)^k sin((2k+1) pi/16)
+__device__ constexpr double kChebX[kP] = {0.98078528040323044913,  0.83146961230254523708,  0.55557023301960222474,
+                                          0.19509032201612826785,  -0.19509032201612826785, -0.55557023301960222474,
+                                          -0.83146961230254523708, -0.98078528040323044913};
+__device__ constexpr double kChebW[kP] = {0.19509032201612826785,  -0.55557023301960222474, 0.83146961230254523708,
+                                          -0.98078528040323044913, 0.98078528040323044913,  -0.83146961230254523708,
+                                          0.55557023301960222474,  -0.19509032201612826785};
+
+struct Levels {
+    int32_t n_levels;                    // node levels 0..n_levels-1, tile width W0 << l
+    int32_t w0;                          // level-0 tile width (32 kb)
+    int32_t n_entries;                   // sum over levels of tiles
+    int32_t off[kMaxLevels + 1];         // first entry of each level
 };
 
 // ---- small helpers

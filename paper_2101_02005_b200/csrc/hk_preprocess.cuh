@@ -1,8 +1,8 @@
 // hk_preprocess.cuh -- steps a1-a3 of the hot path:
 //   line_kernel   : per-line S, Gamma_L, alpha_D, centre bin, extent, sort key   (Eq. 5, 9, 13; L236-239)
 //   gather_kernel : permute records into centre-bin order, apply the launch scale
-//   range_kernel  : per warp tile, the candidate line range and its far-interior parts (L347)
-//   unit_kernel   : per CTA tile, number of (tile, line-chunk) work units
+//   range_kernel  : per level-0 tile, the candidate line range and its split into classes (L347), work-unit counts
+//   node_range_kernel : per (level, tile) of the node hierarchy, the line ranges evaluated at its nodes
 #pragma once
 #include "hk_device.cuh"
 
@@ -31,8 +31,11 @@ struct Params {
     double numin_bins;          // numin / dnu
     int32_t kb;                 // bins per lane (2, 4, 8)
     int32_t n_ct;               // tiles of 32 kb bins
-    int32_t chunk;              // lines per work unit
-    int mode;                   // debug: 0 default, 1 everything through the near kernel, 2 far pairs through the mid kernel
+    int32_t chunk;              // lines per work unit of the direct kernels
+    int32_t chunk_node;         // lines per work unit of the node kernel
+    double sep;                 // node separation: |centre - tile centre| >= sep * half-width
+    int mode;                   // debug: 0 default, 1 everything through the near kernel, 2 far pairs through the mid kernel,
+                                //        3 direct evaluation only (no node hierarchy)
 };
 
 struct DevStats {
@@ -40,9 +43,11 @@ struct DevStats {
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
     int32_t pad;
-    unsigned int unit_counter_far, unit_counter_mid, unit_counter_near, pad2;
-    unsigned long long units_far, units_mid, units_near;
+    unsigned int unit_counter_far, unit_counter_mid, unit_counter_near, unit_counter_node;
+    unsigned long long units_far, units_mid, units_near, units_node;
     unsigned long long pairs_far, pairs_mid, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
+    unsigned long long pairs_node;                         // (line, tile) pairs evaluated at nodes
+    unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
 };
 
 __device__ __forceinline__ bool finite6(double a, double b, double c, double d, double e, double f)
@@ -187,7 +192,8 @@ __global__ void scale_kernel(DevStats* st)
 
 __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ idx_sorted,
                                                      int64_t n, const DevStats* __restrict__ st,
-                                                     float4* __restrict__ recA, float4* __restrict__ recB)
+                                                     float4* __restrict__ recA, float4* __restrict__ recB,
+                                                     float4* __restrict__ recN)
 {
     const int e = st->scale_exp;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
@@ -197,6 +203,9 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
         float c = cK * sqrtf(r.G2 * r.a2) * 0.564189583547756f;
         recA[i] = make_float4(__int_as_float(r.jc), r.f, r.G2, c);
         recB[i] = make_float4(r.a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
+        const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn(r.f * 8192.0f));
+        const uint32_t a19 = ((uint32_t)__float_as_int(r.a2) >> 12) & 0x7FFFFu;
+        recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), r.G2, c);
     }
 }
 
@@ -228,8 +237,100 @@ __device__ __forceinline__ int64_t right_bound(double w1m1, double kap, double n
     return (int64_t)ceil((w1m1 + kap * (numin_bins + 1.0)) / (1.0 - kap)) + 3;
 }
 
-__global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __restrict__ keys, int32_t n,
-                                                    TileRange* __restrict__ tr, DevStats* __restrict__ st)
+// Key thresholds of one tile [w0, w1) of width W (any level) for the node hierarchy.  A line with centre bin jc is
+// "handled at the nodes of this tile or of an ancestor" when loL <= jc <= upL (left of the tile) or dnR <= jc <= hiR
+// (right): the tile lies inside the line's extent, |z|^2 >= Z2 on all of it, and the centre is at least sep half-widths
+// from the tile centre.  The sets of a parent are nested in those of its children.
+struct NodeKeys {
+    int64_t loL, upL, dnR, hiR;
+};
+constexpr int64_t kBigKey = INT64_MAX / 4;
+
+__device__ __forceinline__ NodeKeys node_keys(const Params& p, int64_t w0, int64_t W)
+{
+    const int64_t w1 = min(p.N, w0 + W);
+    const double m = (double)w0 + 0.5 * (double)(W - 1), h = 0.5 * (double)W;
+    NodeKeys k;
+    k.loL = p.uncut ? -kBigKey : w1 - p.cb_floor;
+    k.hiR = p.uncut ? kBigKey : w0 + p.cb_floor - 2;
+    const int64_t sepL = (int64_t)floor(m - p.sep * h) - 1;
+    const int64_t sepR = (int64_t)ceil(m + p.sep * h);
+    k.upL = min(sepL, left_bound((double)w0, p.kappa2, p.numin_bins));
+    k.dnR = max(sepR, right_bound((double)(w1 - 1), p.kappa2, p.numin_bins));
+    // empty sets are written as [lo, lo - 1] / [hi + 1, hi]
+    k.upL = max(k.upL, k.loL - 1);
+    k.dnR = min(k.dnR, k.hiR + 1);
+    return k;
+}
+
+// index of the first sorted line with centre bin >= j (keys are jc - kmin)
+__device__ __forceinline__ int32_t idx_of(const Params& p, const int32_t* __restrict__ keys, int32_t n_act, int64_t j)
+{
+    if (j <= -kBigKey / 2) return 0;
+    if (j >= kBigKey / 2) return n_act;
+    return lower_bound_key(keys, n_act, j - p.kmin);
+}
+
+// One thread per (level, tile) entry: the four index ranges of lines evaluated at this tile's nodes
+// ( = handled here but not by the parent), and the number of work units they make.
+__global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, const int32_t* __restrict__ keys, int32_t n,
+                                                         const TileRange* __restrict__ tr, NodeRange* __restrict__ nr,
+                                                         int32_t* __restrict__ counts, DevStats* __restrict__ st)
+{
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= lv.n_entries) return;
+    int l = 0;
+    while (l + 1 < lv.n_levels && e >= lv.off[l + 1]) ++l;
+    const int64_t j = e - lv.off[l];
+    const int64_t W = (int64_t)lv.w0 << l;
+    const int64_t w0 = j * W;
+    const int32_t n_act = lower_bound_key(keys, n, (int64_t)p.ksent);
+    int32_t a, b, c, d;                          // handled here or above: [a, b) on the left, [c, d) on the right
+    if (l == 0) {                                // the same indices the direct kernels exclude
+        const TileRange t = tr[j];
+        a = t.FL0; b = t.NL; c = t.NR; d = t.FR1;
+    } else {
+        const NodeKeys k = node_keys(p, w0, W);
+        a = idx_of(p, keys, n_act, k.loL);
+        b = max(a, idx_of(p, keys, n_act, k.upL + 1));
+        c = idx_of(p, keys, n_act, k.dnR);
+        d = max(c, idx_of(p, keys, n_act, k.hiR + 1));
+    }
+    int32_t pa = n_act, pb = n_act, pc = 0, pd = 0;   // the parent's sets (none at the top level)
+    if (l + 1 < lv.n_levels) {
+        const int64_t Wp = 2 * W;
+        const NodeKeys k = node_keys(p, (j >> 1) * Wp, Wp);
+        pa = idx_of(p, keys, n_act, k.loL);
+        pb = max(pa, idx_of(p, keys, n_act, k.upL + 1));
+        pc = idx_of(p, keys, n_act, k.dnR);
+        pd = max(pc, idx_of(p, keys, n_act, k.hiR + 1));
+    } else {
+        pa = pb = b;                              // nothing removed: [a, min(b, pa)) = [a, b), [max(a, pb), b) empty
+        pc = pd = d;
+    }
+    NodeRange r;
+    r.a0 = a; r.a1 = max(a, min(b, pa));          // left sliver: inside this tile's reach but not the parent's
+    r.b0 = min(b, max(r.a1, pb)); r.b1 = b;       // left main: closer than the parent's separation
+    r.c0 = c; r.c1 = max(c, min(d, pc));          // right main
+    r.d0 = min(d, max(r.c1, pd)); r.d1 = d;       // right sliver
+    nr[e] = r;
+    const int64_t tot = (int64_t)(r.a1 - r.a0) + (r.b1 - r.b0) + (r.c1 - r.c0) + (r.d1 - r.d0);
+    counts[e] = (int32_t)((tot + p.chunk_node - 1) / p.chunk_node);
+    if (tot) {
+        atomicAdd(&st->pairs_node, (unsigned long long)tot);
+        atomicAdd(&st->bins_node, (unsigned long long)tot * (unsigned long long)(min(p.N, w0 + W) - w0));
+    }
+}
+
+// Per level-0 tile [w0, w1): candidate lines and their split into edge / node-handled / far / mid / centre ranges.
+// A line is "interior" for the tile when every bin of the tile lies inside its extent and at
+// |t| >= max(2 KB, sqrt(Z) a): then |z|^2 >= Z for every (line, bin) pair (Z = Z1: far, Z = Z2: mid)
+// and the interior kernels may run mask-free.  alpha_D = beta nu0 is a function of the centre, so the
+// condition is a bound on the centre bin alone; all bounds are conservative.
+__global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const int32_t* __restrict__ keys, int32_t n,
+                                                    TileRange* __restrict__ tr, int32_t* __restrict__ cnt_far,
+                                                    int32_t* __restrict__ cnt_mid, int32_t* __restrict__ cnt_near,
+                                                    DevStats* __restrict__ st)
 {
     int wt = blockIdx.x * blockDim.x + threadIdx.x;
     if (wt >= p.n_ct) return;
@@ -239,27 +340,27 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __r
     const int64_t w1 = min(p.N, w0 + wb);
     const int32_t n_act = lower_bound_key(keys, n, (int64_t)p.ksent);
     int64_t jlo, jhi;                       // candidate centre bins
-    if (p.uncut) { jlo = INT64_MIN / 2; jhi = INT64_MAX / 2; }
+    if (p.uncut) { jlo = -kBigKey; jhi = kBigKey; }
     else { jlo = w0 - p.cb_ceil - 2; jhi = w1 - 1 + p.cb_ceil + 2; }
     TileRange r;
-    r.A0 = p.uncut ? 0 : lower_bound_key(keys, n_act, jlo - p.kmin);
-    r.A1 = p.uncut ? n_act : lower_bound_key(keys, n_act, jhi + 1 - p.kmin);
+    r.A0 = idx_of(p, keys, n_act, jlo);
+    r.A1 = idx_of(p, keys, n_act, jhi + 1);
     // left of the tile: the extent must reach the tile's last bin (jc >= jLmin)
-    const int64_t jLmin = p.uncut ? INT64_MIN / 2 : w1 - p.cb_floor;
+    const int64_t jLmin = p.uncut ? -kBigKey : w1 - p.cb_floor;
     int64_t jLfar = min(left_bound((double)w0, p.kappa1, p.numin_bins), w0 - 1 - mind);
     int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.numin_bins), w0 - 1 - mind);
     // right of the tile: the extent must reach the tile's first bin (jc <= jRmax)
-    const int64_t jRmax = p.uncut ? INT64_MAX / 2 : w0 + p.cb_floor - 2;
+    const int64_t jRmax = p.uncut ? kBigKey : w0 + p.cb_floor - 2;
     int64_t jRfar = max(right_bound((double)(w1 - 1), p.kappa1, p.numin_bins), w1 - 1 + mind);
     int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.numin_bins), w1 - 1 + mind);
-    if (p.mode == 1) { jLfar = jLmid = INT64_MIN / 2; jRfar = jRmid = INT64_MAX / 2; }
-    if (p.mode == 2) { jLfar = INT64_MIN / 2; jRfar = INT64_MAX / 2; }
-    int32_t fl0 = lower_bound_key(keys, n_act, jLmin - p.kmin);
-    int32_t fl1 = lower_bound_key(keys, n_act, jLfar + 1 - p.kmin);
-    int32_t ml1 = lower_bound_key(keys, n_act, jLmid + 1 - p.kmin);
-    int32_t mr0 = lower_bound_key(keys, n_act, jRmid - p.kmin);
-    int32_t fr0 = lower_bound_key(keys, n_act, jRfar - p.kmin);
-    int32_t fr1 = lower_bound_key(keys, n_act, jRmax + 1 - p.kmin);
+    if (p.mode == 1) { jLfar = jLmid = -kBigKey; jRfar = jRmid = kBigKey; }
+    if (p.mode == 2) { jLfar = -kBigKey; jRfar = kBigKey; }
+    int32_t fl0 = idx_of(p, keys, n_act, jLmin);
+    int32_t fl1 = idx_of(p, keys, n_act, jLfar + 1);
+    int32_t ml1 = idx_of(p, keys, n_act, jLmid + 1);
+    int32_t mr0 = idx_of(p, keys, n_act, jRmid);
+    int32_t fr0 = idx_of(p, keys, n_act, jRfar);
+    int32_t fr1 = idx_of(p, keys, n_act, jRmax + 1);
     // make the sequence monotone inside [A0, A1]; every adjustment only shrinks an interior class
     fl0 = min(max(fl0, r.A0), r.A1);
     fl1 = min(max(fl1, fl0), r.A1);
@@ -267,24 +368,28 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, const int32_t* __r
     fr1 = max(min(fr1, r.A1), ml1);
     fr0 = max(min(fr0, fr1), ml1);
     mr0 = max(min(mr0, fr0), ml1);
-    r.FL0 = fl0; r.FL1 = fl1; r.ML1 = ml1; r.MR0 = mr0; r.FR0 = fr0; r.FR1 = fr1;
+    // node-handled lines (this tile's nodes or an ancestor's): a prefix of the left interior classes and a
+    // suffix of the right ones
+    int32_t nl = fl0, nrr = fr1;
+    if (lv.n_levels > 0) {
+        const NodeKeys k = node_keys(p, w0, wb);
+        nl = min(max(idx_of(p, keys, n_act, k.upL + 1), fl0), ml1);
+        nrr = max(min(idx_of(p, keys, n_act, k.dnR), fr1), mr0);
+    }
+    fl1 = max(fl1, nl);
+    fr0 = min(fr0, nrr);
+    r.FL0 = fl0; r.NL = nl; r.FL1 = fl1; r.ML1 = ml1; r.MR0 = mr0; r.FR0 = fr0; r.NR = nrr; r.FR1 = fr1;
     tr[wt] = r;
     const unsigned long long nb = (unsigned long long)(w1 - w0);
-    const unsigned long long nfar = (unsigned long long)(fl1 - fl0) + (unsigned long long)(fr1 - fr0);
-    const unsigned long long nmid = (unsigned long long)(ml1 - fl1) + (unsigned long long)(fr0 - mr0);
-    const unsigned long long nall = (unsigned long long)(r.A1 - r.A0);
-    if (nfar) atomicAdd(&st->pairs_far, nfar * nb);
-    if (nmid) atomicAdd(&st->pairs_mid, nmid * nb);
-    if (nall > nfar + nmid) atomicAdd(&st->pairs_near, (nall - nfar - nmid) * nb);
-}
-
-// Per CTA tile: number of line chunks over the union of its warp tiles' candidates.
-__global__ void __launch_bounds__(256) unit_kernel(Params p, const TileRange* __restrict__ tr, int32_t* __restrict__ counts)
-{
-    int ct = blockIdx.x * blockDim.x + threadIdx.x;
-    if (ct >= p.n_ct) return;
-    int64_t len = (int64_t)tr[ct].A1 - tr[ct].A0;
-    counts[ct] = len > 0 ? (int32_t)((len + p.chunk - 1) / p.chunk) : 0;
+    const long long nfar = (long long)(fl1 - nl) + (nrr - fr0);
+    const long long nmid = (long long)(ml1 - fl1) + (fr0 - mr0);
+    const long long nnear = (long long)(fl0 - r.A0) + (mr0 - ml1) + (r.A1 - fr1);
+    cnt_far[wt] = (int32_t)((nfar + p.chunk - 1) / p.chunk);
+    cnt_mid[wt] = (int32_t)((nmid + p.chunk - 1) / p.chunk);
+    cnt_near[wt] = (int32_t)((nnear + p.chunk - 1) / p.chunk);
+    if (nfar) atomicAdd(&st->pairs_far, (unsigned long long)nfar * nb);
+    if (nmid) atomicAdd(&st->pairs_mid, (unsigned long long)nmid * nb);
+    if (nnear) atomicAdd(&st->pairs_near, (unsigned long long)nnear * nb);
 }
 
 }  // namespace hk

@@ -98,18 +98,45 @@ def test_uncut_atom_like_sampled_bins(B):
     _check_extents(ext, lines, cond, grid, cut)
 
 
-def test_cross_path_near_vs_default(B):
-    """force every (tile, line) pair through the masked near kernel (mode 1), or the far
-    pairs through the mid kernel (mode 2), and compare with the default far/mid/near split on all bins."""
-    for cfg, n in [(2, 20_000), (4, 6_000)]:
+def test_cross_path_nodes_vs_direct(B):
+    """SURVEY 8(d) cross-path check on ALL bins: the default path (separated tiles at Chebyshev nodes, mode 0)
+    against direct evaluation of every pair (mode 3), against everything through the masked near kernel (mode 1)
+    and against far pairs through the mid kernel (mode 2)."""
+    for cfg, n, tb in [(2, 20_000, 0), (4, 6_000, 0), (4, 6_000, 2), (3, 100_000, 2), (5, 300, 0)]:
         lines, cond, grid, cut = _mini(cfg, n)
-        k0, st0, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=0)
-        assert st0["n_pairs_far"] > 0 and st0["n_pairs_mid"] > 0 and st0["n_pairs_near"] > 0
-        big = k0 >= 1e-8 * k0.max()
+        k0, st0, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=0, tile_bins=tb)
+        assert st0["n_levels"] >= 1 and st0["n_pairs_node"] > 0 and st0["n_pairs_near"] > 0
+        k3, st3, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=3, tile_bins=tb)
+        assert st3["n_levels"] == 0 and st3["n_pairs_node"] == 0 and st3["n_pairs_far"] > 0 and st3["n_pairs_mid"] > 0
+        # every (line, bin) pair of the definition is covered exactly once by one of the four paths
+        for st in (st0, st3):
+            cover = st["n_pairs_far"] + st["n_pairs_mid"] + st["n_bins_node"]
+            assert cover <= st["n_evals"] <= cover + st["n_pairs_near"]
+        big = k3 >= 1e-8 * k3.max()
+        assert np.abs(k0[big] / k3[big] - 1.0).max() <= 3e-5
+        if cfg == 5:
+            continue
         for mode in (1, 2):
-            k1, st1, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=mode)
-            assert st1["n_pairs_far"] == 0
-            assert np.abs(k1[big] / k0[big] - 1.0).max() <= 4e-5
+            k1, st1, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=mode, tile_bins=tb)
+            assert st1["n_pairs_far"] == 0 and st1["n_pairs_node"] == 0
+            assert np.abs(k1[big] / k3[big] - 1.0).max() <= 4e-5
+
+
+@pytest.mark.parametrize("sep", [2.5, 4.0, 6.0])
+def test_node_separation_sweep(B, sep):
+    """The node hierarchy at other separations (fewer / more pairs at nodes) against the oracle."""
+    lines, cond, grid, cut = _mini(2, 20_000)
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_node_separation(sep)
+    k = op.compute(_to_cuda(lines), cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    assert st["n_levels"] >= 1 and st["n_pairs_node"] > 0
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    assert st["n_evals"] == evals
+    check_parity(k.cpu().numpy(), k_ref, rel=(3e-4 if sep < 3 else 1e-4), what=f"node separation {sep}")
+    op.close()
 
 
 @pytest.mark.parametrize("tile_bins", [2, 4, 8])
