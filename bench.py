@@ -245,6 +245,8 @@ def run_ours(args):
     dl = W.make_lines(cfg, n=n, seed=0, device="cuda")      # replicas: every rank holds the whole workload
     op = B.Opacity(*grid)
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_tile_bins(args.tile_bins)
+    op.set_debug_mode(args.mode)
     k = torch.empty(op.N, dtype=torch.float64, device="cuda")
     input_bytes = 6 * 8 * n
     flush = None
@@ -333,7 +335,8 @@ def run_ours(args):
            "voigt_evals_per_s": world * st["n_evals"] * args.steps / (total_ms * 1e-3),
            "evals_per_step": st["n_evals"],
            "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"]},
-           "pairs_by_kernel": {"far": st["n_pairs_far"], "mid": st["n_pairs_mid"], "near": st["n_pairs_near"]},
+           "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
+                               "edge": st["n_pairs_edge"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
            "bins_per_lane": st["bins_per_lane"],
            "phase_ms": phases, "step_ms": step_ms, "roofline": roofline, "clocks": clocks,
            "gpu_launches": int(st["n_launches"]) * args.steps,
@@ -394,6 +397,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--n-lines", type=int, default=0)
+    ap.add_argument("--tile-bins", type=int, default=0, choices=[0, 2, 4, 8], help="bins per lane of a level-0 tile (0: library default)")
+    ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2, 3], help="hk_set_debug_mode (3: direct evaluation only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

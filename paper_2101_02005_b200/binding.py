@@ -20,7 +20,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 HK_OK, HK_EINVAL, HK_ESTATE, HK_ENOSPC, HK_ECUDA, HK_ENOMEM = 0, -1, -2, -3, -4, -5
-HK_Z1, HK_Z2 = 90000.0, 625.0
+HK_Z1, HK_Z2, HK_Z4, HK_Z3 = 90000.0, 625.0, 64.0, 30.25
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
@@ -28,7 +28,7 @@ EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_w
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation",
            "hk_last_cuda_error", "hk_strerror")
-PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "near", "down")
+PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "near", "down")
 
 
 class hk_lines(C.Structure):
@@ -37,8 +37,9 @@ class hk_lines(C.Structure):
 
 class hk_stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n_lines", "n_skipped", "n_off_grid", "n_evals", "n_evals_far",
-                                         "n_evals_mid", "n_evals_core", "n_units_far", "n_units_mid", "n_units_near",
-                                         "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_pairs_node",
+                                         "n_evals_mid", "n_evals_core", "n_evals_gh6", "n_evals_trap", "n_units_far", "n_units_mid", "n_units_near",
+                                         "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_units_edge",
+                                         "n_units_centre", "n_pairs_edge", "n_pairs_centre", "n_pairs_node",
                                          "n_bins_node", "n_launches")] + \
                [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("n_levels", C.c_int32)]
 

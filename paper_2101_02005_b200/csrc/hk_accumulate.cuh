@@ -41,6 +41,8 @@ struct AccArgs {
     // element is the slice's base): n_ct + 1 entries for the direct kernels, n_entries + 1 for the node kernel
     const int32_t* __restrict__ prefix_far;
     const int32_t* __restrict__ prefix_mid;
+    const int32_t* __restrict__ prefix_edge;
+    const int32_t* __restrict__ prefix_centre;
     const int32_t* __restrict__ prefix_near;
     const int32_t* __restrict__ prefix_node;
     DevStats* st;
@@ -261,6 +263,326 @@ __global__ void __launch_bounds__(kThreads, 2) interior_kernel(AccArgs a)
 }
 
 // ---------------------------------------------------------------------------------------
+// edge kernel: tiles only partly inside a line's extent, |z|^2 >= Z2 on the whole tile
+// ---------------------------------------------------------------------------------------
+// Same shape as the mid kernel; the exact integer extent (R7) is applied by selecting the term to zero
+// where the lane's bin lies outside [ilo, ihi] (two compares and a select on the ALU pipe).
+constexpr int kSubE = 512;
+constexpr int kLPTE = kSubE / kThreads;
+
+template <int KB>
+__global__ void __launch_bounds__(kThreads, 2) edge_kernel(AccArgs a)
+{
+    constexpr int kTB = 32 * KB;
+    constexpr int M = KB / 2;
+    static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubE, "red must fit in the staging buffers");
+    __shared__ float4 sm[2][kSubE];       // { -tl, G2, c, 1.5 a2 }
+    __shared__ float2 sm2[2][kSubE];      // { ilo, ihi } relative to the tile
+    __shared__ int s_unit;
+    double* red = reinterpret_cast<double*>(&sm[0][0]);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int32_t* __restrict__ prefix = a.prefix_edge;
+    const int base = prefix[0], total = prefix[a.n_ct];
+
+    float2 tb[M];
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        float b0 = (float)(lane + 64 * m);
+        tb[m] = make_float2(b0, b0 + 32.0f);
+    }
+
+    for (;;) {
+        const int u = next_unit(&a.st->unit_counter_edge, &s_unit) + base;
+        if (u >= total) break;
+        const int ct = find_tile(prefix, a.n_ct, u);
+        const int64_t ct0 = (int64_t)ct * kTB;
+        const TileRange r = a.tr[ct];
+        const int sl0 = r.A0, sl1 = r.EL, sr0 = r.ER, sr1 = r.A1;
+        const int v_lo = (u - prefix[ct]) * a.chunk;
+        const int v_hi = min(v_lo + a.chunk, (sl1 - sl0) + (sr1 - sr0));
+        const int l0 = min(sl0 + v_lo, sl1), l1 = min(sl0 + v_hi, sl1);
+        const int r0 = sr0 + max(v_lo - (sl1 - sl0), 0), r1 = sr0 + max(v_hi - (sl1 - sl0), 0);
+        const int nl = l1 - l0, nt = nl + (r1 - r0);
+        if (nt <= 0) continue;
+        if (threadIdx.x == 0) atomicAdd(&a.st->units_edge, 1ULL);
+
+        float2 acc[M];
+        double acc64[KB];
+#pragma unroll
+        for (int m = 0; m < M; ++m) acc[m] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < KB; ++j) acc64[j] = 0.0;
+        int since_flush = 0;
+
+        float4 preA[kLPTE], preB[kLPTE];
+        auto fetch = [&](int v0) {
+#pragma unroll
+            for (int k = 0; k < kLPTE; ++k) {
+                const int v = v0 + threadIdx.x + k * kThreads;
+                if (v < nt) {
+                    const int li = v < nl ? l0 + v : r0 + (v - nl);
+                    preA[k] = a.recA[li];
+                    preB[k] = a.recB[li];
+                }
+            }
+        };
+        auto stash = [&](int v0, int buf) {
+#pragma unroll
+            for (int k = 0; k < kLPTE; ++k) {
+                const int i = threadIdx.x + k * kThreads;
+                if (v0 + i < nt) {
+                    const int64_t lim = 1 << 24;
+                    const float tl = (float)((int64_t)__float_as_int(preA[k].x) - ct0) + preA[k].y;
+                    int64_t dlo = (int64_t)__float_as_int(preB[k].y) - ct0, dhi = (int64_t)__float_as_int(preB[k].z) - ct0;
+                    dlo = max(-lim, min(lim, dlo));
+                    dhi = max(-lim, min(lim, dhi));
+                    sm[buf][i] = make_float4(-tl, preA[k].z, preA[k].w, 1.5f * preB[k].x);
+                    sm2[buf][i] = make_float2((float)dlo, (float)dhi);
+                }
+            }
+        };
+        fetch(0);
+        stash(0, 0);
+        __syncthreads();
+        int buf = 0;
+        for (int v0 = 0; v0 < nt; v0 += kSubE, buf ^= 1) {
+            const bool more = v0 + kSubE < nt;
+            if (more) fetch(v0 + kSubE);
+            const float4* __restrict__ smb = sm[buf];
+            const float2* __restrict__ smm = sm2[buf];
+            int l, le;
+            warp_share(min(kSubE, nt - v0), warp, l, le);
+            while (l < le) {
+                const int stop = min(le, l + (kFlush - since_flush));
+                since_flush += stop - l;
+                for (; l < stop; ++l) {
+                    const float4 r1 = smb[l];
+                    const float2 ext = smm[l];
+                    const float2 n1 = bcast2(r1.x), g1 = bcast2(r1.y), c1 = bcast2(r1.z);
+                    const float2 A1 = bcast2(r1.w), one = bcast2(1.0f);
+                    const float2 nA2 = bcast2(-1.33333333f * r1.w * r1.y);
+#pragma unroll
+                    for (int m = 0; m < M; ++m) {
+                        const float2 t1 = __fadd2_rn(tb[m], n1);
+                        const float2 q1 = __ffma2_rn(t1, t1, g1);
+                        const float2 rr = rcp2(q1);
+                        const float2 uu = __ffma2_rn(nA2, rr, A1);
+                        const float2 vv = __ffma2_rn(uu, rr, one);
+                        float2 ww = __fmul2_rn(rr, vv);
+                        ww.x = (tb[m].x >= ext.x && tb[m].x <= ext.y) ? ww.x : 0.f;     // exact integer extent (R7)
+                        ww.y = (tb[m].y >= ext.x && tb[m].y <= ext.y) ? ww.y : 0.f;
+                        acc[m] = __ffma2_rn(c1, ww, acc[m]);
+                    }
+                }
+                if (since_flush >= kFlush) {
+#pragma unroll
+                    for (int m = 0; m < M; ++m) {
+                        acc64[2 * m] += (double)acc[m].x;
+                        acc64[2 * m + 1] += (double)acc[m].y;
+                        acc[m] = make_float2(0.f, 0.f);
+                    }
+                    since_flush = 0;
+                }
+            }
+            if (more) stash(v0 + kSubE, buf ^ 1);
+            __syncthreads();
+        }
+        double v[KB];
+#pragma unroll
+        for (int m = 0; m < M; ++m) {
+            v[2 * m] = acc64[2 * m] + (double)acc[m].x;
+            v[2 * m + 1] = acc64[2 * m + 1] + (double)acc[m].y;
+        }
+        flush_tile<KB>(red, v, ct0, a);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// centre kernel: tiles inside the extent that hold bins with |z|^2 < Z2 (the line's core) or lie within 2 KB bins
+// ---------------------------------------------------------------------------------------
+// Row pass (lanes own bins, the warp walks its lines): two-term asymptotic on every bin, the term selected to zero
+// where |z|^2 < Z2.  Core pass (lane <-> line, 32 lines at a time): all lanes step through the SAME bins, each
+// evaluating its own line's core there (adjacent sorted lines have nearly the same width, so the lanes sit in the
+// same |z| ring at the same time); the 32 x 16 values of a half-row go through a shared staging matrix and are
+// summed per bin (a transpose, no atomics), then added to the warp's bin tile in shared memory.
+constexpr int kSubC = 512;
+constexpr int kLPTC = kSubC / kThreads;
+constexpr int kStage = 16;             // bins per staging step of the core pass
+
+template <int KB>
+__global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
+{
+    constexpr int kTB = 32 * KB;
+    constexpr int M = KB / 2;
+    static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubC, "red must fit in the staging buffers");
+    __shared__ float4 smem[2][kSubC];          // A = { -dl, G2, c, 1.5 a2 }, B = { -f, qc, cK, y }
+    __shared__ float stage[kWarps][kStage][33];
+    __shared__ float sacc[kWarps][kTB];
+    __shared__ int s_unit;
+    float4* smA = smem[0];
+    float4* smB = smem[1];
+    double* red = reinterpret_cast<double*>(&smem[0][0]);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int32_t* __restrict__ prefix = a.prefix_centre;
+    const int base = prefix[0], total = prefix[a.n_ct];
+    const float whi = (float)(kTB - 1);
+
+    float2 tb[M];
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        float b0 = (float)(lane + 64 * m);
+        tb[m] = make_float2(b0, b0 + 32.0f);
+    }
+#pragma unroll
+    for (int j = 0; j < KB; ++j) sacc[warp][lane + 32 * j] = 0.f;
+
+    for (;;) {
+        const int u = next_unit(&a.st->unit_counter_centre, &s_unit) + base;
+        if (u >= total) break;
+        const int ct = find_tile(prefix, a.n_ct, u);
+        const int64_t ct0 = (int64_t)ct * kTB;
+        const TileRange r = a.tr[ct];
+        const int c0 = r.CL + (u - prefix[ct]) * a.chunk;
+        const int nt = min(a.chunk, r.CR - c0);
+        if (nt <= 0) continue;
+        if (threadIdx.x == 0) atomicAdd(&a.st->units_centre, 1ULL);
+
+        float2 acc[M];
+        double acc64[KB];
+#pragma unroll
+        for (int m = 0; m < M; ++m) acc[m] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < KB; ++j) acc64[j] = 0.0;
+        int since_flush = 0;
+        auto flush = [&]() {
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                acc64[2 * m] += (double)acc[m].x + (double)sacc[warp][lane + 64 * m];
+                acc64[2 * m + 1] += (double)acc[m].y + (double)sacc[warp][lane + 64 * m + 32];
+                acc[m] = make_float2(0.f, 0.f);
+                sacc[warp][lane + 64 * m] = 0.f;
+                sacc[warp][lane + 64 * m + 32] = 0.f;
+            }
+            since_flush = 0;
+            __syncwarp();
+        };
+
+        float4 preA[kLPTC], preB[kLPTC];
+        auto fetch = [&](int v0) {
+#pragma unroll
+            for (int k = 0; k < kLPTC; ++k) {
+                const int v = v0 + threadIdx.x + k * kThreads;
+                if (v < nt) { preA[k] = a.recA[c0 + v]; preB[k] = a.recB[c0 + v]; }
+            }
+        };
+        auto stash = [&](int v0) {
+#pragma unroll
+            for (int k = 0; k < kLPTC; ++k) {
+                const int i = threadIdx.x + k * kThreads;
+                if (v0 + i < nt) {
+                    const float4 ra = preA[k], rb = preB[k];
+                    const float fdj = (float)((int64_t)__float_as_int(ra.x) - ct0);
+                    const float G2 = ra.z, a2 = rb.x;
+                    smA[i] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
+                    smB[i] = make_float4(-ra.y, HK_Z2 * a2, rb.w, sqrtf(G2) * rsqrtf(a2));
+                }
+            }
+        };
+        fetch(0);
+        for (int v0 = 0; v0 < nt; v0 += kSubC) {
+            __syncthreads();                        // previous batch fully consumed
+            stash(v0);
+            __syncthreads();
+            if (v0 + kSubC < nt) fetch(v0 + kSubC);
+            int wl0, wl1;
+            warp_share(min(kSubC, nt - v0), warp, wl0, wl1);
+            // ---- row pass
+            int l = wl0;
+            while (l < wl1) {
+                const int stop = min(wl1, l + (kFlush - since_flush));
+                since_flush += stop - l;
+                for (; l < stop; ++l) {
+                    const float4 A = smA[l], B = smB[l];
+                    const float2 ndl = bcast2(A.x), nf = bcast2(B.x), g = bcast2(A.y), c = bcast2(A.z);
+                    const float2 A1 = bcast2(A.w), one = bcast2(1.0f);
+                    const float2 nA2 = bcast2(-1.33333333f * A.w * A.y);
+                    const float qc = B.y;
+#pragma unroll
+                    for (int m = 0; m < M; ++m) {
+                        const float2 d = __fadd2_rn(tb[m], ndl);         // exact: both are small integers
+                        const float2 t = __fadd2_rn(d, nf);
+                        const float2 q = __ffma2_rn(t, t, g);
+                        const float2 rr = rcp2(q);
+                        const float2 uu = __ffma2_rn(nA2, rr, A1);
+                        const float2 vv = __ffma2_rn(uu, rr, one);
+                        float2 ww = __fmul2_rn(rr, vv);
+                        ww.x = q.x >= qc ? ww.x : 0.f;                  // the core pass owns these bins
+                        ww.y = q.y >= qc ? ww.y : 0.f;
+                        acc[m] = __ffma2_rn(c, ww, acc[m]);
+                    }
+                }
+                if (since_flush >= kFlush) flush();
+            }
+            // ---- core pass
+#pragma unroll 1
+            for (int lb = wl0; lb < wl1; lb += 32) {
+                const int li = lb + lane;
+                float dl = 0.f, f = 0.f, G2 = 1.f, cK = 0.f, qc = 0.f, y = 1.f, inv_a = 1.f;
+                float clo = 1e9f, chi = -1e9f;
+                if (li < wl1) {
+                    const float4 A = smA[li], B = smB[li];
+                    dl = -A.x; f = -B.x; G2 = A.y; qc = B.y; cK = B.z; y = B.w;
+                    const float h2 = qc - G2;
+                    if (h2 > 0.f) {
+                        const float hw = sqrtf(h2) + 1.0f;                       // |t| < hw covers every q < qc
+                        const float pos = dl + f;
+                        const float lo = fmaxf(ceilf(pos - hw), 0.f), hi = fminf(floorf(pos + hw), whi);
+                        if (hi >= lo) { clo = lo; chi = hi; }
+                    }
+                    inv_a = rsqrtf(A.w * (1.0f / 1.5f));
+                }
+                float bmin = clo, bmax = chi;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    bmin = fminf(bmin, __shfl_xor_sync(0xffffffffu, bmin, o));
+                    bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
+                }
+                if (bmax < bmin) continue;
+                const int b_end = (int)bmax;
+                const int col = lane & (kStage - 1), half = lane >> 4;
+#pragma unroll 1
+                for (int b0 = ((int)bmin) & ~(kStage - 1); b0 <= b_end; b0 += kStage) {
+#pragma unroll 1
+                    for (int s = 0; s < kStage; ++s) {
+                        const float fb = (float)(b0 + s);
+                        float val = 0.f;
+                        if (fb >= clo && fb <= chi) {
+                            const float t = (fb - dl) - f;
+                            const float q = fmaf(t, t, G2);
+                            if (q < qc) val = cK * core_any_K(fabsf(t) * inv_a, y, nullptr);
+                        }
+                        stage[warp][s][lane] = val;
+                    }
+                    __syncwarp();
+                    float sum = 0.f;
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) sum += stage[warp][col][half * 16 + j];
+                    sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+                    if (half == 0 && b0 + col < kTB) sacc[warp][b0 + col] += sum;
+                    __syncwarp();
+                }
+                since_flush += 32;     // the bin tile holds at most 32 lines' terms per bin per batch
+                if (since_flush >= kFlush) flush();
+            }
+        }
+        flush();
+        __syncthreads();               // every warp is done with the staging buffers: red may overwrite them
+        flush_tile<KB>(red, acc64, ct0, a);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // near / edge kernel
 // ---------------------------------------------------------------------------------------
 constexpr int kSubN = 512;             // lines per staged batch
@@ -305,10 +627,10 @@ __device__ __forceinline__ void near_rows(float2 (&acc)[KB / 2], const float2 (&
         acc[m] = __ffma2_rn(cm, ww, acc[m]);
         if (kCore && wide) {
             if (__any_sync(0xffffffffu, in0 && co0)) {
-                if (in0 && co0) acc[m].x = fmaf(B.w, core_K(fabsf(t.x) * inv_a, C.z), acc[m].x);
+                if (in0 && co0) acc[m].x = fmaf(B.w, core_any_K(fabsf(t.x) * inv_a, C.z, nullptr), acc[m].x);
             }
             if (__any_sync(0xffffffffu, in1 && co1)) {
-                if (in1 && co1) acc[m].y = fmaf(B.w, core_K(fabsf(t.y) * inv_a, C.z), acc[m].y);
+                if (in1 && co1) acc[m].y = fmaf(B.w, core_any_K(fabsf(t.y) * inv_a, C.z, nullptr), acc[m].y);
             }
         }
     }
@@ -347,15 +669,16 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
         const int ct = find_tile(prefix, a.n_ct, u);
         const int64_t ct0 = (int64_t)ct * kTB;
         const TileRange r = a.tr[ct];
-        // left-edge, centre and right-edge segments walked as one list; this unit takes lines [v_lo, v_hi) of it
-        const int s0 = r.FL0 - r.A0, s1 = r.MR0 - r.ML1, s2 = r.A1 - r.FR1;
+        // the generic parts of the edge and centre segments walked as one list; this unit takes lines [v_lo, v_hi) of it
+        const int s0 = r.FL0 - r.EL, s1 = r.CL - r.ML1, s2 = r.MR0 - r.CR, s3 = r.ER - r.FR1;
         const int v_lo = (u - prefix[ct]) * a.chunk;
-        const int v_hi = min(v_lo + a.chunk, s0 + s1 + s2);
+        const int v_hi = min(v_lo + a.chunk, s0 + s1 + s2 + s3);
         auto clip = [](int v, int n) { return max(0, min(v, n)); };
-        const int g0 = r.A0 + clip(v_lo, s0), n0 = clip(v_hi, s0) - clip(v_lo, s0);
+        const int g0 = r.EL + clip(v_lo, s0), n0 = clip(v_hi, s0) - clip(v_lo, s0);
         const int g1 = r.ML1 + clip(v_lo - s0, s1), n1 = clip(v_hi - s0, s1) - clip(v_lo - s0, s1);
-        const int g2 = r.FR1 + clip(v_lo - s0 - s1, s2), n2 = clip(v_hi - s0 - s1, s2) - clip(v_lo - s0 - s1, s2);
-        const int nt = n0 + n1 + n2;
+        const int g2 = r.CR + clip(v_lo - s0 - s1, s2), n2 = clip(v_hi - s0 - s1, s2) - clip(v_lo - s0 - s1, s2);
+        const int g3 = r.FR1 + clip(v_lo - s0 - s1 - s2, s3), n3 = clip(v_hi - s0 - s1 - s2, s3) - clip(v_lo - s0 - s1 - s2, s3);
+        const int nt = n0 + n1 + n2 + n3;
         if (nt <= 0) continue;
         if (threadIdx.x == 0) atomicAdd(&a.st->units_near, 1ULL);
 
@@ -386,7 +709,9 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
             for (int k = 0; k < kLPTN; ++k) {
                 const int v = v0 + threadIdx.x + k * kThreads;
                 if (v < nt) {
-                    const int li = v < n0 ? g0 + v : (v < n0 + n1 ? g1 + (v - n0) : g2 + (v - n0 - n1));
+                    const int li = v < n0 ? g0 + v
+                                 : v < n0 + n1 ? g1 + (v - n0)
+                                 : v < n0 + n1 + n2 ? g2 + (v - n0 - n1) : g3 + (v - n0 - n1 - n2);
                     preA[k] = a.recA[li];
                     preB[k] = a.recB[li];
                 }
@@ -478,7 +803,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                         const float d = fb - dlt;
                         const float t = d - f;
                         const float q = fmaf(t, t, G2);
-                        if (q < qc) { val = cK * core_K(fabsf(t) * inv_a, y); bin = (int)fb; }
+                        if (q < qc) { val = cK * core_any_K(fabsf(t) * inv_a, y, nullptr); bin = (int)fb; }
                     }
                     // combine equal bins in the warp (sorted lines: neighbours share bins), one add per distinct bin
                     unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
@@ -637,7 +962,7 @@ __global__ void __launch_bounds__(256) probe_kernel(const float* __restrict__ x,
         int reg;
         if (q >= HK_Z1) { K = term_far(c, q); reg = 0; }
         else if (q >= HK_Z2) { K = c * shape_mid(rcp_approx(q), 1.5f, 2.0f * G2); reg = 1; }
-        else { K = core_K(fabsf(t), G); reg = 2; }
+        else { K = core_any_K(fabsf(t), G, &reg); }
         out[i] = K;
         if (region) region[i] = reg;
     }

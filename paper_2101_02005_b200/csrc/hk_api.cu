@@ -53,7 +53,7 @@ struct Layout {
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
     int32_t n_entries;   // upper bound on (level, tile) entries of the node hierarchy
-    int32_t n_counts;    // work-unit counts: 3 n_ct (far, mid, near) + n_entries (node) + 1
+    int32_t n_counts;    // work-unit counts: 5 n_ct (far, mid, edge, centre, near) + n_entries (node) + 1
 };
 
 bool is_uncut(double cut) { return !(cut > 0.0 && std::isfinite(cut)); }
@@ -87,7 +87,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     Layout L;
     L.n_ct = (int32_t)((c->N + 32 * kMinKB - 1) / (32 * kMinKB));
     L.n_entries = 2 * L.n_ct + kMaxLevels;
-    L.n_counts = 3 * L.n_ct + L.n_entries + 1;
+    L.n_counts = 5 * L.n_ct + L.n_entries + 1;
     size_t nn = (size_t)(n > 0 ? n : 1);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -391,14 +391,17 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
                                             (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
     gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB, recN);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
-    // a3: tile ranges, node ranges and work units.  counts = [far | mid | near | node | 0], one scan.
-    const int n_counts = 3 * p.n_ct + lv.n_entries + 1;
+    // a3: tile ranges, node ranges and work units.  counts = [far | mid | edge | centre | near | node | 0], one scan.
+    const int n_counts = 5 * p.n_ct + lv.n_entries + 1;
     int32_t* cnt_far = counts;
     int32_t* cnt_mid = counts + p.n_ct;
-    int32_t* cnt_near = counts + 2 * p.n_ct;
-    int32_t* cnt_node = counts + 3 * p.n_ct;
+    int32_t* cnt_edge = counts + 2 * p.n_ct;
+    int32_t* cnt_centre = counts + 3 * p.n_ct;
+    int32_t* cnt_near = counts + 4 * p.n_ct;
+    int32_t* cnt_node = counts + 5 * p.n_ct;
     HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
-    range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_near, st);
+    range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_edge, cnt_centre,
+                                                           cnt_near, st);
     ctx->last_launches = 5;
     if (lv.n_entries > 0) {
         HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
@@ -411,8 +414,9 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     // a4-a7: accumulate
     AccArgs a;
     a.recA = recA; a.recB = recB; a.recN = recN; a.tr = tr; a.nr = nr;
-    a.prefix_far = prefix; a.prefix_mid = prefix + p.n_ct; a.prefix_near = prefix + 2 * p.n_ct;
-    a.prefix_node = prefix + 3 * p.n_ct;
+    a.prefix_far = prefix; a.prefix_mid = prefix + p.n_ct; a.prefix_edge = prefix + 2 * p.n_ct;
+    a.prefix_centre = prefix + 3 * p.n_ct; a.prefix_near = prefix + 4 * p.n_ct;
+    a.prefix_node = prefix + 5 * p.n_ct;
     a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc;
     a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.lv = lv;
     const int grid = ctx->n_sm * 2;
@@ -424,6 +428,10 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream);
         if (p.mode != 1) { interior_kernel<KB, true><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
+        if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
+        if (p.mode == 0 || p.mode == 3) { centre_kernel<KB><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
         near_kernel<KB><<<grid, kThreads, 0, stream>>>(a);
         ++ctx->last_launches;
         cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream);
@@ -615,6 +623,8 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_evals_far = (int64_t)(d.n_evals - d.n_cnt_mid);
     host_out->n_evals_mid = (int64_t)(d.n_cnt_mid - d.n_cnt_core);
     host_out->n_evals_core = (int64_t)d.n_cnt_core;
+    host_out->n_evals_gh6 = (int64_t)(d.n_cnt_gh6 - d.n_cnt_trap);
+    host_out->n_evals_trap = (int64_t)d.n_cnt_trap;
     host_out->n_units_far = (int64_t)d.units_far;
     host_out->n_units_mid = (int64_t)d.units_mid;
     host_out->n_units_near = (int64_t)d.units_near;
@@ -624,6 +634,10 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_pairs_near = (int64_t)d.pairs_near;
     host_out->n_launches = ctx->last_launches;
     host_out->n_units_node = (int64_t)d.units_node;
+    host_out->n_units_edge = (int64_t)d.units_edge;
+    host_out->n_units_centre = (int64_t)d.units_centre;
+    host_out->n_pairs_edge = (int64_t)d.pairs_edge;
+    host_out->n_pairs_centre = (int64_t)d.pairs_centre;
     host_out->n_pairs_node = (int64_t)d.pairs_node;
     host_out->n_bins_node = (int64_t)d.bins_node;
     host_out->n_levels = ctx->last_levels;

@@ -40,12 +40,15 @@ struct Params {
 
 struct DevStats {
     unsigned long long n_skipped, n_off_grid, n_evals, n_cnt_mid, n_cnt_core;  // cnt_*: evals with |z|^2 below Z1 / Z2
+    unsigned long long n_cnt_gh6, n_cnt_trap;                                  // ... below Z4 / Z3
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
     int32_t pad;
     unsigned int unit_counter_far, unit_counter_mid, unit_counter_near, unit_counter_node;
-    unsigned long long units_far, units_mid, units_near, units_node;
+    unsigned int unit_counter_edge, unit_counter_centre;
+    unsigned long long units_far, units_mid, units_near, units_node, units_edge, units_centre;
     unsigned long long pairs_far, pairs_mid, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
+    unsigned long long pairs_edge, pairs_centre;
     unsigned long long pairs_node;                         // (line, tile) pairs evaluated at nodes
     unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
 };
@@ -117,7 +120,7 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
                                                    int32_t* __restrict__ key, int32_t* __restrict__ idx,
                                                    DevStats* __restrict__ st)
 {
-    unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cmaxb = 0, cKmaxb = 0;
+    unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cgh6 = 0, ctrap = 0, cmaxb = 0, cKmaxb = 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         LineOut o = line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
         RecU r;
@@ -146,32 +149,36 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
             double t1 = (double)HK_Z1 * ab * ab - Gb * Gb, t2 = (double)HK_Z2 * ab * ab - Gb * Gb;
             cmid += (unsigned long long)count_within(pos, t1 > 0 ? sqrt(t1) : 0.0, o.ilo, o.ihi);
             ccore += (unsigned long long)count_within(pos, t2 > 0 ? sqrt(t2) : 0.0, o.ilo, o.ihi);
+            const double y2 = (Gb * Gb) / (ab * ab);
+            const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
+            cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? sqrt(t4) : 0.0, o.ilo, o.ihi);
+            ctrap += (unsigned long long)count_within(pos, t3 > 0 ? sqrt(t3) : 0.0, o.ilo, o.ihi);
         }
         rec[i] = r;
         key[i] = k;
         idx[i] = (int32_t)i;
     }
     // block reduction of the counters
-    __shared__ unsigned long long sh[7][8];
-    unsigned long long v[7] = {skipped, off, evals, cmid, ccore, cmaxb, cKmaxb};
+    __shared__ unsigned long long sh[9][8];
+    unsigned long long v[9] = {skipped, off, evals, cmid, ccore, cgh6, ctrap, cmaxb, cKmaxb};
 #pragma unroll
-    for (int q = 0; q < 7; ++q) {
+    for (int q = 0; q < 9; ++q) {
         unsigned long long x = v[q];
         for (int o = 16; o > 0; o >>= 1) {
             unsigned long long y = __shfl_xor_sync(0xffffffffu, x, o);
-            x = (q < 5) ? x + y : max(x, y);
+            x = (q < 7) ? x + y : max(x, y);
         }
         if ((threadIdx.x & 31) == 0) sh[q][threadIdx.x >> 5] = x;
     }
     __syncthreads();
-    if (threadIdx.x < 7) {
+    if (threadIdx.x < 9) {
         int q = threadIdx.x;
         unsigned long long x = sh[q][0];
-        for (int w = 1; w < 8; ++w) x = (q < 5) ? x + sh[q][w] : max(x, sh[q][w]);
+        for (int w = 1; w < 8; ++w) x = (q < 7) ? x + sh[q][w] : max(x, sh[q][w]);
         unsigned long long* dst = q == 0 ? &st->n_skipped : q == 1 ? &st->n_off_grid : q == 2 ? &st->n_evals
-                                : q == 3 ? &st->n_cnt_mid : q == 4 ? &st->n_cnt_core : q == 5 ? &st->cmax_bits
-                                : &st->cKmax_bits;
-        if (q < 5) { if (x) atomicAdd(dst, x); }
+                                : q == 3 ? &st->n_cnt_mid : q == 4 ? &st->n_cnt_core : q == 5 ? &st->n_cnt_gh6
+                                : q == 6 ? &st->n_cnt_trap : q == 7 ? &st->cmax_bits : &st->cKmax_bits;
+        if (q < 7) { if (x) atomicAdd(dst, x); }
         else atomicMax(dst, x);
     }
 }
@@ -329,7 +336,8 @@ __global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, co
 // condition is a bound on the centre bin alone; all bounds are conservative.
 __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const int32_t* __restrict__ keys, int32_t n,
                                                     TileRange* __restrict__ tr, int32_t* __restrict__ cnt_far,
-                                                    int32_t* __restrict__ cnt_mid, int32_t* __restrict__ cnt_near,
+                                                    int32_t* __restrict__ cnt_mid, int32_t* __restrict__ cnt_edge,
+                                                    int32_t* __restrict__ cnt_centre, int32_t* __restrict__ cnt_near,
                                                     DevStats* __restrict__ st)
 {
     int wt = blockIdx.x * blockDim.x + threadIdx.x;
@@ -379,16 +387,32 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
     fl1 = max(fl1, nl);
     fr0 = min(fr0, nrr);
     r.FL0 = fl0; r.NL = nl; r.FL1 = fl1; r.ML1 = ml1; r.MR0 = mr0; r.FR0 = fr0; r.NR = nrr; r.FR1 = fr1;
+    // formula-uniform parts of the edge and centre segments (the rest stays with the generic near kernel):
+    //   edge, no core : the tile is only partly inside the extent, but |z|^2 >= Z2 on all of it
+    //   centre, full  : the tile is inside the extent; bins with |z|^2 < Z2 exist
+    r.EL = r.A0; r.ER = r.A1; r.CL = ml1; r.CR = ml1;
+    if (p.mode == 0 || p.mode == 3) {
+        r.EL = min(max(idx_of(p, keys, n_act, jLmid + 1), r.A0), fl0);
+        r.ER = max(min(idx_of(p, keys, n_act, jRmid), r.A1), fr1);
+        r.CL = min(max(idx_of(p, keys, n_act, jLmin), ml1), mr0);
+        r.CR = min(max(idx_of(p, keys, n_act, jRmax + 1), r.CL), mr0);
+    }
     tr[wt] = r;
     const unsigned long long nb = (unsigned long long)(w1 - w0);
     const long long nfar = (long long)(fl1 - nl) + (nrr - fr0);
     const long long nmid = (long long)(ml1 - fl1) + (fr0 - mr0);
-    const long long nnear = (long long)(fl0 - r.A0) + (mr0 - ml1) + (r.A1 - fr1);
+    const long long nedge = (long long)(r.EL - r.A0) + (r.A1 - r.ER);
+    const long long ncen = (long long)(r.CR - r.CL);
+    const long long nnear = (long long)(fl0 - r.EL) + (r.CL - ml1) + (mr0 - r.CR) + (r.ER - fr1);
     cnt_far[wt] = (int32_t)((nfar + p.chunk - 1) / p.chunk);
     cnt_mid[wt] = (int32_t)((nmid + p.chunk - 1) / p.chunk);
+    cnt_edge[wt] = (int32_t)((nedge + p.chunk - 1) / p.chunk);
+    cnt_centre[wt] = (int32_t)((ncen + p.chunk - 1) / p.chunk);
     cnt_near[wt] = (int32_t)((nnear + p.chunk - 1) / p.chunk);
     if (nfar) atomicAdd(&st->pairs_far, (unsigned long long)nfar * nb);
     if (nmid) atomicAdd(&st->pairs_mid, (unsigned long long)nmid * nb);
+    if (nedge) atomicAdd(&st->pairs_edge, (unsigned long long)nedge * nb);
+    if (ncen) atomicAdd(&st->pairs_centre, (unsigned long long)ncen * nb);
     if (nnear) atomicAdd(&st->pairs_near, (unsigned long long)nnear * nb);
 }
 

@@ -105,13 +105,13 @@ def test_cross_path_nodes_vs_direct(B):
     for cfg, n, tb in [(2, 20_000, 0), (4, 6_000, 0), (4, 6_000, 2), (3, 100_000, 2), (5, 300, 0)]:
         lines, cond, grid, cut = _mini(cfg, n)
         k0, st0, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=0, tile_bins=tb)
-        assert st0["n_levels"] >= 1 and st0["n_pairs_node"] > 0 and st0["n_pairs_near"] > 0
+        assert st0["n_levels"] >= 1 and st0["n_pairs_node"] > 0 and st0["n_pairs_centre"] > 0
         k3, st3, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=3, tile_bins=tb)
         assert st3["n_levels"] == 0 and st3["n_pairs_node"] == 0 and st3["n_pairs_far"] > 0 and st3["n_pairs_mid"] > 0
         # every (line, bin) pair of the definition is covered exactly once by one of the four paths
         for st in (st0, st3):
             cover = st["n_pairs_far"] + st["n_pairs_mid"] + st["n_bins_node"]
-            assert cover <= st["n_evals"] <= cover + st["n_pairs_near"]
+            assert cover <= st["n_evals"] <= cover + st["n_pairs_near"] + st["n_pairs_edge"] + st["n_pairs_centre"]
         big = k3 >= 1e-8 * k3.max()
         assert np.abs(k0[big] / k3[big] - 1.0).max() <= 3e-5
         if cfg == 5:
@@ -329,7 +329,7 @@ def test_evaluator_accuracy_map(B):
     ys = np.logspace(-2, 7, 576)
     X, Y = np.meshgrid(xs, ys, indexing="ij")
     # region boundaries +- a few ulp
-    for z2 in (B.HK_Z1, B.HK_Z2):
+    for z2 in (B.HK_Z1, B.HK_Z2, B.HK_Z4, B.HK_Z3, 50.0):
         for yv in np.logspace(-2, math.log10(math.sqrt(z2)) - 1e-3, 64):
             xb = math.sqrt(z2 - yv * yv)
             xe = xb * (1 + np.array([-4, -2, -1, 0, 1, 2, 4]) * 6e-8)
@@ -343,7 +343,7 @@ def test_evaluator_accuracy_map(B):
     ref = O.voigt_K(x32.astype(np.float64), y32.astype(np.float64))
     ok = ref > 1e-30                     # below that the term is far under any bin's tolerance
     rel = np.abs(got - ref) / np.maximum(ref, 1e-300)
-    for r, name in enumerate(("far", "mid", "core")):
+    for r, name in enumerate(("far", "mid", "gauss-hermite 4", "gauss-hermite 6", "trapezoid")):
         m = ok & (reg == r)
         assert m.any()
         worst = rel[m].max()
