@@ -334,7 +334,8 @@ def run_ours(args):
                       "accumulate": "fp32 evaluation, fp32 partial sums of <=128 terms flushed to fp64; fp64 preprocessing and output"},
            "voigt_evals_per_s": world * st["n_evals"] * args.steps / (total_ms * 1e-3),
            "evals_per_step": st["n_evals"],
-           "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"]},
+           "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"],
+                               "core_gh6": st["n_evals_gh6"], "core_trap": st["n_evals_trap"]},
            "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
                                "edge": st["n_pairs_edge"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
            "bins_per_lane": st["bins_per_lane"],

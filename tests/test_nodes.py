@@ -1,0 +1,107 @@
+"""The mathematical claims the separated-tile evaluation rests on, checked on the CPU
+against the fp64 oracle's profile -- no CUDA code involved:
+
+ 1. for a line whose centre is at least `sep` tile half-widths from the centre of a tile and with |z|^2 >= Z2 on the
+    tile, the degree-7 Chebyshev interpolant of S V(nu) over the tile is accurate to 1.6e-6 relative at sep = 4
+    (the error bound section 5 budgets), and degrades as the separation shrinks (why sep = 2.5 needs 3e-4);
+ 2. the restriction of a degree-7 polynomial from a parent tile's nodes to its two children's nodes is exact,
+    so the downward pass adds no error;
+ 3. a sum of interpolants is the interpolant of the sum (linearity), which is what lets lines share node sums.
+"""
+import numpy as np
+import pytest
+
+from oracle import hk_oracle as O
+
+P = 8
+XI = np.cos((2 * np.arange(P) + 1) * np.pi / (2 * P))                    # first-kind Chebyshev points
+BW = (-1.0) ** np.arange(P) * np.sin((2 * np.arange(P) + 1) * np.pi / (2 * P))   # their barycentric weights
+
+
+def bary(nodes_val, xi):
+    """Barycentric evaluation of the degree-(P-1) interpolant through values at XI."""
+    xi = np.atleast_1d(xi).astype(np.float64)
+    d = xi[:, None] - XI[None, :]
+    hit = d == 0.0
+    d[hit] = 1.0
+    w = BW[None, :] / d
+    out = (w * nodes_val[None, :]).sum(1) / w.sum(1)
+    rows, cols = np.nonzero(hit)
+    out[rows] = nodes_val[cols]
+    return out
+
+
+def tile_coords(W):
+    """Bin positions of a W-bin tile (relative to its first bin) and the same in [-1, 1], nodes included:
+    centre (W-1)/2, half-width W/2 -- the convention of the library's node kernel."""
+    b = np.arange(W, dtype=np.float64)
+    hc, hw = 0.5 * (W - 1), 0.5 * W
+    return b, (b - hc) / hw, hc + hw * XI
+
+
+def voigt_bins(t, G, a):
+    """Profile in bin units at offsets t from the centre: Re w((t + iG)/a) / (a sqrt(pi))."""
+    return O.voigt_K(np.abs(t) / a, np.full_like(t, G / a)) / (a * np.sqrt(np.pi))
+
+
+@pytest.mark.parametrize("W", [64, 256, 4096])
+@pytest.mark.parametrize("sep,tol", [(4.0, 1.6e-6), (6.0, 6e-8), (2.5, 1.2e-4)])
+def test_chebyshev_interpolant_of_a_separated_line(W, sep, tol):
+    b, xi, xn = tile_coords(W)
+    hc, hw = 0.5 * (W - 1), 0.5 * W
+    worst = 0.0
+    rng = np.random.default_rng(W)
+    for side in (-1.0, 1.0):
+        for extra in (0.0, 0.3, 2.0, 30.0):
+            pos = hc + side * ((sep + extra) * hw + rng.uniform(0, 1))    # centre, in bins from the tile start
+            dmin = np.abs(b - pos).min()
+            for G in (1e-3 * dmin, 0.05 * dmin, 0.5 * dmin, 3.0 * dmin):   # Lorentz half-width in bins
+                for a in (dmin / 26.0, dmin / 100.0, dmin / 1e4):           # |z| >= 25 on the whole tile
+                    exact = voigt_bins(b - pos, G, a)
+                    interp = bary(voigt_bins(xn - pos, G, a), xi)
+                    worst = max(worst, np.abs(interp / exact - 1.0).max())
+    assert worst <= tol, worst
+    if sep == 2.5:
+        assert worst > 1.5e-6        # closer tiles really are worse: the separation threshold matters
+
+
+def test_parent_to_child_restriction_is_exact():
+    rng = np.random.default_rng(0)
+    coef = rng.normal(size=P)                                   # a random degree-7 polynomial on the parent
+    poly = np.polynomial.chebyshev.Chebyshev(coef)
+    parent_nodes = poly(XI)
+    for child in (0, 1):
+        xi_child_in_parent = (-0.5 if child == 0 else 0.5) + 0.5 * XI
+        got = bary(parent_nodes, xi_child_in_parent)
+        assert np.abs(got - poly(xi_child_in_parent)).max() <= 1e-13
+        # and the child's own interpolant reproduces the parent's polynomial on the child's half
+        x = np.linspace(-1, 1, 33)
+        assert np.abs(bary(got, x) - poly((-0.5 if child == 0 else 0.5) + 0.5 * x)).max() <= 1e-12
+
+
+def test_tile_halving_matches_bin_geometry():
+    """A parent tile of 2W bins and its children of W bins: the children's node positions in bins are the
+    parent's polynomial argument (-+1/2 + xi/2) -- the identity node_down_kernel relies on."""
+    W = 128
+    _, _, xn_parent = tile_coords(2 * W)
+    hc_p, hw_p = 0.5 * (2 * W - 1), 0.5 * (2 * W)
+    for child in (0, 1):
+        _, _, xn = tile_coords(W)
+        pos_in_parent_bins = child * W + xn
+        xi_p = (pos_in_parent_bins - hc_p) / hw_p
+        assert np.abs(xi_p - ((-0.5 if child == 0 else 0.5) + 0.5 * XI)).max() <= 1e-14
+
+
+def test_sum_of_interpolants_is_interpolant_of_sum():
+    W = 256
+    b, xi, xn = tile_coords(W)
+    rng = np.random.default_rng(4)
+    pos = 0.5 * (W - 1) + rng.choice([-1, 1], 50) * rng.uniform(4.0, 40.0, 50) * 0.5 * W
+    G = rng.uniform(0.5, 30.0, 50)
+    a = rng.uniform(0.05, 4.0, 50)
+    S = 10 ** rng.uniform(-6, 2, 50)
+    node_sum = sum(s * voigt_bins(xn - p, g, aa) for s, p, g, aa in zip(S, pos, G, a))
+    exact = sum(s * voigt_bins(b - p, g, aa) for s, p, g, aa in zip(S, pos, G, a))
+    each = sum(bary(s * voigt_bins(xn - p, g, aa), xi) for s, p, g, aa in zip(S, pos, G, a))
+    assert np.abs(bary(node_sum, xi) / each - 1.0).max() <= 1e-12
+    assert np.abs(bary(node_sum, xi) / exact - 1.0).max() <= 1.6e-6
