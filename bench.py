@@ -261,7 +261,6 @@ def run_ours(args):
     for _ in range(max(args.warmup, 0)):
         step()
     torch.cuda.synchronize()
-    st = op.stats()
 
     def barrier():
         torch.cuda.synchronize()
@@ -289,6 +288,7 @@ def run_ours(args):
             phases[p] += v
     barrier()
     clocks = sampler.stop() if sampler else None
+    st = op.stats()
     step_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
     total_ms = float(sum(step_ms))
     if dist is not None:

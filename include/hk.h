@@ -65,7 +65,7 @@ typedef struct {
     int64_t n_evals_mid;   /* HK_Z2 <= |z|^2 < HK_Z1 (2-term asymptotic) */
     int64_t n_evals_core;  /* |z|^2 < HK_Z2: 4-point Gauss-Hermite (>= HK_Z4), 6-point (>= HK_Z3), trapezoid + pole term below */
     int64_t n_evals_gh6;   /* of n_evals_core: HK_Z3 <= |z|^2 < HK_Z4 */
-    int64_t n_evals_trap;  /* of n_evals_core: |z|^2 < HK_Z3 */
+    int64_t n_evals_trap;  /* of n_evals_core: |z|^2 < HK_Z3 (trapezoid, or 10-point Gauss-Hermite when y >= 2) */
     int64_t n_units_far;   /* (tile, line-chunk) work units run by the far kernel */
     int64_t n_units_mid;   /* ... by the mid kernel */
     int64_t n_units_near;  /* ... by the near/edge kernel */
@@ -94,7 +94,7 @@ enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, H
 #define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */
 #define HK_Z2 625.0f   /* |z| >= 25 : two asymptotic terms, relative error <= 1.0e-5 */
 #define HK_Z4 64.0f    /* 8 <= |z| < 25: 4-point Gauss-Hermite rational form, <= 1.0e-6; below: 6-point, <= 7.7e-6 */
-#define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3): trapezoid rule + pole term, <= 2e-6 */
+#define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3): trapezoid rule + pole term, <= 2e-6; 10-point Gauss-Hermite when y >= 2, <= 2.7e-6 */
 #define HK_NODES 8     /* Chebyshev nodes per tile of the separated-tile evaluation */
 
 /* Grid: bin i is the POINT nu_i = numin + i*dnu (R8, R9).  HK_EINVAL if dnu <= 0,
@@ -168,7 +168,8 @@ int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, 
 /* Accuracy probe for the shipped fp32 evaluator (the counterpart of the paper's
  * Fig. 4): out[i] = Re w(x[i] + i y[i]) exactly as the accumulation
  * kernels evaluate it (region chosen by |z|^2 with alpha_D = 1 bin).  DEVICE fp32
- * arrays of n.  region_out (optional, int32): 0 far, 1 mid, 2 Gauss-Hermite 4, 3 Gauss-Hermite 6, 4 trapezoid. */
+ * arrays of n.  region_out (optional, int32): 0 far, 1 mid, 2 Gauss-Hermite 4, 3 Gauss-Hermite 6, 4 trapezoid,
+ * 5 Gauss-Hermite 10 (|z|^2 < HK_Z3 and y >= 2). */
 int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev,
                       int32_t* region_out_dev, void* stream);
 

@@ -400,14 +400,30 @@ __global__ void __launch_bounds__(kThreads, 2) edge_kernel(AccArgs a)
 // ---------------------------------------------------------------------------------------
 // centre kernel: tiles inside the extent that hold bins with |z|^2 < Z2 (the line's core) or lie within 2 KB bins
 // ---------------------------------------------------------------------------------------
-// Row pass (lanes own bins, the warp walks its lines): two-term asymptotic on every bin, the term selected to zero
-// where |z|^2 < Z2.  Core pass (lane <-> line, 32 lines at a time): all lanes step through the SAME bins, each
-// evaluating its own line's core there (adjacent sorted lines have nearly the same width, so the lanes sit in the
-// same |z| ring at the same time); the 32 x 16 values of a half-row go through a shared staging matrix and are
-// summed per bin (a transpose, no atomics), then added to the warp's bin tile in shared memory.
+// Row pass (lanes own bins, the warp walks its lines).  Per (line, tile) one of two row formulas, decided when the
+// line is staged: "Gauss-Hermite 4" rows where the tile holds core bins (valid for every |z|^2 >= Z4, so the whole
+// outer ring 8 <= |z| < 25 -- three quarters of all core evaluations -- is evaluated here, 64 bins per packed
+// instruction) with the term selected to zero where |z|^2 < ql = Z4 a^2; two-term asymptotic rows otherwise (and for
+// the row pairs of a Gauss-Hermite tile that lie wholly beyond the core), zero where |z|^2 < ql = Z2 a^2.
+// Lane pass (lane <-> line, 32 lines at a time) for the bins with q < ql: all lanes step through the SAME bins, each
+// evaluating its own line there; a batch is counting-sorted by y = Gamma_L/alpha_D when it is staged, so the 32 lines
+// of a group have nearly the same centre, Doppler width AND ring boundaries and the lanes run the same evaluator.
+// The 32 x 16 values of a half-row go through a shared staging matrix and are summed per bin (a transpose, no
+// atomics), then added to the warp's bin tile in shared memory.
 constexpr int kSubC = 512;
 constexpr int kLPTC = kSubC / kThreads;
 constexpr int kStage = 16;             // bins per staging step of the core pass
+constexpr int kYClasses = 32;          // classes of y = Gamma_L/alpha_D the lines of a batch are sorted into
+static_assert(kSubC == 32 * 2 * kWarps, "a batch is 2 groups of 32 lines per warp");
+
+// rings of the core evaluator change with y (trapezoid below 5.5, Gauss-Hermite 6 below 8, no core from 25)
+__device__ __forceinline__ int y_class(float y)
+{
+    if (y < 6.0f) return (int)(y * 4.0f);                          // 0..23: class edges at 2 (HK_Y10) and 5.5
+    if (y < 8.0f) return 24 + (int)(y - 6.0f);                     // 24, 25
+    if (y < 25.0f) return 26 + (int)((y - 8.0f) * (5.0f / 17.0f));   // 26..30
+    return 31;
+}
 
 template <int KB>
 __global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
@@ -418,6 +434,7 @@ __global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
     __shared__ float4 smem[2][kSubC];          // A = { -dl, G2, c, 1.5 a2 }, B = { -f, qc, cK, y }
     __shared__ float stage[kWarps][kStage][33];
     __shared__ float sacc[kWarps][kTB];
+    __shared__ int hist[kYClasses];
     __shared__ int s_unit;
     float4* smA = smem[0];
     float4* smB = smem[1];
@@ -476,16 +493,53 @@ __global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
                 if (v < nt) { preA[k] = a.recA[c0 + v]; preB[k] = a.recB[c0 + v]; }
             }
         };
+        // The batch is counting-sorted by y = Gamma_L/alpha_D on its way into shared memory: lines that are neighbours
+        // in centre-bin order have nearly the same centre and Doppler width, so after the sort the 32 lines of a group
+        // also have nearly the same ring boundaries and the lanes of the core pass run the same evaluator.
         auto stash = [&](int v0) {
+            int cls[kLPTC], rk[kLPTC];
+            float yv[kLPTC];
+            if (threadIdx.x < kYClasses) hist[threadIdx.x] = 0;
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < kLPTC; ++k) {
+                const int i = threadIdx.x + k * kThreads;
+                if (v0 + i < nt) {
+                    yv[k] = sqrtf(preA[k].z) * rsqrtf(preB[k].x);
+                    cls[k] = y_class(yv[k]);
+                    rk[k] = atomicAdd(&hist[cls[k]], 1);
+                }
+            }
+            __syncthreads();
+            if (warp == 0) {
+                const int cnt = hist[lane];
+                int inc = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int up = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += up;
+                }
+                hist[lane] = inc - cnt;
+            }
+            __syncthreads();
 #pragma unroll
             for (int k = 0; k < kLPTC; ++k) {
                 const int i = threadIdx.x + k * kThreads;
                 if (v0 + i < nt) {
                     const float4 ra = preA[k], rb = preB[k];
+                    const int dst = hist[cls[k]] + rk[k];
                     const float fdj = (float)((int64_t)__float_as_int(ra.x) - ct0);
                     const float G2 = ra.z, a2 = rb.x;
-                    smA[i] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
-                    smB[i] = make_float4(-ra.y, HK_Z2 * a2, rb.w, sqrtf(G2) * rsqrtf(a2));
+                    // smallest and largest q = t^2 + G2 over the tile's bins (from below / from above)
+                    const float pos = fdj + ra.y;
+                    const float dmin = fmaxf(fmaxf(-pos, pos - whi), 0.f) * 0.999f;
+                    const float dmax = fmaxf(fabsf(pos), fabsf(whi - pos)) * 1.001f;
+                    const float qmin = fmaf(dmin, dmin, G2) * 0.9999f, qmax = fmaf(dmax, dmax, G2);
+                    const float qc = (HK_Z2 / 1.5f) * (1.5f * a2);            // as the row pass recomputes it
+                    // Gauss-Hermite rows: the tile holds core bins and (D1 D2 ~ |z|^8) stays inside fp32
+                    const float ql = (qmin < qc && qmax <= 1.0e9f * a2) ? HK_Z4 * a2 : qc;
+                    smA[dst] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
+                    smB[dst] = make_float4(-ra.y, ql, rb.w, yv[k]);
                 }
             }
         };
@@ -495,47 +549,93 @@ __global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
             stash(v0);
             __syncthreads();
             if (v0 + kSubC < nt) fetch(v0 + kSubC);
-            int wl0, wl1;
-            warp_share(min(kSubC, nt - v0), warp, wl0, wl1);
+            const int nb = min(kSubC, nt - v0);
+            // groups of gs <= 32 sorted lines (every warp gets one when the batch is small); warp w takes groups w and
+            // 15 - w (a cheap high-y group with an expensive low-y one)
+            const int gs = min(32, (nb + kWarps - 1) / kWarps);
+#pragma unroll 1
+            for (int gi = 0; gi < 2; ++gi) {
+            const int grp = gi == 0 ? warp : 2 * kWarps - 1 - warp;
+            const int wl0 = gs * grp, wl1 = min(wl0 + gs, nb);
+            if (wl0 >= wl1) continue;
             // ---- row pass
             int l = wl0;
             while (l < wl1) {
                 const int stop = min(wl1, l + (kFlush - since_flush));
                 since_flush += stop - l;
+#pragma unroll 1
                 for (; l < stop; ++l) {
                     const float4 A = smA[l], B = smB[l];
-                    const float2 ndl = bcast2(A.x), nf = bcast2(B.x), g = bcast2(A.y), c = bcast2(A.z);
-                    const float2 A1 = bcast2(A.w), one = bcast2(1.0f);
-                    const float2 nA2 = bcast2(-1.33333333f * A.w * A.y);
-                    const float qc = B.y;
+                    const float2 ndl = bcast2(A.x), nf = bcast2(B.x), g = bcast2(A.y);
+                    const float qc = (HK_Z2 / 1.5f) * A.w, ql = B.y;
+                    if (ql < qc) {
+                        // Gauss-Hermite 4 in bin units: x^2 = t^2/a^2, s = q/a^2 (hk_device.cuh gh4_K)
+                        constexpr float T1 = 0.27525512860841095f, T2 = 2.7247448713915890f;
+                        constexpr float W1 = 0.5124242247547685f, W2 = 0.05176535879298783f;
+                        const float2 ia2 = bcast2(rcp_approx(A.w * (1.0f / 1.5f))), cky = bcast2(B.z * B.w);
+                        const float2 t1 = bcast2(T1), t2 = bcast2(T2), m1 = bcast2(-4.0f * T1), m2 = bcast2(-4.0f * T2);
+                        const float2 w1 = bcast2(W1), w2 = bcast2(W2);
+                        const float pos = -(A.x + B.x);
 #pragma unroll
-                    for (int m = 0; m < M; ++m) {
-                        const float2 d = __fadd2_rn(tb[m], ndl);         // exact: both are small integers
-                        const float2 t = __fadd2_rn(d, nf);
-                        const float2 q = __ffma2_rn(t, t, g);
-                        const float2 rr = rcp2(q);
-                        const float2 uu = __ffma2_rn(nA2, rr, A1);
-                        const float2 vv = __ffma2_rn(uu, rr, one);
-                        float2 ww = __fmul2_rn(rr, vv);
-                        ww.x = q.x >= qc ? ww.x : 0.f;                  // the core pass owns these bins
-                        ww.y = q.y >= qc ? ww.y : 0.f;
-                        acc[m] = __ffma2_rn(c, ww, acc[m]);
+                        for (int m = 0; m < M; ++m) {
+                            const float2 d = __fadd2_rn(tb[m], ndl);     // exact: both are small integers
+                            const float2 t = __fadd2_rn(d, nf);
+                            const float2 q = __ffma2_rn(t, t, g);
+                            bool far_pair = false;
+                            if (M > 1) {                                 // this pair of rows wholly beyond the core?
+                                const float dist = fmaxf(fmaxf((float)(64 * m) - pos, pos - (float)(64 * m + 63)), 0.f) * 0.999f;
+                                far_pair = fmaf(dist, dist, A.y) * 0.9999f >= qc;
+                            }
+                            if (far_pair) {
+                                const float2 A1 = bcast2(A.w), one = bcast2(1.0f), nA2 = bcast2(-1.33333333f * A.w * A.y);
+                                const float2 rr = rcp2(q);
+                                const float2 uu = __ffma2_rn(nA2, rr, A1);
+                                const float2 vv = __ffma2_rn(uu, rr, one);
+                                acc[m] = __ffma2_rn(bcast2(A.z), __fmul2_rn(rr, vv), acc[m]);
+                            } else {
+                                const float2 x2 = __fmul2_rn(__fmul2_rn(t, t), ia2);
+                                const float2 sz = __fmul2_rn(q, ia2);
+                                const float2 P1 = __fadd2_rn(sz, t1), P2 = __fadd2_rn(sz, t2);
+                                const float2 D1 = __ffma2_rn(P1, P1, __fmul2_rn(m1, x2));
+                                const float2 D2 = __ffma2_rn(P2, P2, __fmul2_rn(m2, x2));
+                                const float2 num = __ffma2_rn(__fmul2_rn(w2, P2), D1, __fmul2_rn(__fmul2_rn(w1, P1), D2));
+                                float2 ww = __fmul2_rn(num, rcp2(__fmul2_rn(D1, D2)));
+                                ww.x = q.x >= ql ? ww.x : 0.f;              // the lane pass owns these bins
+                                ww.y = q.y >= ql ? ww.y : 0.f;
+                                acc[m] = __ffma2_rn(cky, ww, acc[m]);
+                            }
+                        }
+                    } else {
+                        const float2 c = bcast2(A.z), A1 = bcast2(A.w), one = bcast2(1.0f);
+                        const float2 nA2 = bcast2(-1.33333333f * A.w * A.y);
+#pragma unroll
+                        for (int m = 0; m < M; ++m) {
+                            const float2 d = __fadd2_rn(tb[m], ndl);
+                            const float2 t = __fadd2_rn(d, nf);
+                            const float2 q = __ffma2_rn(t, t, g);
+                            const float2 rr = rcp2(q);
+                            const float2 uu = __ffma2_rn(nA2, rr, A1);
+                            const float2 vv = __ffma2_rn(uu, rr, one);
+                            float2 ww = __fmul2_rn(rr, vv);
+                            ww.x = q.x >= ql ? ww.x : 0.f;
+                            ww.y = q.y >= ql ? ww.y : 0.f;
+                            acc[m] = __ffma2_rn(c, ww, acc[m]);
+                        }
                     }
                 }
                 if (since_flush >= kFlush) flush();
             }
-            // ---- core pass
-#pragma unroll 1
-            for (int lb = wl0; lb < wl1; lb += 32) {
-                const int li = lb + lane;
-                float dl = 0.f, f = 0.f, G2 = 1.f, cK = 0.f, qc = 0.f, y = 1.f, inv_a = 1.f;
+            // ---- lane pass: bins with q < ql
+            {
+                const int li = wl0 + lane;
+                float dl = 0.f, f = 0.f, G2 = 1.f, cK = 0.f, ql = 0.f, y = 1.f, inv_a = 1.f;
                 float clo = 1e9f, chi = -1e9f;
                 if (li < wl1) {
                     const float4 A = smA[li], B = smB[li];
-                    dl = -A.x; f = -B.x; G2 = A.y; qc = B.y; cK = B.z; y = B.w;
-                    const float h2 = qc - G2;
+                    dl = -A.x; f = -B.x; G2 = A.y; ql = B.y; cK = B.z; y = B.w;
+                    const float h2 = ql - G2;
                     if (h2 > 0.f) {
-                        const float hw = sqrtf(h2) + 1.0f;                       // |t| < hw covers every q < qc
+                        const float hw = sqrtf(h2) + 1.0f;                       // |t| < hw covers every q < ql
                         const float pos = dl + f;
                         const float lo = fmaxf(ceilf(pos - hw), 0.f), hi = fminf(floorf(pos + hw), whi);
                         if (hi >= lo) { clo = lo; chi = hi; }
@@ -548,33 +648,38 @@ __global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
                     bmin = fminf(bmin, __shfl_xor_sync(0xffffffffu, bmin, o));
                     bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
                 }
-                if (bmax < bmin) continue;
-                const int b_end = (int)bmax;
-                const int col = lane & (kStage - 1), half = lane >> 4;
+                if (bmax >= bmin) {
+                    const int b_end = (int)bmax;
+                    const int col = lane & (kStage - 1), half = lane >> 4;
 #pragma unroll 1
-                for (int b0 = ((int)bmin) & ~(kStage - 1); b0 <= b_end; b0 += kStage) {
-#pragma unroll 1
-                    for (int s = 0; s < kStage; ++s) {
-                        const float fb = (float)(b0 + s);
-                        float val = 0.f;
-                        if (fb >= clo && fb <= chi) {
-                            const float t = (fb - dl) - f;
-                            const float q = fmaf(t, t, G2);
-                            if (q < qc) val = cK * core_any_K(fabsf(t) * inv_a, y, nullptr);
-                        }
-                        stage[warp][s][lane] = val;
-                    }
-                    __syncwarp();
-                    float sum = 0.f;
+                    for (int b0 = (int)bmin; b0 <= b_end; b0 += kStage) {
+                        const int ns = min(kStage, b_end - b0 + 1);              // steps of this block (warp-uniform)
+                        const float e0 = (float)b0 - dl;                         // exact (small integers)
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) sum += stage[warp][col][half * 16 + j];
-                    sum += __shfl_xor_sync(0xffffffffu, sum, 16);
-                    if (half == 0 && b0 + col < kTB) sacc[warp][b0 + col] += sum;
-                    __syncwarp();
+                        for (int s = 0; s < kStage; ++s) {
+                            if (s < ns) {
+                                const float t = (e0 + (float)s) - f;             // the row pass's t, bit for bit
+                                const float q = fmaf(t, t, G2);
+                                float val = 0.f;
+                                if (q < ql) val = cK * core_any_K(fabsf(t) * inv_a, y, nullptr);
+                                stage[warp][s][lane] = val;
+                            }
+                        }
+                        __syncwarp();
+                        float sum = 0.f;
+                        if (col < ns) {
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) sum += stage[warp][col][half * 16 + j];
+                        }
+                        sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+                        if (half == 0 && col < ns) sacc[warp][b0 + col] += sum;
+                        __syncwarp();
+                    }
+                    since_flush += 32;     // the bin tile holds at most 32 lines' terms per bin per batch
+                    if (since_flush >= kFlush) flush();
                 }
-                since_flush += 32;     // the bin tile holds at most 32 lines' terms per bin per batch
-                if (since_flush >= kFlush) flush();
             }
+            }   // groups
         }
         flush();
         __syncthreads();               // every warp is done with the staging buffers: red may overwrite them
@@ -835,7 +940,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
 // positions and kP partial sums in registers; two nodes share one reciprocal.  The partial sums are
 // combined with warp shuffles, then across warps, and reach the (level, tile) node sums with one
 // fp64 atomic per node per work unit.  Formula: two asymptotic terms (valid: |z|^2 >= Z2 on the tile).
-__global__ void __launch_bounds__(kThreads, 2) node_kernel(AccArgs a)
+__global__ void __launch_bounds__(kThreads, 4) node_kernel(AccArgs a)
 {
     constexpr int M = kP / 2;
     __shared__ float red[kWarps][kP];

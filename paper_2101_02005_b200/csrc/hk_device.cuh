@@ -142,6 +142,26 @@ __device__ __forceinline__ float gh6_K(float x2, float s, float y)
     return y * num * rcp_approx(D12 * D3);
 }
 
+// 10-point rule for the innermost region when the pole is far enough from the real axis: for y >= 2 the quadrature
+// converges on all of |z|^2 < HK_Z3 (measured in fp32 against the oracle: <= 2.7e-6), at a quarter of the cost of
+// the trapezoid evaluator with its pole term.
+#define HK_Y10 2.0f
+__device__ __forceinline__ float gh10_K(float x2, float s, float y)
+{
+    constexpr float T1 = 0.11758132021177813f, T2 = 1.074562012436904f, T3 = 3.0859374437175497f,
+                    T4 = 6.41472973366203f, T5 = 11.807189489971735f;                       // t_k^2
+    constexpr float W1 = 0.38888723083644433f, W2 = 0.15287698792389035f, W3 = 0.02156510928733804f,
+                    W4 = 0.0008553914494585371f, W5 = 4.864050625087994e-06f;               // 2 w_k / pi
+    const float A1 = s + T1, A2 = s + T2, A3 = s + T3, A4 = s + T4, A5 = s + T5;
+    const float D1 = fmaf(A1, A1, (-4.0f * T1) * x2), D2 = fmaf(A2, A2, (-4.0f * T2) * x2),
+                D3 = fmaf(A3, A3, (-4.0f * T3) * x2), D4 = fmaf(A4, A4, (-4.0f * T4) * x2),
+                D5 = fmaf(A5, A5, (-4.0f * T5) * x2);
+    float sum = fmaf(W2 * A2, D1, (W1 * A1) * D2) * rcp_approx(D1 * D2);
+    sum = fmaf(fmaf(W4 * A4, D3, (W3 * A3) * D4), rcp_approx(D3 * D4), sum);
+    sum = fmaf(W5 * A5, rcp_approx(D5), sum);
+    return y * sum;
+}
+
 // |z|^2 below which the trapezoid evaluator is used, as a function of y^2
 __device__ __forceinline__ float z3_for(float y2) { return y2 < 1e-6f ? 50.0f : HK_Z3; }
 
@@ -214,6 +234,7 @@ __device__ __forceinline__ float core_any_K(float x, float y, int* region)
     const float x2 = x * x, y2 = y * y, s = x2 + y2;
     if (s >= HK_Z4) { if (region) *region = 2; return gh4_K(x2, s, y); }
     if (s >= z3_for(y2)) { if (region) *region = 3; return gh6_K(x2, s, y); }
+    if (y >= HK_Y10) { if (region) *region = 5; return gh10_K(x2, s, y); }
     if (region) *region = 4;
     return core_K(x, y);
 }

@@ -343,7 +343,7 @@ def test_evaluator_accuracy_map(B):
     ref = O.voigt_K(x32.astype(np.float64), y32.astype(np.float64))
     ok = ref > 1e-30                     # below that the term is far under any bin's tolerance
     rel = np.abs(got - ref) / np.maximum(ref, 1e-300)
-    for r, name in enumerate(("far", "mid", "gauss-hermite 4", "gauss-hermite 6", "trapezoid")):
+    for r, name in enumerate(("far", "mid", "gauss-hermite 4", "gauss-hermite 6", "trapezoid", "gauss-hermite 10")):
         m = ok & (reg == r)
         assert m.any()
         worst = rel[m].max()
