@@ -413,6 +413,7 @@ __global__ void __launch_bounds__(kThreads, 2) edge_kernel(AccArgs a)
 constexpr int kSubC = 512;
 constexpr int kLPTC = kSubC / kThreads;
 constexpr int kStage = 16;             // bins per staging step of the core pass
+constexpr int kCentreCtas = 4;         // resident CTAs per SM the centre kernel is compiled and launched for
 constexpr int kYClasses = 32;          // classes of y = Gamma_L/alpha_D the lines of a batch are sorted into
 static_assert(kSubC == 32 * 2 * kWarps, "a batch is 2 groups of 32 lines per warp");
 
@@ -426,7 +427,7 @@ __device__ __forceinline__ int y_class(float y)
 }
 
 template <int KB>
-__global__ void __launch_bounds__(kThreads, 2) centre_kernel(AccArgs a)
+__global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a)
 {
     constexpr int kTB = 32 * KB;
     constexpr int M = KB / 2;

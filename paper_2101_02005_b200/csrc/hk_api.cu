@@ -75,11 +75,9 @@ constexpr int kMinKB = 2;     // smallest tile geometry: the workspace is sized 
 int pick_kb(const hk_ctx* c, double cut)
 {
     if (c->force_kb) return c->force_kb;
-    if (is_uncut(cut)) return 8;
-    const double cb = cut / c->dnu;
-    if (cb >= 4096.0) return 8;
-    if (cb >= 1024.0) return 4;
-    return 2;
+    // measured (profiles/): with the node hierarchy taking every separated tile, small level-0 tiles win whenever
+    // there is a cut (fewer direct near-field pairs, smaller edge tiles); uncut lists are sparse and favour wide tiles
+    return is_uncut(cut) ? 8 : 2;
 }
 
 Layout make_layout(const hk_ctx* c, int64_t n)
@@ -430,7 +428,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
         if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
-        if (p.mode == 0 || p.mode == 3) { centre_kernel<KB><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        if (p.mode == 0 || p.mode == 3) { centre_kernel<KB><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
         near_kernel<KB><<<grid, kThreads, 0, stream>>>(a);
         ++ctx->last_launches;
