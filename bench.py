@@ -33,7 +33,9 @@ from workload import linelists as W
 METRIC = "lines_per_s"
 UNIT = "lines/s"
 FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM (4 SMSPs x 32), DESIGN.md section 7
-FLOP_PER_EVAL = {"far": 6.0, "mid": 12.0}   # algorithmic FLOPs per Voigt evaluation
+# algorithmic FLOPs per Voigt evaluation by formula (FMA = 2, add/mul/reciprocal = 1):
+# far 1 term, mid 2 terms, 4/6/10-point Gauss-Hermite rational forms, trapezoid rule with pole term
+FLOP = {"far": 6.0, "mid": 12.0, "gh4": 24.0, "gh6": 36.0, "gh10": 52.0, "trap": 125.0}
 
 
 def _workload_name(cfg, n):
@@ -311,18 +313,38 @@ def run_ours(args):
     sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0)
     peak_nominal = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12     # TFLOP/s
     probe_flops, _ = B.probe_fp32_peak(packed=True, iters=20000)
-    # dominant kernel: the far-wing accumulation kernel
-    far_ms = phases["far"]
-    far_flops = FLOP_PER_EVAL["far"] * st["n_pairs_far"]
-    achieved = far_flops / (far_ms * 1e-3) / 1e12 if far_ms > 0 else 0.0
-    roofline = {"bound": "alu", "kernel": f"interior_kernel<{st['bins_per_lane']},false> (far wing)", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+    # per accumulation kernel: algorithmic FLOPs (FLOPs of the formula evaluated, per evaluation the
+    # definition or the node scheme requires; masked-out slots and idle lanes count nothing) / CUDA-event time
+    core = st["n_evals_core"]
+    n_gh4 = core - st["n_evals_gh6"] - st["n_evals_trap"]
+    n_trap = st["n_evals_trap"] - st["n_evals_gh10"]
+    kb = st["bins_per_lane"]
+    kflops = {
+        "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * 8),
+        "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
+        "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
+        "edge": (f"edge_kernel<{kb}>", FLOP["mid"] * 0.5 * st["n_pairs_edge"]),      # half of an edge tile is inside the extent
+        "centre": (f"centre_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
+                   + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * st["n_evals_gh10"] + FLOP["trap"] * n_trap),
+    }
+    kernels = {}
+    for ph, (name, fl) in kflops.items():
+        ms = phases[ph]
+        kernels[ph] = {"kernel": name, "ms": ms, "algorithmic_gflop": fl / 1e9,
+                       "tflops": fl / (ms * 1e-3) / 1e12 if ms > 0 else 0.0,
+                       "frac_of_nominal": (fl / (ms * 1e-3) / 1e12 / peak_nominal) if ms > 0 else 0.0}
+    dom = max(kflops, key=lambda k: phases[k])
+    achieved = kernels[dom]["tflops"]
+    acc_ms = sum(phases[k] for k in kflops)
+    acc_fl = sum(fl for _, fl in kflops.values())
+    roofline = {"bound": "alu", "kernel": kernels[dom]["kernel"], "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                 "frac": achieved / peak_nominal if peak_nominal else None, "traffic": None,
                 "peak_kind": f"nominal FP32: {n_sm} SMs x {FP32_LANES_PER_SM} lanes x 2 FLOP x {sm_max:g} MHz (DESIGN.md 7)",
                 "peak_probe_ffma2": probe_flops / 1e12, "frac_of_probe": achieved / (probe_flops / 1e12),
-                "flop_per_eval": FLOP_PER_EVAL["far"], "evals_per_launch": st["n_pairs_far"], "ms_per_launch": far_ms,
-                "evals_per_s": st["n_pairs_far"] / (far_ms * 1e-3) if far_ms > 0 else 0.0,
-                "evals_per_clk_per_sm": (st["n_pairs_far"] / (far_ms * 1e-3) / n_sm / ((clocks or {}).get("sm_mhz") or sm_max) / 1e6)
-                if far_ms > 0 else 0.0,
+                "ms_per_launch": phases[dom], "share_of_step": phases[dom] / (total_ms / args.steps),
+                "flop_per_eval": FLOP, "kernels": kernels,
+                "all_accumulation_kernels": {"ms": acc_ms, "tflops": acc_fl / (acc_ms * 1e-3) / 1e12 if acc_ms > 0 else 0.0,
+                                             "frac_of_nominal": acc_fl / (acc_ms * 1e-3) / 1e12 / peak_nominal if acc_ms > 0 else 0.0},
                 "hbm_preprocess_gbs": (input_bytes + 40.0 * n) / (phases["preprocess"] * 1e-3) / 1e9 if phases["preprocess"] > 0 else None,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_kind": peaks_kind}
 

@@ -79,6 +79,7 @@ typedef struct {
     int64_t n_pairs_centre; /* (line, bin) slots the centre kernel walked (two-term outside the core, core evaluators inside) */
     int64_t n_pairs_node;  /* (line, tile) pairs evaluated at the tile's HK_NODES Chebyshev nodes (two-term asymptotic) */
     int64_t n_bins_node;   /* (line, bin) pairs those node evaluations stand for */
+    int64_t n_evals_gh10;  /* of n_evals_trap: lines with y >= 2, evaluated by the 10-point Gauss-Hermite rule */
     int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
     int32_t sort_bits;     /* radix-sort key width used */

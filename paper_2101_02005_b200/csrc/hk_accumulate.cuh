@@ -271,7 +271,7 @@ constexpr int kSubE = 512;
 constexpr int kLPTE = kSubE / kThreads;
 
 template <int KB>
-__global__ void __launch_bounds__(kThreads, 2) edge_kernel(AccArgs a)
+__global__ void __launch_bounds__(kThreads, 4) edge_kernel(AccArgs a)
 {
     constexpr int kTB = 32 * KB;
     constexpr int M = KB / 2;

@@ -426,7 +426,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream);
         if (p.mode != 1) { interior_kernel<KB, true><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
-        if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<ctx->n_sm * 4, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
         if (p.mode == 0 || p.mode == 3) { centre_kernel<KB><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
@@ -623,6 +623,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_evals_core = (int64_t)d.n_cnt_core;
     host_out->n_evals_gh6 = (int64_t)(d.n_cnt_gh6 - d.n_cnt_trap);
     host_out->n_evals_trap = (int64_t)d.n_cnt_trap;
+    host_out->n_evals_gh10 = (int64_t)d.n_cnt_gh10;
     host_out->n_units_far = (int64_t)d.units_far;
     host_out->n_units_mid = (int64_t)d.units_mid;
     host_out->n_units_near = (int64_t)d.units_near;

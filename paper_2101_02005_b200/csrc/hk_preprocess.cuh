@@ -41,6 +41,7 @@ struct Params {
 struct DevStats {
     unsigned long long n_skipped, n_off_grid, n_evals, n_cnt_mid, n_cnt_core;  // cnt_*: evals with |z|^2 below Z1 / Z2
     unsigned long long n_cnt_gh6, n_cnt_trap;                                  // ... below Z4 / Z3
+    unsigned long long n_cnt_gh10;                                             // of n_cnt_trap: lines with y >= HK_Y10
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
     int32_t pad;
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
                                                    int32_t* __restrict__ key, int32_t* __restrict__ idx,
                                                    DevStats* __restrict__ st)
 {
-    unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cgh6 = 0, ctrap = 0, cmaxb = 0, cKmaxb = 0;
+    unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cgh6 = 0, ctrap = 0, cgh10 = 0, cmaxb = 0, cKmaxb = 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         LineOut o = line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
         RecU r;
@@ -152,33 +153,35 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
             const double y2 = (Gb * Gb) / (ab * ab);
             const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
             cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? sqrt(t4) : 0.0, o.ilo, o.ihi);
-            ctrap += (unsigned long long)count_within(pos, t3 > 0 ? sqrt(t3) : 0.0, o.ilo, o.ihi);
+            const unsigned long long ntrap = (unsigned long long)count_within(pos, t3 > 0 ? sqrt(t3) : 0.0, o.ilo, o.ihi);
+            ctrap += ntrap;
+            if (y2 >= (double)(HK_Y10 * HK_Y10)) cgh10 += ntrap;
         }
         rec[i] = r;
         key[i] = k;
         idx[i] = (int32_t)i;
     }
     // block reduction of the counters
-    __shared__ unsigned long long sh[9][8];
-    unsigned long long v[9] = {skipped, off, evals, cmid, ccore, cgh6, ctrap, cmaxb, cKmaxb};
+    __shared__ unsigned long long sh[10][8];
+    unsigned long long v[10] = {skipped, off, evals, cmid, ccore, cgh6, ctrap, cgh10, cmaxb, cKmaxb};
 #pragma unroll
-    for (int q = 0; q < 9; ++q) {
+    for (int q = 0; q < 10; ++q) {
         unsigned long long x = v[q];
         for (int o = 16; o > 0; o >>= 1) {
             unsigned long long y = __shfl_xor_sync(0xffffffffu, x, o);
-            x = (q < 7) ? x + y : max(x, y);
+            x = (q < 8) ? x + y : max(x, y);
         }
         if ((threadIdx.x & 31) == 0) sh[q][threadIdx.x >> 5] = x;
     }
     __syncthreads();
-    if (threadIdx.x < 9) {
+    if (threadIdx.x < 10) {
         int q = threadIdx.x;
         unsigned long long x = sh[q][0];
-        for (int w = 1; w < 8; ++w) x = (q < 7) ? x + sh[q][w] : max(x, sh[q][w]);
+        for (int w = 1; w < 8; ++w) x = (q < 8) ? x + sh[q][w] : max(x, sh[q][w]);
         unsigned long long* dst = q == 0 ? &st->n_skipped : q == 1 ? &st->n_off_grid : q == 2 ? &st->n_evals
                                 : q == 3 ? &st->n_cnt_mid : q == 4 ? &st->n_cnt_core : q == 5 ? &st->n_cnt_gh6
-                                : q == 6 ? &st->n_cnt_trap : q == 7 ? &st->cmax_bits : &st->cKmax_bits;
-        if (q < 7) { if (x) atomicAdd(dst, x); }
+                                : q == 6 ? &st->n_cnt_trap : q == 7 ? &st->n_cnt_gh10 : q == 8 ? &st->cmax_bits : &st->cKmax_bits;
+        if (q < 8) { if (x) atomicAdd(dst, x); }
         else atomicMax(dst, x);
     }
 }
