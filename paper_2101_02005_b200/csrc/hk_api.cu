@@ -132,6 +132,7 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
     const double m = c->mass_amu / kNA;                        // grams (L83)
     p.c2_over_T = kH * kC / kKB / c->T;
     p.tfac = kTref / c->T;
+    p.ln_tfac = std::log(p.tfac);
     p.P_atm = c->P_atm;
     p.beta = std::sqrt(2.0 * kKB * c->T / m) / kC;
     p.sfac = 1.0 / (8.0 * kPi * kC * m * c->Q);

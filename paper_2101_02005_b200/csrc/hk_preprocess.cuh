@@ -15,6 +15,7 @@ struct Params {
     // conditions folded into constants (host, fp64)
     double c2_over_T;     // h c / (k_B T)
     double tfac;          // T_ref / T
+    double ln_tfac;       // ln(T_ref / T)
     double P_atm;
     double beta;          // sqrt(2 k_B T / m) / c     (alpha_D = beta nu0)
     double sfac;          // 1 / (8 pi c m Q)
@@ -79,7 +80,7 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
     o.jc = 0; o.ilo = 0; o.ihi = -1; o.pos_f = 0.0;
     if (!o.valid) return o;
     o.alphaD = p.beta * nu0;                                                   // Eq. 13 (L203)
-    o.gammaL = A * p.inv4pic + gam * pow(p.tfac, nx) * p.P_atm;                // Eq. 5 (L91)
+    o.gammaL = A * p.inv4pic + gam * exp(nx * p.ln_tfac) * p.P_atm;            // Eq. 5 (L91): (T_ref/T)^n = e^(n ln(T_ref/T))
     o.S = A * g * p.sfac / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));  // Eq. 9 (L127)
     const double big = 4.0e18;
     double pos = __ddiv_rn(__dsub_rn(nu0, p.numin), p.dnu);
@@ -148,12 +149,12 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
             evals += (unsigned long long)(o.ihi - o.ilo + 1);
             double pos = (double)o.jc + o.pos_f;
             double t1 = (double)HK_Z1 * ab * ab - Gb * Gb, t2 = (double)HK_Z2 * ab * ab - Gb * Gb;
-            cmid += (unsigned long long)count_within(pos, t1 > 0 ? sqrt(t1) : 0.0, o.ilo, o.ihi);
-            ccore += (unsigned long long)count_within(pos, t2 > 0 ? sqrt(t2) : 0.0, o.ilo, o.ihi);
+            cmid += (unsigned long long)count_within(pos, t1 > 0 ? (double)sqrtf((float)t1) : 0.0, o.ilo, o.ihi);
+            ccore += (unsigned long long)count_within(pos, t2 > 0 ? (double)sqrtf((float)t2) : 0.0, o.ilo, o.ihi);
             const double y2 = (Gb * Gb) / (ab * ab);
             const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
-            cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? sqrt(t4) : 0.0, o.ilo, o.ihi);
-            const unsigned long long ntrap = (unsigned long long)count_within(pos, t3 > 0 ? sqrt(t3) : 0.0, o.ilo, o.ihi);
+            cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? (double)sqrtf((float)t4) : 0.0, o.ilo, o.ihi);
+            const unsigned long long ntrap = (unsigned long long)count_within(pos, t3 > 0 ? (double)sqrtf((float)t3) : 0.0, o.ilo, o.ihi);
             ctrap += ntrap;
             if (y2 >= (double)(HK_Y10 * HK_Y10)) cgh10 += ntrap;
         }
