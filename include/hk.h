@@ -128,6 +128,17 @@ int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_c
 int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
                   double* out_k_dev, void* stream);
 
+/* Many (T, P, Q) points on one resident line list in one call (the paper's "multiple pressure points per run",
+ * L361, L733, Table 8: the lines stay on the GPU across the points).  T_K, P_atm, Q: HOST arrays of n_cond
+ * values (the mass of hk_set_conditions applies to all; hk_set_conditions must have been called and its T, P, Q are
+ * left untouched).  out_k_dev: DEVICE array of n_cond x N doubles, row c = k(nu) at condition c, OVERWRITTEN.
+ * Every point is the full definition of hk_compute at that condition; what is shared is what does not depend on the
+ * condition: the order of the lines by centre bin (one sort for the batch) and the workspace.  All conditions are
+ * validated before anything is enqueued (HK_EINVAL as hk_set_conditions).  n_cond == 0 is valid.  Asynchronous like
+ * hk_compute.  hk_get_stats afterwards describes the LAST condition, n_launches the whole batch. */
+int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond,
+                     const double* T_K, const double* P_atm, const double* Q, double* out_k_dev, void* stream);
+
 /* Host-buffer entry (the paper's block pipeline, L183-189, Fig. 6): the six line
  * arrays and out_k are HOST pointers (pinned memory gives asynchronous copies; pageable
  * works, slower).  The list is cut into blocks of block_lines lines (<= 0: default 2^25);

@@ -24,7 +24,7 @@ HK_Z1, HK_Z2, HK_Z4, HK_Z3 = 90000.0, 625.0, 64.0, 30.25
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
-           "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_workspace_bytes_host", "hk_compute_host",
+           "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation",
            "hk_last_cuda_error", "hk_strerror")
@@ -55,6 +55,9 @@ _lib.hk_workspace_bytes.restype = C.c_size_t
 _lib.hk_set_workspace.argtypes = [_vp, _vp, C.c_size_t]
 _lib.hk_compute.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
 _lib.hk_accumulate.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
+_lib.hk_compute_batch.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, C.c_int32, C.POINTER(_d), C.POINTER(_d), C.POINTER(_d),
+                                  _vp, _vp]
+_lib.hk_compute_batch.restype = C.c_int
 _lib.hk_workspace_bytes_host.argtypes = [_vp, _i64, _i64]
 _lib.hk_workspace_bytes_host.restype = C.c_size_t
 _lib.hk_compute_host.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _i64, _vp]
@@ -166,6 +169,21 @@ class Opacity:
         cut = float(cut) if cut is not None else 0.0
         fn = _lib.hk_accumulate if accumulate else _lib.hk_compute
         self._check(fn(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)), "hk_compute")
+        return out
+
+    def compute_batch(self, lines, cut, T, P_atm, Q, out=None, stream=None):
+        """hk_compute_batch: k(nu) at every (T[c], P_atm[c], Q[c]) on the resident lines -> [n_cond, N] fp64 CUDA tensor."""
+        ls, n = _lines_struct(lines)
+        self.ensure_workspace(n)
+        nc = len(T)
+        assert len(P_atm) == nc and len(Q) == nc
+        if out is None:
+            out = torch.empty((nc, self.N), dtype=torch.float64, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == nc * self.N
+        arr = lambda v: (_d * nc)(*[float(x) for x in v])
+        cut = float(cut) if cut is not None else 0.0
+        self._check(_lib.hk_compute_batch(self._ctx, C.byref(ls), n, cut, nc, arr(T), arr(P_atm), arr(Q), out.data_ptr(),
+                                          _stream_ptr(stream)), "hk_compute_batch")
         return out
 
     def compute_host(self, host_lines, cut, out=None, block_lines=0, stream=None):

@@ -331,7 +331,7 @@ int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane)
 }
 
 static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
-                        cudaStream_t stream, bool zero_out)
+                        cudaStream_t stream, bool zero_out, bool reuse_sort = false)
 {
     if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL) return HK_EINVAL;
     if (std::isnan(cut_cm)) return HK_EINVAL;
@@ -386,8 +386,10 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     const int bits = bits_for((uint32_t)p.ksent);
     ctx->last_sort_bits = bits;
     size_t cub_bytes = L.cub_bytes;
-    HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
-                                            (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
+    // the order by centre bin does not depend on (T, P, Q): later conditions of a batch reuse it (hk_compute_batch)
+    if (!reuse_sort)
+        HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
+                                                (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
     gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB, recN);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges, node ranges and work units.  counts = [far | mid | edge | centre | near | node | 0], one scan.
@@ -461,6 +463,29 @@ int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_c
 int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
 {
     return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, false);
+}
+
+int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond, const double* T_K,
+                     const double* P_atm, const double* Q, double* out_k_dev, void* stream_v)
+{
+    if (!ctx || n_cond < 0 || (n_cond > 0 && (!T_K || !P_atm || !Q || !out_k_dev))) return HK_EINVAL;
+    if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
+    for (int32_t c = 0; c < n_cond; ++c) {          // validate everything before enqueueing anything
+        if (!std::isfinite(T_K[c]) || !std::isfinite(P_atm[c]) || !std::isfinite(Q[c])) return HK_EINVAL;
+        if (!(T_K[c] > 0.0) || !(P_atm[c] >= 0.0) || !(Q[c] > 0.0)) return HK_EINVAL;
+    }
+    const double T0 = ctx->T, P0 = ctx->P_atm, Q0 = ctx->Q;
+    int rc = HK_OK;
+    int64_t launches = 0;
+    for (int32_t c = 0; c < n_cond && rc == HK_OK; ++c) {
+        ctx->T = T_K[c]; ctx->P_atm = P_atm[c]; ctx->Q = Q[c];
+        rc = compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev + (size_t)c * (size_t)ctx->N, (cudaStream_t)stream_v, true,
+                          /*reuse_sort=*/c > 0);
+        launches += ctx->last_launches;
+    }
+    ctx->T = T0; ctx->P_atm = P0; ctx->Q = Q0;
+    ctx->last_launches = launches;
+    return rc;
 }
 
 // ---- host-buffer pipeline ---------------------------------------------------------------

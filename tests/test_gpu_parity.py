@@ -176,6 +176,44 @@ def test_host_pipeline_and_accumulate(B):
     op.close()
 
 
+def test_batched_conditions(B):
+    """hk_compute_batch (the paper's many pressure points per run, L361, L733): every row of the
+    batch is the definition at that (T, P, Q) -- checked against the oracle per condition -- and equals the one-shot
+    hk_compute at that condition bit for bit (the shared sort changes no arithmetic)."""
+    lines, cond, grid, cut = _mini(2, 20_000)
+    T = [300.0, 1500.0, 1500.0, 2900.0]
+    P = [1e-3, cond["P_atm"], 25.0, 0.3]
+    Q = [170.0, cond["Q"], cond["Q"], 9000.0]
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    dl = _to_cuda(lines)
+    kb = op.compute_batch(dl, cut, T, P, Q)
+    torch.cuda.synchronize()
+    assert kb.shape == (4, op.N)
+    st = op.stats()
+    for c in range(4):
+        cnd = dict(T=T[c], P_atm=P[c], mass_amu=cond["mass_amu"], Q=Q[c])
+        k_ref, evals = O.opacity_grid(lines, cnd, grid, cut)
+        assert st["n_evals"] == evals
+        check_parity(kb[c].cpu().numpy(), k_ref, what=f"batch condition {c}")
+        op1 = B.Opacity(*grid)
+        op1.set_conditions(T[c], P[c], cond["mass_amu"], Q[c])
+        k1 = op1.compute(dl, cut)
+        torch.cuda.synchronize()
+        big = k_ref >= 1e-8 * k_ref.max()
+        assert np.abs(kb[c].cpu().numpy()[big] / k1.cpu().numpy()[big] - 1.0).max() <= 1e-6   # atomics order only
+        op1.close()
+    # the handle's own conditions are untouched; an empty batch and a bad condition
+    k_after = op.compute(dl, cut)
+    k_ref, _ = O.opacity_grid(lines, cond, grid, cut)
+    check_parity(k_after.cpu().numpy(), k_ref, what="after batch")
+    assert op.compute_batch(dl, cut, [], [], []).shape == (0, op.N)
+    with pytest.raises(B.HKError) as e:
+        op.compute_batch(dl, cut, [300.0, -1.0], [1.0, 1.0], [10.0, 10.0])
+    assert e.value.status == B.HK_EINVAL
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
