@@ -340,7 +340,8 @@ def run_ours(args):
         "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * 8),
         "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
         "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
-        "edge": (f"edge_kernel<{kb}>", FLOP["mid"] * 0.5 * st["n_pairs_edge"]),      # half of an edge tile is inside the extent
+        # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end
+        "edge": (f"edge_kernel<{kb}> + edge_node_kernel", FLOP["mid"] * (0.5 * st["n_pairs_edge"] + 8 * st["n_pairs_edge_node"])),
         "centre": (f"centre_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
                    + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * st["n_evals_gh10"] + FLOP["trap"] * n_trap),
     }
@@ -376,7 +377,7 @@ def run_ours(args):
            "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"],
                                "core_gh6": st["n_evals_gh6"], "core_trap": st["n_evals_trap"]},
            "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
-                               "edge": st["n_pairs_edge"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
+                               "edge": st["n_pairs_edge"], "edge_node_ends": st["n_pairs_edge_node"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
            "bins_per_lane": st["bins_per_lane"],
            "phase_ms": phases, "step_ms": step_ms, "roofline": roofline, "clocks": clocks,
            "gpu_launches": int(st["n_launches"]) * args.steps,

@@ -80,6 +80,7 @@ typedef struct {
     int64_t n_pairs_node;  /* (line, tile) pairs evaluated at the tile's HK_NODES Chebyshev nodes (two-term asymptotic) */
     int64_t n_bins_node;   /* (line, bin) pairs those node evaluations stand for */
     int64_t n_evals_gh10;  /* of n_evals_trap: lines with y >= 2, evaluated by the 10-point Gauss-Hermite rule */
+    int64_t n_pairs_edge_node; /* (line, extent end) pairs evaluated at the nodes of their edge tile (per-bin accumulators) */
     int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
     int32_t sort_bits;     /* radix-sort key width used */
@@ -196,6 +197,9 @@ int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* 
 int hk_set_debug_mode(hk_ctx* ctx, int mode);
 int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane);
 int hk_set_node_separation(hk_ctx* ctx, double sep);
+/* on (default): tiles an extent covers only in part, when separated from the line, are evaluated at the tile's nodes
+ * into per-bin accumulators (128 B per bin of workspace, used while that is <= 1 GiB); off: masked direct evaluation. */
+int hk_set_edge_nodes(hk_ctx* ctx, int on);
 
 int hk_last_cuda_error(const hk_ctx* ctx);
 const char* hk_strerror(int status);

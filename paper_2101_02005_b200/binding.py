@@ -26,7 +26,7 @@ FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
-           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation",
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes",
            "hk_last_cuda_error", "hk_strerror")
 PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "near", "down")
 
@@ -40,7 +40,7 @@ class hk_stats(C.Structure):
                                          "n_evals_mid", "n_evals_core", "n_evals_gh6", "n_evals_trap", "n_units_far", "n_units_mid", "n_units_near",
                                          "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_units_edge",
                                          "n_units_centre", "n_pairs_edge", "n_pairs_centre", "n_pairs_node",
-                                         "n_bins_node", "n_evals_gh10", "n_launches")] + \
+                                         "n_bins_node", "n_evals_gh10", "n_pairs_edge_node", "n_launches")] + \
                [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("n_levels", C.c_int32)]
 
 
@@ -71,6 +71,8 @@ _lib.hk_set_debug_mode.argtypes = [_vp, C.c_int]
 _lib.hk_set_tile_bins.argtypes = [_vp, C.c_int]
 _lib.hk_set_node_separation.argtypes = [_vp, _d]
 _lib.hk_set_node_separation.restype = C.c_int
+_lib.hk_set_edge_nodes.argtypes = [_vp, C.c_int]
+_lib.hk_set_edge_nodes.restype = C.c_int
 _lib.hk_last_cuda_error.argtypes = [_vp]
 _lib.hk_strerror.argtypes = [C.c_int]
 _lib.hk_strerror.restype = C.c_char_p
@@ -145,6 +147,9 @@ class Opacity:
 
     def set_node_separation(self, sep: float):
         self._check(_lib.hk_set_node_separation(self._ctx, sep), "hk_set_node_separation")
+
+    def set_edge_nodes(self, on: bool):
+        self._check(_lib.hk_set_edge_nodes(self._ctx, 1 if on else 0), "hk_set_edge_nodes")
 
     def workspace_bytes(self, n_lines: int) -> int:
         return int(_lib.hk_workspace_bytes(self._ctx, n_lines))

@@ -48,6 +48,7 @@ struct AccArgs {
     DevStats* st;
     double* __restrict__ out_k;
     double* __restrict__ node_acc;             // n_entries x kP node sums (scaled), fp64
+    double* __restrict__ edge_acc;             // [2][N][kP] per-bin node sums of extent ends (scaled), fp64; or null
     int64_t N;
     int32_t n_ct, chunk, chunk_node;
     Levels lv;
@@ -1016,6 +1017,126 @@ __global__ void __launch_bounds__(kThreads, 4) node_kernel(AccArgs a)
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// edge-node kernel: extent ends in separated tiles, evaluated at the tile's kP nodes (edge_keys, hk_preprocess.cuh)
+// ---------------------------------------------------------------------------------------
+// Lanes walk the sorted LINES.  For each end of its extent a lane finds the level-0 tile the end falls in, evaluates
+// its line at that tile's nodes (two-term asymptotic, as node_kernel) and adds the kP values to the accumulators of
+// the bin where the extent ends: side 0 = last bin ihi (the line covers the bins <= ihi of the tile), side 1 = first
+// bin ilo (bins >= ilo).  Neighbouring lines end in the same few bins, so equal bins are summed in the warp first and
+// one lane issues the fp64 atomics.  edge_scan_kernel turns the accumulators into suffix (side 0) / prefix (side 1)
+// sums over each tile, edge_bins_kernel interpolates them onto the bins.  The sum of interpolants over any subset of
+// lines is the interpolant of that subset's node sums, so the per-bin subsets cost nothing extra.
+__device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_t bin, const float (&v)[kP], int lane)
+{
+    unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int64_t b = __shfl_sync(0xffffffffu, bin, leader);
+        const bool mine = (bin == b);
+        const unsigned grp = __ballot_sync(0xffffffffu, mine);
+        if (__popc(grp) == 1) {
+            if (mine) {
+#pragma unroll
+                for (int j = 0; j < kP; ++j) atomicAdd(acc + (size_t)b * kP + j, (double)v[j]);
+            }
+        } else {
+            // every lane ends up with all kP sums; lanes 0..kP-1 then issue ONE atomic each, to consecutive addresses
+            float out = 0.f;
+#pragma unroll
+            for (int j = 0; j < kP; ++j) {
+                float sum = mine ? v[j] : 0.f;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+                if (lane == j) out = sum;
+            }
+            if (lane < kP) atomicAdd(acc + (size_t)b * kP + lane, (double)out);
+        }
+        todo &= ~grp;
+    }
+}
+
+__global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys,
+                                                                 int32_t n)
+{
+    constexpr int M = kP / 2;
+    __shared__ int32_t s_nact;
+    if (threadIdx.x == 0) s_nact = lower_bound_key(keys, n, (int64_t)p.ksent);
+    __syncthreads();
+    const int32_t n_act = s_nact;
+    const int lane = threadIdx.x & 31;
+    const int64_t W = a.lv.w0;
+    float2 xk[M];
+    const double hc = 0.5 * (double)(W - 1), hw = 0.5 * (double)W;
+#pragma unroll
+    for (int m = 0; m < M; ++m) xk[m] = make_float2((float)(hc + hw * kChebX[2 * m]), (float)(hc + hw * kChebX[2 * m + 1]));
+    unsigned long long npairs = 0;
+    const int64_t n_round = ((int64_t)n_act + 31) & ~31LL;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+        const bool live = i < n_act;
+        float4 rn = make_float4(0.f, 0.f, 1.f, 0.f), rb = make_float4(1.f, 0.f, __int_as_float(-1), 0.f);
+        if (live) { rn = a.recN[i]; rb = a.recB[i]; }
+        const int64_t jc = __float_as_int(rn.x), ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);
+        const uint32_t pk = (uint32_t)__float_as_int(rn.y);
+        const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
+        const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
+        const float2 g2 = bcast2(rn.z), c2 = bcast2(rn.w), one = bcast2(1.0f);
+        const float2 A1 = bcast2(1.5f * a2), nA2 = bcast2(-2.0f * a2 * rn.z);
+#pragma unroll 1
+        for (int side = 0; side < 2; ++side) {
+            const int64_t e = side == 0 ? ihi : ilo;
+            bool m = live && ihi >= ilo;
+            const int64_t T0 = m ? (e / W) * W : 0;
+            if (m) {
+                const EdgeKeys k = edge_keys(p, T0, W);
+                m = side == 0 ? (jc <= k.upL) : (jc >= k.dnR);
+            }
+            float v[kP];
+#pragma unroll
+            for (int j = 0; j < kP; ++j) v[j] = 0.f;
+            if (m) {
+                ++npairs;
+                const float2 np2 = bcast2(-((float)(jc - T0) + f));
+#pragma unroll
+                for (int mm = 0; mm < M; ++mm) {
+                    const float2 t = __fadd2_rn(xk[mm], np2);
+                    const float2 q = __ffma2_rn(t, t, g2);
+                    const float R = rcp_approx(q.x * q.y);
+                    const float2 rr = make_float2(R * q.y, R * q.x);
+                    const float2 uu = __ffma2_rn(nA2, rr, A1);
+                    const float2 vv = __ffma2_rn(uu, rr, one);
+                    const float2 ww = __fmul2_rn(c2, __fmul2_rn(rr, vv));
+                    v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                }
+            }
+            warp_add_by_bin(a.edge_acc + (size_t)side * (size_t)a.N * kP, m ? e : -1, v, lane);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) npairs += __shfl_xor_sync(0xffffffffu, npairs, o);
+    if (lane == 0 && npairs) atomicAdd(&a.st->pairs_edge_node, npairs);
+}
+
+// in place: side 0 -> suffix sums over each tile (bins <= the end bin), side 1 -> prefix sums (bins >= the start bin)
+__global__ void __launch_bounds__(256) edge_scan_kernel(AccArgs a)
+{
+    const int64_t W = a.lv.w0;
+    const int64_t n_tiles = (a.N + W - 1) / W;
+    const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (idx >= 2 * n_tiles * kP) return;
+    const int j = (int)(idx % kP);
+    const int64_t tile = (idx / kP) % n_tiles;
+    const int side = (int)(idx / (kP * n_tiles));
+    double* __restrict__ acc = a.edge_acc + (size_t)side * (size_t)a.N * kP;
+    const int64_t b0 = tile * W, b1 = min(a.N, b0 + W);
+    double run = 0.0;
+    if (side == 0) {
+        for (int64_t b = b1 - 1; b >= b0; --b) { run += acc[(size_t)b * kP + j]; acc[(size_t)b * kP + j] = run; }
+    } else {
+        for (int64_t b = b0; b < b1; ++b) { run += acc[(size_t)b * kP + j]; acc[(size_t)b * kP + j] = run; }
+    }
+}
+
 // value at xi (tile-normalised coordinate in [-1, 1]) of the degree-(kP-1) interpolant through the node sums
 __device__ __forceinline__ double cheb_interp(const double* __restrict__ nodes, double xi)
 {
@@ -1052,6 +1173,23 @@ __global__ void __launch_bounds__(256) node_bins_kernel(AccArgs a)
     const double xi = ((double)(b - j * a.lv.w0) - 0.5 * (double)(a.lv.w0 - 1)) / (0.5 * (double)a.lv.w0);
     const double v = cheb_interp(a.node_acc + (size_t)j * kP, xi);
     if (v != 0.0) a.out_k[b] += v * scalbn(1.0, -a.st->scale_exp);
+}
+
+// scanned edge accumulators -> bins of k(nu)
+__global__ void __launch_bounds__(256) edge_bins_kernel(AccArgs a)
+{
+    const int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (b >= a.N) return;
+    const double* __restrict__ r0 = a.edge_acc + (size_t)b * kP;
+    const double* __restrict__ r1 = a.edge_acc + ((size_t)a.N + (size_t)b) * kP;
+    double nodes[kP];
+    bool any = false;
+#pragma unroll
+    for (int j = 0; j < kP; ++j) { nodes[j] = r0[j] + r1[j]; any |= nodes[j] != 0.0; }
+    if (!any) return;
+    const int64_t j0 = b / a.lv.w0;
+    const double xi = ((double)(b - j0 * a.lv.w0) - 0.5 * (double)(a.lv.w0 - 1)) / (0.5 * (double)a.lv.w0);
+    a.out_k[b] += cheb_interp(nodes, xi) * scalbn(1.0, -a.st->scale_exp);
 }
 
 // ---------------------------------------------------------------------------------------

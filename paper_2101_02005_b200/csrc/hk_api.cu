@@ -26,6 +26,7 @@ struct hk_ctx {
     int debug_mode;
     int force_kb;
     double node_sep;
+    int edge_nodes;
     int n_sm;
     // last compute
     bool have_run;
@@ -49,7 +50,8 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, recN, tr, nr, node_acc, counts, prefix, cub;
+    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, recN, tr, nr, node_acc, edge_acc, counts, prefix, cub;
+    size_t edge_acc_bytes;   // 0: grid too large for the per-bin edge accumulators (direct edge kernel only)
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
     int32_t n_entries;   // upper bound on (level, tile) entries of the node hierarchy
@@ -101,6 +103,10 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     L.tr = take((size_t)L.n_ct * sizeof(TileRange));
     L.nr = take((size_t)L.n_entries * sizeof(NodeRange));
     L.node_acc = take((size_t)L.n_entries * kP * sizeof(double));
+    // per-bin node sums of the extent ends: [2][N][kP] fp64 = 128 B per bin, used up to 1 GiB
+    L.edge_acc_bytes = (size_t)2 * (size_t)c->N * kP * sizeof(double);
+    if (L.edge_acc_bytes > ((size_t)1 << 30)) L.edge_acc_bytes = 0;
+    L.edge_acc = take(L.edge_acc_bytes);
     L.counts = take((size_t)L.n_counts * 4);
     L.prefix = take((size_t)L.n_counts * 4);
     L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_counts);
@@ -253,6 +259,7 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     std::memset(c, 0, sizeof(*c));
     c->numin = numin; c->numax = numax; c->dnu = dnu; c->N = (int64_t)Nd;
     c->node_sep = 4.0;
+    c->edge_nodes = 1;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -323,6 +330,13 @@ int hk_set_node_separation(hk_ctx* ctx, double sep)
     return HK_OK;
 }
 
+int hk_set_edge_nodes(hk_ctx* ctx, int on)
+{
+    if (!ctx) return HK_EINVAL;
+    ctx->edge_nodes = on ? 1 : 0;
+    return HK_OK;
+}
+
 int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane)
 {
     if (!ctx || !(bins_per_lane == 0 || bins_per_lane == 2 || bins_per_lane == 4 || bins_per_lane == 8)) return HK_EINVAL;
@@ -342,7 +356,8 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     char* ws = (char*)ctx->ws;
     DevStats* st = (DevStats*)(ws + L.stats);
     const int n = (int)n_lines;
-    const Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm));
+    Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm));
+    p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes) ? 1 : 0;
 
     HK_CUDA(cudaEventRecord(ctx->ev[0], stream));
     HK_CUDA(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
@@ -372,6 +387,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     TileRange* tr = (TileRange*)(ws + L.tr);
     NodeRange* nr = (NodeRange*)(ws + L.nr);
     double* node_acc = (double*)(ws + L.node_acc);
+    double* edge_acc = L.edge_acc_bytes ? (double*)(ws + L.edge_acc) : nullptr;
     int32_t* counts = (int32_t*)(ws + L.counts);
     int32_t* prefix = (int32_t*)(ws + L.prefix);
     const Levels lv = make_levels(ctx, p);
@@ -419,6 +435,8 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     a.prefix_centre = prefix + 3 * p.n_ct; a.prefix_near = prefix + 4 * p.n_ct;
     a.prefix_node = prefix + 5 * p.n_ct;
     a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc;
+    const bool use_edge_nodes = p.edge_nodes && p.mode == 0 && lv.n_levels > 0 && !p.uncut;
+    a.edge_acc = use_edge_nodes ? edge_acc : nullptr;
     a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.lv = lv;
     const int grid = ctx->n_sm * 2;
     if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * 4, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
@@ -430,6 +448,14 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         if (p.mode != 1) { interior_kernel<KB, true><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
         if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<ctx->n_sm * 4, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        if (use_edge_nodes) {
+            cudaMemsetAsync(edge_acc, 0, L.edge_acc_bytes, stream);
+            edge_node_kernel<<<ctx->n_sm * 4, kThreads, 0, stream>>>(p, a, keys_out, n);
+            const int64_t nsc = 2 * ((ctx->N + lv.w0 - 1) / lv.w0) * kP;
+            edge_scan_kernel<<<(int)((nsc + 255) / 256), 256, 0, stream>>>(a);
+            edge_bins_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
+            ctx->last_launches += 3;
+        }
         cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
         if (p.mode == 0 || p.mode == 3) { centre_kernel<KB><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
@@ -664,6 +690,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_pairs_edge = (int64_t)d.pairs_edge;
     host_out->n_pairs_centre = (int64_t)d.pairs_centre;
     host_out->n_pairs_node = (int64_t)d.pairs_node;
+    host_out->n_pairs_edge_node = (int64_t)d.pairs_edge_node;
     host_out->n_bins_node = (int64_t)d.bins_node;
     host_out->n_levels = ctx->last_levels;
     host_out->scale_exp = d.scale_exp;

@@ -35,6 +35,7 @@ struct Params {
     int32_t chunk;              // lines per work unit of the direct kernels
     int32_t chunk_node;         // lines per work unit of the node kernel
     double sep;                 // node separation: |centre - tile centre| >= sep * half-width
+    int edge_nodes;             // 1: separated edge tiles go through per-bin node accumulators (edge_node_kernel)
     int mode;                   // debug: 0 default, 1 everything through the near kernel, 2 far pairs through the mid kernel,
                                 //        3 direct evaluation only (no node hierarchy)
 };
@@ -51,6 +52,7 @@ struct DevStats {
     unsigned long long units_far, units_mid, units_near, units_node, units_edge, units_centre;
     unsigned long long pairs_far, pairs_mid, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
     unsigned long long pairs_edge, pairs_centre;
+    unsigned long long pairs_edge_node;                    // (line, extent end) pairs evaluated at the nodes of their edge tile
     unsigned long long pairs_node;                         // (line, tile) pairs evaluated at nodes
     unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
 };
@@ -274,6 +276,31 @@ __device__ __forceinline__ NodeKeys node_keys(const Params& p, int64_t w0, int64
     return k;
 }
 
+// Extent ends ("edges").  A tile that a line's extent covers only in part, with the line centre at least sep
+// half-widths away and |z|^2 >= Z2 on all of it, is evaluated at the tile's nodes too; the node values go to per-bin
+// accumulators indexed by the bin at which the extent ends and reach the bins through a prefix / suffix sum over the
+// tile (edge_node_kernel).  For the tile [w0, w0 + W): a line LEFT of it (its extent ends inside
+// the tile) qualifies when jc <= upL, a line RIGHT of it (its extent starts inside) when jc >= dnR.  The same
+// thresholds take these lines out of the direct edge kernel's ranges in range_kernel.
+struct EdgeKeys {
+    int64_t upL, dnR;
+};
+
+__device__ __forceinline__ EdgeKeys edge_keys(const Params& p, int64_t w0, int64_t W)
+{
+    const int64_t w1 = min(p.N, w0 + W);
+    const int64_t mind = (int64_t)kMinDistPerKB * p.kb;
+    const double m = (double)w0 + 0.5 * (double)(W - 1), h = 0.5 * (double)W;
+    const int64_t sepL = (int64_t)floor(m - p.sep * h) - 1;
+    const int64_t sepR = (int64_t)ceil(m + p.sep * h);
+    const int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.numin_bins), w0 - 1 - mind);
+    const int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.numin_bins), w1 - 1 + mind);
+    EdgeKeys k;
+    k.upL = min(min(sepL, jLmid), w1 - p.cb_floor - 1);        // and not interior: jc < jLmin = w1 - cb_floor
+    k.dnR = max(max(sepR, jRmid), w0 + p.cb_floor - 1);        // jc > jRmax = w0 + cb_floor - 2
+    return k;
+}
+
 // index of the first sorted line with centre bin >= j (keys are jc - kmin)
 __device__ __forceinline__ int32_t idx_of(const Params& p, const int32_t* __restrict__ keys, int32_t n_act, int64_t j)
 {
@@ -400,6 +427,12 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
         r.ER = max(min(idx_of(p, keys, n_act, jRmid), r.A1), fr1);
         r.CL = min(max(idx_of(p, keys, n_act, jLmin), ml1), mr0);
         r.CR = min(max(idx_of(p, keys, n_act, jRmax + 1), r.CL), mr0);
+    }
+    if (p.edge_nodes && p.mode == 0 && lv.n_levels > 0 && !p.uncut) {
+        // [A0, ESL) and [ESR, A1) go to edge_node_kernel; the direct edge kernel keeps [ESL, EL) and [ER, ESR)
+        const EdgeKeys ek = edge_keys(p, w0, wb);
+        r.A0 = min(max(idx_of(p, keys, n_act, ek.upL + 1), r.A0), r.EL);
+        r.A1 = max(min(idx_of(p, keys, n_act, ek.dnR), r.A1), r.ER);
     }
     tr[wt] = r;
     const unsigned long long nb = (unsigned long long)(w1 - w0);

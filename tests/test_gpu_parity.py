@@ -111,7 +111,8 @@ def test_cross_path_nodes_vs_direct(B):
         # every (line, bin) pair of the definition is covered exactly once by one of the four paths
         for st in (st0, st3):
             cover = st["n_pairs_far"] + st["n_pairs_mid"] + st["n_bins_node"]
-            assert cover <= st["n_evals"] <= cover + st["n_pairs_near"] + st["n_pairs_edge"] + st["n_pairs_centre"]
+            edge_node_bins = st["n_pairs_edge_node"] * 32 * st["bins_per_lane"]
+            assert cover <= st["n_evals"] <= cover + st["n_pairs_near"] + st["n_pairs_edge"] + st["n_pairs_centre"] + edge_node_bins
         big = k3 >= 1e-8 * k3.max()
         assert np.abs(k0[big] / k3[big] - 1.0).max() <= 3e-5
         if cfg == 5:
@@ -120,6 +121,34 @@ def test_cross_path_nodes_vs_direct(B):
             k1, st1, _ = _gpu_k(B, lines, cond, grid, cut, debug_mode=mode, tile_bins=tb)
             assert st1["n_pairs_far"] == 0 and st1["n_pairs_node"] == 0
             assert np.abs(k1[big] / k3[big] - 1.0).max() <= 4e-5
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 20_000), (3, 200_000), (4, 6_000), (1, None)])
+def test_edge_nodes_on_vs_off(B, cfg, n):
+    """Extent ends through the per-bin node accumulators (default) against the masked direct edge kernel, all bins,
+    and both against the oracle."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    dl = _to_cuda(lines)
+    ks = []
+    for on in (True, False):
+        op = B.Opacity(*grid)
+        op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        op.set_edge_nodes(on)
+        k = op.compute(dl, cut)
+        torch.cuda.synchronize()
+        st = op.stats()
+        if on:
+            assert st["n_pairs_edge_node"] > 0
+            n_on_edge = st["n_pairs_edge"]
+        else:
+            assert st["n_pairs_edge_node"] == 0 and st["n_pairs_edge"] > n_on_edge
+        ks.append(k.cpu().numpy())
+        op.close()
+    k_ref, _ = O.opacity_grid(lines, cond, grid, cut)
+    for k in ks:
+        check_parity(k, k_ref, what=f"config {cfg} edge nodes")
+    big = k_ref >= 1e-8 * k_ref.max()
+    assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 3e-5
 
 
 @pytest.mark.parametrize("sep", [2.5, 4.0, 6.0])
