@@ -1066,6 +1066,7 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
     const int32_t n_act = s_nact;
     const int lane = threadIdx.x & 31;
     const int64_t W = a.lv.w0;
+    const int wshift = __ffs(a.lv.w0) - 1;
     float2 xk[M];
     const double hc = 0.5 * (double)(W - 1), hw = 0.5 * (double)W;
 #pragma unroll
@@ -1086,11 +1087,8 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
         for (int side = 0; side < 2; ++side) {
             const int64_t e = side == 0 ? ihi : ilo;
             bool m = live && ihi >= ilo;
-            const int64_t T0 = m ? (e / W) * W : 0;
-            if (m) {
-                const EdgeKeys k = edge_keys(p, T0, W);
-                m = side == 0 ? (jc <= k.upL) : (jc >= k.dnR);
-            }
+            const int64_t T0 = m ? (e >> wshift) << wshift : 0;     // level-0 tiles are 64, 128 or 256 bins
+            if (m) m = side == 0 ? (jc <= edge_key_upL(p, T0, W)) : (jc >= edge_key_dnR(p, T0, W));
             float v[kP];
 #pragma unroll
             for (int j = 0; j < kP; ++j) v[j] = 0.f;

@@ -158,6 +158,8 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
     }
     p.kappa1 = std::sqrt((double)HK_Z1) * p.beta * 1.001;
     p.kappa2 = std::sqrt((double)HK_Z2) * p.beta * 1.001;
+    p.inv1p_k1 = 1.0 / (1.0 + p.kappa1); p.inv1m_k1 = 1.0 / (1.0 - p.kappa1);
+    p.inv1p_k2 = 1.0 / (1.0 + p.kappa2); p.inv1m_k2 = 1.0 / (1.0 - p.kappa2);
     p.numin_bins = c->numin / c->dnu;
     p.kb = pick_kb(c, cut);
     p.n_ct = (int32_t)((c->N + 32 * p.kb - 1) / (32 * p.kb));

@@ -29,6 +29,7 @@ struct Params {
     // tile ranges
     int64_t cb_floor, cb_ceil;  // floor/ceil of cut/dnu (bins)
     double kappa1, kappa2;      // sqrt(Z1) * beta and sqrt(Z2) * beta, slightly inflated
+    double inv1p_k1, inv1m_k1, inv1p_k2, inv1m_k2;   // 1/(1 + kappa), 1/(1 - kappa)
     double numin_bins;          // numin / dnu
     int32_t kb;                 // bins per lane (2, 4, 8)
     int32_t n_ct;               // tiles of 32 kb bins
@@ -238,16 +239,17 @@ __device__ __forceinline__ int32_t lower_bound_key(const int32_t* __restrict__ k
 // |t| >= max(16 KB, sqrt(Z) a): then |z|^2 >= Z for every (line, bin) pair (Z = Z1: far, Z = Z2: mid)
 // and the interior kernels may run mask-free.  alpha_D = beta nu0 is a function of the centre, so the
 // condition is a bound on the centre bin alone; all bounds are conservative.
-__device__ __forceinline__ int64_t left_bound(double w0, double kap, double numin_bins)
+// (the reciprocals 1/(1 + kap), 1/(1 - kap) come from the host: one rounding more, far inside the margin of 3 bins)
+__device__ __forceinline__ int64_t left_bound(double w0, double kap, double inv1p, double numin_bins)
 {
     // pos + 1 <= (w0 - kap numin_bins) / (1 + kap)   =>   w0 - pos >= kap (numin_bins + pos)
-    return (int64_t)floor((w0 - kap * (numin_bins + 1.0)) / (1.0 + kap)) - 3;
+    return (int64_t)floor((w0 - kap * (numin_bins + 1.0)) * inv1p) - 3;
 }
-__device__ __forceinline__ int64_t right_bound(double w1m1, double kap, double numin_bins)
+__device__ __forceinline__ int64_t right_bound(double w1m1, double kap, double inv1m, double numin_bins)
 {
     // pos >= (w1 - 1 + kap numin_bins) / (1 - kap)   =>   pos - (w1 - 1) >= kap (numin_bins + pos)
     if (!(kap < 0.9)) return INT64_MAX / 2;
-    return (int64_t)ceil((w1m1 + kap * (numin_bins + 1.0)) / (1.0 - kap)) + 3;
+    return (int64_t)ceil((w1m1 + kap * (numin_bins + 1.0)) * inv1m) + 3;
 }
 
 // Key thresholds of one tile [w0, w1) of width W (any level) for the node hierarchy.  A line with centre bin jc is
@@ -268,8 +270,8 @@ __device__ __forceinline__ NodeKeys node_keys(const Params& p, int64_t w0, int64
     k.hiR = p.uncut ? kBigKey : w0 + p.cb_floor - 2;
     const int64_t sepL = (int64_t)floor(m - p.sep * h) - 1;
     const int64_t sepR = (int64_t)ceil(m + p.sep * h);
-    k.upL = min(sepL, left_bound((double)w0, p.kappa2, p.numin_bins));
-    k.dnR = max(sepR, right_bound((double)(w1 - 1), p.kappa2, p.numin_bins));
+    k.upL = min(sepL, left_bound((double)w0, p.kappa2, p.inv1p_k2, p.numin_bins));
+    k.dnR = max(sepR, right_bound((double)(w1 - 1), p.kappa2, p.inv1m_k2, p.numin_bins));
     // empty sets are written as [lo, lo - 1] / [hi + 1, hi]
     k.upL = max(k.upL, k.loL - 1);
     k.dnR = min(k.dnR, k.hiR + 1);
@@ -286,18 +288,29 @@ struct EdgeKeys {
     int64_t upL, dnR;
 };
 
-__device__ __forceinline__ EdgeKeys edge_keys(const Params& p, int64_t w0, int64_t W)
+__device__ __forceinline__ int64_t edge_key_upL(const Params& p, int64_t w0, int64_t W)
 {
     const int64_t w1 = min(p.N, w0 + W);
     const int64_t mind = (int64_t)kMinDistPerKB * p.kb;
     const double m = (double)w0 + 0.5 * (double)(W - 1), h = 0.5 * (double)W;
     const int64_t sepL = (int64_t)floor(m - p.sep * h) - 1;
+    const int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.inv1p_k2, p.numin_bins), w0 - 1 - mind);
+    return min(min(sepL, jLmid), w1 - p.cb_floor - 1);           // and not interior: jc < jLmin = w1 - cb_floor
+}
+__device__ __forceinline__ int64_t edge_key_dnR(const Params& p, int64_t w0, int64_t W)
+{
+    const int64_t w1 = min(p.N, w0 + W);
+    const int64_t mind = (int64_t)kMinDistPerKB * p.kb;
+    const double m = (double)w0 + 0.5 * (double)(W - 1), h = 0.5 * (double)W;
     const int64_t sepR = (int64_t)ceil(m + p.sep * h);
-    const int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.numin_bins), w0 - 1 - mind);
-    const int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.numin_bins), w1 - 1 + mind);
+    const int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.inv1m_k2, p.numin_bins), w1 - 1 + mind);
+    return max(max(sepR, jRmid), w0 + p.cb_floor - 1);           // jc > jRmax = w0 + cb_floor - 2
+}
+__device__ __forceinline__ EdgeKeys edge_keys(const Params& p, int64_t w0, int64_t W)
+{
     EdgeKeys k;
-    k.upL = min(min(sepL, jLmid), w1 - p.cb_floor - 1);        // and not interior: jc < jLmin = w1 - cb_floor
-    k.dnR = max(max(sepR, jRmid), w0 + p.cb_floor - 1);        // jc > jRmax = w0 + cb_floor - 2
+    k.upL = edge_key_upL(p, w0, W);
+    k.dnR = edge_key_dnR(p, w0, W);
     return k;
 }
 
@@ -386,12 +399,12 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
     r.A1 = idx_of(p, keys, n_act, jhi + 1);
     // left of the tile: the extent must reach the tile's last bin (jc >= jLmin)
     const int64_t jLmin = p.uncut ? -kBigKey : w1 - p.cb_floor;
-    int64_t jLfar = min(left_bound((double)w0, p.kappa1, p.numin_bins), w0 - 1 - mind);
-    int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.numin_bins), w0 - 1 - mind);
+    int64_t jLfar = min(left_bound((double)w0, p.kappa1, p.inv1p_k1, p.numin_bins), w0 - 1 - mind);
+    int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.inv1p_k2, p.numin_bins), w0 - 1 - mind);
     // right of the tile: the extent must reach the tile's first bin (jc <= jRmax)
     const int64_t jRmax = p.uncut ? kBigKey : w0 + p.cb_floor - 2;
-    int64_t jRfar = max(right_bound((double)(w1 - 1), p.kappa1, p.numin_bins), w1 - 1 + mind);
-    int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.numin_bins), w1 - 1 + mind);
+    int64_t jRfar = max(right_bound((double)(w1 - 1), p.kappa1, p.inv1m_k1, p.numin_bins), w1 - 1 + mind);
+    int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.inv1m_k2, p.numin_bins), w1 - 1 + mind);
     if (p.mode == 1) { jLfar = jLmid = -kBigKey; jRfar = jRmid = kBigKey; }
     if (p.mode == 2) { jLfar = -kBigKey; jRfar = kBigKey; }
     int32_t fl0 = idx_of(p, keys, n_act, jLmin);
