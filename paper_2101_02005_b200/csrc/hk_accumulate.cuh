@@ -415,6 +415,7 @@ constexpr int kSubC = 512;
 constexpr int kLPTC = kSubC / kThreads;
 constexpr int kStage = 16;             // bins per staging step of the core pass
 constexpr int kCentreCtas = 4;         // resident CTAs per SM the centre kernel is compiled and launched for
+constexpr int kNodeCtas = 6;           // resident CTAs per SM of the node kernel
 constexpr int kYClasses = 32;          // classes of y = Gamma_L/alpha_D the lines of a batch are sorted into
 static_assert(kSubC == 32 * 2 * kWarps, "a batch is 2 groups of 32 lines per warp");
 
@@ -942,7 +943,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
 // positions and kP partial sums in registers; two nodes share one reciprocal.  The partial sums are
 // combined with warp shuffles, then across warps, and reach the (level, tile) node sums with one
 // fp64 atomic per node per work unit.  Formula: two asymptotic terms (valid: |z|^2 >= Z2 on the tile).
-__global__ void __launch_bounds__(kThreads, 4) node_kernel(AccArgs a)
+__global__ void __launch_bounds__(kThreads, kNodeCtas) node_kernel(AccArgs a)
 {
     constexpr int M = kP / 2;
     __shared__ float red[kWarps][kP];

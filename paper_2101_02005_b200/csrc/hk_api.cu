@@ -441,7 +441,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     a.edge_acc = use_edge_nodes ? edge_acc : nullptr;
     a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.lv = lv;
     const int grid = ctx->n_sm * 2;
-    if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * 4, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+    if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NODE + 1], stream));
     auto launch = [&](auto kb_tag) {
         constexpr int KB = decltype(kb_tag)::value;

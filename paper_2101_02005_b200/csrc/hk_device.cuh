@@ -221,8 +221,11 @@ __device__ __noinline__ float core_K(float x, float y)
         __sincosf(ph, &sp, &cp);
         const float nr = amp * cp, ni = -amp * sp;
         const float e = __expf(7.85398163f /* 2 pi/h */ * y);
+        // theta = 2 pi frac(x/h - s) in [pi/2, 3pi/2] (cos(theta) <= 0): theta - pi lies in [-pi/2, pi/2], where the
+        // special-function unit's sin/cos are good to ~5e-7 absolute
         float st, ct;
-        sincospif(2.0f * frs, &st, &ct);                  // theta = 2 pi frac(x/h - s), cos(theta) <= 0
+        __sincosf(6.28318531f * (frs - 0.5f), &st, &ct);
+        st = -st; ct = -ct;
         const float dr = fmaf(-e, ct, 1.0f), di = e * st;
         K = fmaf(fmaf(nr, dr, ni * di), rcp_approx(fmaf(dr, dr, di * di)), K);
     }
