@@ -206,12 +206,33 @@ double hko_profile(double nu, double nu0, double gammaL, double alphaD)
  * KNOWS no other line can reach these bins (centres sorted, fixed cut) skip
  * them; passing 0, n is the definition.  Neumaier-compensated sum per bin.
  * evals_out (optional) receives the number of (line, bin) evaluations. */
+/* plinth != 0 (and a finite cut): every term is S (V(nu_i - nu0) - V(cut)), the line with its "plinth" -- its own
+ * value at the cutting length position -- removed from every bin of its extent (section 2.1.1; DESIGN.md
+ * R21: the plinth is the profile AT nu0 +- cut, not at the last grid point inside the extent). */
+void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const double *g,
+                         const double *E, const double *gam, const double *nx,
+                         double T, double P_atm, double mass_amu, double Q,
+                         double numin, double dnu, int64_t N, double cut, int plinth,
+                         int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
+                         double *k_out, int64_t *evals_out);
+
 void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const double *g,
                       const double *E, const double *gam, const double *nx,
                       double T, double P_atm, double mass_amu, double Q,
                       double numin, double dnu, int64_t N, double cut,
                       int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                       double *k_out, int64_t *evals_out)
+{
+    hko_opacity_bins_ex(n, nu0, A, g, E, gam, nx, T, P_atm, mass_amu, Q, numin, dnu, N, cut, 0, nb, bins, l0, l1,
+                        k_out, evals_out);
+}
+
+void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const double *g,
+                         const double *E, const double *gam, const double *nx,
+                         double T, double P_atm, double mass_amu, double Q,
+                         double numin, double dnu, int64_t N, double cut, int plinth,
+                         int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
+                         double *k_out, int64_t *evals_out)
 {
     int64_t nl = l1 - l0;
     if (nl < 0) nl = 0;
@@ -220,6 +241,8 @@ void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const doubl
     double *aD = (double *)malloc(sizeof(double) * (size_t)(nl + 1));
     int64_t *ilo = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nl + 1));
     int64_t *ihi = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nl + 1));
+    double *pl = (double *)malloc(sizeof(double) * (size_t)(nl + 1));   /* V(cut) per line, 0 without plinth removal */
+    const int use_plinth = plinth && cut > 0.0 && isfinite(cut);
     (void)n;
 #pragma omp parallel for schedule(static)
     for (int64_t q = 0; q < nl; ++q) {
@@ -228,7 +251,8 @@ void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const doubl
             line_params(nu0[l], A[l], g[l], E[l], gam[l], nx[l], T, P_atm, mass_amu, Q,
                         &S[q], &gL[q], &aD[q]);
             line_extent(nu0[l], numin, dnu, N, cut, &ilo[q], &ihi[q], &jc);
-        } else { S[q] = 0.0; gL[q] = 0.0; aD[q] = 1.0; ilo[q] = 0; ihi[q] = -1; }
+            pl[q] = use_plinth ? hko_voigt_K(cut / aD[q], gL[q] / aD[q]) : 0.0;
+        } else { S[q] = 0.0; gL[q] = 0.0; aD[q] = 1.0; ilo[q] = 0; ihi[q] = -1; pl[q] = 0.0; }
     }
     int64_t evals = 0;
     const double sqrtpi = sqrt(HKO_PI);
@@ -241,7 +265,7 @@ void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const doubl
             if (i < ilo[q] || i > ihi[q]) continue;
             double x = (nu - nu0[l0 + q]) / aD[q];
             double y = gL[q] / aD[q];
-            double term = S[q] * hko_voigt_K(x, y) / (aD[q] * sqrtpi);
+            double term = S[q] * (hko_voigt_K(x, y) - pl[q]) / (aD[q] * sqrtpi);
             double t = sum + term;                 /* Neumaier */
             if (fabs(sum) >= fabs(term)) comp += (sum - t) + term;
             else comp += (term - t) + sum;
@@ -251,5 +275,5 @@ void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const doubl
         k_out[b] = sum + comp;
     }
     if (evals_out) *evals_out = evals;
-    free(S); free(gL); free(aD); free(ilo); free(ihi);
+    free(S); free(gL); free(aD); free(ilo); free(ihi); free(pl);
 }

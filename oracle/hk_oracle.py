@@ -42,6 +42,11 @@ _lib.hko_opacity_bins.argtypes = [_i64, _pd, _pd, _pd, _pd, _pd, _pd, _d, _d, _d
                                   _d, _d, _i64, _d, _i64, _pi64, _i64, _i64, _pd,
                                   C.POINTER(_i64)]
 
+_lib.hko_opacity_bins_ex.restype = None
+_lib.hko_opacity_bins_ex.argtypes = [_i64, _pd, _pd, _pd, _pd, _pd, _pd, _d, _d, _d, _d,
+                                     _d, _d, _i64, _d, C.c_int, _i64, _pi64, _i64, _i64, _pd,
+                                     C.POINTER(_i64)]
+
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 
 
@@ -99,8 +104,9 @@ def profile(nu, nu0, gammaL, alphaD) -> float:
     return float(_lib.hko_profile(nu, nu0, gammaL, alphaD))
 
 
-def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None):
-    """k at the listed bins, brute force over lines [l0, l1).  -> (k, n_evals)."""
+def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False):
+    """k at the listed bins, brute force over lines [l0, l1).  -> (k, n_evals).
+    plinth=True removes every line's value at the cutting length from its bins (section 2.1.1)."""
     a = [_f64(lines[k]) for k in FIELDS]
     n = a[0].size
     if l1 is None:
@@ -110,9 +116,9 @@ def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None):
     ev = _i64(0)
     numin, numax, dnu = grid
     N = grid_size(numin, numax, dnu)
-    _lib.hko_opacity_bins(n, *a, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"],
-                          numin, dnu, N, float(cut), bins.size, bins, int(l0), int(l1),
-                          out, C.byref(ev))
+    _lib.hko_opacity_bins_ex(n, *a, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"],
+                             numin, dnu, N, float(cut), 1 if plinth else 0, bins.size, bins, int(l0), int(l1),
+                             out, C.byref(ev))
     return out, int(ev.value)
 
 
@@ -120,19 +126,19 @@ def _uncut(cut) -> bool:
     return not (cut > 0.0 and np.isfinite(cut))
 
 
-def opacity_window(lines_sorted, cond, grid, cut, b0, b1):
+def opacity_window(lines_sorted, cond, grid, cut, b0, b1, plinth=False):
     """k on bins [b0, b1) for lines SORTED by nu0 (fixed cut: only lines within
     cut + one bin of the window are passed to the brute-force routine)."""
     numin, numax, dnu = grid
     bins = np.arange(b0, b1, dtype=np.int64)
     nu0 = lines_sorted["nu0"]
     if _uncut(cut):
-        return opacity_bins(lines_sorted, cond, grid, cut, bins)
+        return opacity_bins(lines_sorted, cond, grid, cut, bins, plinth=plinth)
     lo = numin + b0 * dnu - cut - 2.0 * dnu
     hi = numin + (b1 - 1) * dnu + cut + 2.0 * dnu
     l0 = int(np.searchsorted(nu0, lo, side="left"))
     l1 = int(np.searchsorted(nu0, hi, side="right"))
-    return opacity_bins(lines_sorted, cond, grid, cut, bins, l0, l1)
+    return opacity_bins(lines_sorted, cond, grid, cut, bins, l0, l1, plinth=plinth)
 
 
 def sort_lines(lines):
@@ -143,7 +149,7 @@ def sort_lines(lines):
     return {k: _f64(lines[k])[order] for k in FIELDS}
 
 
-def opacity_grid(lines, cond, grid, cut, block=512, presorted=False):
+def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=False):
     """k on every bin of the grid.  -> (k[N], n_evals)."""
     numin, numax, dnu = grid
     N = grid_size(numin, numax, dnu)
@@ -154,7 +160,7 @@ def opacity_grid(lines, cond, grid, cut, block=512, presorted=False):
         block = N
     for b0 in range(0, N, block):
         b1 = min(N, b0 + block)
-        kk, ev = opacity_window(ls, cond, grid, cut, b0, b1)
+        kk, ev = opacity_window(ls, cond, grid, cut, b0, b1, plinth=plinth)
         k[b0:b1] = kk
         evals += ev
     return k, evals
