@@ -110,6 +110,12 @@ int64_t hk_grid_size(const hk_ctx* ctx);
  * P >= 0, all finite. */
 int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, double Q);
 
+/* Plinth removal (section 2.1.1): on != 0 subtracts from every bin of a line's extent that line's own value
+ * at the cutting length position, S V(nu0 +- cut) (needed with continua that already hold the plinths, e.g. CKD).
+ * Off by default; no effect on uncut computations.  Changes hk_workspace_bytes (+ 8 B per bin): set it before the
+ * workspace is sized.  Applies to hk_compute, hk_accumulate, hk_compute_batch and hk_compute_host. */
+int hk_set_plinth(hk_ctx* ctx, int on);
+
 /* Device scratch the caller must provide for hk_compute with up to n_lines lines. */
 size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines);
 int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);

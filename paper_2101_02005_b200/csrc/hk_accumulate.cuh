@@ -48,6 +48,7 @@ struct AccArgs {
     DevStats* st;
     double* __restrict__ out_k;
     double* __restrict__ node_acc;             // n_entries x kP node sums (scaled), fp64
+    double* __restrict__ plinth_acc;           // N + 1 doubles: difference array of the plinths, then its running sum; or null
     double* __restrict__ edge_acc;             // [2][N][kP] per-bin node sums of extent ends (scaled), fp64; or null
     int64_t N;
     int32_t n_ct, chunk, chunk_node;
@@ -1189,6 +1190,71 @@ __global__ void __launch_bounds__(256) edge_bins_kernel(AccArgs a)
     const int64_t j0 = b / a.lv.w0;
     const double xi = ((double)(b - j0 * a.lv.w0) - 0.5 * (double)(a.lv.w0 - 1)) / (0.5 * (double)a.lv.w0);
     a.out_k[b] += cheb_interp(nodes, xi) * scalbn(1.0, -a.st->scale_exp);
+}
+
+// ---------------------------------------------------------------------------------------
+// plinth removal (section 2.1.1): subtract S V(cut) of every line from every bin of its extent
+// ---------------------------------------------------------------------------------------
+// The removed part is a sum of boxes, one per line: -p_l on [ilo, ihi].  Lanes walk the sorted lines, evaluate p_l
+// from the SAME fp32 record the accumulation kernels use (so V - V(cut) goes to zero consistently at the extent's
+// ends) with the same region split, and add -p_l at ilo and +p_l at ihi + 1 of a difference array (equal bins summed
+// in the warp first); a running sum over the bins (CUB) turns it into the box sum, plinth_apply_kernel adds it to k.
+__device__ __forceinline__ void warp_add_scalar_by_bin(double* __restrict__ acc, int64_t bin, double v, int lane)
+{
+    unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int64_t b = __shfl_sync(0xffffffffu, bin, leader);
+        const bool mine = (bin == b);
+        const unsigned grp = __ballot_sync(0xffffffffu, mine);
+        double sum = mine ? v : 0.0;
+        if (__popc(grp) > 1) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        }
+        if (lane == leader) atomicAdd(acc + b, sum);
+        todo &= ~grp;
+    }
+}
+
+__global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys, int32_t n)
+{
+    __shared__ int32_t s_nact;
+    if (threadIdx.x == 0) s_nact = lower_bound_key(keys, n, (int64_t)p.ksent);
+    __syncthreads();
+    const int32_t n_act = s_nact;
+    const int lane = threadIdx.x & 31;
+    const double unscale = scalbn(1.0, -a.st->scale_exp);
+    const int64_t n_round = ((int64_t)n_act + 31) & ~31LL;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+        int64_t ilo = 0, ihi = -1;
+        double pl = 0.0;
+        if (i < n_act) {
+            const float4 ra = a.recA[i], rb = a.recB[i];
+            ilo = __float_as_int(rb.y); ihi = __float_as_int(rb.z);
+            const double G2 = (double)ra.z, a2 = (double)rb.x, cb = p.cut_bins;
+            const double q = cb * cb + G2;
+            if (q >= (double)HK_Z2 * a2) {
+                // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q)
+                pl = (double)ra.w / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
+            } else {
+                const float inv_a = rsqrtf(rb.x);
+                pl = (double)(rb.w * core_any_K((float)cb * inv_a, sqrtf(ra.z) * inv_a, nullptr));
+            }
+            pl *= unscale;
+        }
+        const bool live = ihi >= ilo;
+        warp_add_scalar_by_bin(a.plinth_acc, live ? ilo : -1, -pl, lane);
+        warp_add_scalar_by_bin(a.plinth_acc, live ? ihi + 1 : -1, pl, lane);
+    }
+}
+
+__global__ void __launch_bounds__(256) plinth_apply_kernel(AccArgs a)
+{
+    const int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (b >= a.N) return;
+    const double v = a.plinth_acc[b];              // running sum: minus the plinths of the lines that cover bin b
+    if (v != 0.0) a.out_k[b] += v;
 }
 
 // ---------------------------------------------------------------------------------------

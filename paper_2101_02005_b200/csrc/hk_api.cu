@@ -27,6 +27,7 @@ struct hk_ctx {
     int force_kb;
     double node_sep;
     int edge_nodes;
+    int plinth;
     int n_sm;
     // last compute
     bool have_run;
@@ -50,7 +51,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, recN, tr, nr, node_acc, edge_acc, counts, prefix, cub;
+    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, recN, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
     size_t edge_acc_bytes;   // 0: grid too large for the per-bin edge accumulators (direct edge kernel only)
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
@@ -60,13 +61,15 @@ struct Layout {
 
 bool is_uncut(double cut) { return !(cut > 0.0 && std::isfinite(cut)); }
 
-size_t cub_temp_bytes(int64_t n, int32_t n_ct)
+size_t cub_temp_bytes(int64_t n, int32_t n_ct, int64_t n_bins)
 {
-    size_t b1 = 0, b2 = 0;
+    size_t b1 = 0, b2 = 0, b3 = 0;
+    cub::DeviceScan::InclusiveSum(nullptr, b3, (const double*)nullptr, (double*)nullptr, (int)(n_bins + 1), (cudaStream_t)0);
     cub::DeviceRadixSort::SortPairs(nullptr, b1, (const int32_t*)nullptr, (int32_t*)nullptr, (const int32_t*)nullptr,
                                     (int32_t*)nullptr, (int)n, 0, 32, (cudaStream_t)0);
     cub::DeviceScan::ExclusiveSum(nullptr, b2, (const int32_t*)nullptr, (int32_t*)nullptr, (int)n_ct,
                                   (cudaStream_t)0);
+    if (b3 > b1) b1 = b3;
     return b1 > b2 ? b1 : b2;
 }
 
@@ -107,9 +110,10 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     L.edge_acc_bytes = (size_t)2 * (size_t)c->N * kP * sizeof(double);
     if (L.edge_acc_bytes > ((size_t)1 << 30)) L.edge_acc_bytes = 0;
     L.edge_acc = take(L.edge_acc_bytes);
+    L.plinth_acc = take(c->plinth ? (size_t)(c->N + 1) * sizeof(double) : 0);
     L.counts = take((size_t)L.n_counts * 4);
     L.prefix = take((size_t)L.n_counts * 4);
-    L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_counts);
+    L.cub_bytes = cub_temp_bytes((int64_t)nn, L.n_counts, c->N);
     L.cub = take(L.cub_bytes);
     L.total = off;
     return L;
@@ -166,6 +170,8 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
     p.chunk = chunk;
     p.chunk_node = 16384;
     p.sep = c->node_sep;
+    p.plinth = (c->plinth && !p.uncut) ? 1 : 0;
+    p.cut_bins = cb;
     p.mode = c->debug_mode;
     return p;
 }
@@ -332,6 +338,13 @@ int hk_set_node_separation(hk_ctx* ctx, double sep)
     return HK_OK;
 }
 
+int hk_set_plinth(hk_ctx* ctx, int on)
+{
+    if (!ctx) return HK_EINVAL;
+    ctx->plinth = on ? 1 : 0;
+    return HK_OK;
+}
+
 int hk_set_edge_nodes(hk_ctx* ctx, int on)
 {
     if (!ctx) return HK_EINVAL;
@@ -439,6 +452,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc;
     const bool use_edge_nodes = p.edge_nodes && p.mode == 0 && lv.n_levels > 0 && !p.uncut;
     a.edge_acc = use_edge_nodes ? edge_acc : nullptr;
+    a.plinth_acc = p.plinth ? (double*)(ws + L.plinth_acc) : nullptr;
     a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.lv = lv;
     const int grid = ctx->n_sm * 2;
     if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
@@ -477,6 +491,16 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         }
         node_bins_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
         ++ctx->last_launches;
+    }
+    // plinth removal: difference array over the sorted lines -> running sum over the bins -> subtract
+    if (p.plinth) {
+        HK_CUDA(cudaMemsetAsync(a.plinth_acc, 0, (size_t)(ctx->N + 1) * sizeof(double), stream));
+        plinth_kernel<<<ctx->n_sm * 8, 256, 0, stream>>>(p, a, keys_out, n);
+        cub_bytes = L.cub_bytes;
+        HK_CUDA(cub::DeviceScan::InclusiveSum(ws + L.cub, cub_bytes, (const double*)a.plinth_acc, a.plinth_acc,
+                                              (int)(ctx->N + 1), stream));
+        plinth_apply_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
+        ctx->last_launches += 2;
     }
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_DOWN + 1], stream));
     HK_CUDA(cudaGetLastError());

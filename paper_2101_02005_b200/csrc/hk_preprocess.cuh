@@ -36,6 +36,8 @@ struct Params {
     int32_t chunk;              // lines per work unit of the direct kernels
     int32_t chunk_node;         // lines per work unit of the node kernel
     double sep;                 // node separation: |centre - tile centre| >= sep * half-width
+    int plinth;                 // 1: remove every line's value at the cutting length from its bins (section 2.1.1)
+    double cut_bins;            // cut / dnu
     int edge_nodes;             // 1: separated edge tiles go through per-bin node accumulators (edge_node_kernel)
     int mode;                   // debug: 0 default, 1 everything through the near kernel, 2 far pairs through the mid kernel,
                                 //        3 direct evaluation only (no node hierarchy)

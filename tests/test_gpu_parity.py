@@ -243,6 +243,53 @@ def test_batched_conditions(B):
     op.close()
 
 
+@pytest.mark.parametrize("case", ["config2", "config3", "config4", "resolved", "tiny_cut", "edge_off"])
+def test_plinth_removal(B, case):
+    """hk_set_plinth (section 2.1.1): every line's value at the cutting length removed from
+    its bins, against the oracle's plinth option, at the north_star tolerance (the subtraction is part of the
+    definition here, so the tolerance applies to the difference)."""
+    if case in ("config2", "edge_off"):
+        lines, cond, grid, cut = _mini(2, 20_000)
+    elif case == "config3":
+        lines, cond, grid, cut = _mini(3, 200_000)
+    elif case == "config4":
+        lines, cond, grid, cut = _mini(4, 6_000)
+    else:
+        rng = np.random.default_rng(21)
+        n = 1500
+        lines = _simple_lines(np.sort(rng.uniform(995.0, 1025.0, n)), A=10 ** rng.uniform(-3, 2, n),
+                              E_low=rng.uniform(0, 4000, n), gamma_ref=rng.uniform(0.01, 0.2, n))
+        cond, grid = COND, (1000.0, 1020.5, 0.001)
+        cut = 3.0 if case == "resolved" else 0.004            # tiny: the cut falls inside the line cores
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_plinth(True)
+    op.set_edge_nodes(case != "edge_off")
+    k = op.compute(_to_cuda(lines), cut)
+    torch.cuda.synchronize()
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut, plinth=True)
+    k_raw, _ = O.opacity_grid(lines, cond, grid, cut)
+    assert op.stats()["n_evals"] == evals
+    assert (k_ref < k_raw).any()
+    if case == "tiny_cut":
+        # the cut falls inside the cores: S (V - V(cut)) is a small difference of nearly equal numbers on EVERY bin of
+        # every line, so the error is bounded against the unsubtracted opacity (DESIGN.md section 5, plinth row)
+        err = np.abs(k.cpu().numpy() - k_ref)
+        assert (err <= 1e-4 * k_raw + 1e-8 * k_raw.max()).all(), float((err / np.maximum(k_raw, 1e-300)).max())
+        rel, ab = float((err / np.maximum(k_raw, 1e-300)).max()), 0.0
+    else:
+        rel, ab, frac = check_parity(k.cpu().numpy(), k_ref, what=f"plinth {case}")
+    print(f"plinth {case}: rel={rel:.2e} abs={ab:.2e} removed fraction of the integral {1 - k_ref.sum() / k_raw.sum():.3f}")
+    # uncut: no plinth
+    if case == "config2":
+        ku = op.compute(_to_cuda(lines), 0.0)
+        op.set_plinth(False)
+        ku0 = op.compute(_to_cuda(lines), 0.0)
+        torch.cuda.synchronize()
+        assert torch.equal(ku, ku0) or float((ku / ku0 - 1).abs().max()) <= 1e-6
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
