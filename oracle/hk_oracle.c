@@ -206,13 +206,25 @@ double hko_profile(double nu, double nu0, double gammaL, double alphaD)
  * KNOWS no other line can reach these bins (centres sorted, fixed cut) skip
  * them; passing 0, n is the definition.  Neumaier-compensated sum per bin.
  * evals_out (optional) receives the number of (line, bin) evaluations. */
+/* The selectable line profiles of section 2.1 (L47), each of unit area in nu, as a shape K with V = K/(alpha_D sqrt(pi)):
+ *   0 Voigt    K = Re w(x + i y)
+ *   1 Lorentz  V = Gamma_L/(pi ((nu - nu0)^2 + Gamma_L^2))          => K = y/(sqrt(pi) (x^2 + y^2))
+ *   2 Doppler  V = exp(-x^2)/(alpha_D sqrt(pi))                      => K = exp(-x^2)
+ * (the binned Gaussian of ExoCross is not built). */
+static double shape_K(int profile, double x, double y)
+{
+    if (profile == 1) return y / (sqrt(HKO_PI) * (x * x + y * y));
+    if (profile == 2) return exp(-x * x);
+    return hko_voigt_K(x, y);
+}
+
 /* plinth != 0 (and a finite cut): every term is S (V(nu_i - nu0) - V(cut)), the line with its "plinth" -- its own
  * value at the cutting length position -- removed from every bin of its extent (section 2.1.1; DESIGN.md
  * R21: the plinth is the profile AT nu0 +- cut, not at the last grid point inside the extent). */
 void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const double *g,
                          const double *E, const double *gam, const double *nx,
                          double T, double P_atm, double mass_amu, double Q,
-                         double numin, double dnu, int64_t N, double cut, int plinth,
+                         double numin, double dnu, int64_t N, double cut, int plinth, int profile,
                          int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                          double *k_out, int64_t *evals_out);
 
@@ -223,14 +235,14 @@ void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const doubl
                       int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                       double *k_out, int64_t *evals_out)
 {
-    hko_opacity_bins_ex(n, nu0, A, g, E, gam, nx, T, P_atm, mass_amu, Q, numin, dnu, N, cut, 0, nb, bins, l0, l1,
+    hko_opacity_bins_ex(n, nu0, A, g, E, gam, nx, T, P_atm, mass_amu, Q, numin, dnu, N, cut, 0, 0, nb, bins, l0, l1,
                         k_out, evals_out);
 }
 
 void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const double *g,
                          const double *E, const double *gam, const double *nx,
                          double T, double P_atm, double mass_amu, double Q,
-                         double numin, double dnu, int64_t N, double cut, int plinth,
+                         double numin, double dnu, int64_t N, double cut, int plinth, int profile,
                          int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                          double *k_out, int64_t *evals_out)
 {
@@ -251,7 +263,7 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
             line_params(nu0[l], A[l], g[l], E[l], gam[l], nx[l], T, P_atm, mass_amu, Q,
                         &S[q], &gL[q], &aD[q]);
             line_extent(nu0[l], numin, dnu, N, cut, &ilo[q], &ihi[q], &jc);
-            pl[q] = use_plinth ? hko_voigt_K(cut / aD[q], gL[q] / aD[q]) : 0.0;
+            pl[q] = use_plinth ? shape_K(profile, cut / aD[q], gL[q] / aD[q]) : 0.0;
         } else { S[q] = 0.0; gL[q] = 0.0; aD[q] = 1.0; ilo[q] = 0; ihi[q] = -1; pl[q] = 0.0; }
     }
     int64_t evals = 0;
@@ -265,7 +277,7 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
             if (i < ilo[q] || i > ihi[q]) continue;
             double x = (nu - nu0[l0 + q]) / aD[q];
             double y = gL[q] / aD[q];
-            double term = S[q] * (hko_voigt_K(x, y) - pl[q]) / (aD[q] * sqrtpi);
+            double term = S[q] * (shape_K(profile, x, y) - pl[q]) / (aD[q] * sqrtpi);
             double t = sum + term;                 /* Neumaier */
             if (fabs(sum) >= fabs(term)) comp += (sum - t) + term;
             else comp += (term - t) + sum;

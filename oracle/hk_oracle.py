@@ -44,7 +44,7 @@ _lib.hko_opacity_bins.argtypes = [_i64, _pd, _pd, _pd, _pd, _pd, _pd, _d, _d, _d
 
 _lib.hko_opacity_bins_ex.restype = None
 _lib.hko_opacity_bins_ex.argtypes = [_i64, _pd, _pd, _pd, _pd, _pd, _pd, _d, _d, _d, _d,
-                                     _d, _d, _i64, _d, C.c_int, _i64, _pi64, _i64, _i64, _pd,
+                                     _d, _d, _i64, _d, C.c_int, C.c_int, _i64, _pi64, _i64, _i64, _pd,
                                      C.POINTER(_i64)]
 
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
@@ -104,7 +104,10 @@ def profile(nu, nu0, gammaL, alphaD) -> float:
     return float(_lib.hko_profile(nu, nu0, gammaL, alphaD))
 
 
-def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False):
+PROFILES = {"voigt": 0, "lorentz": 1, "doppler": 2}
+
+
+def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False, profile="voigt"):
     """k at the listed bins, brute force over lines [l0, l1).  -> (k, n_evals).
     plinth=True removes every line's value at the cutting length from its bins (section 2.1.1)."""
     a = [_f64(lines[k]) for k in FIELDS]
@@ -117,7 +120,7 @@ def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False):
     numin, numax, dnu = grid
     N = grid_size(numin, numax, dnu)
     _lib.hko_opacity_bins_ex(n, *a, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"],
-                             numin, dnu, N, float(cut), 1 if plinth else 0, bins.size, bins, int(l0), int(l1),
+                             numin, dnu, N, float(cut), 1 if plinth else 0, PROFILES[profile], bins.size, bins, int(l0), int(l1),
                              out, C.byref(ev))
     return out, int(ev.value)
 
@@ -126,19 +129,19 @@ def _uncut(cut) -> bool:
     return not (cut > 0.0 and np.isfinite(cut))
 
 
-def opacity_window(lines_sorted, cond, grid, cut, b0, b1, plinth=False):
+def opacity_window(lines_sorted, cond, grid, cut, b0, b1, plinth=False, profile="voigt"):
     """k on bins [b0, b1) for lines SORTED by nu0 (fixed cut: only lines within
     cut + one bin of the window are passed to the brute-force routine)."""
     numin, numax, dnu = grid
     bins = np.arange(b0, b1, dtype=np.int64)
     nu0 = lines_sorted["nu0"]
     if _uncut(cut):
-        return opacity_bins(lines_sorted, cond, grid, cut, bins, plinth=plinth)
+        return opacity_bins(lines_sorted, cond, grid, cut, bins, plinth=plinth, profile=profile)
     lo = numin + b0 * dnu - cut - 2.0 * dnu
     hi = numin + (b1 - 1) * dnu + cut + 2.0 * dnu
     l0 = int(np.searchsorted(nu0, lo, side="left"))
     l1 = int(np.searchsorted(nu0, hi, side="right"))
-    return opacity_bins(lines_sorted, cond, grid, cut, bins, l0, l1, plinth=plinth)
+    return opacity_bins(lines_sorted, cond, grid, cut, bins, l0, l1, plinth=plinth, profile=profile)
 
 
 def sort_lines(lines):
@@ -149,7 +152,7 @@ def sort_lines(lines):
     return {k: _f64(lines[k])[order] for k in FIELDS}
 
 
-def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=False):
+def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=False, profile="voigt"):
     """k on every bin of the grid.  -> (k[N], n_evals)."""
     numin, numax, dnu = grid
     N = grid_size(numin, numax, dnu)
@@ -160,7 +163,7 @@ def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=Fals
         block = N
     for b0 in range(0, N, block):
         b1 = min(N, b0 + block)
-        kk, ev = opacity_window(ls, cond, grid, cut, b0, b1, plinth=plinth)
+        kk, ev = opacity_window(ls, cond, grid, cut, b0, b1, plinth=plinth, profile=profile)
         k[b0:b1] = kk
         evals += ev
     return k, evals
