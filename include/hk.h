@@ -110,6 +110,16 @@ int64_t hk_grid_size(const hk_ctx* ctx);
  * P >= 0, all finite. */
 int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, double Q);
 
+/* Line profile (section 2.1: Voigt, and "sometimes pure Doppler and Lorentzian profiles are also used"), unit area:
+ *   HK_PROFILE_VOIGT   Re w(x + i y)/(alpha_D sqrt(pi))                      (default)
+ *   HK_PROFILE_LORENTZ Gamma_L/(pi ((nu - nu0)^2 + Gamma_L^2))
+ *   HK_PROFILE_DOPPLER exp(-((nu - nu0)/alpha_D)^2)/(alpha_D sqrt(pi)); values below e^-40 of the peak are dropped
+ * The binned Gaussian of ExoCross (L47) is not built.  HK_EINVAL for any other value. */
+#define HK_PROFILE_VOIGT 0
+#define HK_PROFILE_LORENTZ 1
+#define HK_PROFILE_DOPPLER 2
+int hk_set_profile(hk_ctx* ctx, int profile);
+
 /* Plinth removal (section 2.1.1): on != 0 subtracts from every bin of a line's extent that line's own value
  * at the cutting length position, S V(nu0 +- cut) (needed with continua that already hold the plinths, e.g. CKD).
  * Off by default; no effect on uncut computations.  Changes hk_workspace_bytes (+ 8 B per bin): set it before the

@@ -28,6 +28,7 @@ struct hk_ctx {
     double node_sep;
     int edge_nodes;
     int plinth;
+    int profile;
     int n_sm;
     // last compute
     bool have_run;
@@ -160,8 +161,10 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
         p.kmin = -(1LL << 30);
         p.ksent = INT32_MAX;
     }
+    p.profile = c->profile;
     p.kappa1 = std::sqrt((double)HK_Z1) * p.beta * 1.001;
     p.kappa2 = std::sqrt((double)HK_Z2) * p.beta * 1.001;
+    if (p.profile == HK_PROFILE_LORENTZ) p.kappa1 = p.kappa2 = 0.0;      // no core, no second term: every pair is "far"
     p.inv1p_k1 = 1.0 / (1.0 + p.kappa1); p.inv1m_k1 = 1.0 / (1.0 - p.kappa1);
     p.inv1p_k2 = 1.0 / (1.0 + p.kappa2); p.inv1m_k2 = 1.0 / (1.0 - p.kappa2);
     p.numin_bins = c->numin / c->dnu;
@@ -338,6 +341,13 @@ int hk_set_node_separation(hk_ctx* ctx, double sep)
     return HK_OK;
 }
 
+int hk_set_profile(hk_ctx* ctx, int profile)
+{
+    if (!ctx || profile < HK_PROFILE_VOIGT || profile > HK_PROFILE_DOPPLER) return HK_EINVAL;
+    ctx->profile = profile;
+    return HK_OK;
+}
+
 int hk_set_plinth(hk_ctx* ctx, int on)
 {
     if (!ctx) return HK_EINVAL;
@@ -421,7 +431,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     if (!reuse_sort)
         HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                                 (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
-    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB, recN);
+    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB, recN, p.profile);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges, node ranges and work units.  counts = [far | mid | edge | centre | near | node | 0], one scan.
     const int n_counts = 5 * p.n_ct + lv.n_entries + 1;

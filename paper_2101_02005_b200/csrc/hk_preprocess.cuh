@@ -36,6 +36,7 @@ struct Params {
     int32_t chunk;              // lines per work unit of the direct kernels
     int32_t chunk_node;         // lines per work unit of the node kernel
     double sep;                 // node separation: |centre - tile centre| >= sep * half-width
+    int profile;                // 0 Voigt, 1 Lorentz (records carry alpha_D = 0), 2 Doppler (records carry Gamma_L = 0)
     int plinth;                 // 1: remove every line's value at the cutting length from its bins (section 2.1.1)
     double cut_bins;            // cut / dnu
     int edge_nodes;             // 1: separated edge tiles go through per-bin node accumulators (edge_node_kernel)
@@ -139,7 +140,7 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
             ++off;
             r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);
         } else {
-            double Gb = o.gammaL / p.dnu, ab = o.alphaD / p.dnu;
+            double Gb = p.profile == HK_PROFILE_DOPPLER ? 0.0 : o.gammaL / p.dnu, ab = o.alphaD / p.dnu;
             r.jc = (int32_t)o.jc;
             r.f = fminf((float)o.pos_f, 0.99999994f);
             r.G2 = (float)(Gb * Gb);
@@ -153,10 +154,11 @@ __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __res
             cKmaxb = max(cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
             evals += (unsigned long long)(o.ihi - o.ilo + 1);
             double pos = (double)o.jc + o.pos_f;
+            if (p.profile == HK_PROFILE_LORENTZ) ab = 0.0;                // region counters: a Lorentzian has no core
             double t1 = (double)HK_Z1 * ab * ab - Gb * Gb, t2 = (double)HK_Z2 * ab * ab - Gb * Gb;
             cmid += (unsigned long long)count_within(pos, t1 > 0 ? (double)sqrtf((float)t1) : 0.0, o.ilo, o.ihi);
             ccore += (unsigned long long)count_within(pos, t2 > 0 ? (double)sqrtf((float)t2) : 0.0, o.ilo, o.ihi);
-            const double y2 = (Gb * Gb) / (ab * ab);
+            const double y2 = ab > 0.0 ? (Gb * Gb) / (ab * ab) : 1.0e300;
             const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
             cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? (double)sqrtf((float)t4) : 0.0, o.ilo, o.ihi);
             const unsigned long long ntrap = (unsigned long long)count_within(pos, t3 > 0 ? (double)sqrtf((float)t3) : 0.0, o.ilo, o.ihi);
@@ -209,7 +211,7 @@ __global__ void scale_kernel(DevStats* st)
 __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ idx_sorted,
                                                      int64_t n, const DevStats* __restrict__ st,
                                                      float4* __restrict__ recA, float4* __restrict__ recB,
-                                                     float4* __restrict__ recN)
+                                                     float4* __restrict__ recN, int profile)
 {
     const int e = st->scale_exp;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
@@ -217,10 +219,13 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
         float cK = (float)scalbn(r.cK, e);
         // c = cK * G a / sqrt(pi)  (Lorentz amplitude S Gamma_L/(pi dnu^2) in bin units)
         float c = cK * sqrtf(r.G2 * r.a2) * 0.564189583547756f;
+        // a pure Lorentzian is what every formula of the accumulation kernels reduces to at alpha_D = 0 (no core,
+        // no second asymptotic term); a pure Gaussian is the Voigt function at Gamma_L = 0 (c = 0: no wings)
+        const float a2 = profile == HK_PROFILE_LORENTZ ? 0.f : r.a2;
         recA[i] = make_float4(__int_as_float(r.jc), r.f, r.G2, c);
-        recB[i] = make_float4(r.a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
+        recB[i] = make_float4(a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
         const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn(r.f * 8192.0f));
-        const uint32_t a19 = ((uint32_t)__float_as_int(r.a2) >> 12) & 0x7FFFFu;
+        const uint32_t a19 = ((uint32_t)__float_as_int(a2) >> 12) & 0x7FFFFu;
         recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), r.G2, c);
     }
 }

@@ -290,6 +290,41 @@ def test_plinth_removal(B, case):
     op.close()
 
 
+@pytest.mark.parametrize("profile", ["lorentz", "doppler"])
+@pytest.mark.parametrize("case", ["config2", "config3", "resolved", "uncut"])
+def test_lorentz_and_doppler_profiles(B, profile, case):
+    """hk_set_profile (section 2.1) against the oracle's profile options, with and
+    without plinth removal."""
+    if case == "config2":
+        lines, cond, grid, cut = _mini(2, 20_000)
+    elif case == "config3":
+        lines, cond, grid, cut = _mini(3, 200_000)
+    elif case == "uncut":
+        lines, cond, grid, cut = _mini(5, 300)
+        grid = (grid[0], 5000.0, grid[2])
+    else:
+        rng = np.random.default_rng(22)
+        n = 1500
+        lines = _simple_lines(np.sort(rng.uniform(995.0, 1025.0, n)), A=10 ** rng.uniform(-3, 2, n),
+                              E_low=rng.uniform(0, 4000, n), gamma_ref=rng.uniform(0.01, 0.2, n))
+        cond, grid, cut = COND, (1000.0, 1020.5, 0.001), 3.0
+    dl = _to_cuda(lines)
+    for plinth in (False, True):
+        op = B.Opacity(*grid)
+        op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        op.set_profile(profile)
+        op.set_plinth(plinth)
+        k = op.compute(dl, cut)
+        torch.cuda.synchronize()
+        k_ref, evals = O.opacity_grid(lines, cond, grid, cut, plinth=plinth, profile=profile)
+        assert op.stats()["n_evals"] == evals
+        rel, ab, frac = check_parity(k.cpu().numpy(), k_ref, what=f"{profile} {case} plinth={plinth}")
+        print(f"{profile} {case} plinth={plinth}: rel={rel:.2e} abs={ab:.2e} frac_rel={frac:.3f}")
+        op.close()
+    with pytest.raises(B.HKError):
+        B.Opacity(*grid).set_profile(7)
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
