@@ -289,3 +289,77 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
     if (evals_out) *evals_out = evals;
     free(S); free(gL); free(aD); free(ilo); free(ihi); free(pl);
 }
+
+/* ---- HITRAN-style inputs --------------------------------------------
+ * Per line: nu0, A, g', E'', gamma_air, gamma_self, n, delta (Table 3-4) and an isotopologue index into a
+ * table of (mass, Q(T), abundance) (species parameter file, L371-373, Table 2).
+ *   Gamma_L = A/(4 pi c) + (T/T_ref)^-n [gamma_air (P - P_self)/P_ref + gamma_self P_self/P_ref]        (Eq. 4)
+ *   centre  = nu0 + delta P      (pressure shift, L238, Table 4 "pressure-dependent line shift", cm^-1/atm; R23:
+ *                                 the profile and the extent are centred there, S and alpha_D use the tabulated nu0)
+ *   alpha_D = (nu0/c) sqrt(2 k_B T/m_iso),  S = abundance_iso x Eq. 9 with m_iso and Q_iso               (R24)
+ * A line with an isotopologue index outside the table, or a non-finite field, contributes nothing (R14). */
+static int line_valid_hitran(double nu0, double A, double g, double E, double ga, double gs, double nx, double dl,
+                             int32_t iso, int32_t n_iso)
+{
+    return isfinite(nu0) && isfinite(A) && isfinite(g) && isfinite(E) && isfinite(ga) && isfinite(gs) &&
+           isfinite(nx) && isfinite(dl) && nu0 > 0.0 && A >= 0.0 && iso >= 0 && iso < n_iso;
+}
+
+void hko_line_params_hitran(int64_t n, const double *nu0, const double *A, const double *g, const double *E,
+                            const double *ga, const double *gs, const double *nx, const double *dl, const int32_t *iso,
+                            double T, double P_atm, double P_self, int32_t n_iso, const double *mass_amu,
+                            const double *Q, const double *abund,
+                            double *S, double *gammaL, double *alphaD, double *centre, int32_t *valid)
+{
+    const double c2 = HKO_H * HKO_C / HKO_KB;
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < n; ++l) {
+        int v = line_valid_hitran(nu0[l], A[l], g[l], E[l], ga[l], gs[l], nx[l], dl[l], iso[l], n_iso);
+        valid[l] = v;
+        S[l] = 0.0; gammaL[l] = 0.0; alphaD[l] = 0.0; centre[l] = 0.0;
+        if (!v) continue;
+        const double m = mass_amu[iso[l]] / HKO_NA;
+        alphaD[l] = (nu0[l] / HKO_C) * sqrt(2.0 * HKO_KB * T / m);
+        gammaL[l] = A[l] / (4.0 * HKO_PI * HKO_C)
+                    + pow(T / HKO_TREF, -nx[l]) * (ga[l] * (P_atm - P_self) + gs[l] * P_self);     /* P_ref = 1 atm */
+        S[l] = abund[iso[l]] * A[l] * g[l] / (8.0 * HKO_PI * HKO_C * m * nu0[l] * nu0[l] * Q[iso[l]])
+               * exp(-c2 * E[l] / T) * (-expm1(-c2 * nu0[l] / T));
+        centre[l] = nu0[l] + dl[l] * P_atm;
+    }
+}
+
+/* k at the listed bins from already computed per-line parameters: the same brute-force sum as hko_opacity_bins
+ * (membership by the integer extent of the shifted centre, Neumaier-compensated). */
+void hko_opacity_bins_params(int64_t n, const double *centre, const double *S, const double *gammaL,
+                             const double *alphaD, const int32_t *valid, double numin, double dnu, int64_t N, double cut,
+                             int64_t nb, const int64_t *bins, double *k_out, int64_t *evals_out)
+{
+    int64_t *ilo = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n + 1));
+    int64_t *ihi = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n + 1));
+#pragma omp parallel for schedule(static)
+    for (int64_t l = 0; l < n; ++l) {
+        int64_t jc;
+        if (valid[l]) line_extent(centre[l], numin, dnu, N, cut, &ilo[l], &ihi[l], &jc);
+        else { ilo[l] = 0; ihi[l] = -1; }
+    }
+    int64_t evals = 0;
+    const double sqrtpi = sqrt(HKO_PI);
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : evals)
+    for (int64_t b = 0; b < nb; ++b) {
+        int64_t i = bins[b];
+        double nu = numin + (double)i * dnu;
+        double sum = 0.0, comp = 0.0;
+        for (int64_t l = 0; l < n; ++l) {
+            if (i < ilo[l] || i > ihi[l]) continue;
+            double term = S[l] * hko_voigt_K((nu - centre[l]) / alphaD[l], gammaL[l] / alphaD[l]) / (alphaD[l] * sqrtpi);
+            double t = sum + term;
+            if (fabs(sum) >= fabs(term)) comp += (sum - t) + term;
+            else comp += (term - t) + sum;
+            sum = t;
+            ++evals;
+        }
+        k_out[b] = sum + comp;
+    }
+    if (evals_out) *evals_out = evals;
+    free(ilo); free(ihi);
+}

@@ -167,3 +167,57 @@ def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=Fals
         k[b0:b1] = kk
         evals += ev
     return k, evals
+
+
+# ---- HITRAN-style inputs -------------------------------------------------
+HITRAN_FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_air", "gamma_self", "n_exp", "delta")
+_lib.hko_line_params_hitran.restype = None
+_lib.hko_line_params_hitran.argtypes = [_i64] + [_pd] * 8 + [_pi32, _d, _d, _d, C.c_int32, _pd, _pd, _pd,
+                                                          _pd, _pd, _pd, _pd, _pi32]
+_lib.hko_opacity_bins_params.restype = None
+_lib.hko_opacity_bins_params.argtypes = [_i64, _pd, _pd, _pd, _pd, _pi32, _d, _d, _i64, _d, _i64, _pi64, _pd,
+                                         C.POINTER(_i64)]
+
+
+def line_params_hitran(lines, cond):
+    """cond: T, P_atm, P_self_atm, isos = [(mass_amu, Q, abundance), ...].
+    -> S, gammaL, alphaD, centre (= nu0 + delta P), valid."""
+    a = [_f64(lines[k]) for k in HITRAN_FIELDS]
+    iso = np.ascontiguousarray(lines["iso"], dtype=np.int32)
+    n = a[0].size
+    isos = np.asarray(cond["isos"], dtype=np.float64).reshape(-1, 3)
+    S, gL, aD, ctr = (np.empty(n) for _ in range(4))
+    valid = np.empty(n, dtype=np.int32)
+    _lib.hko_line_params_hitran(n, *a, iso, cond["T"], cond["P_atm"], cond["P_self_atm"], isos.shape[0],
+                                _f64(isos[:, 0]), _f64(isos[:, 1]), _f64(isos[:, 2]), S, gL, aD, ctr, valid)
+    return S, gL, aD, ctr, valid
+
+
+def opacity_grid_hitran(lines, cond, grid, cut, block=512):
+    """k on every bin for HITRAN-style lines.  -> (k[N], n_evals)."""
+    numin, numax, dnu = grid
+    N = grid_size(numin, numax, dnu)
+    S, gL, aD, ctr, valid = line_params_hitran(lines, cond)
+    order = np.argsort(np.where(valid > 0, ctr, np.inf), kind="stable")
+    S, gL, aD, ctr, valid = (np.ascontiguousarray(v[order]) for v in (S, gL, aD, ctr, valid))
+    nv = int((valid > 0).sum())
+    k = np.zeros(N)
+    evals = 0
+    step = N if _uncut(cut) else block
+    for b0 in range(0, N, step):
+        b1 = min(N, b0 + step)
+        if _uncut(cut):
+            l0, l1 = 0, nv
+        else:                      # a caller's knowledge: no line further than the cut (+ a bin) from the block reaches it
+            l0 = int(np.searchsorted(ctr[:nv], numin + b0 * dnu - cut - 2.0 * dnu, side="left"))
+            l1 = int(np.searchsorted(ctr[:nv], numin + (b1 - 1) * dnu + cut + 2.0 * dnu, side="right"))
+        bins = np.arange(b0, b1, dtype=np.int64)
+        out = np.empty(bins.size)
+        ev = _i64(0)
+        sl = slice(l0, l1)
+        _lib.hko_opacity_bins_params(l1 - l0, _f64(ctr[sl]), _f64(S[sl]), _f64(gL[sl]), _f64(aD[sl]),
+                                     np.ascontiguousarray(valid[sl]), numin, dnu, N, float(cut), bins.size, bins, out,
+                                     C.byref(ev))
+        k[b0:b1] = out
+        evals += int(ev.value)
+    return k, evals
