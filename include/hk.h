@@ -156,6 +156,43 @@ int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cu
 int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond,
                      const double* T_K, const double* P_atm, const double* Q, double* out_k_dev, void* stream);
 
+/* ---- HITRAN-style inputs (Table 3-4: nu, E_L, A, delta, gamma_air, gamma_self, n per line) -----------
+ * Nine SoA DEVICE arrays of n_lines elements, read-only: eight fp64 and the int32 isotopologue index of each line
+ * into the table given to hk_set_conditions_hitran (the species parameter file's isotopologue list, L371-373). */
+typedef struct {
+    const double* nu0;        /* tabulated line centre, cm^-1 */
+    const double* A;          /* Einstein A, s^-1 */
+    const double* g_up;       /* upper-state degeneracy */
+    const double* E_low;      /* lower-state energy, cm^-1 */
+    const double* gamma_air;  /* air-broadening coefficient at T_ref, cm^-1/atm */
+    const double* gamma_self; /* self-broadening coefficient at T_ref, cm^-1/atm */
+    const double* n_exp;      /* temperature exponent n */
+    const double* delta;      /* pressure shift, cm^-1/atm */
+    const int32_t* iso;       /* isotopologue index, 0 .. n_iso-1 */
+} hk_lines_hitran;
+
+/* Conditions for HITRAN-style lists:
+ *   Gamma_L = A/(4 pi c) + (T/T_ref)^-n [gamma_air (P - P_self)/P_ref + gamma_self P_self/P_ref]        (Eq. 4)
+ *   centre  = nu0 + delta P        (pressure shift, L238; the reason the paper re-sorts the lines)
+ *   alpha_D = (nu0/c) sqrt(2 k_B T/m_iso);  S = abundance_iso x Eq. 9 with m_iso and Q_iso(T)
+ * The profile and the integer extent are centred on the SHIFTED centre; S and alpha_D use the tabulated nu0
+ * (R23, R24).  mass_amu, Q, abundance: HOST arrays of n_iso (1..16) entries.  HK_EINVAL unless T > 0,
+ * 0 <= P_self <= P, masses and Q > 0, abundances >= 0, all finite.  A line whose iso is outside the table contributes
+ * nothing (counted in n_skipped).  Also sets the ExoMol-style conditions to (T, P, mass[0], Q[0]). */
+int hk_set_conditions_hitran(hk_ctx* ctx, double T_K, double P_atm, double P_self_atm, int32_t n_iso,
+                             const double* mass_amu, const double* Q, const double* abundance);
+
+/* hk_compute for a HITRAN-style list: same hot path after the per-line preprocessing; workspace as hk_compute
+ * (hk_workspace_bytes).  HK_ESTATE before hk_set_conditions_hitran. */
+int hk_compute_hitran(hk_ctx* ctx, const hk_lines_hitran* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
+                      void* stream);
+
+/* Per-line parameters and integer extents (of the shifted centre, for cut_cm) as the preprocess kernel computes
+ * them: parity of step a1 for HITRAN-style lists.  DEVICE arrays of n_lines, any may be NULL.  Synchronises. */
+int hk_get_line_params_hitran(hk_ctx* ctx, const hk_lines_hitran* lines, int64_t n_lines, double cut_cm, double* S_dev,
+                              double* gammaL_dev, double* alphaD_dev, int32_t* ilo_dev, int32_t* ihi_dev,
+                              int32_t* jc_dev, void* stream);
+
 /* Host-buffer entry (the paper's block pipeline, L183-189, Fig. 6): the six line
  * arrays and out_k are HOST pointers (pinned memory gives asynchronous copies; pageable
  * works, slower).  The list is cut into blocks of block_lines lines (<= 0: default 2^25);

@@ -27,12 +27,20 @@ EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_w
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile",
+           "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
            "hk_last_cuda_error", "hk_strerror")
 PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "near", "down")
 
 
 class hk_lines(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in FIELDS]
+
+
+HITRAN_FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_air", "gamma_self", "n_exp", "delta")
+
+
+class hk_lines_hitran(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k in HITRAN_FIELDS] + [("iso", C.c_void_p)]
 
 
 class hk_stats(C.Structure):
@@ -58,6 +66,12 @@ _lib.hk_accumulate.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
 _lib.hk_compute_batch.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, C.c_int32, C.POINTER(_d), C.POINTER(_d), C.POINTER(_d),
                                   _vp, _vp]
 _lib.hk_compute_batch.restype = C.c_int
+_lib.hk_set_conditions_hitran.argtypes = [_vp, _d, _d, _d, C.c_int32, C.POINTER(_d), C.POINTER(_d), C.POINTER(_d)]
+_lib.hk_set_conditions_hitran.restype = C.c_int
+_lib.hk_compute_hitran.argtypes = [_vp, C.POINTER(hk_lines_hitran), _i64, _d, _vp, _vp]
+_lib.hk_compute_hitran.restype = C.c_int
+_lib.hk_get_line_params_hitran.argtypes = [_vp, C.POINTER(hk_lines_hitran), _i64, _d, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.hk_get_line_params_hitran.restype = C.c_int
 _lib.hk_workspace_bytes_host.argtypes = [_vp, _i64, _i64]
 _lib.hk_workspace_bytes_host.restype = C.c_size_t
 _lib.hk_compute_host.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _i64, _vp]
@@ -109,6 +123,22 @@ def _lines_struct(lines, host=False):
         t = lines[k]
         if not (t.is_cuda != host and t.dtype == torch.float64 and t.is_contiguous()):
             raise ValueError(f"lines[{k!r}] must be a contiguous {'CPU' if host else 'CUDA'} float64 tensor")
+        if n is None:
+            n = t.numel()
+        elif t.numel() != n:
+            raise ValueError("line arrays differ in length")
+        setattr(ls, k, t.data_ptr())
+    return ls, n
+
+
+def _hitran_struct(lines):
+    ls = hk_lines_hitran()
+    n = None
+    for k in HITRAN_FIELDS + ("iso",):
+        t = lines[k]
+        want = torch.int32 if k == "iso" else torch.float64
+        if not (t.is_cuda and t.dtype == want and t.is_contiguous()):
+            raise ValueError(f"lines[{k!r}] must be a contiguous CUDA {want} tensor")
         if n is None:
             n = t.numel()
         elif t.numel() != n:
@@ -202,6 +232,36 @@ class Opacity:
         self._check(_lib.hk_compute_batch(self._ctx, C.byref(ls), n, cut, nc, arr(T), arr(P_atm), arr(Q), out.data_ptr(),
                                           _stream_ptr(stream)), "hk_compute_batch")
         return out
+
+    def set_conditions_hitran(self, T, P_atm, P_self_atm, isos):
+        """isos: [(mass_amu, Q, abundance), ...] (hk_set_conditions_hitran)."""
+        n = len(isos)
+        arr = lambda j: (_d * n)(*[float(x[j]) for x in isos])
+        self._check(_lib.hk_set_conditions_hitran(self._ctx, T, P_atm, P_self_atm, n, arr(0), arr(1), arr(2)),
+                    "hk_set_conditions_hitran")
+
+    def compute_hitran(self, lines, cut, out=None, stream=None):
+        """hk_compute_hitran: HITRAN-style lines (HITRAN_FIELDS + int32 'iso') -> k(nu)."""
+        ls, n = _hitran_struct(lines)
+        self.ensure_workspace(n)
+        if out is None:
+            out = torch.empty(self.N, dtype=torch.float64, device="cuda")
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.N
+        cut = float(cut) if cut is not None else 0.0
+        self._check(_lib.hk_compute_hitran(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)),
+                    "hk_compute_hitran")
+        return out
+
+    def line_params_hitran(self, lines, cut, stream=None):
+        """-> S, gammaL, alphaD (fp64), ilo, ihi, jc (int32) of HITRAN-style lines."""
+        ls, n = _hitran_struct(lines)
+        S, gL, aD = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+        ilo, ihi, jc = (torch.empty(n, dtype=torch.int32, device="cuda") for _ in range(3))
+        cut = float(cut) if cut is not None else 0.0
+        self._check(_lib.hk_get_line_params_hitran(self._ctx, C.byref(ls), n, cut, S.data_ptr(), gL.data_ptr(), aD.data_ptr(),
+                                                   ilo.data_ptr(), ihi.data_ptr(), jc.data_ptr(), _stream_ptr(stream)),
+                    "hk_get_line_params_hitran")
+        return S, gL, aD, ilo, ihi, jc
 
     def compute_host(self, host_lines, cut, out=None, block_lines=0, stream=None):
         """Host-buffer entry (hk_compute_host): CPU fp64 tensors in (pinned for async copies), CPU fp64

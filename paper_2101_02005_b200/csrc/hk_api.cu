@@ -29,6 +29,11 @@ struct hk_ctx {
     int edge_nodes;
     int plinth;
     int profile;
+    // HITRAN-style conditions (hk_set_conditions_hitran)
+    bool have_hitran;
+    double P_self;
+    int32_t n_iso;
+    double iso_mass[kMaxIso], iso_Q[kMaxIso], iso_ab[kMaxIso];
     int n_sm;
     // last compute
     bool have_run;
@@ -133,7 +138,7 @@ int fail_cuda(hk_ctx* c, cudaError_t e)
     } while (0)
 
 // Fill the per-launch constants (step a0).
-Params make_params(const hk_ctx* c, double cut, int32_t chunk)
+Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = false)
 {
     Params p;
     std::memset(&p, 0, sizeof(p));
@@ -148,6 +153,18 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk)
     p.beta = std::sqrt(2.0 * kKB * c->T / m) / kC;
     p.sfac = 1.0 / (8.0 * kPi * kC * m * c->Q);
     p.inv4pic = 1.0 / (4.0 * kPi * kC);
+    if (hitran) {
+        // per isotopologue: Doppler factor and abundance / (8 pi c m Q); the tile bounds use the widest Doppler factor
+        p.P_self = c->P_self;
+        p.n_iso = c->n_iso;
+        p.beta = 0.0;
+        for (int j = 0; j < c->n_iso; ++j) {
+            const double mj = c->iso_mass[j] / kNA;
+            p.beta_iso[j] = std::sqrt(2.0 * kKB * c->T / mj) / kC;
+            p.sfac_iso[j] = c->iso_ab[j] / (8.0 * kPi * kC * mj * c->iso_Q[j]);
+            if (p.beta_iso[j] > p.beta) p.beta = p.beta_iso[j];
+        }
+    }
     p.uncut = is_uncut(cut) ? 1 : 0;
     p.cut = p.uncut ? 0.0 : cut;
     double cb = p.uncut ? 0.0 : cut / c->dnu;
@@ -226,11 +243,12 @@ int bits_for(uint32_t v)
 __global__ void __launch_bounds__(256) extents_kernel(Params p, const double* __restrict__ nu0, const double* __restrict__ A,
                                                       const double* __restrict__ g, const double* __restrict__ E,
                                                       const double* __restrict__ gam, const double* __restrict__ nx,
-                                                      int64_t n, int32_t* ilo, int32_t* ihi, int32_t* jc, double* S,
-                                                      double* gL, double* aD)
+                                                      LineExtra ex, int64_t n, int32_t* ilo, int32_t* ihi, int32_t* jc,
+                                                      double* S, double* gL, double* aD)
 {
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        LineOut o = line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
+        LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
         bool live = o.valid && o.ilo <= o.ihi;
         if (ilo) ilo[i] = live ? (int32_t)o.ilo : 0;
         if (ihi) ihi[i] = live ? (int32_t)o.ihi : -1;
@@ -370,7 +388,7 @@ int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane)
 }
 
 static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
-                        cudaStream_t stream, bool zero_out, bool reuse_sort = false)
+                        cudaStream_t stream, bool zero_out, bool reuse_sort = false, const LineExtra* extra = nullptr)
 {
     if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL) return HK_EINVAL;
     if (std::isnan(cut_cm)) return HK_EINVAL;
@@ -381,7 +399,8 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     char* ws = (char*)ctx->ws;
     DevStats* st = (DevStats*)(ws + L.stats);
     const int n = (int)n_lines;
-    Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm));
+    Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm), extra != nullptr);
+    const LineExtra ex = extra ? *extra : LineExtra{nullptr, nullptr, nullptr};
     p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes) ? 1 : 0;
 
     HK_CUDA(cudaEventRecord(ctx->ev[0], stream));
@@ -420,7 +439,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
 
     // a1: per-line parameters, keys
     line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
-                                                      lines->n_exp, n, recU, keys_in, idx_in, st);
+                                                      lines->n_exp, ex, n, recU, keys_in, idx_in, st);
     scale_kernel<<<1, 1, 0, stream>>>(st);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
     // a2: order by centre bin
@@ -668,8 +687,8 @@ int hk_get_extents(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, int32_t*
     if (n_lines > 0) {
         const Params p = make_params(ctx, ctx->last_cut, 512);
         extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
-                                                                   lines->gamma_ref, lines->n_exp, n_lines, ilo_dev,
-                                                                   ihi_dev, jc_dev, nullptr, nullptr, nullptr);
+                                                                   lines->gamma_ref, lines->n_exp, LineExtra{nullptr, nullptr, nullptr},
+                                                                   n_lines, ilo_dev, ihi_dev, jc_dev, nullptr, nullptr, nullptr);
         HK_CUDA(cudaGetLastError());
     }
     HK_CUDA(cudaStreamSynchronize(stream));
@@ -685,8 +704,68 @@ int hk_get_line_params(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, doub
     if (n_lines > 0) {
         const Params p = make_params(ctx, 0.0, 512);
         extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
-                                                                   lines->gamma_ref, lines->n_exp, n_lines, nullptr,
-                                                                   nullptr, nullptr, S_dev, gammaL_dev, alphaD_dev);
+                                                                   lines->gamma_ref, lines->n_exp, LineExtra{nullptr, nullptr, nullptr},
+                                                                   n_lines, nullptr, nullptr, nullptr, S_dev, gammaL_dev, alphaD_dev);
+        HK_CUDA(cudaGetLastError());
+    }
+    HK_CUDA(cudaStreamSynchronize(stream));
+    return HK_OK;
+}
+
+// ---- HITRAN-style inputs ------------------------------------------------------------------
+namespace {
+bool hitran_ok(const hk_lines_hitran* l)
+{
+    return l && l->nu0 && l->A && l->g_up && l->E_low && l->gamma_air && l->gamma_self && l->n_exp && l->delta && l->iso;
+}
+hk_lines as_lines(const hk_lines_hitran* l)
+{
+    return hk_lines{l->nu0, l->A, l->g_up, l->E_low, l->gamma_air, l->n_exp};
+}
+}  // namespace
+
+int hk_set_conditions_hitran(hk_ctx* ctx, double T_K, double P_atm, double P_self_atm, int32_t n_iso, const double* mass_amu,
+                             const double* Q, const double* abundance)
+{
+    if (!ctx || n_iso < 1 || n_iso > kMaxIso || !mass_amu || !Q || !abundance) return HK_EINVAL;
+    if (!std::isfinite(T_K) || !std::isfinite(P_atm) || !std::isfinite(P_self_atm)) return HK_EINVAL;
+    if (!(T_K > 0.0) || !(P_atm >= 0.0) || !(P_self_atm >= 0.0) || !(P_self_atm <= P_atm)) return HK_EINVAL;
+    for (int j = 0; j < n_iso; ++j) {
+        if (!std::isfinite(mass_amu[j]) || !std::isfinite(Q[j]) || !std::isfinite(abundance[j])) return HK_EINVAL;
+        if (!(mass_amu[j] > 0.0) || !(Q[j] > 0.0) || !(abundance[j] >= 0.0)) return HK_EINVAL;
+    }
+    ctx->T = T_K; ctx->P_atm = P_atm; ctx->P_self = P_self_atm; ctx->n_iso = n_iso;
+    for (int j = 0; j < n_iso; ++j) { ctx->iso_mass[j] = mass_amu[j]; ctx->iso_Q[j] = Q[j]; ctx->iso_ab[j] = abundance[j]; }
+    ctx->mass_amu = mass_amu[0]; ctx->Q = Q[0];           // the ExoMol-style entry points see isotopologue 0
+    ctx->have_cond = true;
+    ctx->have_hitran = true;
+    return HK_OK;
+}
+
+int hk_compute_hitran(hk_ctx* ctx, const hk_lines_hitran* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
+                      void* stream_v)
+{
+    if (!ctx || n_lines < 0 || (n_lines > 0 && !hitran_ok(lines))) return HK_EINVAL;
+    if (!ctx->have_hitran) return HK_ESTATE;
+    hk_lines base = n_lines > 0 ? as_lines(lines) : hk_lines{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    LineExtra ex = n_lines > 0 ? LineExtra{lines->gamma_self, lines->delta, lines->iso} : LineExtra{nullptr, nullptr, nullptr};
+    return compute_impl(ctx, &base, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true, false, &ex);
+}
+
+int hk_get_line_params_hitran(hk_ctx* ctx, const hk_lines_hitran* lines, int64_t n_lines, double cut_cm, double* S_dev,
+                              double* gammaL_dev, double* alphaD_dev, int32_t* ilo_dev, int32_t* ihi_dev, int32_t* jc_dev,
+                              void* stream_v)
+{
+    if (!ctx || n_lines < 0 || (n_lines > 0 && !hitran_ok(lines)) || std::isnan(cut_cm)) return HK_EINVAL;
+    if (!ctx->have_hitran) return HK_ESTATE;
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    if (n_lines > 0) {
+        const Params p = make_params(ctx, cut_cm, 512, true);
+        extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
+                                                                   lines->gamma_air, lines->n_exp,
+                                                                   LineExtra{lines->gamma_self, lines->delta, lines->iso},
+                                                                   n_lines, ilo_dev, ihi_dev, jc_dev, S_dev, gammaL_dev,
+                                                                   alphaD_dev);
         HK_CUDA(cudaGetLastError());
     }
     HK_CUDA(cudaStreamSynchronize(stream));

@@ -8,6 +8,15 @@
 
 namespace hk {
 
+constexpr int kMaxIso = 16;               // isotopologues per species (HITRAN-style inputs)
+
+// extra per-line arrays of HITRAN-style inputs (all null for ExoMol-style lists)
+struct LineExtra {
+    const double* gam_self;
+    const double* delta;
+    const int32_t* iso;
+};
+
 struct Params {
     // grid
     double numin, dnu;
@@ -20,6 +29,10 @@ struct Params {
     double beta;          // sqrt(2 k_B T / m) / c     (alpha_D = beta nu0)
     double sfac;          // 1 / (8 pi c m Q)
     double inv4pic;       // 1 / (4 pi c)
+    // HITRAN-style inputs (n_iso > 0): Eq. 4 self pressure, per-isotopologue beta and abundance / (8 pi c m Q)
+    double P_self;
+    int32_t n_iso;
+    double beta_iso[kMaxIso], sfac_iso[kMaxIso];
     // cut
     double cut;           // cm^-1 (ignored when uncut)
     int uncut;
@@ -76,19 +89,31 @@ struct LineOut {
 
 // The fp64 arithmetic of step a1.  Extents use IEEE operations in exactly the order
 // SURVEY.md 8(c).4 states (no contraction: explicit _rn intrinsics).
+// gs, dl, iso: gamma_self, pressure shift and isotopologue index of HITRAN-style inputs (ignored when p.n_iso == 0)
 __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double A, double g, double E,
-                                             double gam, double nx)
+                                             double gam, double nx, double gs = 0.0, double dl = 0.0, int32_t iso = 0)
 {
     LineOut o;
     o.valid = finite6(nu0, A, g, E, gam, nx) && nu0 > 0.0 && A >= 0.0;
+    if (p.n_iso > 0) o.valid = o.valid && isfinite(gs) && isfinite(dl) && iso >= 0 && iso < p.n_iso;
     o.on_grid = false;
     o.S = o.gammaL = o.alphaD = 0.0;
     o.jc = 0; o.ilo = 0; o.ihi = -1; o.pos_f = 0.0;
     if (!o.valid) return o;
+    double ctr = nu0;                                                          // centre of the profile and of the extent
+    if (p.n_iso > 0) {
+        // Eq. 4 (L87), pressure shift (L238, Table 4), isotopologue table (L371-373); R23, R24
+        o.alphaD = p.beta_iso[iso] * nu0;
+        o.gammaL = A * p.inv4pic + exp(nx * p.ln_tfac) * (gam * (p.P_atm - p.P_self) + gs * p.P_self);
+        o.S = A * g * p.sfac_iso[iso] / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));
+        ctr = nu0 + dl * p.P_atm;
+    } else {
     o.alphaD = p.beta * nu0;                                                   // Eq. 13 (L203)
     o.gammaL = A * p.inv4pic + gam * exp(nx * p.ln_tfac) * p.P_atm;            // Eq. 5 (L91): (T_ref/T)^n = e^(n ln(T_ref/T))
     o.S = A * g * p.sfac / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));  // Eq. 9 (L127)
+    }
     const double big = 4.0e18;
+    nu0 = ctr;
     double pos = __ddiv_rn(__dsub_rn(nu0, p.numin), p.dnu);
     double c = floor(pos);
     c = fmin(fmax(c, -big), big);
@@ -124,13 +149,14 @@ __device__ __forceinline__ int64_t count_within(double pos, double T, int64_t il
 __global__ void __launch_bounds__(256) line_kernel(Params p, const double* __restrict__ nu0,
                                                    const double* __restrict__ A, const double* __restrict__ g,
                                                    const double* __restrict__ E, const double* __restrict__ gam,
-                                                   const double* __restrict__ nx, int64_t n, RecU* __restrict__ rec,
-                                                   int32_t* __restrict__ key, int32_t* __restrict__ idx,
-                                                   DevStats* __restrict__ st)
+                                                   const double* __restrict__ nx, LineExtra ex, int64_t n,
+                                                   RecU* __restrict__ rec, int32_t* __restrict__ key,
+                                                   int32_t* __restrict__ idx, DevStats* __restrict__ st)
 {
     unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cgh6 = 0, ctrap = 0, cgh10 = 0, cmaxb = 0, cKmaxb = 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        LineOut o = line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
+        LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
         RecU r;
         int32_t k = p.ksent;
         r.jc = 0; r.f = 0.f; r.G2 = 0.f; r.a2 = 0.f; r.ilo = 0; r.ihi = -1; r.cK = 0.0;

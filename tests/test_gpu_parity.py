@@ -325,6 +325,56 @@ def test_lorentz_and_doppler_profiles(B, profile, case):
         B.Opacity(*grid).set_profile(7)
 
 
+def test_hitran_style_inputs(B):
+    """hk_compute_hitran: Eq. 4 air/self broadening, pressure shift, isotopologue table, against
+    the oracle's HITRAN path -- per-line parameters to 1e-12, integer extents of the SHIFTED centres exactly, k(nu) at
+    the north_star tolerance -- plus the reduction to the ExoMol entry point."""
+    n = 20_000
+    hl = W.make_lines_hitran(n, seed=0)
+    lines = {k: v.numpy() for k, v in hl.items()}
+    lines["iso"][17] = 9                                       # outside the table: skipped
+    cond, grid, cut = dict(W.HITRAN_COND), W.CONFIGS[2]["grid"], W.CONFIGS[2]["cut"]
+    dl = {k: torch.as_tensor(v).cuda() for k, v in lines.items()}
+    op = B.Opacity(*grid)
+    with pytest.raises(B.HKError) as e:
+        op.compute_hitran(dl, cut)
+    assert e.value.status == B.HK_ESTATE
+    op.set_conditions_hitran(cond["T"], cond["P_atm"], cond["P_self_atm"], cond["isos"])
+    k = op.compute_hitran(dl, cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    S0, gL0, aD0, ctr, valid = O.line_params_hitran(lines, cond)
+    assert st["n_skipped"] == 1 and valid.sum() == n - 1
+    S, gL, aD, ilo, ihi, jc = (t.cpu().numpy() for t in op.line_params_hitran(dl, cut))
+    v = valid > 0
+    assert np.abs(S[v] / S0[v] - 1).max() <= 1e-12 and np.abs(gL[v] / gL0[v] - 1).max() <= 1e-12
+    assert np.abs(aD[v] / aD0[v] - 1).max() <= 1e-13
+    N = O.grid_size(*grid)
+    ilo0, ihi0, jc0 = O.extents(ctr, valid, grid[0], grid[2], N, cut)
+    empty = ilo0 > ihi0
+    assert np.array_equal(ilo.astype(np.int64), np.where(empty, 0, ilo0))
+    assert np.array_equal(ihi.astype(np.int64), np.where(empty, -1, ihi0))
+    assert np.array_equal(jc.astype(np.int64)[v], jc0[v])
+    assert (jc0[v] != np.floor((lines["nu0"][v] - grid[0]) / grid[2])).mean() > 0.5      # the shift really moves bins
+    k_ref, evals = O.opacity_grid_hitran(lines, cond, grid, cut)
+    assert st["n_evals"] == evals
+    rel, ab, frac = check_parity(k.cpu().numpy(), k_ref, what="hitran")
+    print(f"hitran: rel={rel:.2e} abs={ab:.2e} frac_rel={frac:.3f}")
+    with pytest.raises(B.HKError):
+        op.set_conditions_hitran(1000.0, 1.0, 2.0, cond["isos"])           # P_self > P
+    # one isotopologue, air = self, no shift: the ExoMol entry point on the same handle
+    ex = W.to_numpy(W.make_lines(2, n=5000, seed=0))
+    h1 = {k2: ex[k2] for k2 in ("nu0", "A", "g_up", "E_low", "n_exp")}
+    h1.update(gamma_air=ex["gamma_ref"], gamma_self=ex["gamma_ref"], delta=np.zeros(5000), iso=np.zeros(5000, dtype=np.int32))
+    op.set_conditions_hitran(1500.0, 0.9, 0.2, [(18.0, 2000.0, 1.0)])
+    ka = op.compute_hitran({k2: torch.as_tensor(v2).cuda() for k2, v2 in h1.items()}, cut).clone()
+    kb = op.compute(_to_cuda(ex), cut)
+    torch.cuda.synchronize()
+    big = kb >= 1e-8 * kb.max()
+    assert float((ka[big] / kb[big] - 1).abs().max()) <= 1e-6
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])

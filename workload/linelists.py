@@ -138,3 +138,22 @@ def conditions(cfg: int):
 
 def to_numpy(lines):
     return {k: v.detach().cpu().numpy() for k, v in lines.items()}
+
+
+# ---- HITRAN-shaped list: the mid-molecule generator plus the extra HITRAN columns -------------
+HITRAN_FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_air", "gamma_self", "n_exp", "delta")
+HITRAN_ISOS = ((18.0106, 2000.0, 0.99732), (20.0148, 2016.0, 0.00200), (19.0148, 11940.0, 0.00037))   # mass, Q, abundance
+HITRAN_COND = dict(T=1500.0, P_atm=5.0, P_self_atm=0.5, isos=HITRAN_ISOS)
+
+
+def make_lines_hitran(n: int, seed: int = 0, device="cpu"):
+    """Config-2-shaped centres and strengths; gamma_air as gamma_ref, gamma_self 2-5 x gamma_air, pressure shift
+    uniform on [-0.02, 0.01] cm^-1/atm, isotopologue 0 / 1 / 2 with probability 0.95 / 0.03 / 0.02.  Unsorted."""
+    base = make_lines(2, n=n, seed=seed, device=device)
+    out = {k: base[k] for k in ("nu0", "A", "g_up", "E_low", "n_exp")}
+    out["gamma_air"] = base["gamma_ref"]
+    out["gamma_self"] = base["gamma_ref"] * (2.0 + 3.0 * uniform(seed, 2, 40, n, device))
+    out["delta"] = -0.02 + 0.03 * uniform(seed, 2, 41, n, device)
+    u = uniform(seed, 2, 42, n, device)
+    out["iso"] = ((u >= 0.95).to(torch.int32) + (u >= 0.98).to(torch.int32))
+    return out
