@@ -146,7 +146,7 @@ __device__ __forceinline__ int64_t count_within(double pos, double T, int64_t il
     return hi >= lo ? (int64_t)(hi - lo) + 1 : 0;
 }
 
-__global__ void __launch_bounds__(256) line_kernel(Params p, const double* __restrict__ nu0,
+__global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __restrict__ nu0,
                                                    const double* __restrict__ A, const double* __restrict__ g,
                                                    const double* __restrict__ E, const double* __restrict__ gam,
                                                    const double* __restrict__ nx, LineExtra ex, int64_t n,

@@ -553,12 +553,13 @@ def test_evaluator_accuracy_map(B):
 
 # ---- bench-size parity on sampled outputs ----------------------------------------------
 
-def _full_size_sampled(B, cfg, n_windows, width, n=None):
+def _full_size_sampled(B, cfg, n_windows, width, n=None, plinth=False):
     c = W.CONFIGS[cfg]
     cond, grid, cut = W.conditions(cfg), c["grid"], c["cut"]
     dl = W.make_lines(cfg, n=n, seed=0, device="cuda")
     op = B.Opacity(*grid)
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_plinth(plinth)
     k = op.compute(dl, cut)
     torch.cuda.synchronize()
     st = op.stats()
@@ -584,7 +585,7 @@ def _full_size_sampled(B, cfg, n_windows, width, n=None):
         else:
             sub = {f: v.cpu().numpy() for f, v in dl.items()}
         bins = np.arange(b0, b1, dtype=np.int64)
-        k_ref, _ = O.opacity_bins(sub, cond, grid, cut, bins)
+        k_ref, _ = O.opacity_bins(sub, cond, grid, cut, bins, plinth=plinth)
         rel, _, _ = check_parity(k[b0:b1].cpu().numpy(), k_ref, kmax=kmax, what=f"config {cfg} window {b0}")
         worst = max(worst, rel)
     # exact integer work count from the extents, all lines (O(n))
@@ -605,8 +606,8 @@ def test_config5_full_size_sampled(B):
     print(f"config 5 full: worst rel {worst:.2e}")
 
 
-@pytest.mark.parametrize("cfg", [3, 4])
-def test_bt2_shaped_full_size_sampled(B, cfg):
+@pytest.mark.parametrize("cfg,plinth", [(3, False), (4, False), (3, True)])
+def test_bt2_shaped_full_size_sampled(B, cfg, plinth):
     """The bench workload (config 4) and its coarse twin (config 3) at 5e8 lines, in the launch
     configuration bench.py times; the oracle sums every line within the cut on sampled bins."""
     import gc
@@ -615,5 +616,5 @@ def test_bt2_shaped_full_size_sampled(B, cfg):
     free, _ = torch.cuda.mem_get_info()
     if free < 120e9:
         pytest.skip("needs ~110 GB of device memory")
-    worst, st = _full_size_sampled(B, cfg, 6 if cfg == 4 else 10, 8 if cfg == 4 else 32)
-    print(f"config {cfg} full: worst rel {worst:.2e}, evals {st['n_evals']:.3e}")
+    worst, st = _full_size_sampled(B, cfg, 6 if cfg == 4 else 10, 8 if cfg == 4 else 32, plinth=plinth)
+    print(f"config {cfg} full (plinth {plinth}): worst rel {worst:.2e}, evals {st['n_evals']:.3e}")
