@@ -1043,16 +1043,29 @@ __device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_
                 for (int j = 0; j < kP; ++j) atomicAdd(acc + (size_t)b * kP + j, (double)v[j]);
             }
         } else {
-            // every lane ends up with all kP sums; lanes 0..kP-1 then issue ONE atomic each, to consecutive addresses
-            float out = 0.f;
+            // transposing reduction: each exchange halves the values a lane carries (8 -> 4 -> 2 -> 1 over lane bits
+            // 4, 3, 2), two butterfly steps finish bits 1, 0: 9 shuffles instead of 40.  Lane l then holds the sum of
+            // value j = (bit4, bit3, bit2 of l); the lanes with l % 4 == 0 issue one atomic each.
+            static_assert(kP == 8, "the fold below is written for 8 nodes");
+            float a[8], b4[4], c2[2];
 #pragma unroll
-            for (int j = 0; j < kP; ++j) {
-                float sum = mine ? v[j] : 0.f;
+            for (int j = 0; j < 8; ++j) a[j] = mine ? v[j] : 0.f;
+            const bool h4 = (lane & 16) != 0, h3 = (lane & 8) != 0, h2 = (lane & 4) != 0;
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-                if (lane == j) out = sum;
+            for (int j = 0; j < 4; ++j) {
+                const float send = h4 ? a[j] : a[j + 4], keep = h4 ? a[j + 4] : a[j];
+                b4[j] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
             }
-            if (lane < kP) atomicAdd(acc + (size_t)b * kP + lane, (double)out);
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const float send = h3 ? b4[j] : b4[j + 2], keep = h3 ? b4[j + 2] : b4[j];
+                c2[j] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+            }
+            float d = (h2 ? c2[1] : c2[0]) + __shfl_xor_sync(0xffffffffu, h2 ? c2[0] : c2[1], 4);
+            d += __shfl_xor_sync(0xffffffffu, d, 2);
+            d += __shfl_xor_sync(0xffffffffu, d, 1);
+            const int j = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+            if ((lane & 3) == 0) atomicAdd(acc + (size_t)b * kP + j, (double)d);
         }
         todo &= ~grp;
     }
