@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a
     constexpr int kTB = 32 * KB;
     constexpr int M = KB / 2;
     static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubC, "red must fit in the staging buffers");
-    __shared__ float4 smem[2][kSubC];          // A = { -dl, G2, c, 1.5 a2 }, B = { -f, qc, cK, y }
+    __shared__ float4 smem[2][kSubC];          // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y } (see stash)
     __shared__ float stage[kWarps][kStage][33];
     __shared__ float sacc[kWarps][kTB];
     __shared__ int hist[kYClasses];
@@ -542,8 +542,15 @@ __global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a
                     const float qc = (HK_Z2 / 1.5f) * (1.5f * a2);            // as the row pass recomputes it
                     // Gauss-Hermite rows: the tile holds core bins and (D1 D2 ~ |z|^8) stays inside fp32
                     const float ql = (qmin < qc && qmax <= 1.0e9f * a2) ? HK_Z4 * a2 : qc;
-                    smA[dst] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
-                    smB[dst] = make_float4(-ra.y, ql, rb.w, yv[k]);
+                    // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y }: Gauss-Hermite rows (B.y < 0) carry P = cK y and
+                    // Q = 1/a^2, two-term rows P = c (Lorentz amplitude) and Q = 1.5 a^2 -- what the row pass needs, ready
+                    if (ql < qc) {
+                        smA[dst] = make_float4(-fdj, G2, rb.w * yv[k], 1.0f / a2);
+                        smB[dst] = make_float4(-ra.y, -ql, rb.w, yv[k]);
+                    } else {
+                        smA[dst] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
+                        smB[dst] = make_float4(-ra.y, ql, rb.w, yv[k]);
+                    }
                 }
             }
         };
@@ -569,45 +576,32 @@ __global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a
                 since_flush += stop - l;
 #pragma unroll 1
                 for (; l < stop; ++l) {
-                    const float4 A = smA[l], B = smB[l];
-                    const float2 ndl = bcast2(A.x), nf = bcast2(B.x), g = bcast2(A.y);
-                    const float qc = (HK_Z2 / 1.5f) * A.w, ql = B.y;
-                    if (ql < qc) {
+                    const float4 A = smA[l];
+                    const float2 Bxy = *reinterpret_cast<const float2*>(&smB[l]);
+                    const float2 ndl = bcast2(A.x), nf = bcast2(Bxy.x), g = bcast2(A.y);
+                    const float ql = fabsf(Bxy.y);
+                    if (Bxy.y < 0.f) {
                         // Gauss-Hermite 4 in bin units: x^2 = t^2/a^2, s = q/a^2 (hk_device.cuh gh4_K)
                         constexpr float T1 = 0.27525512860841095f, T2 = 2.7247448713915890f;
                         constexpr float W1 = 0.5124242247547685f, W2 = 0.05176535879298783f;
-                        const float2 ia2 = bcast2(rcp_approx(A.w * (1.0f / 1.5f))), cky = bcast2(B.z * B.w);
+                        const float2 ia2 = bcast2(A.w), cky = bcast2(A.z);
                         const float2 t1 = bcast2(T1), t2 = bcast2(T2), m1 = bcast2(-4.0f * T1), m2 = bcast2(-4.0f * T2);
                         const float2 w1 = bcast2(W1), w2 = bcast2(W2);
-                        const float pos = -(A.x + B.x);
 #pragma unroll
                         for (int m = 0; m < M; ++m) {
                             const float2 d = __fadd2_rn(tb[m], ndl);     // exact: both are small integers
                             const float2 t = __fadd2_rn(d, nf);
                             const float2 q = __ffma2_rn(t, t, g);
-                            bool far_pair = false;
-                            if (M > 1) {                                 // this pair of rows wholly beyond the core?
-                                const float dist = fmaxf(fmaxf((float)(64 * m) - pos, pos - (float)(64 * m + 63)), 0.f) * 0.999f;
-                                far_pair = fmaf(dist, dist, A.y) * 0.9999f >= qc;
-                            }
-                            if (far_pair) {
-                                const float2 A1 = bcast2(A.w), one = bcast2(1.0f), nA2 = bcast2(-1.33333333f * A.w * A.y);
-                                const float2 rr = rcp2(q);
-                                const float2 uu = __ffma2_rn(nA2, rr, A1);
-                                const float2 vv = __ffma2_rn(uu, rr, one);
-                                acc[m] = __ffma2_rn(bcast2(A.z), __fmul2_rn(rr, vv), acc[m]);
-                            } else {
-                                const float2 x2 = __fmul2_rn(__fmul2_rn(t, t), ia2);
-                                const float2 sz = __fmul2_rn(q, ia2);
-                                const float2 P1 = __fadd2_rn(sz, t1), P2 = __fadd2_rn(sz, t2);
-                                const float2 D1 = __ffma2_rn(P1, P1, __fmul2_rn(m1, x2));
-                                const float2 D2 = __ffma2_rn(P2, P2, __fmul2_rn(m2, x2));
-                                const float2 num = __ffma2_rn(__fmul2_rn(w2, P2), D1, __fmul2_rn(__fmul2_rn(w1, P1), D2));
-                                float2 ww = __fmul2_rn(num, rcp2(__fmul2_rn(D1, D2)));
-                                ww.x = q.x >= ql ? ww.x : 0.f;              // the lane pass owns these bins
-                                ww.y = q.y >= ql ? ww.y : 0.f;
-                                acc[m] = __ffma2_rn(cky, ww, acc[m]);
-                            }
+                            const float2 x2 = __fmul2_rn(__fmul2_rn(t, t), ia2);
+                            const float2 sz = __fmul2_rn(q, ia2);
+                            const float2 P1 = __fadd2_rn(sz, t1), P2 = __fadd2_rn(sz, t2);
+                            const float2 D1 = __ffma2_rn(P1, P1, __fmul2_rn(m1, x2));
+                            const float2 D2 = __ffma2_rn(P2, P2, __fmul2_rn(m2, x2));
+                            const float2 num = __ffma2_rn(__fmul2_rn(w2, P2), D1, __fmul2_rn(__fmul2_rn(w1, P1), D2));
+                            float2 ww = __fmul2_rn(num, rcp2(__fmul2_rn(D1, D2)));
+                            ww.x = q.x >= ql ? ww.x : 0.f;                  // the lane pass owns these bins
+                            ww.y = q.y >= ql ? ww.y : 0.f;
+                            acc[m] = __ffma2_rn(cky, ww, acc[m]);
                         }
                     } else {
                         const float2 c = bcast2(A.z), A1 = bcast2(A.w), one = bcast2(1.0f);
@@ -636,7 +630,7 @@ __global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a
                 float clo = 1e9f, chi = -1e9f;
                 if (li < wl1) {
                     const float4 A = smA[li], B = smB[li];
-                    dl = -A.x; f = -B.x; G2 = A.y; ql = B.y; cK = B.z; y = B.w;
+                    dl = -A.x; f = -B.x; G2 = A.y; ql = fabsf(B.y); cK = B.z; y = B.w;
                     const float h2 = ql - G2;
                     if (h2 > 0.f) {
                         const float hw = sqrtf(h2) + 1.0f;                       // |t| < hw covers every q < ql
@@ -644,7 +638,7 @@ __global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a
                         const float lo = fmaxf(ceilf(pos - hw), 0.f), hi = fminf(floorf(pos + hw), whi);
                         if (hi >= lo) { clo = lo; chi = hi; }
                     }
-                    inv_a = rsqrtf(A.w * (1.0f / 1.5f));
+                    inv_a = B.y < 0.f ? sqrtf(A.w) : rsqrtf(A.w * (1.0f / 1.5f));
                 }
                 float bmin = clo, bmax = chi;
 #pragma unroll
