@@ -225,7 +225,7 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
                          const double *E, const double *gam, const double *nx,
                          double T, double P_atm, double mass_amu, double Q,
                          double numin, double dnu, int64_t N, double cut, int plinth, int profile,
-                         int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
+                         int cut_mode, int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                          double *k_out, int64_t *evals_out);
 
 void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const double *g,
@@ -235,7 +235,7 @@ void hko_opacity_bins(int64_t n, const double *nu0, const double *A, const doubl
                       int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                       double *k_out, int64_t *evals_out)
 {
-    hko_opacity_bins_ex(n, nu0, A, g, E, gam, nx, T, P_atm, mass_amu, Q, numin, dnu, N, cut, 0, 0, nb, bins, l0, l1,
+    hko_opacity_bins_ex(n, nu0, A, g, E, gam, nx, T, P_atm, mass_amu, Q, numin, dnu, N, cut, 0, 0, 0, nb, bins, l0, l1,
                         k_out, evals_out);
 }
 
@@ -243,7 +243,7 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
                          const double *E, const double *gam, const double *nx,
                          double T, double P_atm, double mass_amu, double Q,
                          double numin, double dnu, int64_t N, double cut, int plinth, int profile,
-                         int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
+                         int cut_mode, int64_t nb, const int64_t *bins, int64_t l0, int64_t l1,
                          double *k_out, int64_t *evals_out)
 {
     int64_t nl = l1 - l0;
@@ -262,8 +262,21 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
         if (line_valid(nu0[l], A[l], g[l], E[l], gam[l], nx[l])) {
             line_params(nu0[l], A[l], g[l], E[l], gam[l], nx[l], T, P_atm, mass_amu, Q,
                         &S[q], &gL[q], &aD[q]);
-            line_extent(nu0[l], numin, dnu, N, cut, &ilo[q], &ihi[q], &jc);
-            pl[q] = use_plinth ? shape_K(profile, cut / aD[q], gL[q] / aD[q]) : 0.0;
+            /* cutting length of this line (L239: "a fixed cutting length, a fraction of the Doppler half-width, or a
+             * fraction of the Lorentzian half-width"; R25): cut_mode 0: cut in cm^-1; 1: cut x Gamma_L;
+             * 2: cut x Gamma_D, Gamma_D = alpha_D sqrt(ln 2) (L193-206) */
+            double cl = cut;
+            if (cut > 0.0 && isfinite(cut)) {
+                if (cut_mode == 1) cl = cut * gL[q];
+                else if (cut_mode == 2) cl = cut * aD[q] * sqrt(log(2.0));
+            }
+            if ((cut_mode == 1 || cut_mode == 2) && cut > 0.0 && isfinite(cut) && !(cl > 0.0)) {
+                ilo[q] = 0; ihi[q] = -1;                       /* zero width: the line has no extent */
+                pl[q] = 0.0;
+            } else {
+                line_extent(nu0[l], numin, dnu, N, cl, &ilo[q], &ihi[q], &jc);
+                pl[q] = use_plinth ? shape_K(profile, cl / aD[q], gL[q] / aD[q]) : 0.0;
+            }
         } else { S[q] = 0.0; gL[q] = 0.0; aD[q] = 1.0; ilo[q] = 0; ihi[q] = -1; pl[q] = 0.0; }
     }
     int64_t evals = 0;

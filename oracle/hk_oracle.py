@@ -44,7 +44,7 @@ _lib.hko_opacity_bins.argtypes = [_i64, _pd, _pd, _pd, _pd, _pd, _pd, _d, _d, _d
 
 _lib.hko_opacity_bins_ex.restype = None
 _lib.hko_opacity_bins_ex.argtypes = [_i64, _pd, _pd, _pd, _pd, _pd, _pd, _d, _d, _d, _d,
-                                     _d, _d, _i64, _d, C.c_int, C.c_int, _i64, _pi64, _i64, _i64, _pd,
+                                     _d, _d, _i64, _d, C.c_int, C.c_int, C.c_int, _i64, _pi64, _i64, _i64, _pd,
                                      C.POINTER(_i64)]
 
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
@@ -107,7 +107,10 @@ def profile(nu, nu0, gammaL, alphaD) -> float:
 PROFILES = {"voigt": 0, "lorentz": 1, "doppler": 2}
 
 
-def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False, profile="voigt"):
+CUT_MODES = {"fixed": 0, "lorentz": 1, "doppler": 2}
+
+
+def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False, profile="voigt", cut_mode="fixed"):
     """k at the listed bins, brute force over lines [l0, l1).  -> (k, n_evals).
     plinth=True removes every line's value at the cutting length from its bins (section 2.1.1)."""
     a = [_f64(lines[k]) for k in FIELDS]
@@ -120,7 +123,7 @@ def opacity_bins(lines, cond, grid, cut, bins, l0=0, l1=None, plinth=False, prof
     numin, numax, dnu = grid
     N = grid_size(numin, numax, dnu)
     _lib.hko_opacity_bins_ex(n, *a, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"],
-                             numin, dnu, N, float(cut), 1 if plinth else 0, PROFILES[profile], bins.size, bins, int(l0), int(l1),
+                             numin, dnu, N, float(cut), 1 if plinth else 0, PROFILES[profile], CUT_MODES[cut_mode], bins.size, bins, int(l0), int(l1),
                              out, C.byref(ev))
     return out, int(ev.value)
 
@@ -129,19 +132,20 @@ def _uncut(cut) -> bool:
     return not (cut > 0.0 and np.isfinite(cut))
 
 
-def opacity_window(lines_sorted, cond, grid, cut, b0, b1, plinth=False, profile="voigt"):
+def opacity_window(lines_sorted, cond, grid, cut, b0, b1, plinth=False, profile="voigt", cut_mode="fixed", reach=None):
     """k on bins [b0, b1) for lines SORTED by nu0 (fixed cut: only lines within
     cut + one bin of the window are passed to the brute-force routine)."""
     numin, numax, dnu = grid
     bins = np.arange(b0, b1, dtype=np.int64)
     nu0 = lines_sorted["nu0"]
     if _uncut(cut):
-        return opacity_bins(lines_sorted, cond, grid, cut, bins, plinth=plinth, profile=profile)
-    lo = numin + b0 * dnu - cut - 2.0 * dnu
-    hi = numin + (b1 - 1) * dnu + cut + 2.0 * dnu
+        return opacity_bins(lines_sorted, cond, grid, cut, bins, plinth=plinth, profile=profile, cut_mode=cut_mode)
+    reach = cut if reach is None else reach          # the largest cutting length of any line (a caller's knowledge)
+    lo = numin + b0 * dnu - reach - 2.0 * dnu
+    hi = numin + (b1 - 1) * dnu + reach + 2.0 * dnu
     l0 = int(np.searchsorted(nu0, lo, side="left"))
     l1 = int(np.searchsorted(nu0, hi, side="right"))
-    return opacity_bins(lines_sorted, cond, grid, cut, bins, l0, l1, plinth=plinth, profile=profile)
+    return opacity_bins(lines_sorted, cond, grid, cut, bins, l0, l1, plinth=plinth, profile=profile, cut_mode=cut_mode)
 
 
 def sort_lines(lines):
@@ -152,18 +156,23 @@ def sort_lines(lines):
     return {k: _f64(lines[k])[order] for k in FIELDS}
 
 
-def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=False, profile="voigt"):
+def opacity_grid(lines, cond, grid, cut, block=512, presorted=False, plinth=False, profile="voigt", cut_mode="fixed"):
     """k on every bin of the grid.  -> (k[N], n_evals)."""
     numin, numax, dnu = grid
     N = grid_size(numin, numax, dnu)
     ls = lines if presorted else sort_lines(lines)
     k = np.zeros(N)
     evals = 0
+    reach = None
+    if cut_mode != "fixed" and not _uncut(cut):
+        _, gL, aD, valid = line_params(ls, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        w = gL if cut_mode == "lorentz" else aD * np.sqrt(np.log(2.0))
+        reach = float(cut) * float(np.max(np.where(valid > 0, w, 0.0), initial=0.0))
     if _uncut(cut):
         block = N
     for b0 in range(0, N, block):
         b1 = min(N, b0 + block)
-        kk, ev = opacity_window(ls, cond, grid, cut, b0, b1, plinth=plinth, profile=profile)
+        kk, ev = opacity_window(ls, cond, grid, cut, b0, b1, plinth=plinth, profile=profile, cut_mode=cut_mode, reach=reach)
         k[b0:b1] = kk
         evals += ev
     return k, evals
