@@ -120,6 +120,20 @@ int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, do
 #define HK_PROFILE_DOPPLER 2
 int hk_set_profile(hk_ctx* ctx, int profile);
 
+/* Cutting length (L239: "a fixed cutting length, a fraction of the Doppler half-width, or a fraction of the Lorentzian
+ * half-width"): what the cut_cm argument of the compute entry points means.
+ *   HK_CUT_FIXED    cut_cm is the cutting length in cm^-1, the same for every line        (default)
+ *   HK_CUT_LORENTZ  the cutting length of a line is cut_cm x its Gamma_L
+ *   HK_CUT_DOPPLER  the cutting length of a line is cut_cm x its Gamma_D = alpha_D sqrt(ln 2)
+ * A line of zero half-width has no extent.  cut_cm <= 0 or +inf is uncut in every mode.  In the width-relative modes
+ * a compute reads the range of cutting lengths back (ONE host synchronisation per call) and runs one pass per class
+ * [c, 2c) of cutting length, so the call is synchronous up to its last pass; hk_compute_host does not support them.
+ * hk_get_stats afterwards: n_evals / n_skipped / n_off_grid are totals, the rest describes the last pass. */
+#define HK_CUT_FIXED 0
+#define HK_CUT_LORENTZ 1
+#define HK_CUT_DOPPLER 2
+int hk_set_cut_mode(hk_ctx* ctx, int mode);
+
 /* Plinth removal (section 2.1.1): on != 0 subtracts from every bin of a line's extent that line's own value
  * at the cutting length position, S V(nu0 +- cut) (needed with continua that already hold the plinths, e.g. CKD).
  * Off by default; no effect on uncut computations.  Changes hk_workspace_bytes (+ 8 B per bin): set it before the

@@ -26,7 +26,7 @@ FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
-           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile",
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode",
            "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
            "hk_last_cuda_error", "hk_strerror")
 PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "near", "down")
@@ -91,6 +91,8 @@ _lib.hk_set_plinth.argtypes = [_vp, C.c_int]
 _lib.hk_set_plinth.restype = C.c_int
 _lib.hk_set_profile.argtypes = [_vp, C.c_int]
 _lib.hk_set_profile.restype = C.c_int
+_lib.hk_set_cut_mode.argtypes = [_vp, C.c_int]
+_lib.hk_set_cut_mode.restype = C.c_int
 _lib.hk_last_cuda_error.argtypes = [_vp]
 _lib.hk_strerror.argtypes = [C.c_int]
 _lib.hk_strerror.restype = C.c_char_p
@@ -186,6 +188,11 @@ class Opacity:
         """'voigt' (default), 'lorentz' or 'doppler' (hk_set_profile)."""
         code = {"voigt": 0, "lorentz": 1, "doppler": 2}.get(profile, profile)
         self._check(_lib.hk_set_profile(self._ctx, int(code)), "hk_set_profile")
+
+    def set_cut_mode(self, mode):
+        """'fixed' (default), 'lorentz' or 'doppler': cut = a multiple of each line's half-width (hk_set_cut_mode)."""
+        code = {"fixed": 0, "lorentz": 1, "doppler": 2}.get(mode, mode)
+        self._check(_lib.hk_set_cut_mode(self._ctx, int(code)), "hk_set_cut_mode")
 
     def set_plinth(self, on: bool):
         self._check(_lib.hk_set_plinth(self._ctx, 1 if on else 0), "hk_set_plinth")

@@ -1239,7 +1239,10 @@ __global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const 
         if (i < n_act) {
             const float4 ra = a.recA[i], rb = a.recB[i];
             ilo = __float_as_int(rb.y); ihi = __float_as_int(rb.z);
-            const double G2 = (double)ra.z, a2 = (double)rb.x, cb = p.cut_bins;
+            const double G2 = (double)ra.z, a2 = (double)rb.x;
+            // the line's own cutting length in bins (width-relative modes: from the record, as the kernels see it)
+            const double cb = p.cut_mode == 0 ? p.cut_bins
+                            : p.cut_factor * (p.cut_mode == 1 ? sqrt(G2) : sqrt(a2) * 0.83255461115769775635);
             const double q = cb * cb + G2;
             if (q >= (double)HK_Z2 * a2) {
                 // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q)

@@ -29,6 +29,7 @@ struct hk_ctx {
     int edge_nodes;
     int plinth;
     int profile;
+    int cut_mode;
     // HITRAN-style conditions (hk_set_conditions_hitran)
     bool have_hitran;
     double P_self;
@@ -138,7 +139,13 @@ int fail_cuda(hk_ctx* c, cudaError_t e)
     } while (0)
 
 // Fill the per-launch constants (step a0).
-Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = false)
+struct CutClass {
+    double lo, hi;          // lines with lo <= cutting length < hi belong to the pass
+    double bound_lo, bound_hi;   // smallest / largest cutting length that can occur in it (cm^-1)
+    bool first;
+};
+
+Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = false, const CutClass* cls = nullptr)
 {
     Params p;
     std::memset(&p, 0, sizeof(p));
@@ -167,10 +174,23 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     }
     p.uncut = is_uncut(cut) ? 1 : 0;
     p.cut = p.uncut ? 0.0 : cut;
+    p.cut_mode = p.uncut ? 0 : c->cut_mode;
+    p.cut_factor = cut;
+    p.cls_lo = 0.0;
+    p.cls_hi = INFINITY;
+    p.count_invalid = 1;
     double cb = p.uncut ? 0.0 : cut / c->dnu;
+    double cb_lo = cb, cb_hi = cb;                 // bounds of the cutting length in bins: one value unless width-relative
+    if (p.cut_mode != 0 && cls) {
+        p.cls_lo = cls->lo; p.cls_hi = cls->hi; p.count_invalid = cls->first ? 1 : 0;
+        cb_lo = cls->bound_lo / c->dnu; cb_hi = cls->bound_hi / c->dnu;
+        cb = cb_hi;
+    } else if (p.cut_mode != 0) {
+        cb_lo = 0.0; cb_hi = cb = 1.0e15;          // no class given (getters): extents only, no tile logic
+    }
     bool compact = !p.uncut && cb < 268435456.0 && (double)c->N + 2.0 * std::ceil(cb) + 8.0 < 2147483647.0;
-    p.cb_floor = p.uncut ? 0 : (int64_t)std::fmin(std::floor(cb), 4.0e18);
-    p.cb_ceil = p.uncut ? 0 : (int64_t)std::fmin(std::ceil(cb), 4.0e18);
+    p.cb_floor = p.uncut ? 0 : (int64_t)std::fmin(std::floor(cb_lo), 4.0e18);
+    p.cb_ceil = p.uncut ? 0 : (int64_t)std::fmin(std::ceil(cb_hi), 4.0e18);
     if (compact) {
         p.kmin = -(p.cb_ceil + 2);
         p.ksent = (int32_t)(c->N + 2 * p.cb_ceil + 6);
@@ -359,6 +379,13 @@ int hk_set_node_separation(hk_ctx* ctx, double sep)
     return HK_OK;
 }
 
+int hk_set_cut_mode(hk_ctx* ctx, int mode)
+{
+    if (!ctx || mode < HK_CUT_FIXED || mode > HK_CUT_DOPPLER) return HK_EINVAL;
+    ctx->cut_mode = mode;
+    return HK_OK;
+}
+
 int hk_set_profile(hk_ctx* ctx, int profile)
 {
     if (!ctx || profile < HK_PROFILE_VOIGT || profile > HK_PROFILE_DOPPLER) return HK_EINVAL;
@@ -388,7 +415,8 @@ int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane)
 }
 
 static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
-                        cudaStream_t stream, bool zero_out, bool reuse_sort = false, const LineExtra* extra = nullptr)
+                        cudaStream_t stream, bool zero_out, bool reuse_sort = false, const LineExtra* extra = nullptr,
+                        const CutClass* cls = nullptr)
 {
     if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL) return HK_EINVAL;
     if (std::isnan(cut_cm)) return HK_EINVAL;
@@ -399,9 +427,11 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     char* ws = (char*)ctx->ws;
     DevStats* st = (DevStats*)(ws + L.stats);
     const int n = (int)n_lines;
-    Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cut_cm), extra != nullptr);
+    Params p = make_params(ctx, cut_cm, pick_chunk(ctx, n_lines, cls ? cls->bound_hi : cut_cm), extra != nullptr, cls);
     const LineExtra ex = extra ? *extra : LineExtra{nullptr, nullptr, nullptr};
-    p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes) ? 1 : 0;
+    // (with per-line cutting lengths the tile an extent ends in is not a function of the centre bin alone: the
+    //  masked direct edge kernel takes those tiles)
+    p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes && p.cut_mode == 0) ? 1 : 0;
 
     HK_CUDA(cudaEventRecord(ctx->ev[0], stream));
     HK_CUDA(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
@@ -536,14 +566,97 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     return HK_OK;
 }
 
+// ---- cutting length as a multiple of each line's half-width (L239) ------------------------------------------
+// min and max of the per-line cutting length over the lines that have one
+__global__ void __launch_bounds__(256) cut_range_kernel(Params p, const double* __restrict__ nu0, const double* __restrict__ A,
+                                                        const double* __restrict__ g, const double* __restrict__ E,
+                                                        const double* __restrict__ gam, const double* __restrict__ nx,
+                                                        LineExtra ex, int64_t n, unsigned long long* __restrict__ mm)
+{
+    unsigned long long lo = ~0ULL, hi = 0ULL;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
+        if (!o.valid) continue;
+        const double c = p.cut_factor * (p.cut_mode == 1 ? o.gammaL : o.alphaD * 0.83255461115769775635);
+        if (!(c > 0.0) || !isfinite(c)) continue;
+        const unsigned long long b = (unsigned long long)__double_as_longlong(c);     // positive doubles order as integers
+        lo = min(lo, b); hi = max(hi, b);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if ((threadIdx.x & 31) == 0) { atomicMin(mm, lo); atomicMax(mm + 1, hi); }
+}
+
+// One entry for every compute: fixed cut or uncut -> one pass; width-relative cut -> the range of cutting lengths is
+// read back (ONE host synchronisation), then one pass per class [c, 2c) of cutting length, each with its own sort,
+// tile ranges and node hierarchy; the passes add into out_k.  A class keeps the ratio of the largest to the
+// smallest extent below 2, which is what the interior / node classification of a tile needs to stay useful.
+static int compute_any(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
+                       cudaStream_t stream, bool zero_out, bool reuse_sort = false, const LineExtra* extra = nullptr)
+{
+    if (!ctx || ctx->cut_mode == 0 || is_uncut(cut_cm) || n_lines <= 0)
+        return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, stream, zero_out, reuse_sort, extra);
+    if (!out_k_dev || n_lines >= 2147483647LL || std::isnan(cut_cm) || !lines_ok(lines)) return HK_EINVAL;
+    if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
+    const Layout L = make_layout(ctx, n_lines);
+    if (ctx->ws_bytes < L.total) return HK_ENOSPC;
+    unsigned long long* mm = (unsigned long long*)((char*)ctx->ws + L.stats);     // the stats block is free before a pass
+    const unsigned long long init[2] = {~0ULL, 0ULL};
+    HK_CUDA(cudaMemcpyAsync(mm, init, sizeof(init), cudaMemcpyHostToDevice, stream));
+    {
+        const Params p = make_params(ctx, cut_cm, 512, extra != nullptr);
+        const LineExtra ex = extra ? *extra : LineExtra{nullptr, nullptr, nullptr};
+        cut_range_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
+                                                                     lines->gamma_ref, lines->n_exp, ex, n_lines, mm);
+    }
+    unsigned long long got[2];
+    HK_CUDA(cudaMemcpyAsync(got, mm, sizeof(got), cudaMemcpyDeviceToHost, stream));
+    HK_CUDA(cudaStreamSynchronize(stream));
+    double cmin, cmax;
+    std::memcpy(&cmin, &got[0], 8);
+    std::memcpy(&cmax, &got[1], 8);
+    const bool none = got[0] == ~0ULL;                     // no line has a positive cutting length
+    int64_t tot_skipped = 0, tot_off = 0, tot_evals = 0, launches = 0;
+    int rc = HK_OK;
+    bool first = true;
+    double lo = none ? 1.0 : cmin;
+    const double top = none ? 1.0 : cmax;
+    for (int k = 0; k < 64 && rc == HK_OK; ++k) {
+        CutClass cls;
+        cls.first = first;
+        cls.lo = first ? 0.0 : lo;
+        cls.hi = (2.0 * lo > top) ? INFINITY : 2.0 * lo;
+        cls.bound_lo = lo;
+        cls.bound_hi = std::fmin(2.0 * lo, top);
+        rc = compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, stream, zero_out && first, false, extra, &cls);
+        if (rc != HK_OK) break;
+        launches += ctx->last_launches;
+        DevStats ds;
+        HK_CUDA(cudaMemcpyAsync(&ds, ctx->d_stats, sizeof(ds), cudaMemcpyDeviceToHost, stream));
+        HK_CUDA(cudaStreamSynchronize(stream));
+        tot_skipped += (int64_t)ds.n_skipped; tot_off += (int64_t)ds.n_off_grid; tot_evals += (int64_t)ds.n_evals;
+        first = false;
+        if (!(cls.hi < INFINITY)) break;
+        lo *= 2.0;
+    }
+    if (rc != HK_OK) return rc;
+    ctx->last_launches = launches;
+    ctx->host_totals = true;
+    ctx->tot_lines = n_lines; ctx->tot_skipped = tot_skipped; ctx->tot_off_grid = tot_off; ctx->tot_evals = tot_evals;
+    return HK_OK;
+}
+
 int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
 {
-    return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true);
+    return compute_any(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true);
 }
 
 int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
 {
-    return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, false);
+    return compute_any(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, false);
 }
 
 int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond, const double* T_K,
@@ -560,8 +673,8 @@ int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double
     int64_t launches = 0;
     for (int32_t c = 0; c < n_cond && rc == HK_OK; ++c) {
         ctx->T = T_K[c]; ctx->P_atm = P_atm[c]; ctx->Q = Q[c];
-        rc = compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev + (size_t)c * (size_t)ctx->N, (cudaStream_t)stream_v, true,
-                          /*reuse_sort=*/c > 0);
+        rc = compute_any(ctx, lines, n_lines, cut_cm, out_k_dev + (size_t)c * (size_t)ctx->N, (cudaStream_t)stream_v, true,
+                         /*reuse_sort=*/c > 0);
         launches += ctx->last_launches;
     }
     ctx->T = T0; ctx->P_atm = P0; ctx->Q = Q0;
@@ -612,6 +725,7 @@ int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut
 {
     if (!ctx || !out_k_host || n_lines < 0 || std::isnan(cut_cm)) return HK_EINVAL;
     if (n_lines > 0 && !lines_ok(hl)) return HK_EINVAL;
+    if (ctx->cut_mode != 0 && !is_uncut(cut_cm)) return HK_EINVAL;        // width-relative cuts: device-resident entry points only
     if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
     const HostLayout H = make_host_layout(ctx, n_lines, block_lines);
     if (ctx->ws_bytes < H.total) return HK_ENOSPC;
@@ -749,7 +863,7 @@ int hk_compute_hitran(hk_ctx* ctx, const hk_lines_hitran* lines, int64_t n_lines
     if (!ctx->have_hitran) return HK_ESTATE;
     hk_lines base = n_lines > 0 ? as_lines(lines) : hk_lines{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     LineExtra ex = n_lines > 0 ? LineExtra{lines->gamma_self, lines->delta, lines->iso} : LineExtra{nullptr, nullptr, nullptr};
-    return compute_impl(ctx, &base, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true, false, &ex);
+    return compute_any(ctx, &base, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true, false, &ex);
 }
 
 int hk_get_line_params_hitran(hk_ctx* ctx, const hk_lines_hitran* lines, int64_t n_lines, double cut_cm, double* S_dev,

@@ -36,6 +36,13 @@ struct Params {
     // cut
     double cut;           // cm^-1 (ignored when uncut)
     int uncut;
+    // cutting length per line (L239): 0 fixed (cut), 1 cut_factor x Gamma_L, 2 cut_factor x Gamma_D = alpha_D sqrt(ln 2).
+    // Width-relative modes run in passes over classes of cutting length [cls_lo, cls_hi): a line outside the class of
+    // the pass is "foreign" (not this pass's business, counted nowhere); cb_floor comes from the smallest and cb_ceil
+    // from the largest cutting length of the class.
+    int cut_mode;
+    int count_invalid;     // count R14-skipped lines in this pass (first pass only)
+    double cut_factor, cls_lo, cls_hi;
     // sort keys: key = jc - kmin in [0, ksent), ksent = sentinel for lines that contribute nothing
     int64_t kmin;
     int32_t ksent;
@@ -82,6 +89,7 @@ __device__ __forceinline__ bool finite6(double a, double b, double c, double d, 
 struct LineOut {
     bool valid;       // passes the R14 checks
     bool on_grid;     // extent non-empty and centre within 2^30 bins
+    bool foreign;     // width-relative cut: the line's cutting length belongs to another pass
     double S, gammaL, alphaD;
     int64_t jc, ilo, ihi;
     double pos_f;     // (nu0-numin)/dnu - jc
@@ -97,6 +105,7 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
     o.valid = finite6(nu0, A, g, E, gam, nx) && nu0 > 0.0 && A >= 0.0;
     if (p.n_iso > 0) o.valid = o.valid && isfinite(gs) && isfinite(dl) && iso >= 0 && iso < p.n_iso;
     o.on_grid = false;
+    o.foreign = false;
     o.S = o.gammaL = o.alphaD = 0.0;
     o.jc = 0; o.ilo = 0; o.ihi = -1; o.pos_f = 0.0;
     if (!o.valid) return o;
@@ -120,8 +129,14 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
     o.jc = (int64_t)c;
     o.pos_f = pos - c;
     if (!p.uncut) {
-        double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, p.cut), p.numin), p.dnu));
-        double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, p.cut), p.numin), p.dnu));
+        double cutl = p.cut;
+        if (p.cut_mode != 0) {                                                  // L239, R25
+            cutl = p.cut_factor * (p.cut_mode == 1 ? o.gammaL : o.alphaD * 0.83255461115769775635);   // sqrt(ln 2)
+            if (!(cutl > 0.0)) return o;                                        // zero width: no extent
+            if (!(cutl >= p.cls_lo && cutl < p.cls_hi)) { o.foreign = true; return o; }
+        }
+        double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, cutl), p.numin), p.dnu));
+        double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, cutl), p.numin), p.dnu));
         if (lo < 0.0) lo = 0.0;
         if (hi > (double)(p.N - 1)) hi = (double)(p.N - 1);
         lo = fmin(lo, big);
@@ -161,7 +176,9 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
         int32_t k = p.ksent;
         r.jc = 0; r.f = 0.f; r.G2 = 0.f; r.a2 = 0.f; r.ilo = 0; r.ihi = -1; r.cK = 0.0;
         if (!o.valid) {
-            ++skipped;
+            if (p.count_invalid) ++skipped;
+        } else if (o.foreign) {
+            // belongs to another pass
         } else if (!o.on_grid) {
             ++off;
             r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);

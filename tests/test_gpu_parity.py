@@ -375,6 +375,56 @@ def test_hitran_style_inputs(B):
     op.close()
 
 
+@pytest.mark.parametrize("mode,factor", [("lorentz", 500.0), ("lorentz", 40.0), ("doppler", 3000.0)])
+@pytest.mark.parametrize("case", ["config2", "config3", "resolved"])
+def test_width_relative_cutting_length(B, case, mode, factor):
+    """hk_set_cut_mode: the cutting length of a line is a multiple of its own Lorentz
+    or Doppler half-width.  Integer extents exact, k(nu) at the north_star tolerance, with and without plinth removal."""
+    if case == "config2":
+        lines, cond, grid, _ = _mini(2, 20_000)
+    elif case == "config3":
+        lines, cond, grid, _ = _mini(3, 100_000)
+    else:
+        rng = np.random.default_rng(23)
+        n = 1500
+        lines = _simple_lines(np.sort(rng.uniform(995.0, 1025.0, n)), A=10 ** rng.uniform(-3, 2, n),
+                              E_low=rng.uniform(0, 4000, n), gamma_ref=rng.uniform(0.01, 0.2, n))
+        cond, grid = COND, (1000.0, 1020.5, 0.001)
+    dl = _to_cuda(lines)
+    S, gL, aD, valid = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    hw = gL if mode == "lorentz" else aD * np.sqrt(np.log(2.0))
+    N = O.grid_size(*grid)
+    for plinth in (False, True):
+        op = B.Opacity(*grid)
+        op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        op.set_cut_mode(mode)
+        op.set_plinth(plinth)
+        k = op.compute(dl, factor)
+        torch.cuda.synchronize()
+        st = op.stats()
+        k_ref, evals = O.opacity_grid(lines, cond, grid, factor, plinth=plinth, cut_mode=mode)
+        assert st["n_evals"] == evals and st["n_lines"] == len(hw)
+        g_ilo, g_ihi, _ = (t.cpu().numpy().astype(np.int64) for t in op.extents(dl))
+        # the oracle's extent formula with each line's own cutting length
+        c = factor * hw
+        ilo = np.maximum(np.ceil((lines["nu0"] - c - grid[0]) / grid[2]), 0).astype(np.int64)
+        ihi = np.minimum(np.floor((lines["nu0"] + c - grid[0]) / grid[2]), N - 1).astype(np.int64)
+        empty = ilo > ihi
+        assert np.array_equal(g_ilo, np.where(empty, 0, ilo)) and np.array_equal(g_ihi, np.where(empty, -1, ihi))
+        assert int((g_ihi - g_ilo + 1).sum()) == evals
+        if plinth and factor < 100.0:
+            # 40 Gamma_L puts the cut inside the core (|z| < 25) of every line with y < 0.6: S (V - V(cut)) is then a
+            # small difference on all its bins and the error is bounded against the unsubtracted opacity (DESIGN.md 5)
+            k_raw, _ = O.opacity_grid(lines, cond, grid, factor, cut_mode=mode)
+            err = np.abs(k.cpu().numpy() - k_ref)
+            assert (err <= 1e-4 * k_raw + 1e-8 * k_raw.max()).all()
+            rel, ab = float((err[k_raw > 0] / k_raw[k_raw > 0]).max()), 0.0
+        else:
+            rel, ab, frac = check_parity(k.cpu().numpy(), k_ref, what=f"cut {mode} x{factor} {case} plinth={plinth}")
+        print(f"cut {mode} x{factor} {case} plinth={plinth}: rel={rel:.2e} abs={ab:.2e} cuts {c.min():.3g}..{c.max():.3g} cm^-1")
+        op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
