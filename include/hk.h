@@ -170,6 +170,14 @@ int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cu
 int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond,
                      const double* T_K, const double* P_atm, const double* Q, double* out_k_dev, void* stream);
 
+/* A wavenumber axis made of bands of different resolution (L218: "it is possible to use a different wavenumber
+ * resolution for different bands"): one context per band (its own numin, numax, dnu, conditions and workspace; the
+ * workspaces may be one buffer if the bands run on one stream), one output array per band; every band is the full
+ * definition of hk_compute on its own grid, so a line near a band edge contributes to both bands through its clamped
+ * extent.  ctxs, out_k_dev: HOST arrays of n_bands pointers.  All bands are checked before anything is enqueued. */
+int hk_compute_bands(hk_ctx* const* ctxs, int32_t n_bands, const hk_lines* lines, int64_t n_lines, double cut_cm,
+                     double* const* out_k_dev, void* stream);
+
 /* ---- HITRAN-style inputs (Table 3-4: nu, E_L, A, delta, gamma_air, gamma_self, n per line) -----------
  * Nine SoA DEVICE arrays of n_lines elements, read-only: eight fp64 and the int32 isotopologue index of each line
  * into the table given to hk_set_conditions_hitran (the species parameter file's isotopologue list, L371-373). */

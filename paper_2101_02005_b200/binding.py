@@ -26,7 +26,7 @@ FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
-           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode",
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode", "hk_compute_bands",
            "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
            "hk_last_cuda_error", "hk_strerror")
 PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "near", "down")
@@ -93,6 +93,8 @@ _lib.hk_set_profile.argtypes = [_vp, C.c_int]
 _lib.hk_set_profile.restype = C.c_int
 _lib.hk_set_cut_mode.argtypes = [_vp, C.c_int]
 _lib.hk_set_cut_mode.restype = C.c_int
+_lib.hk_compute_bands.argtypes = [C.POINTER(_vp), C.c_int32, C.POINTER(hk_lines), _i64, _d, C.POINTER(_vp), _vp]
+_lib.hk_compute_bands.restype = C.c_int
 _lib.hk_last_cuda_error.argtypes = [_vp]
 _lib.hk_strerror.argtypes = [C.c_int]
 _lib.hk_strerror.restype = C.c_char_p
@@ -306,6 +308,24 @@ class Opacity:
         s = hk_stats()
         self._check(_lib.hk_get_stats(self._ctx, C.byref(s)), "hk_get_stats")
         return {k: int(getattr(s, k)) for k, _ in hk_stats._fields_}
+
+
+def compute_bands(ops, lines, cut, outs=None, stream=None):
+    """hk_compute_bands: `ops` is a list of Opacity objects, one per band of the wavenumber axis (each with its own
+    resolution and conditions set); -> list of fp64 CUDA tensors, one per band."""
+    ls, n = _lines_struct(lines)
+    nb = len(ops)
+    if outs is None:
+        outs = [torch.empty(op.N, dtype=torch.float64, device="cuda") for op in ops]
+    for op, o in zip(ops, outs):
+        op.ensure_workspace(n)
+        assert o.is_cuda and o.dtype == torch.float64 and o.is_contiguous() and o.numel() == op.N
+    ctxs = (_vp * nb)(*[op._ctx for op in ops])
+    ptrs = (_vp * nb)(*[o.data_ptr() for o in outs])
+    st = _lib.hk_compute_bands(ctxs, nb, C.byref(ls), n, float(cut) if cut is not None else 0.0, ptrs, _stream_ptr(stream))
+    if st != HK_OK:
+        raise HKError(st, "hk_compute_bands")
+    return outs
 
 
 def probe_fp32_peak(packed=True, iters=4096, stream=None):

@@ -826,6 +826,22 @@ int hk_get_line_params(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, doub
     return HK_OK;
 }
 
+// ---- bands of different resolution (L218) ---------------------------------------------------
+int hk_compute_bands(hk_ctx* const* ctxs, int32_t n_bands, const hk_lines* lines, int64_t n_lines, double cut_cm,
+                     double* const* out_k_dev, void* stream_v)
+{
+    if (n_bands < 0 || (n_bands > 0 && (!ctxs || !out_k_dev))) return HK_EINVAL;
+    for (int32_t b = 0; b < n_bands; ++b) {
+        if (!ctxs[b] || !out_k_dev[b]) return HK_EINVAL;
+        if (!ctxs[b]->have_cond || !ctxs[b]->ws) return HK_ESTATE;
+    }
+    for (int32_t b = 0; b < n_bands; ++b) {
+        const int rc = compute_any(ctxs[b], lines, n_lines, cut_cm, out_k_dev[b], (cudaStream_t)stream_v, true);
+        if (rc != HK_OK) return rc;
+    }
+    return HK_OK;
+}
+
 // ---- HITRAN-style inputs ------------------------------------------------------------------
 namespace {
 bool hitran_ok(const hk_lines_hitran* l)

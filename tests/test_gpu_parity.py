@@ -425,6 +425,32 @@ def test_width_relative_cutting_length(B, case, mode, factor):
         op.close()
 
 
+def test_bands_of_different_resolution(B):
+    """hk_compute_bands: three bands at 0.05 / 0.01 / 0.1 cm^-1; every band against the oracle on its own
+    grid (lines near a band edge reach into both bands)."""
+    lines, cond, _, cut = _mini(2, 20_000)
+    bands = [(0.0, 3000.0, 0.05), (3000.0, 4200.0, 0.01), (4200.0, 10000.0, 0.1)]
+    ops = []
+    for g in bands:
+        op = B.Opacity(*g)
+        op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        ops.append(op)
+    outs = B.compute_bands(ops, _to_cuda(lines), cut)
+    torch.cuda.synchronize()
+    total = 0
+    for g, op, k in zip(bands, ops, outs):
+        k_ref, evals = O.opacity_grid(lines, cond, g, cut)
+        assert op.stats()["n_evals"] == evals
+        total += evals
+        check_parity(k.cpu().numpy(), k_ref, what=f"band {g}")
+    assert total > 0
+    with pytest.raises(B.HKError) as e:
+        B.compute_bands(ops + [B.Opacity(0.0, 1.0, 0.1)], _to_cuda(lines), cut)      # a band without conditions
+    assert e.value.status == B.HK_ESTATE
+    for op in ops:
+        op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
