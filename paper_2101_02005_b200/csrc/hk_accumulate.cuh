@@ -87,19 +87,20 @@ __device__ __forceinline__ void warp_share(int n, int warp, int& w0, int& w1)
 
 // combine the warps' partial sums (red aliases the staging buffers: call after a __syncthreads that
 // follows the last read of them) and add the tile to k(nu)
-template <int KB>
+template <int KB, int W = kWarps>
 __device__ __forceinline__ void flush_tile(double* red, const double (&v)[KB], int64_t ct0, const AccArgs& a)
 {
+    constexpr int kWarps = W;
     constexpr int kTB = 32 * KB;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
     for (int j = 0; j < KB; ++j) red[warp * kTB + lane + 32 * j] = v[j];
     __syncthreads();
-    if (threadIdx.x < kTB) {
+    for (int i = threadIdx.x; i < kTB; i += 32 * kWarps) {
         double s = 0.0;
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) s += red[w * kTB + threadIdx.x];
-        const int64_t b = ct0 + threadIdx.x;
+        for (int w = 0; w < kWarps; ++w) s += red[w * kTB + i];
+        const int64_t b = ct0 + i;
         s *= scalbn(1.0, -a.st->scale_exp);
         if (b < a.N && s != 0.0) atomicAdd(a.out_k + b, s);
     }
@@ -429,9 +430,12 @@ __device__ __forceinline__ int y_class(float y)
     return 31;
 }
 
-template <int KB>
-__global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a)
+// W = warps per CTA: 8 for dense lists; 2 for sparse ones (few lines per tile: a work unit is a handful of lines, and
+// four times as many small CTAs keep four times as many units in flight)
+template <int KB, int W>
+__global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_kernel(AccArgs a)
 {
+    constexpr int kWarps = W, kThreads = 32 * W, kSubC = 64 * W, kLPTC = kSubC / kThreads;   // shadow the 8-warp values
     constexpr int kTB = 32 * KB;
     constexpr int M = KB / 2;
     static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubC, "red must fit in the staging buffers");
@@ -681,7 +685,7 @@ __global__ void __launch_bounds__(kThreads, kCentreCtas) centre_kernel(AccArgs a
         }
         flush();
         __syncthreads();               // every warp is done with the staging buffers: red may overwrite them
-        flush_tile<KB>(red, acc64, ct0, a);
+        flush_tile<KB, W>(red, acc64, ct0, a);
     }
 }
 

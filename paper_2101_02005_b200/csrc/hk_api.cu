@@ -532,7 +532,16 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
             ctx->last_launches += 3;
         }
         cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
-        if (p.mode == 0 || p.mode == 3) { centre_kernel<KB><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+        if (p.mode == 0 || p.mode == 3) {
+            // sparse lists (fewer than 256 lines per level-0 tile on average): 2-warp CTAs, four times as many
+            if ((double)n_lines * (32.0 * KB) < 32.0 * (double)ctx->N)
+                centre_kernel<KB, 1><<<ctx->n_sm * kCentreCtas * 8, 32, 0, stream>>>(a);
+            else if ((double)n_lines * (32.0 * KB) < 256.0 * (double)ctx->N)
+                centre_kernel<KB, 2><<<ctx->n_sm * kCentreCtas * 4, 64, 0, stream>>>(a);
+            else
+                centre_kernel<KB, kWarps><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a);
+            ++ctx->last_launches;
+        }
         cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
         near_kernel<KB><<<grid, kThreads, 0, stream>>>(a);
         ++ctx->last_launches;
