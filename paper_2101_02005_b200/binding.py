@@ -168,7 +168,7 @@ class Opacity:
             raise HKError(st, where, _lib.hk_last_cuda_error(self._ctx))
 
     def close(self):
-        if getattr(self, "_ctx", None):
+        if getattr(self, "_ctx", None) and _lib is not None:      # (_lib is gone when the interpreter shuts down)
             _lib.hk_destroy(self._ctx)
             self._ctx = None
 
