@@ -210,11 +210,20 @@ double hko_profile(double nu, double nu0, double gammaL, double alphaD)
  *   0 Voigt    K = Re w(x + i y)
  *   1 Lorentz  V = Gamma_L/(pi ((nu - nu0)^2 + Gamma_L^2))          => K = y/(sqrt(pi) (x^2 + y^2))
  *   2 Doppler  V = exp(-x^2)/(alpha_D sqrt(pi))                      => K = exp(-x^2)
- * (the binned Gaussian of ExoCross is not built). */
-static double shape_K(int profile, double x, double y)
+ *   3 binned Gaussian: the Doppler profile averaged over each bin (see below) */
+static double shape_K(int profile, double x, double y, double hx)
 {
     if (profile == 1) return y / (sqrt(HKO_PI) * (x * x + y * y));
     if (profile == 2) return exp(-x * x);
+    if (profile == 3) {
+        /* "binned Gaussian integrated cross section" of ExoCross (L47; PAPER.md prints no formula: DESIGN.md R26):
+         * the Doppler profile averaged over the bin [nu_i - dnu/2, nu_i + dnu/2],
+         *   V_i = (1/(2 dnu)) [erf(x + hx) - erf(x - hx)],  hx = dnu/(2 alpha_D)  =>  K = V alpha_D sqrt(pi).
+         * erfc in the tails, where the two erf are both within rounding of 1. */
+        double u = fabs(x), lo = u - hx, hi = u + hx;
+        double d = lo >= 0.0 ? erfc(lo) - erfc(hi) : erf(hi) - erf(lo);
+        return sqrt(HKO_PI) / (4.0 * hx) * d;
+    }
     return hko_voigt_K(x, y);
 }
 
@@ -275,7 +284,7 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
                 pl[q] = 0.0;
             } else {
                 line_extent(nu0[l], numin, dnu, N, cl, &ilo[q], &ihi[q], &jc);
-                pl[q] = use_plinth ? shape_K(profile, cl / aD[q], gL[q] / aD[q]) : 0.0;
+                pl[q] = use_plinth ? shape_K(profile, cl / aD[q], gL[q] / aD[q], dnu / (2.0 * aD[q])) : 0.0;
             }
         } else { S[q] = 0.0; gL[q] = 0.0; aD[q] = 1.0; ilo[q] = 0; ihi[q] = -1; pl[q] = 0.0; }
     }
@@ -290,7 +299,7 @@ void hko_opacity_bins_ex(int64_t n, const double *nu0, const double *A, const do
             if (i < ilo[q] || i > ihi[q]) continue;
             double x = (nu - nu0[l0 + q]) / aD[q];
             double y = gL[q] / aD[q];
-            double term = S[q] * (shape_K(profile, x, y) - pl[q]) / (aD[q] * sqrtpi);
+            double term = S[q] * (shape_K(profile, x, y, dnu / (2.0 * aD[q])) - pl[q]) / (aD[q] * sqrtpi);
             double t = sum + term;                 /* Neumaier */
             if (fabs(sum) >= fabs(term)) comp += (sum - t) + term;
             else comp += (term - t) + sum;

@@ -104,7 +104,7 @@ def profile(nu, nu0, gammaL, alphaD) -> float:
     return float(_lib.hko_profile(nu, nu0, gammaL, alphaD))
 
 
-PROFILES = {"voigt": 0, "lorentz": 1, "doppler": 2}
+PROFILES = {"voigt": 0, "lorentz": 1, "doppler": 2, "binned_gaussian": 3}
 
 
 CUT_MODES = {"fixed": 0, "lorentz": 1, "doppler": 2}

@@ -71,3 +71,29 @@ def test_plinth_uses_the_selected_profile():
     k1, _ = O.opacity_grid(L, COND, grid, cut, profile="lorentz", plinth=True)
     inside = k0 > 0
     assert np.abs((k0 - k1)[inside] - S[0] * gL[0] / (np.pi * (cut * cut + gL[0] ** 2))).max() <= 1e-12 * k0.max()
+
+
+def test_binned_gaussian_conserves_the_integral_and_reaches_its_limits():
+    """Bin average of the Doppler profile (R26): sum_i V_i dnu = 1 at ANY resolution (the erf differences
+    telescope), the Doppler profile when the line is resolved, one bin of height 1/dnu when it is not."""
+    L = _one()
+    S, gL, aD, _ = O.line_params(L, **COND)
+    a = aD[0]
+    for dnu in (a / 40.0, a / 3.0, a * 2.5, a * 300.0):
+        n = 2000
+        grid = (500.0 - (n + 0.3) * dnu, 500.0 + (n - 0.3) * dnu, dnu)       # centre 0.3 bins off a grid point
+        k, _ = O.opacity_grid(L, COND, grid, 0.0, profile="binned_gaussian")
+        assert k.sum() * dnu == pytest.approx(S[0], rel=1e-10)
+        if dnu < a / 30.0:
+            kd, _ = O.opacity_grid(L, COND, grid, 0.0, profile="doppler")
+            x = (grid[0] + np.arange(k.size) * dnu - 500.0) / a
+            m = np.abs(x) < 3.0
+            h = dnu / (2 * a)
+            assert np.abs(k[m] / kd[m] - (1.0 + h * h * (2 * x[m] ** 2 - 1) / 3.0)).max() <= 1e-6   # second-order bin average
+        if dnu > 100.0 * a:
+            jc = int(np.argmax(k))
+            assert k[jc] * dnu == pytest.approx(S[0], rel=1e-10) and np.count_nonzero(k > 1e-30 * k[jc]) == 1
+    # symmetric about the centre when it sits on a grid point
+    grid = (500.0 - 50 * a, 500.0 + 50 * a, a / 4.0)
+    k, _ = O.opacity_grid(L, COND, grid, 0.0, profile="binned_gaussian")
+    assert np.abs(k[1:] - k[1:][::-1]).max() <= 1e-9 * k.max()         # (grid points round differently left and right)
