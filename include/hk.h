@@ -114,10 +114,14 @@ int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, do
  *   HK_PROFILE_VOIGT   Re w(x + i y)/(alpha_D sqrt(pi))                      (default)
  *   HK_PROFILE_LORENTZ Gamma_L/(pi ((nu - nu0)^2 + Gamma_L^2))
  *   HK_PROFILE_DOPPLER exp(-((nu - nu0)/alpha_D)^2)/(alpha_D sqrt(pi)); values below e^-40 of the peak are dropped
- * The binned Gaussian of ExoCross (L47) is not built.  HK_EINVAL for any other value. */
+ *   HK_PROFILE_BINNED_GAUSSIAN  the "binned Gaussian integrated cross section" of ExoCross (L47): the Doppler profile
+ *                      averaged over each bin, (1/(2 dnu)) [erf((nu_i + dnu/2 - nu0)/alpha_D) - erf((nu_i - dnu/2 - nu0)/alpha_D)]
+ *                      (PAPER.md names it and prints no formula: DESIGN.md R26); conserves sum_i V_i dnu = 1 at any resolution
+ * HK_EINVAL for any other value. */
 #define HK_PROFILE_VOIGT 0
 #define HK_PROFILE_LORENTZ 1
 #define HK_PROFILE_DOPPLER 2
+#define HK_PROFILE_BINNED_GAUSSIAN 3
 int hk_set_profile(hk_ctx* ctx, int profile);
 
 /* Cutting length (L239: "a fixed cutting length, a fraction of the Doppler half-width, or a fraction of the Lorentzian

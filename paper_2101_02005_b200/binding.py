@@ -187,8 +187,8 @@ class Opacity:
         self._check(_lib.hk_set_node_separation(self._ctx, sep), "hk_set_node_separation")
 
     def set_profile(self, profile):
-        """'voigt' (default), 'lorentz' or 'doppler' (hk_set_profile)."""
-        code = {"voigt": 0, "lorentz": 1, "doppler": 2}.get(profile, profile)
+        """'voigt' (default), 'lorentz', 'doppler' or 'binned_gaussian' (hk_set_profile)."""
+        code = {"voigt": 0, "lorentz": 1, "doppler": 2, "binned_gaussian": 3}.get(profile, profile)
         self._check(_lib.hk_set_profile(self._ctx, int(code)), "hk_set_profile")
 
     def set_cut_mode(self, mode):

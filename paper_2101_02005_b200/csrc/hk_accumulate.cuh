@@ -52,6 +52,7 @@ struct AccArgs {
     double* __restrict__ edge_acc;             // [2][N][kP] per-bin node sums of extent ends (scaled), fp64; or null
     int64_t N;
     int32_t n_ct, chunk, chunk_node;
+    int32_t profile;                           // HK_PROFILE_*: only the binned Gaussian changes the kernels' core evaluation
     Levels lv;
 };
 
@@ -432,7 +433,8 @@ __device__ __forceinline__ int y_class(float y)
 
 // W = warps per CTA: 8 for dense lists; 2 for sparse ones (few lines per tile: a work unit is a handful of lines, and
 // four times as many small CTAs keep four times as many units in flight)
-template <int KB, int W>
+// kBinned: the binned-Gaussian profile (its own instantiation, so that the Voigt path carries none of its code)
+template <int KB, int W, bool kBinned>
 __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_kernel(AccArgs a)
 {
     constexpr int kWarps = W, kThreads = 32 * W, kSubC = 64 * W, kLPTC = kSubC / kThreads;   // shadow the 8-warp values
@@ -545,10 +547,11 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                     const float qmin = fmaf(dmin, dmin, G2) * 0.9999f, qmax = fmaf(dmax, dmax, G2);
                     const float qc = (HK_Z2 / 1.5f) * (1.5f * a2);            // as the row pass recomputes it
                     // Gauss-Hermite rows: the tile holds core bins and (D1 D2 ~ |z|^8) stays inside fp32
-                    const float ql = (qmin < qc && qmax <= 1.0e9f * a2) ? HK_Z4 * a2 : qc;
+                    constexpr bool binned = kBinned;
+                    const float ql = binned ? binned_ql(a2) : (qmin < qc && qmax <= 1.0e9f * a2) ? HK_Z4 * a2 : qc;
                     // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y }: Gauss-Hermite rows (B.y < 0) carry P = cK y and
                     // Q = 1/a^2, two-term rows P = c (Lorentz amplitude) and Q = 1.5 a^2 -- what the row pass needs, ready
-                    if (ql < qc) {
+                    if (!binned && ql < qc) {
                         smA[dst] = make_float4(-fdj, G2, rb.w * yv[k], 1.0f / a2);
                         smB[dst] = make_float4(-ra.y, -ql, rb.w, yv[k]);
                     } else {
@@ -663,7 +666,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                                 const float t = (e0 + (float)s) - f;             // the row pass's t, bit for bit
                                 const float q = fmaf(t, t, G2);
                                 float val = 0.f;
-                                if (q < ql) val = cK * core_any_K(fabsf(t) * inv_a, y, nullptr);
+                                if (q < ql) val = cK * (kBinned ? binned_K(fabsf(t), inv_a) : core_any_K(fabsf(t) * inv_a, y, nullptr));
                                 stage[warp][s][lane] = val;
                             }
                         }
@@ -705,13 +708,13 @@ constexpr int kFlagWide = 8;           // core spans >= 16 bins: evaluated in th
 // C = { ilo - ct0, ihi - ct0, y, flags }.
 template <int KB, bool kTwoTerm, bool kMask, bool kCore>
 __device__ __forceinline__ void near_rows(float2 (&acc)[KB / 2], const float2 (&tb)[KB / 2], const float4 A,
-                                          const float4 B, const float4 C, const bool wide)
+                                          const float4 B, const float4 C, const bool wide, const int profile = 0)
 {
     const float2 ndl = bcast2(-A.x), nf = bcast2(-A.y), g = bcast2(A.z);
     const float2 A1 = bcast2(B.x), nA2 = bcast2(B.y), one = bcast2(1.0f);
     const float c = A.w, qc = B.z, lo = C.x, hi = C.y;
     float inv_a = 0.f;
-    if (kCore && wide) inv_a = rsqrtf(qc * (1.0f / HK_Z2));
+    if (kCore && wide) inv_a = profile == HK_PROFILE_BINNED_GAUSSIAN ? C.z : rsqrtf(qc * (1.0f / HK_Z2));
 #pragma unroll
     for (int m = 0; m < KB / 2; ++m) {
         const float2 d = __fadd2_rn(tb[m], ndl);            // exact: both are small integers
@@ -734,10 +737,10 @@ __device__ __forceinline__ void near_rows(float2 (&acc)[KB / 2], const float2 (&
         acc[m] = __ffma2_rn(cm, ww, acc[m]);
         if (kCore && wide) {
             if (__any_sync(0xffffffffu, in0 && co0)) {
-                if (in0 && co0) acc[m].x = fmaf(B.w, core_any_K(fabsf(t.x) * inv_a, C.z, nullptr), acc[m].x);
+                if (in0 && co0) acc[m].x = fmaf(B.w, core_eval(profile, fabsf(t.x), inv_a, C.z), acc[m].x);
             }
             if (__any_sync(0xffffffffu, in1 && co1)) {
-                if (in1 && co1) acc[m].y = fmaf(B.w, core_any_K(fabsf(t.y) * inv_a, C.z, nullptr), acc[m].y);
+                if (in1 && co1) acc[m].y = fmaf(B.w, core_eval(profile, fabsf(t.y), inv_a, C.z), acc[m].y);
             }
         }
     }
@@ -837,7 +840,8 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                     dhi = max(-lim, min(lim, dhi));
                     const float fdj = (float)dj, flo = (float)dlo, fhi = (float)dhi;
                     const float G2 = ra.z, a2 = rb.x;
-                    const float qc = HK_Z2 * a2;
+                    const bool binned = a.profile == HK_PROFILE_BINNED_GAUSSIAN;
+                    const float qc = binned ? binned_ql(a2) : HK_Z2 * a2;
                     // smallest q = t^2 + G2 over the tile's bins, from below
                     const float pos = fdj + ra.y;
                     const float dist = fmaxf(fmaxf(-pos, pos - whi), 0.f) * 0.999f;
@@ -845,11 +849,12 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                     int flags = 0;
                     if (flo <= 0.f && fhi >= whi) flags |= kFlagFull;
                     if (qmin >= qc) flags |= kFlagNoCore;
-                    if (qmin >= HK_Z1 * a2) flags |= kFlagFar;
+                    if (qmin >= fmaxf(HK_Z1 * a2, qc)) flags |= kFlagFar;
                     if ((qc - G2) >= kWideCore) flags |= kFlagWide;
                     smA[i] = make_float4(fdj, ra.y, G2, ra.w);
                     smB[i] = make_float4(1.5f * a2, -2.0f * a2 * G2, qc, rb.w);
-                    smC[i] = make_float4(flo, fhi, sqrtf(G2) * rsqrtf(a2), __int_as_float(flags));
+                    // C.z: y for the Voigt evaluators; the binned Gaussian needs 1/a instead (its y is 0)
+                    smC[i] = make_float4(flo, fhi, binned ? rsqrtf(a2) : sqrtf(G2) * rsqrtf(a2), __int_as_float(flags));
                 }
             }
         };
@@ -873,7 +878,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                     if (flags & kFlagFull) near_rows<KB, true, false, false>(acc, tb, A, B, C, false);
                     else near_rows<KB, true, true, false>(acc, tb, A, B, C, false);
                 } else {
-                    near_rows<KB, true, true, true>(acc, tb, A, B, C, (flags & kFlagWide) != 0);
+                    near_rows<KB, true, true, true>(acc, tb, A, B, C, (flags & kFlagWide) != 0, a.profile);
                 }
                 if (++since_flush >= kFlush) flush();
             }
@@ -901,7 +906,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) maxcnt = max(maxcnt, __shfl_xor_sync(0xffffffffu, maxcnt, o));
                 if (maxcnt == 0) continue;
-                const float inv_a = rsqrtf(fmaxf(qc, 1e-30f) * (1.0f / HK_Z2));
+                const float inv_a = a.profile == HK_PROFILE_BINNED_GAUSSIAN ? y : rsqrtf(fmaxf(qc, 1e-30f) * (1.0f / HK_Z2));
                 for (int o = 0; o < maxcnt; ++o) {
                     float val = 0.f;
                     int bin = -1;
@@ -910,7 +915,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                         const float d = fb - dlt;
                         const float t = d - f;
                         const float q = fmaf(t, t, G2);
-                        if (q < qc) { val = cK * core_any_K(fabsf(t) * inv_a, y, nullptr); bin = (int)fb; }
+                        if (q < qc) { val = cK * core_eval(a.profile, fabsf(t), inv_a, y); bin = (int)fb; }
                     }
                     // combine equal bins in the warp (sorted lines: neighbours share bins), one add per distinct bin
                     unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
@@ -1248,7 +1253,9 @@ __global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const 
             const double cb = p.cut_mode == 0 ? p.cut_bins
                             : p.cut_factor * (p.cut_mode == 1 ? sqrt(G2) : sqrt(a2) * 0.83255461115769775635);
             const double q = cb * cb + G2;
-            if (q >= (double)HK_Z2 * a2) {
+            if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) {
+                if (q < (double)binned_ql(rb.x)) pl = (double)(rb.w * binned_K((float)cb, rsqrtf(rb.x)));
+            } else if (q >= (double)HK_Z2 * a2) {
                 // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q)
                 pl = (double)ra.w / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
             } else {

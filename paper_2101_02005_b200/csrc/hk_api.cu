@@ -388,7 +388,7 @@ int hk_set_cut_mode(hk_ctx* ctx, int mode)
 
 int hk_set_profile(hk_ctx* ctx, int profile)
 {
-    if (!ctx || profile < HK_PROFILE_VOIGT || profile > HK_PROFILE_DOPPLER) return HK_EINVAL;
+    if (!ctx || profile < HK_PROFILE_VOIGT || profile > HK_PROFILE_BINNED_GAUSSIAN) return HK_EINVAL;
     ctx->profile = profile;
     return HK_OK;
 }
@@ -508,7 +508,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     a.prefix_far = prefix; a.prefix_mid = prefix + p.n_ct; a.prefix_edge = prefix + 2 * p.n_ct;
     a.prefix_centre = prefix + 3 * p.n_ct; a.prefix_near = prefix + 4 * p.n_ct;
     a.prefix_node = prefix + 5 * p.n_ct;
-    a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc;
+    a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc; a.profile = p.profile;
     const bool use_edge_nodes = p.edge_nodes && p.mode == 0 && lv.n_levels > 0 && !p.uncut;
     a.edge_acc = use_edge_nodes ? edge_acc : nullptr;
     a.plinth_acc = p.plinth ? (double*)(ws + L.plinth_acc) : nullptr;
@@ -534,12 +534,17 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
         if (p.mode == 0 || p.mode == 3) {
             // sparse lists (fewer than 256 lines per level-0 tile on average): 2-warp CTAs, four times as many
-            if ((double)n_lines * (32.0 * KB) < 32.0 * (double)ctx->N)
-                centre_kernel<KB, 1><<<ctx->n_sm * kCentreCtas * 8, 32, 0, stream>>>(a);
-            else if ((double)n_lines * (32.0 * KB) < 256.0 * (double)ctx->N)
-                centre_kernel<KB, 2><<<ctx->n_sm * kCentreCtas * 4, 64, 0, stream>>>(a);
-            else
-                centre_kernel<KB, kWarps><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a);
+            auto centre = [&](auto binned_tag) {
+                constexpr bool kB = decltype(binned_tag)::value;
+                if ((double)n_lines * (32.0 * KB) < 32.0 * (double)ctx->N)
+                    centre_kernel<KB, 1, kB><<<ctx->n_sm * kCentreCtas * 8, 32, 0, stream>>>(a);
+                else if ((double)n_lines * (32.0 * KB) < 256.0 * (double)ctx->N)
+                    centre_kernel<KB, 2, kB><<<ctx->n_sm * kCentreCtas * 4, 64, 0, stream>>>(a);
+                else
+                    centre_kernel<KB, kWarps, kB><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a);
+            };
+            if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) centre(std::true_type());
+            else centre(std::false_type());
             ++ctx->last_launches;
         }
         cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);

@@ -183,7 +183,8 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             ++off;
             r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);
         } else {
-            double Gb = p.profile == HK_PROFILE_DOPPLER ? 0.0 : o.gammaL / p.dnu, ab = o.alphaD / p.dnu;
+            double Gb = (p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN) ? 0.0 : o.gammaL / p.dnu;
+            double ab = o.alphaD / p.dnu;
             r.jc = (int32_t)o.jc;
             r.f = fminf((float)o.pos_f, 0.99999994f);
             r.G2 = (float)(Gb * Gb);

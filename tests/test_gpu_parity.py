@@ -290,7 +290,7 @@ def test_plinth_removal(B, case):
     op.close()
 
 
-@pytest.mark.parametrize("profile", ["lorentz", "doppler"])
+@pytest.mark.parametrize("profile", ["lorentz", "doppler", "binned_gaussian"])
 @pytest.mark.parametrize("case", ["config2", "config3", "resolved", "uncut"])
 def test_lorentz_and_doppler_profiles(B, profile, case):
     """hk_set_profile (section 2.1) against the oracle's profile options, with and
