@@ -31,7 +31,7 @@ constexpr int32_t kKeySentinelBias = 1;  // sentinel key = kmax + 1
 // ---- unsorted per-line record written by the preprocess kernel (32 B)
 struct __align__(16) RecU {
     int32_t jc;      // centre bin floor((nu0-numin)/dnu)
-    float f;         // sub-bin offset in [0,1)
+    float f;         // sub-bin offset from the NEAREST grid point, [-1/2, 1/2]; sign bit set (-0 too): the point is jc + 1
     float G2;        // (Gamma_L/dnu)^2
     float a2;        // (alpha_D/dnu)^2
     int32_t ilo;     // inclusive integer extent
@@ -40,7 +40,8 @@ struct __align__(16) RecU {
 };
 
 // sorted records consumed by the accumulation kernels: two float4 streams
-//   A = { jc (int bits), f, G2, c }        c  = scale * S * Gamma_L/(pi dnu^2)   (Lorentz amplitude, bin units)
+//   A = { jp (int bits), f, G2, c }        centre = jp + f, jp the NEAREST grid point, f in [-1/2, 1/2];
+//                                          c  = scale * S * Gamma_L/(pi dnu^2)   (Lorentz amplitude, bin units)
 //   B = { a2, ilo (int bits), ihi (int bits), cK }   cK = scale * S/(alpha_D sqrt(pi))
 
 //   N = { jc (int bits), (f13 << 19) | a2_19, G2, c }   compact record of the node kernel: f13 = sub-bin offset in

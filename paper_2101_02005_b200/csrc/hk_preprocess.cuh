@@ -186,7 +186,10 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             double Gb = (p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN) ? 0.0 : o.gammaL / p.dnu;
             double ab = o.alphaD / p.dnu;
             r.jc = (int32_t)o.jc;
-            r.f = fminf((float)o.pos_f, 0.99999994f);
+            // sub-bin offset relative to the NEAREST grid point, in [-1/2, 1/2]: the profile is sampled at grid points, so
+            // a centre that (almost) coincides with one needs its tiny offset at full relative precision (a narrow
+            // Lorentzian sampled at its peak).  Negative (sign bit set, -0 included): the nearest point is jc + 1.
+            r.f = (float)(o.pos_f > 0.5 ? o.pos_f - 1.0 : o.pos_f);
             r.G2 = (float)(Gb * Gb);
             r.a2 = (float)(ab * ab);
             r.ilo = (int32_t)o.ilo;
@@ -266,9 +269,10 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
         // a pure Lorentzian is what every formula of the accumulation kernels reduces to at alpha_D = 0 (no core,
         // no second asymptotic term); a pure Gaussian is the Voigt function at Gamma_L = 0 (c = 0: no wings)
         const float a2 = profile == HK_PROFILE_LORENTZ ? 0.f : r.a2;
-        recA[i] = make_float4(__int_as_float(r.jc), r.f, r.G2, c);
+        const bool up = signbit(r.f);                                  // centre = (jc + 1) + f with f <= 0
+        recA[i] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, r.G2, c);
         recB[i] = make_float4(a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
-        const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn(r.f * 8192.0f));
+        const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));   // floor-based, [0, 1)
         const uint32_t a19 = ((uint32_t)__float_as_int(a2) >> 12) & 0x7FFFFu;
         recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), r.G2, c);
     }

@@ -451,6 +451,48 @@ def test_bands_of_different_resolution(B):
         op.close()
 
 
+@pytest.mark.parametrize("seed", range(40))
+def test_randomised_small_cases(B, seed):
+    """Differential fuzz: random grids (offset, span, resolution from 1e-3 to 1 cm^-1), cuts from below a bin to beyond
+    the grid or none, conditions, line densities from one line to dense, every tile geometry and both extent-end paths,
+    against the oracle on all bins at the north_star tolerance, with exact integer work counts."""
+    rng = np.random.default_rng(1000 + seed)
+    dnu = float(10 ** rng.uniform(-3, 0))
+    nbins = int(rng.integers(1, 60_000))
+    numin = float(rng.choice([0.0, rng.uniform(0.0, 2.0e4)]))
+    grid = (numin, numin + nbins * dnu, dnu)
+    span = nbins * dnu
+    cut = float(rng.choice([0.0, 10 ** rng.uniform(np.log10(0.3 * dnu), np.log10(3.0 * span + 10 * dnu))]))
+    n = int(rng.choice([1, 2, 30, 400, 3000]))
+    pad = min(cut if cut > 0 else 5.0, 50.0)
+    nu0 = np.abs(rng.uniform(numin - pad, numin + span + pad, n)) + 1e-3
+    if rng.random() < 0.3:
+        nu0[: n // 2] = numin + dnu * rng.integers(0, nbins, n // 2)          # centres exactly on grid points
+    lines = _simple_lines(nu0, A=10 ** rng.uniform(-6, 4, n), g_up=rng.integers(1, 30, n).astype(float),
+                          E_low=rng.uniform(0, 8000, n), gamma_ref=10 ** rng.uniform(-3, -0.3, n),
+                          n_exp=rng.uniform(0.4, 0.8, n))
+    cond = dict(T=float(rng.uniform(200, 3000)), P_atm=float(10 ** rng.uniform(-3, 1.7)),
+                mass_amu=float(rng.uniform(2, 200)), Q=float(10 ** rng.uniform(0, 4)))
+    profile = str(rng.choice(["voigt", "voigt", "lorentz"]))
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_profile(profile)
+    op.set_tile_bins(int(rng.choice([0, 2, 4, 8])))
+    op.set_edge_nodes(bool(rng.integers(0, 2)))
+    dl = _to_cuda(lines)
+    k = op.compute(dl, cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut, profile=profile)
+    ext = tuple(t.cpu().numpy() for t in op.extents(dl))
+    assert _check_extents(ext, lines, cond, grid, cut) == evals == st["n_evals"]
+    if k_ref.max() > 0:
+        check_parity(k.cpu().numpy(), k_ref, what=f"fuzz {seed}: grid {grid} cut {cut:g} n {n} {profile} {cond}")
+    else:
+        assert float(k.abs().max()) == 0.0
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
