@@ -1211,9 +1211,9 @@ __global__ void __launch_bounds__(256) edge_bins_kernel(AccArgs a)
 // ---------------------------------------------------------------------------------------
 // plinth removal (section 2.1.1): subtract S V(cut) of every line from every bin of its extent
 // ---------------------------------------------------------------------------------------
-// The removed part is a sum of boxes, one per line: -p_l on [ilo, ihi].  Lanes walk the sorted lines, evaluate p_l
-// from the SAME fp32 record the accumulation kernels use (so V - V(cut) goes to zero consistently at the extent's
-// ends) with the same region split, and add -p_l at ilo and +p_l at ihi + 1 of a difference array (equal bins summed
+// The removed part is a sum of boxes, one per line: -p_l on [ilo, ihi].  Lanes walk the lines, evaluate p_l from the
+// SAME fp32 widths the accumulation kernels use (so V - V(cut) goes to zero consistently at the extent's ends) with
+// the same region split, and add -p_l at ilo and +p_l at ihi + 1 of a difference array (equal bins summed
 // in the warp first); a running sum over the bins (CUB) turns it into the box sum, plinth_apply_kernel adds it to k.
 __device__ __forceinline__ void warp_add_scalar_by_bin(double* __restrict__ acc, int64_t bin, double v, int lane)
 {
@@ -1233,36 +1233,39 @@ __device__ __forceinline__ void warp_add_scalar_by_bin(double* __restrict__ acc,
     }
 }
 
-__global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys, int32_t n)
+__global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const RecU* __restrict__ rec, int64_t n)
 {
-    __shared__ int32_t s_nact;
-    if (threadIdx.x == 0) s_nact = lower_bound_key(keys, n, (int64_t)p.ksent);
-    __syncthreads();
-    const int32_t n_act = s_nact;
+    // over the UNSORTED per-line records: they hold the true widths (the profile variants zero one of them only in the
+    // sorted records), which a width-relative cutting length needs, and the unscaled fp64 amplitude
     const int lane = threadIdx.x & 31;
-    const double unscale = scalbn(1.0, -a.st->scale_exp);
-    const int64_t n_round = ((int64_t)n_act + 31) & ~31LL;
+    const int64_t n_round = (n + 31) & ~31LL;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
         int64_t ilo = 0, ihi = -1;
         double pl = 0.0;
-        if (i < n_act) {
-            const float4 ra = a.recA[i], rb = a.recB[i];
-            ilo = __float_as_int(rb.y); ihi = __float_as_int(rb.z);
-            const double G2 = (double)ra.z, a2 = (double)rb.x;
-            // the line's own cutting length in bins (width-relative modes: from the record, as the kernels see it)
-            const double cb = p.cut_mode == 0 ? p.cut_bins
-                            : p.cut_factor * (p.cut_mode == 1 ? sqrt(G2) : sqrt(a2) * 0.83255461115769775635);
-            const double q = cb * cb + G2;
-            if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) {
-                if (q < (double)binned_ql(rb.x)) pl = (double)(rb.w * binned_K((float)cb, rsqrtf(rb.x)));
-            } else if (q >= (double)HK_Z2 * a2) {
-                // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q)
-                pl = (double)ra.w / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
-            } else {
-                const float inv_a = rsqrtf(rb.x);
-                pl = (double)(rb.w * core_any_K((float)cb * inv_a, sqrtf(ra.z) * inv_a, nullptr));
+        if (i < n) {
+            const RecU r = rec[i];
+            ilo = r.ilo; ihi = r.ihi;
+            if (ihi >= ilo) {
+                const double G2t = (double)r.G2, a2 = (double)r.a2;
+                // the line's own cutting length in bins
+                const double cb = p.cut_mode == 0 ? p.cut_bins
+                                : p.cut_factor * (p.cut_mode == 1 ? sqrt(G2t) : sqrt(a2) * 0.83255461115769775635);
+                const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
+                const double G2 = gauss ? 0.0 : G2t;
+                const double q = cb * cb + G2;
+                const double c = r.cK * sqrt(G2 * a2) * 0.56418958354775628695;        // Lorentz amplitude, as gather_kernel
+                if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) {
+                    if (q < (double)binned_ql(r.a2)) pl = r.cK * (double)binned_K((float)cb, rsqrtf(r.a2));
+                } else if (p.profile == HK_PROFILE_LORENTZ) {
+                    pl = c / q;
+                } else if (q >= (double)HK_Z2 * a2) {
+                    // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q)
+                    pl = c / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
+                } else {
+                    const float inv_a = rsqrtf(r.a2);
+                    pl = r.cK * (double)core_any_K((float)cb * inv_a, sqrtf((float)G2) * inv_a, nullptr);
+                }
             }
-            pl *= unscale;
         }
         const bool live = ihi >= ilo;
         warp_add_scalar_by_bin(a.plinth_acc, live ? ilo : -1, -pl, lane);

@@ -568,7 +568,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     // plinth removal: difference array over the sorted lines -> running sum over the bins -> subtract
     if (p.plinth) {
         HK_CUDA(cudaMemsetAsync(a.plinth_acc, 0, (size_t)(ctx->N + 1) * sizeof(double), stream));
-        plinth_kernel<<<ctx->n_sm * 8, 256, 0, stream>>>(p, a, keys_out, n);
+        plinth_kernel<<<ctx->n_sm * 8, 256, 0, stream>>>(p, a, recU, (int64_t)n);
         cub_bytes = L.cub_bytes;
         HK_CUDA(cub::DeviceScan::InclusiveSum(ws + L.cub, cub_bytes, (const double*)a.plinth_acc, a.plinth_acc,
                                               (int)(ctx->N + 1), stream));

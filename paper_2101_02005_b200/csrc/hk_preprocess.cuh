@@ -183,8 +183,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             ++off;
             r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);
         } else {
-            double Gb = (p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN) ? 0.0 : o.gammaL / p.dnu;
-            double ab = o.alphaD / p.dnu;
+            double Gb = o.gammaL / p.dnu, ab = o.alphaD / p.dnu;     // the record keeps the TRUE widths (gather_kernel applies the profile)
             r.jc = (int32_t)o.jc;
             // sub-bin offset relative to the NEAREST grid point, in [-1/2, 1/2]: the profile is sampled at grid points, so
             // a centre that (almost) coincides with one needs its tiny offset at full relative precision (a narrow
@@ -195,7 +194,9 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             r.ilo = (int32_t)o.ilo;
             r.ihi = (int32_t)o.ihi;
             r.cK = o.S / (o.alphaD * 1.772453850905516027298);          // S/(alpha_D sqrt(pi))
-            double cl = o.S * Gb / (kPi * p.dnu);                       // Lorentz amplitude in bin units
+            const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
+            double cl = gauss ? 0.0 : o.S * Gb / (kPi * p.dnu);         // Lorentz amplitude in bin units (none for a Gaussian)
+            if (gauss) Gb = 0.0;                                        // region counters below: y = 0
             k = (int32_t)(o.jc - p.kmin);
             cmaxb = max(cmaxb, (unsigned long long)__double_as_longlong(cl));
             cKmaxb = max(cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
@@ -265,16 +266,18 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
         const RecU r = rec[idx_sorted[i]];
         float cK = (float)scalbn(r.cK, e);
         // c = cK * G a / sqrt(pi)  (Lorentz amplitude S Gamma_L/(pi dnu^2) in bin units)
-        float c = cK * sqrtf(r.G2 * r.a2) * 0.564189583547756f;
+        const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
+        const float G2 = gauss ? 0.f : r.G2;
+        float c = cK * sqrtf(G2 * r.a2) * 0.564189583547756f;
         // a pure Lorentzian is what every formula of the accumulation kernels reduces to at alpha_D = 0 (no core,
         // no second asymptotic term); a pure Gaussian is the Voigt function at Gamma_L = 0 (c = 0: no wings)
         const float a2 = profile == HK_PROFILE_LORENTZ ? 0.f : r.a2;
         const bool up = signbit(r.f);                                  // centre = (jc + 1) + f with f <= 0
-        recA[i] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, r.G2, c);
+        recA[i] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, G2, c);
         recB[i] = make_float4(a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
         const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));   // floor-based, [0, 1)
         const uint32_t a19 = ((uint32_t)__float_as_int(a2) >> 12) & 0x7FFFFu;
-        recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), r.G2, c);
+        recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), G2, c);
     }
 }
 
@@ -350,7 +353,10 @@ __device__ __forceinline__ int64_t edge_key_upL(const Params& p, int64_t w0, int
     const double m = (double)w0 + 0.5 * (double)(W - 1), h = 0.5 * (double)W;
     const int64_t sepL = (int64_t)floor(m - p.sep * h) - 1;
     const int64_t jLmid = min(left_bound((double)w0, p.kappa2, p.inv1p_k2, p.numin_bins), w0 - 1 - mind);
-    return min(min(sepL, jLmid), w1 - p.cb_floor - 1);           // and not interior: jc < jLmin = w1 - cb_floor
+    // and clearly not interior: jc <= jLmin - 2 = w1 - cb_floor - 2.  (ihi = jc + floor(cut/dnu) + 0 or 1: a line with
+    // jc = jLmin - 1 may cover the tile completely and end in the NEXT one, which the centre bin alone cannot tell;
+    // such pairs stay with the masked direct kernel, and every pair kept here has its extent end inside this tile)
+    return min(min(sepL, jLmid), w1 - p.cb_floor - 2);
 }
 __device__ __forceinline__ int64_t edge_key_dnR(const Params& p, int64_t w0, int64_t W)
 {
@@ -359,7 +365,7 @@ __device__ __forceinline__ int64_t edge_key_dnR(const Params& p, int64_t w0, int
     const double m = (double)w0 + 0.5 * (double)(W - 1), h = 0.5 * (double)W;
     const int64_t sepR = (int64_t)ceil(m + p.sep * h);
     const int64_t jRmid = max(right_bound((double)(w1 - 1), p.kappa2, p.inv1m_k2, p.numin_bins), w1 - 1 + mind);
-    return max(max(sepR, jRmid), w0 + p.cb_floor - 1);           // jc > jRmax = w0 + cb_floor - 2
+    return max(max(sepR, jRmid), w0 + p.cb_floor);               // jc >= jRmax + 2 = w0 + cb_floor (same argument, mirrored)
 }
 __device__ __forceinline__ EdgeKeys edge_keys(const Params& p, int64_t w0, int64_t W)
 {

@@ -493,6 +493,60 @@ def test_randomised_small_cases(B, seed):
     op.close()
 
 
+@pytest.mark.parametrize("seed", range(40))
+def test_randomised_variants(B, seed):
+    """Differential fuzz of the variants: every profile, plinth removal, width-relative cutting lengths, in random
+    combinations on random small problems.  With plinth removal the error is bounded against the unsubtracted opacity
+    (the cut may fall inside the cores); otherwise the north_star tolerance."""
+    rng = np.random.default_rng(5000 + seed)
+    dnu = float(10 ** rng.uniform(-3, -0.5))
+    nbins = int(rng.integers(200, 40_000))
+    numin = float(rng.choice([0.0, rng.uniform(0.0, 2.0e4)]))
+    grid = (numin, numin + nbins * dnu, dnu)
+    span = nbins * dnu
+    n = int(rng.choice([3, 50, 800, 3000]))
+    nu0 = np.abs(rng.uniform(numin - 2.0, numin + span + 2.0, n)) + 1e-3
+    lines = _simple_lines(nu0, A=10 ** rng.uniform(-6, 4, n), g_up=rng.integers(1, 30, n).astype(float),
+                          E_low=rng.uniform(0, 8000, n), gamma_ref=10 ** rng.uniform(-2.5, -0.3, n),
+                          n_exp=rng.uniform(0.4, 0.8, n))
+    cond = dict(T=float(rng.uniform(200, 3000)), P_atm=float(10 ** rng.uniform(-2, 1.7)),
+                mass_amu=float(rng.uniform(2, 200)), Q=float(10 ** rng.uniform(0, 4)))
+    profile = str(rng.choice(["voigt", "lorentz", "doppler", "binned_gaussian"]))
+    plinth = bool(rng.integers(0, 2))
+    mode = str(rng.choice(["fixed", "lorentz", "doppler"]))
+    cut = float(10 ** rng.uniform(np.log10(2 * dnu), np.log10(span))) if mode == "fixed" else float(10 ** rng.uniform(1, 3.5))
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_profile(profile)
+    op.set_plinth(plinth)
+    op.set_cut_mode(mode)
+    dl = _to_cuda(lines)
+    k = op.compute(dl, cut).cpu().numpy()
+    torch.cuda.synchronize()
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut, plinth=plinth, profile=profile, cut_mode=mode)
+    what = f"variants {seed}: {profile} plinth={plinth} cut {mode} {cut:g} grid {grid} n {n} {cond}"
+    assert op.stats()["n_evals"] == evals, what
+    assert np.all(np.isfinite(k)), what
+    if profile in ("doppler", "binned_gaussian"):
+        # a Gaussian is dropped below e^-40 of its peak (DESIGN.md R22): if no grid point comes closer than that to
+        # any line, the whole spectrum is "far tail" and there is nothing to compare
+        S, gL, aD, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        if k_ref.max() < 1e-15 * float((S / (aD * np.sqrt(np.pi))).max()):
+            assert float(np.abs(k).max()) <= 1e-15 * float((S / (aD * np.sqrt(np.pi))).max())
+            op.close()
+            return
+    if plinth:
+        k_raw, _ = O.opacity_grid(lines, cond, grid, cut, profile=profile, cut_mode=mode)
+        err = np.abs(k - k_ref)
+        bad = err > 1e-4 * k_raw + 1e-8 * max(k_raw.max(), 1e-300)
+        assert not bad.any(), (what, int(bad.sum()), float((err / np.maximum(k_raw, 1e-300))[bad].max()))
+    elif k_ref.max() > 0:
+        check_parity(k, k_ref, what=what)
+    else:
+        assert float(np.abs(k).max()) == 0.0
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
