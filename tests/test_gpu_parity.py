@@ -16,6 +16,9 @@ from parity_util import check_parity, sample_windows
 
 pytestmark = pytest.mark.gpu
 
+import os
+N_FUZZ = int(os.environ.get("HK_FUZZ_SEEDS", "40"))     # cases per randomised differential test (more: HK_FUZZ_SEEDS=400)
+
 
 @pytest.fixture(scope="module")
 def B():
@@ -451,7 +454,7 @@ def test_bands_of_different_resolution(B):
         op.close()
 
 
-@pytest.mark.parametrize("seed", range(40))
+@pytest.mark.parametrize("seed", range(N_FUZZ))
 def test_randomised_small_cases(B, seed):
     """Differential fuzz: random grids (offset, span, resolution from 1e-3 to 1 cm^-1), cuts from below a bin to beyond
     the grid or none, conditions, line densities from one line to dense, every tile geometry and both extent-end paths,
@@ -493,7 +496,7 @@ def test_randomised_small_cases(B, seed):
     op.close()
 
 
-@pytest.mark.parametrize("seed", range(40))
+@pytest.mark.parametrize("seed", range(N_FUZZ))
 def test_randomised_variants(B, seed):
     """Differential fuzz of the variants: every profile, plinth removal, width-relative cutting lengths, in random
     combinations on random small problems.  With plinth removal the error is bounded against the unsubtracted opacity
@@ -527,21 +530,27 @@ def test_randomised_variants(B, seed):
     what = f"variants {seed}: {profile} plinth={plinth} cut {mode} {cut:g} grid {grid} n {n} {cond}"
     assert op.stats()["n_evals"] == evals, what
     assert np.all(np.isfinite(k)), what
+    peak = 0.0
     if profile in ("doppler", "binned_gaussian"):
+        peak = float((lambda S, gL, aD, v: (S / (aD * np.sqrt(np.pi))).max())(*O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])))
         # a Gaussian is dropped below e^-40 of its peak (R22): if no grid point comes closer than that to
         # any line, the whole spectrum is "far tail" and there is nothing to compare
-        S, gL, aD, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
-        if k_ref.max() < 1e-15 * float((S / (aD * np.sqrt(np.pi))).max()):
-            assert float(np.abs(k).max()) <= 1e-15 * float((S / (aD * np.sqrt(np.pi))).max())
+        k_unsub = k_ref if not plinth else O.opacity_grid(lines, cond, grid, cut, profile=profile, cut_mode=mode)[0]
+        if k_unsub.max() < 1e-15 * peak:
+            assert float(np.abs(k).max()) <= 1e-15 * peak
             op.close()
             return
-    if plinth:
-        k_raw, _ = O.opacity_grid(lines, cond, grid, cut, profile=profile, cut_mode=mode)
+    # Gaussian profiles: terms below e^-40 of a line's own peak are dropped (R22), an absolute error of at most
+    # 4.3e-18 x peak per line; the binned Gaussian's edge bins of very narrow lines are good to ~2x 2^-25/a (R26)
+    gauss = profile in ("doppler", "binned_gaussian")
+    drop = 4.3e-18 * peak * n if gauss else 0.0
+    rel = 3e-4 if profile == "binned_gaussian" else 1e-4
+    k_raw = k_ref if not plinth else O.opacity_grid(lines, cond, grid, cut, profile=profile, cut_mode=mode)[0]
+    if k_raw.max() > 0:
         err = np.abs(k - k_ref)
-        bad = err > 1e-4 * k_raw + 1e-8 * max(k_raw.max(), 1e-300)
+        base = k_raw if plinth else np.where(k_ref >= 1e-8 * k_ref.max(), k_ref, 0.0)
+        bad = err > rel * base + 1e-8 * k_raw.max() + drop
         assert not bad.any(), (what, int(bad.sum()), float((err / np.maximum(k_raw, 1e-300))[bad].max()))
-    elif k_ref.max() > 0:
-        check_parity(k, k_ref, what=what)
     else:
         assert float(np.abs(k).max()) == 0.0
     op.close()
