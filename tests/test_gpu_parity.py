@@ -467,6 +467,12 @@ def test_randomised_small_cases(B, seed):
     span = nbins * dnu
     cut = float(rng.choice([0.0, 10 ** rng.uniform(np.log10(0.3 * dnu), np.log10(3.0 * span + 10 * dnu))]))
     n = int(rng.choice([1, 2, 30, 400, 3000]))
+    if seed % 4 == 3:                                  # dense: many lines per tile (the 8-warp centre kernel, long chunks)
+        n = 20_000
+        if nbins > 1500:
+            nbins = int(rng.integers(1, 1500))
+            grid = (numin, numin + nbins * dnu, dnu)
+            span = nbins * dnu
     pad = min(cut if cut > 0 else 5.0, 50.0)
     nu0 = np.abs(rng.uniform(numin - pad, numin + span + pad, n)) + 1e-3
     if rng.random() < 0.3:
