@@ -113,7 +113,7 @@ int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, do
 /* Line profile (section 2.1: Voigt, and "sometimes pure Doppler and Lorentzian profiles are also used"), unit area:
  *   HK_PROFILE_VOIGT   Re w(x + i y)/(alpha_D sqrt(pi))                      (default)
  *   HK_PROFILE_LORENTZ Gamma_L/(pi ((nu - nu0)^2 + Gamma_L^2))
- *   HK_PROFILE_DOPPLER exp(-((nu - nu0)/alpha_D)^2)/(alpha_D sqrt(pi)); values below e^-40 of the peak are dropped
+ *   HK_PROFILE_DOPPLER exp(-((nu - nu0)/alpha_D)^2)/(alpha_D sqrt(pi)); values below e^-88 of the peak are dropped
  *   HK_PROFILE_BINNED_GAUSSIAN  the "binned Gaussian integrated cross section" of ExoCross (L47): the Doppler profile
  *                      averaged over each bin, (1/(2 dnu)) [erf((nu_i + dnu/2 - nu0)/alpha_D) - erf((nu_i - dnu/2 - nu0)/alpha_D)]
  *                      (PAPER.md names it and prints no formula: DESIGN.md R26); conserves sum_i V_i dnu = 1 at any resolution

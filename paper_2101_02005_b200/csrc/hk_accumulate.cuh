@@ -548,7 +548,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                     const float qc = (HK_Z2 / 1.5f) * (1.5f * a2);            // as the row pass recomputes it
                     // Gauss-Hermite rows: the tile holds core bins and (D1 D2 ~ |z|^8) stays inside fp32
                     constexpr bool binned = kBinned;
-                    const float ql = binned ? binned_ql(a2) : (qmin < qc && qmax <= 1.0e9f * a2) ? HK_Z4 * a2 : qc;
+                    const float ql = binned ? binned_ql(a2) : (qmin < qc && qmax <= 1.0e9f * a2) ? (G2 == 0.f ? 88.0f : HK_Z4) * a2 : qc;   // (pure Gaussian: see z3_for)
                     // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y }: Gauss-Hermite rows (B.y < 0) carry P = cK y and
                     // Q = 1/a^2, two-term rows P = c (Lorentz amplitude) and Q = 1.5 a^2 -- what the row pass needs, ready
                     if (!binned && ql < qc) {

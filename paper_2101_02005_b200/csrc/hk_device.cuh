@@ -164,7 +164,9 @@ __device__ __forceinline__ float gh10_K(float x2, float s, float y)
 }
 
 // |z|^2 below which the trapezoid evaluator is used, as a function of y^2
-__device__ __forceinline__ float z3_for(float y2) { return y2 < 1e-6f ? 50.0f : HK_Z3; }
+// (y = 0 exactly, the pure Gaussian of the Doppler profile: exp(-x^2) is ALL there is, followed down to e^-88, the
+//  end of the fp32 range)
+__device__ __forceinline__ float z3_for(float y2) { return y2 == 0.f ? 88.0f : y2 < 1e-6f ? 50.0f : HK_Z3; }
 
 // Re w(x + i y) for |z|^2 < HK_Z2, x >= 0, y > 0: ring by |z|^2
 __device__ __forceinline__ float core_any_K(float x, float y, int* region);
@@ -210,8 +212,8 @@ __device__ __noinline__ float core_K(float x, float y)
     sum = fmaf(on ? wA[10] : wB[10], rcp_approx(q[10]), sum);
     float K = sum * (y * (h / 3.14159265358979f));
     const float re2 = fmaf(x, x, -y2);
-    if (y < 3.92699082f /* pi/h */ && re2 < 40.0f) {
-        // + Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) };  below exp(-40) the term is < 1e-10 of K
+    if (y < 3.92699082f /* pi/h */ && re2 < 88.0f) {
+        // + Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) }  (re2 >= 40 is reached by y = 0 only, see z3_for)
         const float amp = 2.0f * __expf(-re2);
         // exp(-z^2) = exp(-re2) (cos phi - i sin phi), phi = 2 x y reduced to [-pi, pi] first
         const float phi = 2.0f * x * y;
@@ -236,8 +238,9 @@ __device__ __noinline__ float core_K(float x, float y)
 __device__ __forceinline__ float core_any_K(float x, float y, int* region)
 {
     const float x2 = x * x, y2 = y * y, s = x2 + y2;
-    if (s >= HK_Z4) { if (region) *region = 2; return gh4_K(x2, s, y); }
-    if (s >= z3_for(y2)) { if (region) *region = 3; return gh6_K(x2, s, y); }
+    const float z3 = z3_for(y2);
+    if (s >= fmaxf(HK_Z4, z3)) { if (region) *region = 2; return gh4_K(x2, s, y); }
+    if (s >= z3) { if (region) *region = 3; return gh6_K(x2, s, y); }
     if (y >= HK_Y10) { if (region) *region = 5; return gh10_K(x2, s, y); }
     if (region) *region = 4;
     return core_K(x, y);

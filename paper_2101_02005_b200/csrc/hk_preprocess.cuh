@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             cmid += (unsigned long long)count_within(pos, t1 > 0 ? (double)sqrtf((float)t1) : 0.0, o.ilo, o.ihi);
             ccore += (unsigned long long)count_within(pos, t2 > 0 ? (double)sqrtf((float)t2) : 0.0, o.ilo, o.ihi);
             const double y2 = ab > 0.0 ? (Gb * Gb) / (ab * ab) : 1.0e300;
-            const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
+            const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 == 0.0 ? 88.0 : y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
             cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? (double)sqrtf((float)t4) : 0.0, o.ilo, o.ihi);
             const unsigned long long ntrap = (unsigned long long)count_within(pos, t3 > 0 ? (double)sqrtf((float)t3) : 0.0, o.ilo, o.ihi);
             ctrap += ntrap;
