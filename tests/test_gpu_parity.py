@@ -562,6 +562,43 @@ def test_randomised_variants(B, seed):
     op.close()
 
 
+@pytest.mark.parametrize("seed", range(N_FUZZ))
+def test_randomised_hitran(B, seed):
+    """Differential fuzz of the HITRAN-style entry point: random self / air pressures, shifts of many bins, 1-4
+    isotopologues, against the oracle (extent counts exact, north_star tolerance)."""
+    rng = np.random.default_rng(9000 + seed)
+    dnu = float(10 ** rng.uniform(-3, -0.5))
+    nbins = int(rng.integers(50, 30_000))
+    numin = float(rng.choice([0.0, rng.uniform(0.0, 2.0e4)]))
+    grid = (numin, numin + nbins * dnu, dnu)
+    span = nbins * dnu
+    n = int(rng.choice([5, 300, 3000]))
+    n_iso = int(rng.integers(1, 5))
+    isos = [(float(rng.uniform(2, 200)), float(10 ** rng.uniform(0, 4)), float(10 ** rng.uniform(-4, 0))) for _ in range(n_iso)]
+    P = float(10 ** rng.uniform(-3, 1.7))
+    cond = dict(T=float(rng.uniform(200, 3000)), P_atm=P, P_self_atm=float(rng.uniform(0, 1) * P), isos=isos)
+    lines = dict(nu0=np.abs(rng.uniform(numin - 3.0, numin + span + 3.0, n)) + 1e-3, A=10 ** rng.uniform(-6, 4, n),
+                 g_up=rng.integers(1, 30, n).astype(float), E_low=rng.uniform(0, 8000, n),
+                 gamma_air=10 ** rng.uniform(-2.5, -0.3, n), gamma_self=10 ** rng.uniform(-2.5, 0.0, n),
+                 n_exp=rng.uniform(0.3, 0.9, n), delta=rng.uniform(-0.05, 0.05, n),
+                 iso=rng.integers(0, n_iso + (1 if seed % 5 == 0 else 0), n).astype(np.int32))   # some outside the table
+    cut = float(rng.choice([0.0, 10 ** rng.uniform(np.log10(2 * dnu), np.log10(span + 1.0))]))
+    op = B.Opacity(*grid)
+    op.set_conditions_hitran(cond["T"], cond["P_atm"], cond["P_self_atm"], isos)
+    dl = {k2: torch.as_tensor(v2).cuda() for k2, v2 in lines.items()}
+    k = op.compute_hitran(dl, cut).cpu().numpy()
+    torch.cuda.synchronize()
+    k_ref, evals = O.opacity_grid_hitran(lines, cond, grid, cut)
+    what = f"hitran fuzz {seed}: grid {grid} cut {cut:g} n {n} {cond}"
+    st = op.stats()
+    assert st["n_evals"] == evals and st["n_skipped"] == int((lines["iso"] >= n_iso).sum()), what
+    if k_ref.max() > 0:
+        check_parity(k, k_ref, what=what)
+    else:
+        assert float(np.abs(k).max()) == 0.0
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
