@@ -777,9 +777,11 @@ def test_evaluator_accuracy_map(B):
 
 # ---- bench-size parity on sampled outputs ----------------------------------------------
 
-def _full_size_sampled(B, cfg, n_windows, width, n=None, plinth=False):
+def _full_size_sampled(B, cfg, n_windows, width, n=None, plinth=False, cut_override=None):
     c = W.CONFIGS[cfg]
     cond, grid, cut = W.conditions(cfg), c["grid"], c["cut"]
+    if cut_override is not None:
+        cut = cut_override
     dl = W.make_lines(cfg, n=n, seed=0, device="cuda")
     op = B.Opacity(*grid)
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
@@ -830,8 +832,8 @@ def test_config5_full_size_sampled(B):
     print(f"config 5 full: worst rel {worst:.2e}")
 
 
-@pytest.mark.parametrize("cfg,plinth", [(3, False), (4, False), (3, True)])
-def test_bt2_shaped_full_size_sampled(B, cfg, plinth):
+@pytest.mark.parametrize("cfg,plinth,cut", [(3, False, None), (4, False, None), (3, True, None), (3, False, 25.037), (4, False, 99.99631)])
+def test_bt2_shaped_full_size_sampled(B, cfg, plinth, cut):
     """The bench workload (config 4) and its coarse twin (config 3) at 5e8 lines, in the launch
     configuration bench.py times; the oracle sums every line within the cut on sampled bins."""
     import gc
@@ -840,5 +842,5 @@ def test_bt2_shaped_full_size_sampled(B, cfg, plinth):
     free, _ = torch.cuda.mem_get_info()
     if free < 120e9:
         pytest.skip("needs ~110 GB of device memory")
-    worst, st = _full_size_sampled(B, cfg, 6 if cfg == 4 else 10, 8 if cfg == 4 else 32, plinth=plinth)
+    worst, st = _full_size_sampled(B, cfg, 6 if cfg == 4 else 10, 8 if cfg == 4 else 32, plinth=plinth, cut_override=cut)
     print(f"config {cfg} full (plinth {plinth}): worst rel {worst:.2e}, evals {st['n_evals']:.3e}")
