@@ -599,6 +599,62 @@ def test_randomised_hitran(B, seed):
     op.close()
 
 
+@pytest.mark.parametrize("seed", range(max(4, N_FUZZ // 4)))
+def test_randomised_entry_points(B, seed):
+    """The other entry points on random small problems: block-wise hk_accumulate, hk_compute_host with a random block
+    size, hk_compute_batch with three conditions, hk_compute_bands -- each against the oracle."""
+    rng = np.random.default_rng(13000 + seed)
+    dnu = float(10 ** rng.uniform(-2.5, -0.5))
+    nbins = int(rng.integers(100, 20_000))
+    numin = float(rng.choice([0.0, rng.uniform(0.0, 1.0e4)]))
+    grid = (numin, numin + nbins * dnu, dnu)
+    span = nbins * dnu
+    n = int(rng.choice([7, 500, 4000]))
+    lines = _simple_lines(np.abs(rng.uniform(numin - 2.0, numin + span + 2.0, n)) + 1e-3, A=10 ** rng.uniform(-6, 4, n),
+                          g_up=rng.integers(1, 30, n).astype(float), E_low=rng.uniform(0, 8000, n),
+                          gamma_ref=10 ** rng.uniform(-2.5, -0.3, n), n_exp=rng.uniform(0.4, 0.8, n))
+    cond = dict(T=float(rng.uniform(200, 3000)), P_atm=float(10 ** rng.uniform(-2, 1.7)),
+                mass_amu=float(rng.uniform(2, 200)), Q=float(10 ** rng.uniform(0, 4)))
+    cut = float(rng.choice([0.0, 10 ** rng.uniform(np.log10(2 * dnu), np.log10(span))]))
+    plinth = bool(rng.integers(0, 2))
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut, plinth=plinth)
+    k_raw = k_ref if not plinth else O.opacity_grid(lines, cond, grid, cut)[0]
+
+    def ok(k, ref=k_ref, raw=k_raw, what=""):
+        err = np.abs(np.asarray(k) - ref)
+        base = raw if plinth else np.where(ref >= 1e-8 * ref.max(), ref, 0.0)
+        bad = err > 1e-4 * base + 1e-8 * max(raw.max(), 1e-300)
+        assert not bad.any(), (f"entry points {seed} {what}: cut {cut:g} plinth {plinth} grid {grid} n {n}", int(bad.sum()))
+
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    op.set_plinth(plinth)
+    dl = _to_cuda(lines)
+    # blocks through hk_accumulate
+    k = torch.zeros(op.N, dtype=torch.float64, device="cuda")
+    cuts = sorted(set([0, n] + [int(x) for x in rng.integers(0, n + 1, 3)]))
+    for a0, a1 in zip(cuts[:-1], cuts[1:]):
+        op.compute({f: v[a0:a1].contiguous() for f, v in dl.items()}, cut, out=k, accumulate=True)
+    torch.cuda.synchronize()
+    ok(k.cpu().numpy(), what="accumulate")
+    # host pipeline
+    hl = {f: torch.as_tensor(v).pin_memory() for f, v in lines.items()}
+    kh = op.compute_host(hl, cut, block_lines=int(rng.integers(1, n + 5)))
+    assert op.stats()["n_evals"] == evals
+    ok(kh.numpy(), what="host")
+    # batch: the handle's own condition in the middle
+    Ts, Ps, Qs = [cond["T"] * 0.5, cond["T"], cond["T"] * 1.3], [cond["P_atm"] * 2, cond["P_atm"], 0.0], [cond["Q"], cond["Q"], 7.0]
+    kb = op.compute_batch(dl, cut, Ts, Ps, Qs).cpu().numpy()
+    ok(kb[1], what="batch[1]")
+    for c in (0, 2):
+        cc = dict(T=Ts[c], P_atm=Ps[c], mass_amu=cond["mass_amu"], Q=Qs[c])
+        r = O.opacity_grid(lines, cc, grid, cut, plinth=plinth)[0]
+        rr = r if not plinth else O.opacity_grid(lines, cc, grid, cut)[0]
+        if rr.max() > 0:
+            ok(kb[c], ref=r, raw=rr, what=f"batch[{c}]")
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
