@@ -149,12 +149,13 @@ size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines);
 int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
 
 /* Enqueue the whole hot path on `stream` (a cudaStream_t passed as void*; NULL is
- * the legacy default stream): preprocess -> bucket/sort -> tile ranges -> node, far, mid and
- * near accumulation kernels -> interpolation of the node sums -> k in out_k_dev.  out_k_dev (N doubles) is
- * OVERWRITTEN.  cut_cm > 0 and finite: fixed cutting length from the centre,
- * inclusive integer extent (R7); cut_cm <= 0 or +inf: uncut.  Lines need not be
- * sorted.  n_lines == 0 is valid (k = 0).  Returns after enqueueing, without
- * synchronising; every buffer must stay alive until the stream drains. */
+ * the legacy default stream): preprocess -> sort by centre bin -> tile ranges -> node, far, mid, extent-end,
+ * centre and near accumulation kernels -> interpolation of the node sums (-> plinth removal) -> k in out_k_dev.
+ * out_k_dev (N doubles) is OVERWRITTEN.  cut_cm > 0 and finite: cutting length from the centre (cm^-1, or a
+ * multiple of the line's half-width: hk_set_cut_mode), inclusive integer extent (R7); cut_cm <= 0 or +inf: uncut.
+ * Lines need not be sorted.  n_lines == 0 is valid (k = 0).  Returns after enqueueing, without synchronising
+ * (except in the width-relative cut modes, see hk_set_cut_mode); every buffer must stay alive until the stream
+ * drains.  The profile, plinth and cut-mode settings of the context apply. */
 int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
                double* out_k_dev, void* stream);
 
