@@ -655,6 +655,38 @@ def test_randomised_entry_points(B, seed):
     op.close()
 
 
+@pytest.mark.parametrize("cut", [25.0, 0.0])
+def test_large_grid_few_lines(B, cut):
+    """2e7 bins (beyond the 1 GiB budget of the per-bin extent-end accumulators: the direct edge kernel takes over, and
+    the node hierarchy grows to its deepest), a few thousand lines; sampled bins against the oracle."""
+    grid = (0.0, 20000.0, 0.001)
+    n = 3000 if cut > 0 else 300
+    lines = W.to_numpy(W.make_lines(2, n=n, seed=3))
+    lines["nu0"] = lines["nu0"] * 2.0                      # spread over the whole grid
+    cond = W.conditions(2)
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    k = op.compute(_to_cuda(lines), cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    N = op.N
+    assert N == 20_000_000 and st["n_pairs_edge_node"] == 0 and st["n_levels"] >= 5
+    rng = np.random.default_rng(8)
+    bins = set(rng.integers(0, N, 4000).tolist()) | {0, 1, N - 2, N - 1}
+    S, _, _, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    for l in np.argsort(S)[-6:]:
+        jc = int(lines["nu0"][l] / grid[2])
+        for off in (0, int(cut / grid[2]) if cut > 0 else 5000):
+            bins |= set(range(max(0, jc + off - 40), min(N, jc + off + 40))) | set(range(max(0, jc - off - 40), min(N, jc - off + 40)))
+    bins = np.array(sorted(bins), dtype=np.int64)
+    k_ref, _ = O.opacity_bins(lines, cond, grid, cut, bins)
+    kmax = float(k.max())
+    check_parity(k[torch.as_tensor(bins, device="cuda")].cpu().numpy(), k_ref, kmax=kmax, what=f"large grid cut {cut}")
+    ilo, ihi, _ = op.extents(_to_cuda(lines))
+    assert int((ihi.long() - ilo.long() + 1).sum()) == st["n_evals"]
+    op.close()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
