@@ -687,6 +687,32 @@ def test_large_grid_few_lines(B, cut):
     op.close()
 
 
+@pytest.mark.parametrize("cut", [25.0, 0.0])
+def test_billion_bin_grid(B, cut):
+    """Towards the maximum grid size (N < 2^31): 1.2e9 bins at 1e-5 cm^-1, 500 lines; uncut that is 6e11 (line, bin)
+    terms through 22 levels of the node hierarchy.  Sampled bins against the oracle."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 30e9:
+        pytest.skip("needs ~16 GB of device memory")
+    grid = (0.0, 12000.0, 1e-5)
+    lines = W.to_numpy(W.make_lines(2, n=500, seed=4))
+    cond = W.conditions(2)
+    op = B.Opacity(*grid)
+    assert op.N == 1_200_000_000
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    k = op.compute(_to_cuda(lines), cut)
+    torch.cuda.synchronize()
+    st = op.stats()
+    assert st["n_evals"] == (500 * op.N if cut == 0.0 else st["n_evals"]) and st["n_levels"] >= 14
+    rng = np.random.default_rng(1)
+    bins = np.unique(np.concatenate([rng.integers(0, op.N, 3000), [0, op.N - 1], (lines["nu0"][:20] / grid[2]).astype(np.int64)]))
+    k_ref, _ = O.opacity_bins(lines, cond, grid, cut, bins)
+    check_parity(k[torch.as_tensor(bins, device="cuda")].cpu().numpy(), k_ref, kmax=float(k.max()), what=f"1.2e9 bins cut {cut}")
+    op.close()
+    del k
+    torch.cuda.empty_cache()
+
+
 # ---- per-line parameters (step a1) ----------------------------------------------------
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 5])
