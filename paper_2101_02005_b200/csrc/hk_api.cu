@@ -44,6 +44,9 @@ struct hk_ctx {
     int32_t last_sort_bits, last_kb, last_levels;
     int64_t last_launches;
     DevStats* d_stats;
+    const RecU* last_recU;       // unsorted records of the last pass (for the on-demand region counts)
+    int last_profile;
+    bool regions_done;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
     bool host_totals;
     int64_t tot_lines, tot_skipped, tot_off_grid, tot_evals;
@@ -442,6 +445,8 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     ctx->last_cut = cut_cm;
     ctx->last_stream = stream;
     ctx->d_stats = st;
+    ctx->last_recU = nullptr;
+    ctx->regions_done = false;
     ctx->last_sort_bits = 0;
     ctx->last_launches = 0;
     ctx->last_kb = p.kb;
@@ -465,6 +470,8 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     int32_t* counts = (int32_t*)(ws + L.counts);
     int32_t* prefix = (int32_t*)(ws + L.prefix);
     const Levels lv = make_levels(ctx, p);
+    ctx->last_recU = recU;
+    ctx->last_profile = p.profile;
     ctx->last_levels = lv.n_levels;
 
     // a1: per-line parameters, keys
@@ -923,6 +930,15 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     DevStats d;
     std::memset(&d, 0, sizeof(d));
     HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
+    if (ctx->d_stats && ctx->last_recU && !ctx->regions_done && ctx->last_n > 0) {
+        // per-region evaluation counts, derived from the records on demand (kept out of the hot path)
+        const int64_t nl = ctx->last_n;                 // (block pipelines and class passes: the last block / pass)
+        if (nl > 0) {
+            region_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_recU, nl, ctx->last_profile, ctx->d_stats);
+            HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
+        }
+        ctx->regions_done = true;
+    }
     if (ctx->d_stats) HK_CUDA(cudaMemcpy(&d, ctx->d_stats, sizeof(d), cudaMemcpyDeviceToHost));
     std::memset(host_out, 0, sizeof(*host_out));
     host_out->n_lines = ctx->last_n;

@@ -201,17 +201,8 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             cmaxb = max(cmaxb, (unsigned long long)__double_as_longlong(cl));
             cKmaxb = max(cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
             evals += (unsigned long long)(o.ihi - o.ilo + 1);
-            double pos = (double)o.jc + o.pos_f;
-            if (p.profile == HK_PROFILE_LORENTZ) ab = 0.0;                // region counters: a Lorentzian has no core
-            double t1 = (double)HK_Z1 * ab * ab - Gb * Gb, t2 = (double)HK_Z2 * ab * ab - Gb * Gb;
-            cmid += (unsigned long long)count_within(pos, t1 > 0 ? (double)sqrtf((float)t1) : 0.0, o.ilo, o.ihi);
-            ccore += (unsigned long long)count_within(pos, t2 > 0 ? (double)sqrtf((float)t2) : 0.0, o.ilo, o.ihi);
-            const double y2 = ab > 0.0 ? (Gb * Gb) / (ab * ab) : 1.0e300;
-            const double t4 = (double)HK_Z4 * ab * ab - Gb * Gb, t3 = (y2 == 0.0 ? 88.0 : y2 < 1e-6 ? 50.0 : (double)HK_Z3) * ab * ab - Gb * Gb;
-            cgh6 += (unsigned long long)count_within(pos, t4 > 0 ? (double)sqrtf((float)t4) : 0.0, o.ilo, o.ihi);
-            const unsigned long long ntrap = (unsigned long long)count_within(pos, t3 > 0 ? (double)sqrtf((float)t3) : 0.0, o.ilo, o.ihi);
-            ctrap += ntrap;
-            if (y2 >= (double)(HK_Y10 * HK_Y10)) cgh10 += ntrap;
+            // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
+            //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
         }
         rec[i] = r;
         key[i] = k;
@@ -239,6 +230,39 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
                                 : q == 6 ? &st->n_cnt_trap : q == 7 ? &st->n_cnt_gh10 : q == 8 ? &st->cmax_bits : &st->cKmax_bits;
         if (q < 8) { if (x) atomicAdd(dst, x); }
         else atomicMax(dst, x);
+    }
+}
+
+// Per-region evaluation counts (hk_stats.n_evals_far / mid / core / gh6 / trap / gh10) from the unsorted records of the
+// last compute: for each line the number of bins of its extent with |z|^2 below each threshold.  Run on demand.
+__global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restrict__ rec, int64_t n, int profile,
+                                                           DevStats* __restrict__ st)
+{
+    unsigned long long c[5] = {0, 0, 0, 0, 0};           // below Z1, Z2, Z4, Z3 (trapezoid region), of that with y >= 2
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const RecU r = rec[i];
+        if (r.ihi < r.ilo) continue;
+        const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
+        const double G2 = gauss ? 0.0 : (double)r.G2, a2 = profile == HK_PROFILE_LORENTZ ? 0.0 : (double)r.a2;
+        const double pos = (double)r.jc + (signbit(r.f) ? 1.0 + (double)r.f : (double)r.f);
+        const double y2 = a2 > 0.0 ? G2 / a2 : 1.0e300;
+        const double z3 = y2 == 0.0 ? 88.0 : y2 < 1e-6 ? 50.0 : (double)HK_Z3;
+        const double t[4] = {(double)HK_Z1 * a2 - G2, (double)HK_Z2 * a2 - G2, (double)HK_Z4 * a2 - G2, z3 * a2 - G2};
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            c[q] += (unsigned long long)count_within(pos, t[q] > 0 ? (double)sqrtf((float)t[q]) : 0.0, r.ilo, r.ihi);
+        if (y2 >= (double)(HK_Y10 * HK_Y10))
+            c[4] += (unsigned long long)count_within(pos, t[3] > 0 ? (double)sqrtf((float)t[3]) : 0.0, r.ilo, r.ihi);
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+        unsigned long long x = c[q];
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        if ((threadIdx.x & 31) == 0 && x) {
+            unsigned long long* dst = q == 0 ? &st->n_cnt_mid : q == 1 ? &st->n_cnt_core : q == 2 ? &st->n_cnt_gh6
+                                    : q == 3 ? &st->n_cnt_trap : &st->n_cnt_gh10;
+            atomicAdd(dst, x);
+        }
     }
 }
 
