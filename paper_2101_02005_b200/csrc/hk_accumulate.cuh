@@ -7,21 +7,28 @@
 // Lines arrive sorted by centre bin, so the lines that can reach a tile are one contiguous index
 // range, split by range_kernel into
 //   [A0,FL0) left-edge | [FL0,NL) node-handled | [NL,FL1) far | [FL1,ML1) mid | [ML1,MR0) centre |
-//   [MR0,FR0) mid | [FR0,NR) far | [NR,FR1) node-handled | [FR1,A1) right-edge
+//   [MR0,FR0) mid | [FR0,NR) far | [NR,FR1) node-handled | [FR1,A1) right-edge     (TileRange, hk_device.cuh)
 // Node-handled pairs (tile separated from the line) are evaluated at Chebyshev nodes
 // by node_kernel on a binary hierarchy of tiles and interpolated onto the bins at the end.
 // A work unit is (tile, chunk of a kernel's own classes); units are handed out by an atomic counter to a
 // persistent grid (a multiple of the SM count).  fp32 partial sums are flushed into fp64 registers
 // every kFlush lines.
 //
+//   node_kernel               (a5)        : separated (line, tile) pairs at the tile's 8 Chebyshev nodes, every level of
+//        the hierarchy; node_down_kernel / node_bins_kernel bring the node sums down to the bins.
 //   interior_kernel<KB,false> (a5, "far") : pairs whose whole tile is inside the extent and has
 //        |z|^2 >= Z1: branch-free Lorentzian, two lines share one reciprocal, packed fp32 (FFMA2).
 //   interior_kernel<KB,true>  (a5, "mid") : same shape, |z|^2 >= Z2: two-term asymptotic, mask-free.
-//   near_kernel<KB>           (a4)        : extent edges and line centres.  Row pass: exact integer
-//        extent mask + two-term asymptotic where |z|^2 >= Z2, and the trapezoid evaluator in place
-//        for lines whose core (|z|^2 < Z2) spans >= 16 bins.  Lane pass, for narrower cores: lanes
+//   edge_node_kernel          (a4)        : extent ends in separated tiles, at the tile's nodes into per-bin accumulators
+//        (edge_scan_kernel, edge_bins_kernel finish); edge_kernel<KB>: the masked direct form for the other ends.
+//   centre_kernel<KB,W,binned> (a4)       : tiles inside the extent that hold a line's core.  Row pass (Gauss-Hermite 4
+//        or two-term rows) + lane pass for |z| < 8 on batches counting-sorted by y.  The dominant kernel.
+//   near_kernel<KB>           (a4)        : the generic remainder (tiles partly outside the extent that hold core
+//        bins).  Row pass: exact integer extent mask + two-term asymptotic where |z|^2 >= Z2, and the core
+//        evaluator in place for lines whose core spans >= 16 bins.  Lane pass, for narrower cores: lanes
 //        walk lines, each lane evaluates its own line's core bins; equal bins are combined in the
 //        warp and added to a bin tile staged in shared memory.
+//   plinth_kernel             (optional)  : the per-line plinths as a difference array, summed over the bins by CUB.
 //
 // The paper's kernel (L243-330) walks lines in threads and nu-points serially with a
 // shared-memory K_s and four launches per block (AL/AR/B/C, L354); what is kept is the idea
