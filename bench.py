@@ -161,24 +161,28 @@ class OracleSample:
         return width
 
 
-def _evals_per_line(dl, cfg):
-    """Exact mean extent (bins per line) of the workload, from the integer extent formula (fp64, torch)."""
+def _evals_per_line(dl, cfg, O):
+    """Exact mean extent (bins per line) of the workload: the oracle's integer extents (oracle.hk_oracle.extents -- this
+    is the baseline leg, which the oracle may serve), block by block over the list."""
     c = W.CONFIGS[cfg]
     numin, numax, dnu = c["grid"]
-    N = int(np.floor((numax - numin) / dnu + 0.5))
+    N = O.grid_size(numin, numax, dnu)
     if not c["cut"] > 0:
         return float(N)
     nu0 = dl["nu0"]
-    lo = torch.ceil((nu0 - c["cut"] - numin) / dnu).clamp_(min=0)
-    hi = torch.floor((nu0 + c["cut"] - numin) / dnu).clamp_(max=N - 1)
-    return float((hi - lo + 1).clamp_(min=0).sum() / nu0.numel())
+    total, block = 0, 1 << 24
+    for i in range(0, nu0.numel(), block):
+        h = nu0[i:i + block].cpu().numpy()
+        ilo, ihi, _ = O.extents(h, None, numin, dnu, N, c["cut"])
+        total += int(np.maximum(ihi - ilo + 1, 0).sum())
+    return total / float(nu0.numel())
 
 
 def cpu_baseline(dl, cfg, n_lines, seconds=15.0):
     samp = OracleSample(dl, cfg)
     width = samp.size_for(seconds)
     t, ev = samp.run()
-    epl = _evals_per_line(dl, cfg)
+    epl = _evals_per_line(dl, cfg, samp.O)
     rate = ev / t
     return {"value": rate / epl, "unit": UNIT, "cores": samp.O.num_threads(), "kind": "oracle",
             "evals_per_s": rate, "seconds": t,
@@ -196,7 +200,7 @@ def run_reference(args):
     dl = W.make_lines(cfg, n=n, seed=0, device=dev)            # input generation only; the oracle runs on the host
     samp = OracleSample(dl, cfg)
     width = samp.size_for(8.0)
-    epl = _evals_per_line(dl, cfg)
+    epl = _evals_per_line(dl, cfg, samp.O)
     for _ in range(args.warmup):
         samp.run()
     tt, ee = 0.0, 0

@@ -113,10 +113,14 @@ int hk_set_conditions(hk_ctx* ctx, double T_K, double P_atm, double mass_amu, do
 /* Line profile (section 2.1: Voigt, and "sometimes pure Doppler and Lorentzian profiles are also used"), unit area:
  *   HK_PROFILE_VOIGT   Re w(x + i y)/(alpha_D sqrt(pi))                      (default)
  *   HK_PROFILE_LORENTZ Gamma_L/(pi ((nu - nu0)^2 + Gamma_L^2))
- *   HK_PROFILE_DOPPLER exp(-((nu - nu0)/alpha_D)^2)/(alpha_D sqrt(pi)); values below e^-88 of the peak are dropped
+ *   HK_PROFILE_DOPPLER exp(-((nu - nu0)/alpha_D)^2)/(alpha_D sqrt(pi))
  *   HK_PROFILE_BINNED_GAUSSIAN  the "binned Gaussian integrated cross section" of ExoCross (L47): the Doppler profile
  *                      averaged over each bin, (1/(2 dnu)) [erf((nu_i + dnu/2 - nu0)/alpha_D) - erf((nu_i - dnu/2 - nu0)/alpha_D)]
  *                      (PAPER.md names it and prints no formula: DESIGN.md R26); conserves sum_i V_i dnu = 1 at any resolution
+ * Dynamic range of one launch (every profile): the fp32 evaluation carries ONE power-of-two scale per launch, set from
+ * the largest line amplitude of the list; a term more than ~166 binades (1e-50; Gaussian profiles: 226 binades, 1e-68)
+ * below the largest amplitude is flushed to zero.  Such terms are below every tolerance unless the WHOLE spectrum
+ * is -- a pure Gaussian is followed down to exp(-157) of its peak, where that range ends.
  * HK_EINVAL for any other value. */
 #define HK_PROFILE_VOIGT 0
 #define HK_PROFILE_LORENTZ 1
@@ -271,7 +275,8 @@ int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* 
  * mode 1: every pair through the near/edge kernel; mode 2: far pairs through the mid (two-term) kernel
  * (modes 1-3 do not use the node hierarchy).
  * hk_set_node_separation: a (line, tile) pair is evaluated at nodes when the line centre is at least
- * `sep` tile half-widths from the tile centre (default 4; < 1.5 disables the hierarchy).
+ * `sep` tile half-widths from the tile centre (default 4; 0 disables the hierarchy; HK_EINVAL for 0 < sep < 3, where the
+ * degree-7 interpolant leaves the error budget of DESIGN.md section 5, and for sep > 64).
  * hk_set_tile_bins: bins per lane 2, 4 or 8 (a warp owns 32x, a CTA 256x); 0 = chosen from
  * the cut (include/hk.h hk_stats.bins_per_lane reports the choice). */
 int hk_set_debug_mode(hk_ctx* ctx, int mode);

@@ -522,7 +522,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
             for (int k = 0; k < kLPTC; ++k) {
                 const int i = threadIdx.x + k * kThreads;
                 if (v0 + i < nt) {
-                    yv[k] = sqrtf(preA[k].z) * rsqrtf(preB[k].x);
+                    yv[k] = kBinned ? 0.f : sqrtf(preA[k].z) * rsqrtf(preB[k].x);      // (binned: A.z carries flo, not G2)
                     cls[k] = y_class(yv[k]);
                     rk[k] = atomicAdd(&hist[cls[k]], 1);
                 }
@@ -546,7 +546,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                     const float4 ra = preA[k], rb = preB[k];
                     const int dst = hist[cls[k]] + rk[k];
                     const float fdj = (float)((int64_t)__float_as_int(ra.x) - ct0);
-                    const float G2 = ra.z, a2 = rb.x;
+                    const float G2 = kBinned ? 0.f : ra.z, a2 = rb.x;
                     // smallest and largest q = t^2 + G2 over the tile's bins (from below / from above)
                     const float pos = fdj + ra.y;
                     const float dmin = fmaxf(fmaxf(-pos, pos - whi), 0.f) * 0.999f;
@@ -555,7 +555,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                     const float qc = (HK_Z2 / 1.5f) * (1.5f * a2);            // as the row pass recomputes it
                     // Gauss-Hermite rows: the tile holds core bins and (D1 D2 ~ |z|^8) stays inside fp32
                     constexpr bool binned = kBinned;
-                    const float ql = binned ? binned_ql(a2) : (qmin < qc && qmax <= 1.0e9f * a2) ? (G2 == 0.f ? 88.0f : HK_Z4) * a2 : qc;   // (pure Gaussian: see z3_for)
+                    const float ql = binned ? binned_ql(a2) : (qmin < qc && qmax <= 1.0e9f * a2) ? (G2 == 0.f ? HK_ZG : HK_Z4) * a2 : qc;   // (pure Gaussian: see z3_for)
                     // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y }: Gauss-Hermite rows (B.y < 0) carry P = cK y and
                     // Q = 1/a^2, two-term rows P = c (Lorentz amplitude) and Q = 1.5 a^2 -- what the row pass needs, ready
                     if (!binned && ql < qc) {
@@ -563,7 +563,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                         smB[dst] = make_float4(-ra.y, -ql, rb.w, yv[k]);
                     } else {
                         smA[dst] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
-                        smB[dst] = make_float4(-ra.y, ql, rb.w, yv[k]);
+                        smB[dst] = make_float4(-ra.y, ql, rb.w, kBinned ? ra.z : yv[k]);     // binned: the low part of f
                     }
                 }
             }
@@ -652,7 +652,7 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                         const float lo = fmaxf(ceilf(pos - hw), 0.f), hi = fminf(floorf(pos + hw), whi);
                         if (hi >= lo) { clo = lo; chi = hi; }
                     }
-                    inv_a = B.y < 0.f ? sqrtf(A.w) : rsqrtf(A.w * (1.0f / 1.5f));
+                    inv_a = B.y < 0.f ? sqrtf(A.w) : sqrtf(1.5f / A.w);          // IEEE sqrt and division: a Gaussian tail amplifies an error of x by 2 x^2
                 }
                 float bmin = clo, bmax = chi;
 #pragma unroll
@@ -673,7 +673,9 @@ __global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_ker
                                 const float t = (e0 + (float)s) - f;             // the row pass's t, bit for bit
                                 const float q = fmaf(t, t, G2);
                                 float val = 0.f;
-                                if (q < ql) val = cK * (kBinned ? binned_K(fabsf(t), inv_a) : core_any_K(fabsf(t) * inv_a, y, nullptr));
+                                if (q < ql) val = kBinned ? cK * binned_K(e0 + (float)s, f, y, inv_a)          // y: flo here
+                                                  : y == 0.f ? gauss_term(cK, fabsf(t) * inv_a)
+                                                             : cK * core_any_K(fabsf(t) * inv_a, y, nullptr);
                                 stage[warp][s][lane] = val;
                             }
                         }
@@ -711,17 +713,19 @@ constexpr int kFlagNoCore = 2;         // |z|^2 >= Z2 on every bin of the tile
 constexpr int kFlagFar = 4;            // |z|^2 >= Z1 on every bin of the tile: one term is enough
 constexpr int kFlagWide = 8;           // core spans >= 16 bins: evaluated in the row pass
 
-// One line against the warp's KB rows of 32 bins.  A = { jc - ct0, f, G2, c }, B = { A1, -A2, qc, cK },
-// C = { ilo - ct0, ihi - ct0, y, flags }.
+// One line against the warp's KB rows of 32 bins.  A = { jc - ct0, f, G2, c }, B = { A1, -A2 (binned Gaussian: the low
+// part of f), qc, cK }, C = { ilo - ct0, ihi - ct0, y (binned Gaussian: dnu/alpha_D), flags }.
 template <int KB, bool kTwoTerm, bool kMask, bool kCore>
 __device__ __forceinline__ void near_rows(float2 (&acc)[KB / 2], const float2 (&tb)[KB / 2], const float4 A,
                                           const float4 B, const float4 C, const bool wide, const int profile = 0)
 {
     const float2 ndl = bcast2(-A.x), nf = bcast2(-A.y), g = bcast2(A.z);
     const float2 A1 = bcast2(B.x), nA2 = bcast2(B.y), one = bcast2(1.0f);
-    const float c = A.w, qc = B.z, lo = C.x, hi = C.y;
+    const float2 c = bcast2(A.w);
+    const float qc = B.z, lo = C.x, hi = C.y;
+    const bool binned = profile == HK_PROFILE_BINNED_GAUSSIAN;
     float inv_a = 0.f;
-    if (kCore && wide) inv_a = profile == HK_PROFILE_BINNED_GAUSSIAN ? C.z : rsqrtf(qc * (1.0f / HK_Z2));
+    if (kCore && wide) inv_a = binned ? C.z : sqrtf(HK_Z2 / qc);
 #pragma unroll
     for (int m = 0; m < KB / 2; ++m) {
         const float2 d = __fadd2_rn(tb[m], ndl);            // exact: both are small integers
@@ -740,14 +744,19 @@ __device__ __forceinline__ void near_rows(float2 (&acc)[KB / 2], const float2 (&
             in1 = (tb[m].y >= lo) && (tb[m].y <= hi);
         }
         if (kCore) { co0 = q.x < qc; co1 = q.y < qc; }
-        const float2 cm = make_float2((in0 && !co0) ? c : 0.f, (in1 && !co1) ? c : 0.f);
-        acc[m] = __ffma2_rn(cm, ww, acc[m]);
+        // selected, not multiplied by a zero amplitude: 1/q at q = 0 (a zero-width line on a grid point) is not finite
+        if (kMask || kCore) {
+            ww.x = (in0 && !co0) ? ww.x : 0.f;
+            ww.y = (in1 && !co1) ? ww.y : 0.f;
+        }
+        acc[m] = __ffma2_rn(c, ww, acc[m]);
         if (kCore && wide) {
+            const float flo = binned ? B.y : 0.f;
             if (__any_sync(0xffffffffu, in0 && co0)) {
-                if (in0 && co0) acc[m].x = fmaf(B.w, core_eval(profile, fabsf(t.x), inv_a, C.z), acc[m].x);
+                if (in0 && co0) acc[m].x += core_term(profile, B.w, d.x, A.y, flo, inv_a, C.z);
             }
             if (__any_sync(0xffffffffu, in1 && co1)) {
-                if (in1 && co1) acc[m].y = fmaf(B.w, core_eval(profile, fabsf(t.y), inv_a, C.z), acc[m].y);
+                if (in1 && co1) acc[m].y += core_term(profile, B.w, d.y, A.y, flo, inv_a, C.z);
             }
         }
     }
@@ -846,8 +855,8 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                     dlo = max(-lim, min(lim, dlo));
                     dhi = max(-lim, min(lim, dhi));
                     const float fdj = (float)dj, flo = (float)dlo, fhi = (float)dhi;
-                    const float G2 = ra.z, a2 = rb.x;
                     const bool binned = a.profile == HK_PROFILE_BINNED_GAUSSIAN;
+                    const float G2 = binned ? 0.f : ra.z, a2 = rb.x;          // (binned: A.z carries the low part of f)
                     const float qc = binned ? binned_ql(a2) : HK_Z2 * a2;
                     // smallest q = t^2 + G2 over the tile's bins, from below
                     const float pos = fdj + ra.y;
@@ -859,9 +868,9 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                     if (qmin >= fmaxf(HK_Z1 * a2, qc)) flags |= kFlagFar;
                     if ((qc - G2) >= kWideCore) flags |= kFlagWide;
                     smA[i] = make_float4(fdj, ra.y, G2, ra.w);
-                    smB[i] = make_float4(1.5f * a2, -2.0f * a2 * G2, qc, rb.w);
+                    smB[i] = make_float4(1.5f * a2, binned ? ra.z : -2.0f * a2 * G2, qc, rb.w);
                     // C.z: y for the Voigt evaluators; the binned Gaussian needs 1/a instead (its y is 0)
-                    smC[i] = make_float4(flo, fhi, binned ? rsqrtf(a2) : sqrtf(G2) * rsqrtf(a2), __int_as_float(flags));
+                    smC[i] = make_float4(flo, fhi, binned ? sqrtf(1.0f / a2) : sqrtf(G2 / a2), __int_as_float(flags));
                 }
             }
         };
@@ -893,7 +902,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
 #pragma unroll 1
             for (int lb = wl0; lb < wl1; lb += 32) {
                 const int l = lb + lane;
-                float dlt = 0.f, f = 0.f, G2 = 0.f, cK = 0.f, qc = 0.f, y = 0.f;
+                float dlt = 0.f, f = 0.f, flo = 0.f, G2 = 0.f, cK = 0.f, qc = 0.f, y = 0.f;
                 int cnt = 0;
                 float clo = 0.f;
                 if (l < wl1) {
@@ -901,6 +910,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                     const int flags = __float_as_int(C.w);
                     if (!(flags & (kFlagNoCore | kFlagWide))) {
                         dlt = A.x; f = A.y; G2 = A.z; cK = B.w; qc = B.z; y = C.z;
+                        if (a.profile == HK_PROFILE_BINNED_GAUSSIAN) flo = B.y;
                         const float h2 = qc - G2;
                         const float hw = sqrtf(fmaxf(h2, 0.f)) + 1.0f;           // |t| < hw covers every q < qc
                         const float pos = dlt + f;
@@ -913,7 +923,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) maxcnt = max(maxcnt, __shfl_xor_sync(0xffffffffu, maxcnt, o));
                 if (maxcnt == 0) continue;
-                const float inv_a = a.profile == HK_PROFILE_BINNED_GAUSSIAN ? y : rsqrtf(fmaxf(qc, 1e-30f) * (1.0f / HK_Z2));
+                const float inv_a = a.profile == HK_PROFILE_BINNED_GAUSSIAN ? y : sqrtf(HK_Z2 / fmaxf(qc, 1e-30f));
                 for (int o = 0; o < maxcnt; ++o) {
                     float val = 0.f;
                     int bin = -1;
@@ -922,7 +932,7 @@ __global__ void __launch_bounds__(kThreads, 2) near_kernel(AccArgs a)
                         const float d = fb - dlt;
                         const float t = d - f;
                         const float q = fmaf(t, t, G2);
-                        if (q < qc) { val = cK * core_eval(a.profile, fabsf(t), inv_a, y); bin = (int)fb; }
+                        if (q < qc) { val = core_term(a.profile, cK, d, f, flo, inv_a, y); bin = (int)fb; }
                     }
                     // combine equal bins in the warp (sorted lines: neighbours share bins), one add per distinct bin
                     unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
@@ -1262,7 +1272,7 @@ __global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const 
                 const double q = cb * cb + G2;
                 const double c = r.cK * sqrt(G2 * a2) * 0.56418958354775628695;        // Lorentz amplitude, as gather_kernel
                 if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) {
-                    if (q < (double)binned_ql(r.a2)) pl = r.cK * (double)binned_K((float)cb, rsqrtf(r.a2));
+                    if (q < (double)binned_ql(r.a2)) pl = r.cK * (double)binned_K((float)cb, 0.f, 0.f, rsqrtf(r.a2));
                 } else if (p.profile == HK_PROFILE_LORENTZ) {
                     pl = c / q;
                 } else if (q >= (double)HK_Z2 * a2) {
@@ -1270,7 +1280,10 @@ __global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const 
                     pl = c / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
                 } else {
                     const float inv_a = rsqrtf(r.a2);
-                    pl = r.cK * (double)core_any_K((float)cb * inv_a, sqrtf((float)G2) * inv_a, nullptr);
+                    const float x = (float)cb * inv_a, y = sqrtf((float)G2) * inv_a;
+                    // (a pure Gaussian through the same scaled fp32 evaluation as its bins, so that both vanish together)
+                    pl = y == 0.f ? (double)gauss_term((float)scalbn(r.cK, a.st->scale_exp), x) * scalbn(1.0, -a.st->scale_exp)
+                                  : r.cK * (double)core_any_K(x, y, nullptr);
                 }
             }
         }

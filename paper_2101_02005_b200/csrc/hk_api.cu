@@ -61,7 +61,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, recA, recB, recN, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
+    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
     size_t edge_acc_bytes;   // 0: grid too large for the per-bin edge accumulators (direct edge kernel only)
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
@@ -110,6 +110,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     L.idx_in = take(nn * 4);
     L.idx_out = take(nn * 4);
     L.recU = take(nn * sizeof(RecU));
+    L.flo = take(c->profile == HK_PROFILE_BINNED_GAUSSIAN ? nn * 4 : 0);   // low part of the sub-bin offset (R26)
     L.recA = take(nn * 16);
     L.recB = take(nn * 16);
     L.recN = take(nn * 16);
@@ -377,7 +378,8 @@ int hk_set_debug_mode(hk_ctx* ctx, int mode)
 
 int hk_set_node_separation(hk_ctx* ctx, double sep)
 {
-    if (!ctx || !std::isfinite(sep) || sep < 0.0 || sep > 64.0) return HK_EINVAL;
+    // 0 switches the node hierarchy off; below 3 half-widths the degree-7 interpolant leaves the error budget
+    if (!ctx || !std::isfinite(sep) || sep < 0.0 || sep > 64.0 || (sep > 0.0 && sep < 3.0)) return HK_EINVAL;
     ctx->node_sep = sep;
     return HK_OK;
 }
@@ -460,6 +462,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     int32_t* idx_in = (int32_t*)(ws + L.idx_in);
     int32_t* idx_out = (int32_t*)(ws + L.idx_out);
     RecU* recU = (RecU*)(ws + L.recU);
+    float* flo = p.profile == HK_PROFILE_BINNED_GAUSSIAN ? (float*)(ws + L.flo) : nullptr;
     float4* recA = (float4*)(ws + L.recA);
     float4* recB = (float4*)(ws + L.recB);
     float4* recN = (float4*)(ws + L.recN);
@@ -476,7 +479,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
 
     // a1: per-line parameters, keys
     line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
-                                                      lines->n_exp, ex, n, recU, keys_in, idx_in, st);
+                                                      lines->n_exp, ex, n, recU, keys_in, idx_in, flo, st);
     scale_kernel<<<1, 1, 0, stream>>>(st);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
     // a2: order by centre bin
@@ -487,7 +490,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     if (!reuse_sort)
         HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                                 (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
-    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, n, st, recA, recB, recN, p.profile);
+    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, p.profile);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges, node ranges and work units.  counts = [far | mid | edge | centre | near | node | 0], one scan.
     const int n_counts = 5 * p.n_ct + lv.n_entries + 1;
@@ -645,13 +648,17 @@ static int compute_any(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, doub
     bool first = true;
     double lo = none ? 1.0 : cmin;
     const double top = none ? 1.0 : cmax;
-    for (int k = 0; k < 64 && rc == HK_OK; ++k) {
+    // classes [lo, 2 lo) until the largest cutting length is covered; the 64th class is open-ended (its tile bounds come
+    // from [lo, top], correct for any ratio, only less sharp), so no line is ever left out however wide the range
+    constexpr int kMaxClasses = 64;
+    for (int k = 0; k < kMaxClasses && rc == HK_OK; ++k) {
         CutClass cls;
         cls.first = first;
         cls.lo = first ? 0.0 : lo;
-        cls.hi = (2.0 * lo > top) ? INFINITY : 2.0 * lo;
+        const bool last = (2.0 * lo > top) || k == kMaxClasses - 1;
+        cls.hi = last ? INFINITY : 2.0 * lo;
         cls.bound_lo = lo;
-        cls.bound_hi = std::fmin(2.0 * lo, top);
+        cls.bound_hi = last ? top : 2.0 * lo;
         rc = compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, stream, zero_out && first, false, extra, &cls);
         if (rc != HK_OK) break;
         launches += ctx->last_launches;

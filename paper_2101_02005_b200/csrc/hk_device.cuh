@@ -163,10 +163,33 @@ __device__ __forceinline__ float gh10_K(float x2, float s, float y)
     return y * sum;
 }
 
-// |z|^2 below which the trapezoid evaluator is used, as a function of y^2
-// (y = 0 exactly, the pure Gaussian of the Doppler profile: exp(-x^2) is ALL there is, followed down to e^-88, the
-//  end of the fp32 range)
-__device__ __forceinline__ float z3_for(float y2) { return y2 == 0.f ? 88.0f : y2 < 1e-6f ? 50.0f : HK_Z3; }
+// |z|^2 below which the innermost evaluator is used, as a function of y^2
+// (y = 0 exactly, the pure Gaussian of the Doppler profile: exp(-x^2) is ALL there is.  It is evaluated together with
+//  its amplitude, gauss_term below, and followed down to x^2 = HK_ZG: with the launch scale putting the largest
+//  amplitude at 2^100 that is the end of the fp32 range, 2^-126 -- DESIGN.md R22)
+#define HK_ZG 157.0f
+__device__ __forceinline__ float z3_for(float y2) { return y2 == 0.f ? HK_ZG : y2 < 1e-6f ? 50.0f : HK_Z3; }
+
+// cK exp(-x^2) for a pure Gaussian, amplitude and exponent combined BEFORE the exponential so that the product is
+// followed to the end of the fp32 range even where exp(-x^2) alone would underflow (x^2 > 87).  The exponent is
+// split so that its rounding error stays below 2^-22 up to x^2 = HK_ZG.
+__device__ __forceinline__ float gauss_term(float cK, float x)
+{
+    constexpr float L2E_HI = 1.44269502162933349609375f;      // log2(e) = HI + LO
+    constexpr float L2E_LO = 1.925963033500011e-08f;
+    const float x2 = x * x;
+    const float x2l = fmaf(x, x, -x2);                        // x^2 = x2 + x2l exactly
+    const float p = x2 * L2E_HI;                              // x^2 log2(e) = p + e
+    float e = fmaf(x2, L2E_HI, -p);
+    e = fmaf(x2, L2E_LO, e);
+    e = fmaf(x2l, L2E_HI, e);
+    const float n = rintf(p);                                 // p - n is exact (p < 2^8)
+    const float v = exp2f(n - p) * fmaf(-0.693147180559945f, e, 1.0f);
+    // cK v 2^-n in two steps: 2^-n alone may lie below the fp32 range while the product does not
+    const int k = min((int)n, 250), k1 = k >> 1;
+    const float s1 = __int_as_float((127 - k1) << 23), s2 = __int_as_float((127 - (k - k1)) << 23);
+    return ((cK * s1) * v) * s2;
+}
 
 // Re w(x + i y) for |z|^2 < HK_Z2, x >= 0, y > 0: ring by |z|^2
 __device__ __forceinline__ float core_any_K(float x, float y, int* region);
@@ -238,6 +261,7 @@ __device__ __noinline__ float core_K(float x, float y)
 __device__ __forceinline__ float core_any_K(float x, float y, int* region)
 {
     const float x2 = x * x, y2 = y * y, s = x2 + y2;
+    if (y == 0.f) { if (region) *region = 4; return __expf(-x2); }     // pure Gaussian (with its amplitude: gauss_term)
     const float z3 = z3_for(y2);
     if (s >= fmaxf(HK_Z4, z3)) { if (region) *region = 2; return gh4_K(x2, s, y); }
     if (s >= z3) { if (region) *region = 3; return gh6_K(x2, s, y); }
@@ -247,28 +271,37 @@ __device__ __forceinline__ float core_any_K(float x, float y, int* region)
 }
 
 // ---- binned Gaussian (HK_PROFILE_BINNED_GAUSSIAN): the Doppler profile averaged over the bin -------------------
-// K = V alpha_D sqrt(pi) = (a sqrt(pi)/2) [erf((|t| + 1/2)/a) - erf((|t| - 1/2)/a)] in bin units (a = alpha_D/dnu);
-// erfc in the tails; for a > 64 bins the second-order bin average exp(-x^2)(1 + h^2 (2 x^2 - 1)/3), h = 1/(2a),
-// is exact to 1.4e-7 and avoids the cancellation of two nearly equal erfc.  Zero beyond |t| = 1/2 + 6 a.
-__device__ __forceinline__ float binned_K(float t_abs, float inv_a)
+// K = V alpha_D sqrt(pi) = (a sqrt(pi)/2) [erf(e_hi/a) - erf(e_lo/a)] in bin units (a = alpha_D/dnu), e_hi / e_lo the
+// signed distances from the line centre to the bin's upper / lower edge; erfc in the tails; for a > 64 bins the
+// second-order bin average exp(-x^2)(1 + h^2 (2 x^2 - 1)/3), h = 1/(2a), is exact to 1.4e-7 and avoids the
+// cancellation of two nearly equal erfc.  Zero beyond |t| = 1/2 + 6 a.
+// The edge distances come from the bin offset d = b - jp (an exact small integer) and the sub-bin offset of the centre
+// as a hi/lo pair f + flo (R26): for a line much narrower than a bin whose centre lies within a few a of a
+// bin edge, the share of the neighbouring bin depends on (1/2 - |f|)/a, which one fp32 f resolves to 2^-26/a only.
+__device__ __forceinline__ float binned_K(float d, float f, float flo, float inv_a)
 {
     if (inv_a < (1.0f / 64.0f)) {
-        const float x = t_abs * inv_a, h = 0.5f * inv_a;
+        const float x = (d - f) * inv_a, h = 0.5f * inv_a;
         return __expf(-x * x) * fmaf(h * h * (1.0f / 3.0f), fmaf(2.0f * x, x, -1.0f), 1.0f);
     }
-    const float lo = (t_abs - 0.5f) * inv_a, hi = (t_abs + 0.5f) * inv_a;
-    const float d = lo >= 0.f ? erfcf(lo) - erfcf(hi) : erff(hi) - erff(lo);
-    return 0.886226925452758f * d / inv_a;
+    // (d +- 1/2) - f is exact whenever the result is small (Sterbenz), which is when it matters
+    const float lo = (((d - 0.5f) - f) - flo) * inv_a, hi = (((d + 0.5f) - f) - flo) * inv_a;
+    const float dd = lo >= 0.f ? erfcf(lo) - erfcf(hi) : hi <= 0.f ? erfcf(-hi) - erfcf(-lo) : erff(hi) - erff(lo);
+    return 0.886226925452758f * dd / inv_a;
 }
 __device__ __forceinline__ float binned_ql(float a2)
 {
     const float h = fmaf(6.0f, sqrtf(a2), 0.5f);
     return h * h;
 }
-// the value at |t| bins from the centre where the row formulas do not apply: by profile
-__device__ __forceinline__ float core_eval(int profile, float t_abs, float inv_a, float y)
+// S V of one (line, bin) pair where the row formulas do not apply, amplitude included: by profile.
+// d = b - jp, t = d - f (the row pass's t), inv_a = dnu/alpha_D, y = Gamma_L/alpha_D, cK = scale S/(alpha_D sqrt(pi)).
+__device__ __forceinline__ float core_term(int profile, float cK, float d, float f, float flo, float inv_a, float y)
 {
-    return profile == HK_PROFILE_BINNED_GAUSSIAN ? binned_K(t_abs, inv_a) : core_any_K(t_abs * inv_a, y, nullptr);
+    if (profile == HK_PROFILE_BINNED_GAUSSIAN) return cK * binned_K(d, f, flo, inv_a);
+    const float x = fabsf(d - f) * inv_a;
+    if (y == 0.f) return gauss_term(cK, x);
+    return cK * core_any_K(x, y, nullptr);
 }
 
 }  // namespace hk

@@ -104,6 +104,7 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
     LineOut o;
     o.valid = finite6(nu0, A, g, E, gam, nx) && nu0 > 0.0 && A >= 0.0;
     if (p.n_iso > 0) o.valid = o.valid && isfinite(gs) && isfinite(dl) && iso >= 0 && iso < p.n_iso;
+
     o.on_grid = false;
     o.foreign = false;
     o.S = o.gammaL = o.alphaD = 0.0;
@@ -115,12 +116,15 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
         o.alphaD = p.beta_iso[iso] * nu0;
         o.gammaL = A * p.inv4pic + exp(nx * p.ln_tfac) * (gam * (p.P_atm - p.P_self) + gs * p.P_self);
         o.S = A * g * p.sfac_iso[iso] / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));
-        ctr = nu0 + dl * p.P_atm;
+        ctr = __dadd_rn(nu0, __dmul_rn(dl, p.P_atm));                          // two roundings, as the oracle (no FMA contraction)
     } else {
     o.alphaD = p.beta * nu0;                                                   // Eq. 13 (L203)
     o.gammaL = A * p.inv4pic + gam * exp(nx * p.ln_tfac) * p.P_atm;            // Eq. 5 (L91): (T_ref/T)^n = e^(n ln(T_ref/T))
     o.S = A * g * p.sfac / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));  // Eq. 9 (L127)
     }
+    // (a width or strength that overflows fp64 -- finite fields, absurd exponents -- is treated like a non-finite
+    //  field, R14: the line is skipped)
+    if (!isfinite(o.gammaL) || !isfinite(o.S)) { o.valid = false; o.S = o.gammaL = o.alphaD = 0.0; return o; }
     const double big = 4.0e18;
     nu0 = ctr;
     double pos = __ddiv_rn(__dsub_rn(nu0, p.numin), p.dnu);
@@ -166,7 +170,8 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
                                                    const double* __restrict__ E, const double* __restrict__ gam,
                                                    const double* __restrict__ nx, LineExtra ex, int64_t n,
                                                    RecU* __restrict__ rec, int32_t* __restrict__ key,
-                                                   int32_t* __restrict__ idx, DevStats* __restrict__ st)
+                                                   int32_t* __restrict__ idx, float* __restrict__ flo,
+                                                   DevStats* __restrict__ st)
 {
     unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cgh6 = 0, ctrap = 0, cgh10 = 0, cmaxb = 0, cKmaxb = 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
@@ -188,7 +193,9 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             // sub-bin offset relative to the NEAREST grid point, in [-1/2, 1/2]: the profile is sampled at grid points, so
             // a centre that (almost) coincides with one needs its tiny offset at full relative precision (a narrow
             // Lorentzian sampled at its peak).  Negative (sign bit set, -0 included): the nearest point is jc + 1.
-            r.f = (float)(o.pos_f > 0.5 ? o.pos_f - 1.0 : o.pos_f);
+            const double fd = o.pos_f > 0.5 ? o.pos_f - 1.0 : o.pos_f;
+            r.f = (float)fd;
+            if (flo) flo[i] = (float)(fd - (double)r.f);                // low part (binned Gaussian only, R26)
             r.G2 = (float)(Gb * Gb);
             r.a2 = (float)(ab * ab);
             r.ilo = (int32_t)o.ilo;
@@ -204,6 +211,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
             //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
         }
+        if (flo && k == p.ksent) flo[i] = 0.f;
         rec[i] = r;
         key[i] = k;
         idx[i] = (int32_t)i;
@@ -246,7 +254,7 @@ __global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restric
         const double G2 = gauss ? 0.0 : (double)r.G2, a2 = profile == HK_PROFILE_LORENTZ ? 0.0 : (double)r.a2;
         const double pos = (double)r.jc + (signbit(r.f) ? 1.0 + (double)r.f : (double)r.f);
         const double y2 = a2 > 0.0 ? G2 / a2 : 1.0e300;
-        const double z3 = y2 == 0.0 ? 88.0 : y2 < 1e-6 ? 50.0 : (double)HK_Z3;
+        const double z3 = y2 == 0.0 ? (double)HK_ZG : y2 < 1e-6 ? 50.0 : (double)HK_Z3;
         const double t[4] = {(double)HK_Z1 * a2 - G2, (double)HK_Z2 * a2 - G2, (double)HK_Z4 * a2 - G2, z3 * a2 - G2};
 #pragma unroll
         for (int q = 0; q < 4; ++q)
@@ -275,32 +283,42 @@ __global__ void scale_kernel(DevStats* st)
     int e = 0;
     if (cmax > 0.0 && isfinite(cmax)) e = 40 - ilogb(cmax);
     if (cKmax > 0.0 && isfinite(cKmax)) e = min(e, 100 - ilogb(cKmax));
-    if (!(cmax > 0.0) && cKmax > 0.0 && isfinite(cKmax)) e = 60 - ilogb(cKmax);
+    // no Lorentz amplitude at all (Doppler / binned Gaussian): the largest Gaussian amplitude goes to 2^100, which leaves
+    // 226 binades below it -- exp(-x^2) is followed down to x^2 = HK_ZG (gauss_term, hk_device.cuh)
+    if (!(cmax > 0.0) && cKmax > 0.0 && isfinite(cKmax)) e = 100 - ilogb(cKmax);
     e = max(-900, min(900, e));
     st->scale_exp = e;
 }
 
 __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ idx_sorted,
-                                                     int64_t n, const DevStats* __restrict__ st,
+                                                     const float* __restrict__ flo, int64_t n,
+                                                     const DevStats* __restrict__ st,
                                                      float4* __restrict__ recA, float4* __restrict__ recB,
                                                      float4* __restrict__ recN, int profile)
 {
     const int e = st->scale_exp;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const RecU r = rec[idx_sorted[i]];
+        const int32_t src = idx_sorted[i];
+        const RecU r = rec[src];
         float cK = (float)scalbn(r.cK, e);
         // c = cK * G a / sqrt(pi)  (Lorentz amplitude S Gamma_L/(pi dnu^2) in bin units)
         const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
-        const float G2 = gauss ? 0.f : r.G2;
+        float G2 = gauss ? 0.f : r.G2;
         float c = cK * sqrtf(G2 * r.a2) * 0.564189583547756f;
+        // a Lorentzian of zero (or fp32-denormal) width contributes nothing anywhere but would give 0/0 on a grid point
+        // it coincides with: keep it out with c = 0 and a harmless width
+        if (profile == HK_PROFILE_LORENTZ && !(G2 >= 1.0e-30f)) { G2 = 1.0f; c = 0.f; }
         // a pure Lorentzian is what every formula of the accumulation kernels reduces to at alpha_D = 0 (no core,
         // no second asymptotic term); a pure Gaussian is the Voigt function at Gamma_L = 0 (c = 0: no wings)
         const float a2 = profile == HK_PROFILE_LORENTZ ? 0.f : r.a2;
         const bool up = signbit(r.f);                                  // centre = (jc + 1) + f with f <= 0
-        recA[i] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, G2, c);
+        // (binned Gaussian: G2 = 0 and c = 0 everywhere, and the free slot carries the low part of the sub-bin offset)
+        recA[i] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, (flo && profile == HK_PROFILE_BINNED_GAUSSIAN) ? flo[src] : G2, c);
         recB[i] = make_float4(a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
-        const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));   // floor-based, [0, 1)
-        const uint32_t a19 = ((uint32_t)__float_as_int(a2) >> 12) & 0x7FFFFu;
+        // node record: offset from jc in [0, 1) rounded to the nearest 1/8192 (|error| <= 2^-14 bins; 8192 clamps to 8191),
+        // a2 rounded to nearest at 11 mantissa bits (|error| <= 2^-12 relative, unbiased)
+        const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));
+        const uint32_t a19 = (((uint32_t)__float_as_int(a2) + 0x800u) >> 12) & 0x7FFFFu;
         recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), G2, c);
     }
 }

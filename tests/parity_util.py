@@ -27,6 +27,22 @@ def check_parity(k_gpu, k_ref, kmax=None, rel=REL_TOL, floor=FLOOR, what=""):
     return relerr, abserr, float(big.mean())
 
 
+def check_parity_plinth(k_gpu, k_ref, k_raw, rel=REL_TOL, floor=FLOOR, what=""):
+    """Tolerance with plinth removal (section 2.1.1; R27).  The paper defines the result as
+    the line opacity minus its value at the cutting length and stores opacities in single precision (L367): a
+    difference of two stored-precision numbers is defined to a fraction of the UNSUBTRACTED value, so the north_star
+    pair is applied with the opacity before removal as the reference magnitude: |k - k_ref| <= rel k_raw + floor
+    max(k_raw) on every bin.  Where the removed part is negligible this is the plain north_star tolerance."""
+    k_gpu = np.asarray(k_gpu, dtype=np.float64)
+    assert np.all(np.isfinite(k_gpu)), f"{what}: non-finite GPU output"
+    err = np.abs(k_gpu - k_ref)
+    kmax = float(k_raw.max()) if k_raw.size else 0.0
+    bad = err > rel * k_raw + floor * kmax
+    worst = float((err / np.maximum(k_raw, 1e-300))[k_raw >= floor * kmax].max()) if (k_raw >= floor * kmax).any() else 0.0
+    assert not bad.any(), f"{what}: {int(bad.sum())} bins beyond {rel:g} x unsubtracted k (worst {worst:.3e})"
+    return worst
+
+
 def sample_windows(N, n_windows, width, rng):
     """Stratified windows of `width` contiguous bins incl. the first and last."""
     if N <= n_windows * width:
