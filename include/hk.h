@@ -90,7 +90,8 @@ typedef struct {
 
 /* Phases of one hk_compute, timed with CUDA events on the caller's stream. */
 enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, HK_PH_FAR = 4, HK_PH_MID = 5, HK_PH_EDGE = 6,
-       HK_PH_CENTRE = 7, HK_PH_NEAR = 8, HK_PH_DOWN = 9, HK_PH_COUNT = 10 };
+       HK_PH_CENTRE = 7 /* line centres, row kernel */, HK_PH_LANE = 8 /* line centres, innermost bins */, HK_PH_NEAR = 9,
+       HK_PH_DOWN = 10, HK_PH_COUNT = 11 };
 
 /* Region thresholds on |z|^2 = x^2 + y^2 used by the fp32 evaluator. */
 #define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */

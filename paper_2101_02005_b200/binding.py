@@ -29,7 +29,7 @@ EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_w
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode", "hk_compute_bands",
            "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
            "hk_last_cuda_error", "hk_strerror")
-PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "near", "down")
+PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "lane", "near", "down")
 
 
 class hk_lines(C.Structure):

@@ -9,7 +9,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhk.so")
 SOURCES = ["hk_api.cu"]
-HEADERS = ["hk_device.cuh", "hk_preprocess.cuh", "hk_accumulate.cuh", os.path.join("..", "..", "include", "hk.h")]
+HEADERS = ["hk_device.cuh", "hk_preprocess.cuh", "hk_accumulate.cuh", "hk_centre.cuh", "hk_gh_tables.cuh",
+           os.path.join("..", "..", "include", "hk.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]

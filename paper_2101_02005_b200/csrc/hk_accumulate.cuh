@@ -42,6 +42,7 @@ struct AccArgs {
     const float4* __restrict__ recA;
     const float4* __restrict__ recB;
     const float4* __restrict__ recN;
+    const float4* __restrict__ recC;           // { dnu/alpha_D, -f dnu/alpha_D, y^2, 1/(cK y) }: the centre kernels' per-line part
     const TileRange* __restrict__ tr;
     const NodeRange* __restrict__ nr;
     // exclusive scans of the work-unit counts (one concatenated scan; each kernel reads its own slice, whose first
@@ -50,6 +51,7 @@ struct AccArgs {
     const int32_t* __restrict__ prefix_mid;
     const int32_t* __restrict__ prefix_edge;
     const int32_t* __restrict__ prefix_centre;
+    const int32_t* __restrict__ prefix_lane;   // the same line ranges in longer chunks (centre_lane_kernel)
     const int32_t* __restrict__ prefix_near;
     const int32_t* __restrict__ prefix_node;
     DevStats* st;
@@ -58,7 +60,7 @@ struct AccArgs {
     double* __restrict__ plinth_acc;           // N + 1 doubles: difference array of the plinths, then its running sum; or null
     double* __restrict__ edge_acc;             // [2][N][kP] per-bin node sums of extent ends (scaled), fp64; or null
     int64_t N;
-    int32_t n_ct, chunk, chunk_node;
+    int32_t n_ct, chunk, chunk_node, chunk_centre, chunk_lane;
     int32_t profile;                           // HK_PROFILE_*: only the binned Gaussian changes the kernels' core evaluation
     Levels lv;
 };
@@ -408,298 +410,11 @@ __global__ void __launch_bounds__(kThreads, 4) edge_kernel(AccArgs a)
     }
 }
 
-// ---------------------------------------------------------------------------------------
-// centre kernel: tiles inside the extent that hold bins with |z|^2 < Z2 (the line's core) or lie within 2 KB bins
-// ---------------------------------------------------------------------------------------
-// Row pass (lanes own bins, the warp walks its lines).  Per (line, tile) one of two row formulas, decided when the
-// line is staged: "Gauss-Hermite 4" rows where the tile holds core bins (valid for every |z|^2 >= Z4, so the whole
-// outer ring 8 <= |z| < 25 -- three quarters of all core evaluations -- is evaluated here, 64 bins per packed
-// instruction) with the term selected to zero where |z|^2 < ql = Z4 a^2; two-term asymptotic rows otherwise (and for
-// the row pairs of a Gauss-Hermite tile that lie wholly beyond the core), zero where |z|^2 < ql = Z2 a^2.
-// Lane pass (lane <-> line, 32 lines at a time) for the bins with q < ql: all lanes step through the SAME bins, each
-// evaluating its own line there; a batch is counting-sorted by y = Gamma_L/alpha_D when it is staged, so the 32 lines
-// of a group have nearly the same centre, Doppler width AND ring boundaries and the lanes run the same evaluator.
-// The 32 x 16 values of a half-row go through a shared staging matrix and are summed per bin (a transpose, no
-// atomics), then added to the warp's bin tile in shared memory.
-constexpr int kSubC = 512;
-constexpr int kLPTC = kSubC / kThreads;
-constexpr int kStage = 16;             // bins per staging step of the core pass
-constexpr int kCentreCtas = 4;         // resident CTAs per SM the centre kernel is compiled and launched for
 constexpr int kNodeCtas = 6;           // resident CTAs per SM of the node kernel
-constexpr int kYClasses = 32;          // classes of y = Gamma_L/alpha_D the lines of a batch are sorted into
-static_assert(kSubC == 32 * 2 * kWarps, "a batch is 2 groups of 32 lines per warp");
 
-// rings of the core evaluator change with y (trapezoid below 5.5, Gauss-Hermite 6 below 8, no core from 25)
-__device__ __forceinline__ int y_class(float y)
-{
-    if (y < 6.0f) return (int)(y * 4.0f);                          // 0..23: class edges at 2 (HK_Y10) and 5.5
-    if (y < 8.0f) return 24 + (int)(y - 6.0f);                     // 24, 25
-    if (y < 25.0f) return 26 + (int)((y - 8.0f) * (5.0f / 17.0f));   // 26..30
-    return 31;
-}
-
-// W = warps per CTA: 8 for dense lists; 2 for sparse ones (few lines per tile: a work unit is a handful of lines, and
-// four times as many small CTAs keep four times as many units in flight)
-// kBinned: the binned-Gaussian profile (its own instantiation, so that the Voigt path carries none of its code)
-template <int KB, int W, bool kBinned>
-__global__ void __launch_bounds__(32 * W, (kCentreCtas * kWarps) / W) centre_kernel(AccArgs a)
-{
-    constexpr int kWarps = W, kThreads = 32 * W, kSubC = 64 * W, kLPTC = kSubC / kThreads;   // shadow the 8-warp values
-    constexpr int kTB = 32 * KB;
-    constexpr int M = KB / 2;
-    static_assert(sizeof(double) * kWarps * kTB <= sizeof(float4) * 2 * kSubC, "red must fit in the staging buffers");
-    __shared__ float4 smem[2][kSubC];          // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y } (see stash)
-    __shared__ float stage[kWarps][kStage][33];
-    __shared__ float sacc[kWarps][kTB];
-    __shared__ int hist[kYClasses];
-    __shared__ int s_unit;
-    float4* smA = smem[0];
-    float4* smB = smem[1];
-    double* red = reinterpret_cast<double*>(&smem[0][0]);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int32_t* __restrict__ prefix = a.prefix_centre;
-    const int base = prefix[0], total = prefix[a.n_ct];
-    const float whi = (float)(kTB - 1);
-
-    float2 tb[M];
-#pragma unroll
-    for (int m = 0; m < M; ++m) {
-        float b0 = (float)(lane + 64 * m);
-        tb[m] = make_float2(b0, b0 + 32.0f);
-    }
-#pragma unroll
-    for (int j = 0; j < KB; ++j) sacc[warp][lane + 32 * j] = 0.f;
-
-    for (;;) {
-        const int u = next_unit(&a.st->unit_counter_centre, &s_unit) + base;
-        if (u >= total) break;
-        const int ct = find_tile(prefix, a.n_ct, u);
-        const int64_t ct0 = (int64_t)ct * kTB;
-        const TileRange r = a.tr[ct];
-        const int c0 = r.CL + (u - prefix[ct]) * a.chunk;
-        const int nt = min(a.chunk, r.CR - c0);
-        if (nt <= 0) continue;
-        if (threadIdx.x == 0) atomicAdd(&a.st->units_centre, 1ULL);
-
-        float2 acc[M];
-        double acc64[KB];
-#pragma unroll
-        for (int m = 0; m < M; ++m) acc[m] = make_float2(0.f, 0.f);
-#pragma unroll
-        for (int j = 0; j < KB; ++j) acc64[j] = 0.0;
-        int since_flush = 0;
-        auto flush = [&]() {
-            __syncwarp();
-#pragma unroll
-            for (int m = 0; m < M; ++m) {
-                acc64[2 * m] += (double)acc[m].x + (double)sacc[warp][lane + 64 * m];
-                acc64[2 * m + 1] += (double)acc[m].y + (double)sacc[warp][lane + 64 * m + 32];
-                acc[m] = make_float2(0.f, 0.f);
-                sacc[warp][lane + 64 * m] = 0.f;
-                sacc[warp][lane + 64 * m + 32] = 0.f;
-            }
-            since_flush = 0;
-            __syncwarp();
-        };
-
-        float4 preA[kLPTC], preB[kLPTC];
-        auto fetch = [&](int v0) {
-#pragma unroll
-            for (int k = 0; k < kLPTC; ++k) {
-                const int v = v0 + threadIdx.x + k * kThreads;
-                if (v < nt) { preA[k] = a.recA[c0 + v]; preB[k] = a.recB[c0 + v]; }
-            }
-        };
-        // The batch is counting-sorted by y = Gamma_L/alpha_D on its way into shared memory: lines that are neighbours
-        // in centre-bin order have nearly the same centre and Doppler width, so after the sort the 32 lines of a group
-        // also have nearly the same ring boundaries and the lanes of the core pass run the same evaluator.
-        auto stash = [&](int v0) {
-            int cls[kLPTC], rk[kLPTC];
-            float yv[kLPTC];
-            if (threadIdx.x < kYClasses) hist[threadIdx.x] = 0;
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < kLPTC; ++k) {
-                const int i = threadIdx.x + k * kThreads;
-                if (v0 + i < nt) {
-                    yv[k] = kBinned ? 0.f : sqrtf(preA[k].z) * rsqrtf(preB[k].x);      // (binned: A.z carries flo, not G2)
-                    cls[k] = y_class(yv[k]);
-                    rk[k] = atomicAdd(&hist[cls[k]], 1);
-                }
-            }
-            __syncthreads();
-            if (warp == 0) {
-                const int cnt = hist[lane];
-                int inc = cnt;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int up = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += up;
-                }
-                hist[lane] = inc - cnt;
-            }
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < kLPTC; ++k) {
-                const int i = threadIdx.x + k * kThreads;
-                if (v0 + i < nt) {
-                    const float4 ra = preA[k], rb = preB[k];
-                    const int dst = hist[cls[k]] + rk[k];
-                    const float fdj = (float)((int64_t)__float_as_int(ra.x) - ct0);
-                    const float G2 = kBinned ? 0.f : ra.z, a2 = rb.x;
-                    // smallest and largest q = t^2 + G2 over the tile's bins (from below / from above)
-                    const float pos = fdj + ra.y;
-                    const float dmin = fmaxf(fmaxf(-pos, pos - whi), 0.f) * 0.999f;
-                    const float dmax = fmaxf(fabsf(pos), fabsf(whi - pos)) * 1.001f;
-                    const float qmin = fmaf(dmin, dmin, G2) * 0.9999f, qmax = fmaf(dmax, dmax, G2);
-                    const float qc = (HK_Z2 / 1.5f) * (1.5f * a2);            // as the row pass recomputes it
-                    // Gauss-Hermite rows: the tile holds core bins and (D1 D2 ~ |z|^8) stays inside fp32
-                    constexpr bool binned = kBinned;
-                    const float ql = binned ? binned_ql(a2) : (qmin < qc && qmax <= 1.0e9f * a2) ? (G2 == 0.f ? HK_ZG : HK_Z4) * a2 : qc;   // (pure Gaussian: see z3_for)
-                    // A = { -dl, G2, P, Q }, B = { -f, +-ql, cK, y }: Gauss-Hermite rows (B.y < 0) carry P = cK y and
-                    // Q = 1/a^2, two-term rows P = c (Lorentz amplitude) and Q = 1.5 a^2 -- what the row pass needs, ready
-                    if (!binned && ql < qc) {
-                        smA[dst] = make_float4(-fdj, G2, rb.w * yv[k], 1.0f / a2);
-                        smB[dst] = make_float4(-ra.y, -ql, rb.w, yv[k]);
-                    } else {
-                        smA[dst] = make_float4(-fdj, G2, ra.w, 1.5f * a2);
-                        smB[dst] = make_float4(-ra.y, ql, rb.w, kBinned ? ra.z : yv[k]);     // binned: the low part of f
-                    }
-                }
-            }
-        };
-        fetch(0);
-        for (int v0 = 0; v0 < nt; v0 += kSubC) {
-            __syncthreads();                        // previous batch fully consumed
-            stash(v0);
-            __syncthreads();
-            if (v0 + kSubC < nt) fetch(v0 + kSubC);
-            const int nb = min(kSubC, nt - v0);
-            // groups of gs <= 32 sorted lines (every warp gets one when the batch is small); warp w takes groups w and
-            // 15 - w (a cheap high-y group with an expensive low-y one)
-            const int gs = min(32, (nb + kWarps - 1) / kWarps);
-#pragma unroll 1
-            for (int gi = 0; gi < 2; ++gi) {
-            const int grp = gi == 0 ? warp : 2 * kWarps - 1 - warp;
-            const int wl0 = gs * grp, wl1 = min(wl0 + gs, nb);
-            if (wl0 >= wl1) continue;
-            // ---- row pass
-            int l = wl0;
-            while (l < wl1) {
-                const int stop = min(wl1, l + (kFlush - since_flush));
-                since_flush += stop - l;
-#pragma unroll 1
-                for (; l < stop; ++l) {
-                    const float4 A = smA[l];
-                    const float2 Bxy = *reinterpret_cast<const float2*>(&smB[l]);
-                    const float2 ndl = bcast2(A.x), nf = bcast2(Bxy.x), g = bcast2(A.y);
-                    const float ql = fabsf(Bxy.y);
-                    if (Bxy.y < 0.f) {
-                        // Gauss-Hermite 4 in bin units: x^2 = t^2/a^2, s = q/a^2 (hk_device.cuh gh4_K)
-                        constexpr float T1 = 0.27525512860841095f, T2 = 2.7247448713915890f;
-                        constexpr float W1 = 0.5124242247547685f, W2 = 0.05176535879298783f;
-                        const float2 ia2 = bcast2(A.w), cky = bcast2(A.z);
-                        const float2 t1 = bcast2(T1), t2 = bcast2(T2), m1 = bcast2(-4.0f * T1), m2 = bcast2(-4.0f * T2);
-                        const float2 w1 = bcast2(W1), w2 = bcast2(W2);
-#pragma unroll
-                        for (int m = 0; m < M; ++m) {
-                            const float2 d = __fadd2_rn(tb[m], ndl);     // exact: both are small integers
-                            const float2 t = __fadd2_rn(d, nf);
-                            const float2 q = __ffma2_rn(t, t, g);
-                            const float2 x2 = __fmul2_rn(__fmul2_rn(t, t), ia2);
-                            const float2 sz = __fmul2_rn(q, ia2);
-                            const float2 P1 = __fadd2_rn(sz, t1), P2 = __fadd2_rn(sz, t2);
-                            const float2 D1 = __ffma2_rn(P1, P1, __fmul2_rn(m1, x2));
-                            const float2 D2 = __ffma2_rn(P2, P2, __fmul2_rn(m2, x2));
-                            const float2 num = __ffma2_rn(__fmul2_rn(w2, P2), D1, __fmul2_rn(__fmul2_rn(w1, P1), D2));
-                            float2 ww = __fmul2_rn(num, rcp2(__fmul2_rn(D1, D2)));
-                            ww.x = q.x >= ql ? ww.x : 0.f;                  // the lane pass owns these bins
-                            ww.y = q.y >= ql ? ww.y : 0.f;
-                            acc[m] = __ffma2_rn(cky, ww, acc[m]);
-                        }
-                    } else {
-                        const float2 c = bcast2(A.z), A1 = bcast2(A.w), one = bcast2(1.0f);
-                        const float2 nA2 = bcast2(-1.33333333f * A.w * A.y);
-#pragma unroll
-                        for (int m = 0; m < M; ++m) {
-                            const float2 d = __fadd2_rn(tb[m], ndl);
-                            const float2 t = __fadd2_rn(d, nf);
-                            const float2 q = __ffma2_rn(t, t, g);
-                            const float2 rr = rcp2(q);
-                            const float2 uu = __ffma2_rn(nA2, rr, A1);
-                            const float2 vv = __ffma2_rn(uu, rr, one);
-                            float2 ww = __fmul2_rn(rr, vv);
-                            ww.x = q.x >= ql ? ww.x : 0.f;
-                            ww.y = q.y >= ql ? ww.y : 0.f;
-                            acc[m] = __ffma2_rn(c, ww, acc[m]);
-                        }
-                    }
-                }
-                if (since_flush >= kFlush) flush();
-            }
-            // ---- lane pass: bins with q < ql
-            {
-                const int li = wl0 + lane;
-                float dl = 0.f, f = 0.f, G2 = 1.f, cK = 0.f, ql = 0.f, y = 1.f, inv_a = 1.f;
-                float clo = 1e9f, chi = -1e9f;
-                if (li < wl1) {
-                    const float4 A = smA[li], B = smB[li];
-                    dl = -A.x; f = -B.x; G2 = A.y; ql = fabsf(B.y); cK = B.z; y = B.w;
-                    const float h2 = ql - G2;
-                    if (h2 > 0.f) {
-                        const float hw = sqrtf(h2) + 1.0f;                       // |t| < hw covers every q < ql
-                        const float pos = dl + f;
-                        const float lo = fmaxf(ceilf(pos - hw), 0.f), hi = fminf(floorf(pos + hw), whi);
-                        if (hi >= lo) { clo = lo; chi = hi; }
-                    }
-                    inv_a = B.y < 0.f ? sqrtf(A.w) : sqrtf(1.5f / A.w);          // IEEE sqrt and division: a Gaussian tail amplifies an error of x by 2 x^2
-                }
-                float bmin = clo, bmax = chi;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-                    bmin = fminf(bmin, __shfl_xor_sync(0xffffffffu, bmin, o));
-                    bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
-                }
-                if (bmax >= bmin) {
-                    const int b_end = (int)bmax;
-                    const int col = lane & (kStage - 1), half = lane >> 4;
-#pragma unroll 1
-                    for (int b0 = (int)bmin; b0 <= b_end; b0 += kStage) {
-                        const int ns = min(kStage, b_end - b0 + 1);              // steps of this block (warp-uniform)
-                        const float e0 = (float)b0 - dl;                         // exact (small integers)
-#pragma unroll
-                        for (int s = 0; s < kStage; ++s) {
-                            if (s < ns) {
-                                const float t = (e0 + (float)s) - f;             // the row pass's t, bit for bit
-                                const float q = fmaf(t, t, G2);
-                                float val = 0.f;
-                                if (q < ql) val = kBinned ? cK * binned_K(e0 + (float)s, f, y, inv_a)          // y: flo here
-                                                  : y == 0.f ? gauss_term(cK, fabsf(t) * inv_a)
-                                                             : cK * core_any_K(fabsf(t) * inv_a, y, nullptr);
-                                stage[warp][s][lane] = val;
-                            }
-                        }
-                        __syncwarp();
-                        float sum = 0.f;
-                        if (col < ns) {
-#pragma unroll
-                            for (int j = 0; j < 16; ++j) sum += stage[warp][col][half * 16 + j];
-                        }
-                        sum += __shfl_xor_sync(0xffffffffu, sum, 16);
-                        if (half == 0 && col < ns) sacc[warp][b0 + col] += sum;
-                        __syncwarp();
-                    }
-                    since_flush += 32;     // the bin tile holds at most 32 lines' terms per bin per batch
-                    if (since_flush >= kFlush) flush();
-                }
-            }
-            }   // groups
-        }
-        flush();
-        __syncthreads();               // every warp is done with the staging buffers: red may overwrite them
-        flush_tile<KB, W>(red, acc64, ct0, a);
-    }
-}
+}  // namespace hk
+#include "hk_centre.cuh"               // the line centres: centre_row_kernel, centre_lane_kernel
+namespace hk {
 
 // ---------------------------------------------------------------------------------------
 // near / edge kernel
@@ -1315,7 +1030,13 @@ __global__ void __launch_bounds__(256) probe_kernel(const float* __restrict__ x,
         int reg;
         if (q >= HK_Z1) { K = term_far(c, q); reg = 0; }
         else if (q >= HK_Z2) { K = c * shape_mid(rcp_approx(q), 1.5f, 2.0f * G2); reg = 1; }
-        else { K = core_any_K(fabsf(t), G, &reg); }
+        else {
+            K = core_any_K(fabsf(t), G, &reg);
+            // regions 2 and 3 as the row kernel evaluates them: the expanded rational forms (hk_centre.cuh)
+            if (reg == 2) K = gh4_row_K(t * t, G2, G);
+            if (reg == 3) K = gh6_row_K(t * t, G2, G);
+            if (reg == 5) K = gh10_row_K(t * t, G2, G);
+        }
         out[i] = K;
         if (region) region[i] = reg;
     }

@@ -61,12 +61,12 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
+    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, recC, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
     size_t edge_acc_bytes;   // 0: grid too large for the per-bin edge accumulators (direct edge kernel only)
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
     int32_t n_entries;   // upper bound on (level, tile) entries of the node hierarchy
-    int32_t n_counts;    // work-unit counts: 5 n_ct (far, mid, edge, centre, near) + n_entries (node) + 1
+    int32_t n_counts;    // work-unit counts: 6 n_ct (far, mid, edge, centre, near, lane) + n_entries (node) + 1
 };
 
 bool is_uncut(double cut) { return !(cut > 0.0 && std::isfinite(cut)); }
@@ -100,7 +100,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     Layout L;
     L.n_ct = (int32_t)((c->N + 32 * kMinKB - 1) / (32 * kMinKB));
     L.n_entries = 2 * L.n_ct + kMaxLevels;
-    L.n_counts = 5 * L.n_ct + L.n_entries + 1;
+    L.n_counts = 6 * L.n_ct + L.n_entries + 1;
     size_t nn = (size_t)(n > 0 ? n : 1);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
@@ -114,6 +114,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     L.recA = take(nn * 16);
     L.recB = take(nn * 16);
     L.recN = take(nn * 16);
+    L.recC = take(nn * 16);
     L.tr = take((size_t)L.n_ct * sizeof(TileRange));
     L.nr = take((size_t)L.n_entries * sizeof(NodeRange));
     L.node_acc = take((size_t)L.n_entries * kP * sizeof(double));
@@ -213,6 +214,8 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     p.n_ct = (int32_t)((c->N + 32 * p.kb - 1) / (32 * p.kb));
     p.chunk = chunk;
     p.chunk_node = 16384;
+    p.chunk_centre = 2048;
+    p.chunk_lane = 16384;
     p.sep = c->node_sep;
     p.plinth = (c->plinth && !p.uncut) ? 1 : 0;
     p.cut_bins = cb;
@@ -466,6 +469,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     float4* recA = (float4*)(ws + L.recA);
     float4* recB = (float4*)(ws + L.recB);
     float4* recN = (float4*)(ws + L.recN);
+    float4* recC = (float4*)(ws + L.recC);
     TileRange* tr = (TileRange*)(ws + L.tr);
     NodeRange* nr = (NodeRange*)(ws + L.nr);
     double* node_acc = (double*)(ws + L.node_acc);
@@ -490,19 +494,20 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     if (!reuse_sort)
         HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                                 (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
-    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, p.profile);
+    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, recC, p.profile);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges, node ranges and work units.  counts = [far | mid | edge | centre | near | node | 0], one scan.
-    const int n_counts = 5 * p.n_ct + lv.n_entries + 1;
+    const int n_counts = 6 * p.n_ct + lv.n_entries + 1;
     int32_t* cnt_far = counts;
     int32_t* cnt_mid = counts + p.n_ct;
     int32_t* cnt_edge = counts + 2 * p.n_ct;
     int32_t* cnt_centre = counts + 3 * p.n_ct;
     int32_t* cnt_near = counts + 4 * p.n_ct;
-    int32_t* cnt_node = counts + 5 * p.n_ct;
+    int32_t* cnt_lane = counts + 5 * p.n_ct;
+    int32_t* cnt_node = counts + 6 * p.n_ct;
     HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
     range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_edge, cnt_centre,
-                                                           cnt_near, st);
+                                                           cnt_near, cnt_lane, st);
     ctx->last_launches = 5;
     if (lv.n_entries > 0) {
         HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
@@ -514,15 +519,16 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_RANGES + 1], stream));
     // a4-a7: accumulate
     AccArgs a;
-    a.recA = recA; a.recB = recB; a.recN = recN; a.tr = tr; a.nr = nr;
+    a.recA = recA; a.recB = recB; a.recN = recN; a.recC = recC; a.tr = tr; a.nr = nr;
     a.prefix_far = prefix; a.prefix_mid = prefix + p.n_ct; a.prefix_edge = prefix + 2 * p.n_ct;
     a.prefix_centre = prefix + 3 * p.n_ct; a.prefix_near = prefix + 4 * p.n_ct;
-    a.prefix_node = prefix + 5 * p.n_ct;
+    a.prefix_lane = prefix + 5 * p.n_ct;
+    a.prefix_node = prefix + 6 * p.n_ct;
     a.st = st; a.out_k = out_k_dev; a.node_acc = node_acc; a.profile = p.profile;
     const bool use_edge_nodes = p.edge_nodes && p.mode == 0 && lv.n_levels > 0 && !p.uncut;
     a.edge_acc = use_edge_nodes ? edge_acc : nullptr;
     a.plinth_acc = p.plinth ? (double*)(ws + L.plinth_acc) : nullptr;
-    a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.lv = lv;
+    a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.chunk_centre = p.chunk_centre; a.chunk_lane = p.chunk_lane; a.lv = lv;
     const int grid = ctx->n_sm * 2;
     if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NODE + 1], stream));
@@ -543,21 +549,30 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         }
         cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
         if (p.mode == 0 || p.mode == 3) {
-            // sparse lists (fewer than 256 lines per level-0 tile on average): 2-warp CTAs, four times as many
-            auto centre = [&](auto binned_tag) {
-                constexpr bool kB = decltype(binned_tag)::value;
-                if ((double)n_lines * (32.0 * KB) < 32.0 * (double)ctx->N)
-                    centre_kernel<KB, 1, kB><<<ctx->n_sm * kCentreCtas * 8, 32, 0, stream>>>(a);
-                else if ((double)n_lines * (32.0 * KB) < 256.0 * (double)ctx->N)
-                    centre_kernel<KB, 2, kB><<<ctx->n_sm * kCentreCtas * 4, 64, 0, stream>>>(a);
-                else
-                    centre_kernel<KB, kWarps, kB><<<ctx->n_sm * kCentreCtas, kThreads, 0, stream>>>(a);
-            };
-            if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) centre(std::true_type());
-            else centre(std::false_type());
-            ++ctx->last_launches;
+            // rows (lanes own bins): nothing to do for the Gaussian profiles, whose records carry no Lorentz amplitude
+            const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
+            if (!gauss) { centre_row_kernel<KB><<<ctx->n_sm * kRowCtas, 32 * kRowWarps, 0, stream>>>(a); ++ctx->last_launches; }
         }
         cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
+        if (p.mode == 0 || p.mode == 3) {
+            // innermost bins (lane <-> line): none for a pure Lorentzian.  Sparse lists (fewer than 256 lines per level-0
+            // tile on average) run 2- or 1-warp CTAs, four or eight times as many: a work unit there is a handful of lines
+            if (p.profile != HK_PROFILE_LORENTZ) {
+                auto lanek = [&](auto binned_tag) {
+                    constexpr bool kB = decltype(binned_tag)::value;
+                    if ((double)n_lines * (32.0 * KB) < 32.0 * (double)ctx->N)
+                        centre_lane_kernel<KB, 1, kB><<<ctx->n_sm * kLaneCtas * 8, 32, 0, stream>>>(a);
+                    else if ((double)n_lines * (32.0 * KB) < 256.0 * (double)ctx->N)
+                        centre_lane_kernel<KB, 2, kB><<<ctx->n_sm * kLaneCtas * 4, 64, 0, stream>>>(a);
+                    else
+                        centre_lane_kernel<KB, 8, kB><<<ctx->n_sm * kLaneCtas, 256, 0, stream>>>(a);
+                };
+                if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) lanek(std::true_type());
+                else lanek(std::false_type());
+                ++ctx->last_launches;
+            }
+        }
+        cudaEventRecord(ctx->ev[HK_PH_LANE + 1], stream);
         near_kernel<KB><<<grid, kThreads, 0, stream>>>(a);
         ++ctx->last_launches;
         cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream);

@@ -55,6 +55,8 @@ struct Params {
     int32_t n_ct;               // tiles of 32 kb bins
     int32_t chunk;              // lines per work unit of the direct kernels
     int32_t chunk_node;         // lines per work unit of the node kernel
+    int32_t chunk_centre;       // lines per work unit of the centre row kernel (a warp)
+    int32_t chunk_lane;         // lines per work unit of the centre lane kernel (a CTA)
     double sep;                 // node separation: |centre - tile centre| >= sep * half-width
     int profile;                // 0 Voigt, 1 Lorentz (records carry alpha_D = 0), 2 Doppler (records carry Gamma_L = 0)
     int plinth;                 // 1: remove every line's value at the cutting length from its bins (section 2.1.1)
@@ -72,7 +74,7 @@ struct DevStats {
     int32_t scale_exp;
     int32_t pad;
     unsigned int unit_counter_far, unit_counter_mid, unit_counter_near, unit_counter_node;
-    unsigned int unit_counter_edge, unit_counter_centre;
+    unsigned int unit_counter_edge, unit_counter_centre, unit_counter_lane, pad2;
     unsigned long long units_far, units_mid, units_near, units_node, units_edge, units_centre;
     unsigned long long pairs_far, pairs_mid, pairs_near;   // (line, bin) slots per kernel, from the tile ranges
     unsigned long long pairs_edge, pairs_centre;
@@ -294,7 +296,7 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
                                                      const float* __restrict__ flo, int64_t n,
                                                      const DevStats* __restrict__ st,
                                                      float4* __restrict__ recA, float4* __restrict__ recB,
-                                                     float4* __restrict__ recN, int profile)
+                                                     float4* __restrict__ recN, float4* __restrict__ recC, int profile)
 {
     const int e = st->scale_exp;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
@@ -320,6 +322,17 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
         const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));
         const uint32_t a19 = (((uint32_t)__float_as_int(a2) + 0x800u) >> 12) & 0x7FFFFu;
         recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), G2, c);
+        // the per-line part of the centre kernels (hk_centre.cuh): IEEE roots and quotients, once per line.
+        // ip = 1/(cK y), the reciprocal amplitude of the Gauss-Hermite rows; 0: no such rows (G = 0, or an amplitude
+        // below the range of the launch)
+        float inva = 0.f, y2 = 0.f, ip = 0.f;
+        if (a2 > 0.f) {
+            inva = __fsqrt_rn(__fdiv_rn(1.0f, a2));          // the Gaussian tail amplifies an error of x by 2 x^2
+            y2 = gauss ? 0.f : __fdiv_rn(G2, a2);
+            const float P = cK * __fsqrt_rn(y2);
+            if (P > 1.0e-30f && c != 0.f) ip = __fdiv_rn(1.0f, P);
+        }
+        recC[i] = make_float4(inva, __fmul_rn(-r.f, inva), y2, ip);
     }
 }
 
@@ -485,7 +498,7 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
                                                     TileRange* __restrict__ tr, int32_t* __restrict__ cnt_far,
                                                     int32_t* __restrict__ cnt_mid, int32_t* __restrict__ cnt_edge,
                                                     int32_t* __restrict__ cnt_centre, int32_t* __restrict__ cnt_near,
-                                                    DevStats* __restrict__ st)
+                                                    int32_t* __restrict__ cnt_lane, DevStats* __restrict__ st)
 {
     int wt = blockIdx.x * blockDim.x + threadIdx.x;
     if (wt >= p.n_ct) return;
@@ -560,7 +573,8 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
     cnt_far[wt] = (int32_t)((nfar + p.chunk - 1) / p.chunk);
     cnt_mid[wt] = (int32_t)((nmid + p.chunk - 1) / p.chunk);
     cnt_edge[wt] = (int32_t)((nedge + p.chunk - 1) / p.chunk);
-    cnt_centre[wt] = (int32_t)((ncen + p.chunk - 1) / p.chunk);
+    cnt_centre[wt] = (int32_t)((ncen + p.chunk_centre - 1) / p.chunk_centre);
+    cnt_lane[wt] = (int32_t)((ncen + p.chunk_lane - 1) / p.chunk_lane);
     cnt_near[wt] = (int32_t)((nnear + p.chunk - 1) / p.chunk);
     if (nfar) atomicAdd(&st->pairs_far, (unsigned long long)nfar * nb);
     if (nmid) atomicAdd(&st->pairs_mid, (unsigned long long)nmid * nb);
