@@ -253,6 +253,115 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def _kernel_flops(st):
+    """Algorithmic FLOPs per accumulation kernel (FLOPs of the formula evaluated, per evaluation the
+    definition or the node scheme requires; masked-out slots and idle lanes count nothing) -> {phase: (kernel, flops)}."""
+    core = st["n_evals_core"]
+    n_gh4 = core - st["n_evals_gh6"] - st["n_evals_trap"]
+    n_trap = st["n_evals_trap"] - st["n_evals_gh10"]
+    g10_row = st["n_evals_gh10_row"]
+    g10_lane = st["n_evals_gh10"] - g10_row
+    kb = st["bins_per_lane"]
+    return {
+        "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * 8),
+        "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
+        "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
+        # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end
+        "edge": (f"edge_kernel<{kb}> + edge_node_kernel", FLOP["mid"] * (0.5 * st["n_pairs_edge"] + 8 * st["n_pairs_edge_node"])),
+        # line centres, rows: two-term outside the core, Gauss-Hermite 4 / 6 rings, the 10-point class of wide lines
+        "centre": (f"centre_row_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
+                   + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * g10_row),
+        # line centres, innermost bins: trapezoid rule with pole term (y < 2), 10-point rule of narrow lines
+        "lane": (f"centre_lane_kernel<{kb}>", FLOP["gh10"] * g10_lane + FLOP["trap"] * n_trap),
+    }
+
+
+def _timed(op, dl, cut, steps, warmup, flush, barrier=None):
+    """warmup untimed + `steps` timed hk_compute calls -> (per-step ms list, mean phase ms, stats)."""
+    k = torch.empty(op.N, dtype=torch.float64, device="cuda")
+    for _ in range(max(warmup, 0)):
+        if flush is not None:
+            flush.fill_(1)
+        op.compute(dl, cut, out=k)
+    torch.cuda.synchronize()
+    if barrier is not None:
+        barrier()
+    phases = {p: 0.0 for p in PHASE_NAMES}
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps)]
+    for i in range(steps):
+        if flush is not None:
+            flush.fill_(1)
+        ev[2 * i].record()
+        op.compute(dl, cut, out=k)
+        ev[2 * i + 1].record()
+        for p, v in op.phase_ms().items():                   # CUDA events recorded by the library on this stream
+            phases[p] += v
+    torch.cuda.synchronize()
+    if barrier is not None:
+        barrier()
+    step_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(steps)]
+    for p in phases:
+        phases[p] /= steps
+    return step_ms, phases, op.stats(), k
+
+
+PHASE_NAMES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "lane", "near", "down")
+
+
+def _roofline_kernels(st, phases, peak_nominal):
+    kflops = _kernel_flops(st)
+    kernels = {}
+    for ph, (name, fl) in kflops.items():
+        ms = phases[ph]
+        kernels[ph] = {"kernel": name, "ms": ms, "algorithmic_gflop": fl / 1e9,
+                       "tflops": fl / (ms * 1e-3) / 1e12 if ms > 0 else 0.0,
+                       "frac_of_nominal": (fl / (ms * 1e-3) / 1e12 / peak_nominal) if ms > 0 else 0.0}
+    acc_ms = sum(phases[k] for k in kflops)
+    acc_fl = sum(fl for _, fl in kflops.values())
+    allk = {"ms": acc_ms, "tflops": acc_fl / (acc_ms * 1e-3) / 1e12 if acc_ms > 0 else 0.0,
+            "frac_of_nominal": acc_fl / (acc_ms * 1e-3) / 1e12 / peak_nominal if acc_ms > 0 else 0.0}
+    return kernels, allk
+
+
+def _ncu_onepass(kernel_prefix):
+    """Per-launch DRAM traffic and executed FP32 work of a kernel from the committed one-pass ncu capture of this
+    command at the full workload size (profiles/r02_onepass_config4.csv; profiles/r02_onepass_config4.md states the
+    command).  -> dict or None."""
+    path = os.path.join(ROOT, "profiles", "r02_onepass_config4.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    rows = {}
+    try:
+        with open(path, newline="") as f:
+            rd = csv.reader(l for l in f if l.startswith('"'))
+            hdr = next(rd)
+            ix = {h: i for i, h in enumerate(hdr)}
+            for r in rd:
+                if len(r) != len(hdr) or not r[ix["ID"]].isdigit():
+                    continue
+                name = r[ix["Kernel Name"]]
+                if not name.startswith(kernel_prefix):
+                    continue
+                v = float(r[ix["Metric Value"]].replace(",", ""))
+                unit = r[ix["Metric Unit"]]
+                scale = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12, "us": 1e-6, "ms": 1e-3, "ns": 1e-9,
+                         "msecond": 1e-3, "usecond": 1e-6, "nsecond": 1e-9, "second": 1.0}.get(unit, 1.0)
+                rows.setdefault(r[ix["ID"]], {})[r[ix["Metric Name"]]] = v * scale
+    except Exception:
+        return None
+    if not rows:
+        return None
+    n = len(rows)
+    mean = lambda key: sum(d.get(key, 0.0) for d in rows.values()) / n
+    g = lambda op: mean(f"smsp__sass_thread_inst_executed_op_{op}_pred_on.sum")
+    return {"launches": n, "dram_bytes": mean("dram__bytes_read.sum") + mean("dram__bytes_write.sum"),
+            "seconds": mean("gpu__time_duration.sum"),
+            "fp32_flop_executed": 2.0 * g("ffma") + g("fadd") + g("fmul"),
+            "issue_active_pct": mean("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+            "file": "profiles/r02_onepass_config4.csv"}
+
+
 def run_ours(args):
     from paper_2101_02005_b200 import binding as B       # raises if libhk.so is missing: no CPU fallback
 
@@ -274,20 +383,10 @@ def run_ours(args):
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
     op.set_tile_bins(args.tile_bins)
     op.set_debug_mode(args.mode)
-    k = torch.empty(op.N, dtype=torch.float64, device="cuda")
     input_bytes = 6 * 8 * n
     flush = None
     if input_bytes < 256e6:                                  # inputs smaller than ~2x L2: flush L2 between iterations
         flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
-
-    def step():
-        if flush is not None:
-            flush.fill_(1)
-        op.compute(dl, cut, out=k)
-
-    for _ in range(max(args.warmup, 0)):
-        step()
-    torch.cuda.synchronize()
 
     def barrier():
         torch.cuda.synchronize()
@@ -300,27 +399,13 @@ def run_ours(args):
         gpu_id = gpu_id if gpu_id.startswith("GPU-") else "GPU-" + gpu_id
     except Exception:
         gpu_id = str(local)
+    # warm-up first, then the clock sampler brackets the timed region only
+    _timed(op, dl, cut, 0, args.warmup, flush)
     sampler = ClockSampler(gpu_id) if rank == 0 else None
-    phases = {p: 0.0 for p in B.PHASES}
-    step_ms = []
-    barrier()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps)]
-    for i in range(args.steps):
-        if flush is not None:
-            flush.fill_(1)
-        ev[2 * i].record()
-        op.compute(dl, cut, out=k)
-        ev[2 * i + 1].record()
-        for p, v in op.phase_ms().items():                   # CUDA events recorded by the library on this stream
-            phases[p] += v
-    barrier()
+    step_ms, phases, st, k = _timed(op, dl, cut, args.steps, 0, flush, barrier)
     clocks = sampler.stop() if sampler else None
-    st = op.stats()
-    step_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(args.steps)]
     total_ms = max_over_ranks(float(sum(step_ms)), dist, "cuda")
     value = replicas_value(n, args.steps, world, total_ms)
-    for p in phases:
-        phases[p] /= args.steps
 
     if rank != 0:
         if dist is not None:
@@ -333,42 +418,33 @@ def run_ours(args):
     n_sm = props.multi_processor_count
     sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0)
     peak_nominal = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12     # TFLOP/s
-    probe_flops, _ = B.probe_fp32_peak(packed=True, iters=20000)
-    # per accumulation kernel: algorithmic FLOPs (FLOPs of the formula evaluated, per evaluation the
-    # definition or the node scheme requires; masked-out slots and idle lanes count nothing) / CUDA-event time
-    core = st["n_evals_core"]
-    n_gh4 = core - st["n_evals_gh6"] - st["n_evals_trap"]
-    n_trap = st["n_evals_trap"] - st["n_evals_gh10"]
-    kb = st["bins_per_lane"]
-    kflops = {
-        "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * 8),
-        "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
-        "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
-        # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end
-        "edge": (f"edge_kernel<{kb}> + edge_node_kernel", FLOP["mid"] * (0.5 * st["n_pairs_edge"] + 8 * st["n_pairs_edge_node"])),
-        "centre": (f"centre_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
-                   + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * st["n_evals_gh10"] + FLOP["trap"] * n_trap),
-    }
-    kernels = {}
-    for ph, (name, fl) in kflops.items():
-        ms = phases[ph]
-        kernels[ph] = {"kernel": name, "ms": ms, "algorithmic_gflop": fl / 1e9,
-                       "tflops": fl / (ms * 1e-3) / 1e12 if ms > 0 else 0.0,
-                       "frac_of_nominal": (fl / (ms * 1e-3) / 1e12 / peak_nominal) if ms > 0 else 0.0}
-    dom = max(kflops, key=lambda k: phases[k])
+    # the FP32 pipe measured by the library's own probes (>= 200 ms each), with the SM clock read inside the kernel
+    probes = {}
+    for kind in B.PROBE_KINDS:
+        ops, mhz, ms = B.probe_fp32_ops(kind, iters=60000 if kind == "mufu_rcp" else 250000)
+        probes[kind] = {"lane_ops_per_clk_per_sm": ops / (mhz * 1e6) / n_sm if mhz > 0 else None, "sm_mhz": mhz, "ms": ms,
+                        "tera_ops_per_s": ops / 1e12}
+    probe_flops = 2.0 * probes["ffma2"]["tera_ops_per_s"] * 1e12
+    kernels, allk = _roofline_kernels(st, phases, peak_nominal)
+    dom = max(kernels, key=lambda kk: phases[kk])
     achieved = kernels[dom]["tflops"]
-    acc_ms = sum(phases[k] for k in kflops)
-    acc_fl = sum(fl for _, fl in kflops.values())
     roofline = {"bound": "alu", "kernel": kernels[dom]["kernel"], "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                 "frac": achieved / peak_nominal if peak_nominal else None, "traffic": None,
                 "peak_kind": f"nominal FP32: {n_sm} SMs x {FP32_LANES_PER_SM} lanes x 2 FLOP x {sm_max:g} MHz (DESIGN.md 7)",
                 "peak_probe_ffma2": probe_flops / 1e12, "frac_of_probe": achieved / (probe_flops / 1e12),
+                "probes": probes,
                 "ms_per_launch": phases[dom], "share_of_step": phases[dom] / (total_ms / args.steps),
-                "flop_per_eval": FLOP, "kernels": kernels,
-                "all_accumulation_kernels": {"ms": acc_ms, "tflops": acc_fl / (acc_ms * 1e-3) / 1e12 if acc_ms > 0 else 0.0,
-                                             "frac_of_nominal": acc_fl / (acc_ms * 1e-3) / 1e12 / peak_nominal if acc_ms > 0 else 0.0},
+                "flop_per_eval": FLOP, "kernels": kernels, "all_accumulation_kernels": allk,
                 "hbm_preprocess_gbs": (input_bytes + 40.0 * n) / (phases["preprocess"] * 1e-3) / 1e9 if phases["preprocess"] > 0 else None,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_kind": peaks_kind}
+    if cfg == 4 and n == c["n"] and args.mode == 0 and args.tile_bins == 0:
+        one = _ncu_onepass(kernels[dom]["kernel"].split("<")[0])
+        if one is not None:
+            # measure (b) of SURVEY 8(d): executed FP32 thread instructions (FFMA x 2 + FADD + FMUL) over the ncu
+            # duration of the same launch; traffic = DRAM bytes of that launch
+            roofline["traffic"] = one["dram_bytes"]
+            roofline["frac_issue"] = one["fp32_flop_executed"] / one["seconds"] / 1e12 / peak_nominal if one["seconds"] > 0 else None
+            roofline["ncu_onepass"] = one
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -379,13 +455,64 @@ def run_ours(args):
            "voigt_evals_per_s": world * st["n_evals"] * args.steps / (total_ms * 1e-3),
            "evals_per_step": st["n_evals"],
            "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"],
-                               "core_gh6": st["n_evals_gh6"], "core_trap": st["n_evals_trap"]},
+                               "core_gh6": st["n_evals_gh6"], "core_trap": st["n_evals_trap"], "core_gh10": st["n_evals_gh10"],
+                               "core_gh10_row": st["n_evals_gh10_row"]},
            "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
                                "edge": st["n_pairs_edge"], "edge_node_ends": st["n_pairs_edge_node"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
-           "bins_per_lane": st["bins_per_lane"],
+           "bins_per_lane": st["bins_per_lane"], "sorted_input": st["n_unsorted"] == 0,
            "phase_ms": phases, "step_ms": step_ms, "roofline": roofline, "clocks": clocks,
            "gpu_launches": int(st["n_launches"]) * args.steps,
            "paper_context": "paper: ~1e7 lines/s (BT2, 0.01 cm^-1, cut 25, RTX 2080 Ti, incl. read; PAPER.md L7, Table 8 L778) -- other hardware and cut"}
+
+    # ---- the other configs of BASELINE.json and the batched-conditions path, under the same clock (N = 1) -------------
+    if not args.no_other_configs and world == 1 and cfg == 4 and args.mode == 0:
+        others = {}
+        for oc in (1, 2, 3, 5):
+            cc = W.CONFIGS[oc]
+            n_o = cc["n"] if not args.n_lines else min(cc["n"], n)
+            same = oc == 3 and n_o == n                       # configs 3 and 4 share the line arrays
+            dl_o = dl if same else W.make_lines(oc, n=n_o, seed=0, device="cuda")
+            cond_o = W.conditions(oc)
+            op_o = B.Opacity(*cc["grid"])
+            op_o.set_conditions(cond_o["T"], cond_o["P_atm"], cond_o["mass_amu"], cond_o["Q"])
+            fl_o = None
+            if 48 * n_o < 256e6:
+                fl_o = flush if flush is not None else torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+                flush = fl_o
+            sm_o, ph_o, st_o, _ = _timed(op_o, dl_o, cc["cut"], 5, 3, fl_o)
+            ms_o = float(np.median(sm_o))
+            _, allk_o = _roofline_kernels(st_o, ph_o, peak_nominal)
+            others[str(oc)] = {"workload": _workload_name(oc, n_o), "ms_per_step": ms_o, "lines_per_s": n_o / (ms_o * 1e-3),
+                               "voigt_evals_per_s": st_o["n_evals"] / (ms_o * 1e-3), "phase_ms": ph_o,
+                               "roofline_frac_all_kernels": allk_o["frac_of_nominal"], "steps": 5, "warmup": 3,
+                               "bins_per_lane": st_o["bins_per_lane"], "sorted_input": st_o["n_unsorted"] == 0}
+            if oc == 2:
+                # NEXT-1: ten pressure points on the resident config-2 list in one hk_compute_batch (Table 8
+                # L781-786), against the same ten points as separate hk_compute calls
+                Ps = [float(x) for x in np.logspace(-3, 1, 10)]
+                Ts, Qs = [cond_o["T"]] * 10, [cond_o["Q"]] * 10
+                kb_out = torch.empty((10, op_o.N), dtype=torch.float64, device="cuda")
+                e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+                op_o.compute_batch(dl_o, cc["cut"], Ts, Ps, Qs, out=kb_out)           # warm-up
+                torch.cuda.synchronize()
+                e0.record()
+                op_o.compute_batch(dl_o, cc["cut"], Ts, Ps, Qs, out=kb_out)
+                e1.record()
+                for ci in range(10):
+                    op_o.set_conditions(Ts[ci], Ps[ci], cond_o["mass_amu"], Qs[ci])
+                    op_o.compute(dl_o, cc["cut"], out=kb_out[ci])
+                e2.record()
+                torch.cuda.synchronize()
+                out["batch"] = {"workload": _workload_name(2, n_o) + ", 10 pressure points 1e-3..10 atm", "n_cond": 10,
+                                "ms_total": e0.elapsed_time(e1), "ms_per_cond": e0.elapsed_time(e1) / 10,
+                                "ms_single": e1.elapsed_time(e2) / 10, "ms_separate_total": e1.elapsed_time(e2)}
+                del kb_out
+            op_o.close()
+            del op_o
+            if not same:
+                del dl_o
+            torch.cuda.empty_cache()
+        out["other_configs"] = others
 
     # ---- end to end through the host-buffer entry of the C ABI --------------------------
     if not args.no_e2e and world == 1:
@@ -445,6 +572,7 @@ def main():
     ap.add_argument("--tile-bins", type=int, default=0, choices=[0, 2, 4, 8], help="bins per lane of a level-0 tile (0: library default)")
     ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2, 3], help="hk_set_debug_mode (3: direct evaluation only)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip configs 1, 2, 3, 5 and the batch leg after the headline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

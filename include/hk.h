@@ -63,9 +63,9 @@ typedef struct {
     int64_t n_evals;       /* sum over lines of (i_hi - i_lo + 1): Voigt evaluations */
     int64_t n_evals_far;   /* of those, |z|^2 >= HK_Z1 (1-term asymptotic = Lorentzian) */
     int64_t n_evals_mid;   /* HK_Z2 <= |z|^2 < HK_Z1 (2-term asymptotic) */
-    int64_t n_evals_core;  /* |z|^2 < HK_Z2: 4-point Gauss-Hermite (>= HK_Z4), 6-point (>= HK_Z3), trapezoid + pole term below */
-    int64_t n_evals_gh6;   /* of n_evals_core: HK_Z3 <= |z|^2 < HK_Z4 */
-    int64_t n_evals_trap;  /* of n_evals_core: |z|^2 < HK_Z3 (trapezoid, or 10-point Gauss-Hermite when y >= 2) */
+    int64_t n_evals_core;  /* |z|^2 < HK_Z2: 4-point Gauss-Hermite (outer ring), 6-point, trapezoid + pole term innermost */
+    int64_t n_evals_gh6;   /* of n_evals_core: the 6-point ring (HK_Z3 <= |z|^2 < HK_Z4 at small y; see HK_Z4 for its dependence on y) */
+    int64_t n_evals_trap;  /* of n_evals_core: |z|^2 < HK_Z3 and y < 3 (trapezoid, or 10-point Gauss-Hermite when y >= 2) */
     int64_t n_units_far;   /* (tile, line-chunk) work units run by the far kernel */
     int64_t n_units_mid;   /* ... by the mid kernel */
     int64_t n_units_near;  /* ... by the near/edge kernel */
@@ -82,6 +82,11 @@ typedef struct {
     int64_t n_evals_gh10;  /* of n_evals_trap: lines with y >= 2, evaluated by the 10-point Gauss-Hermite rule */
     int64_t n_pairs_edge_node; /* (line, extent end) pairs evaluated at the nodes of their edge tile (per-bin accumulators) */
     int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
+    int64_t n_plinth_illcond; /* plinth removal: lines with V(cut) > V(0) / HK_PLINTH_RATIO, whose difference V - V(cut) is
+                                 ill-conditioned in fp32 (see hk_set_plinth: 0 means the subtracted result meets the tolerance) */
+    int64_t n_evals_gh10_row; /* of n_evals_gh10: evaluated by the row kernel (lines at least 0.85 bins wide per 64 bins of tile); the rest by the lane kernel */
+    int64_t n_unsorted;    /* adjacent pairs of the input list out of centre-bin order (0: the list arrived sorted and the
+                              radix sort was skipped on the device) */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */
     int32_t sort_bits;     /* radix-sort key width used */
     int32_t bins_per_lane; /* tile geometry used: a level-0 tile is 32 x this many bins */
@@ -96,8 +101,10 @@ enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, H
 /* Region thresholds on |z|^2 = x^2 + y^2 used by the fp32 evaluator. */
 #define HK_Z1 90000.0f /* |z| >= 300: one asymptotic term, relative error <= 1.7e-5 */
 #define HK_Z2 625.0f   /* |z| >= 25 : two asymptotic terms, relative error <= 1.0e-5 */
-#define HK_Z4 64.0f    /* 8 <= |z| < 25: 4-point Gauss-Hermite rational form, <= 1.0e-6; below: 6-point, <= 7.7e-6 */
-#define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3): trapezoid rule + pole term, <= 2e-6; 10-point Gauss-Hermite when y >= 2, <= 2.7e-6 */
+#define HK_Z4 49.0f    /* 7 <= |z| < 25: 4-point Gauss-Hermite rational form, <= 3e-6; below: 6-point.  The rings shrink as y grows
+                          (the pole moves away from the real axis): 4 points from |z|^2 >= 36 for y >= 1.5, >= 30.25 for y >= 3, and
+                          on the whole core for y >= 4.5; 6 points on the whole core for y >= 3 (hk_device.cuh: z4_for, z3_for) */
+#define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3) and y < 3: trapezoid rule + pole term, <= 2e-6; 10-point Gauss-Hermite when y >= 2, <= 2.7e-6 */
 #define HK_NODES 8     /* Chebyshev nodes per tile of the separated-tile evaluation */
 
 /* Grid: bin i is the POINT nu_i = numin + i*dnu (R8, R9).  HK_EINVAL if dnu <= 0,
@@ -146,14 +153,27 @@ int hk_set_cut_mode(hk_ctx* ctx, int mode);
 /* Plinth removal (section 2.1.1): on != 0 subtracts from every bin of a line's extent that line's own value
  * at the cutting length position, S V(nu0 +- cut) (needed with continua that already hold the plinths, e.g. CKD).
  * Off by default; no effect on uncut computations.  Changes hk_workspace_bytes (+ 8 B per bin): set it before the
- * workspace is sized.  Applies to hk_compute, hk_accumulate, hk_compute_batch and hk_compute_host. */
+ * workspace is sized.  Applies to hk_compute, hk_accumulate, hk_compute_batch and hk_compute_host.
+ * Accuracy contract: S (V - V(cut)) is a difference of two fp32 evaluations, each good to a few 1e-7 (rounding) to
+ * 1e-6 (inside the core) of ITSELF.  While every line's value at its cutting length is small against its peak,
+ * V(cut) <= V(0) / HK_PLINTH_RATIO -- the normal use: a cut of many half-widths -- the SUBTRACTED opacity meets the
+ * tolerance of the library (1e-4 per bin relative to the result, 1e-8 max(k) below that: the bins next to the extent's
+ * ends, where the difference vanishes, fall under the absolute branch).  A line that does not is counted in
+ * hk_stats.n_plinth_illcond (cut inside the line's core, or shorter than ~23 Lorentz half-widths); in the bins such
+ * lines dominate the result is then good to 1e-4 of the opacity BEFORE removal only -- no fp32 evaluation can do better
+ * -- and a caller who needs more must use a longer cut. */
+#define HK_PLINTH_RATIO 512.0
 int hk_set_plinth(hk_ctx* ctx, int on);
 
 /* Device scratch the caller must provide for hk_compute with up to n_lines lines. */
 size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines);
 int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
 
-/* Enqueue the whole hot path on `stream` (a cudaStream_t passed as void*; NULL is
+/* Reproducibility: bins receive their partial sums through fp64 atomic adds whose order is not fixed, so two runs of
+ * the same call agree to the rounding of an fp64 sum (~1e-16 relative), not bit for bit (the paper notes the same of
+ * its summation order, L666).  Integer outputs (extents, counts) are exact and reproducible.
+ *
+ * Enqueue the whole hot path on `stream` (a cudaStream_t passed as void*; NULL is
  * the legacy default stream): preprocess -> sort by centre bin -> tile ranges -> node, far, mid, extent-end,
  * centre and near accumulation kernels -> interpolation of the node sums (-> plinth removal) -> k in out_k_dev.
  * out_k_dev (N doubles) is OVERWRITTEN.  cut_cm > 0 and finite: cutting length from the centre (cm^-1, or a
@@ -238,9 +258,15 @@ size_t hk_workspace_bytes_host(const hk_ctx* ctx, int64_t n_lines, int64_t block
 int hk_compute_host(hk_ctx* ctx, const hk_lines* host_lines, int64_t n_lines, double cut_cm,
                     double* out_k_host, int64_t block_lines, void* stream);
 
-/* Integer extents of the lines of the LAST hk_compute, in the caller's line order
+/* Integer extents of the lines of the LAST compute, in the caller's line order
  * (int32 DEVICE arrays of n_lines; skipped / off-grid lines get ilo = 0, ihi = -1,
- * jc as computed (0 for skipped)).  Any pointer may be NULL.  Synchronises. */
+ * jc as computed (0 for skipped)).  Any pointer may be NULL.  Synchronises.
+ * When n_lines equals that of the last compute and it ran as one pass (hk_compute / hk_accumulate / hk_compute_hitran
+ * with a fixed cut or none, a single-block hk_compute_host) the values are the ones that compute WROTE -- read from its
+ * per-line records, shifted centres and all -- and `lines` is not read (may be NULL).  Otherwise (width-relative
+ * cutting lengths, several blocks: the record buffer held one pass at a time) they are recomputed from `lines` with
+ * the conditions, cut and cut mode of the last compute; HK_ESTATE in that case after hk_compute_hitran (use
+ * hk_get_line_params_hitran). */
 int hk_get_extents(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, int32_t* ilo_dev,
                    int32_t* ihi_dev, int32_t* jc_dev, void* stream);
 
@@ -257,10 +283,18 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out);
  * HK_PH_COUNT floats.  Synchronises. */
 int hk_get_phase_ms(hk_ctx* ctx, float* out_ms);
 
-/* FP32 issue-rate probe for the roofline denominator ("measure an FFMA
- * peak"): runs a register-resident chain of independent packed FMAs on every SM and
- * returns the achieved FLOP/s (2 per FMA) in *flops_out (HOST) and the kernel time.
- * packed != 0 uses fma.rn.f32x2 (FFMA2), else scalar FFMA. */
+/* FP32 issue-rate probes for the roofline denominator ("measure an FFMA peak and the clock actually
+ * held"): 16 independent register-resident chains per thread on every SM (4 CTAs x 512 threads per SM), one
+ * instruction kind per launch:
+ *   kind 0  FFMA2 (fma.rn.f32x2), three distinct register operands      3  FADD2 (add.rn.f32x2)
+ *        1  scalar FFMA, three register operands                        4  FMUL2 (mul.rn.f32x2)
+ *        2  FFMA2 with scalar multiplier and addend (broadcast form)    5  MUFU.RCP (rcp.approx.ftz.f32)
+ * *lane_ops_per_s (HOST): fp32 lane operations per second (an FMA is one operation: x2 for FLOP/s);
+ * *sm_clock_mhz (HOST, may be NULL): SM cycles / nanoseconds measured INSIDE the kernel (clock64 / globaltimer), i.e.
+ * the SM clock actually held during the probe; *ms_out (may be NULL): kernel time.  Run it with iters large enough
+ * for >= 200 ms when the point is the sustained clock.  Synchronises.
+ * hk_probe_fp32_peak(packed, ...) = 2 x the kind-0 (packed != 0) or kind-1 rate, in FLOP/s. */
+int hk_probe_fp32_ops(int kind, int iters, double* lane_ops_per_s, double* sm_clock_mhz, float* ms_out, void* stream);
 int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, void* stream);
 
 /* Accuracy probe for the shipped fp32 evaluator (the counterpart of the paper's

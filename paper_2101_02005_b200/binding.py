@@ -20,12 +20,12 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 HK_OK, HK_EINVAL, HK_ESTATE, HK_ENOSPC, HK_ECUDA, HK_ENOMEM = 0, -1, -2, -3, -4, -5
-HK_Z1, HK_Z2, HK_Z4, HK_Z3 = 90000.0, 625.0, 64.0, 30.25
+HK_Z1, HK_Z2, HK_Z4, HK_Z3 = 90000.0, 625.0, 49.0, 30.25
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
-           "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak",
+           "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak", "hk_probe_fp32_ops",
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode", "hk_compute_bands",
            "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
            "hk_last_cuda_error", "hk_strerror")
@@ -48,7 +48,8 @@ class hk_stats(C.Structure):
                                          "n_evals_mid", "n_evals_core", "n_evals_gh6", "n_evals_trap", "n_units_far", "n_units_mid", "n_units_near",
                                          "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_units_edge",
                                          "n_units_centre", "n_pairs_edge", "n_pairs_centre", "n_pairs_node",
-                                         "n_bins_node", "n_evals_gh10", "n_pairs_edge_node", "n_launches")] + \
+                                         "n_bins_node", "n_evals_gh10", "n_pairs_edge_node", "n_launches",
+                                         "n_plinth_illcond", "n_evals_gh10_row", "n_unsorted")] + \
                [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("n_levels", C.c_int32)]
 
 
@@ -77,6 +78,8 @@ _lib.hk_workspace_bytes_host.restype = C.c_size_t
 _lib.hk_compute_host.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _i64, _vp]
 _lib.hk_get_phase_ms.argtypes = [_vp, C.POINTER(C.c_float)]
 _lib.hk_probe_fp32_peak.argtypes = [C.c_int, C.c_int, C.POINTER(_d), C.POINTER(C.c_float), _vp]
+_lib.hk_probe_fp32_ops.argtypes = [C.c_int, C.c_int, C.POINTER(_d), C.POINTER(_d), C.POINTER(C.c_float), _vp]
+_lib.hk_probe_fp32_ops.restype = C.c_int
 _lib.hk_get_extents.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _vp, _vp]
 _lib.hk_get_line_params.argtypes = [_vp, C.POINTER(hk_lines), _i64, _vp, _vp, _vp, _vp]
 _lib.hk_get_stats.argtypes = [_vp, C.POINTER(hk_stats)]
@@ -290,10 +293,16 @@ class Opacity:
         self._check(_lib.hk_get_phase_ms(self._ctx, arr), "hk_get_phase_ms")
         return {k: float(arr[i]) for i, k in enumerate(PHASES)}
 
-    def extents(self, lines, stream=None):
-        ls, n = _lines_struct(lines)
-        ilo, ihi, jc = (torch.empty(n, dtype=torch.int32, device="cuda") for _ in range(3))
-        self._check(_lib.hk_get_extents(self._ctx, C.byref(ls), n, ilo.data_ptr(), ihi.data_ptr(), jc.data_ptr(),
+    def extents(self, lines=None, n=None, stream=None):
+        """hk_get_extents: (ilo, ihi, jc) of the last compute.  `lines` may be None (pass n = the last compute's line
+        count) when that compute ran as one pass: the library then returns what it wrote."""
+        if lines is not None:
+            ls, n = _lines_struct(lines)
+            lp = C.byref(ls)
+        else:
+            lp = None
+        ilo, ihi, jc = (torch.empty(int(n), dtype=torch.int32, device="cuda") for _ in range(3))
+        self._check(_lib.hk_get_extents(self._ctx, lp, int(n), ilo.data_ptr(), ihi.data_ptr(), jc.data_ptr(),
                                         _stream_ptr(stream)), "hk_get_extents")
         return ilo, ihi, jc
 
@@ -326,6 +335,19 @@ def compute_bands(ops, lines, cut, outs=None, stream=None):
     if st != HK_OK:
         raise HKError(st, "hk_compute_bands")
     return outs
+
+
+PROBE_KINDS = ("ffma2", "ffma", "ffma2_bcast", "fadd2", "fmul2", "mufu_rcp")
+
+
+def probe_fp32_ops(kind, iters=4096, stream=None):
+    """hk_probe_fp32_ops -> (fp32 lane operations per second, SM clock in MHz measured inside the kernel, ms)."""
+    code = PROBE_KINDS.index(kind) if isinstance(kind, str) else int(kind)
+    ops, mhz, ms = _d(0.0), _d(0.0), C.c_float(0.0)
+    st = _lib.hk_probe_fp32_ops(code, iters, C.byref(ops), C.byref(mhz), C.byref(ms), _stream_ptr(stream))
+    if st != HK_OK:
+        raise HKError(st, "hk_probe_fp32_ops")
+    return ops.value, mhz.value, ms.value
 
 
 def probe_fp32_peak(packed=True, iters=4096, stream=None):

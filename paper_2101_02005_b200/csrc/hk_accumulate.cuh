@@ -811,6 +811,7 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
 {
     constexpr int M = kP / 2;
     __shared__ int32_t s_nact;
+    apply_shift_bound(p, a.st);
     if (threadIdx.x == 0) s_nact = lower_bound_key(keys, n, (int64_t)p.ksent);
     __syncthreads();
     const int32_t n_act = s_nact;
@@ -971,6 +972,7 @@ __global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const 
     // sorted records), which a width-relative cutting length needs, and the unscaled fp64 amplitude
     const int lane = threadIdx.x & 31;
     const int64_t n_round = (n + 31) & ~31LL;
+    unsigned long long in_core = 0;        // lines whose value at the cut is not small against their peak (hk_stats.n_plinth_illcond)
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
         int64_t ilo = 0, ihi = -1;
         double pl = 0.0;
@@ -986,26 +988,37 @@ __global__ void __launch_bounds__(256) plinth_kernel(Params p, AccArgs a, const 
                 const double G2 = gauss ? 0.0 : G2t;
                 const double q = cb * cb + G2;
                 const double c = r.cK * sqrt(G2 * a2) * 0.56418958354775628695;        // Lorentz amplitude, as gather_kernel
+                double peak = 0.0;                                                      // the line's value at its centre
                 if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) {
                     if (q < (double)binned_ql(r.a2)) pl = r.cK * (double)binned_K((float)cb, 0.f, 0.f, rsqrtf(r.a2));
+                    peak = r.cK * (double)binned_K(0.f, 0.f, 0.f, rsqrtf(r.a2));
                 } else if (p.profile == HK_PROFILE_LORENTZ) {
                     pl = c / q;
-                } else if (q >= (double)HK_Z2 * a2) {
-                    // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q)
-                    pl = c / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
+                    peak = c / G2;
                 } else {
+                    // two asymptotic terms in bin units: c/q (1 + (1.5 a^2 - 2 a^2 G^2/q)/q); inside the core the fp32 evaluator
                     const float inv_a = rsqrtf(r.a2);
-                    const float x = (float)cb * inv_a, y = sqrtf((float)G2) * inv_a;
-                    // (a pure Gaussian through the same scaled fp32 evaluation as its bins, so that both vanish together)
-                    pl = y == 0.f ? (double)gauss_term((float)scalbn(r.cK, a.st->scale_exp), x) * scalbn(1.0, -a.st->scale_exp)
-                                  : r.cK * (double)core_any_K(x, y, nullptr);
+                    const float y = sqrtf((float)G2) * inv_a;
+                    if (q >= (double)HK_Z2 * a2) pl = c / q * (1.0 + (1.5 * a2 - 2.0 * a2 * G2 / q) / q);
+                    else {
+                        const float x = (float)cb * inv_a;
+                        // (a pure Gaussian through the same scaled fp32 evaluation as its bins, so that both vanish together)
+                        pl = y == 0.f ? (double)gauss_term((float)scalbn(r.cK, a.st->scale_exp), x) * scalbn(1.0, -a.st->scale_exp)
+                                      : r.cK * (double)core_any_K(x, y, nullptr);
+                    }
+                    peak = G2 >= (double)HK_Z2 * a2 ? c / G2 * (1.0 - 0.5 * a2 / G2) : y == 0.f ? r.cK : r.cK * (double)core_any_K(0.f, y, nullptr);
                 }
+                // S (V - V(cut)) is ill-conditioned in fp32 when V(cut) is not small against the peak (hk.h, hk_set_plinth)
+                if (pl * (double)HK_PLINTH_RATIO > peak) ++in_core;
             }
         }
         const bool live = ihi >= ilo;
         warp_add_scalar_by_bin(a.plinth_acc, live ? ilo : -1, -pl, lane);
         warp_add_scalar_by_bin(a.plinth_acc, live ? ihi + 1 : -1, pl, lane);
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) in_core += __shfl_xor_sync(0xffffffffu, in_core, o);
+    if (lane == 0 && in_core) atomicAdd(&a.st->n_plinth_illcond, in_core);
 }
 
 __global__ void __launch_bounds__(256) plinth_apply_kernel(AccArgs a)
@@ -1043,27 +1056,42 @@ __global__ void __launch_bounds__(256) probe_kernel(const float* __restrict__ x,
 }
 
 // ---------------------------------------------------------------------------------------
-// FP32 issue-rate probe (roofline denominator): 32 independent FMA chains per thread
+// FP32 issue-rate probes (roofline denominator): 16 independent register-resident chains per thread.
+// kind 0: FFMA2 with three distinct register operands   1: scalar FFMA, three register operands
+//      2: FFMA2 whose multiplier and addend are scalars broadcast to both halves (the row kernels' form)
+//      3: FADD2   4: FMUL2   5: MUFU.RCP (one per chain step)
+// clk[0] = SM cycles (clock64) and clk[1] = nanoseconds (globaltimer) block 0 spent in the loop: their ratio is the SM
+// clock actually held while the probe ran.
 // ---------------------------------------------------------------------------------------
-template <bool kPacked>
-__global__ void __launch_bounds__(512) fp32_peak_kernel(int iters, float* __restrict__ sink)
+template <int kKind>
+__global__ void __launch_bounds__(512) fp32_probe_kernel(int iters, float* __restrict__ sink, long long* __restrict__ clk)
 {
     float2 acc[16];
 #pragma unroll
     for (int j = 0; j < 16; ++j) acc[j] = make_float2(1.0f + j + threadIdx.x * 1e-3f, 0.5f + j);
     const float2 a = make_float2(0.999999f, 1.000001f), b = make_float2(1e-7f, -1e-7f);
+    const long long t0 = clock64();
+    unsigned long long g0, g1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
 #pragma unroll 1
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-            if (kPacked) acc[j] = __ffma2_rn(acc[j], a, b);
-            else { acc[j].x = fmaf(acc[j].x, a.x, b.x); acc[j].y = fmaf(acc[j].y, a.y, b.y); }
+            if (kKind == 0) acc[j] = __ffma2_rn(acc[j], a, b);
+            else if (kKind == 1) { acc[j].x = fmaf(acc[j].x, a.x, b.x); acc[j].y = fmaf(acc[j].y, a.y, b.y); }
+            else if (kKind == 2) acc[j] = __ffma2_rn(acc[j], make_float2(a.x, a.x), make_float2(b.x, b.x));
+            else if (kKind == 3) acc[j] = __fadd2_rn(acc[j], b);
+            else if (kKind == 4) acc[j] = __fmul2_rn(acc[j], a);
+            else acc[j].x = rcp_approx(acc[j].x);
         }
     }
+    const long long t1 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
     float s = 0.f;
 #pragma unroll
     for (int j = 0; j < 16; ++j) s += acc[j].x + acc[j].y;
     if (s == 123.456f) *sink = s;
+    if (threadIdx.x == 0 && blockIdx.x == 0) { clk[0] = t1 - t0; clk[1] = (long long)(g1 - g0); }
 }
 
 }  // namespace hk

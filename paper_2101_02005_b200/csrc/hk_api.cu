@@ -48,8 +48,11 @@ struct hk_ctx {
     int last_profile;
     bool regions_done;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
-    bool host_totals;
-    int64_t tot_lines, tot_skipped, tot_off_grid, tot_evals;
+    bool host_totals;            // the counts of the last call are totals kept on the device (d_totals)
+    int64_t tot_lines;
+    DevTotals* d_totals;
+    bool last_multi;             // the last call ran several passes / blocks: recU holds the last one only
+    bool last_hitran;
     // phase events (recorded on the caller's stream) and the host-pipeline resources
     cudaEvent_t ev[HK_PH_COUNT + 1];
     cudaStream_t copy_stream;
@@ -61,7 +64,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, recC, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
+    size_t stats, totals, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, recC, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
     size_t edge_acc_bytes;   // 0: grid too large for the per-bin edge accumulators (direct edge kernel only)
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
@@ -105,6 +108,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
     L.stats = take(sizeof(DevStats));
+    L.totals = take(sizeof(DevTotals));      // (fixed offset: survives the per-block layouts of hk_compute_host)
     L.keys_in = take(nn * 4);
     L.keys_out = take(nn * 4);
     L.idx_in = take(nn * 4);
@@ -286,6 +290,17 @@ __global__ void __launch_bounds__(256) extents_kernel(Params p, const double* __
     }
 }
 
+__global__ void __launch_bounds__(256) extents_from_records_kernel(const RecU* __restrict__ rec, int64_t n, int32_t* ilo,
+                                                                   int32_t* ihi, int32_t* jc)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const RecU r = rec[i];
+        if (ilo) ilo[i] = r.ihi >= r.ilo ? r.ilo : 0;
+        if (ihi) ihi[i] = r.ihi >= r.ilo ? r.ihi : -1;
+        if (jc) jc[i] = r.jc;
+    }
+}
+
 bool lines_ok(const hk_lines* l)
 {
     return l && l->nu0 && l->A && l->g_up && l->E_low && l->gamma_ref && l->n_exp;
@@ -446,6 +461,9 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     if (zero_out) HK_CUDA(cudaMemsetAsync(out_k_dev, 0, (size_t)ctx->N * sizeof(double), stream));
     ctx->have_run = true;
     ctx->host_totals = false;
+    ctx->last_multi = false;
+    ctx->last_hitran = extra != nullptr;
+    ctx->d_totals = (DevTotals*)(ws + L.totals);
     ctx->last_n = n_lines;
     ctx->last_cut = cut_cm;
     ctx->last_stream = stream;
@@ -532,28 +550,32 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     const int grid = ctx->n_sm * 2;
     if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NODE + 1], stream));
-    auto launch = [&](auto kb_tag) {
+    // every CUDA call inside is checked: the first failure is returned and nothing more is enqueued
+    auto launch = [&](auto kb_tag) -> cudaError_t {
         constexpr int KB = decltype(kb_tag)::value;
+        cudaError_t e = cudaSuccess;
+#define HK_TRY(call) do { e = (call); if (e != cudaSuccess) return e; } while (0)
         if (p.mode != 1 && p.mode != 2) { interior_kernel<KB, false><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
-        cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream);
+        HK_TRY(cudaEventRecord(ctx->ev[HK_PH_FAR + 1], stream));
         if (p.mode != 1) { interior_kernel<KB, true><<<grid, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
-        cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream);
+        HK_TRY(cudaEventRecord(ctx->ev[HK_PH_MID + 1], stream));
         if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<ctx->n_sm * 4, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         if (use_edge_nodes) {
-            cudaMemsetAsync(edge_acc, 0, L.edge_acc_bytes, stream);
+            HK_TRY(cudaMemsetAsync(edge_acc, 0, L.edge_acc_bytes, stream));
             edge_node_kernel<<<ctx->n_sm * 4, kThreads, 0, stream>>>(p, a, keys_out, n);
             const int64_t nsc = 2 * ((ctx->N + lv.w0 - 1) / lv.w0) * kP;
             edge_scan_kernel<<<(int)((nsc + 255) / 256), 256, 0, stream>>>(a);
             edge_bins_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
             ctx->last_launches += 3;
         }
-        cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream);
+        HK_TRY(cudaGetLastError());
+        HK_TRY(cudaEventRecord(ctx->ev[HK_PH_EDGE + 1], stream));
         if (p.mode == 0 || p.mode == 3) {
             // rows (lanes own bins): nothing to do for the Gaussian profiles, whose records carry no Lorentz amplitude
             const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
             if (!gauss) { centre_row_kernel<KB><<<ctx->n_sm * kRowCtas, 32 * kRowWarps, 0, stream>>>(a); ++ctx->last_launches; }
         }
-        cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream);
+        HK_TRY(cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream));
         if (p.mode == 0 || p.mode == 3) {
             // innermost bins (lane <-> line): none for a pure Lorentzian.  Sparse lists (fewer than 256 lines per level-0
             // tile on average) run 2- or 1-warp CTAs, four or eight times as many: a work unit there is a handful of lines
@@ -572,14 +594,17 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
                 ++ctx->last_launches;
             }
         }
-        cudaEventRecord(ctx->ev[HK_PH_LANE + 1], stream);
+        HK_TRY(cudaEventRecord(ctx->ev[HK_PH_LANE + 1], stream));
         near_kernel<KB><<<grid, kThreads, 0, stream>>>(a);
         ++ctx->last_launches;
-        cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream);
+        HK_TRY(cudaGetLastError());
+        HK_TRY(cudaEventRecord(ctx->ev[HK_PH_NEAR + 1], stream));
+#undef HK_TRY
+        return e;
     };
-    if (p.kb == 8) launch(std::integral_constant<int, 8>());
-    else if (p.kb == 4) launch(std::integral_constant<int, 4>());
-    else launch(std::integral_constant<int, 2>());
+    if (p.kb == 8) HK_CUDA(launch(std::integral_constant<int, 8>()));
+    else if (p.kb == 4) HK_CUDA(launch(std::integral_constant<int, 4>()));
+    else HK_CUDA(launch(std::integral_constant<int, 2>()));
     // downward pass: parents' polynomials onto the children's nodes, level-0 nodes onto the bins
     if (lv.n_entries > 0) {
         for (int l = lv.n_levels - 1; l >= 1; --l) {
@@ -658,7 +683,9 @@ static int compute_any(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, doub
     std::memcpy(&cmin, &got[0], 8);
     std::memcpy(&cmax, &got[1], 8);
     const bool none = got[0] == ~0ULL;                     // no line has a positive cutting length
-    int64_t tot_skipped = 0, tot_off = 0, tot_evals = 0, launches = 0;
+    int64_t launches = 0;
+    DevTotals* totals = (DevTotals*)((char*)ctx->ws + L.totals);
+    HK_CUDA(cudaMemsetAsync(totals, 0, sizeof(DevTotals), stream));
     int rc = HK_OK;
     bool first = true;
     double lo = none ? 1.0 : cmin;
@@ -677,18 +704,17 @@ static int compute_any(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, doub
         rc = compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, stream, zero_out && first, false, extra, &cls);
         if (rc != HK_OK) break;
         launches += ctx->last_launches;
-        DevStats ds;
-        HK_CUDA(cudaMemcpyAsync(&ds, ctx->d_stats, sizeof(ds), cudaMemcpyDeviceToHost, stream));
-        HK_CUDA(cudaStreamSynchronize(stream));
-        tot_skipped += (int64_t)ds.n_skipped; tot_off += (int64_t)ds.n_off_grid; tot_evals += (int64_t)ds.n_evals;
+        add_totals_kernel<<<1, 1, 0, stream>>>(ctx->d_stats, totals);      // per-pass counters summed on the device
         first = false;
         if (!(cls.hi < INFINITY)) break;
         lo *= 2.0;
     }
     if (rc != HK_OK) return rc;
+    HK_CUDA(cudaGetLastError());
     ctx->last_launches = launches;
     ctx->host_totals = true;
-    ctx->tot_lines = n_lines; ctx->tot_skipped = tot_skipped; ctx->tot_off_grid = tot_off; ctx->tot_evals = tot_evals;
+    ctx->last_multi = true;
+    ctx->tot_lines = n_lines;
     return HK_OK;
 }
 
@@ -779,12 +805,13 @@ int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut
     double* k_dev = (double*)(base + H.k);
     const double* src[6] = {hl ? hl->nu0 : nullptr, hl ? hl->A : nullptr, hl ? hl->g_up : nullptr,
                             hl ? hl->E_low : nullptr, hl ? hl->gamma_ref : nullptr, hl ? hl->n_exp : nullptr};
-    int64_t tot_skipped = 0, tot_off = 0, tot_evals = 0;
     int rc = HK_OK;
     // the per-block device scratch is the front of the caller's workspace
     ctx->ws = base + H.dev_ws;
     ctx->ws_bytes = H.stage[0] - H.dev_ws;
+    DevTotals* totals = (DevTotals*)((char*)ctx->ws + make_layout(ctx, 1).totals);   // (fixed offset in every block's layout)
     cudaError_t e = cudaMemsetAsync(k_dev, 0, (size_t)ctx->N * sizeof(double), stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(totals, 0, sizeof(DevTotals), stream);
     const int64_t n_blocks = n_lines > 0 ? (n_lines + B - 1) / B : 0;
     auto enqueue_copy = [&](int64_t b) -> cudaError_t {
         const int s = (int)(b & 1);
@@ -812,14 +839,9 @@ int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut
         if (rc != HK_OK) break;
         e = cudaEventRecord(ctx->ev_done[s], stream);
         if (e != cudaSuccess) break;
-        // per-block counters: read back after the block (the stats buffer is reused by the next one)
-        DevStats ds;
-        e = cudaMemcpyAsync(&ds, ctx->d_stats, sizeof(ds), cudaMemcpyDeviceToHost, stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
-        if (e != cudaSuccess) break;
-        tot_skipped += (int64_t)ds.n_skipped;
-        tot_off += (int64_t)ds.n_off_grid;
-        tot_evals += (int64_t)ds.n_evals;
+        // per-block counters: summed on the device (the stats buffer is reused by the next block), no host synchronisation
+        if (ctx->d_stats) add_totals_kernel<<<1, 1, 0, stream>>>(ctx->d_stats, totals);
+        e = cudaGetLastError();
     }
     if (e == cudaSuccess && rc == HK_OK)
         e = cudaMemcpyAsync(out_k_host, k_dev, (size_t)ctx->N * sizeof(double), cudaMemcpyDeviceToHost, stream);
@@ -831,22 +853,39 @@ int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut
     if (e != cudaSuccess) return fail_cuda(ctx, e);
     if (n_blocks == 0) { ctx->have_run = true; ctx->last_n = 0; ctx->last_stream = stream; ctx->d_stats = nullptr; }
     ctx->host_totals = true;
-    ctx->tot_lines = n_lines; ctx->tot_skipped = tot_skipped; ctx->tot_off_grid = tot_off; ctx->tot_evals = tot_evals;
+    ctx->last_multi = n_blocks > 1;
+    ctx->d_totals = totals;
+    ctx->tot_lines = n_lines;
     return HK_OK;
 }
 
 int hk_get_extents(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, int32_t* ilo_dev, int32_t* ihi_dev,
                    int32_t* jc_dev, void* stream_v)
 {
-    if (!ctx || n_lines < 0 || (n_lines > 0 && !lines_ok(lines))) return HK_EINVAL;
+    if (!ctx || n_lines < 0) return HK_EINVAL;
     if (!ctx->have_cond || !ctx->have_run) return HK_ESTATE;
     cudaStream_t stream = (cudaStream_t)stream_v;
-    if (n_lines > 0) {
-        const Params p = make_params(ctx, ctx->last_cut, 512);
-        extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
-                                                                   lines->gamma_ref, lines->n_exp, LineExtra{nullptr, nullptr, nullptr},
-                                                                   n_lines, ilo_dev, ihi_dev, jc_dev, nullptr, nullptr, nullptr);
-        HK_CUDA(cudaGetLastError());
+    const bool from_records = ctx->last_recU && !ctx->last_multi && n_lines == ctx->last_n;
+    if (from_records) {
+        // what the last compute wrote (unsorted records are in the caller's line order): valid after hk_compute,
+        // hk_accumulate, hk_compute_hitran and a single-block hk_compute_host; `lines` is not read
+        if (n_lines > 0) {
+            if (stream != ctx->last_stream) HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
+            extents_from_records_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(ctx->last_recU, n_lines, ilo_dev, ihi_dev, jc_dev);
+            HK_CUDA(cudaGetLastError());
+        }
+    } else {
+        // several passes or blocks shared the record buffer (width-relative cutting lengths, hk_compute_host with more
+        // than one block, a different n_lines): recompute from the lines with the conditions and cut of the last compute
+        if (ctx->last_hitran) return HK_ESTATE;                  // HITRAN-style lists: hk_get_line_params_hitran
+        if (n_lines > 0 && !lines_ok(lines)) return HK_EINVAL;
+        if (n_lines > 0) {
+            const Params p = make_params(ctx, ctx->last_cut, 512);
+            extents_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
+                                                                       lines->gamma_ref, lines->n_exp, LineExtra{nullptr, nullptr, nullptr},
+                                                                       n_lines, ilo_dev, ihi_dev, jc_dev, nullptr, nullptr, nullptr);
+            HK_CUDA(cudaGetLastError());
+        }
     }
     HK_CUDA(cudaStreamSynchronize(stream));
     return HK_OK;
@@ -956,7 +995,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
         // per-region evaluation counts, derived from the records on demand (kept out of the hot path)
         const int64_t nl = ctx->last_n;                 // (block pipelines and class passes: the last block / pass)
         if (nl > 0) {
-            region_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_recU, nl, ctx->last_profile, ctx->d_stats);
+            region_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_recU, nl, ctx->last_profile, ctx->last_kb, ctx->d_stats);
             HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
         }
         ctx->regions_done = true;
@@ -992,11 +1031,18 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_levels = ctx->last_levels;
     host_out->scale_exp = d.scale_exp;
     host_out->sort_bits = ctx->last_sort_bits;
+    host_out->n_plinth_illcond = (int64_t)d.n_plinth_illcond;
+    host_out->n_unsorted = (int64_t)d.n_unsorted;
+    host_out->n_evals_gh10_row = (int64_t)d.n_cnt_gh10_row;
     if (ctx->host_totals) {
+        DevTotals t;
+        std::memset(&t, 0, sizeof(t));
+        if (ctx->d_totals && ctx->tot_lines > 0) HK_CUDA(cudaMemcpy(&t, ctx->d_totals, sizeof(t), cudaMemcpyDeviceToHost));
         host_out->n_lines = ctx->tot_lines;
-        host_out->n_skipped = ctx->tot_skipped;
-        host_out->n_off_grid = ctx->tot_off_grid;
-        host_out->n_evals = ctx->tot_evals;
+        host_out->n_skipped = (int64_t)t.n_skipped;
+        host_out->n_off_grid = (int64_t)t.n_off_grid;
+        host_out->n_evals = (int64_t)t.n_evals;
+        host_out->n_plinth_illcond = (int64_t)t.n_plinth_illcond;
     }
     return HK_OK;
 }
@@ -1013,35 +1059,55 @@ int hk_get_phase_ms(hk_ctx* ctx, float* out_ms)
     return HK_OK;
 }
 
-int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, void* stream_v)
+int hk_probe_fp32_ops(int kind, int iters, double* lane_ops_per_s, double* sm_clock_mhz, float* ms_out, void* stream_v)
 {
-    if (iters < 1 || !flops_out) return HK_EINVAL;
+    if (iters < 1 || kind < 0 || kind > 5 || !lane_ops_per_s) return HK_EINVAL;
     cudaStream_t stream = (cudaStream_t)stream_v;
     int dev = 0, n_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return HK_ECUDA;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HK_ECUDA;
     float* sink = nullptr;
+    long long* clk = nullptr;
     if (cudaMalloc(&sink, sizeof(float)) != cudaSuccess) return HK_ECUDA;
+    if (cudaMalloc(&clk, 2 * sizeof(long long)) != cudaSuccess) { cudaFree(sink); return HK_ECUDA; }
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     const int blocks = n_sm * 4, threads = 512;
     for (int rep = 0; rep < 2; ++rep) {      // first launch warms up
         cudaEventRecord(e0, stream);
-        if (packed) fp32_peak_kernel<true><<<blocks, threads, 0, stream>>>(iters, sink);
-        else fp32_peak_kernel<false><<<blocks, threads, 0, stream>>>(iters, sink);
+        switch (kind) {
+            case 0: fp32_probe_kernel<0><<<blocks, threads, 0, stream>>>(iters, sink, clk); break;
+            case 1: fp32_probe_kernel<1><<<blocks, threads, 0, stream>>>(iters, sink, clk); break;
+            case 2: fp32_probe_kernel<2><<<blocks, threads, 0, stream>>>(iters, sink, clk); break;
+            case 3: fp32_probe_kernel<3><<<blocks, threads, 0, stream>>>(iters, sink, clk); break;
+            case 4: fp32_probe_kernel<4><<<blocks, threads, 0, stream>>>(iters, sink, clk); break;
+            default: fp32_probe_kernel<5><<<blocks, threads, 0, stream>>>(iters, sink, clk); break;
+        }
         cudaEventRecord(e1, stream);
     }
     cudaError_t e = cudaStreamSynchronize(stream);
     float ms = 0.f;
+    long long h[2] = {0, 1};
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e == cudaSuccess) e = cudaMemcpy(h, clk, sizeof(h), cudaMemcpyDeviceToHost);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(sink);
+    cudaFree(sink); cudaFree(clk);
     if (e != cudaSuccess) return HK_ECUDA;
-    // 16 independent accumulators x 2 floats (packed) or 32 scalars; 2 FLOP per FMA
-    const double fmas = (double)blocks * threads * (double)iters * 32.0;
-    *flops_out = 2.0 * fmas / ((double)ms * 1e-3);
+    // 16 chains x 2 floats per step (MUFU: 16 x 1)
+    const double ops = (double)blocks * threads * (double)iters * (kind == 5 ? 16.0 : 32.0);
+    *lane_ops_per_s = ops / ((double)ms * 1e-3);
+    if (sm_clock_mhz) *sm_clock_mhz = h[1] > 0 ? (double)h[0] / (double)h[1] * 1e3 : 0.0;
     if (ms_out) *ms_out = ms;
     return HK_OK;
+}
+
+int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, void* stream_v)
+{
+    if (!flops_out) return HK_EINVAL;
+    double ops = 0.0;
+    const int rc = hk_probe_fp32_ops(packed ? 0 : 1, iters, &ops, nullptr, ms_out, stream_v);
+    *flops_out = 2.0 * ops;                   // 2 FLOP per FMA
+    return rc;
 }
 
 int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev, int32_t* region_out_dev,

@@ -88,8 +88,9 @@ __device__ __forceinline__ CentreLine centre_setup(const float4 ra, const float4
         return L;
     }
     if (Xmin + L.y2 >= HK_Z2) return L;          // no core bin in this tile
-    if (Xmin + L.y2 >= HK_Z4) { L.row = has_gh ? kRowR4 : kRowNone; return L; }
-    L.xl = z3_for(L.y2) - L.y2;
+    const float z3 = z3_for(L.y2);                                 // (both shrink to nothing as y grows: hk_device.cuh)
+    if (Xmin + L.y2 >= fmaxf(z4_for(L.y2), z3)) { L.row = has_gh ? kRowR4 : kRowNone; return L; }
+    L.xl = z3 - L.y2;                                              // (<= 0 for y >= 3: the 6-point rows take the whole tile)
     L.row = has_gh ? kRowR6m : kRowNone;
     if (L.xl > 0.f && Xmin < L.xl) {
         // innermost bins.  y >= 2: the 10-point rule converges on all of them -- as a row over the whole tile when X^10

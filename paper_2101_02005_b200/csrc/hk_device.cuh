@@ -163,12 +163,28 @@ __device__ __forceinline__ float gh10_K(float x2, float s, float y)
     return y * sum;
 }
 
+// The Gauss-Hermite rules converge faster the farther the pole lies from the real axis: the region each one is good
+// for grows with y.  Measured in fp64 against the oracle's w(z) on a lattice (worst case always at the smallest |z|):
+//   4 points: <= 3.0e-6 for |z|^2 >= 49 (any y), >= 36 (y >= 1.5), >= 30.25 (y >= 3); on ALL of the core for y >= 4.5 (5.7e-6)
+//   6 points: <= 4.8e-7 for |z|^2 >= 30.25 (any y);                                   on ALL of the core for y >= 3 (3.6e-6)
+//  10 points: on all of the core for y >= 2 (2.6e-6)
+// so a line with y >= 4.5 -- the majority at high pressure -- has no inner rings at all.
+#define HK_Y4 4.5f
+#define HK_Y6 3.0f
+// |z|^2 below which the 4-point rule is not used, as a function of y^2
+__device__ __forceinline__ float z4_for(float y2)
+{
+    return y2 >= HK_Y4 * HK_Y4 ? 0.f : y2 >= HK_Y6 * HK_Y6 ? HK_Z3 : y2 >= 2.25f ? 36.0f : HK_Z4;
+}
 // |z|^2 below which the innermost evaluator is used, as a function of y^2
 // (y = 0 exactly, the pure Gaussian of the Doppler profile: exp(-x^2) is ALL there is.  It is evaluated together with
 //  its amplitude, gauss_term below, and followed down to x^2 = HK_ZG: with the launch scale putting the largest
 //  amplitude at 2^100 that is the end of the fp32 range, 2^-126 -- DESIGN.md R22)
 #define HK_ZG 157.0f
-__device__ __forceinline__ float z3_for(float y2) { return y2 == 0.f ? HK_ZG : y2 < 1e-6f ? 50.0f : HK_Z3; }
+__device__ __forceinline__ float z3_for(float y2)
+{
+    return y2 == 0.f ? HK_ZG : y2 >= HK_Y6 * HK_Y6 ? 0.f : y2 < 1e-6f ? 50.0f : HK_Z3;
+}
 
 // cK exp(-x^2) for a pure Gaussian, amplitude and exponent combined BEFORE the exponential so that the product is
 // followed to the end of the fp32 range even where exp(-x^2) alone would underflow (x^2 > 87).  The exponent is
@@ -263,7 +279,7 @@ __device__ __forceinline__ float core_any_K(float x, float y, int* region)
     const float x2 = x * x, y2 = y * y, s = x2 + y2;
     if (y == 0.f) { if (region) *region = 4; return __expf(-x2); }     // pure Gaussian (with its amplitude: gauss_term)
     const float z3 = z3_for(y2);
-    if (s >= fmaxf(HK_Z4, z3)) { if (region) *region = 2; return gh4_K(x2, s, y); }
+    if (s >= fmaxf(z4_for(y2), z3)) { if (region) *region = 2; return gh4_K(x2, s, y); }
     if (s >= z3) { if (region) *region = 3; return gh6_K(x2, s, y); }
     if (y >= HK_Y10) { if (region) *region = 5; return gh10_K(x2, s, y); }
     if (region) *region = 4;

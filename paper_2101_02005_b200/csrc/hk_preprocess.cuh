@@ -70,6 +70,7 @@ struct DevStats {
     unsigned long long n_skipped, n_off_grid, n_evals, n_cnt_mid, n_cnt_core;  // cnt_*: evals with |z|^2 below Z1 / Z2
     unsigned long long n_cnt_gh6, n_cnt_trap;                                  // ... below Z4 / Z3
     unsigned long long n_cnt_gh10;                                             // of n_cnt_trap: lines with y >= HK_Y10
+    unsigned long long n_cnt_gh10_row;                                         // of n_cnt_gh10: lines wide enough for the row kernel's 10-point class
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
     int32_t pad;
@@ -81,7 +82,31 @@ struct DevStats {
     unsigned long long pairs_edge_node;                    // (line, extent end) pairs evaluated at the nodes of their edge tile
     unsigned long long pairs_node;                         // (line, tile) pairs evaluated at nodes
     unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
+    unsigned long long shift_bits;                         // max |delta P| over the lines (cm^-1) as double bits (pressure shift)
+    unsigned long long n_plinth_illcond;                   // plinth removal: lines whose cutting length falls inside their core
+    unsigned long long n_unsorted;                         // adjacent pairs of valid lines out of centre-bin order (input order)
 };
+
+// Totals over the blocks of hk_compute_host / the class passes of a width-relative cut, kept on the device so that the
+// per-block counters need no host synchronisation (read back once at the end).
+struct DevTotals {
+    unsigned long long n_skipped, n_off_grid, n_evals, n_plinth_illcond;
+};
+__global__ void add_totals_kernel(const DevStats* __restrict__ st, DevTotals* __restrict__ tot)
+{
+    tot->n_skipped += st->n_skipped; tot->n_off_grid += st->n_off_grid; tot->n_evals += st->n_evals;
+    tot->n_plinth_illcond += st->n_plinth_illcond;
+}
+
+// The tile bounds (left_bound / right_bound) assume alpha_D = beta x centre.  With a pressure shift the profile is
+// centred at nu0 + delta P while alpha_D uses the tabulated nu0 (R23), so alpha_D <= beta (centre + s) with
+// s = max |delta P| over the list (found by line_kernel): the bounds stay conservative BY CONSTRUCTION when the origin
+// of the wavenumber axis they see is moved down by s.  Kernels that evaluate the bounds call this first.
+__device__ __forceinline__ void apply_shift_bound(Params& p, const DevStats* __restrict__ st)
+{
+    const double s = __longlong_as_double((long long)st->shift_bits);
+    if (s > 0.0) p.numin_bins += s / p.dnu;
+}
 
 __device__ __forceinline__ bool finite6(double a, double b, double c, double d, double e, double f)
 {
@@ -95,6 +120,7 @@ struct LineOut {
     double S, gammaL, alphaD;
     int64_t jc, ilo, ihi;
     double pos_f;     // (nu0-numin)/dnu - jc
+    double shift;     // |delta P|, cm^-1 (0 without pressure shift)
 };
 
 // The fp64 arithmetic of step a1.  Extents use IEEE operations in exactly the order
@@ -110,7 +136,7 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
     o.on_grid = false;
     o.foreign = false;
     o.S = o.gammaL = o.alphaD = 0.0;
-    o.jc = 0; o.ilo = 0; o.ihi = -1; o.pos_f = 0.0;
+    o.jc = 0; o.ilo = 0; o.ihi = -1; o.pos_f = 0.0; o.shift = 0.0;
     if (!o.valid) return o;
     double ctr = nu0;                                                          // centre of the profile and of the extent
     if (p.n_iso > 0) {
@@ -119,6 +145,7 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
         o.gammaL = A * p.inv4pic + exp(nx * p.ln_tfac) * (gam * (p.P_atm - p.P_self) + gs * p.P_self);
         o.S = A * g * p.sfac_iso[iso] / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));
         ctr = __dadd_rn(nu0, __dmul_rn(dl, p.P_atm));                          // two roundings, as the oracle (no FMA contraction)
+        o.shift = fabs(ctr - nu0);
     } else {
     o.alphaD = p.beta * nu0;                                                   // Eq. 13 (L203)
     o.gammaL = A * p.inv4pic + gam * exp(nx * p.ln_tfac) * p.P_atm;            // Eq. 5 (L91): (T_ref/T)^n = e^(n ln(T_ref/T))
@@ -175,7 +202,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
                                                    int32_t* __restrict__ idx, float* __restrict__ flo,
                                                    DevStats* __restrict__ st)
 {
-    unsigned long long skipped = 0, off = 0, evals = 0, cmid = 0, ccore = 0, cgh6 = 0, ctrap = 0, cgh10 = 0, cmaxb = 0, cKmaxb = 0;
+    unsigned long long skipped = 0, off = 0, evals = 0, cmaxb = 0, cKmaxb = 0, shiftb = 0;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
                                 : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
@@ -210,6 +237,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             cmaxb = max(cmaxb, (unsigned long long)__double_as_longlong(cl));
             cKmaxb = max(cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
             evals += (unsigned long long)(o.ihi - o.ilo + 1);
+            shiftb = max(shiftb, (unsigned long long)__double_as_longlong(o.shift));
             // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
             //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
         }
@@ -218,37 +246,35 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
         key[i] = k;
         idx[i] = (int32_t)i;
     }
-    // block reduction of the counters
-    __shared__ unsigned long long sh[10][8];
-    unsigned long long v[10] = {skipped, off, evals, cmid, ccore, cgh6, ctrap, cgh10, cmaxb, cKmaxb};
+    // block reduction of the counters: three sums, three maxima (positive doubles order as their bit patterns)
+    __shared__ unsigned long long sh[6][8];
+    unsigned long long v[6] = {skipped, off, evals, cmaxb, cKmaxb, shiftb};
 #pragma unroll
-    for (int q = 0; q < 10; ++q) {
+    for (int q = 0; q < 6; ++q) {
         unsigned long long x = v[q];
         for (int o = 16; o > 0; o >>= 1) {
             unsigned long long y = __shfl_xor_sync(0xffffffffu, x, o);
-            x = (q < 8) ? x + y : max(x, y);
+            x = (q < 3) ? x + y : max(x, y);
         }
         if ((threadIdx.x & 31) == 0) sh[q][threadIdx.x >> 5] = x;
     }
     __syncthreads();
-    if (threadIdx.x < 10) {
+    if (threadIdx.x < 6) {
         int q = threadIdx.x;
         unsigned long long x = sh[q][0];
-        for (int w = 1; w < 8; ++w) x = (q < 8) ? x + sh[q][w] : max(x, sh[q][w]);
+        for (int w = 1; w < 8; ++w) x = (q < 3) ? x + sh[q][w] : max(x, sh[q][w]);
         unsigned long long* dst = q == 0 ? &st->n_skipped : q == 1 ? &st->n_off_grid : q == 2 ? &st->n_evals
-                                : q == 3 ? &st->n_cnt_mid : q == 4 ? &st->n_cnt_core : q == 5 ? &st->n_cnt_gh6
-                                : q == 6 ? &st->n_cnt_trap : q == 7 ? &st->n_cnt_gh10 : q == 8 ? &st->cmax_bits : &st->cKmax_bits;
-        if (q < 8) { if (x) atomicAdd(dst, x); }
-        else atomicMax(dst, x);
+                                : q == 3 ? &st->cmax_bits : q == 4 ? &st->cKmax_bits : &st->shift_bits;
+        if (x) { if (q < 3) atomicAdd(dst, x); else atomicMax(dst, x); }
     }
 }
 
 // Per-region evaluation counts (hk_stats.n_evals_far / mid / core / gh6 / trap / gh10) from the unsorted records of the
 // last compute: for each line the number of bins of its extent with |z|^2 below each threshold.  Run on demand.
-__global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restrict__ rec, int64_t n, int profile,
+__global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restrict__ rec, int64_t n, int profile, int kb,
                                                            DevStats* __restrict__ st)
 {
-    unsigned long long c[5] = {0, 0, 0, 0, 0};           // below Z1, Z2, Z4, Z3 (trapezoid region), of that with y >= 2
+    unsigned long long c[6] = {0, 0, 0, 0, 0, 0};        // below Z1, Z2, Z4, Z3 (trapezoid region), of that with y >= 2, of that in rows
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const RecU r = rec[i];
         if (r.ihi < r.ilo) continue;
@@ -256,21 +282,25 @@ __global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restric
         const double G2 = gauss ? 0.0 : (double)r.G2, a2 = profile == HK_PROFILE_LORENTZ ? 0.0 : (double)r.a2;
         const double pos = (double)r.jc + (signbit(r.f) ? 1.0 + (double)r.f : (double)r.f);
         const double y2 = a2 > 0.0 ? G2 / a2 : 1.0e300;
-        const double z3 = y2 == 0.0 ? (double)HK_ZG : y2 < 1e-6 ? 50.0 : (double)HK_Z3;
-        const double t[4] = {(double)HK_Z1 * a2 - G2, (double)HK_Z2 * a2 - G2, (double)HK_Z4 * a2 - G2, z3 * a2 - G2};
+        const double z3 = (double)z3_for((float)fmin(y2, 1.0e30)), z4 = fmax((double)z4_for((float)fmin(y2, 1.0e30)), z3);
+        const double t[4] = {(double)HK_Z1 * a2 - G2, (double)HK_Z2 * a2 - G2, z4 * a2 - G2, z3 * a2 - G2};
 #pragma unroll
         for (int q = 0; q < 4; ++q)
             c[q] += (unsigned long long)count_within(pos, t[q] > 0 ? (double)sqrtf((float)t[q]) : 0.0, r.ilo, r.ihi);
-        if (y2 >= (double)(HK_Y10 * HK_Y10))
-            c[4] += (unsigned long long)count_within(pos, t[3] > 0 ? (double)sqrtf((float)t[3]) : 0.0, r.ilo, r.ihi);
+        if (y2 >= (double)(HK_Y10 * HK_Y10)) {
+            const unsigned long long c10 = (unsigned long long)count_within(pos, t[3] > 0 ? (double)sqrtf((float)t[3]) : 0.0, r.ilo, r.ihi);
+            c[4] += c10;
+            // the row kernel evaluates these bins itself (class R10) when alpha_D >= 0.85 bins per 64 bins of tile (centre_setup)
+            if (a2 > 0.0 && 1.0 / sqrt(a2) < 1.0 / (0.85 * (double)(kb / 2))) c[5] += c10;
+        }
     }
 #pragma unroll
-    for (int q = 0; q < 5; ++q) {
+    for (int q = 0; q < 6; ++q) {
         unsigned long long x = c[q];
         for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
         if ((threadIdx.x & 31) == 0 && x) {
             unsigned long long* dst = q == 0 ? &st->n_cnt_mid : q == 1 ? &st->n_cnt_core : q == 2 ? &st->n_cnt_gh6
-                                    : q == 3 ? &st->n_cnt_trap : &st->n_cnt_gh10;
+                                    : q == 3 ? &st->n_cnt_trap : q == 4 ? &st->n_cnt_gh10 : &st->n_cnt_gh10_row;
             atomicAdd(dst, x);
         }
     }
@@ -446,6 +476,7 @@ __global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, co
 {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= lv.n_entries) return;
+    apply_shift_bound(p, st);
     int l = 0;
     while (l + 1 < lv.n_levels && e >= lv.off[l + 1]) ++l;
     const int64_t j = e - lv.off[l];
@@ -502,6 +533,7 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
 {
     int wt = blockIdx.x * blockDim.x + threadIdx.x;
     if (wt >= p.n_ct) return;
+    apply_shift_bound(p, st);
     const int wb = 32 * p.kb;
     const int64_t mind = (int64_t)kMinDistPerKB * p.kb;
     const int64_t w0 = (int64_t)wt * wb;
