@@ -30,6 +30,10 @@ import torch
 
 from workload import linelists as W
 
+import re
+# Chebyshev nodes per separated tile the library is built with (include/hk.h)
+HK_NODES = int(re.search(r"#define HK_NODES (\d+)", open(os.path.join(ROOT, "include", "hk.h")).read()).group(1))
+
 METRIC = "lines_per_s"
 UNIT = "lines/s"
 FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM (4 SMSPs x 32), DESIGN.md section 7
@@ -263,11 +267,11 @@ def _kernel_flops(st):
     g10_lane = st["n_evals_gh10"] - g10_row
     kb = st["bins_per_lane"]
     return {
-        "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * 8),
+        "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * HK_NODES),
         "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
         "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
         # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end
-        "edge": (f"edge_kernel<{kb}> + edge_node_kernel", FLOP["mid"] * (0.5 * st["n_pairs_edge"] + 8 * st["n_pairs_edge_node"])),
+        "edge": (f"edge_kernel<{kb}> + edge_node_kernel", FLOP["mid"] * (0.5 * st["n_pairs_edge"] + HK_NODES * st["n_pairs_edge_node"])),
         # line centres, rows: two-term outside the core, Gauss-Hermite 4 / 6 rings, the 10-point class of wide lines
         "centre": (f"centre_row_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
                    + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * g10_row),
@@ -301,8 +305,8 @@ def _timed(op, dl, cut, steps, warmup, flush, barrier=None):
         barrier()
     step_ms = [ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(steps)]
     for p in phases:
-        phases[p] /= steps
-    return step_ms, phases, op.stats(), k
+        phases[p] /= max(steps, 1)
+    return step_ms, phases, (op.stats() if steps > 0 else None), k
 
 
 PHASE_NAMES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "lane", "near", "down")
@@ -383,6 +387,8 @@ def run_ours(args):
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
     op.set_tile_bins(args.tile_bins)
     op.set_debug_mode(args.mode)
+    if args.node_sep is not None:
+        op.set_node_separation(args.node_sep)
     input_bytes = 6 * 8 * n
     flush = None
     if input_bytes < 256e6:                                  # inputs smaller than ~2x L2: flush L2 between iterations
@@ -437,7 +443,7 @@ def run_ours(args):
                 "flop_per_eval": FLOP, "kernels": kernels, "all_accumulation_kernels": allk,
                 "hbm_preprocess_gbs": (input_bytes + 40.0 * n) / (phases["preprocess"] * 1e-3) / 1e9 if phases["preprocess"] > 0 else None,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_kind": peaks_kind}
-    if cfg == 4 and n == c["n"] and args.mode == 0 and args.tile_bins == 0:
+    if cfg == 4 and n == c["n"] and args.mode == 0 and args.tile_bins == 0 and args.node_sep is None:
         one = _ncu_onepass(kernels[dom]["kernel"].split("<")[0])
         if one is not None:
             # measure (b) of SURVEY 8(d): executed FP32 thread instructions (FFMA x 2 + FADD + FMUL) over the ncu
@@ -465,7 +471,7 @@ def run_ours(args):
            "paper_context": "paper: ~1e7 lines/s (BT2, 0.01 cm^-1, cut 25, RTX 2080 Ti, incl. read; PAPER.md L7, Table 8 L778) -- other hardware and cut"}
 
     # ---- the other configs of BASELINE.json and the batched-conditions path, under the same clock (N = 1) -------------
-    if not args.no_other_configs and world == 1 and cfg == 4 and args.mode == 0:
+    if not args.no_other_configs and world == 1 and cfg == 4 and args.mode == 0 and args.node_sep is None:
         others = {}
         for oc in (1, 2, 3, 5):
             cc = W.CONFIGS[oc]
@@ -571,6 +577,7 @@ def main():
     ap.add_argument("--n-lines", type=int, default=0)
     ap.add_argument("--tile-bins", type=int, default=0, choices=[0, 2, 4, 8], help="bins per lane of a level-0 tile (0: library default)")
     ap.add_argument("--mode", type=int, default=0, choices=[0, 1, 2, 3], help="hk_set_debug_mode (3: direct evaluation only)")
+    ap.add_argument("--node-sep", type=float, default=None, help="hk_set_node_separation (sweeps; default: the library's 4)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip configs 1, 2, 3, 5 and the batch leg after the headline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -105,7 +105,10 @@ enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, H
                           (the pole moves away from the real axis): 4 points from |z|^2 >= 36 for y >= 1.5, >= 30.25 for y >= 3, and
                           on the whole core for y >= 4.5; 6 points on the whole core for y >= 3 (hk_device.cuh: z4_for, z3_for) */
 #define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3) and y < 3: trapezoid rule + pole term, <= 2e-6; 10-point Gauss-Hermite when y >= 2, <= 2.7e-6 */
-#define HK_NODES 8     /* Chebyshev nodes per tile of the separated-tile evaluation */
+#ifndef HK_NODES
+#define HK_NODES 12    /* Chebyshev nodes per tile of the separated-tile evaluation; 8, 10 or 12 */
+#endif
+#define HK_NODE_SEP (HK_NODES == 8 ? 4.0 : HK_NODES == 10 ? 2.5 : 2.0) /* default separation, tile half-widths: interpolation error <= 6e-6 */
 
 /* Grid: bin i is the POINT nu_i = numin + i*dnu (R8, R9).  HK_EINVAL if dnu <= 0,
  * numax <= numin, a non-finite argument, N < 1 or N too large. */

@@ -410,7 +410,7 @@ __global__ void __launch_bounds__(kThreads, 4) edge_kernel(AccArgs a)
     }
 }
 
-constexpr int kNodeCtas = 6;           // resident CTAs per SM of the node kernel
+constexpr int kNodeCtas = kP <= 8 ? 6 : 4;   // resident CTAs per SM of the node kernel (register budget grows with the node count)
 
 }  // namespace hk
 #include "hk_centre.cuh"               // the line centres: centre_row_kernel, centre_lane_kernel
@@ -780,8 +780,9 @@ __device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_
         } else {
             // transposing reduction: each exchange halves the values a lane carries (8 -> 4 -> 2 -> 1 over lane bits
             // 4, 3, 2), two butterfly steps finish bits 1, 0: 9 shuffles instead of 40.  Lane l then holds the sum of
-            // value j = (bit4, bit3, bit2 of l); the lanes with l % 4 == 0 issue one atomic each.
-            static_assert(kP == 8, "the fold below is written for 8 nodes");
+            // value j = (bit4, bit3, bit2 of l); the lanes with l % 4 == 0 issue one atomic each.  Nodes beyond the
+            // first eight (kP = 10, 12) go through a second, shorter fold of the same kind.
+            static_assert(kP == 8 || kP == 10 || kP == 12, "the folds below are written for 8, 10 or 12 nodes");
             float a[8], b4[4], c2[2];
 #pragma unroll
             for (int j = 0; j < 8; ++j) a[j] = mine ? v[j] : 0.f;
@@ -801,6 +802,32 @@ __device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_
             d += __shfl_xor_sync(0xffffffffu, d, 1);
             const int j = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
             if ((lane & 3) == 0) atomicAdd(acc + (size_t)b * kP + j, (double)d);
+            if constexpr (kP == 12) {
+                // values 8..11: 4 -> 2 -> 1 over lane bits 4, 3, then three butterfly steps; lane l holds j = 8 + (bit4, bit3)
+                float e[4], f2[2];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) e[q] = mine ? v[8 + q] : 0.f;
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const float send = h4 ? e[q] : e[q + 2], keep = h4 ? e[q + 2] : e[q];
+                    f2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+                }
+                float g = (h3 ? f2[1] : f2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? f2[0] : f2[1], 8);
+                g += __shfl_xor_sync(0xffffffffu, g, 4);
+                g += __shfl_xor_sync(0xffffffffu, g, 2);
+                g += __shfl_xor_sync(0xffffffffu, g, 1);
+                const int jj = 8 + ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
+                if ((lane & 7) == 0) atomicAdd(acc + (size_t)b * kP + jj, (double)g);
+            } else if constexpr (kP == 10) {
+                // values 8, 9: 2 -> 1 over lane bit 4, then four butterfly steps; lane l holds j = 8 + bit4
+                const float e0 = mine ? v[8] : 0.f, e1 = mine ? v[kP - 1] : 0.f;
+                float g = (h4 ? e1 : e0) + __shfl_xor_sync(0xffffffffu, h4 ? e0 : e1, 16);
+                g += __shfl_xor_sync(0xffffffffu, g, 8);
+                g += __shfl_xor_sync(0xffffffffu, g, 4);
+                g += __shfl_xor_sync(0xffffffffu, g, 2);
+                g += __shfl_xor_sync(0xffffffffu, g, 1);
+                if ((lane & 15) == 0) atomicAdd(acc + (size_t)b * kP + 8 + ((lane >> 4) & 1), (double)g);
+            }
         }
         todo &= ~grp;
     }

@@ -329,7 +329,7 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     if (!c) return HK_ENOMEM;
     std::memset(c, 0, sizeof(*c));
     c->numin = numin; c->numax = numax; c->dnu = dnu; c->N = (int64_t)Nd;
-    c->node_sep = 4.0;
+    c->node_sep = HK_NODE_SEP;
     c->edge_nodes = 1;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -396,8 +396,9 @@ int hk_set_debug_mode(hk_ctx* ctx, int mode)
 
 int hk_set_node_separation(hk_ctx* ctx, double sep)
 {
-    // 0 switches the node hierarchy off; below 3 half-widths the degree-7 interpolant leaves the error budget
-    if (!ctx || !std::isfinite(sep) || sep < 0.0 || sep > 64.0 || (sep > 0.0 && sep < 3.0)) return HK_EINVAL;
+    // 0 switches the node hierarchy off; closer than the default minus a quarter of a half-width the interpolant leaves the error
+    // budget (tests/test_nodes.py)
+    if (!ctx || !std::isfinite(sep) || sep < 0.0 || sep > 64.0 || (sep > 0.0 && sep < HK_NODE_SEP - 0.25)) return HK_EINVAL;
     ctx->node_sep = sep;
     return HK_OK;
 }

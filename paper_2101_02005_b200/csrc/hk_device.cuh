@@ -61,15 +61,37 @@ struct __align__(16) NodeRange {
 };
 
 // ---- Chebyshev nodes of the separated-tile evaluation ----------------
-constexpr int kP = 8;                    // nodes per tile: degree-7 interpolant
+constexpr int kP = HK_NODES;             // nodes per tile: degree-(kP-1) interpolant
 constexpr int kMaxLevels = 24;
-// xi_k = cos((2k+1) pi/16); barycentric weights (-1)^k sin((2k+1) pi/16)
+// xi_k = cos((2k+1) pi/(2 kP)); barycentric weights (-1)^k sin((2k+1) pi/(2 kP))
+#if HK_NODES == 8
 __device__ constexpr double kChebX[kP] = {0.98078528040323044913,  0.83146961230254523708,  0.55557023301960222474,
                                           0.19509032201612826785,  -0.19509032201612826785, -0.55557023301960222474,
                                           -0.83146961230254523708, -0.98078528040323044913};
 __device__ constexpr double kChebW[kP] = {0.19509032201612826785,  -0.55557023301960222474, 0.83146961230254523708,
                                           -0.98078528040323044913, 0.98078528040323044913,  -0.83146961230254523708,
                                           0.55557023301960222474,  -0.19509032201612826785};
+#elif HK_NODES == 10
+__device__ constexpr double kChebX[kP] = {0.98768834059513772619,  0.89100652418836786236,  0.7071067811865475244,
+                                          0.45399049973954679156,  0.15643446504023086901,  -0.15643446504023086901,
+                                          -0.45399049973954679156, -0.7071067811865475244,  -0.89100652418836786236,
+                                          -0.98768834059513772619};
+__device__ constexpr double kChebW[kP] = {0.15643446504023086901,  -0.45399049973954679156, 0.7071067811865475244,
+                                          -0.89100652418836786236, 0.98768834059513772619,  -0.98768834059513772619,
+                                          0.89100652418836786236,  -0.7071067811865475244,  0.45399049973954679156,
+                                          -0.15643446504023086901};
+#elif HK_NODES == 12
+__device__ constexpr double kChebX[kP] = {0.99144486137381041114,  0.92387953251128675613,  0.79335334029123516458,
+                                          0.60876142900872063942,  0.38268343236508977173,  0.13052619222005159155,
+                                          -0.13052619222005159155, -0.38268343236508977173, -0.60876142900872063942,
+                                          -0.79335334029123516458, -0.92387953251128675613, -0.99144486137381041114};
+__device__ constexpr double kChebW[kP] = {0.13052619222005159155,  -0.38268343236508977173, 0.60876142900872063942,
+                                          -0.79335334029123516458, 0.92387953251128675613,  -0.99144486137381041114,
+                                          0.99144486137381041114,  -0.92387953251128675613, 0.79335334029123516458,
+                                          -0.60876142900872063942, 0.38268343236508977173,  -0.13052619222005159155};
+#else
+#error "HK_NODES must be 8, 10 or 12"
+#endif
 
 struct Levels {
     int32_t n_levels;                    // node levels 0..n_levels-1, tile width W0 << l
@@ -210,69 +232,107 @@ __device__ __forceinline__ float gauss_term(float cK, float x)
 // Re w(x + i y) for |z|^2 < HK_Z2, x >= 0, y > 0: ring by |z|^2
 __device__ __forceinline__ float core_any_K(float x, float y, int* region);
 
-// Re w(x + i y), x >= 0, y > 0, intended for x^2 + y^2 < ~700.
+// Re w(x + i y), x >= 0, 0 < y < 2 (< pi/h), intended for x^2 + y^2 < ~60.
 // K = (h y/pi) sum_n exp(-t_n^2)/((x-t_n)^2 + y^2) + pole term, t_n = (n + s) h, h = 0.8, n = -5..5
 // (Matta & Reichel 1971 / Hunter & Regan 1972: the family Algorithm 916, which the paper uses in region C
 // (L156), belongs to).  Two node sets (s = 0, 1/2), chosen per evaluation so that x is never within h/4
-// of a node; two nodes share one reciprocal.  The oracle uses h = 1/2, 29 nodes, fp64 and no node shift.
-__device__ __noinline__ float core_K(float x, float y)
+// of a node.  The oracle uses h = 1/2, 29 nodes, fp64 and no node shift.
+// Cost (the lane kernel is bound by instruction issue and by the special-function unit alike): the squared distances
+// to the nodes are formed two at a time (packed fp32), THREE nodes share one reciprocal, and the pole term rides on
+// the last reciprocal: 4 reciprocals per evaluation; everything that depends on y alone (TrapLine) is worked out once
+// per line.  Pole term, with E = exp(-2 pi y/h) and theta = 2 pi (x/h - s):
+//   Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) } = 2 exp(y^2 - 2 pi y/h) exp(-x^2) [cos(2xy)(E - cos theta) - sin(2xy) sin theta]
+//                                                      / [(E - cos theta)^2 + sin^2 theta]
+// (numerator and denominator divided by exp(4 pi y/h): nothing in it grows with y).
+struct TrapLine {
+    float y2, yk, ie, amp0, ty;        // y^2, y h/pi, exp(-2 pi y/h), 2 exp(y^2 - 2 pi y/h), 2 y
+};
+__device__ __forceinline__ TrapLine trap_line(float y)
 {
-    constexpr float h = 0.8f;
-    constexpr float inv_h = 1.25f;
-    // weights exp(-((n+s)h)^2), n = -5..5, for s = 0 and s = 1/2
-    constexpr float wA[11] = {1.12535175e-07f, 3.57128496e-05f, 3.15111160e-03f, 7.73047404e-02f,
-                              5.27292424e-01f, 1.0f,            5.27292424e-01f, 7.73047404e-02f,
-                              3.15111160e-03f, 3.57128496e-05f, 1.12535175e-07f};
-    constexpr float wB[11] = {2.35257520e-06f, 3.93669041e-04f, 1.83156389e-02f, 2.36927759e-01f,
-                              8.52143789e-01f, 8.52143789e-01f, 2.36927759e-01f, 1.83156389e-02f,
-                              3.93669041e-04f, 2.35257520e-06f, 3.90893843e-09f};
+    TrapLine L;
+    L.y2 = y * y;
+    L.yk = y * (0.8f / 3.14159265358979f);
+    L.ie = __expf(-7.85398163f * y);                        // 2 pi/h = 7.854
+    L.amp0 = 2.0f * __expf(fmaf(-7.85398163f, y, L.y2));
+    L.ty = y + y;
+    return L;
+}
+// weights exp(-((n+s)h)^2), n = -5..6 (the twelfth is there to make four triples; its weight is nil), s = 0 and s = 1/2
+#define HK_TRAP_WA {1.12535175e-07f, 3.57128496e-05f, 3.15111160e-03f, 7.73047404e-02f, 5.27292424e-01f, 1.0f, \
+                    5.27292424e-01f, 7.73047404e-02f, 3.15111160e-03f, 3.57128496e-05f, 1.12535175e-07f, 0.0f}
+#define HK_TRAP_WB {2.35257520e-06f, 3.93669041e-04f, 1.83156389e-02f, 2.36927759e-01f, 8.52143789e-01f, 8.52143789e-01f, \
+                    2.36927759e-01f, 1.83156389e-02f, 3.93669041e-04f, 2.35257520e-06f, 3.90893843e-09f, 0.0f}
+// wtab: the 24 weights in shared memory (A then B; fill with trap_weights_to_shared) or nullptr (selected from immediates)
+__device__ __forceinline__ void trap_weights_to_shared(float* wtab, int tid)
+{
+    constexpr float wA[12] = HK_TRAP_WA, wB[12] = HK_TRAP_WB;
+    if (tid < 12) wtab[tid] = wA[tid];
+    else if (tid < 24) wtab[tid] = wB[tid - 12];
+}
+__device__ __forceinline__ float trap_K(float x, const TrapLine& L, const float* __restrict__ wtab)
+{
+    constexpr float h = 0.8f, inv_h = 1.25f;
     const float u = x * inv_h;
     const float fr = u - floorf(u);
     const bool on = (fr >= 0.25f) && (fr < 0.75f);        // integer nodes are >= h/4 away
     const float s = on ? 0.0f : 0.5f;
     const float us = u - s;
     const float frs = us - floorf(us);                    // in [1/4, 3/4]
-    const float y2 = y * y;
     const float xs = fmaf(-s, h, x);                      // x - s h
-    float q[11];
+    // q_n = (xs - (n - 5) h)^2 + y^2, n = 0..11, two at a time
+    float2 q[6];
+    float2 d = make_float2(xs + 5.0f * h, xs + 4.0f * h);
+    const float2 y2 = make_float2(L.y2, L.y2), step = make_float2(-2.0f * h, -2.0f * h);
+    q[0] = __ffma2_rn(d, d, y2);
 #pragma unroll
-    for (int n = 0; n < 11; ++n) {
-        const float d = xs - (float)(n - 5) * h;
-        q[n] = fmaf(d, d, y2);                            // >= (h/4)^2
+    for (int k = 1; k < 6; ++k) {
+        d = __fadd2_rn(d, step);
+        q[k] = __ffma2_rn(d, d, y2);                      // >= (h/4)^2
     }
-    float sum = 0.0f;
+    float w[12];
+    if (wtab) {
+        const float4* w4 = reinterpret_cast<const float4*>(wtab) + (on ? 0 : 3);
+        const float4 w0 = w4[0], w1 = w4[1], w2 = w4[2];
+        w[0] = w0.x; w[1] = w0.y; w[2] = w0.z; w[3] = w0.w; w[4] = w1.x; w[5] = w1.y; w[6] = w1.z; w[7] = w1.w;
+        w[8] = w2.x; w[9] = w2.y; w[10] = w2.z; w[11] = w2.w;
+    } else {
+        constexpr float wA[12] = HK_TRAP_WA, wB[12] = HK_TRAP_WB;
 #pragma unroll
-    for (int n = 0; n < 10; n += 2) {
-        // w1/q1 + w2/q2 = (w1 q2 + w2 q1)/(q1 q2)
-        const float w1 = on ? wA[n] : wB[n], w2 = on ? wA[n + 1] : wB[n + 1];
-        const float num = fmaf(w2, q[n], w1 * q[n + 1]);
-        sum = fmaf(num, rcp_approx(q[n] * q[n + 1]), sum);
+        for (int n = 0; n < 12; ++n) w[n] = on ? wA[n] : wB[n];
     }
-    sum = fmaf(on ? wA[10] : wB[10], rcp_approx(q[10]), sum);
-    float K = sum * (y * (h / 3.14159265358979f));
-    const float re2 = fmaf(x, x, -y2);
-    if (y < 3.92699082f /* pi/h */ && re2 < 88.0f) {
-        // + Re{ 2 exp(-z^2) / (1 - exp(-2 pi i (z/h - s))) }  (re2 >= 40 is reached by y = 0 only, see z3_for)
-        const float amp = 2.0f * __expf(-re2);
-        // exp(-z^2) = exp(-re2) (cos phi - i sin phi), phi = 2 x y reduced to [-pi, pi] first
-        const float phi = 2.0f * x * y;
-        const float kk = rintf(phi * 0.159154943f);
-        float ph = fmaf(-kk, 6.28318548f, phi);
-        ph = fmaf(-kk, -1.74845553e-07f, ph);             // 2 pi = 6.28318548 - 1.74845553e-07
-        float sp, cp;
-        __sincosf(ph, &sp, &cp);
-        const float nr = amp * cp, ni = -amp * sp;
-        const float e = __expf(7.85398163f /* 2 pi/h */ * y);
-        // theta = 2 pi frac(x/h - s) in [pi/2, 3pi/2] (cos(theta) <= 0): theta - pi lies in [-pi/2, pi/2], where the
-        // special-function unit's sin/cos are good to ~5e-7 absolute
-        float st, ct;
-        __sincosf(6.28318531f * (frs - 0.5f), &st, &ct);
-        st = -st; ct = -ct;
-        const float dr = fmaf(-e, ct, 1.0f), di = e * st;
-        K = fmaf(fmaf(nr, dr, ni * di), rcp_approx(fmaf(dr, dr, di * di)), K);
+    const float qq[12] = {q[0].x, q[0].y, q[1].x, q[1].y, q[2].x, q[2].y, q[3].x, q[3].y, q[4].x, q[4].y, q[5].x, q[5].y};
+    // w_a/q_a + w_b/q_b + w_c/q_c = (w_a q_b q_c + (w_b q_c + w_c q_b) q_a) / (q_a q_b q_c)
+    float sum = 0.0f, num3 = 0.f, den3 = 1.f;
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+        const float qa = qq[3 * t], qb = qq[3 * t + 1], qc = qq[3 * t + 2];
+        const float qbc = qb * qc;
+        const float m = fmaf(w[3 * t + 1], qc, w[3 * t + 2] * qb);
+        const float num = fmaf(m, qa, w[3 * t] * qbc);
+        const float den = qa * qbc;
+        if (t < 3) sum = fmaf(num, rcp_approx(den), sum);
+        else { num3 = num; den3 = den; }
     }
-    return K;
+    // pole term over the last triple's denominator
+    const float g = __expf(-x * x);
+    const float phi = L.ty * x;                           // 2 x y, reduced to [-pi, pi] first
+    const float kk = rintf(phi * 0.159154943f);
+    float ph = fmaf(-kk, 6.28318548f, phi);
+    ph = fmaf(-kk, -1.74845553e-07f, ph);                 // 2 pi = 6.28318548 - 1.74845553e-07
+    float sp, cp;
+    __sincosf(ph, &sp, &cp);
+    // theta = 2 pi frac(x/h - s) in [pi/2, 3pi/2] (cos(theta) <= 0): theta - pi lies in [-pi/2, pi/2], where the
+    // special-function unit's sin/cos are good to ~5e-7 absolute
+    float st, ct;
+    __sincosf(6.28318531f * (frs - 0.5f), &st, &ct);
+    st = -st; ct = -ct;
+    const float a = L.ie - ct;                            // >= exp(-2 pi y/h) > 0
+    const float pn = (L.amp0 * g) * fmaf(cp, a, -sp * st);
+    const float pd = fmaf(a, a, st * st);
+    const float top = fmaf(L.yk * num3, pd, pn * den3);
+    return fmaf(sum, L.yk, top * rcp_approx(den3 * pd));
 }
+__device__ __noinline__ float core_K(float x, float y) { return trap_K(x, trap_line(y), nullptr); }
 
 __device__ __forceinline__ float core_any_K(float x, float y, int* region)
 {

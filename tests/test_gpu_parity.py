@@ -3,6 +3,8 @@ oracle on the same seeded inputs.  Tolerance (BASELINE.json north_star): relativ
 error <= 1e-4 per bin where oracle >= 1e-8 max(k), absolute <= 1e-8 max(k) elsewhere;
 integer extents and centre bins exact."""
 import math
+import os
+import re
 
 import numpy as np
 import pytest
@@ -13,6 +15,9 @@ from oracle import hk_oracle as O
 from workload import linelists as W
 
 from parity_util import check_parity, check_parity_plinth, sample_windows
+
+_HK_NODES = int(re.search(r"#define HK_NODES (\d+)", open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "..", "include", "hk.h")).read()).group(1))
+B_SEP_MIN = {8: 4.0, 10: 2.5, 12: 2.0}[_HK_NODES] - 0.25     # smallest node separation hk_set_node_separation accepts
 
 pytestmark = pytest.mark.gpu
 
@@ -157,9 +162,12 @@ def test_edge_nodes_on_vs_off(B, cfg, n):
     assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 3e-5
 
 
-@pytest.mark.parametrize("sep", [3.0, 4.0, 6.0])
+@pytest.mark.parametrize("sep", [B_SEP_MIN, 2.0, 3.0, 4.0, 6.0])
 def test_node_separation_sweep(B, sep):
-    """The node hierarchy at other separations (fewer / more pairs at nodes) against the oracle."""
+    """The node hierarchy at other separations (fewer / more pairs at nodes) against the oracle, down to the smallest
+    the library accepts (its default minus a quarter of a tile half-width: interpolation error 4.5e-5 worst case, tests/test_nodes.py)."""
+    if sep < B_SEP_MIN:
+        pytest.skip("below the smallest separation of this build")
     lines, cond, grid, cut = _mini(2, 20_000)
     op = B.Opacity(*grid)
     op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
@@ -172,7 +180,7 @@ def test_node_separation_sweep(B, sep):
     assert st["n_evals"] == evals
     check_parity(k.cpu().numpy(), k_ref, what=f"node separation {sep}")
     with pytest.raises(B.HKError):
-        op.set_node_separation(2.5)              # below 3 half-widths the degree-7 interpolant is outside the error budget
+        op.set_node_separation(B_SEP_MIN - 0.125)  # closer than that the interpolant is outside the error budget
     op.close()
 
 
