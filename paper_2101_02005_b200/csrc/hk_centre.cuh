@@ -434,20 +434,14 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
 // ---------------------------------------------------------------------------------------
 constexpr int kStage = 16;             // bins per staging step
 constexpr int kLaneCtas = 4;           // resident CTAs per SM (8 warps each) the lane kernel is compiled and launched for
-constexpr int kYClasses = 32;          // classes of y = Gamma_L/alpha_D the lines of a batch are sorted into
-
-// rings of the evaluators change with y (trapezoid below 2, no inner region from 5.5); the last class holds the lines
-// without lane-pass bins in this tile
-__device__ __forceinline__ int y_class(float y2)
-{
-    return min(30, (int)(sqrtf(y2) * 5.5f));         // 0..30: class edges at 2 (HK_Y10) and every 2/11 in between
-}
+constexpr int kYClasses = 32;          // classes the pooled lines are sorted into (one per evaluator: kLane*)
 
 // the value of one (line, bin) pair of the lane pass, amplitude included
-__device__ __forceinline__ float lane_value(int type, float cK, float x, float X, float y, float y2)
+__device__ __forceinline__ float lane_value(int type, float cK, float x, float X, float y, float y2, const TrapLine& TL,
+                                            const float* __restrict__ wtab)
 {
+    if (type == kLaneTrap) return cK * trap_K<true>(x, TL, wtab);
     if (type == kLaneGH10) return cK * gh10_K(X, X + y2, y);
-    if (type == kLaneTrap) return cK * core_K(x, y);
     if (type == kLaneGauss) return gauss_term(cK, x);
     return cK * core_any_K(x, y, nullptr);           // narrow lines: every ring of the core
 }
@@ -455,8 +449,9 @@ __device__ __forceinline__ float lane_value(int type, float cK, float x, float X
 // W = warps per CTA: 8 for dense lists; 2 or 1 for sparse ones (few lines per tile: a work unit is a handful of lines,
 // and more small CTAs keep more units in flight).
 // Only a minority of the (line, tile) visits of a unit has lane-pass bins, so the visits that do are POOLED in shared
-// memory across the staged batches; when the pool is full (or the unit ends) it is counting-sorted by y and dealt to
-// the warps in groups of 32 -- every warp busy, every lane of a group live, and the lines of a group alike.
+// memory across the staged batches; when the pool is full (or the unit ends) it is counting-sorted by evaluator and dealt
+// to the warps in groups of 32 -- every warp busy, every lane of a group live and running the same code.  Within a class
+// the lines keep (roughly) their order by centre, so the 32 rings of a group overlap and the lanes are busy on the same bins.
 template <int KB, int W, bool kBinned>
 __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kernel(AccArgs a)
 {
@@ -471,6 +466,9 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
     __shared__ float sacc[kWarps][kTB];
     __shared__ int hist[kYClasses];
     __shared__ int s_unit, s_pool_n, s_next;
+    __shared__ __align__(16) float wtab[24];   // trapezoid weights of the two node sets (trap_K)
+    trap_weights_to_shared(wtab, threadIdx.x);
+    if (kThreads < 24 && threadIdx.x == 0) { for (int i = kThreads; i < 24; ++i) trap_weights_to_shared(wtab, i); }
     double* red = reinterpret_cast<double*>(&stage[0][0][0]);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int32_t* __restrict__ prefix = a.prefix_lane;
@@ -538,6 +536,7 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                 bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
             }
             if (bmax < bmin) return;
+            const TrapLine TL = trap_line(type == kLaneTrap ? y : 1.0f);   // what the trapezoid rule needs of the line alone
             const int b_end = (int)bmax;
             const int col = lane & (kStage - 1), half = lane >> 4;
 #pragma unroll 1
@@ -550,7 +549,7 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                     const float un = __fmaf_rn(d, inva, nfa);            // the row pass's u and X, bit for bit
                     const float X = __fmul_rn(un, un);
                     float val = 0.f;
-                    if (X < xl) val = kBinned ? cK * binned_K(d, f, y2, inva) : lane_value(type, cK, fabsf(un), X, y, y2);
+                    if (X < xl) val = kBinned ? cK * binned_K(d, f, y2, inva) : lane_value(type, cK, fabsf(un), X, y, y2, TL, wtab);
                     stage[warp][s][lane] = val;
                 }
                 __syncwarp();
@@ -566,8 +565,8 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
             since_flush += 32;     // the bin tile holds at most 32 lines' terms per bin per group
             if (since_flush >= kFlush) flush();
         };
-        // sort the pool by y (lines that are neighbours in centre-bin order have nearly the same centre and Doppler
-        // width, so after the sort the 32 lines of a group also share evaluator and ring width) and work it off
+        // sort the pool by evaluator (lines that are neighbours in centre-bin order have nearly the same centre and Doppler
+        // width, so the 32 lines of a group also share ring position and width) and work it off
         auto run_pool = [&](int n) {
             int cls[kPPT], rk[kPPT];
             if (threadIdx.x < kYClasses) hist[threadIdx.x] = 0;
@@ -579,7 +578,7 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                 cls[k] = -1;
                 if (i < n) {
                     const float4 B = poolB[i];
-                    cls[k] = (kBinned || __float_as_int(B.z) == kLaneFull) ? 31 : y_class(B.y);
+                    cls[k] = kBinned ? 0 : __float_as_int(B.z);            // the evaluator (kLane*)
                     rk[k] = atomicAdd(&hist[cls[k]], 1);
                 }
             }

@@ -269,6 +269,7 @@ __device__ __forceinline__ void trap_weights_to_shared(float* wtab, int tid)
     if (tid < 12) wtab[tid] = wA[tid];
     else if (tid < 24) wtab[tid] = wB[tid - 12];
 }
+template <bool kSmemW>
 __device__ __forceinline__ float trap_K(float x, const TrapLine& L, const float* __restrict__ wtab)
 {
     constexpr float h = 0.8f, inv_h = 1.25f;
@@ -289,29 +290,32 @@ __device__ __forceinline__ float trap_K(float x, const TrapLine& L, const float*
         d = __fadd2_rn(d, step);
         q[k] = __ffma2_rn(d, d, y2);                      // >= (h/4)^2
     }
-    float w[12];
-    if (wtab) {
-        const float4* w4 = reinterpret_cast<const float4*>(wtab) + (on ? 0 : 3);
-        const float4 w0 = w4[0], w1 = w4[1], w2 = w4[2];
-        w[0] = w0.x; w[1] = w0.y; w[2] = w0.z; w[3] = w0.w; w[4] = w1.x; w[5] = w1.y; w[6] = w1.z; w[7] = w1.w;
-        w[8] = w2.x; w[9] = w2.y; w[10] = w2.z; w[11] = w2.w;
-    } else {
-        constexpr float wA[12] = HK_TRAP_WA, wB[12] = HK_TRAP_WB;
-#pragma unroll
-        for (int n = 0; n < 12; ++n) w[n] = on ? wA[n] : wB[n];
-    }
-    const float qq[12] = {q[0].x, q[0].y, q[1].x, q[1].y, q[2].x, q[2].y, q[3].x, q[3].y, q[4].x, q[4].y, q[5].x, q[5].y};
     // w_a/q_a + w_b/q_b + w_c/q_c = (w_a q_b q_c + (w_b q_c + w_c q_b) q_a) / (q_a q_b q_c)
-    float sum = 0.0f, num3 = 0.f, den3 = 1.f;
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-        const float qa = qq[3 * t], qb = qq[3 * t + 1], qc = qq[3 * t + 2];
-        const float qbc = qb * qc;
-        const float m = fmaf(w[3 * t + 1], qc, w[3 * t + 2] * qb);
-        const float num = fmaf(m, qa, w[3 * t] * qbc);
-        const float den = qa * qbc;
-        if (t < 3) sum = fmaf(num, rcp_approx(den), sum);
-        else { num3 = num; den3 = den; }
+    float sum, num3, den3;
+    {
+        float4 w0, w1, w2;
+        if (kSmemW) {
+            const float4* w4 = reinterpret_cast<const float4*>(wtab) + (on ? 0 : 3);
+            w0 = w4[0]; w1 = w4[1]; w2 = w4[2];
+        } else {
+            constexpr float wA[12] = HK_TRAP_WA, wB[12] = HK_TRAP_WB;
+            w0 = make_float4(on ? wA[0] : wB[0], on ? wA[1] : wB[1], on ? wA[2] : wB[2], on ? wA[3] : wB[3]);
+            w1 = make_float4(on ? wA[4] : wB[4], on ? wA[5] : wB[5], on ? wA[6] : wB[6], on ? wA[7] : wB[7]);
+            w2 = make_float4(on ? wA[8] : wB[8], on ? wA[9] : wB[9], on ? wA[10] : wB[10], 0.0f);
+        }
+#define HK_TRIPLE(qa, qb, qc, wa, wb, wc, num, den)                 \
+        const float den##_bc = (qb) * (qc);                          \
+        const float num = fmaf(fmaf((wb), (qc), (wc) * (qb)), (qa), (wa) * den##_bc); \
+        const float den = (qa) * den##_bc;
+        HK_TRIPLE(q[0].x, q[0].y, q[1].x, w0.x, w0.y, w0.z, n0, d0)
+        HK_TRIPLE(q[1].y, q[2].x, q[2].y, w0.w, w1.x, w1.y, n1, d1)
+        HK_TRIPLE(q[3].x, q[3].y, q[4].x, w1.z, w1.w, w2.x, n2, d2)
+        HK_TRIPLE(q[4].y, q[5].x, q[5].y, w2.y, w2.z, w2.w, n3, d3)
+#undef HK_TRIPLE
+        sum = n0 * rcp_approx(d0);
+        sum = fmaf(n1, rcp_approx(d1), sum);
+        sum = fmaf(n2, rcp_approx(d2), sum);
+        num3 = n3; den3 = d3;
     }
     // pole term over the last triple's denominator
     const float g = __expf(-x * x);
@@ -332,7 +336,7 @@ __device__ __forceinline__ float trap_K(float x, const TrapLine& L, const float*
     const float top = fmaf(L.yk * num3, pd, pn * den3);
     return fmaf(sum, L.yk, top * rcp_approx(den3 * pd));
 }
-__device__ __noinline__ float core_K(float x, float y) { return trap_K(x, trap_line(y), nullptr); }
+__device__ __noinline__ float core_K(float x, float y) { return trap_K<false>(x, trap_line(y), nullptr); }
 
 __device__ __forceinline__ float core_any_K(float x, float y, int* region)
 {
