@@ -267,7 +267,7 @@ def _kernel_flops(st):
     g10_lane = st["n_evals_gh10"] - g10_row
     kb = st["bins_per_lane"]
     return {
-        "node": ("node_kernel", FLOP["mid"] * st["n_pairs_node"] * HK_NODES),
+        "node": ("node_kernel", (FLOP["mid"] * (st["n_pairs_node"] - st["n_pairs_node_far"]) + FLOP["far"] * st["n_pairs_node_far"]) * HK_NODES),
         "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
         "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
         # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end

@@ -709,27 +709,45 @@ __global__ void __launch_bounds__(kThreads, kNodeCtas) node_kernel(AccArgs a)
             xk[m] = make_float2((float)(hc + hw * kChebX[2 * m]), (float)(hc + hw * kChebX[2 * m + 1]));
             acc[m] = make_float2(0.f, 0.f);
         }
-        for (int v = v_lo + (int)threadIdx.x; v < v_hi; v += kThreads) {
+        for (int v0 = v_lo + 32 * warp; v0 < v_hi; v0 += kThreads) {        // (warp-uniform trip count)
+            const int v = v0 + lane;
+            const bool live = v < v_hi;
             const int li = v < s0 ? r.a0 + v
                          : v < s0 + s1 ? r.b0 + (v - s0)
                          : v < s0 + s1 + s2 ? r.c0 + (v - s0 - s1) : r.d0 + (v - s0 - s1 - s2);
-            const float4 rec = a.recN[li];
+            float4 rec = make_float4(0.f, 0.f, 1.f, 0.f);
+            if (live) rec = a.recN[li];
             const uint32_t pk = (uint32_t)__float_as_int(rec.y);
             const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
-            const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
             const float npos = -((float)((int64_t)__float_as_int(rec.x) - tile0) + f);
-            const float2 np2 = bcast2(npos), g2 = bcast2(rec.z), c2 = bcast2(rec.w), one = bcast2(1.0f);
-            const float2 A1 = bcast2(1.5f * a2), nA2 = bcast2(-2.0f * a2 * rec.z);
+            const float2 np2 = bcast2(npos), g2 = bcast2(rec.z), c2 = bcast2(rec.w);
+            // far from the tile (|z|^2 >= Z1 on all of it: a prefix of the left lists, a suffix of the right ones): the
+            // Lorentzian alone.  The lines of a warp are neighbours in the sorted order, so a warp is almost always all far
+            // or all near; in a mixed warp the far lines run the two-term form with a^2 = 0, which is the same value bit
+            // for bit -- what a (line, tile) pair contributes never depends on its neighbours
+            const bool far = !live || li < r.fL || li >= r.fR;
+            if (__all_sync(0xffffffffu, far)) {
 #pragma unroll
-            for (int m = 0; m < M; ++m) {
-                const float2 t = __fadd2_rn(xk[m], np2);
-                const float2 q = __ffma2_rn(t, t, g2);
-                const float R = rcp_approx(q.x * q.y);             // 1/q.x = R q.y, 1/q.y = R q.x
-                const float2 rr = make_float2(R * q.y, R * q.x);
-                const float2 uu = __ffma2_rn(nA2, rr, A1);
-                const float2 vv = __ffma2_rn(uu, rr, one);
-                const float2 ww = __fmul2_rn(rr, vv);
-                acc[m] = __ffma2_rn(c2, ww, acc[m]);
+                for (int m = 0; m < M; ++m) {
+                    const float2 t = __fadd2_rn(xk[m], np2);
+                    const float2 q = __ffma2_rn(t, t, g2);
+                    const float R = rcp_approx(q.x * q.y);             // 1/q.x = R q.y, 1/q.y = R q.x
+                    acc[m] = __ffma2_rn(c2, make_float2(R * q.y, R * q.x), acc[m]);
+                }
+            } else {
+                const float a2 = far ? 0.f : __int_as_float((int)((pk & 0x7FFFFu) << 12));
+                const float2 one = bcast2(1.0f), A1 = bcast2(1.5f * a2), nA2 = bcast2(-2.0f * a2 * rec.z);
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    const float2 t = __fadd2_rn(xk[m], np2);
+                    const float2 q = __ffma2_rn(t, t, g2);
+                    const float R = rcp_approx(q.x * q.y);             // 1/q.x = R q.y, 1/q.y = R q.x
+                    const float2 rr = make_float2(R * q.y, R * q.x);
+                    const float2 uu = __ffma2_rn(nA2, rr, A1);
+                    const float2 vv = __ffma2_rn(uu, rr, one);
+                    const float2 ww = __fmul2_rn(rr, vv);
+                    acc[m] = __ffma2_rn(c2, ww, acc[m]);
+                }
             }
         }
 #pragma unroll

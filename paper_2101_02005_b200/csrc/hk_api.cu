@@ -1034,6 +1034,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->sort_bits = ctx->last_sort_bits;
     host_out->n_plinth_illcond = (int64_t)d.n_plinth_illcond;
     host_out->n_unsorted = (int64_t)d.n_unsorted;
+    host_out->n_pairs_node_far = (int64_t)d.pairs_node_far;
     host_out->n_evals_gh10_row = (int64_t)d.n_cnt_gh10_row;
     if (ctx->host_totals) {
         DevTotals t;

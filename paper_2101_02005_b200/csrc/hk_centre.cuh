@@ -536,32 +536,43 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                 bmax = fmaxf(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
             }
             if (bmax < bmin) return;
-            const TrapLine TL = trap_line(type == kLaneTrap ? y : 1.0f);   // what the trapezoid rule needs of the line alone
+            TrapLine TL = trap_line(type == kLaneTrap ? y : 1.0f);   // what the trapezoid rule needs of the line alone
+            asm volatile("" : "+f"(TL.ie), "+f"(TL.amp0));           // (kept in registers: not recomputed per bin)
+            // groups are sorted by evaluator: when every live lane of the group runs the trapezoid rule (the common case) the
+            // bin loop is compiled without the dispatch
+            const bool all_trap = !kBinned && __all_sync(0xffffffffu, type == kLaneTrap || type == kLaneNone);
             const int b_end = (int)bmax;
             const int col = lane & (kStage - 1), half = lane >> 4;
+            auto bins = [&](auto trap_only) {
+                constexpr bool kTrapOnly = decltype(trap_only)::value;
 #pragma unroll 1
-            for (int b0 = (int)bmin; b0 <= b_end; b0 += kStage) {
-                const int ns = min(kStage, b_end - b0 + 1);              // steps of this block (warp-uniform)
-                const float e0 = (float)b0 - dl;                         // exact (small integers)
+                for (int b0 = (int)bmin; b0 <= b_end; b0 += kStage) {
+                    const int ns = min(kStage, b_end - b0 + 1);              // steps of this block (warp-uniform)
+                    float d = (float)b0 - dl;                                // exact (small integers)
 #pragma unroll 2
-                for (int s = 0; s < ns; ++s) {
-                    const float d = e0 + (float)s;
-                    const float un = __fmaf_rn(d, inva, nfa);            // the row pass's u and X, bit for bit
-                    const float X = __fmul_rn(un, un);
-                    float val = 0.f;
-                    if (X < xl) val = kBinned ? cK * binned_K(d, f, y2, inva) : lane_value(type, cK, fabsf(un), X, y, y2, TL, wtab);
-                    stage[warp][s][lane] = val;
-                }
-                __syncwarp();
-                float sum = 0.f;
-                if (col < ns) {
+                    for (int s = 0; s < ns; ++s, d += 1.0f) {
+                        const float un = __fmaf_rn(d, inva, nfa);            // the row pass's u and X, bit for bit
+                        const float X = __fmul_rn(un, un);
+                        float val = 0.f;
+                        if (X < xl) {
+                            if (kTrapOnly) val = cK * trap_K<true>(fabsf(un), TL, wtab);
+                            else val = kBinned ? cK * binned_K(d, f, y2, inva) : lane_value(type, cK, fabsf(un), X, y, y2, TL, wtab);
+                        }
+                        stage[warp][s][lane] = val;
+                    }
+                    __syncwarp();
+                    float sum = 0.f;
+                    if (col < ns) {
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) sum += stage[warp][col][half * 16 + j];
+                        for (int j = 0; j < 16; ++j) sum += stage[warp][col][half * 16 + j];
+                    }
+                    sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+                    if (half == 0 && col < ns) sacc[warp][b0 + col] += sum;
+                    __syncwarp();
                 }
-                sum += __shfl_xor_sync(0xffffffffu, sum, 16);
-                if (half == 0 && col < ns) sacc[warp][b0 + col] += sum;
-                __syncwarp();
-            }
+            };
+            if (all_trap) bins(std::true_type());
+            else bins(std::false_type());
             since_flush += 32;     // the bin tile holds at most 32 lines' terms per bin per group
             if (since_flush >= kFlush) flush();
         };

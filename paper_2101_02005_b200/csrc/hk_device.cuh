@@ -56,8 +56,10 @@ struct __align__(8) TileRange {
 };
 
 // per (level, tile) entry of the node hierarchy: four index ranges of sorted lines evaluated at the tile's nodes
-struct __align__(16) NodeRange {
+struct __align__(8) NodeRange {
     int32_t a0, a1, b0, b1, c0, c1, d0, d1;
+    int32_t fL, fR;      // lines with index < fL (left ranges) or >= fR (right ranges) have |z|^2 >= Z1 on the whole tile:
+                         // one asymptotic term is enough (the lists are sorted by centre, so far lines are a prefix / suffix)
 };
 
 // ---- Chebyshev nodes of the separated-tile evaluation ----------------

@@ -82,6 +82,7 @@ struct DevStats {
     unsigned long long pairs_edge_node;                    // (line, extent end) pairs evaluated at the nodes of their edge tile
     unsigned long long pairs_node;                         // (line, tile) pairs evaluated at nodes
     unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
+    unsigned long long pairs_node_far;                     // of pairs_node: |z|^2 >= Z1 on the whole tile (one asymptotic term)
     unsigned long long shift_bits;                         // max |delta P| over the lines (cm^-1) as double bits (pressure shift)
     unsigned long long n_plinth_illcond;                   // plinth removal: lines whose cutting length falls inside their core
     unsigned long long n_unsorted;                         // adjacent pairs of valid lines out of centre-bin order (input order)
@@ -511,10 +512,16 @@ __global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, co
     r.b0 = min(b, max(r.a1, pb)); r.b1 = b;       // left main: closer than the parent's separation
     r.c0 = c; r.c1 = max(c, min(d, pc));          // right main
     r.d0 = min(d, max(r.c1, pd)); r.d1 = d;       // right sliver
+    // where one asymptotic term suffices on the whole tile (|z|^2 >= Z1): the same bound range_kernel uses for "far"
+    r.fL = idx_of(p, keys, n_act, left_bound((double)w0, p.kappa1, p.inv1p_k1, p.numin_bins) + 1);
+    r.fR = idx_of(p, keys, n_act, right_bound((double)(min(p.N, w0 + W) - 1), p.kappa1, p.inv1m_k1, p.numin_bins));
     nr[e] = r;
     const int64_t tot = (int64_t)(r.a1 - r.a0) + (r.b1 - r.b0) + (r.c1 - r.c0) + (r.d1 - r.d0);
     counts[e] = (int32_t)((tot + p.chunk_node - 1) / p.chunk_node);
     if (tot) {
+        const int64_t nfar = (int64_t)max(0, min(r.a1, r.fL) - r.a0) + max(0, min(r.b1, r.fL) - r.b0)
+                           + max(0, r.c1 - max(r.c0, r.fR)) + max(0, r.d1 - max(r.d0, r.fR));
+        if (nfar) atomicAdd(&st->pairs_node_far, (unsigned long long)nfar);
         atomicAdd(&st->pairs_node, (unsigned long long)tot);
         atomicAdd(&st->bins_node, (unsigned long long)tot * (unsigned long long)(min(p.N, w0 + W) - w0));
     }
