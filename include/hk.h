@@ -85,6 +85,7 @@ typedef struct {
     int64_t n_plinth_illcond; /* plinth removal: lines with V(cut) > V(0) / HK_PLINTH_RATIO, whose difference V - V(cut) is
                                  ill-conditioned in fp32 (see hk_set_plinth: 0 means the subtracted result meets the tolerance) */
     int64_t n_evals_gh10_row; /* of n_evals_gh10: evaluated by the row kernel (lines at least 0.85 bins wide per 64 bins of tile); the rest by the lane kernel */
+    int64_t n_pairs_node_eval; /* (line, tile) pairs the node kernel evaluated; equals n_pairs_node (checked by the tests) */
     int64_t n_pairs_node_far; /* of n_pairs_node: |z|^2 >= HK_Z1 on the whole tile, evaluated with one asymptotic term */
     int64_t n_unsorted;    /* adjacent pairs of the input list out of centre-bin order (0: the list arrived sorted and the
                               radix sort was skipped on the device) */

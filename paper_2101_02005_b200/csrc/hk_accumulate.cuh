@@ -782,6 +782,61 @@ __global__ void __launch_bounds__(kThreads, kNodeCtas) node_kernel(AccArgs a)
 // one lane issues the fp64 atomics.  edge_scan_kernel turns the accumulators into suffix (side 0) / prefix (side 1)
 // sums over each tile, edge_bins_kernel interpolates them onto the bins.  The sum of interpolants over any subset of
 // lines is the interpolant of that subset's node sums, so the per-bin subsets cost nothing extra.
+// Sum kP per-lane values over the lanes with `mine` set and add the kP sums to dst[0..kP) (fp64 atomics).
+// Transposing reduction: each exchange halves the values a lane carries (8 -> 4 -> 2 -> 1 over lane bits 4, 3, 2), two
+// butterfly steps finish bits 1, 0: 9 shuffles instead of 40.  Lane l then holds the sum of value j = (bit4, bit3, bit2
+// of l); the lanes with l % 4 == 0 issue one atomic each.  Nodes beyond the first eight (kP = 10, 12) go through a
+// second, shorter fold of the same kind.  Called by all 32 lanes.
+__device__ __forceinline__ void warp_fold_add(double* __restrict__ dst, const float (&v)[kP], bool mine, int lane)
+{
+    static_assert(kP == 8 || kP == 10 || kP == 12, "the folds below are written for 8, 10 or 12 nodes");
+    float a[8], b4[4], c2[2];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = mine ? v[j] : 0.f;
+    const bool h4 = (lane & 16) != 0, h3 = (lane & 8) != 0, h2 = (lane & 4) != 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float send = h4 ? a[j] : a[j + 4], keep = h4 ? a[j + 4] : a[j];
+        b4[j] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const float send = h3 ? b4[j] : b4[j + 2], keep = h3 ? b4[j + 2] : b4[j];
+        c2[j] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    float d = (h2 ? c2[1] : c2[0]) + __shfl_xor_sync(0xffffffffu, h2 ? c2[0] : c2[1], 4);
+    d += __shfl_xor_sync(0xffffffffu, d, 2);
+    d += __shfl_xor_sync(0xffffffffu, d, 1);
+    const int j = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+    if ((lane & 3) == 0 && d != 0.f) atomicAdd(dst + j, (double)d);
+    if constexpr (kP == 12) {
+        // values 8..11: 4 -> 2 -> 1 over lane bits 4, 3, then three butterfly steps; lane l holds j = 8 + (bit4, bit3)
+        float e[4], f2[2];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) e[q] = mine ? v[8 + q] : 0.f;
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const float send = h4 ? e[q] : e[q + 2], keep = h4 ? e[q + 2] : e[q];
+            f2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+        }
+        float g = (h3 ? f2[1] : f2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? f2[0] : f2[1], 8);
+        g += __shfl_xor_sync(0xffffffffu, g, 4);
+        g += __shfl_xor_sync(0xffffffffu, g, 2);
+        g += __shfl_xor_sync(0xffffffffu, g, 1);
+        const int jj = 8 + ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
+        if ((lane & 7) == 0 && g != 0.f) atomicAdd(dst + jj, (double)g);
+    } else if constexpr (kP == 10) {
+        // values 8, 9: 2 -> 1 over lane bit 4, then four butterfly steps; lane l holds j = 8 + bit4
+        const float e0 = mine ? v[8] : 0.f, e1 = mine ? v[kP - 1] : 0.f;
+        float g = (h4 ? e1 : e0) + __shfl_xor_sync(0xffffffffu, h4 ? e0 : e1, 16);
+        g += __shfl_xor_sync(0xffffffffu, g, 8);
+        g += __shfl_xor_sync(0xffffffffu, g, 4);
+        g += __shfl_xor_sync(0xffffffffu, g, 2);
+        g += __shfl_xor_sync(0xffffffffu, g, 1);
+        if ((lane & 15) == 0 && g != 0.f) atomicAdd(dst + 8 + ((lane >> 4) & 1), (double)g);
+    }
+}
+
 __device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_t bin, const float (&v)[kP], int lane)
 {
     unsigned todo = __ballot_sync(0xffffffffu, bin >= 0);
@@ -796,59 +851,218 @@ __device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_
                 for (int j = 0; j < kP; ++j) atomicAdd(acc + (size_t)b * kP + j, (double)v[j]);
             }
         } else {
-            // transposing reduction: each exchange halves the values a lane carries (8 -> 4 -> 2 -> 1 over lane bits
-            // 4, 3, 2), two butterfly steps finish bits 1, 0: 9 shuffles instead of 40.  Lane l then holds the sum of
-            // value j = (bit4, bit3, bit2 of l); the lanes with l % 4 == 0 issue one atomic each.  Nodes beyond the
-            // first eight (kP = 10, 12) go through a second, shorter fold of the same kind.
-            static_assert(kP == 8 || kP == 10 || kP == 12, "the folds below are written for 8, 10 or 12 nodes");
-            float a[8], b4[4], c2[2];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) a[j] = mine ? v[j] : 0.f;
-            const bool h4 = (lane & 16) != 0, h3 = (lane & 8) != 0, h2 = (lane & 4) != 0;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const float send = h4 ? a[j] : a[j + 4], keep = h4 ? a[j + 4] : a[j];
-                b4[j] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-            }
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                const float send = h3 ? b4[j] : b4[j + 2], keep = h3 ? b4[j + 2] : b4[j];
-                c2[j] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-            }
-            float d = (h2 ? c2[1] : c2[0]) + __shfl_xor_sync(0xffffffffu, h2 ? c2[0] : c2[1], 4);
-            d += __shfl_xor_sync(0xffffffffu, d, 2);
-            d += __shfl_xor_sync(0xffffffffu, d, 1);
-            const int j = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-            if ((lane & 3) == 0) atomicAdd(acc + (size_t)b * kP + j, (double)d);
-            if constexpr (kP == 12) {
-                // values 8..11: 4 -> 2 -> 1 over lane bits 4, 3, then three butterfly steps; lane l holds j = 8 + (bit4, bit3)
-                float e[4], f2[2];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) e[q] = mine ? v[8 + q] : 0.f;
-#pragma unroll
-                for (int q = 0; q < 2; ++q) {
-                    const float send = h4 ? e[q] : e[q + 2], keep = h4 ? e[q + 2] : e[q];
-                    f2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-                }
-                float g = (h3 ? f2[1] : f2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? f2[0] : f2[1], 8);
-                g += __shfl_xor_sync(0xffffffffu, g, 4);
-                g += __shfl_xor_sync(0xffffffffu, g, 2);
-                g += __shfl_xor_sync(0xffffffffu, g, 1);
-                const int jj = 8 + ((lane >> 4) & 1) * 2 + ((lane >> 3) & 1);
-                if ((lane & 7) == 0) atomicAdd(acc + (size_t)b * kP + jj, (double)g);
-            } else if constexpr (kP == 10) {
-                // values 8, 9: 2 -> 1 over lane bit 4, then four butterfly steps; lane l holds j = 8 + bit4
-                const float e0 = mine ? v[8] : 0.f, e1 = mine ? v[kP - 1] : 0.f;
-                float g = (h4 ? e1 : e0) + __shfl_xor_sync(0xffffffffu, h4 ? e0 : e1, 16);
-                g += __shfl_xor_sync(0xffffffffu, g, 8);
-                g += __shfl_xor_sync(0xffffffffu, g, 4);
-                g += __shfl_xor_sync(0xffffffffu, g, 2);
-                g += __shfl_xor_sync(0xffffffffu, g, 1);
-                if ((lane & 15) == 0) atomicAdd(acc + (size_t)b * kP + 8 + ((lane >> 4) & 1), (double)g);
-            }
+            warp_fold_add(acc + (size_t)b * kP, v, mine, lane);
         }
         todo &= ~grp;
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// node kernel, line-stationary form: a CTA keeps a chunk of consecutive sorted lines in shared memory and walks the
+// (level, tile) entries those lines are evaluated at
+// ---------------------------------------------------------------------------------------
+// node_kernel above is entry-stationary: a work unit is (entry, chunk of its lines), every line record is fetched once
+// per entry it belongs to (~19 times) and every unit starts with a search for its entry.  Here the loop order is turned
+// round: the records of kNLChunk consecutive lines are staged ONCE (16 B per line), the entries that hold any of them
+// are found from the geometry (a generous superset of tiles per level, then the exact index ranges of NodeRange decide
+// membership, so every (line, tile) pair is evaluated exactly once, as node_range_kernel counted it), and each warp
+// walks those entries with its 256 lines, 8 per lane, before ONE fold + 12 atomics per (warp, entry).
+constexpr int kNLChunk = 2048;                    // lines per chunk
+constexpr int kNLPerLane = kNLChunk / kThreads;   // lines per lane per entry
+constexpr int kNLMaxEnt = 256;                    // entries resolved per round (one candidate per thread)
+
+struct __align__(16) NLEntry {
+    NodeRange r;
+    int32_t e, l;
+    int32_t D;           // (centre bin of the chunk's first line) - (first bin of the tile)
+    int32_t pad;
+};
+constexpr size_t kNLSmemBytes = sizeof(float4) * kNLChunk + sizeof(NLEntry) * kNLMaxEnt;
+
+// tile-index intervals [lo[i], hi[i]] (i < 3, disjoint, possibly empty) of level l that can hold lines with centre bins
+// in [jlo, jhi]; a superset -- membership is decided by NodeRange
+__device__ __forceinline__ void nl_candidates(const Params& p, const Levels& lv, int l, int64_t jlo, int64_t jhi,
+                                               int64_t (&lo)[3], int64_t (&hi)[3])
+{
+    const int64_t W = (int64_t)lv.w0 << l;
+    const int64_t nt = lv.off[l + 1] - lv.off[l];
+    const bool top = l + 1 == lv.n_levels;
+    auto tdiv = [&](int64_t b) { return b >= 0 ? b / W : -((-b + W - 1) / W); };     // floor(b / W)
+    for (int i = 0; i < 3; ++i) { lo[i] = 0; hi[i] = -1; }
+    // lines the parent does not take: closer than the parent's separation, or inside the core bound of the parent tile
+    double rc = 1.0e18;
+    if (p.kappa2 < 0.9) rc = p.kappa2 * (p.numin_bins + (double)jhi + 2.0) / (1.0 - p.kappa2) + 8.0;
+    const double ra_d = fmax((p.sep + 0.5) * (double)W, rc + 1.5 * (double)W) + (double)W + 8.0;
+    const int64_t big = (int64_t)1 << 40;
+    const int64_t RA = ra_d < (double)big ? (int64_t)ra_d : big;
+    if (p.uncut) {
+        if (top || RA >= big) { lo[0] = 0; hi[0] = nt - 1; }
+        else { lo[0] = tdiv(jlo - RA); hi[0] = tdiv(jhi + RA); }
+    } else {
+        const int64_t reach = p.cb_ceil + W + 8;
+        if (top || 2 * reach / W <= 40 || RA >= reach) { lo[0] = tdiv(jlo - reach); hi[0] = tdiv(jhi + reach); }
+        else {
+            // left extent end (the parent tile is not inside the extent, the child is), centre, right extent end
+            lo[0] = tdiv(jlo - p.cb_ceil - W - 8); hi[0] = tdiv(jhi - p.cb_floor + 2 * W + 8);
+            lo[1] = tdiv(jlo - RA);                hi[1] = tdiv(jhi + RA);
+            lo[2] = tdiv(jlo + p.cb_floor - 2 * W - 8); hi[2] = tdiv(jhi + p.cb_ceil + W + 8);
+        }
+    }
+    int64_t prev = -1;
+    for (int i = 0; i < 3; ++i) {                 // clip to the level, make disjoint (they are ordered left to right)
+        lo[i] = max(lo[i], max((int64_t)0, prev + 1));
+        hi[i] = min(hi[i], nt - 1);
+        if (hi[i] >= lo[i]) prev = hi[i];
+    }
+}
+
+__global__ void __launch_bounds__(kThreads, kNodeCtas) node_lines_kernel(Params p, AccArgs a)
+{
+    constexpr int M = kP / 2;
+    extern __shared__ __align__(16) unsigned char nl_smem[];      // kNLSmemBytes, opted in by the host (> 48 KB)
+    float4* sRec = reinterpret_cast<float4*>(nl_smem);            // [kNLChunk] recN with the centre bin relative to the chunk's first
+    NLEntry* sEnt = reinterpret_cast<NLEntry*>(nl_smem + sizeof(float4) * kNLChunk);   // [kNLMaxEnt]
+    __shared__ float sXk[kMaxLevels][kP];         // node positions of a tile of each level, relative to its first bin
+    __shared__ int64_t sLo[kMaxLevels][3], sHi[kMaxLevels][3];
+    __shared__ int sCnt[kMaxLevels + 1];          // candidates before level l
+    __shared__ int s_nent;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const Levels& lv = a.lv;
+    apply_shift_bound(p, a.st);
+    for (int i = threadIdx.x; i < lv.n_levels * kP; i += kThreads) {
+        const int l = i / kP, k = i - l * kP;
+        const int64_t W = (int64_t)lv.w0 << l;
+        sXk[l][k] = (float)(0.5 * (double)(W - 1) + 0.5 * (double)W * kChebX[k]);
+    }
+    const int n_act = a.st->n_act;
+    const int n_chunks = (n_act + kNLChunk - 1) / kNLChunk;
+    unsigned long long n_eval = 0;                // (line, tile) pairs this thread evaluated
+    for (int chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
+        const int c_lo = chunk * kNLChunk, c_hi = min(c_lo + kNLChunk, n_act);
+        const int64_t jc0 = __float_as_int(a.recN[c_lo].x), jc1 = __float_as_int(a.recN[c_hi - 1].x);
+        __syncthreads();                          // the previous chunk is done with the shared arrays
+#pragma unroll
+        for (int k = 0; k < kNLPerLane; ++k) {
+            const int i = threadIdx.x + k * kThreads;
+            float4 o = make_float4(0.f, 0.f, 1.f, 0.f);
+            if (c_lo + i < c_hi) {
+                o = a.recN[c_lo + i];
+                o.x = __int_as_float((int)((int64_t)__float_as_int(o.x) - jc0));      // (fits: the list is sorted, |jc| < 2^30)
+            }
+            sRec[i] = o;
+        }
+        if (threadIdx.x < lv.n_levels) {
+            int64_t lo[3], hi[3];
+            nl_candidates(p, lv, threadIdx.x, jc0, jc1, lo, hi);
+            for (int i = 0; i < 3; ++i) { sLo[threadIdx.x][i] = lo[i]; sHi[threadIdx.x][i] = hi[i]; }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int tot = 0;
+            for (int l = 0; l < lv.n_levels; ++l) {
+                sCnt[l] = tot;
+                for (int i = 0; i < 3; ++i) tot += (int)max((int64_t)0, sHi[l][i] - sLo[l][i] + 1);
+            }
+            sCnt[lv.n_levels] = tot;
+        }
+        __syncthreads();
+        const int n_cand = sCnt[lv.n_levels];
+        for (int round0 = 0; round0 < n_cand; round0 += kNLMaxEnt) {
+            if (threadIdx.x == 0) s_nent = 0;
+            __syncthreads();
+            const int ci = round0 + threadIdx.x;
+            if (ci < n_cand) {
+                int l = 0;
+                while (l + 1 < lv.n_levels && ci >= sCnt[l + 1]) ++l;
+                int64_t off = ci - sCnt[l], j = -1;
+                for (int i = 0; i < 3 && j < 0; ++i) {
+                    const int64_t c = max((int64_t)0, sHi[l][i] - sLo[l][i] + 1);
+                    if (off < c) j = sLo[l][i] + off; else off -= c;
+                }
+                const int e = lv.off[l] + (int)j;
+                const NodeRange r = a.nr[e];
+                auto ov = [&](int x0, int x1) { return x1 > x0 && x0 < c_hi && x1 > c_lo; };
+                if (ov(r.a0, r.a1) || ov(r.b0, r.b1) || ov(r.c0, r.c1) || ov(r.d0, r.d1)) {
+                    const int slot = atomicAdd(&s_nent, 1);
+                    NLEntry E;
+                    E.r = r; E.e = e; E.l = l; E.pad = 0;
+                    E.D = (int32_t)(jc0 - j * ((int64_t)lv.w0 << l));           // |.| < 2^31: both lie within 2^30 bins of the grid
+                    sEnt[slot] = E;
+                }
+            }
+            __syncthreads();
+            const int nent = s_nent;
+            const int wl = c_lo + warp * (32 * kNLPerLane), wh = min(wl + 32 * kNLPerLane, c_hi);
+            for (int ei = 0; ei < nent; ++ei) {
+                const NodeRange r = sEnt[ei].r;
+                auto ovw = [&](int x0, int x1) { return x1 > x0 && x0 < wh && x1 > wl; };
+                if (!(ovw(r.a0, r.a1) || ovw(r.b0, r.b1) || ovw(r.c0, r.c1) || ovw(r.d0, r.d1))) continue;   // (warp-uniform)
+                const int l = sEnt[ei].l;
+                const int D = sEnt[ei].D;
+                float2 xk[M], acc[M];
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    xk[m] = make_float2(sXk[l][2 * m], sXk[l][2 * m + 1]);
+                    acc[m] = make_float2(0.f, 0.f);
+                }
+                const float4* __restrict__ wrec = sRec + warp * (32 * kNLPerLane);
+                const int fLr = r.fL - wl, fRr = r.fR - wl;        // far boundaries relative to the warp's first line
+                // the members among this warp's lines: up to four runs [s, e) of offsets (one, in dense lists); every
+                // bound below is warp-uniform, the lanes only compare their own offset with it
+                auto run = [&](int x0, int x1) {
+                    const int s_ = max(x0, wl) - wl, e_ = min(x1, wh) - wl;
+                    if (e_ <= s_) return;
+                    if (lane == 0) n_eval += (unsigned)(e_ - s_);
+                    // far from the tile (|z|^2 >= Z1 on all of it): the Lorentzian alone; a mixed warp runs the two-term
+                    // form with a^2 = 0 for its far lines, which is the same value bit for bit
+                    const bool all_far = e_ <= fLr || s_ >= fRr, none_far = s_ >= fLr && e_ <= fRr;
+#pragma unroll 1
+                    for (int o0 = s_ & ~31; o0 < e_; o0 += 32) {
+                        const int o = o0 + lane;
+                        const bool member = o >= s_ && o < e_;
+                        const float4 rec = wrec[o];
+                        const uint32_t pk = (uint32_t)__float_as_int(rec.y);
+                        const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
+                        const float2 np2 = bcast2(-((float)(__float_as_int(rec.x) + D) + f)), g2 = bcast2(rec.z),
+                                     c2 = bcast2(member ? rec.w : 0.f);
+                        const bool far = all_far || (!none_far && (!member || o < fLr || o >= fRr));
+                        if (all_far || (!none_far && __all_sync(0xffffffffu, far))) {
+#pragma unroll
+                            for (int m = 0; m < M; ++m) {
+                                const float2 t = __fadd2_rn(xk[m], np2);
+                                const float2 q = __ffma2_rn(t, t, g2);
+                                const float R = rcp_approx(q.x * q.y);             // 1/q.x = R q.y, 1/q.y = R q.x
+                                acc[m] = __ffma2_rn(c2, make_float2(R * q.y, R * q.x), acc[m]);
+                            }
+                        } else {
+                            const float a2 = far ? 0.f : __int_as_float((int)((pk & 0x7FFFFu) << 12));
+                            const float2 one = bcast2(1.0f), A1 = bcast2(1.5f * a2), nA2 = bcast2(-2.0f * a2 * rec.z);
+#pragma unroll
+                            for (int m = 0; m < M; ++m) {
+                                const float2 t = __fadd2_rn(xk[m], np2);
+                                const float2 q = __ffma2_rn(t, t, g2);
+                                const float R = rcp_approx(q.x * q.y);
+                                const float2 rr = make_float2(R * q.y, R * q.x);
+                                const float2 uu = __ffma2_rn(nA2, rr, A1);
+                                const float2 vv = __ffma2_rn(uu, rr, one);
+                                const float2 ww = __fmul2_rn(rr, vv);
+                                acc[m] = __ffma2_rn(c2, ww, acc[m]);
+                            }
+                        }
+                    }
+                };
+                run(r.a0, r.a1); run(r.b0, r.b1); run(r.c0, r.c1); run(r.d0, r.d1);
+                float v[kP];
+#pragma unroll
+                for (int m = 0; m < M; ++m) { v[2 * m] = acc[m].x; v[2 * m + 1] = acc[m].y; }
+                warp_fold_add(a.node_acc + (size_t)sEnt[ei].e * kP, v, true, lane);
+            }
+            __syncthreads();                      // the entry list is rewritten by the next round
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) n_eval += __shfl_xor_sync(0xffffffffu, n_eval, o);
+    if (lane == 0 && n_eval) atomicAdd(&a.st->pairs_node_eval, n_eval);
 }
 
 __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys,

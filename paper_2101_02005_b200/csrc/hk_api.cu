@@ -27,6 +27,7 @@ struct hk_ctx {
     int force_kb;
     double node_sep;
     int edge_nodes;
+    int node_entry_stationary;   // test knob: the entry-stationary node kernel instead of the line-stationary one
     int plinth;
     int profile;
     int cut_mode;
@@ -549,7 +550,14 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     a.plinth_acc = p.plinth ? (double*)(ws + L.plinth_acc) : nullptr;
     a.N = ctx->N; a.n_ct = p.n_ct; a.chunk = p.chunk; a.chunk_node = p.chunk_node; a.chunk_centre = p.chunk_centre; a.chunk_lane = p.chunk_lane; a.lv = lv;
     const int grid = ctx->n_sm * 2;
-    if (lv.n_entries > 0) { node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
+    if (lv.n_entries > 0) {
+        if (ctx->node_entry_stationary) node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a);
+        else {
+            HK_CUDA(cudaFuncSetAttribute(node_lines_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNLSmemBytes));
+            node_lines_kernel<<<ctx->n_sm * kNodeCtas, kThreads, kNLSmemBytes, stream>>>(p, a);
+        }
+        ++ctx->last_launches;
+    }
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_NODE + 1], stream));
     // every CUDA call inside is checked: the first failure is returned and nothing more is enqueued
     auto launch = [&](auto kb_tag) -> cudaError_t {
@@ -1035,6 +1043,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_plinth_illcond = (int64_t)d.n_plinth_illcond;
     host_out->n_unsorted = (int64_t)d.n_unsorted;
     host_out->n_pairs_node_far = (int64_t)d.pairs_node_far;
+    host_out->n_pairs_node_eval = (int64_t)d.pairs_node_eval;
     host_out->n_evals_gh10_row = (int64_t)d.n_cnt_gh10_row;
     if (ctx->host_totals) {
         DevTotals t;

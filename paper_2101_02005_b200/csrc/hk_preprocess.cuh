@@ -73,7 +73,7 @@ struct DevStats {
     unsigned long long n_cnt_gh10_row;                                         // of n_cnt_gh10: lines wide enough for the row kernel's 10-point class
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
-    int32_t pad;
+    int32_t n_act;                                         // sorted lines with a real key (the rest carry the sentinel)
     unsigned int unit_counter_far, unit_counter_mid, unit_counter_near, unit_counter_node;
     unsigned int unit_counter_edge, unit_counter_centre, unit_counter_lane, pad2;
     unsigned long long units_far, units_mid, units_near, units_node, units_edge, units_centre;
@@ -82,6 +82,7 @@ struct DevStats {
     unsigned long long pairs_edge_node;                    // (line, extent end) pairs evaluated at the nodes of their edge tile
     unsigned long long pairs_node;                         // (line, tile) pairs evaluated at nodes
     unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
+    unsigned long long pairs_node_eval;                    // (line, tile) pairs the node kernel evaluated: must equal pairs_node
     unsigned long long pairs_node_far;                     // of pairs_node: |z|^2 >= Z1 on the whole tile (one asymptotic term)
     unsigned long long shift_bits;                         // max |delta P| over the lines (cm^-1) as double bits (pressure shift)
     unsigned long long n_plinth_illcond;                   // plinth removal: lines whose cutting length falls inside their core
@@ -484,6 +485,7 @@ __global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, co
     const int64_t W = (int64_t)lv.w0 << l;
     const int64_t w0 = j * W;
     const int32_t n_act = lower_bound_key(keys, n, (int64_t)p.ksent);
+    if (e == 0) st->n_act = n_act;
     int32_t a, b, c, d;                          // handled here or above: [a, b) on the left, [c, d) on the right
     if (l == 0) {                                // the same indices the direct kernels exclude
         const TileRange t = tr[j];

@@ -27,7 +27,20 @@ N_FUZZ = int(os.environ.get("HK_FUZZ_SEEDS", "40"))     # cases per randomised d
 
 @pytest.fixture(scope="module")
 def B():
+    """The binding, with one invariant checked on EVERY hk_get_stats of this module: the node kernel finds the entries of
+    its lines from the geometry, so the (line, tile) pairs it evaluated must be exactly the pairs node_range_kernel
+    counted -- a missed or doubled entry would show here before it shows in k(nu)."""
     from paper_2101_02005_b200 import binding
+    if not getattr(binding.Opacity, "_stats_checked", False):
+        plain = binding.Opacity.stats
+
+        def stats(self):
+            st = plain(self)
+            assert st["n_pairs_node_eval"] == st["n_pairs_node"], (st["n_pairs_node_eval"], st["n_pairs_node"])
+            return st
+
+        binding.Opacity.stats = stats
+        binding.Opacity._stats_checked = True
     return binding
 
 
