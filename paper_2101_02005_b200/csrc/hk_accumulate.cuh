@@ -1092,7 +1092,6 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
         const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
         const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
         const float2 g2 = bcast2(rn.z), c2 = bcast2(rn.w), one = bcast2(1.0f);
-        const float2 A1 = bcast2(1.5f * a2), nA2 = bcast2(-2.0f * a2 * rn.z);
 #pragma unroll 1
         for (int side = 0; side < 2; ++side) {
             const int64_t e = side == 0 ? ihi : ilo;
@@ -1102,19 +1101,38 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
             float v[kP];
 #pragma unroll
             for (int j = 0; j < kP; ++j) v[j] = 0.f;
+            // |z|^2 >= Z1 on the whole edge tile (the usual case: the extent ends many widths from the centre): one
+            // asymptotic term; a line that needs two runs the same code with its a^2, so a warp takes one path and the
+            // value of a pair never depends on its neighbours
+            const float dist = (float)(side == 0 ? T0 - jc : jc - (T0 + W - 1)) - 1.0f;
+            const bool far = !m || fmaf(dist, dist, rn.z) >= 1.001f * HK_Z1 * a2;
+            const bool all_far = __all_sync(0xffffffffu, far);
             if (m) {
                 ++npairs;
                 const float2 np2 = bcast2(-((float)(jc - T0) + f));
+                if (all_far) {
 #pragma unroll
-                for (int mm = 0; mm < M; ++mm) {
-                    const float2 t = __fadd2_rn(xk[mm], np2);
-                    const float2 q = __ffma2_rn(t, t, g2);
-                    const float R = rcp_approx(q.x * q.y);
-                    const float2 rr = make_float2(R * q.y, R * q.x);
-                    const float2 uu = __ffma2_rn(nA2, rr, A1);
-                    const float2 vv = __ffma2_rn(uu, rr, one);
-                    const float2 ww = __fmul2_rn(c2, __fmul2_rn(rr, vv));
-                    v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                    for (int mm = 0; mm < M; ++mm) {
+                        const float2 t = __fadd2_rn(xk[mm], np2);
+                        const float2 q = __ffma2_rn(t, t, g2);
+                        const float R = rcp_approx(q.x * q.y);
+                        const float2 ww = __fmul2_rn(c2, make_float2(R * q.y, R * q.x));
+                        v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                    }
+                } else {
+                    const float a2e = far ? 0.f : a2;
+                    const float2 A1 = bcast2(1.5f * a2e), nA2 = bcast2(-2.0f * a2e * rn.z);
+#pragma unroll
+                    for (int mm = 0; mm < M; ++mm) {
+                        const float2 t = __fadd2_rn(xk[mm], np2);
+                        const float2 q = __ffma2_rn(t, t, g2);
+                        const float R = rcp_approx(q.x * q.y);
+                        const float2 rr = make_float2(R * q.y, R * q.x);
+                        const float2 uu = __ffma2_rn(nA2, rr, A1);
+                        const float2 vv = __ffma2_rn(uu, rr, one);
+                        const float2 ww = __fmul2_rn(c2, __fmul2_rn(rr, vv));
+                        v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                    }
                 }
             }
             warp_add_by_bin(a.edge_acc + (size_t)side * (size_t)a.N * kP, m ? e : -1, v, lane);

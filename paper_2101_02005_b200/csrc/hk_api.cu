@@ -201,6 +201,7 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     bool compact = !p.uncut && cb < 268435456.0 && (double)c->N + 2.0 * std::ceil(cb) + 8.0 < 2147483647.0;
     p.cb_floor = p.uncut ? 0 : (int64_t)std::fmin(std::floor(cb_lo), 4.0e18);
     p.cb_ceil = p.uncut ? 0 : (int64_t)std::fmin(std::ceil(cb_hi), 4.0e18);
+    p.compact = compact ? 1 : 0;
     if (compact) {
         p.kmin = -(p.cb_ceil + 2);
         p.ksent = (int32_t)(c->N + 2 * p.cb_ceil + 6);
@@ -508,13 +509,30 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
     // a2: order by centre bin
     const int bits = bits_for((uint32_t)p.ksent);
-    ctx->last_sort_bits = bits;
     size_t cub_bytes = L.cub_bytes;
+    // compact keys (any fixed cut): counting sort with the gather fused into the scatter; the bucket array and the scan's
+    // scratch live in the radix sort's scratch, which this path does not use
+    const int64_t buckets = (int64_t)p.ksent + 2;
+    size_t scan_bytes = 0;
+    cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, (const int32_t*)nullptr, (int32_t*)nullptr, (int)buckets, stream);
+    const bool counting = p.compact && buckets < 2147483647LL && align_up((size_t)buckets * 4) + scan_bytes <= L.cub_bytes;
+    ctx->last_sort_bits = counting ? 0 : bits;
     // the order by centre bin does not depend on (T, P, Q): later conditions of a batch reuse it (hk_compute_batch)
-    if (!reuse_sort)
+    if (reuse_sort) {
+        gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, recC, p.profile);
+    } else if (counting) {
+        int32_t* hist = (int32_t*)(ws + L.cub);
+        void* scan_tmp = ws + L.cub + align_up((size_t)buckets * 4);
+        HK_CUDA(cudaMemsetAsync(hist, 0, (size_t)buckets * 4, stream));
+        key_hist_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(keys_in, n, hist, st);
+        HK_CUDA(cub::DeviceScan::ExclusiveSum(scan_tmp, scan_bytes, (const int32_t*)hist, hist, (int)buckets, stream));
+        scatter_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, keys_in, flo, n, hist, st, keys_out, idx_out, recA, recB, recN,
+                                                            recC, p.profile);
+    } else {
         HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                                 (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
-    gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, recC, p.profile);
+        gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, recC, p.profile);
+    }
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
     // a3: tile ranges, node ranges and work units.  counts = [far | mid | edge | centre | near | node | 0], one scan.
     const int n_counts = 6 * p.n_ct + lv.n_entries + 1;
@@ -528,7 +546,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
     range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_edge, cnt_centre,
                                                            cnt_near, cnt_lane, st);
-    ctx->last_launches = 5;
+    ctx->last_launches = counting && !reuse_sort ? 6 : 5;   // line, scale, (hist,) gather / scatter, range (+ node range below)
     if (lv.n_entries > 0) {
         HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
         node_range_kernel<<<(lv.n_entries + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, nr, cnt_node, st);

@@ -46,6 +46,7 @@ struct Params {
     // sort keys: key = jc - kmin in [0, ksent), ksent = sentinel for lines that contribute nothing
     int64_t kmin;
     int32_t ksent;
+    int32_t compact;            // keys span [0, ksent] with ksent ~ N + 2 cut/dnu: a counting sort by key is possible
     // tile ranges
     int64_t cb_floor, cb_ceil;  // floor/ceil of cut/dnu (bins)
     double kappa1, kappa2;      // sqrt(Z1) * beta and sqrt(Z2) * beta, slightly inflated
@@ -324,6 +325,45 @@ __global__ void scale_kernel(DevStats* st)
     st->scale_exp = e;
 }
 
+// The sorted records of one line (recA, recB, recN, recC at position `pos`) from its unsorted record.
+__device__ __forceinline__ void write_sorted_records(const RecU& r, float flo_v, bool have_flo, int e, int profile, int64_t pos,
+                                                     float4* __restrict__ recA, float4* __restrict__ recB,
+                                                     float4* __restrict__ recN, float4* __restrict__ recC)
+{
+    float cK = (float)scalbn(r.cK, e);
+    // c = cK * G a / sqrt(pi)  (Lorentz amplitude S Gamma_L/(pi dnu^2) in bin units)
+    const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
+    float G2 = gauss ? 0.f : r.G2;
+    float c = cK * sqrtf(G2 * r.a2) * 0.564189583547756f;
+    // a Lorentzian of zero (or fp32-denormal) width contributes nothing anywhere but would give 0/0 on a grid point
+    // it coincides with: keep it out with c = 0 and a harmless width
+    if (profile == HK_PROFILE_LORENTZ && !(G2 >= 1.0e-30f)) { G2 = 1.0f; c = 0.f; }
+    // a pure Lorentzian is what every formula of the accumulation kernels reduces to at alpha_D = 0 (no core,
+    // no second asymptotic term); a pure Gaussian is the Voigt function at Gamma_L = 0 (c = 0: no wings)
+    const float a2 = profile == HK_PROFILE_LORENTZ ? 0.f : r.a2;
+    const bool up = signbit(r.f);                                  // centre = (jc + 1) + f with f <= 0
+    // (binned Gaussian: G2 = 0 and c = 0 everywhere, and the free slot carries the low part of the sub-bin offset)
+    recA[pos] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, (have_flo && profile == HK_PROFILE_BINNED_GAUSSIAN) ? flo_v : G2, c);
+    recB[pos] = make_float4(a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
+    // node record: offset from jc in [0, 1) rounded to the nearest 1/8192 (|error| <= 2^-14 bins; 8192 clamps to 8191),
+    // a2 rounded to nearest at 11 mantissa bits (|error| <= 2^-12 relative, unbiased)
+    const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));
+    const uint32_t a19 = (((uint32_t)__float_as_int(a2) + 0x800u) >> 12) & 0x7FFFFu;
+    recN[pos] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), G2, c);
+    // the per-line part of the centre kernels (hk_centre.cuh): IEEE roots and quotients, once per line.
+    // ip = 1/(cK y), the reciprocal amplitude of the Gauss-Hermite rows; 0: no such rows (G = 0, or an amplitude
+    // below the range of the launch)
+    float inva = 0.f, y2 = 0.f, ip = 0.f;
+    if (a2 > 0.f) {
+        inva = __fsqrt_rn(__fdiv_rn(1.0f, a2));          // the Gaussian tail amplifies an error of x by 2 x^2
+        y2 = gauss ? 0.f : __fdiv_rn(G2, a2);
+        const float P = cK * __fsqrt_rn(y2);
+        if (P > 1.0e-30f && c != 0.f) ip = __fdiv_rn(1.0f, P);
+    }
+    recC[pos] = make_float4(inva, __fmul_rn(-r.f, inva), y2, ip);
+}
+
+// Permute by the index array of a sort (CUB path, and the later conditions of a batch, which reuse the order).
 __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ idx_sorted,
                                                      const float* __restrict__ flo, int64_t n,
                                                      const DevStats* __restrict__ st,
@@ -333,38 +373,60 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
     const int e = st->scale_exp;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const int32_t src = idx_sorted[i];
-        const RecU r = rec[src];
-        float cK = (float)scalbn(r.cK, e);
-        // c = cK * G a / sqrt(pi)  (Lorentz amplitude S Gamma_L/(pi dnu^2) in bin units)
-        const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
-        float G2 = gauss ? 0.f : r.G2;
-        float c = cK * sqrtf(G2 * r.a2) * 0.564189583547756f;
-        // a Lorentzian of zero (or fp32-denormal) width contributes nothing anywhere but would give 0/0 on a grid point
-        // it coincides with: keep it out with c = 0 and a harmless width
-        if (profile == HK_PROFILE_LORENTZ && !(G2 >= 1.0e-30f)) { G2 = 1.0f; c = 0.f; }
-        // a pure Lorentzian is what every formula of the accumulation kernels reduces to at alpha_D = 0 (no core,
-        // no second asymptotic term); a pure Gaussian is the Voigt function at Gamma_L = 0 (c = 0: no wings)
-        const float a2 = profile == HK_PROFILE_LORENTZ ? 0.f : r.a2;
-        const bool up = signbit(r.f);                                  // centre = (jc + 1) + f with f <= 0
-        // (binned Gaussian: G2 = 0 and c = 0 everywhere, and the free slot carries the low part of the sub-bin offset)
-        recA[i] = make_float4(__int_as_float(r.jc + (up ? 1 : 0)), r.f, (flo && profile == HK_PROFILE_BINNED_GAUSSIAN) ? flo[src] : G2, c);
-        recB[i] = make_float4(a2, __int_as_float(r.ilo), __int_as_float(r.ihi), cK);
-        // node record: offset from jc in [0, 1) rounded to the nearest 1/8192 (|error| <= 2^-14 bins; 8192 clamps to 8191),
-        // a2 rounded to nearest at 11 mantissa bits (|error| <= 2^-12 relative, unbiased)
-        const uint32_t f13 = min(8191u, (uint32_t)__float2int_rn((up ? 1.0f + r.f : r.f) * 8192.0f));
-        const uint32_t a19 = (((uint32_t)__float_as_int(a2) + 0x800u) >> 12) & 0x7FFFFu;
-        recN[i] = make_float4(__int_as_float(r.jc), __int_as_float((int)((f13 << 19) | a19)), G2, c);
-        // the per-line part of the centre kernels (hk_centre.cuh): IEEE roots and quotients, once per line.
-        // ip = 1/(cK y), the reciprocal amplitude of the Gauss-Hermite rows; 0: no such rows (G = 0, or an amplitude
-        // below the range of the launch)
-        float inva = 0.f, y2 = 0.f, ip = 0.f;
-        if (a2 > 0.f) {
-            inva = __fsqrt_rn(__fdiv_rn(1.0f, a2));          // the Gaussian tail amplifies an error of x by 2 x^2
-            y2 = gauss ? 0.f : __fdiv_rn(G2, a2);
-            const float P = cK * __fsqrt_rn(y2);
-            if (P > 1.0e-30f && c != 0.f) ip = __fdiv_rn(1.0f, P);
-        }
-        recC[i] = make_float4(inva, __fmul_rn(-r.f, inva), y2, ip);
+        write_sorted_records(rec[src], flo ? flo[src] : 0.f, flo != nullptr, e, profile, i, recA, recB, recN, recC);
+    }
+}
+
+// ---- counting sort by centre bin (step a2 when the keys are compact: any fixed cut) --------------------------------
+// Only the GROUPING by key matters to the accumulation kernels (their line ranges are key ranges), not the order inside
+// a key.  So: histogram of the keys -> exclusive scan -> every line takes the next free slot of its key's bucket and
+// writes its sorted records there, straight from the unsorted record (the gather is the scatter).  Lanes of a warp
+// with equal keys -- neighbours, in a list that arrives sorted -- are served by ONE atomic.  A list that is already
+// in order costs one streaming pass; nothing is decided on the host.
+__global__ void __launch_bounds__(256) key_hist_kernel(const int32_t* __restrict__ key, int64_t n, int32_t* __restrict__ hist,
+                                                       DevStats* __restrict__ st)
+{
+    const int lane = threadIdx.x & 31;
+    unsigned long long unsorted = 0;
+    const int64_t n_round = (n + 31) & ~31LL;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+        const bool live = i < n;
+        const int32_t k = live ? key[i] : -1;
+        int32_t prev = __shfl_up_sync(0xffffffffu, k, 1);
+        if (lane == 0) prev = i > 0 ? key[i - 1] : k;
+        if (live && i > 0 && k < prev) ++unsorted;
+        const unsigned peers = __match_any_sync(0xffffffffu, k);
+        if (live && lane == __ffs(peers) - 1) atomicAdd(hist + k, __popc(peers));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) unsorted += __shfl_xor_sync(0xffffffffu, unsorted, o);
+    if (lane == 0 && unsorted) atomicAdd(&st->n_unsorted, unsorted);
+}
+
+__global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ key,
+                                                      const float* __restrict__ flo, int64_t n, int32_t* __restrict__ cursor,
+                                                      const DevStats* __restrict__ st, int32_t* __restrict__ key_sorted,
+                                                      int32_t* __restrict__ idx_sorted, float4* __restrict__ recA,
+                                                      float4* __restrict__ recB, float4* __restrict__ recN,
+                                                      float4* __restrict__ recC, int profile)
+{
+    const int e = st->scale_exp;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const int64_t n_round = (n + 31) & ~31LL;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+        const bool live = i < n;
+        const int32_t k = live ? key[i] : -1;
+        const unsigned peers = __match_any_sync(0xffffffffu, k);
+        const int leader = __ffs(peers) - 1;
+        int32_t base = 0;
+        if (live && lane == leader) base = atomicAdd(cursor + k, __popc(peers));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (!live) continue;
+        const int64_t pos = (int64_t)base + __popc(peers & lt_mask);
+        key_sorted[pos] = k;
+        idx_sorted[pos] = (int32_t)i;
+        write_sorted_records(rec[i], flo ? flo[i] : 0.f, flo != nullptr, e, profile, pos, recA, recB, recN, recC);
     }
 }
 
