@@ -52,7 +52,8 @@ __device__ __forceinline__ CentreLine centre_setup(const float4 ra, const float4
 {
     constexpr float whi = (float)(32 * KB - 1);
     CentreLine L;
-    const float fdj = (float)((int64_t)__float_as_int(ra.x) - ct0);
+    // (32-bit difference: a line of this tile's centre range lies within a core radius of the tile)
+    const float fdj = (float)(__float_as_int(ra.x) - (int)ct0);
     const bool binned = profile == HK_PROFILE_BINNED_GAUSSIAN;
     L.ndl = -fdj; L.nf = -ra.y;
     L.G2 = binned ? 0.f : ra.z; L.flo = binned ? ra.z : 0.f;         // (binned: the slot carries the low part of f)
@@ -168,7 +169,7 @@ __device__ __forceinline__ float gh6_row_K(float X, float Y, float y)
 // row kernel
 // ---------------------------------------------------------------------------------------
 constexpr int kRowWarps = 8;           // warps per CTA (independent of each other)
-constexpr int kRowCtas = 5;            // resident CTAs per SM the kernel is compiled and launched for
+constexpr int kRowCtas = 4;            // resident CTAs per SM the kernel is compiled and launched for
 
 template <int KB>
 __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(AccArgs a)
@@ -184,8 +185,14 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
     //    1/P at no cost, the numerator stays in range for any amplitude, and a denominator that overflows -- a line 40
     //    orders of magnitude below the strongest -- gives a reciprocal of zero)
     __shared__ float4 rec[kRowWarps][6][32];
+    // Visits of the two heavy classes (R6m, R10) are not expanded where they are staged -- that would run ~130 divergent
+    // instructions per batch for the few lanes that need them -- but PARKED ({ ndl, nfa, inva, xl | ip }, { y^2, ip }),
+    // and expanded 32 at a time, every lane busy on the same polynomial tables, when a park fills up or the unit ends.
+    __shared__ float4 park[kRowWarps][2][2][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float4 (*rw)[32] = rec[warp];
+    float4 (*pk6)[32] = park[warp][0];
+    float4 (*pk10)[32] = park[warp][1];
     const int32_t* __restrict__ prefix = a.prefix_centre;
     const int base = prefix[0], total = prefix[a.n_ct];
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -215,15 +222,132 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
         for (int m = 0; m < M; ++m) acc[m] = make_float2(0.f, 0.f);
 #pragma unroll
         for (int j = 0; j < KB; ++j) acc64[j] = 0.0;
+        int since = 0;                          // lines whose terms the fp32 partial sums hold (at most kFlush + 64)
+        auto spill = [&]() {
+            if (since >= kFlush - 32) {
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    acc64[2 * m] += (double)acc[m].x;
+                    acc64[2 * m + 1] += (double)acc[m].y;
+                    acc[m] = make_float2(0.f, 0.f);
+                }
+                since = 0;
+            }
+        };
+        // ---- R6m: P N(X)/D(X), quintic over monic sextic, zero where X < xl; records rw[0..3][0..n)
+        auto run_r6 = [&](int n) {
+#pragma unroll 2
+            for (int l = 0; l < n; ++l) {
+                const float4 ea = rw[0][l], eb = rw[1][l], ec = rw[2][l], ed = rw[3][l];
+                const float2 ndl = bcast2(ea.x), nfa = bcast2(ea.y), ia = bcast2(ea.z);
+                const float xl = ea.w;
+                const float2 n0 = bcast2(eb.x), n1 = bcast2(eb.y), n2c = bcast2(eb.z), n3 = bcast2(eb.w);
+                const float2 n4c = bcast2(ec.x), d0 = bcast2(ec.y), d1 = bcast2(ec.z), d2 = bcast2(ec.w);
+                const float2 d3 = bcast2(ed.x), d4 = bcast2(ed.y), d5 = bcast2(ed.z), ip = bcast2(ed.w), n5 = bcast2(kGhN);
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    const float2 d = __fadd2_rn(tb[m], ndl);
+                    const float2 un = __ffma2_rn(d, ia, nfa);
+                    const float2 X = __fmul2_rn(un, un);
+                    float2 N = __ffma2_rn(n5, X, n4c);
+                    N = __ffma2_rn(N, X, n3);
+                    N = __ffma2_rn(N, X, n2c);
+                    N = __ffma2_rn(N, X, n1);
+                    N = __ffma2_rn(N, X, n0);
+                    float2 Dn = __ffma2_rn(X, ip, d5);
+                    Dn = __ffma2_rn(Dn, X, d4);
+                    Dn = __ffma2_rn(Dn, X, d3);
+                    Dn = __ffma2_rn(Dn, X, d2);
+                    Dn = __ffma2_rn(Dn, X, d1);
+                    Dn = __ffma2_rn(Dn, X, d0);
+                    float2 R = rcp2(Dn);
+                    R.x = X.x >= xl ? R.x : 0.f;                        // the lane pass owns these bins
+                    R.y = X.y >= xl ? R.y : 0.f;
+                    acc[m] = __ffma2_rn(N, R, acc[m]);
+                }
+            }
+        };
+        // ---- R10: N(X)/D'(X), degree 9 over degree 10, the whole tile (y >= 2); records rw[0..5][0..n)
+        auto run_r10 = [&](int n) {
+#pragma unroll 1
+            for (int l = 0; l < n; ++l) {
+                const float4 ea = rw[0][l], eb = rw[1][l], ec = rw[2][l], ed = rw[3][l], ee = rw[4][l], ef = rw[5][l];
+                const float2 ndl = bcast2(ea.x), nfa = bcast2(ea.y), ia = bcast2(ea.z), ip = bcast2(ea.w);
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    const float2 d = __fadd2_rn(tb[m], ndl);
+                    const float2 un = __ffma2_rn(d, ia, nfa);
+                    const float2 X = __fmul2_rn(un, un);
+                    float2 N = __ffma2_rn(bcast2(kGhN), X, bcast2(ed.x));
+                    N = __ffma2_rn(N, X, bcast2(ec.w));
+                    N = __ffma2_rn(N, X, bcast2(ec.z));
+                    N = __ffma2_rn(N, X, bcast2(ec.y));
+                    N = __ffma2_rn(N, X, bcast2(ec.x));
+                    N = __ffma2_rn(N, X, bcast2(eb.w));
+                    N = __ffma2_rn(N, X, bcast2(eb.z));
+                    N = __ffma2_rn(N, X, bcast2(eb.y));
+                    N = __ffma2_rn(N, X, bcast2(eb.x));
+                    float2 Dn = __ffma2_rn(X, ip, bcast2(ef.z));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ef.y));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ef.x));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ee.w));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ee.z));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ee.y));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ee.x));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ed.w));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ed.z));
+                    Dn = __ffma2_rn(Dn, X, bcast2(ed.y));
+                    acc[m] = __ffma2_rn(N, rcp2(Dn), acc[m]);
+                }
+            }
+        };
+        int cnt6 = 0, cnt10 = 0;                // parked visits (warp-uniform)
+        // expand the parked visits of one class into row records and evaluate them (rw must be free: call after a __syncwarp
+        // that follows its last read)
+        auto flush6 = [&]() {
+            if (lane < cnt6) {
+                const float4 p0 = pk6[0][lane], p1 = pk6[1][lane];
+                float n[5], d[6];
+                gh6_coeffs(p1.x, n, d);
+                const float ip = p1.y;
+                rw[0][lane] = p0;                                        // { ndl, nfa, inva, xl }
+                rw[1][lane] = make_float4(n[0], n[1], n[2], n[3]);
+                rw[2][lane] = make_float4(n[4], d[0] * ip, d[1] * ip, d[2] * ip);
+                rw[3][lane] = make_float4(d[3] * ip, d[4] * ip, d[5] * ip, ip);
+            }
+            __syncwarp();
+            run_r6(cnt6);
+            since += cnt6; cnt6 = 0;
+            spill();
+            __syncwarp();
+        };
+        auto flush10 = [&]() {
+            if (lane < cnt10) {
+                const float4 p0 = pk10[0][lane], p1 = pk10[1][lane];
+                float n[9], d[10];
+                gh10_coeffs(p1.x, n, d);
+                const float ip = p1.y;
+                rw[0][lane] = p0;                                        // { ndl, nfa, inva, ip }
+                rw[1][lane] = make_float4(n[0], n[1], n[2], n[3]);
+                rw[2][lane] = make_float4(n[4], n[5], n[6], n[7]);
+                rw[3][lane] = make_float4(n[8], d[0] * ip, d[1] * ip, d[2] * ip);
+                rw[4][lane] = make_float4(d[3] * ip, d[4] * ip, d[5] * ip, d[6] * ip);
+                rw[5][lane] = make_float4(d[7] * ip, d[8] * ip, d[9] * ip, 0.f);
+            }
+            __syncwarp();
+            run_r10(cnt10);
+            since += cnt10; cnt10 = 0;
+            spill();
+            __syncwarp();
+        };
 
         float4 ra = make_float4(0.f, 0.f, 1.f, 0.f), rcc = make_float4(0.f, 0.f, 0.f, 0.f);
         if (lane < nt) { ra = a.recA[c0 + lane]; rcc = a.recC[c0 + lane]; }
-        int batch = 0;
-        for (int v0 = 0; v0 < nt; v0 += 32, ++batch) {
+        for (int v0 = 0; v0 < nt; v0 += 32) {
             // ---- stage 32 lines: one per lane
             int rc = kRowNone;
-            float4 A, B, C, D, E, F;
-            A = B = C = D = E = F = make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 A, B, C, P1;
+            A = B = C = P1 = make_float4(0.f, 0.f, 0.f, 0.f);
             if (v0 + lane < nt) {
                 const CentreLine L = centre_setup<KB>(ra, rcc, ct0, a.profile);
                 rc = L.row;
@@ -234,22 +358,9 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
                     A = make_float4(L.ndl, L.nfa, L.inva, ip);
                     B = make_float4(n[0], n[1], n[2], d[3] * ip);
                     C = make_float4(d[0] * ip, d[1] * ip, d[2] * ip, 0.f);
-                } else if (rc == kRowR6m) {
-                    float n[5], d[6];
-                    gh6_coeffs(L.y2, n, d);
-                    A = make_float4(L.ndl, L.nfa, L.inva, L.xl);
-                    B = make_float4(n[0], n[1], n[2], n[3]);
-                    C = make_float4(n[4], d[0] * ip, d[1] * ip, d[2] * ip);
-                    D = make_float4(d[3] * ip, d[4] * ip, d[5] * ip, ip);
-                } else if (rc == kRowR10) {
-                    float n[9], d[10];
-                    gh10_coeffs(L.y2, n, d);
-                    A = make_float4(L.ndl, L.nfa, L.inva, ip);
-                    B = make_float4(n[0], n[1], n[2], n[3]);
-                    C = make_float4(n[4], n[5], n[6], n[7]);
-                    D = make_float4(n[8], d[0] * ip, d[1] * ip, d[2] * ip);
-                    E = make_float4(d[3] * ip, d[4] * ip, d[5] * ip, d[6] * ip);
-                    F = make_float4(d[7] * ip, d[8] * ip, d[9] * ip, 0.f);
+                } else if (rc == kRowR6m || rc == kRowR10) {
+                    A = make_float4(L.ndl, L.nfa, L.inva, rc == kRowR6m ? L.xl : ip);
+                    P1 = make_float4(L.y2, ip, 0.f, 0.f);
                 } else if (rc == kRowR2 || rc == kRowR2m) {
                     const float a2 = L.inva > 0.f ? rcp_approx(L.inva * L.inva) : 0.f;   // (second-order term only)
                     A = make_float4(L.ndl, L.nf, L.G2, L.c);
@@ -263,18 +374,20 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
             const unsigned m4 = __ballot_sync(0xffffffffu, rc == kRowR4), m6 = __ballot_sync(0xffffffffu, rc == kRowR6m);
             const unsigned m10 = __ballot_sync(0xffffffffu, rc == kRowR10);
             const int n2 = __popc(m2), n2m = __popc(m2m), n4 = __popc(m4), n6 = __popc(m6), n10 = __popc(m10);
+            __syncwarp();                       // the previous batch's records are consumed
+            // park the heavy visits (a park that would overflow is worked off first)
+            if (cnt6 + n6 > 32) flush6();
+            if (cnt10 + n10 > 32) flush10();
+            if (rc == kRowR6m) { const int s = cnt6 + __popc(m6 & lt_mask); pk6[0][s] = A; pk6[1][s] = P1; }
+            if (rc == kRowR10) { const int s = cnt10 + __popc(m10 & lt_mask); pk10[0][s] = A; pk10[1][s] = P1; }
+            cnt6 += n6; cnt10 += n10;
             int slot = -1;
             if (rc == kRowR2) slot = __popc(m2 & lt_mask);
             else if (rc == kRowR2m) slot = n2 + __popc(m2m & lt_mask);
             else if (rc == kRowR4) slot = n2 + n2m + __popc(m4 & lt_mask);
-            else if (rc == kRowR6m) slot = n2 + n2m + n4 + __popc(m6 & lt_mask);
-            else if (rc == kRowR10) slot = n2 + n2m + n4 + n6 + __popc(m10 & lt_mask);
-            __syncwarp();                       // the previous batch's records are consumed
             if (slot >= 0) {
                 rw[0][slot] = A; rw[1][slot] = B;
                 if (rc >= kRowR2m) rw[2][slot] = C;
-                if (rc >= kRowR6m) rw[3][slot] = D;
-                if (rc == kRowR10) { rw[4][slot] = E; rw[5][slot] = F; }
             }
             __syncwarp();
             int l = 0;
@@ -343,81 +456,13 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
                     acc[m] = __ffma2_rn(N, rcp2(Dn), acc[m]);
                 }
             }
-            // ---- R6m: P N(X)/D(X), quintic over monic sextic, zero where X < xl
-            const int e6 = e4 + n6;
-#pragma unroll 2
-            for (; l < e6; ++l) {
-                const float4 ea = rw[0][l], eb = rw[1][l], ec = rw[2][l], ed = rw[3][l];
-                const float2 ndl = bcast2(ea.x), nfa = bcast2(ea.y), ia = bcast2(ea.z);
-                const float xl = ea.w;
-                const float2 n0 = bcast2(eb.x), n1 = bcast2(eb.y), n2c = bcast2(eb.z), n3 = bcast2(eb.w);
-                const float2 n4c = bcast2(ec.x), d0 = bcast2(ec.y), d1 = bcast2(ec.z), d2 = bcast2(ec.w);
-                const float2 d3 = bcast2(ed.x), d4 = bcast2(ed.y), d5 = bcast2(ed.z), ip = bcast2(ed.w), n5 = bcast2(kGhN);
-#pragma unroll
-                for (int m = 0; m < M; ++m) {
-                    const float2 d = __fadd2_rn(tb[m], ndl);
-                    const float2 un = __ffma2_rn(d, ia, nfa);
-                    const float2 X = __fmul2_rn(un, un);
-                    float2 N = __ffma2_rn(n5, X, n4c);
-                    N = __ffma2_rn(N, X, n3);
-                    N = __ffma2_rn(N, X, n2c);
-                    N = __ffma2_rn(N, X, n1);
-                    N = __ffma2_rn(N, X, n0);
-                    float2 Dn = __ffma2_rn(X, ip, d5);
-                    Dn = __ffma2_rn(Dn, X, d4);
-                    Dn = __ffma2_rn(Dn, X, d3);
-                    Dn = __ffma2_rn(Dn, X, d2);
-                    Dn = __ffma2_rn(Dn, X, d1);
-                    Dn = __ffma2_rn(Dn, X, d0);
-                    float2 R = rcp2(Dn);
-                    R.x = X.x >= xl ? R.x : 0.f;                        // the lane pass owns these bins
-                    R.y = X.y >= xl ? R.y : 0.f;
-                    acc[m] = __ffma2_rn(N, R, acc[m]);
-                }
-            }
-            // ---- R10: N(X)/D'(X), degree 9 over degree 10, the whole tile (y >= 2)
-            const int e10 = e6 + n10;
-#pragma unroll 1
-            for (; l < e10; ++l) {
-                const float4 ea = rw[0][l], eb = rw[1][l], ec = rw[2][l], ed = rw[3][l], ee = rw[4][l], ef = rw[5][l];
-                const float2 ndl = bcast2(ea.x), nfa = bcast2(ea.y), ia = bcast2(ea.z), ip = bcast2(ea.w);
-#pragma unroll
-                for (int m = 0; m < M; ++m) {
-                    const float2 d = __fadd2_rn(tb[m], ndl);
-                    const float2 un = __ffma2_rn(d, ia, nfa);
-                    const float2 X = __fmul2_rn(un, un);
-                    float2 N = __ffma2_rn(bcast2(kGhN), X, bcast2(ed.x));
-                    N = __ffma2_rn(N, X, bcast2(ec.w));
-                    N = __ffma2_rn(N, X, bcast2(ec.z));
-                    N = __ffma2_rn(N, X, bcast2(ec.y));
-                    N = __ffma2_rn(N, X, bcast2(ec.x));
-                    N = __ffma2_rn(N, X, bcast2(eb.w));
-                    N = __ffma2_rn(N, X, bcast2(eb.z));
-                    N = __ffma2_rn(N, X, bcast2(eb.y));
-                    N = __ffma2_rn(N, X, bcast2(eb.x));
-                    float2 Dn = __ffma2_rn(X, ip, bcast2(ef.z));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ef.y));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ef.x));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ee.w));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ee.z));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ee.y));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ee.x));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ed.w));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ed.z));
-                    Dn = __ffma2_rn(Dn, X, bcast2(ed.y));
-                    acc[m] = __ffma2_rn(N, rcp2(Dn), acc[m]);
-                }
-            }
-            // fp32 partial sums hold at most kFlush = 128 lines' terms
-            if ((batch & 3) == 3) {
-#pragma unroll
-                for (int m = 0; m < M; ++m) {
-                    acc64[2 * m] += (double)acc[m].x;
-                    acc64[2 * m + 1] += (double)acc[m].y;
-                    acc[m] = make_float2(0.f, 0.f);
-                }
-            }
+            // fp32 partial sums hold at most kFlush + 64 lines' terms
+            since += e4;
+            spill();
         }
+        __syncwarp();
+        if (cnt6 > 0) flush6();
+        if (cnt10 > 0) flush10();
         const double sc = scalbn(1.0, -a.st->scale_exp);
 #pragma unroll
         for (int m = 0; m < M; ++m) {
