@@ -866,10 +866,12 @@ __device__ __forceinline__ void warp_add_by_bin(double* __restrict__ acc, int64_
 // round: the records of kNLChunk consecutive lines are staged ONCE (16 B per line), the entries that hold any of them
 // are found from the geometry (a generous superset of tiles per level, then the exact index ranges of NodeRange decide
 // membership, so every (line, tile) pair is evaluated exactly once, as node_range_kernel counted it), and each warp
-// walks those entries with its 256 lines, 8 per lane, before ONE fold + 12 atomics per (warp, entry).
+// walks those entries with its 512 lines, 16 per lane, before ONE fold + 12 atomics per (warp, entry).
 constexpr int kNLChunk = 2048;                    // lines per chunk
-constexpr int kNLPerLane = kNLChunk / kThreads;   // lines per lane per entry
-constexpr int kNLMaxEnt = 256;                    // entries resolved per round (one candidate per thread)
+constexpr int kNLThreads = 128;                  // threads per CTA: 4 warps of 512 lines
+constexpr int kNLCtas = 5;                       // resident CTAs per SM (40 KB of shared memory each)
+constexpr int kNLPerLane = kNLChunk / kNLThreads; // lines per lane per entry: amortises the per-(warp, entry) work
+constexpr int kNLMaxEnt = kNLThreads;            // entries resolved per round (one candidate per thread)
 
 struct __align__(16) NLEntry {
     NodeRange r;
@@ -916,7 +918,7 @@ __device__ __forceinline__ void nl_candidates(const Params& p, const Levels& lv,
     }
 }
 
-__global__ void __launch_bounds__(kThreads, kNodeCtas) node_lines_kernel(Params p, AccArgs a)
+__global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params p, AccArgs a)
 {
     constexpr int M = kP / 2;
     extern __shared__ __align__(16) unsigned char nl_smem[];      // kNLSmemBytes, opted in by the host (> 48 KB)
@@ -929,7 +931,7 @@ __global__ void __launch_bounds__(kThreads, kNodeCtas) node_lines_kernel(Params 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const Levels& lv = a.lv;
     apply_shift_bound(p, a.st);
-    for (int i = threadIdx.x; i < lv.n_levels * kP; i += kThreads) {
+    for (int i = threadIdx.x; i < lv.n_levels * kP; i += kNLThreads) {
         const int l = i / kP, k = i - l * kP;
         const int64_t W = (int64_t)lv.w0 << l;
         sXk[l][k] = (float)(0.5 * (double)(W - 1) + 0.5 * (double)W * kChebX[k]);
@@ -943,7 +945,7 @@ __global__ void __launch_bounds__(kThreads, kNodeCtas) node_lines_kernel(Params 
         __syncthreads();                          // the previous chunk is done with the shared arrays
 #pragma unroll
         for (int k = 0; k < kNLPerLane; ++k) {
-            const int i = threadIdx.x + k * kThreads;
+            const int i = threadIdx.x + k * kNLThreads;
             float4 o = make_float4(0.f, 0.f, 1.f, 0.f);
             if (c_lo + i < c_hi) {
                 o = a.recN[c_lo + i];

@@ -572,7 +572,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         if (ctx->node_entry_stationary) node_kernel<<<ctx->n_sm * kNodeCtas, kThreads, 0, stream>>>(a);
         else {
             HK_CUDA(cudaFuncSetAttribute(node_lines_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNLSmemBytes));
-            node_lines_kernel<<<ctx->n_sm * kNodeCtas, kThreads, kNLSmemBytes, stream>>>(p, a);
+            node_lines_kernel<<<ctx->n_sm * kNLCtas, kNLThreads, kNLSmemBytes, stream>>>(p, a);
         }
         ++ctx->last_launches;
     }
