@@ -623,7 +623,7 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
         };
         // sort the pool by evaluator (lines that are neighbours in centre-bin order have nearly the same centre and Doppler
         // width, so the 32 lines of a group also share ring position and width) and work it off
-        auto run_pool = [&](int n) {
+        auto run_pool = [&](int n, bool final) {
             int cls[kPPT], rk[kPPT];
             if (threadIdx.x < kYClasses) hist[threadIdx.x] = 0;
             if (threadIdx.x == 0) s_next = 0;
@@ -652,7 +652,9 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                 if (cls[k] >= 0) order[off + rk[k]] = (unsigned short)(threadIdx.x + k * kThreads);
             }
             __syncthreads();
-            const int n_grp = (n + 31) >> 5;
+            // only FULL groups are worked off before the unit's last pool: the remainder (< 32 lines, the tail of the sorted
+            // order) goes back to the front of the pool and waits for company
+            const int n_grp = final ? (n + 31) >> 5 : n >> 5;
             for (;;) {
                 int grp = 0;
                 if (lane == 0) grp = atomicAdd(&s_next, 1);
@@ -660,8 +662,12 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                 if (grp >= n_grp) break;
                 run_group(32 * grp, min(32 * grp + 32, n));
             }
+            const int rest = final ? 0 : n - 32 * n_grp;
+            float4 keepA = make_float4(0.f, 0.f, 0.f, 0.f), keepB = keepA;
+            if ((int)threadIdx.x < rest) { const int li = order[32 * n_grp + threadIdx.x]; keepA = poolA[li]; keepB = poolB[li]; }
             __syncthreads();
-            if (threadIdx.x == 0) s_pool_n = 0;
+            if ((int)threadIdx.x < rest) { poolA[threadIdx.x] = keepA; poolB[threadIdx.x] = keepB; }
+            if (threadIdx.x == 0) s_pool_n = rest;
         };
 
         if (threadIdx.x == 0) s_pool_n = 0;
@@ -683,7 +689,7 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
             if (v0 + kSubC < nt) fetch(v0 + kSubC);
             const int n = s_pool_n;
             const bool last = v0 + kSubC >= nt;
-            if (n > kCap - kSubC || (last && n > 0)) { any_work = true; run_pool(n); }
+            if (n > kCap - kSubC || (last && n > 0)) { any_work = true; run_pool(n, last); }
         }
         flush();
         __syncthreads();               // every warp is done with the staging matrix: red may overwrite it
