@@ -358,12 +358,14 @@ def _ncu_onepass(kernel_prefix):
         return None
     n = len(rows)
     mean = lambda key: sum(d.get(key, 0.0) for d in rows.values()) / n
-    g = lambda op: mean(f"smsp__sass_thread_inst_executed_op_{op}_pred_on.sum")
+    g = lambda op: mean(f"sm__sass_thread_inst_executed_op_{op}_pred_on.sum")
+    # executed FP32 lane operations: scalar FFMA / FADD / FMUL thread instructions, and the packed forms (two lanes each)
+    fl = 2.0 * g("ffma") + g("fadd") + g("fmul") + 2.0 * (2.0 * g("ffma2") + g("fadd2") + g("fmul2"))
     return {"launches": n, "dram_bytes": mean("dram__bytes_read.sum") + mean("dram__bytes_write.sum"),
-            "seconds": mean("gpu__time_duration.sum"),
-            "fp32_flop_executed": 2.0 * g("ffma") + g("fadd") + g("fmul"),
+            "seconds": mean("gpu__time_duration.sum"), "fp32_flop_executed": fl,
             "issue_active_pct": mean("smsp__issue_active.avg.pct_of_peak_sustained_active"),
-            "file": "profiles/r02_onepass_config4.csv"}
+            "fma_pipe_active_pct": mean("sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active"),
+            "file": "profiles/r02_onepass_config4.csv (command in profiles/r02_onepass_config4.md)"}
 
 
 def run_ours(args):

@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
             }
             // ---- R4: P N(X)/D(X), cubic over monic quartic
             const int e4 = e2m + n4;
-#pragma unroll 2
+#pragma unroll 4
             for (; l < e4; ++l) {
                 const float4 ea = rw[0][l], eb = rw[1][l], ec = rw[2][l];
                 const float2 ndl = bcast2(ea.x), nfa = bcast2(ea.y), ia = bcast2(ea.z), ip = bcast2(ea.w);
