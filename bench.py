@@ -345,7 +345,7 @@ def _ncu_onepass(kernel_prefix):
                 if len(r) != len(hdr) or not r[ix["ID"]].isdigit():
                     continue
                 name = r[ix["Kernel Name"]]
-                if not name.startswith(kernel_prefix):
+                if kernel_prefix not in name.split("(")[0]:
                     continue
                 v = float(r[ix["Metric Value"]].replace(",", ""))
                 unit = r[ix["Metric Unit"]]
