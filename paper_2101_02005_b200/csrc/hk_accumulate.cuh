@@ -1067,6 +1067,13 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
     if (lane == 0 && n_eval) atomicAdd(&a.st->pairs_node_eval, n_eval);
 }
 
+// Work is dealt in BLOCKS of kEdgeBlock consecutive sorted lines per warp, one side at a time: along the sorted list the end
+// bins are (nearly) non-decreasing, and in a dense list 32 consecutive lines end in the SAME bin for many batches in a
+// row.  While that lasts the lanes just keep adding their node values in registers; the transposing fold and the 12
+// atomics come once per run, when the warp-uniform bin changes (a batch whose lanes disagree goes through
+// warp_add_by_bin as before).
+constexpr int kEdgeBlock = 1024;
+
 __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys,
                                                                  int32_t n)
 {
@@ -1077,67 +1084,100 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
     __syncthreads();
     const int32_t n_act = s_nact;
     const int lane = threadIdx.x & 31;
-    const int64_t W = a.lv.w0;
+    const int W = a.lv.w0;
     const int wshift = __ffs(a.lv.w0) - 1;
     float2 xk[M];
     const double hc = 0.5 * (double)(W - 1), hw = 0.5 * (double)W;
 #pragma unroll
     for (int m = 0; m < M; ++m) xk[m] = make_float2((float)(hc + hw * kChebX[2 * m]), (float)(hc + hw * kChebX[2 * m + 1]));
     unsigned long long npairs = 0;
-    const int64_t n_round = ((int64_t)n_act + 31) & ~31LL;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
-        const bool live = i < n_act;
-        float4 rn = make_float4(0.f, 0.f, 1.f, 0.f), rb = make_float4(1.f, 0.f, __int_as_float(-1), 0.f);
-        if (live) { rn = a.recN[i]; rb = a.recB[i]; }
-        const int64_t jc = __float_as_int(rn.x), ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);
-        const uint32_t pk = (uint32_t)__float_as_int(rn.y);
-        const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
-        const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
-        const float2 g2 = bcast2(rn.z), c2 = bcast2(rn.w), one = bcast2(1.0f);
+    const int n_blocks = (n_act + kEdgeBlock - 1) / kEdgeBlock;
+    const int warps_total = gridDim.x * (kThreads / 32), warp_global = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
+    const float2 one = bcast2(1.0f);
+    for (int blk = warp_global; blk < n_blocks; blk += warps_total) {
+        const int i0 = blk * kEdgeBlock, i1 = min(i0 + kEdgeBlock, n_act);
 #pragma unroll 1
         for (int side = 0; side < 2; ++side) {
-            const int64_t e = side == 0 ? ihi : ilo;
-            bool m = live && ihi >= ilo;
-            const int64_t T0 = m ? (e >> wshift) << wshift : 0;     // level-0 tiles are 64, 128 or 256 bins
-            if (m) m = side == 0 ? (jc <= edge_key_upL(p, T0, W)) : (jc >= edge_key_dnR(p, T0, W));
-            float v[kP];
+            double* __restrict__ acc = a.edge_acc + (size_t)side * (size_t)a.N * kP;
+            float run[kP];                        // this lane's share of the current run (all lanes: bin run_bin)
+            int run_bin = -1;
 #pragma unroll
-            for (int j = 0; j < kP; ++j) v[j] = 0.f;
-            // |z|^2 >= Z1 on the whole edge tile (the usual case: the extent ends many widths from the centre): one
-            // asymptotic term; a line that needs two runs the same code with its a^2, so a warp takes one path and the
-            // value of a pair never depends on its neighbours
-            const float dist = (float)(side == 0 ? T0 - jc : jc - (T0 + W - 1)) - 1.0f;
-            const bool far = !m || fmaf(dist, dist, rn.z) >= 1.001f * HK_Z1 * a2;
-            const bool all_far = __all_sync(0xffffffffu, far);
-            if (m) {
-                ++npairs;
-                const float2 np2 = bcast2(-((float)(jc - T0) + f));
-                if (all_far) {
+            for (int j = 0; j < kP; ++j) run[j] = 0.f;
+#pragma unroll 1
+            for (int ib = i0; ib < i1; ib += 32) {
+                const int i = ib + lane;
+                const bool live = i < i1;
+                float4 rn = make_float4(0.f, 0.f, 1.f, 0.f), rb = make_float4(1.f, 0.f, __int_as_float(-1), 0.f);
+                if (live) { rn = a.recN[i]; rb = a.recB[i]; }
+                const int jc = __float_as_int(rn.x), ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);
+                const int e = side == 0 ? ihi : ilo;
+                bool m = live && ihi >= ilo;
+                const int T0 = m ? (e >> wshift) << wshift : 0;     // level-0 tiles are 64, 128 or 256 bins
+                if (m) m = side == 0 ? ((int64_t)jc <= edge_key_upL(p, T0, W)) : ((int64_t)jc >= edge_key_dnR(p, T0, W));
+                float v[kP];
 #pragma unroll
-                    for (int mm = 0; mm < M; ++mm) {
-                        const float2 t = __fadd2_rn(xk[mm], np2);
-                        const float2 q = __ffma2_rn(t, t, g2);
-                        const float R = rcp_approx(q.x * q.y);
-                        const float2 ww = __fmul2_rn(c2, make_float2(R * q.y, R * q.x));
-                        v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
-                    }
-                } else {
-                    const float a2e = far ? 0.f : a2;
-                    const float2 A1 = bcast2(1.5f * a2e), nA2 = bcast2(-2.0f * a2e * rn.z);
+                for (int j = 0; j < kP; ++j) v[j] = 0.f;
+                // |z|^2 >= Z1 on the whole edge tile (the usual case: the extent ends many widths from the centre): one
+                // asymptotic term; a line that needs two runs the same code with its a^2, so a warp takes one path and the
+                // value of a pair never depends on its neighbours
+                const uint32_t pk = (uint32_t)__float_as_int(rn.y);
+                const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
+                const float dist = (float)(side == 0 ? T0 - jc : jc - (T0 + W - 1)) - 1.0f;
+                const bool far = !m || fmaf(dist, dist, rn.z) >= 1.001f * HK_Z1 * a2;
+                const bool all_far = __all_sync(0xffffffffu, far);
+                if (m) {
+                    ++npairs;
+                    const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
+                    const float2 np2 = bcast2(-((float)(jc - T0) + f)), g2 = bcast2(rn.z), c2 = bcast2(rn.w);
+                    if (all_far) {
 #pragma unroll
-                    for (int mm = 0; mm < M; ++mm) {
-                        const float2 t = __fadd2_rn(xk[mm], np2);
-                        const float2 q = __ffma2_rn(t, t, g2);
-                        const float R = rcp_approx(q.x * q.y);
-                        const float2 rr = make_float2(R * q.y, R * q.x);
-                        const float2 uu = __ffma2_rn(nA2, rr, A1);
-                        const float2 vv = __ffma2_rn(uu, rr, one);
-                        const float2 ww = __fmul2_rn(c2, __fmul2_rn(rr, vv));
-                        v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                        for (int mm = 0; mm < M; ++mm) {
+                            const float2 t = __fadd2_rn(xk[mm], np2);
+                            const float2 q = __ffma2_rn(t, t, g2);
+                            const float R = rcp_approx(q.x * q.y);
+                            const float2 ww = __fmul2_rn(c2, make_float2(R * q.y, R * q.x));
+                            v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                        }
+                    } else {
+                        const float a2e = far ? 0.f : a2;
+                        const float2 A1 = bcast2(1.5f * a2e), nA2 = bcast2(-2.0f * a2e * rn.z);
+#pragma unroll
+                        for (int mm = 0; mm < M; ++mm) {
+                            const float2 t = __fadd2_rn(xk[mm], np2);
+                            const float2 q = __ffma2_rn(t, t, g2);
+                            const float R = rcp_approx(q.x * q.y);
+                            const float2 rr = make_float2(R * q.y, R * q.x);
+                            const float2 uu = __ffma2_rn(nA2, rr, A1);
+                            const float2 vv = __ffma2_rn(uu, rr, one);
+                            const float2 ww = __fmul2_rn(c2, __fmul2_rn(rr, vv));
+                            v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
+                        }
                     }
                 }
+                // lanes that end in the run's bin join it; if the others agree on ONE bin (the list is sorted: a batch
+                // straddles at most a bin boundary or two) the run is folded and a new one starts with them
+                const bool in_run = m && e == run_bin;
+                if (__any_sync(0xffffffffu, in_run)) {
+#pragma unroll
+                    for (int j = 0; j < kP; ++j) run[j] += in_run ? v[j] : 0.f;
+                }
+                const bool rest = m && !in_run;
+                const unsigned rest_mask = __ballot_sync(0xffffffffu, rest);
+                if (rest_mask == 0u) continue;
+                if (run_bin >= 0) {                // the run ends here: fold it
+                    warp_fold_add(acc + (size_t)run_bin * kP, run, true, lane);
+                    run_bin = -1;
+                }
+                const int e1 = __shfl_sync(0xffffffffu, e, __ffs(rest_mask) - 1);
+                if (__all_sync(0xffffffffu, !rest || e == e1)) {
+                    run_bin = e1;
+#pragma unroll
+                    for (int j = 0; j < kP; ++j) run[j] = rest ? v[j] : 0.f;
+                } else {
+                    warp_add_by_bin(acc, rest ? (int64_t)e : -1, v, lane);
+                }
             }
-            warp_add_by_bin(a.edge_acc + (size_t)side * (size_t)a.N * kP, m ? e : -1, v, lane);
+            if (run_bin >= 0) warp_fold_add(acc + (size_t)run_bin * kP, run, true, lane);
         }
     }
 #pragma unroll
