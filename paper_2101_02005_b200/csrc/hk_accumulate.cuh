@@ -1067,12 +1067,12 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
     if (lane == 0 && n_eval) atomicAdd(&a.st->pairs_node_eval, n_eval);
 }
 
-// Work is dealt in BLOCKS of kEdgeBlock consecutive sorted lines per warp, one side at a time: along the sorted list the end
+// Work is dealt in BLOCKS of kEdgeBlock consecutive sorted lines per warp (small enough for the second side to find the records in cache), one side at a time: along the sorted list the end
 // bins are (nearly) non-decreasing, and in a dense list 32 consecutive lines end in the SAME bin for many batches in a
 // row.  While that lasts the lanes just keep adding their node values in registers; the transposing fold and the 12
 // atomics come once per run, when the warp-uniform bin changes (a batch whose lanes disagree goes through
 // warp_add_by_bin as before).
-constexpr int kEdgeBlock = 1024;
+constexpr int kEdgeBlock = 256;
 
 __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys,
                                                                  int32_t n)
@@ -1101,6 +1101,8 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
             double* __restrict__ acc = a.edge_acc + (size_t)side * (size_t)a.N * kP;
             float run[kP];                        // this lane's share of the current run (all lanes: bin run_bin)
             int run_bin = -1;
+            int key_T0 = -1;                      // the tile whose key threshold this lane computed last (fp64: kept)
+            int64_t key_thr = 0;
 #pragma unroll
             for (int j = 0; j < kP; ++j) run[j] = 0.f;
 #pragma unroll 1
@@ -1113,7 +1115,10 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
                 const int e = side == 0 ? ihi : ilo;
                 bool m = live && ihi >= ilo;
                 const int T0 = m ? (e >> wshift) << wshift : 0;     // level-0 tiles are 64, 128 or 256 bins
-                if (m) m = side == 0 ? ((int64_t)jc <= edge_key_upL(p, T0, W)) : ((int64_t)jc >= edge_key_dnR(p, T0, W));
+                if (m) {
+                    if (T0 != key_T0) { key_thr = side == 0 ? edge_key_upL(p, T0, W) : edge_key_dnR(p, T0, W); key_T0 = T0; }
+                    m = side == 0 ? (int64_t)jc <= key_thr : (int64_t)jc >= key_thr;
+                }
                 float v[kP];
 #pragma unroll
                 for (int j = 0; j < kP; ++j) v[j] = 0.f;
