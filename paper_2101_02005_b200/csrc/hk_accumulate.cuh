@@ -1091,11 +1091,13 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
 #pragma unroll
     for (int m = 0; m < M; ++m) xk[m] = make_float2((float)(hc + hw * kChebX[2 * m]), (float)(hc + hw * kChebX[2 * m + 1]));
     unsigned long long npairs = 0;
-    const int n_blocks = (n_act + kEdgeBlock - 1) / kEdgeBlock;
     const int warps_total = gridDim.x * (kThreads / 32), warp_global = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
+    // (short lists: smaller blocks, so that every warp of the grid has one)
+    const int blk_lines = 32 * max(1, min(kEdgeBlock / 32, n_act / (32 * warps_total)));
+    const int n_blocks = (n_act + blk_lines - 1) / blk_lines;
     const float2 one = bcast2(1.0f);
     for (int blk = warp_global; blk < n_blocks; blk += warps_total) {
-        const int i0 = blk * kEdgeBlock, i1 = min(i0 + kEdgeBlock, n_act);
+        const int i0 = blk * blk_lines, i1 = min(i0 + blk_lines, n_act);
 #pragma unroll 1
         for (int side = 0; side < 2; ++side) {
             double* __restrict__ acc = a.edge_acc + (size_t)side * (size_t)a.N * kP;

@@ -604,17 +604,17 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         }
         HK_TRY(cudaEventRecord(ctx->ev[HK_PH_CENTRE + 1], stream));
         if (p.mode == 0 || p.mode == 3) {
-            // innermost bins (lane <-> line): none for a pure Lorentzian.  Sparse lists (fewer than 256 lines per level-0
-            // tile on average) run 2- or 1-warp CTAs, four or eight times as many: a work unit there is a handful of lines
+            // innermost bins (lane <-> line): none for a pure Lorentzian.  Small CTAs: the pooled visits of a unit are dealt to
+            // the CTA's warps in groups of 32 between block-level barriers, and with 8 warps a third of them waited at
+            // those barriers (measured on config 4: 8 warps 30.0 ms, 4: 28.4, 2: 27.9, 1: 29.8).  Very sparse lists (fewer
+            // than 32 lines per level-0 tile on average) run 1-warp CTAs: a work unit there is a handful of lines
             if (p.profile != HK_PROFILE_LORENTZ) {
                 auto lanek = [&](auto binned_tag) {
                     constexpr bool kB = decltype(binned_tag)::value;
                     if ((double)n_lines * (32.0 * KB) < 32.0 * (double)ctx->N)
                         centre_lane_kernel<KB, 1, kB><<<ctx->n_sm * kLaneCtas * 8, 32, 0, stream>>>(a);
-                    else if ((double)n_lines * (32.0 * KB) < 256.0 * (double)ctx->N)
-                        centre_lane_kernel<KB, 2, kB><<<ctx->n_sm * kLaneCtas * 4, 64, 0, stream>>>(a);
                     else
-                        centre_lane_kernel<KB, 8, kB><<<ctx->n_sm * kLaneCtas, 256, 0, stream>>>(a);
+                        centre_lane_kernel<KB, 2, kB><<<ctx->n_sm * kLaneCtas * 4, 64, 0, stream>>>(a);
                 };
                 if (p.profile == HK_PROFILE_BINNED_GAUSSIAN) lanek(std::true_type());
                 else lanek(std::false_type());
