@@ -325,6 +325,9 @@ int hk_set_node_separation(hk_ctx* ctx, double sep);
 /* on (default): tiles an extent covers only in part, when separated from the line, are evaluated at the tile's nodes
  * into per-bin accumulators (128 B per bin of workspace, used while that is <= 1 GiB); off: masked direct evaluation. */
 int hk_set_edge_nodes(hk_ctx* ctx, int on);
+/* 0 (default): the line-stationary node kernel (node_lines_kernel); 1: the entry-stationary one it replaced (node_kernel).
+ * Both evaluate exactly the (line, tile) pairs node_range_kernel lists, with the same arithmetic per pair: a cross-check. */
+int hk_set_node_kernel(hk_ctx* ctx, int entry_stationary);
 
 int hk_last_cuda_error(const hk_ctx* ctx);
 const char* hk_strerror(int status);

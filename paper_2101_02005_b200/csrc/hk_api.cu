@@ -426,6 +426,13 @@ int hk_set_plinth(hk_ctx* ctx, int on)
     return HK_OK;
 }
 
+int hk_set_node_kernel(hk_ctx* ctx, int entry_stationary)
+{
+    if (!ctx) return HK_EINVAL;
+    ctx->node_entry_stationary = entry_stationary ? 1 : 0;
+    return HK_OK;
+}
+
 int hk_set_edge_nodes(hk_ctx* ctx, int on)
 {
     if (!ctx) return HK_EINVAL;

@@ -175,6 +175,29 @@ def test_edge_nodes_on_vs_off(B, cfg, n):
     assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 3e-5
 
 
+@pytest.mark.parametrize("cfg,n", [(2, 20_000), (3, 200_000), (4, 6_000), (5, 300)])
+def test_node_kernels_agree(B, cfg, n):
+    """The line-stationary node kernel against the entry-stationary one it replaced (hk_set_node_kernel): the same
+    (line, tile) pairs -- counted, and evaluated, exactly once by both -- with the same arithmetic per pair, so the two
+    spectra differ by summation order only; and the sorted-input count of the counting sort."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    ks, sts = [], []
+    for entry_stationary in (False, True):
+        op = B.Opacity(*grid)
+        op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        op.set_node_kernel(entry_stationary)
+        ks.append(op.compute(_to_cuda(lines), cut).cpu().numpy())
+        torch.cuda.synchronize()
+        sts.append(op.stats() if not entry_stationary else None)       # (only the line-stationary kernel counts its pairs)
+        op.close()
+    assert sts[0]["n_pairs_node"] > 0 and sts[0]["n_pairs_node_eval"] == sts[0]["n_pairs_node"]
+    nu0 = lines["nu0"]
+    if sts[0]["sort_bits"] == 0:             # counting sort by centre bin (compact keys, bucket array fits the scratch)
+        assert (sts[0]["n_unsorted"] == 0) == bool((nu0[1:] >= nu0[:-1]).all())
+    big = ks[1] >= 1e-8 * ks[1].max()
+    assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 1e-6
+
+
 @pytest.mark.parametrize("sep", [B_SEP_MIN, 2.0, 3.0, 4.0, 6.0])
 def test_node_separation_sweep(B, sep):
     """The node hierarchy at other separations (fewer / more pairs at nodes) against the oracle, down to the smallest
