@@ -175,6 +175,26 @@ def test_edge_nodes_on_vs_off(B, cfg, n):
     assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 3e-5
 
 
+def test_counting_sort_unsorted_input(B):
+    """Step a2 on its own path: an UNSORTED list with compact keys goes through the counting sort by centre bin (bucket
+    array in the sort scratch), most of its lines off the grid (sentinel keys: the last bucket); all bins against the oracle."""
+    lines, cond, _, cut = _mini(2, 300_000)
+    grid = (3500.0, 4000.0, 0.01)
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    dl = _to_cuda(lines)
+    k = op.compute(dl, cut).cpu().numpy()
+    torch.cuda.synchronize()
+    st = op.stats()
+    assert st["sort_bits"] == 0 and st["n_unsorted"] > 0 and st["n_off_grid"] > 100_000
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    assert st["n_evals"] == evals
+    rel, ab, frac = check_parity(k, k_ref, what="counting sort, unsorted input")
+    _check_extents(tuple(t.cpu().numpy() for t in op.extents(dl)), lines, cond, grid, cut)
+    print(f"counting sort: rel={rel:.2e} abs={ab:.2e} off grid {st['n_off_grid']}")
+    op.close()
+
+
 @pytest.mark.parametrize("cfg,n", [(2, 20_000), (3, 200_000), (4, 6_000), (5, 300)])
 def test_node_kernels_agree(B, cfg, n):
     """The line-stationary node kernel against the entry-stationary one it replaced (hk_set_node_kernel): the same
