@@ -34,9 +34,12 @@
  * w(z) is the definition.  Pinned in tests/test_oracle_faddeeva.py against
  * numerical quadrature, erfcx, the Gaussian/Lorentzian limits and the
  * asymptotic series.  y == 0 is the pure Gaussian exp(-x^2).
- * Known limit: when x sits on a node and y -> 0 the two terms cancel like
- * h/(pi y); relative accuracy ~1e-16 h/(pi y) (pinned down to y = 1e-7 in
- * tests/test_oracle_faddeeva.py).  The workloads have y >= ~1e-2.
+ * Known limit: when x sits on or next to a node and y -> 0 the node's term
+ * and the pole term cancel like h/(pi y); the phase of the pole term is
+ * formed from the distance to the nearest node, which keeps the relative
+ * accuracy at ~1e-16 h/(pi y) (pinned on and around the nodes down to
+ * y = 1e-10 in tests/test_oracle_faddeeva.py: P = 0 leaves natural widths
+ * only, y ~ 1e-9).
  *
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): w(z) as above; profile
  * area, limits and wing loss; S by a decimal hand calculation, scaling laws and
@@ -101,7 +104,12 @@ double hko_voigt_K(double x, double y)
         double phi = 2.0 * x * y;                   /* exp(-z^2) = e^{-re2} (cos phi - i sin phi) */
         double nr = amp * cos(phi), ni = -amp * sin(phi);
         double em1 = expm1(2.0 * HKO_PI * y / h);   /* e - 1, e = exp(2 pi y/h) */
-        double th = 2.0 * HKO_PI * x / h;           /* exp(-2 pi i z/h) = e (cos th - i sin th) */
+        /* exp(-2 pi i z/h) = e (cos th - i sin th), th = 2 pi x/h.  It has period h in x, so th is formed from the
+         * distance to the NEAREST node (an exact subtraction), not from x: next to a node and for y of the same size
+         * as that distance the pole term and the node's term are both ~h/(pi y) and must cancel to full precision,
+         * which the rounding of 2 pi x/h (1e-16 x 4 pi x absolute) would spoil */
+        double xr = x - h * nearbyint(x / h);
+        double th = 2.0 * HKO_PI * xr / h;
         double sh = sin(0.5 * th);
         /* 1 - e cos th written as 2 sin^2(th/2) - (e-1) cos th: no cancellation
          * when x is on a node (th = 2 pi n) and y is small */

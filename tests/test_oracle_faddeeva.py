@@ -48,6 +48,26 @@ def test_gaussian_limit():
     np.testing.assert_allclose(O.voigt_K(x, np.full_like(x, y)), np.exp(-x * x) + lin, rtol=2e-9)
 
 
+def test_near_the_trapezoid_nodes_at_tiny_y():
+    """x within ~y of a node of the oracle's own trapezoid rule (multiples of h = 1/2), y down to 1e-10: there the node
+    term and the pole term are both ~h/(pi y) and cancel, and the phase of exp(-2 pi i z/h) must be formed from the
+    DISTANCE to the nearest node, not from x (found by a P = 0 parity case: natural widths only, y ~ 1e-9, a grid point
+    1e-8 Doppler widths from x = 1: the oracle was off by 3 %).  Reference: the first-order expansion
+    K = exp(-x^2) - (2y/sqrt(pi)) (1 - 2 x D(x)) with Dawson's integral D (error O(y^2) <= 1e-16), and scipy's wofz."""
+    for node in (0.0, 0.5, 1.0, 1.5, 3.0, 5.5):
+        for d in (0.0, 1e-15, 1e-12, -1e-10, 1e-9, -1e-8, 1e-7, 1e-6, -1e-5, 1e-3):
+            for y in (1e-10, 1e-9, 8e-9, 1e-7, 1e-6, 1e-4):
+                x = abs(node + d)
+                lin = math.exp(-x * x) - 2.0 * y / math.sqrt(math.pi) * (1.0 - 2.0 * x * float(special.dawsn(x)))
+                got = float(O.voigt_K(x, y))
+                # (ON a node the two terms cancel like h/(pi y): ~1e-16 h/(pi y) relative is the rule's own limit, stated in
+                #  the oracle's header; 2e-6 at y = 1e-10 is still 50 times below the parity tolerance)
+                tol = 1e-9 + 2e-16 / y
+                if y <= 1e-6:           # (the expansion itself is good to O(y^2))
+                    assert got == pytest.approx(lin, rel=tol + 100.0 * y * y), (node, d, y)
+                assert got == pytest.approx(float(special.wofz(complex(x, y)).real), rel=tol), (node, d, y)
+
+
 def test_lorentzian_limit_and_asymptotic_series():
     # |z| -> inf: K -> y/(sqrt(pi)|z|^2) (1 + (3x^2-y^2)/(2|z|^4))
     for x, y in [(300.0, 0.5), (1e4, 2.0), (50.0, 400.0), (0.0, 1e3), (1e6, 1e-2), (2e3, 2e3)]:
