@@ -199,7 +199,11 @@ int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cu
  * values (the mass of hk_set_conditions applies to all; hk_set_conditions must have been called and its T, P, Q are
  * left untouched).  out_k_dev: DEVICE array of n_cond x N doubles, row c = k(nu) at condition c, OVERWRITTEN.
  * Every point is the full definition of hk_compute at that condition; what is shared is what does not depend on the
- * condition: the order of the lines by centre bin (one sort for the batch) and the workspace.  All conditions are
+ * condition: the order of the lines by centre bin (one sort for the batch) and the workspace -- and, between consecutive
+ * points that differ in PRESSURE only (same T and Q: the paper's pressure sweeps), everything but the Lorentz widths:
+ * strengths, Doppler widths, centre bins, extents, tile and node ranges are kept and one streaming pass rewrites
+ * (Gamma_L/dnu)^2 and what follows from it in the sorted records (plain Voigt profile, fixed cut or none, no plinth
+ * removal; otherwise the point runs the full preprocess on the shared order).  Order the points by temperature.  All conditions are
  * validated before anything is enqueued (HK_EINVAL as hk_set_conditions).  n_cond == 0 is valid.  Asynchronous like
  * hk_compute.  hk_get_stats afterwards describes the LAST condition, n_launches the whole batch. */
 int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond,

@@ -448,7 +448,7 @@ int hk_set_tile_bins(hk_ctx* ctx, int bins_per_lane)
 }
 
 static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
-                        cudaStream_t stream, bool zero_out, bool reuse_sort = false, const LineExtra* extra = nullptr,
+                        cudaStream_t stream, bool zero_out, int reuse = 0, const LineExtra* extra = nullptr,
                         const CutClass* cls = nullptr)
 {
     if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL) return HK_EINVAL;
@@ -466,8 +466,12 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     //  masked direct edge kernel takes those tiles)
     p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes && p.cut_mode == 0) ? 1 : 0;
 
+    // reuse (batched conditions on one resident list): 0 nothing, 1 the order of the lines by centre bin (any change of
+    // condition), 2 everything but the Lorentz widths (same T, Q, mass: only the pressure moved)
+    const bool reuse_sort = reuse >= 1, widths_only = reuse == 2;
     HK_CUDA(cudaEventRecord(ctx->ev[0], stream));
-    HK_CUDA(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
+    if (widths_only) reset_run_kernel<<<1, 1, 0, stream>>>(st);
+    else HK_CUDA(cudaMemsetAsync(st, 0, sizeof(DevStats), stream));
     if (zero_out) HK_CUDA(cudaMemsetAsync(out_k_dev, 0, (size_t)ctx->N * sizeof(double), stream));
     ctx->have_run = true;
     ctx->host_totals = false;
@@ -509,6 +513,15 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     ctx->last_profile = p.profile;
     ctx->last_levels = lv.n_levels;
 
+    if (widths_only) {
+        rewidth_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->A, lines->gamma_ref, lines->n_exp, idx_out, st, recA, recB,
+                                                            recN, recC);
+        HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
+        HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_SORT + 1], stream));
+        if (lv.n_entries > 0) HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
+        HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_RANGES + 1], stream));
+        ctx->last_launches = 2;
+    } else {
     // a1: per-line parameters, keys
     line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
                                                       lines->n_exp, ex, n, recU, keys_in, idx_in, flo, st);
@@ -562,6 +575,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     cub_bytes = L.cub_bytes;
     HK_CUDA(cub::DeviceScan::ExclusiveSum(ws + L.cub, cub_bytes, (const int32_t*)counts, prefix, n_counts, stream));
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_RANGES + 1], stream));
+    }
     // a4-a7: accumulate
     AccArgs a;
     a.recA = recA; a.recB = recB; a.recN = recN; a.recC = recC; a.tr = tr; a.nr = nr;
@@ -653,7 +667,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     if (p.plinth) {
         HK_CUDA(cudaMemsetAsync(a.plinth_acc, 0, (size_t)(ctx->N + 1) * sizeof(double), stream));
         plinth_kernel<<<ctx->n_sm * 8, 256, 0, stream>>>(p, a, recU, (int64_t)n);
-        cub_bytes = L.cub_bytes;
+        size_t cub_bytes = L.cub_bytes;
         HK_CUDA(cub::DeviceScan::InclusiveSum(ws + L.cub, cub_bytes, (const double*)a.plinth_acc, a.plinth_acc,
                                               (int)(ctx->N + 1), stream));
         plinth_apply_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
@@ -693,10 +707,10 @@ __global__ void __launch_bounds__(256) cut_range_kernel(Params p, const double* 
 // tile ranges and node hierarchy; the passes add into out_k.  A class keeps the ratio of the largest to the
 // smallest extent below 2, which is what the interior / node classification of a tile needs to stay useful.
 static int compute_any(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev,
-                       cudaStream_t stream, bool zero_out, bool reuse_sort = false, const LineExtra* extra = nullptr)
+                       cudaStream_t stream, bool zero_out, int reuse = 0, const LineExtra* extra = nullptr)
 {
     if (!ctx || ctx->cut_mode == 0 || is_uncut(cut_cm) || n_lines <= 0)
-        return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, stream, zero_out, reuse_sort, extra);
+        return compute_impl(ctx, lines, n_lines, cut_cm, out_k_dev, stream, zero_out, reuse, extra);
     if (!out_k_dev || n_lines >= 2147483647LL || std::isnan(cut_cm) || !lines_ok(lines)) return HK_EINVAL;
     if (!ctx->have_cond || !ctx->ws) return HK_ESTATE;
     const Layout L = make_layout(ctx, n_lines);
@@ -776,8 +790,15 @@ int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double
     int64_t launches = 0;
     for (int32_t c = 0; c < n_cond && rc == HK_OK; ++c) {
         ctx->T = T_K[c]; ctx->P_atm = P_atm[c]; ctx->Q = Q[c];
+        // what the previous condition of the batch left in the workspace is reused as far as it still holds: the order by
+        // centre bin always; everything but the Lorentz widths when only the pressure moved (plain Voigt profile, fixed cut
+        // or none, no plinth -- whose kernel reads the unsorted records)
+        int reuse = c > 0 ? 1 : 0;
+        if (c > 0 && T_K[c] == T_K[c - 1] && Q[c] == Q[c - 1] && ctx->profile == HK_PROFILE_VOIGT && !ctx->plinth &&
+            (ctx->cut_mode == 0 || is_uncut(cut_cm)) && ctx->debug_mode == 0)
+            reuse = 2;
         rc = compute_any(ctx, lines, n_lines, cut_cm, out_k_dev + (size_t)c * (size_t)ctx->N, (cudaStream_t)stream_v, true,
-                         /*reuse_sort=*/c > 0);
+                         reuse);
         launches += ctx->last_launches;
     }
     ctx->T = T0; ctx->P_atm = P0; ctx->Q = Q0;

@@ -430,6 +430,51 @@ __global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ r
     }
 }
 
+// ---- batched conditions that differ in PRESSURE only (hk_compute_batch, the paper's "multiple pressure points") ------
+// With T, Q and the mass unchanged, the strength, the Doppler width, the centre bin, the extent and the order of the
+// lines -- and with them the tile and node ranges -- are those of the previous condition; only Gamma_L moves.  One
+// streaming pass over the SORTED records puts the new (Gamma_L/dnu)^2 and what follows from it (Lorentz amplitude, y^2,
+// 1/(cK y)) in place, from the same fp64 expression line_kernel uses (Eq. 5), read through the sort's permutation.
+__global__ void __launch_bounds__(256) rewidth_kernel(Params p, const double* __restrict__ A, const double* __restrict__ gam,
+                                                      const double* __restrict__ nx, const int32_t* __restrict__ idx_sorted,
+                                                      const DevStats* __restrict__ st, float4* __restrict__ recA,
+                                                      const float4* __restrict__ recB, float4* __restrict__ recN,
+                                                      float4* __restrict__ recC)
+{
+    const int64_t n_act = st->n_act;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_act; i += (int64_t)gridDim.x * blockDim.x) {
+        const int32_t src = idx_sorted[i];
+        const double gammaL = A[src] * p.inv4pic + gam[src] * exp(nx[src] * p.ln_tfac) * p.P_atm;      // Eq. 5 (L91), as line_math
+        const double Gb = gammaL / p.dnu;
+        const float G2 = (float)(Gb * Gb);
+        const float4 rb = recB[i];
+        const float a2 = rb.x, cK = rb.w;
+        const float c = cK * sqrtf(G2 * a2) * 0.564189583547756f;
+        float4 ra = recA[i], rn = recN[i], rc = recC[i];
+        ra.z = G2; ra.w = c;
+        rn.z = G2; rn.w = c;
+        float y2 = 0.f, ip = 0.f;
+        if (a2 > 0.f) {
+            y2 = __fdiv_rn(G2, a2);
+            const float P = cK * __fsqrt_rn(y2);
+            if (P > 1.0e-30f && c != 0.f) ip = __fdiv_rn(1.0f, P);
+        }
+        rc.z = y2; rc.w = ip;
+        recA[i] = ra; recN[i] = rn; recC[i] = rc;
+    }
+}
+
+// the counters a run recounts (work-unit cursors, evaluated pairs); everything else in DevStats stays as the previous
+// condition of the batch left it
+__global__ void reset_run_kernel(DevStats* st)
+{
+    st->unit_counter_far = st->unit_counter_mid = st->unit_counter_near = st->unit_counter_node = 0u;
+    st->unit_counter_edge = st->unit_counter_centre = st->unit_counter_lane = 0u;
+    st->units_far = st->units_mid = st->units_near = st->units_node = st->units_edge = st->units_centre = 0ULL;
+    st->pairs_node_eval = 0ULL;
+    st->pairs_edge_node = 0ULL;
+}
+
 // first index with key >= v in the sorted key array
 __device__ __forceinline__ int32_t lower_bound_key(const int32_t* __restrict__ keys, int32_t n, int64_t v)
 {

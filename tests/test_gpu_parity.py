@@ -315,6 +315,29 @@ def test_batched_conditions(B):
     op.close()
 
 
+@pytest.mark.parametrize("cfg,n", [(2, 20_000), (4, 6_000), (5, 300)])
+def test_batch_pressure_sweep(B, cfg, n):
+    """The paper's use of a batch: many PRESSURES at one temperature (L361, L733).  From the second point on only the
+    Lorentz widths are recomputed (rewidth_kernel: same order, ranges and node lists); every point against the oracle,
+    P = 0 (natural widths only) included."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    P = [1e-3, 0.0, 1.0, 30.0, 0.2]
+    T, Q = [cond["T"]] * len(P), [cond["Q"]] * len(P)
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    dl = _to_cuda(lines)
+    kb = op.compute_batch(dl, cut, T, P, Q).cpu().numpy()
+    torch.cuda.synchronize()
+    st = op.stats()
+    for c in range(len(P)):
+        cnd = dict(T=T[c], P_atm=P[c], mass_amu=cond["mass_amu"], Q=Q[c])
+        k_ref, evals = O.opacity_grid(lines, cnd, grid, cut)
+        assert st["n_evals"] == evals
+        rel, ab, frac = check_parity(kb[c], k_ref, what=f"config {cfg} pressure point {c} (P = {P[c]} atm)")
+        print(f"pressure sweep config {cfg} P={P[c]:g}: rel={rel:.2e} abs={ab:.2e}")
+    op.close()
+
+
 def _oracle_illcond(lines, cond, grid, cut, slack=1.0):
     """Oracle-side count of the lines (with an extent) whose value at the fixed cutting length exceeds 1/512 of their
     peak value (HK_PLINTH_RATIO: the accuracy contract of hk_set_plinth); slack scales the threshold."""
