@@ -392,7 +392,7 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
             __syncwarp();
             int l = 0;
             // ---- R2: c r (1 + r (A1 - A2 r)), r = 1/(t^2 + G^2)
-#pragma unroll 2
+#pragma unroll 4
             for (; l < n2; ++l) {
                 const float4 ea = rw[0][l];
                 const float2 eb = *reinterpret_cast<const float2*>(&rw[1][l]);
