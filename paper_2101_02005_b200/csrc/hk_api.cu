@@ -522,29 +522,27 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_RANGES + 1], stream));
         ctx->last_launches = 2;
     } else {
-    // a1: per-line parameters, keys
-    line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
-                                                      lines->n_exp, ex, n, recU, keys_in, idx_in, flo, st);
-    scale_kernel<<<1, 1, 0, stream>>>(st);
-    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
-    // a2: order by centre bin
+    // a2 (decided first): compact keys (any fixed cut) go through a counting sort with the gather fused into the scatter;
+    // the bucket array and the scan's scratch live in the radix sort's scratch, which that path does not use
     const int bits = bits_for((uint32_t)p.ksent);
     size_t cub_bytes = L.cub_bytes;
-    // compact keys (any fixed cut): counting sort with the gather fused into the scatter; the bucket array and the scan's
-    // scratch live in the radix sort's scratch, which this path does not use
     const int64_t buckets = (int64_t)p.ksent + 2;
     size_t scan_bytes = 0;
     cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, (const int32_t*)nullptr, (int32_t*)nullptr, (int)buckets, stream);
     const bool counting = p.compact && buckets < 2147483647LL && align_up((size_t)buckets * 4) + scan_bytes <= L.cub_bytes;
     ctx->last_sort_bits = counting ? 0 : bits;
+    int32_t* hist = (counting && !reuse_sort) ? (int32_t*)(ws + L.cub) : nullptr;
+    if (hist) HK_CUDA(cudaMemsetAsync(hist, 0, (size_t)buckets * 4, stream));
+    // a1: per-line parameters, keys (and the histogram of the keys)
+    line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
+                                                      lines->n_exp, ex, n, recU, keys_in, counting ? nullptr : idx_in, flo, hist, st);
+    scale_kernel<<<1, 1, 0, stream>>>(st);
+    HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
     // the order by centre bin does not depend on (T, P, Q): later conditions of a batch reuse it (hk_compute_batch)
     if (reuse_sort) {
         gather_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, idx_out, flo, n, st, recA, recB, recN, recC, p.profile);
     } else if (counting) {
-        int32_t* hist = (int32_t*)(ws + L.cub);
         void* scan_tmp = ws + L.cub + align_up((size_t)buckets * 4);
-        HK_CUDA(cudaMemsetAsync(hist, 0, (size_t)buckets * 4, stream));
-        key_hist_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(keys_in, n, hist, st);
         HK_CUDA(cub::DeviceScan::ExclusiveSum(scan_tmp, scan_bytes, (const int32_t*)hist, hist, (int)buckets, stream));
         scatter_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, keys_in, flo, n, hist, st, keys_out, idx_out, recA, recB, recN,
                                                             recC, p.profile);
@@ -566,7 +564,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
     range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_edge, cnt_centre,
                                                            cnt_near, cnt_lane, st);
-    ctx->last_launches = counting && !reuse_sort ? 6 : 5;   // line, scale, (hist,) gather / scatter, range (+ node range below)
+    ctx->last_launches = 5;   // line, scale, gather / scatter, range (+ node range below)
     if (lv.n_entries > 0) {
         HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
         node_range_kernel<<<(lv.n_entries + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, nr, cnt_node, st);

@@ -203,14 +203,20 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
                                                    const double* __restrict__ nx, LineExtra ex, int64_t n,
                                                    RecU* __restrict__ rec, int32_t* __restrict__ key,
                                                    int32_t* __restrict__ idx, float* __restrict__ flo,
-                                                   DevStats* __restrict__ st)
+                                                   int32_t* __restrict__ hist, DevStats* __restrict__ st)
 {
+    // idx: identity permutation for the radix sort (null with the counting sort); hist: the counting sort's buckets (null
+    // otherwise) -- the histogram of the keys rides along here, its atomics hidden under the fp64 arithmetic: lanes of a
+    // warp with equal keys (neighbours, in a list that arrives sorted) are served by ONE atomic
     unsigned long long skipped = 0, off = 0, evals = 0, cmaxb = 0, cKmaxb = 0, shiftb = 0;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t n_round = hist ? ((n + 31) & ~31LL) : n;                   // (warp-uniform trip count for the match)
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+        int32_t k = -1;                         // (lanes past the end of the list take part in the match only)
+        if (i < n) {
         LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
                                 : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
         RecU r;
-        int32_t k = p.ksent;
+        k = p.ksent;
         r.jc = 0; r.f = 0.f; r.G2 = 0.f; r.a2 = 0.f; r.ilo = 0; r.ihi = -1; r.cK = 0.0;
         if (!o.valid) {
             if (p.count_invalid) ++skipped;
@@ -247,7 +253,12 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
         if (flo && k == p.ksent) flo[i] = 0.f;
         rec[i] = r;
         key[i] = k;
-        idx[i] = (int32_t)i;
+        if (idx) idx[i] = (int32_t)i;
+        }
+        if (hist) {
+            const unsigned peers = __match_any_sync(0xffffffffu, k);
+            if (k >= 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + k, __popc(peers));
+        }
     }
     // block reduction of the counters: three sums, three maxima (positive doubles order as their bit patterns)
     __shared__ unsigned long long sh[6][8];
@@ -379,33 +390,13 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
 
 // ---- counting sort by centre bin (step a2 when the keys are compact: any fixed cut) --------------------------------
 // Only the GROUPING by key matters to the accumulation kernels (their line ranges are key ranges), not the order inside
-// a key.  So: histogram of the keys -> exclusive scan -> every line takes the next free slot of its key's bucket and
+// a key.  So: histogram of the keys (in line_kernel) -> exclusive scan -> every line takes the next free slot of its key's bucket and
 // writes its sorted records there, straight from the unsorted record (the gather is the scatter).  Lanes of a warp
 // with equal keys -- neighbours, in a list that arrives sorted -- are served by ONE atomic.  A list that is already
 // in order costs one streaming pass; nothing is decided on the host.
-__global__ void __launch_bounds__(256) key_hist_kernel(const int32_t* __restrict__ key, int64_t n, int32_t* __restrict__ hist,
-                                                       DevStats* __restrict__ st)
-{
-    const int lane = threadIdx.x & 31;
-    unsigned long long unsorted = 0;
-    const int64_t n_round = (n + 31) & ~31LL;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
-        const bool live = i < n;
-        const int32_t k = live ? key[i] : -1;
-        int32_t prev = __shfl_up_sync(0xffffffffu, k, 1);
-        if (lane == 0) prev = i > 0 ? key[i - 1] : k;
-        if (live && i > 0 && k < prev) ++unsorted;
-        const unsigned peers = __match_any_sync(0xffffffffu, k);
-        if (live && lane == __ffs(peers) - 1) atomicAdd(hist + k, __popc(peers));
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) unsorted += __shfl_xor_sync(0xffffffffu, unsorted, o);
-    if (lane == 0 && unsorted) atomicAdd(&st->n_unsorted, unsorted);
-}
-
 __global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ key,
                                                       const float* __restrict__ flo, int64_t n, int32_t* __restrict__ cursor,
-                                                      const DevStats* __restrict__ st, int32_t* __restrict__ key_sorted,
+                                                      DevStats* __restrict__ st, int32_t* __restrict__ key_sorted,
                                                       int32_t* __restrict__ idx_sorted, float4* __restrict__ recA,
                                                       float4* __restrict__ recB, float4* __restrict__ recN,
                                                       float4* __restrict__ recC, int profile)
@@ -414,9 +405,13 @@ __global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ r
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     const int64_t n_round = (n + 31) & ~31LL;
+    unsigned long long unsorted = 0;             // adjacent pairs out of key order in the caller's list (hk_stats.n_unsorted)
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
         const bool live = i < n;
         const int32_t k = live ? key[i] : -1;
+        int32_t prev = __shfl_up_sync(0xffffffffu, k, 1);
+        if (lane == 0) prev = (live && i > 0) ? key[i - 1] : k;
+        if (live && i > 0 && k < prev) ++unsorted;
         const unsigned peers = __match_any_sync(0xffffffffu, k);
         const int leader = __ffs(peers) - 1;
         int32_t base = 0;
@@ -428,6 +423,9 @@ __global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ r
         idx_sorted[pos] = (int32_t)i;
         write_sorted_records(rec[i], flo ? flo[i] : 0.f, flo != nullptr, e, profile, pos, recA, recB, recN, recC);
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) unsorted += __shfl_xor_sync(0xffffffffu, unsorted, o);
+    if (lane == 0 && unsorted) atomicAdd(&st->n_unsorted, unsorted);
 }
 
 // ---- batched conditions that differ in PRESSURE only (hk_compute_batch, the paper's "multiple pressure points") ------
