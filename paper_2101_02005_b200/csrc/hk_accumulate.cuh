@@ -1074,7 +1074,7 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
 // warp_add_by_bin as before).
 constexpr int kEdgeBlock = 256;
 
-__global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys,
+__global__ void __launch_bounds__(kThreads, 3) edge_node_kernel(Params p, AccArgs a, const int32_t* __restrict__ keys,
                                                                  int32_t n)
 {
     constexpr int M = kP / 2;
@@ -1107,12 +1107,16 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
             int64_t key_thr = 0;
 #pragma unroll
             for (int j = 0; j < kP; ++j) run[j] = 0.f;
+            // (the next batch's records are in flight while this one is evaluated)
+            float4 rn_n = make_float4(0.f, 0.f, 1.f, 0.f), rb_n = make_float4(1.f, 0.f, __int_as_float(-1), 0.f);
+            if (i0 + lane < i1) { rn_n = a.recN[i0 + lane]; rb_n = a.recB[i0 + lane]; }
 #pragma unroll 1
             for (int ib = i0; ib < i1; ib += 32) {
                 const int i = ib + lane;
                 const bool live = i < i1;
-                float4 rn = make_float4(0.f, 0.f, 1.f, 0.f), rb = make_float4(1.f, 0.f, __int_as_float(-1), 0.f);
-                if (live) { rn = a.recN[i]; rb = a.recB[i]; }
+                const float4 rn = rn_n, rb = rb_n;
+                rn_n = make_float4(0.f, 0.f, 1.f, 0.f); rb_n = make_float4(1.f, 0.f, __int_as_float(-1), 0.f);
+                if (i + 32 < i1) { rn_n = a.recN[i + 32]; rb_n = a.recB[i + 32]; }
                 const int jc = __float_as_int(rn.x), ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);
                 const int e = side == 0 ? ihi : ilo;
                 bool m = live && ihi >= ilo;
@@ -1121,22 +1125,22 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
                     if (T0 != key_T0) { key_thr = side == 0 ? edge_key_upL(p, T0, W) : edge_key_dnR(p, T0, W); key_T0 = T0; }
                     m = side == 0 ? (int64_t)jc <= key_thr : (int64_t)jc >= key_thr;
                 }
-                float v[kP];
-#pragma unroll
-                for (int j = 0; j < kP; ++j) v[j] = 0.f;
                 // |z|^2 >= Z1 on the whole edge tile (the usual case: the extent ends many widths from the centre): one
                 // asymptotic term; a line that needs two runs the same code with its a^2, so a warp takes one path and the
-                // value of a pair never depends on its neighbours
+                // value of a pair never depends on its neighbours.  Every lane evaluates -- a lane without a pair with
+                // amplitude 0 -- so that the batch runs without divergence
                 const uint32_t pk = (uint32_t)__float_as_int(rn.y);
                 const float a2 = __int_as_float((int)((pk & 0x7FFFFu) << 12));
                 const float dist = (float)(side == 0 ? T0 - jc : jc - (T0 + W - 1)) - 1.0f;
                 const bool far = !m || fmaf(dist, dist, rn.z) >= 1.001f * HK_Z1 * a2;
-                const bool all_far = __all_sync(0xffffffffu, far);
-                if (m) {
-                    ++npairs;
+                const unsigned has = __ballot_sync(0xffffffffu, m);
+                if (has == 0u) continue;
+                npairs += m ? 1u : 0u;
+                float v[kP];
+                {
                     const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
-                    const float2 np2 = bcast2(-((float)(jc - T0) + f)), g2 = bcast2(rn.z), c2 = bcast2(rn.w);
-                    if (all_far) {
+                    const float2 np2 = bcast2(-((float)(jc - T0) + f)), g2 = bcast2(rn.z), c2 = bcast2(m ? rn.w : 0.f);
+                    if (__all_sync(0xffffffffu, far)) {
 #pragma unroll
                         for (int mm = 0; mm < M; ++mm) {
                             const float2 t = __fadd2_rn(xk[mm], np2);
@@ -1160,6 +1164,12 @@ __global__ void __launch_bounds__(kThreads, 4) edge_node_kernel(Params p, AccArg
                             v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
                         }
                     }
+                }
+                // the whole batch ends in the run's bin (lanes without a pair carry zeros): the common case
+                if (run_bin >= 0 && __all_sync(0xffffffffu, !m || e == run_bin)) {
+#pragma unroll
+                    for (int j = 0; j < kP; ++j) run[j] += v[j];
+                    continue;
                 }
                 // lanes that end in the run's bin join it; if the others agree on ONE bin (the list is sorted: a batch
                 // straddles at most a bin boundary or two) the run is folded and a new one starts with them

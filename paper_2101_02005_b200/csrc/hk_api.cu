@@ -608,7 +608,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         if (p.mode == 0 || p.mode == 3) { edge_kernel<KB><<<ctx->n_sm * 4, kThreads, 0, stream>>>(a); ++ctx->last_launches; }
         if (use_edge_nodes) {
             HK_TRY(cudaMemsetAsync(edge_acc, 0, L.edge_acc_bytes, stream));
-            edge_node_kernel<<<ctx->n_sm * 4, kThreads, 0, stream>>>(p, a, keys_out, n);
+            edge_node_kernel<<<ctx->n_sm * 3, kThreads, 0, stream>>>(p, a, keys_out, n);
             const int64_t nsc = 2 * ((ctx->N + lv.w0 - 1) / lv.w0) * kP;
             edge_scan_kernel<<<(int)((nsc + 255) / 256), 256, 0, stream>>>(a);
             edge_bins_kernel<<<(int)((ctx->N + 255) / 256), 256, 0, stream>>>(a);
