@@ -161,6 +161,7 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     std::memset(&p, 0, sizeof(p));
     p.numin = c->numin;
     p.dnu = c->dnu;
+    p.inv_dnu = 1.0 / c->dnu;
     p.N = c->N;
     const double m = c->mass_amu / kNA;                        // grams (L83)
     p.c2_over_T = kH * kC / kKB / c->T;

@@ -20,6 +20,7 @@ struct LineExtra {
 struct Params {
     // grid
     double numin, dnu;
+    double inv_dnu;       // 1/dnu: for the quantities that end up in fp32 records (the integer extents use true divisions)
     int64_t N;
     // conditions folded into constants (host, fp64)
     double c2_over_T;     // h c / (k_B T)
@@ -226,7 +227,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             ++off;
             r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);
         } else {
-            double Gb = o.gammaL / p.dnu, ab = o.alphaD / p.dnu;     // the record keeps the TRUE widths (gather_kernel applies the profile)
+            double Gb = o.gammaL * p.inv_dnu, ab = o.alphaD * p.inv_dnu;   // the record keeps the TRUE widths (the scatter applies the profile)
             r.jc = (int32_t)o.jc;
             // sub-bin offset relative to the NEAREST grid point, in [-1/2, 1/2]: the profile is sampled at grid points, so
             // a centre that (almost) coincides with one needs its tiny offset at full relative precision (a narrow
@@ -240,7 +241,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             r.ihi = (int32_t)o.ihi;
             r.cK = o.S / (o.alphaD * 1.772453850905516027298);          // S/(alpha_D sqrt(pi))
             const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
-            double cl = gauss ? 0.0 : o.S * Gb / (kPi * p.dnu);         // Lorentz amplitude in bin units (none for a Gaussian)
+            double cl = gauss ? 0.0 : o.S * Gb * (p.inv_dnu * 0.31830988618379067154);   // Lorentz amplitude in bin units, S Gb/(pi dnu) (none for a Gaussian)
             if (gauss) Gb = 0.0;                                        // region counters below: y = 0
             k = (int32_t)(o.jc - p.kmin);
             cmaxb = max(cmaxb, (unsigned long long)__double_as_longlong(cl));
