@@ -93,6 +93,8 @@ typedef struct {
     int32_t sort_bits;     /* radix-sort key width used */
     int32_t bins_per_lane; /* tile geometry used: a level-0 tile is 32 x this many bins */
     int32_t n_levels;      /* levels of the node hierarchy used (0: direct evaluation only) */
+    int32_t single_pass;   /* 1: the records of the last compute were written by the single-pass preprocess (hk_set_single_pass) */
+    int32_t reserved0;
 } hk_stats;
 
 /* Phases of one hk_compute, timed with CUDA events on the caller's stream. */
@@ -174,9 +176,11 @@ int hk_set_plinth(hk_ctx* ctx, int on);
 size_t hk_workspace_bytes(const hk_ctx* ctx, int64_t n_lines);
 int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
 
-/* Reproducibility: bins receive their partial sums through fp64 atomic adds whose order is not fixed, so two runs of
- * the same call agree to the rounding of an fp64 sum (~1e-16 relative), not bit for bit (the paper notes the same of
- * its summation order, L666).  Integer outputs (extents, counts) are exact and reproducible.
+/* Reproducibility: lines of one centre bin keep no fixed order among themselves (counting sort; the single-pass
+ * preprocess keeps the caller's), fp32 partial sums of up to 128 terms follow that order, and bins receive them through
+ * fp64 atomic adds whose order is not fixed either: two runs of the same call agree to the rounding of those sums
+ * (a few 1e-7 of the local k at most, usually far less), not bit for bit (the paper notes the same of its summation
+ * order, L666).  Integer outputs (extents, counts) are exact and reproducible.
  *
  * Enqueue the whole hot path on `stream` (a cudaStream_t passed as void*; NULL is
  * the legacy default stream): preprocess -> sort by centre bin -> tile ranges -> node, far, mid, extent-end,
@@ -332,6 +336,18 @@ int hk_set_edge_nodes(hk_ctx* ctx, int on);
 /* 0 (default): the line-stationary node kernel (node_lines_kernel); 1: the entry-stationary one it replaced (node_kernel).
  * Both evaluate exactly the (line, tile) pairs node_range_kernel lists, with the same arithmetic per pair: a cross-check. */
 int hk_set_node_kernel(hk_ctx* ctx, int entry_stationary);
+/* Single-pass preprocess (default on).  Line lists are stored in wavenumber order (L216-218) and a caller's conditions
+ * move little between calls, so every compute leaves a 16-byte HINT in the workspace: "the list arrived in centre-bin
+ * order with every line valid and on the grid" and the exponent of its launch scale.  The next hk_compute / hk_accumulate
+ * / hk_compute_hitran on that workspace (fixed cut, no plinth, not the binned Gaussian) then writes the sorted fp32
+ * records in ONE pass over the lines, and checks both assumptions on the device while it does: a line without a key, a
+ * pair out of order, or a hinted scale more than 8 binades from the one this call's own maxima ask for, and the call
+ * runs the ordinary two passes (per-line parameters, then counting sort) after all -- same launches either way, nothing
+ * decided on the host.  Same fp64 and fp32 arithmetic per line on both paths; the launch scale is a power of two, so
+ * the result does not depend on which path ran (beyond fp32 under/overflow 2^100 away from the largest amplitude).
+ * The first compute on a workspace, an unsorted list and a list with lines off the grid always take the two passes.
+ * hk_stats.single_pass says which path the last compute took.  off: always two passes. */
+int hk_set_single_pass(hk_ctx* ctx, int on);
 
 int hk_last_cuda_error(const hk_ctx* ctx);
 const char* hk_strerror(int status);

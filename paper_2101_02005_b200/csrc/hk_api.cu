@@ -45,7 +45,11 @@ struct hk_ctx {
     int32_t last_sort_bits, last_kb, last_levels;
     int64_t last_launches;
     DevStats* d_stats;
-    const RecU* last_recU;       // unsorted records of the last pass (for the on-demand region counts)
+    // sorted records of the last pass (for the on-demand region counts and hk_get_extents) with the sort's permutation
+    const float4 *last_recA, *last_recB, *last_recN;
+    const int32_t* last_idx;
+    int single_pass;             // 1 (default): a list the previous compute found sorted is preprocessed in one pass
+    bool hint_ready;             // the DevHint of the bound workspace has been initialised
     int last_profile;
     bool regions_done;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
@@ -65,7 +69,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t stats, totals, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, recC, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
+    size_t stats, totals, hint, keys_in, keys_out, idx_in, idx_out, recU, flo, recA, recB, recN, recC, tr, nr, node_acc, edge_acc, plinth_acc, counts, prefix, cub;
     size_t edge_acc_bytes;   // 0: grid too large for the per-bin edge accumulators (direct edge kernel only)
     size_t cub_bytes, total;
     int32_t n_ct;        // level-0 tiles of the smallest geometry
@@ -110,6 +114,7 @@ Layout make_layout(const hk_ctx* c, int64_t n)
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
     L.stats = take(sizeof(DevStats));
     L.totals = take(sizeof(DevTotals));      // (fixed offset: survives the per-block layouts of hk_compute_host)
+    L.hint = take(sizeof(DevHint));          // (fixed offset too: carried from one compute to the next)
     L.keys_in = take(nn * 4);
     L.keys_out = take(nn * 4);
     L.idx_in = take(nn * 4);
@@ -170,6 +175,7 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     p.P_atm = c->P_atm;
     p.beta = std::sqrt(2.0 * kKB * c->T / m) / kC;
     p.sfac = 1.0 / (8.0 * kPi * kC * m * c->Q);
+    p.cKfac = p.sfac / (p.beta * std::sqrt(kPi));
     p.inv4pic = 1.0 / (4.0 * kPi * kC);
     if (hitran) {
         // per isotopologue: Doppler factor and abundance / (8 pi c m Q); the tile bounds use the widest Doppler factor
@@ -180,6 +186,7 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
             const double mj = c->iso_mass[j] / kNA;
             p.beta_iso[j] = std::sqrt(2.0 * kKB * c->T / mj) / kC;
             p.sfac_iso[j] = c->iso_ab[j] / (8.0 * kPi * kC * mj * c->iso_Q[j]);
+            p.cKfac_iso[j] = p.sfac_iso[j] / (p.beta_iso[j] * std::sqrt(kPi));
             if (p.beta_iso[j] > p.beta) p.beta = p.beta_iso[j];
         }
     }
@@ -293,14 +300,17 @@ __global__ void __launch_bounds__(256) extents_kernel(Params p, const double* __
     }
 }
 
-__global__ void __launch_bounds__(256) extents_from_records_kernel(const RecU* __restrict__ rec, int64_t n, int32_t* ilo,
-                                                                   int32_t* ihi, int32_t* jc)
+// extents and centre bins as the last compute wrote them into its sorted records, back in the caller's line order
+__global__ void __launch_bounds__(256) extents_from_records_kernel(const float4* __restrict__ recB, const float4* __restrict__ recN,
+                                                                   const int32_t* __restrict__ idx_sorted, int64_t n,
+                                                                   int32_t* ilo, int32_t* ihi, int32_t* jc)
 {
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const RecU r = rec[i];
-        if (ilo) ilo[i] = r.ihi >= r.ilo ? r.ilo : 0;
-        if (ihi) ihi[i] = r.ihi >= r.ilo ? r.ihi : -1;
-        if (jc) jc[i] = r.jc;
+        const float4 rb = recB[i];
+        const int32_t src = idx_sorted[i], lo = __float_as_int(rb.y), hi = __float_as_int(rb.z);
+        if (ilo) ilo[src] = hi >= lo ? lo : 0;
+        if (ihi) ihi[src] = hi >= lo ? hi : -1;
+        if (jc) jc[src] = __float_as_int(recN[i].x);
     }
 }
 
@@ -334,6 +344,7 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     c->numin = numin; c->numax = numax; c->dnu = dnu; c->N = (int64_t)Nd;
     c->node_sep = HK_NODE_SEP;
     c->edge_nodes = 1;
+    c->single_pass = 1;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -387,6 +398,14 @@ int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes)
     ctx->ws = dev_ptr;
     ctx->ws_bytes = bytes;
     ctx->have_run = false;
+    ctx->hint_ready = false;
+    return HK_OK;
+}
+
+int hk_set_single_pass(hk_ctx* ctx, int on)
+{
+    if (!ctx) return HK_EINVAL;
+    ctx->single_pass = on ? 1 : 0;
     return HK_OK;
 }
 
@@ -483,7 +502,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     ctx->last_cut = cut_cm;
     ctx->last_stream = stream;
     ctx->d_stats = st;
-    ctx->last_recU = nullptr;
+    ctx->last_recA = nullptr;
     ctx->regions_done = false;
     ctx->last_sort_bits = 0;
     ctx->last_launches = 0;
@@ -510,7 +529,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     int32_t* counts = (int32_t*)(ws + L.counts);
     int32_t* prefix = (int32_t*)(ws + L.prefix);
     const Levels lv = make_levels(ctx, p);
-    ctx->last_recU = recU;
+    ctx->last_recA = recA; ctx->last_recB = recB; ctx->last_recN = recN; ctx->last_idx = idx_out;
     ctx->last_profile = p.profile;
     ctx->last_levels = lv.n_levels;
 
@@ -533,11 +552,24 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     const bool counting = p.compact && buckets < 2147483647LL && align_up((size_t)buckets * 4) + scan_bytes <= L.cub_bytes;
     ctx->last_sort_bits = counting ? 0 : bits;
     int32_t* hist = (counting && !reuse_sort) ? (int32_t*)(ws + L.cub) : nullptr;
+    // a1 + a2 in one pass for a list the previous compute on this workspace found sorted (line_sorted_kernel); the two
+    // passes below then return at once.  Decided on the device: the launch sequence is the same either way.
+    DevHint* hint = (DevHint*)(ws + L.hint);
+    if (!ctx->hint_ready) { HK_CUDA(cudaMemsetAsync(hint, 0, sizeof(DevHint), stream)); ctx->hint_ready = true; }
+    const bool try_single = ctx->single_pass && hist && !flo && !p.plinth && p.cut_mode == 0 && !cls && p.mode == 0;
+    const DevHint* skip = try_single ? hint : nullptr;
+    if (try_single) {
+        line_sorted_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low,
+                                                                lines->gamma_ref, lines->n_exp, ex, n, hint, st, keys_out,
+                                                                idx_out, recA, recB, recN, recC);
+        single_pass_decide_kernel<<<1, 1, 0, stream>>>(st, hint);
+    }
     if (hist) HK_CUDA(cudaMemsetAsync(hist, 0, (size_t)buckets * 4, stream));
     // a1: per-line parameters, keys (and the histogram of the keys)
     line_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->nu0, lines->A, lines->g_up, lines->E_low, lines->gamma_ref,
-                                                      lines->n_exp, ex, n, recU, keys_in, counting ? nullptr : idx_in, flo, hist, st);
-    scale_kernel<<<1, 1, 0, stream>>>(st);
+                                                      lines->n_exp, ex, n, recU, keys_in, counting ? nullptr : idx_in, flo, hist, st,
+                                                      skip);
+    scale_kernel<<<1, 1, 0, stream>>>(st, skip);
     HK_CUDA(cudaEventRecord(ctx->ev[HK_PH_PREPROCESS + 1], stream));
     // the order by centre bin does not depend on (T, P, Q): later conditions of a batch reuse it (hk_compute_batch)
     if (reuse_sort) {
@@ -546,7 +578,9 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
         void* scan_tmp = ws + L.cub + align_up((size_t)buckets * 4);
         HK_CUDA(cub::DeviceScan::ExclusiveSum(scan_tmp, scan_bytes, (const int32_t*)hist, hist, (int)buckets, stream));
         scatter_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(recU, keys_in, flo, n, hist, st, keys_out, idx_out, recA, recB, recN,
-                                                            recC, p.profile);
+                                                            recC, p.profile, skip);
+        // what the next compute may assume (only this path knows whether the list arrived in order)
+        hint_update_kernel<<<1, 1, 0, stream>>>(st, hint);
     } else {
         HK_CUDA(cub::DeviceRadixSort::SortPairs(ws + L.cub, cub_bytes, (const int32_t*)keys_in, keys_out,
                                                 (const int32_t*)idx_in, idx_out, n, 0, bits, stream));
@@ -565,7 +599,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
     range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_edge, cnt_centre,
                                                            cnt_near, cnt_lane, st);
-    ctx->last_launches = 5;   // line, scale, gather / scatter, range (+ node range below)
+    ctx->last_launches = 5 + (try_single ? 2 : 0) + ((counting && !reuse_sort) ? 1 : 0);   // line, scale, gather / scatter, range (+ single pass and its decision, hint; node range below)
     if (lv.n_entries > 0) {
         HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
         node_range_kernel<<<(lv.n_entries + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, nr, cnt_node, st);
@@ -863,6 +897,7 @@ int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut
     // the per-block device scratch is the front of the caller's workspace
     ctx->ws = base + H.dev_ws;
     ctx->ws_bytes = H.stage[0] - H.dev_ws;
+    ctx->hint_ready = false;                     // (the hint lives in the workspace: another base, another hint)
     DevTotals* totals = (DevTotals*)((char*)ctx->ws + make_layout(ctx, 1).totals);   // (fixed offset in every block's layout)
     cudaError_t e = cudaMemsetAsync(k_dev, 0, (size_t)ctx->N * sizeof(double), stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(totals, 0, sizeof(DevTotals), stream);
@@ -903,6 +938,7 @@ int hk_compute_host(hk_ctx* ctx, const hk_lines* hl, int64_t n_lines, double cut
     cudaStreamSynchronize(ctx->copy_stream);
     ctx->ws = base;
     ctx->ws_bytes = full_bytes;
+    ctx->hint_ready = false;
     if (rc != HK_OK) return rc;
     if (e != cudaSuccess) return fail_cuda(ctx, e);
     if (n_blocks == 0) { ctx->have_run = true; ctx->last_n = 0; ctx->last_stream = stream; ctx->d_stats = nullptr; }
@@ -919,13 +955,14 @@ int hk_get_extents(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, int32_t*
     if (!ctx || n_lines < 0) return HK_EINVAL;
     if (!ctx->have_cond || !ctx->have_run) return HK_ESTATE;
     cudaStream_t stream = (cudaStream_t)stream_v;
-    const bool from_records = ctx->last_recU && !ctx->last_multi && n_lines == ctx->last_n;
+    const bool from_records = ctx->last_recA && !ctx->last_multi && n_lines == ctx->last_n;
     if (from_records) {
-        // what the last compute wrote (unsorted records are in the caller's line order): valid after hk_compute,
+        // what the last compute wrote (sorted records, put back in the caller's line order): valid after hk_compute,
         // hk_accumulate, hk_compute_hitran and a single-block hk_compute_host; `lines` is not read
         if (n_lines > 0) {
             if (stream != ctx->last_stream) HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
-            extents_from_records_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(ctx->last_recU, n_lines, ilo_dev, ihi_dev, jc_dev);
+            extents_from_records_kernel<<<grid_for(ctx, n_lines), 256, 0, stream>>>(ctx->last_recB, ctx->last_recN, ctx->last_idx, n_lines,
+                                                                                  ilo_dev, ihi_dev, jc_dev);
             HK_CUDA(cudaGetLastError());
         }
     } else {
@@ -1045,11 +1082,12 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     DevStats d;
     std::memset(&d, 0, sizeof(d));
     HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
-    if (ctx->d_stats && ctx->last_recU && !ctx->regions_done && ctx->last_n > 0) {
+    if (ctx->d_stats && ctx->last_recA && !ctx->regions_done && ctx->last_n > 0) {
         // per-region evaluation counts, derived from the records on demand (kept out of the hot path)
         const int64_t nl = ctx->last_n;                 // (block pipelines and class passes: the last block / pass)
         if (nl > 0) {
-            region_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_recU, nl, ctx->last_profile, ctx->last_kb, ctx->d_stats);
+            region_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_recA, ctx->last_recB, nl, ctx->last_profile,
+                                                                                 ctx->last_kb, ctx->d_stats);
             HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
         }
         ctx->regions_done = true;
@@ -1087,6 +1125,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->sort_bits = ctx->last_sort_bits;
     host_out->n_plinth_illcond = (int64_t)d.n_plinth_illcond;
     host_out->n_unsorted = (int64_t)d.n_unsorted;
+    host_out->single_pass = d.single_pass;
     host_out->n_pairs_node_far = (int64_t)d.pairs_node_far;
     host_out->n_pairs_node_eval = (int64_t)d.pairs_node_eval;
     host_out->n_evals_gh10_row = (int64_t)d.n_cnt_gh10_row;

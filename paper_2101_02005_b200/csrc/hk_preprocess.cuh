@@ -29,11 +29,12 @@ struct Params {
     double P_atm;
     double beta;          // sqrt(2 k_B T / m) / c     (alpha_D = beta nu0)
     double sfac;          // 1 / (8 pi c m Q)
+    double cKfac;         // sfac / (beta sqrt(pi)): S / (alpha_D sqrt(pi)) = A g' cKfac e^(-c2 E/T) (1 - e^(-c2 nu0/T)) / nu0^3
     double inv4pic;       // 1 / (4 pi c)
     // HITRAN-style inputs (n_iso > 0): Eq. 4 self pressure, per-isotopologue beta and abundance / (8 pi c m Q)
     double P_self;
     int32_t n_iso;
-    double beta_iso[kMaxIso], sfac_iso[kMaxIso];
+    double beta_iso[kMaxIso], sfac_iso[kMaxIso], cKfac_iso[kMaxIso];
     // cut
     double cut;           // cm^-1 (ignored when uncut)
     int uncut;
@@ -89,7 +90,19 @@ struct DevStats {
     unsigned long long shift_bits;                         // max |delta P| over the lines (cm^-1) as double bits (pressure shift)
     unsigned long long n_plinth_illcond;                   // plinth removal: lines whose cutting length falls inside their core
     unsigned long long n_unsorted;                         // adjacent pairs of valid lines out of centre-bin order (input order)
+    unsigned long long n_nokey;                            // lines that carry the sentinel key (invalid, off the grid, foreign)
+    unsigned long long single_bad;                         // single-pass preprocess: lines that break its assumption (no key, or out of order)
+    int32_t single_pass, pad3;                             // 1: the records of this launch were written by line_sorted_kernel
 };
+
+// What one compute leaves for the next one on the same workspace (a1/a2): a list that arrived in
+// centre-bin order with every line on the grid, and the exponent of its launch scale.  A HINT, nothing more: the next
+// compute writes its sorted records in one pass on the strength of it, checks both assumptions on the device while it
+// does so, and runs the two-pass path after all when one of them fails.
+struct DevHint {
+    int32_t valid, sorted, exp, skip_two_pass;
+};
+constexpr int kScaleWindow = 8;      // the single pass stands when the hinted scale puts the largest amplitude within 2^(40 +- 8)
 
 // Totals over the blocks of hk_compute_host / the class passes of a width-relative cut, kept on the device so that the
 // per-block counters need no host synchronisation (read back once at the end).
@@ -117,11 +130,21 @@ __device__ __forceinline__ bool finite6(double a, double b, double c, double d, 
     return isfinite(a) && isfinite(b) && isfinite(c) && isfinite(d) && isfinite(e) && isfinite(f);
 }
 
+// the bin a centre falls in, as line_math computes it (same operations, same order)
+__device__ __forceinline__ int64_t centre_bin(const Params& p, double ctr)
+{
+    const double big = 4.0e18;
+    double c = floor(__ddiv_rn(__dsub_rn(ctr, p.numin), p.dnu));
+    c = fmin(fmax(c, -big), big);
+    return (int64_t)c;
+}
+
 struct LineOut {
     bool valid;       // passes the R14 checks
     bool on_grid;     // extent non-empty and centre within 2^30 bins
     bool foreign;     // width-relative cut: the line's cutting length belongs to another pass
     double S, gammaL, alphaD;
+    double cK;        // S / (alpha_D sqrt(pi))
     int64_t jc, ilo, ihi;
     double pos_f;     // (nu0-numin)/dnu - jc
     double shift;     // |delta P|, cm^-1 (0 without pressure shift)
@@ -139,25 +162,33 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
 
     o.on_grid = false;
     o.foreign = false;
-    o.S = o.gammaL = o.alphaD = 0.0;
+    o.S = o.gammaL = o.alphaD = o.cK = 0.0;
     o.jc = 0; o.ilo = 0; o.ihi = -1; o.pos_f = 0.0; o.shift = 0.0;
     if (!o.valid) return o;
     double ctr = nu0;                                                          // centre of the profile and of the extent
+    // Eq. 9 (L127) with one reciprocal: S = A g' sfac w / nu0^2 and S / (alpha_D sqrt(pi)) = A g' cKfac w / nu0^3,
+    // w = e^(-c2 E/T) (1 - e^(-c2 nu0/T)); 1 - e^-x through expm1 only where the difference would cancel (x < 1)
+    const double inv_nu = 1.0 / nu0;
+    const double xs = p.c2_over_T * nu0;
+    const double stim = xs < 1.0 ? -expm1(-xs) : 1.0 - exp(-xs);
+    const double w = A * g * (inv_nu * inv_nu) * exp(-p.c2_over_T * E) * stim;
     if (p.n_iso > 0) {
         // Eq. 4 (L87), pressure shift (L238, Table 4), isotopologue table (L371-373); R23, R24
         o.alphaD = p.beta_iso[iso] * nu0;
         o.gammaL = A * p.inv4pic + exp(nx * p.ln_tfac) * (gam * (p.P_atm - p.P_self) + gs * p.P_self);
-        o.S = A * g * p.sfac_iso[iso] / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));
+        o.S = w * p.sfac_iso[iso];
+        o.cK = w * inv_nu * p.cKfac_iso[iso];
         ctr = __dadd_rn(nu0, __dmul_rn(dl, p.P_atm));                          // two roundings, as the oracle (no FMA contraction)
         o.shift = fabs(ctr - nu0);
     } else {
     o.alphaD = p.beta * nu0;                                                   // Eq. 13 (L203)
     o.gammaL = A * p.inv4pic + gam * exp(nx * p.ln_tfac) * p.P_atm;            // Eq. 5 (L91): (T_ref/T)^n = e^(n ln(T_ref/T))
-    o.S = A * g * p.sfac / (nu0 * nu0) * exp(-p.c2_over_T * E) * (-expm1(-p.c2_over_T * nu0));  // Eq. 9 (L127)
+    o.S = w * p.sfac;                                                          // Eq. 9 (L127)
+    o.cK = w * inv_nu * p.cKfac;
     }
     // (a width or strength that overflows fp64 -- finite fields, absurd exponents -- is treated like a non-finite
     //  field, R14: the line is skipped)
-    if (!isfinite(o.gammaL) || !isfinite(o.S)) { o.valid = false; o.S = o.gammaL = o.alphaD = 0.0; return o; }
+    if (!isfinite(o.gammaL) || !isfinite(o.S) || !isfinite(o.cK)) { o.valid = false; o.S = o.gammaL = o.alphaD = o.cK = 0.0; return o; }
     const double big = 4.0e18;
     nu0 = ctr;
     double pos = __ddiv_rn(__dsub_rn(nu0, p.numin), p.dnu);
@@ -198,112 +229,137 @@ __device__ __forceinline__ int64_t count_within(double pos, double T, int64_t il
     return hi >= lo ? (int64_t)(hi - lo) + 1 : 0;
 }
 
+struct LineCounters {
+    unsigned long long skipped, off, evals, cmaxb, cKmaxb, shiftb, nokey;
+};
+
+// The unsorted record and the key of one line from its fp64 parameters; flo_v: low part of the sub-bin offset (binned
+// Gaussian only, R26).  Lines that contribute nothing keep the sentinel key and an empty extent.
+__device__ __forceinline__ int32_t line_record(const Params& p, const LineOut& o, RecU& r, float& flo_v, LineCounters& c)
+{
+    int32_t k = p.ksent;
+    flo_v = 0.f;
+    r.jc = 0; r.f = 0.f; r.G2 = 0.f; r.a2 = 0.f; r.ilo = 0; r.ihi = -1; r.cK = 0.0;
+    if (!o.valid) {
+        if (p.count_invalid) ++c.skipped;
+    } else if (o.foreign) {
+        // belongs to another pass
+    } else if (!o.on_grid) {
+        ++c.off;
+        r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);
+    } else {
+        double Gb = o.gammaL * p.inv_dnu, ab = o.alphaD * p.inv_dnu;   // the record keeps the TRUE widths (the scatter applies the profile)
+        r.jc = (int32_t)o.jc;
+        // sub-bin offset relative to the NEAREST grid point, in [-1/2, 1/2]: the profile is sampled at grid points, so
+        // a centre that (almost) coincides with one needs its tiny offset at full relative precision (a narrow
+        // Lorentzian sampled at its peak).  Negative (sign bit set, -0 included): the nearest point is jc + 1.
+        const double fd = o.pos_f > 0.5 ? o.pos_f - 1.0 : o.pos_f;
+        r.f = (float)fd;
+        flo_v = (float)(fd - (double)r.f);
+        r.G2 = (float)(Gb * Gb);
+        r.a2 = (float)(ab * ab);
+        r.ilo = (int32_t)o.ilo;
+        r.ihi = (int32_t)o.ihi;
+        r.cK = o.cK;                                                // S/(alpha_D sqrt(pi))
+        const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
+        double cl = gauss ? 0.0 : o.S * Gb * (p.inv_dnu * 0.31830988618379067154);   // Lorentz amplitude in bin units, S Gb/(pi dnu) (none for a Gaussian)
+        k = (int32_t)(o.jc - p.kmin);
+        c.cmaxb = max(c.cmaxb, (unsigned long long)__double_as_longlong(cl));
+        c.cKmaxb = max(c.cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
+        c.evals += (unsigned long long)(o.ihi - o.ilo + 1);
+        c.shiftb = max(c.shiftb, (unsigned long long)__double_as_longlong(o.shift));
+        // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
+        //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
+    }
+    if (k == p.ksent) ++c.nokey;
+    return k;
+}
+
+// block reduction of the per-line counters: sums and maxima (positive doubles order as their bit patterns)
+__device__ __forceinline__ void reduce_line_counters(const LineCounters& c, unsigned long long bad, DevStats* __restrict__ st)
+{
+    __shared__ unsigned long long sh[8][8];
+    unsigned long long v[8] = {c.skipped, c.off, c.evals, c.nokey, bad, c.cmaxb, c.cKmaxb, c.shiftb};
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        unsigned long long x = v[q];
+        for (int o = 16; o > 0; o >>= 1) {
+            unsigned long long y = __shfl_xor_sync(0xffffffffu, x, o);
+            x = (q < 5) ? x + y : max(x, y);
+        }
+        if ((threadIdx.x & 31) == 0) sh[q][threadIdx.x >> 5] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        int q = threadIdx.x;
+        unsigned long long x = sh[q][0];
+        for (int w = 1; w < 8; ++w) x = (q < 5) ? x + sh[q][w] : max(x, sh[q][w]);
+        unsigned long long* dst = q == 0 ? &st->n_skipped : q == 1 ? &st->n_off_grid : q == 2 ? &st->n_evals
+                                : q == 3 ? &st->n_nokey : q == 4 ? &st->single_bad
+                                : q == 5 ? &st->cmax_bits : q == 6 ? &st->cKmax_bits : &st->shift_bits;
+        if (x) { if (q < 5) atomicAdd(dst, x); else atomicMax(dst, x); }
+    }
+}
+
 __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __restrict__ nu0,
                                                    const double* __restrict__ A, const double* __restrict__ g,
                                                    const double* __restrict__ E, const double* __restrict__ gam,
                                                    const double* __restrict__ nx, LineExtra ex, int64_t n,
                                                    RecU* __restrict__ rec, int32_t* __restrict__ key,
                                                    int32_t* __restrict__ idx, float* __restrict__ flo,
-                                                   int32_t* __restrict__ hist, DevStats* __restrict__ st)
+                                                   int32_t* __restrict__ hist, DevStats* __restrict__ st,
+                                                   const DevHint* __restrict__ hint)
 {
     // idx: identity permutation for the radix sort (null with the counting sort); hist: the counting sort's buckets (null
     // otherwise) -- the histogram of the keys rides along here, its atomics hidden under the fp64 arithmetic: lanes of a
-    // warp with equal keys (neighbours, in a list that arrives sorted) are served by ONE atomic
-    unsigned long long skipped = 0, off = 0, evals = 0, cmaxb = 0, cKmaxb = 0, shiftb = 0;
+    // warp with equal keys (neighbours, in a list that arrives sorted) are served by ONE atomic.
+    // hint (nullable): the single pass (line_sorted_kernel) has done this launch's work already
+    if (hint && hint->skip_two_pass) return;
+    LineCounters c = {0, 0, 0, 0, 0, 0, 0};
     const int64_t n_round = hist ? ((n + 31) & ~31LL) : n;                   // (warp-uniform trip count for the match)
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
         int32_t k = -1;                         // (lanes past the end of the list take part in the match only)
         if (i < n) {
-        LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
-                                : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
-        RecU r;
-        k = p.ksent;
-        r.jc = 0; r.f = 0.f; r.G2 = 0.f; r.a2 = 0.f; r.ilo = 0; r.ihi = -1; r.cK = 0.0;
-        if (!o.valid) {
-            if (p.count_invalid) ++skipped;
-        } else if (o.foreign) {
-            // belongs to another pass
-        } else if (!o.on_grid) {
-            ++off;
-            r.jc = (int32_t)max(min(o.jc, (int64_t)INT32_MAX), (int64_t)INT32_MIN);
-        } else {
-            double Gb = o.gammaL * p.inv_dnu, ab = o.alphaD * p.inv_dnu;   // the record keeps the TRUE widths (the scatter applies the profile)
-            r.jc = (int32_t)o.jc;
-            // sub-bin offset relative to the NEAREST grid point, in [-1/2, 1/2]: the profile is sampled at grid points, so
-            // a centre that (almost) coincides with one needs its tiny offset at full relative precision (a narrow
-            // Lorentzian sampled at its peak).  Negative (sign bit set, -0 included): the nearest point is jc + 1.
-            const double fd = o.pos_f > 0.5 ? o.pos_f - 1.0 : o.pos_f;
-            r.f = (float)fd;
-            if (flo) flo[i] = (float)(fd - (double)r.f);                // low part (binned Gaussian only, R26)
-            r.G2 = (float)(Gb * Gb);
-            r.a2 = (float)(ab * ab);
-            r.ilo = (int32_t)o.ilo;
-            r.ihi = (int32_t)o.ihi;
-            r.cK = o.S / (o.alphaD * 1.772453850905516027298);          // S/(alpha_D sqrt(pi))
-            const bool gauss = p.profile == HK_PROFILE_DOPPLER || p.profile == HK_PROFILE_BINNED_GAUSSIAN;
-            double cl = gauss ? 0.0 : o.S * Gb * (p.inv_dnu * 0.31830988618379067154);   // Lorentz amplitude in bin units, S Gb/(pi dnu) (none for a Gaussian)
-            if (gauss) Gb = 0.0;                                        // region counters below: y = 0
-            k = (int32_t)(o.jc - p.kmin);
-            cmaxb = max(cmaxb, (unsigned long long)__double_as_longlong(cl));
-            cKmaxb = max(cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
-            evals += (unsigned long long)(o.ihi - o.ilo + 1);
-            shiftb = max(shiftb, (unsigned long long)__double_as_longlong(o.shift));
-            // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
-            //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
-        }
-        if (flo && k == p.ksent) flo[i] = 0.f;
-        rec[i] = r;
-        key[i] = k;
-        if (idx) idx[i] = (int32_t)i;
+            LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                    : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
+            RecU r;
+            float flo_v;
+            k = line_record(p, o, r, flo_v, c);
+            if (flo) flo[i] = flo_v;
+            rec[i] = r;
+            key[i] = k;
+            if (idx) idx[i] = (int32_t)i;
         }
         if (hist) {
             const unsigned peers = __match_any_sync(0xffffffffu, k);
             if (k >= 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + k, __popc(peers));
         }
     }
-    // block reduction of the counters: three sums, three maxima (positive doubles order as their bit patterns)
-    __shared__ unsigned long long sh[6][8];
-    unsigned long long v[6] = {skipped, off, evals, cmaxb, cKmaxb, shiftb};
-#pragma unroll
-    for (int q = 0; q < 6; ++q) {
-        unsigned long long x = v[q];
-        for (int o = 16; o > 0; o >>= 1) {
-            unsigned long long y = __shfl_xor_sync(0xffffffffu, x, o);
-            x = (q < 3) ? x + y : max(x, y);
-        }
-        if ((threadIdx.x & 31) == 0) sh[q][threadIdx.x >> 5] = x;
-    }
-    __syncthreads();
-    if (threadIdx.x < 6) {
-        int q = threadIdx.x;
-        unsigned long long x = sh[q][0];
-        for (int w = 1; w < 8; ++w) x = (q < 3) ? x + sh[q][w] : max(x, sh[q][w]);
-        unsigned long long* dst = q == 0 ? &st->n_skipped : q == 1 ? &st->n_off_grid : q == 2 ? &st->n_evals
-                                : q == 3 ? &st->cmax_bits : q == 4 ? &st->cKmax_bits : &st->shift_bits;
-        if (x) { if (q < 3) atomicAdd(dst, x); else atomicMax(dst, x); }
-    }
+    reduce_line_counters(c, 0ULL, st);
 }
 
-// Per-region evaluation counts (hk_stats.n_evals_far / mid / core / gh6 / trap / gh10) from the unsorted records of the
+// Per-region evaluation counts (hk_stats.n_evals_far / mid / core / gh6 / trap / gh10) from the sorted records of the
 // last compute: for each line the number of bins of its extent with |z|^2 below each threshold.  Run on demand.
-__global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restrict__ rec, int64_t n, int profile, int kb,
-                                                           DevStats* __restrict__ st)
+__global__ void __launch_bounds__(256) region_stats_kernel(const float4* __restrict__ recA, const float4* __restrict__ recB,
+                                                           int64_t n, int profile, int kb, DevStats* __restrict__ st)
 {
     unsigned long long c[6] = {0, 0, 0, 0, 0, 0};        // below Z1, Z2, Z4, Z3 (trapezoid region), of that with y >= 2, of that in rows
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        const RecU r = rec[i];
-        if (r.ihi < r.ilo) continue;
+        const float4 ra = recA[i], rb = recB[i];
+        const int32_t ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);
+        if (ihi < ilo) continue;
         const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
-        const double G2 = gauss ? 0.0 : (double)r.G2, a2 = profile == HK_PROFILE_LORENTZ ? 0.0 : (double)r.a2;
-        const double pos = (double)r.jc + (signbit(r.f) ? 1.0 + (double)r.f : (double)r.f);
+        // (recA.z: G2, or the low part of the offset for the binned Gaussian; recB.x: a2, 0 for a pure Lorentzian)
+        const double G2 = gauss ? 0.0 : (double)ra.z, a2 = (double)rb.x;
+        const double pos = (double)__float_as_int(ra.x) + (double)ra.y;      // nearest grid point + offset in [-1/2, 1/2]
         const double y2 = a2 > 0.0 ? G2 / a2 : 1.0e300;
         const double z3 = (double)z3_for((float)fmin(y2, 1.0e30)), z4 = fmax((double)z4_for((float)fmin(y2, 1.0e30)), z3);
         const double t[4] = {(double)HK_Z1 * a2 - G2, (double)HK_Z2 * a2 - G2, z4 * a2 - G2, z3 * a2 - G2};
 #pragma unroll
         for (int q = 0; q < 4; ++q)
-            c[q] += (unsigned long long)count_within(pos, t[q] > 0 ? (double)sqrtf((float)t[q]) : 0.0, r.ilo, r.ihi);
+            c[q] += (unsigned long long)count_within(pos, t[q] > 0 ? (double)sqrtf((float)t[q]) : 0.0, ilo, ihi);
         if (y2 >= (double)(HK_Y10 * HK_Y10)) {
-            const unsigned long long c10 = (unsigned long long)count_within(pos, t[3] > 0 ? (double)sqrtf((float)t[3]) : 0.0, r.ilo, r.ihi);
+            const unsigned long long c10 = (unsigned long long)count_within(pos, t[3] > 0 ? (double)sqrtf((float)t[3]) : 0.0, ilo, ihi);
             c[4] += c10;
             // the row kernel evaluates these bins itself (class R10) when alpha_D >= 0.85 bins per 64 bins of tile (centre_setup)
             if (a2 > 0.0 && 1.0 / sqrt(a2) < 1.0 / (0.85 * (double)(kb / 2))) c[5] += c10;
@@ -321,9 +377,9 @@ __global__ void __launch_bounds__(256) region_stats_kernel(const RecU* __restric
     }
 }
 
-// One thread: power-of-two launch scale from the maxima (max Lorentz amplitude -> 2^40,
-// and cK kept below 2^100), DESIGN.md section 4 "dynamic range".
-__global__ void scale_kernel(DevStats* st)
+// Power-of-two launch scale from the maxima (max Lorentz amplitude -> 2^40, and cK kept below 2^100), DESIGN.md
+// section 4 "dynamic range".
+__device__ __forceinline__ int scale_exp_of(const DevStats* st)
 {
     double cmax = __longlong_as_double((long long)st->cmax_bits);
     double cKmax = __longlong_as_double((long long)st->cKmax_bits);
@@ -333,16 +389,45 @@ __global__ void scale_kernel(DevStats* st)
     // no Lorentz amplitude at all (Doppler / binned Gaussian): the largest Gaussian amplitude goes to 2^100, which leaves
     // 226 binades below it -- exp(-x^2) is followed down to x^2 = HK_ZG (gauss_term, hk_device.cuh)
     if (!(cmax > 0.0) && cKmax > 0.0 && isfinite(cKmax)) e = 100 - ilogb(cKmax);
-    e = max(-900, min(900, e));
-    st->scale_exp = e;
+    return max(-900, min(900, e));
+}
+
+// One thread, after line_kernel (two-pass path).
+__global__ void scale_kernel(DevStats* st, const DevHint* __restrict__ hint)
+{
+    if (hint && hint->skip_two_pass) return;
+    st->scale_exp = scale_exp_of(st);
+}
+
+// One thread, after line_sorted_kernel: did the single pass stand?  It does when it ran at all (the hint said "sorted"),
+// met no line without a key and no pair out of order, and the hinted scale is within kScaleWindow binades of the scale
+// this launch's own maxima ask for.  Otherwise the counters it left are cleared and the two-pass path runs.
+__global__ void single_pass_decide_kernel(DevStats* st, DevHint* hint)
+{
+    const bool ran = hint->valid && hint->sorted;
+    const int e = scale_exp_of(st);
+    const bool ok = ran && st->single_bad == 0ULL && abs(e - hint->exp) <= kScaleWindow;
+    hint->skip_two_pass = ok ? 1 : 0;
+    st->single_pass = ok ? 1 : 0;
+    if (ok) { st->scale_exp = hint->exp; return; }
+    st->n_skipped = st->n_off_grid = st->n_evals = st->n_nokey = st->single_bad = 0ULL;
+    st->cmax_bits = st->cKmax_bits = st->shift_bits = 0ULL;
+}
+
+// One thread, after the records are in place (either path): what this launch knows, for the next one.
+__global__ void hint_update_kernel(const DevStats* __restrict__ st, DevHint* hint)
+{
+    hint->exp = scale_exp_of(st);
+    hint->sorted = st->single_pass ? 1 : (st->n_unsorted == 0ULL && st->n_nokey == 0ULL ? 1 : 0);
+    hint->valid = 1;
 }
 
 // The sorted records of one line (recA, recB, recN, recC at position `pos`) from its unsorted record.
-__device__ __forceinline__ void write_sorted_records(const RecU& r, float flo_v, bool have_flo, int e, int profile, int64_t pos,
+__device__ __forceinline__ void write_sorted_records(const RecU& r, float flo_v, bool have_flo, double scale, int profile, int64_t pos,
                                                      float4* __restrict__ recA, float4* __restrict__ recB,
                                                      float4* __restrict__ recN, float4* __restrict__ recC)
 {
-    float cK = (float)scalbn(r.cK, e);
+    float cK = (float)(r.cK * scale);                              // scale = 2^scale_exp: exact
     // c = cK * G a / sqrt(pi)  (Lorentz amplitude S Gamma_L/(pi dnu^2) in bin units)
     const bool gauss = profile == HK_PROFILE_DOPPLER || profile == HK_PROFILE_BINNED_GAUSSIAN;
     float G2 = gauss ? 0.f : r.G2;
@@ -375,6 +460,93 @@ __device__ __forceinline__ void write_sorted_records(const RecU& r, float flo_v,
     recC[pos] = make_float4(inva, __fmul_rn(-r.f, inva), y2, ip);
 }
 
+// ---- single-pass preprocess (steps a1 + a2 in one kernel) -----------------------------------------------------------
+// Line lists are stored in wavenumber order, and conditions change little from one call to the next.  When the previous
+// compute on this workspace saw a list in centre-bin order with every line on the grid (DevHint), the sorted position of
+// line i is i, and with the previous launch scale as a stand-in for this one the fp32 records can be written as the
+// fp64 parameters are formed: no unsorted record, no key array, no histogram, no scatter.  Both assumptions are CHECKED
+// here (single_bad counts lines without a key and adjacent pairs out of order; the maxima give this launch's own
+// scale) and single_pass_decide_kernel discards the result when one fails.  Same fp64 arithmetic (line_math,
+// line_record) and same record arithmetic (write_sorted_records) as the two-pass path.
+// The six fp64 fields of the NEXT iteration's line travel global -> shared with cp.async (8 B per field per thread,
+// no registers held) while the current line's exponentials and divisions run: every thread reads back only what it
+// copied itself, so cp.async.wait_group is all the synchronisation there is.
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+
+__global__ void __launch_bounds__(256, 4) line_sorted_kernel(Params p, const double* __restrict__ nu0,
+                                                          const double* __restrict__ A, const double* __restrict__ g,
+                                                          const double* __restrict__ E, const double* __restrict__ gam,
+                                                          const double* __restrict__ nx, LineExtra ex, int64_t n,
+                                                          const DevHint* __restrict__ hint, DevStats* __restrict__ st,
+                                                          int32_t* __restrict__ key_sorted, int32_t* __restrict__ idx_sorted,
+                                                          float4* __restrict__ recA, float4* __restrict__ recB,
+                                                          float4* __restrict__ recN, float4* __restrict__ recC)
+{
+    if (!(hint->valid && hint->sorted)) return;
+    constexpr int kAhead = 2;                     // iterations in flight ahead of the one being computed
+    __shared__ double stage[kAhead + 1][6][256];
+    const double* const src[6] = {nu0, A, g, E, gam, nx};
+    const double scale = scalbn(1.0, hint->exp);
+    const int lane = threadIdx.x & 31;
+    LineCounters c = {0, 0, 0, 0, 0, 0, 0};
+    unsigned long long bad = 0;
+    const int64_t n_round = (n + 31) & ~31LL;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+#pragma unroll
+    for (int a = 0; a < kAhead; ++a) {
+        if (i + a * stride < n) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) cp_async8(&stage[a][q][threadIdx.x], src[q] + (i + a * stride));
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    for (int buf = 0; i < n_round; i += stride, buf = (buf == kAhead ? 0 : buf + 1)) {
+        const int64_t i_next = i + kAhead * stride;
+        const int nbuf = buf == 0 ? kAhead : buf - 1;                  // (buf + kAhead) mod (kAhead + 1)
+        if (i_next < n) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) cp_async8(&stage[nbuf][q][threadIdx.x], src[q] + i_next);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group %0;" ::"n"(kAhead) : "memory");   // this iteration's fields have landed
+        const bool live = i < n;
+        int64_t jc = INT64_MAX;                  // (lanes past the end: never "before" their neighbour)
+        RecU r;
+        int32_t k = p.ksent;
+        if (live) {
+            const double v0 = stage[buf][0][threadIdx.x], v1 = stage[buf][1][threadIdx.x], v2 = stage[buf][2][threadIdx.x],
+                         v3 = stage[buf][3][threadIdx.x], v4 = stage[buf][4][threadIdx.x], v5 = stage[buf][5][threadIdx.x];
+            LineOut o = p.n_iso > 0 ? line_math(p, v0, v1, v2, v3, v4, v5, ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                    : line_math(p, v0, v1, v2, v3, v4, v5);
+            float flo_v;
+            k = line_record(p, o, r, flo_v, c);
+            jc = o.jc;
+            if (k == p.ksent) ++bad;
+        }
+        // in order?  against the line before (lane 0: that line's centre bin again, from its wavenumber)
+        int64_t prev = __shfl_up_sync(0xffffffffu, jc, 1);
+        if (lane == 0) {
+            prev = jc;
+            if (live && i > 0) {
+                double ctr = nu0[i - 1];
+                if (p.n_iso > 0) ctr = __dadd_rn(ctr, __dmul_rn(ex.delta[i - 1], p.P_atm));
+                prev = centre_bin(p, ctr);
+            }
+        }
+        if (!live) continue;
+        if (jc < prev) ++bad;
+        key_sorted[i] = k;
+        idx_sorted[i] = (int32_t)i;
+        write_sorted_records(r, 0.f, false, scale, p.profile, i, recA, recB, recN, recC);
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    reduce_line_counters(c, bad, st);
+}
+
 // Permute by the index array of a sort (CUB path, and the later conditions of a batch, which reuse the order).
 __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ rec, const int32_t* __restrict__ idx_sorted,
                                                      const float* __restrict__ flo, int64_t n,
@@ -382,10 +554,10 @@ __global__ void __launch_bounds__(256) gather_kernel(const RecU* __restrict__ re
                                                      float4* __restrict__ recA, float4* __restrict__ recB,
                                                      float4* __restrict__ recN, float4* __restrict__ recC, int profile)
 {
-    const int e = st->scale_exp;
+    const double scale = scalbn(1.0, st->scale_exp);
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const int32_t src = idx_sorted[i];
-        write_sorted_records(rec[src], flo ? flo[src] : 0.f, flo != nullptr, e, profile, i, recA, recB, recN, recC);
+        write_sorted_records(rec[src], flo ? flo[src] : 0.f, flo != nullptr, scale, profile, i, recA, recB, recN, recC);
     }
 }
 
@@ -400,9 +572,11 @@ __global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ r
                                                       DevStats* __restrict__ st, int32_t* __restrict__ key_sorted,
                                                       int32_t* __restrict__ idx_sorted, float4* __restrict__ recA,
                                                       float4* __restrict__ recB, float4* __restrict__ recN,
-                                                      float4* __restrict__ recC, int profile)
+                                                      float4* __restrict__ recC, int profile,
+                                                      const DevHint* __restrict__ hint)
 {
-    const int e = st->scale_exp;
+    if (hint && hint->skip_two_pass) return;
+    const double scale = scalbn(1.0, st->scale_exp);
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     const int64_t n_round = (n + 31) & ~31LL;
@@ -422,7 +596,7 @@ __global__ void __launch_bounds__(256) scatter_kernel(const RecU* __restrict__ r
         const int64_t pos = (int64_t)base + __popc(peers & lt_mask);
         key_sorted[pos] = k;
         idx_sorted[pos] = (int32_t)i;
-        write_sorted_records(rec[i], flo ? flo[i] : 0.f, flo != nullptr, e, profile, pos, recA, recB, recN, recC);
+        write_sorted_records(rec[i], flo ? flo[i] : 0.f, flo != nullptr, scale, profile, pos, recA, recB, recN, recC);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) unsorted += __shfl_xor_sync(0xffffffffu, unsorted, o);

@@ -195,6 +195,104 @@ def test_counting_sort_unsorted_input(B):
     op.close()
 
 
+def _stat_ints(st):
+    """the integer work counts that must not depend on how the records were written"""
+    keys = ("n_lines", "n_skipped", "n_off_grid", "n_evals", "n_evals_far", "n_evals_mid", "n_evals_core", "n_evals_gh6",
+            "n_evals_trap", "n_evals_gh10", "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_pairs_edge", "n_pairs_centre",
+            "n_pairs_node", "n_bins_node", "n_pairs_edge_node", "n_pairs_node_far", "bins_per_lane", "n_levels")
+    return {k: st[k] for k in keys}
+
+
+@pytest.mark.parametrize("cfg,n", [(3, 200_000), (4, 6_000), (2, 20_000), (1, None)])
+def test_single_pass_preprocess(B, cfg, n):
+    """Steps a1 + a2 in one kernel (line_sorted_kernel): the SECOND compute on a workspace, when the first found the list
+    sorted with every line on the grid, writes its sorted records in one pass.  Checked: which path ran (hk_stats.single_pass;
+    never on a first call, never for an unsorted list), the result of the single pass against the oracle on all bins, the
+    extents from its records, every integer work count equal to the two-pass path's, and the two results equal to the
+    rounding of the fp32 partial sums."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    sorted_in = bool((np.diff(lines["nu0"]) >= 0).all())
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    dl = _to_cuda(lines)
+    k1 = op.compute(dl, cut).cpu().numpy()
+    st1 = op.stats()
+    assert st1["single_pass"] == 0
+    k2 = op.compute(dl, cut).cpu().numpy()
+    st2 = op.stats()
+    ext2 = tuple(t.cpu().numpy() for t in op.extents(None, n=len(lines["nu0"])))
+    # (sort_bits == 0: the counting sort ran, which is the path that learns whether the list arrived in order; a few
+    #  thousand lines on millions of bins go through the radix sort and never take the single pass)
+    expect = sorted_in and st1["sort_bits"] == 0 and st1["n_off_grid"] == 0 and st1["n_skipped"] == 0
+    assert st2["single_pass"] == (1 if expect else 0), (sorted_in, st1)
+    assert expect or cfg != 3
+    assert _stat_ints(st1) == _stat_ints(st2) and st1["scale_exp"] == st2["scale_exp"]
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    assert st2["n_evals"] == evals == _check_extents(ext2, lines, cond, grid, cut)
+    rel, ab, _ = check_parity(k2, k_ref, what=f"config {cfg}, second compute")
+    # (the order of the lines inside one centre bin differs between the paths, and fp32 partial sums follow it)
+    same = np.abs(k2 - k1).max() / k_ref.max()
+    assert same <= 2e-6, same
+    # switched off: two passes again, same counts
+    op.set_single_pass(False)
+    k3 = op.compute(dl, cut).cpu().numpy()
+    st3 = op.stats()
+    assert st3["single_pass"] == 0 and _stat_ints(st3) == _stat_ints(st1)
+    assert np.abs(k3 - k1).max() / k_ref.max() <= 2e-6
+    print(f"config {cfg}: sorted {sorted_in}, single pass {st2['single_pass']}, rel={rel:.2e} abs={ab:.2e}, 1st vs 2nd {same:.1e}")
+    op.close()
+
+
+def test_single_pass_falls_back(B):
+    """The hint is checked on the device every time.  After a sorted list has set it: (a) the same workspace gets an
+    UNSORTED list, (b) a sorted list with one invalid and one off-grid line, (c) conditions that move the launch scale by
+    more than the window (T 1500 -> 200 K, Q x 1e6), (d) conditions that move it by less -- (a)-(c) must run the two passes,
+    (d) the single pass with the HINTED scale; all four against the oracle."""
+    lines, cond, grid, cut = _mini(3, 200_000)
+    n = len(lines["nu0"])
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+
+    def run(ln, cd, expect, what):
+        op.set_conditions(cd["T"], cd["P_atm"], cd["mass_amu"], cd["Q"])
+        k = op.compute(_to_cuda(ln), cut).cpu().numpy()
+        st = op.stats()
+        k_ref, evals = O.opacity_grid(ln, cd, grid, cut)
+        assert st["n_evals"] == evals
+        rel, ab, _ = check_parity(k, k_ref, what=what)
+        assert st["single_pass"] == expect, (what, st["single_pass"])
+        print(f"{what}: single pass {st['single_pass']}, scale 2^{st['scale_exp']}, rel={rel:.2e}")
+        return st
+
+    s0 = run(lines, cond, 0, "first call")
+    run(lines, cond, 1, "second call")
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(n)
+    shuffled = {k: v[perm] for k, v in lines.items()}
+    run(shuffled, cond, 0, "(a) unsorted list after a sorted one")
+    run(shuffled, cond, 0, "(a) unsorted list again")
+    run(lines, cond, 0, "sorted list after an unsorted one (two passes: the hint said unsorted)")
+    run(lines, cond, 1, "sorted list, hint restored")
+    bad = {k: v.copy() for k, v in lines.items()}
+    bad["A"][n // 3] = np.nan
+    bad["nu0"][-1] = grid[1] + 10 * cut
+    sb = run(bad, cond, 0, "(b) sorted list with an invalid and an off-grid line")
+    assert sb["n_skipped"] == 1 and sb["n_off_grid"] == 1
+    run(bad, cond, 0, "(b) again")
+    run(lines, cond, 0, "clean list after (b)")
+    run(lines, cond, 1, "clean list, hint restored")
+    cold = dict(cond, T=200.0, Q=cond["Q"] * 1.0e6)
+    sc = run(lines, cold, 0, "(c) T 1500 -> 200 K, Q x 1e6")
+    assert abs(sc["scale_exp"] - s0["scale_exp"]) > 8, (sc["scale_exp"], s0["scale_exp"])
+    run(lines, cold, 1, "(c) again")
+    near = dict(cold, T=230.0, P_atm=cond["P_atm"] * 3.0, Q=cold["Q"] * 7.0)
+    sd = run(lines, near, 1, "(d) T 200 -> 230 K, 3 x P, Q x 7")
+    assert sd["scale_exp"] == sc["scale_exp"]          # the hinted scale was used, not this call's own
+    se = run(lines, near, 1, "(d) again")
+    assert se["scale_exp"] != sd["scale_exp"]          # ... and the hint was re-centred on this call's maxima
+    op.close()
+
+
 @pytest.mark.parametrize("cfg,n", [(2, 20_000), (3, 200_000), (4, 6_000), (5, 300)])
 def test_node_kernels_agree(B, cfg, n):
     """The line-stationary node kernel against the entry-stationary one it replaced (hk_set_node_kernel): the same
@@ -1042,7 +1140,7 @@ def test_evaluator_accuracy_map(B):
 
 # ---- bench-size parity on sampled outputs ----------------------------------------------
 
-def _full_size_sampled(B, cfg, n_windows, width, n=None, plinth=False, cut_override=None, special=False):
+def _full_size_sampled(B, cfg, n_windows, width, n=None, plinth=False, cut_override=None, special=False, twice=False):
     """The CUDA path on the whole workload; the oracle on sampled windows of contiguous bins, every bin summed over all
     lines within its cut.  Windows: stratified over the grid, always the first and the last; with special=True also the
     densest region of the list, the window holding the GPU's maximum and the bins at +- cut of the strongest line
@@ -1059,6 +1157,18 @@ def _full_size_sampled(B, cfg, n_windows, width, n=None, plinth=False, cut_overr
     k = op.compute(dl, cut)
     torch.cuda.synchronize()
     st = op.stats()
+    if twice:
+        # what bench.py times is a REPEATED compute on one workspace: for a sorted list that is the single-pass
+        # preprocess (line_sorted_kernel).  The windows below check that second result; the first one must agree with it.
+        k_first = k.clone()
+        st_first = st
+        k = op.compute(dl, cut, out=k)
+        torch.cuda.synchronize()
+        st = op.stats()
+        assert st_first["single_pass"] == 0 and st["single_pass"] == 1
+        assert _stat_ints(st) == _stat_ints(st_first) and st["scale_exp"] == st_first["scale_exp"]
+        assert float((k - k_first).abs().max() / k.max()) <= 2e-6      # (fp32 partial sums of <= 128 terms in another order)
+        del k_first
     N = op.N
     rng = np.random.default_rng(cfg)
     wins = sample_windows(N, n_windows, width, rng)
@@ -1141,7 +1251,7 @@ def test_bt2_shaped_full_size_sampled(B, cfg, plinth, cut):
         pytest.skip("needs ~110 GB of device memory")
     if not plinth and cut is None:
         # the plain headline configs: 64 windows x 64 bins, with the special windows
-        worst, st = _full_size_sampled(B, cfg, 60, 64, special=True)
+        worst, st = _full_size_sampled(B, cfg, 60, 64, special=True, twice=True)
     else:
         worst, st = _full_size_sampled(B, cfg, 6 if cfg == 4 else 10, 8 if cfg == 4 else 32, plinth=plinth, cut_override=cut)
     print(f"config {cfg} full (plinth {plinth}): worst rel {worst:.2e}, evals {st['n_evals']:.3e}")
