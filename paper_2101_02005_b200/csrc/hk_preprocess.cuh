@@ -301,6 +301,43 @@ __device__ __forceinline__ void reduce_line_counters(const LineCounters& c, unsi
     }
 }
 
+// The six fp64 fields of the lines kAhead iterations AHEAD travel global -> shared with cp.async (8 B per field per
+// thread, no registers held) while the current line's exponentials and divisions run: every thread reads back only
+// what it copied itself, so cp.async.wait_group is all the synchronisation there is.
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+constexpr int kAhead = 2;
+struct LineStage {
+    double (*stage)[6][256];                     // [kAhead + 1][6][256] in shared memory
+    const double* src[6];
+    int buf;
+    __device__ __forceinline__ void issue(int slot, int64_t i, int64_t n) const
+    {
+        if (i < n) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) cp_async8(&stage[slot][q][threadIdx.x], src[q] + i);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    __device__ __forceinline__ void prime(int64_t i, int64_t stride, int64_t n)
+    {
+        buf = 0;
+#pragma unroll
+        for (int a = 0; a < kAhead; ++a) issue(a, i + a * stride, n);
+    }
+    // start the copy for iteration i + kAhead strides, wait for iteration i's
+    __device__ __forceinline__ void step(int64_t i, int64_t stride, int64_t n) const
+    {
+        issue(buf == 0 ? kAhead : buf - 1, i + kAhead * stride, n);     // slot (buf + kAhead) mod (kAhead + 1)
+        asm volatile("cp.async.wait_group %0;" ::"n"(kAhead) : "memory");
+    }
+    __device__ __forceinline__ double get(int q) const { return stage[buf][q][threadIdx.x]; }
+    __device__ __forceinline__ void next() { buf = (buf == kAhead) ? 0 : buf + 1; }
+    __device__ __forceinline__ void drain() const { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+};
+
 __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __restrict__ nu0,
                                                    const double* __restrict__ A, const double* __restrict__ g,
                                                    const double* __restrict__ E, const double* __restrict__ gam,
@@ -315,13 +352,20 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
     // warp with equal keys (neighbours, in a list that arrives sorted) are served by ONE atomic.
     // hint (nullable): the single pass (line_sorted_kernel) has done this launch's work already
     if (hint && hint->skip_two_pass) return;
+    __shared__ double stage[kAhead + 1][6][256];
+    LineStage ls = {stage, {nu0, A, g, E, gam, nx}, 0};
     LineCounters c = {0, 0, 0, 0, 0, 0, 0};
     const int64_t n_round = hist ? ((n + 31) & ~31LL) : n;                   // (warp-uniform trip count for the match)
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n_round; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    ls.prime(i, stride, n);
+    for (; i < n_round; i += stride, ls.next()) {
+        ls.step(i, stride, n);
         int32_t k = -1;                         // (lanes past the end of the list take part in the match only)
         if (i < n) {
-            LineOut o = p.n_iso > 0 ? line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i], ex.gam_self[i], ex.delta[i], ex.iso[i])
-                                    : line_math(p, nu0[i], A[i], g[i], E[i], gam[i], nx[i]);
+            LineOut o = p.n_iso > 0 ? line_math(p, ls.get(0), ls.get(1), ls.get(2), ls.get(3), ls.get(4), ls.get(5),
+                                                ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                    : line_math(p, ls.get(0), ls.get(1), ls.get(2), ls.get(3), ls.get(4), ls.get(5));
             RecU r;
             float flo_v;
             k = line_record(p, o, r, flo_v, c);
@@ -335,6 +379,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
             if (k >= 0 && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(hist + k, __popc(peers));
         }
     }
+    ls.drain();
     reduce_line_counters(c, 0ULL, st);
 }
 
@@ -468,15 +513,7 @@ __device__ __forceinline__ void write_sorted_records(const RecU& r, float flo_v,
 // here (single_bad counts lines without a key and adjacent pairs out of order; the maxima give this launch's own
 // scale) and single_pass_decide_kernel discards the result when one fails.  Same fp64 arithmetic (line_math,
 // line_record) and same record arithmetic (write_sorted_records) as the two-pass path.
-// The six fp64 fields of the NEXT iteration's line travel global -> shared with cp.async (8 B per field per thread,
-// no registers held) while the current line's exponentials and divisions run: every thread reads back only what it
-// copied itself, so cp.async.wait_group is all the synchronisation there is.
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
-}
-
-__global__ void __launch_bounds__(256, 4) line_sorted_kernel(Params p, const double* __restrict__ nu0,
+__global__ void __launch_bounds__(256, 3) line_sorted_kernel(Params p, const double* __restrict__ nu0,
                                                           const double* __restrict__ A, const double* __restrict__ g,
                                                           const double* __restrict__ E, const double* __restrict__ gam,
                                                           const double* __restrict__ nx, LineExtra ex, int64_t n,
@@ -486,9 +523,8 @@ __global__ void __launch_bounds__(256, 4) line_sorted_kernel(Params p, const dou
                                                           float4* __restrict__ recN, float4* __restrict__ recC)
 {
     if (!(hint->valid && hint->sorted)) return;
-    constexpr int kAhead = 2;                     // iterations in flight ahead of the one being computed
     __shared__ double stage[kAhead + 1][6][256];
-    const double* const src[6] = {nu0, A, g, E, gam, nx};
+    LineStage ls = {stage, {nu0, A, g, E, gam, nx}, 0};
     const double scale = scalbn(1.0, hint->exp);
     const int lane = threadIdx.x & 31;
     LineCounters c = {0, 0, 0, 0, 0, 0, 0};
@@ -496,32 +532,17 @@ __global__ void __launch_bounds__(256, 4) line_sorted_kernel(Params p, const dou
     const int64_t n_round = (n + 31) & ~31LL;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-#pragma unroll
-    for (int a = 0; a < kAhead; ++a) {
-        if (i + a * stride < n) {
-#pragma unroll
-            for (int q = 0; q < 6; ++q) cp_async8(&stage[a][q][threadIdx.x], src[q] + (i + a * stride));
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    }
-    for (int buf = 0; i < n_round; i += stride, buf = (buf == kAhead ? 0 : buf + 1)) {
-        const int64_t i_next = i + kAhead * stride;
-        const int nbuf = buf == 0 ? kAhead : buf - 1;                  // (buf + kAhead) mod (kAhead + 1)
-        if (i_next < n) {
-#pragma unroll
-            for (int q = 0; q < 6; ++q) cp_async8(&stage[nbuf][q][threadIdx.x], src[q] + i_next);
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        asm volatile("cp.async.wait_group %0;" ::"n"(kAhead) : "memory");   // this iteration's fields have landed
+    ls.prime(i, stride, n);
+    for (; i < n_round; i += stride, ls.next()) {
+        ls.step(i, stride, n);
         const bool live = i < n;
         int64_t jc = INT64_MAX;                  // (lanes past the end: never "before" their neighbour)
         RecU r;
         int32_t k = p.ksent;
         if (live) {
-            const double v0 = stage[buf][0][threadIdx.x], v1 = stage[buf][1][threadIdx.x], v2 = stage[buf][2][threadIdx.x],
-                         v3 = stage[buf][3][threadIdx.x], v4 = stage[buf][4][threadIdx.x], v5 = stage[buf][5][threadIdx.x];
-            LineOut o = p.n_iso > 0 ? line_math(p, v0, v1, v2, v3, v4, v5, ex.gam_self[i], ex.delta[i], ex.iso[i])
-                                    : line_math(p, v0, v1, v2, v3, v4, v5);
+            LineOut o = p.n_iso > 0 ? line_math(p, ls.get(0), ls.get(1), ls.get(2), ls.get(3), ls.get(4), ls.get(5),
+                                                ex.gam_self[i], ex.delta[i], ex.iso[i])
+                                    : line_math(p, ls.get(0), ls.get(1), ls.get(2), ls.get(3), ls.get(4), ls.get(5));
             float flo_v;
             k = line_record(p, o, r, flo_v, c);
             jc = o.jc;
@@ -543,7 +564,7 @@ __global__ void __launch_bounds__(256, 4) line_sorted_kernel(Params p, const dou
         idx_sorted[i] = (int32_t)i;
         write_sorted_records(r, 0.f, false, scale, p.profile, i, recA, recB, recN, recC);
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    ls.drain();
     reduce_line_counters(c, bad, st);
 }
 
