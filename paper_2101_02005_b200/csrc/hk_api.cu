@@ -50,6 +50,7 @@ struct hk_ctx {
     const int32_t* last_idx;
     int single_pass;             // 1 (default): a list the previous compute found sorted is preprocessed in one pass
     bool hint_ready;             // the DevHint of the bound workspace has been initialised
+    bool in_batch;               // inside hk_compute_batch: tile ranges may serve later conditions with other widths
     int last_profile;
     bool regions_done;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
@@ -223,6 +224,8 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     if (p.profile == HK_PROFILE_LORENTZ) p.kappa1 = p.kappa2 = 0.0;      // no core, no second term: every pair is "far"
     p.inv1p_k1 = 1.0 / (1.0 + p.kappa1); p.inv1m_k1 = 1.0 / (1.0 - p.kappa1);
     p.inv1p_k2 = 1.0 / (1.0 + p.kappa2); p.inv1m_k2 = 1.0 / (1.0 - p.kappa2);
+    p.kappa3 = std::sqrt((double)HK_ZG) * p.beta * 1.005;
+    p.inv1p_k3 = 1.0 / (1.0 + p.kappa3); p.inv1m_k3 = 1.0 / (1.0 - p.kappa3);
     p.numin_bins = c->numin / c->dnu;
     p.kb = pick_kb(c, cut);
     p.n_ct = (int32_t)((c->N + 32 * p.kb - 1) / (32 * p.kb));
@@ -485,6 +488,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     // (with per-line cutting lengths the tile an extent ends in is not a function of the centre bin alone: the
     //  masked direct edge kernel takes those tiles)
     p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes && p.cut_mode == 0) ? 1 : 0;
+    p.lane_tight = ctx->in_batch ? 0 : 1;
 
     // reuse (batched conditions on one resident list): 0 nothing, 1 the order of the lines by centre bin (any change of
     // condition), 2 everything but the Lorentz widths (same T, Q, mass: only the pressure moved)
@@ -821,6 +825,7 @@ int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double
     const double T0 = ctx->T, P0 = ctx->P_atm, Q0 = ctx->Q;
     int rc = HK_OK;
     int64_t launches = 0;
+    ctx->in_batch = true;
     for (int32_t c = 0; c < n_cond && rc == HK_OK; ++c) {
         ctx->T = T_K[c]; ctx->P_atm = P_atm[c]; ctx->Q = Q[c];
         // what the previous condition of the batch left in the workspace is reused as far as it still holds: the order by
@@ -834,6 +839,7 @@ int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double
                          reuse);
         launches += ctx->last_launches;
     }
+    ctx->in_batch = false;
     ctx->T = T0; ctx->P_atm = P0; ctx->Q = Q0;
     ctx->last_launches = launches;
     return rc;

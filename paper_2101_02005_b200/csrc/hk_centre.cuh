@@ -528,8 +528,8 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
         const int ct = find_tile(prefix, a.n_ct, u);
         const int64_t ct0 = (int64_t)ct * kTB;
         const TileRange r = a.tr[ct];
-        const int c0 = r.CL + (u - prefix[ct]) * a.chunk_lane;
-        const int nt = min(a.chunk_lane, r.CR - c0);
+        const int c0 = r.LL + (u - prefix[ct]) * a.chunk_lane;       // (lines that can have innermost bins here: range_kernel)
+        const int nt = min(a.chunk_lane, r.LR - c0);
         if (nt <= 0) continue;
 
         double acc64[KB];

@@ -51,8 +51,9 @@ struct __align__(16) RecU {
 //   [A0,EL) left edge, no core | [EL,FL0) left edge, generic | [FL0,NL) node-handled | [NL,FL1) far | [FL1,ML1) mid |
 //   [ML1,CL) centre, generic | [CL,CR) centre, tile inside the extent | [CR,MR0) centre, generic |
 //   [MR0,FR0) mid | [FR0,NR) far | [NR,FR1) node-handled | [FR1,ER) right edge, generic | [ER,A1) right edge, no core
+// [LL,LR) inside [CL,CR): the lines that can have innermost bins (lane-pass work, hk_centre.cuh) in this tile
 struct __align__(8) TileRange {
-    int32_t A0, EL, FL0, NL, FL1, ML1, CL, CR, MR0, FR0, NR, FR1, ER, A1;
+    int32_t A0, EL, FL0, NL, FL1, ML1, CL, CR, MR0, FR0, NR, FR1, ER, A1, LL, LR;
 };
 
 // per (level, tile) entry of the node hierarchy: four index ranges of sorted lines evaluated at the tile's nodes

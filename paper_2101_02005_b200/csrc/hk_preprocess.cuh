@@ -52,7 +52,8 @@ struct Params {
     // tile ranges
     int64_t cb_floor, cb_ceil;  // floor/ceil of cut/dnu (bins)
     double kappa1, kappa2;      // sqrt(Z1) * beta and sqrt(Z2) * beta, slightly inflated
-    double inv1p_k1, inv1m_k1, inv1p_k2, inv1m_k2;   // 1/(1 + kappa), 1/(1 - kappa)
+    double kappa3;              // sqrt(ZG) * beta: beyond it no line has innermost (lane-pass) bins
+    double inv1p_k1, inv1m_k1, inv1p_k2, inv1m_k2, inv1p_k3, inv1m_k3;   // 1/(1 + kappa), 1/(1 - kappa)
     double numin_bins;          // numin / dnu
     int32_t kb;                 // bins per lane (2, 4, 8)
     int32_t n_ct;               // tiles of 32 kb bins
@@ -64,6 +65,8 @@ struct Params {
     int profile;                // 0 Voigt, 1 Lorentz (records carry alpha_D = 0), 2 Doppler (records carry Gamma_L = 0)
     int plinth;                 // 1: remove every line's value at the cutting length from its bins (section 2.1.1)
     double cut_bins;            // cut / dnu
+    int lane_tight;             // 1: the lane-pass candidate range uses the largest z3_for(y^2) of THIS launch's lines
+                                //    (0: any y -- ranges that later conditions of a batch reuse with other widths)
     int edge_nodes;             // 1: separated edge tiles go through per-bin node accumulators (edge_node_kernel)
     int mode;                   // debug: 0 default, 1 everything through the near kernel, 2 far pairs through the mid kernel,
                                 //        3 direct evaluation only (no node hierarchy)
@@ -91,6 +94,7 @@ struct DevStats {
     unsigned long long n_plinth_illcond;                   // plinth removal: lines whose cutting length falls inside their core
     unsigned long long n_unsorted;                         // adjacent pairs of valid lines out of centre-bin order (input order)
     unsigned long long n_nokey;                            // lines that carry the sentinel key (invalid, off the grid, foreign)
+    unsigned long long z3max_bits;                         // largest z3_for(y^2) over the lines (fp32 bits): how far innermost bins reach
     unsigned long long single_bad;                         // single-pass preprocess: lines that break its assumption (no key, or out of order)
     int32_t single_pass, pad3;                             // 1: the records of this launch were written by line_sorted_kernel
 };
@@ -230,7 +234,7 @@ __device__ __forceinline__ int64_t count_within(double pos, double T, int64_t il
 }
 
 struct LineCounters {
-    unsigned long long skipped, off, evals, cmaxb, cKmaxb, shiftb, nokey;
+    unsigned long long skipped, off, evals, cmaxb, cKmaxb, shiftb, nokey, z3b;
 };
 
 // The unsorted record and the key of one line from its fp64 parameters; flo_v: low part of the sub-bin offset (binned
@@ -268,6 +272,9 @@ __device__ __forceinline__ int32_t line_record(const Params& p, const LineOut& o
         c.cKmaxb = max(c.cKmaxb, (unsigned long long)__double_as_longlong(r.cK));
         c.evals += (unsigned long long)(o.ihi - o.ilo + 1);
         c.shiftb = max(c.shiftb, (unsigned long long)__double_as_longlong(o.shift));
+        // (y^2 exactly as write_sorted_records forms it)
+        const float y2f = (gauss || !(r.a2 > 0.f)) ? 0.f : __fdiv_rn(r.G2, r.a2);
+        c.z3b = max(c.z3b, (unsigned long long)__float_as_uint(z3_for(y2f)));
         // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
         //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
     }
@@ -278,10 +285,10 @@ __device__ __forceinline__ int32_t line_record(const Params& p, const LineOut& o
 // block reduction of the per-line counters: sums and maxima (positive doubles order as their bit patterns)
 __device__ __forceinline__ void reduce_line_counters(const LineCounters& c, unsigned long long bad, DevStats* __restrict__ st)
 {
-    __shared__ unsigned long long sh[8][8];
-    unsigned long long v[8] = {c.skipped, c.off, c.evals, c.nokey, bad, c.cmaxb, c.cKmaxb, c.shiftb};
+    __shared__ unsigned long long sh[9][8];
+    unsigned long long v[9] = {c.skipped, c.off, c.evals, c.nokey, bad, c.cmaxb, c.cKmaxb, c.shiftb, c.z3b};
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
+    for (int q = 0; q < 9; ++q) {
         unsigned long long x = v[q];
         for (int o = 16; o > 0; o >>= 1) {
             unsigned long long y = __shfl_xor_sync(0xffffffffu, x, o);
@@ -290,13 +297,13 @@ __device__ __forceinline__ void reduce_line_counters(const LineCounters& c, unsi
         if ((threadIdx.x & 31) == 0) sh[q][threadIdx.x >> 5] = x;
     }
     __syncthreads();
-    if (threadIdx.x < 8) {
+    if (threadIdx.x < 9) {
         int q = threadIdx.x;
         unsigned long long x = sh[q][0];
         for (int w = 1; w < 8; ++w) x = (q < 5) ? x + sh[q][w] : max(x, sh[q][w]);
         unsigned long long* dst = q == 0 ? &st->n_skipped : q == 1 ? &st->n_off_grid : q == 2 ? &st->n_evals
                                 : q == 3 ? &st->n_nokey : q == 4 ? &st->single_bad
-                                : q == 5 ? &st->cmax_bits : q == 6 ? &st->cKmax_bits : &st->shift_bits;
+                                : q == 5 ? &st->cmax_bits : q == 6 ? &st->cKmax_bits : q == 7 ? &st->shift_bits : &st->z3max_bits;
         if (x) { if (q < 5) atomicAdd(dst, x); else atomicMax(dst, x); }
     }
 }
@@ -354,7 +361,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
     if (hint && hint->skip_two_pass) return;
     __shared__ double stage[kAhead + 1][6][256];
     LineStage ls = {stage, {nu0, A, g, E, gam, nx}, 0};
-    LineCounters c = {0, 0, 0, 0, 0, 0, 0};
+    LineCounters c = {0, 0, 0, 0, 0, 0, 0, 0};
     const int64_t n_round = hist ? ((n + 31) & ~31LL) : n;                   // (warp-uniform trip count for the match)
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -456,7 +463,7 @@ __global__ void single_pass_decide_kernel(DevStats* st, DevHint* hint)
     st->single_pass = ok ? 1 : 0;
     if (ok) { st->scale_exp = hint->exp; return; }
     st->n_skipped = st->n_off_grid = st->n_evals = st->n_nokey = st->single_bad = 0ULL;
-    st->cmax_bits = st->cKmax_bits = st->shift_bits = 0ULL;
+    st->cmax_bits = st->cKmax_bits = st->shift_bits = st->z3max_bits = 0ULL;
 }
 
 // One thread, after the records are in place (either path): what this launch knows, for the next one.
@@ -527,7 +534,7 @@ __global__ void __launch_bounds__(256, 3) line_sorted_kernel(Params p, const dou
     LineStage ls = {stage, {nu0, A, g, E, gam, nx}, 0};
     const double scale = scalbn(1.0, hint->exp);
     const int lane = threadIdx.x & 31;
-    LineCounters c = {0, 0, 0, 0, 0, 0, 0};
+    LineCounters c = {0, 0, 0, 0, 0, 0, 0, 0};
     unsigned long long bad = 0;
     const int64_t n_round = (n + 31) & ~31LL;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -899,6 +906,23 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
         r.CL = min(max(idx_of(p, keys, n_act, jLmin), ml1), mr0);
         r.CR = min(max(idx_of(p, keys, n_act, jRmax + 1), r.CL), mr0);
     }
+    // lane-pass candidates (centre_setup, hk_centre.cuh): innermost bins lie within sqrt(ZG) alpha_D of the centre
+    // (z3_for <= HK_ZG; the binned Gaussian: 1/2 + 6 alpha_D), or within the whole core of a line narrower than
+    // 0.224 kb/2 bins (25 alpha_D < 5.6 kb/2 bins); centre_setup's own test is 0.2 % generous, kappa3 0.5 %
+    r.LL = r.CL; r.LR = r.CR;
+    if (p.mode == 0 || p.mode == 3) {
+        const int64_t dmin = 6 * (int64_t)(p.kb / 2) + 3;
+        double kap3 = p.kappa3, i1p = p.inv1p_k3, i1m = p.inv1m_k3;
+        if (p.lane_tight) {
+            // the largest z3_for(y^2) over this launch's lines (line_record): 30.25 for a list with y^2 >= 1e-6 throughout
+            const float z3m = __uint_as_float((unsigned)st->z3max_bits);
+            if (z3m > 0.f && z3m < HK_ZG) { kap3 = sqrt((double)z3m) * p.beta * 1.005; i1p = 1.0 / (1.0 + kap3); i1m = 1.0 / (1.0 - kap3); }
+        }
+        const int64_t jLl = min(left_bound((double)w0, kap3, i1p, p.numin_bins), w0 - 1 - dmin);
+        const int64_t jRl = max(right_bound((double)(w1 - 1), kap3, i1m, p.numin_bins), w1 - 1 + dmin);
+        r.LL = min(max(idx_of(p, keys, n_act, jLl + 1), r.CL), r.CR);
+        r.LR = max(min(idx_of(p, keys, n_act, jRl), r.CR), r.LL);
+    }
     if (p.edge_nodes && p.mode == 0 && lv.n_levels > 0 && !p.uncut) {
         // [A0, ESL) and [ESR, A1) go to edge_node_kernel; the direct edge kernel keeps [ESL, EL) and [ER, ESR)
         const EdgeKeys ek = edge_keys(p, w0, wb);
@@ -916,7 +940,7 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
     cnt_mid[wt] = (int32_t)((nmid + p.chunk - 1) / p.chunk);
     cnt_edge[wt] = (int32_t)((nedge + p.chunk - 1) / p.chunk);
     cnt_centre[wt] = (int32_t)((ncen + p.chunk_centre - 1) / p.chunk_centre);
-    cnt_lane[wt] = (int32_t)((ncen + p.chunk_lane - 1) / p.chunk_lane);
+    cnt_lane[wt] = (int32_t)(((long long)(r.LR - r.LL) + p.chunk_lane - 1) / p.chunk_lane);
     cnt_near[wt] = (int32_t)((nnear + p.chunk - 1) / p.chunk);
     if (nfar) atomicAdd(&st->pairs_far, (unsigned long long)nfar * nb);
     if (nmid) atomicAdd(&st->pairs_mid, (unsigned long long)nmid * nb);

@@ -1280,6 +1280,35 @@ def test_zero_width_line_on_a_grid_point(B, profile):
     op.close()
 
 
+@pytest.mark.parametrize("mix", ["y_large", "y_tiny", "mixed"])
+def test_lane_candidate_range_follows_the_widest_inner_region(B, mix):
+    """range_kernel lists, per tile, the lines that can have innermost (lane-pass) bins there, from the largest
+    z3_for(y^2) over the launch's lines: 30.25 where y^2 >= 1e-6 throughout, 50 once a line lies below that (157 with a
+    pure Gaussian: the Doppler-profile tests).  Wide lines (alpha_D ~ 15 bins: the inner region spans several level-0
+    tiles) of either kind, alone and mixed in one list, all bins against the oracle -- a range one class too tight
+    would drop the outer part of the inner region of the tiny-y lines."""
+    rng = np.random.default_rng(77)
+    grid, cut = (20000.0, 20060.0, 0.005), 6.0
+    n = 240
+    nu0 = np.sort(rng.uniform(20000.5, 20059.5, n))
+    tiny = {"y_large": np.zeros(n, bool), "y_tiny": np.ones(n, bool), "mixed": rng.random(n) < 0.1}[mix]
+    # beta = sqrt(2 k T / m)/c = 3.7e-6 at 3000 K, m = 40: alpha_D = 0.074 cm^-1 = 15 bins; y = 0.17 or 7e-5
+    cond = dict(T=3000.0, P_atm=1.0, mass_amu=40.0, Q=10.0)
+    lines = _simple_lines(nu0, A=10 ** rng.uniform(-1, 1, n), gamma_ref=np.where(tiny, 2.0e-5, 0.05))
+    _, gL, aD, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    y2 = (gL / aD) ** 2
+    assert np.all(y2[tiny] < 1e-6) and np.all(y2[~tiny] > 1e-3) and 10 < np.median(aD) / grid[2] < 20
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    k = op.compute(_to_cuda(lines), cut).cpu().numpy()
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    st = op.stats()
+    assert st["n_evals"] == evals and st["n_evals_trap"] > 0
+    rel, ab, _ = check_parity(k, k_ref, what=f"lane candidate range, {mix}")
+    print(f"lane candidate range {mix}: rel={rel:.2e} abs={ab:.2e}, innermost evaluations {st['n_evals_trap']}")
+    op.close()
+
+
 def test_binned_gaussian_narrow_lines_at_bin_edges(B):
     """Lines 3000 times narrower than a bin whose centres lie within a few alpha_D of a bin edge (R26): the
     neighbouring bin's share, erfc((edge - nu0)/alpha_D)/2, needs the sub-bin offset to better than one fp32."""
