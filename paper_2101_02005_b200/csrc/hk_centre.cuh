@@ -514,6 +514,7 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
     __shared__ __align__(16) float wtab[24];   // trapezoid weights of the two node sets (trap_K)
     trap_weights_to_shared(wtab, threadIdx.x);
     if (kThreads < 24 && threadIdx.x == 0) { for (int i = kThreads; i < 24; ++i) trap_weights_to_shared(wtab, i); }
+    const float* const wsh = trap_weights_address(wtab);
     double* red = reinterpret_cast<double*>(&stage[0][0][0]);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int32_t* __restrict__ prefix = a.prefix_lane;
@@ -600,8 +601,8 @@ __global__ void __launch_bounds__(32 * W, (kLaneCtas * 8) / W) centre_lane_kerne
                         const float X = __fmul_rn(un, un);
                         float val = 0.f;
                         if (X < xl) {
-                            if (kTrapOnly) val = cK * trap_K<true>(fabsf(un), TL, wtab);
-                            else val = kBinned ? cK * binned_K(d, f, y2, inva) : lane_value(type, cK, fabsf(un), X, y, y2, TL, wtab);
+                            if (kTrapOnly) val = cK * trap_K<true>(fabsf(un), TL, wsh);
+                            else val = kBinned ? cK * binned_K(d, f, y2, inva) : lane_value(type, cK, fabsf(un), X, y, y2, TL, wsh);
                         }
                         stage[warp][s][lane] = val;
                     }

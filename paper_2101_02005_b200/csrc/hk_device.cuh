@@ -265,12 +265,19 @@ __device__ __forceinline__ TrapLine trap_line(float y)
                     5.27292424e-01f, 7.73047404e-02f, 3.15111160e-03f, 3.57128496e-05f, 1.12535175e-07f, 0.0f}
 #define HK_TRAP_WB {2.35257520e-06f, 3.93669041e-04f, 1.83156389e-02f, 2.36927759e-01f, 8.52143789e-01f, 8.52143789e-01f, \
                     2.36927759e-01f, 1.83156389e-02f, 3.93669041e-04f, 2.35257520e-06f, 3.90893843e-09f, 0.0f}
-// wtab: the 24 weights in shared memory (A then B; fill with trap_weights_to_shared) or nullptr (selected from immediates)
+// wtab: the 24 weights in shared memory (A then B; fill with trap_weights_to_shared), passed as their address in the
+// shared window (trap_weights_address) -- or nullptr (selected from immediates)
 __device__ __forceinline__ void trap_weights_to_shared(float* wtab, int tid)
 {
     constexpr float wA[12] = HK_TRAP_WA, wB[12] = HK_TRAP_WB;
     if (tid < 12) wtab[tid] = wA[tid];
     else if (tid < 24) wtab[tid] = wB[tid - 12];
+}
+__device__ __forceinline__ const float* trap_weights_address(const float* wtab_shared)
+{
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(wtab_shared);
+    asm volatile("" : "+r"(a));                 // (kept in a register: not rebuilt per evaluation)
+    return reinterpret_cast<const float*>((uintptr_t)a);
 }
 template <bool kSmemW>
 __device__ __forceinline__ float trap_K(float x, const TrapLine& L, const float* __restrict__ wtab)
@@ -298,8 +305,12 @@ __device__ __forceinline__ float trap_K(float x, const TrapLine& L, const float*
     {
         float4 w0, w1, w2;
         if (kSmemW) {
-            const float4* w4 = reinterpret_cast<const float4*>(wtab) + (on ? 0 : 3);
-            w0 = w4[0]; w1 = w4[1]; w2 = w4[2];
+            // (wtab is a SHARED-window address here, formed once by the caller: the generic pointer made the compiler
+            //  rebuild the window base, seven uniform instructions, at every evaluation)
+            const uint32_t wa = (uint32_t)(uintptr_t)wtab + (on ? 0u : 48u);
+            asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(w0.x), "=f"(w0.y), "=f"(w0.z), "=f"(w0.w) : "r"(wa));
+            asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+16];" : "=f"(w1.x), "=f"(w1.y), "=f"(w1.z), "=f"(w1.w) : "r"(wa));
+            asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+32];" : "=f"(w2.x), "=f"(w2.y), "=f"(w2.z), "=f"(w2.w) : "r"(wa));
         } else {
             constexpr float wA[12] = HK_TRAP_WA, wB[12] = HK_TRAP_WB;
             w0 = make_float4(on ? wA[0] : wB[0], on ? wA[1] : wB[1], on ? wA[2] : wB[2], on ? wA[3] : wB[3]);
