@@ -193,6 +193,24 @@ int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes);
 int hk_compute(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
                double* out_k_dev, void* stream);
 
+/* hk_compute for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the workspace is a static device array inside the library, HK_STATIC_WS_BYTES
+ * (32 MiB) that every GPU which loads libhk.so holds until the process exits.  The call allocates nothing and frees
+ * nothing (no cudaMalloc / cudaFree / allocating library routine; the temporary storage of the CUB scans and sorts lies
+ * in the array too), needs no hk_set_workspace, and leaves a workspace bound with hk_set_workspace as it was.  Same
+ * definition, arguments, asynchrony and results as hk_compute (lines and out_k_dev are the caller's device buffers),
+ * for problems with hk_workspace_bytes(ctx, n_lines) <= HK_STATIC_WS_BYTES: about 1e5 lines on 5e4 bins, or 2e5 lines
+ * on 1e4 bins (~140 B per line + ~200 B per bin); anything larger returns HK_ENOSPC before touching the GPU.  Fixed
+ * cutting length or none only (HK_ESTATE in the width-relative cut modes).  The first call on a device resolves the
+ * array's device address (cudaGetSymbolAddress; HK_ECUDA with hk_last_cuda_error if that fails).
+ * ONE array per device, shared by every context and every call: it holds the last call's contents (what must start at
+ * zero is cleared on `stream` by the call itself), so two calls whose GPU work OVERLAPS -- different streams, different
+ * contexts, different host threads -- race; order them on one stream or with events.  hk_get_stats / hk_get_extents /
+ * hk_get_phase_ms afterwards describe this call as long as no later hk_compute_static has run. */
+#define HK_STATIC_WS_BYTES (32u << 20)
+int hk_compute_static(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,
+                      double* out_k_dev, void* stream);
+
 /* Same as hk_compute but ADDS into out_k_dev instead of overwriting it (line lists that
  * arrive in blocks, L187: the sum over lines is order-independent, R16). */
 int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm,

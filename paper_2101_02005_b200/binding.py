@@ -21,10 +21,11 @@ _lib = C.CDLL(LIB_PATH)
 
 HK_OK, HK_EINVAL, HK_ESTATE, HK_ENOSPC, HK_ECUDA, HK_ENOMEM = 0, -1, -2, -3, -4, -5
 HK_Z1, HK_Z2, HK_Z4, HK_Z3 = 90000.0, 625.0, 49.0, 30.25
+HK_STATIC_WS_BYTES = 32 << 20     # include/hk.h: the static device workspace of hk_compute_static
 FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
-           "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
+           "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_static", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak", "hk_probe_fp32_ops",
            "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_node_kernel", "hk_set_single_pass", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode", "hk_compute_bands",
            "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
@@ -65,6 +66,8 @@ _lib.hk_workspace_bytes.restype = C.c_size_t
 _lib.hk_set_workspace.argtypes = [_vp, _vp, C.c_size_t]
 _lib.hk_compute.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
 _lib.hk_accumulate.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
+_lib.hk_compute_static.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, _vp, _vp]
+_lib.hk_compute_static.restype = C.c_int
 _lib.hk_compute_batch.argtypes = [_vp, C.POINTER(hk_lines), _i64, _d, C.c_int32, C.POINTER(_d), C.POINTER(_d), C.POINTER(_d),
                                   _vp, _vp]
 _lib.hk_compute_batch.restype = C.c_int
@@ -239,6 +242,16 @@ class Opacity:
         cut = float(cut) if cut is not None else 0.0
         fn = _lib.hk_accumulate if accumulate else _lib.hk_compute
         self._check(fn(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)), "hk_compute")
+        return out
+
+    def compute_static(self, lines, cut, out, stream=None):
+        """hk_compute_static: hk_compute on the library's static device workspace (HK_STATIC_WS_BYTES): no allocation on
+        the call path -- `out` is the caller's, no workspace tensor is created.  HKError(HK_ENOSPC) beyond the limit."""
+        ls, n = _lines_struct(lines)
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.N
+        cut = float(cut) if cut is not None else 0.0
+        self._check(_lib.hk_compute_static(self._ctx, C.byref(ls), n, cut, out.data_ptr(), _stream_ptr(stream)),
+                    "hk_compute_static")
         return out
 
     def compute_batch(self, lines, cut, T, P_atm, Q, out=None, stream=None):

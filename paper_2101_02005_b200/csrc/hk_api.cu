@@ -813,6 +813,61 @@ int hk_accumulate(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cu
     return compute_any(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, false);
 }
 
+}  // extern "C"
+
+// ---- hk_compute_static: the hot path on a workspace nobody allocates -------------------------------------------------
+// The workspace of hk_compute is the caller's (hk_set_workspace).  A caller that cannot allocate device memory at all gets
+// this one instead: HK_STATIC_WS_BYTES of device memory that belong to the library image (every GPU that loads libhk.so
+// holds them until the process exits).  In HOST code the name g_static_ws is a host-side stand-in, not a device address:
+// the address the kernels need comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_ws[HK_STATIC_WS_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+void* g_static_ws_addr[kMaxDevices];          // per device ordinal; null until resolved
+
+// -> HK_OK and the device address of g_static_ws on the CURRENT device
+int static_ws_address(hk_ctx* ctx, void** out)
+{
+    int dev = -1;
+    HK_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return HK_EINVAL;
+    if (!g_static_ws_addr[dev]) {
+        void* p = nullptr;
+        HK_CUDA(cudaGetSymbolAddress(&p, g_static_ws));
+        if (!p || ((uintptr_t)p & 255u) != 0) return HK_ECUDA;
+        g_static_ws_addr[dev] = p;
+    }
+    *out = g_static_ws_addr[dev];
+    return HK_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int hk_compute_static(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, double* out_k_dev, void* stream_v)
+{
+    if (!ctx || !out_k_dev || n_lines < 0 || n_lines >= 2147483647LL || std::isnan(cut_cm)) return HK_EINVAL;
+    if (n_lines > 0 && !lines_ok(lines)) return HK_EINVAL;
+    if (!ctx->have_cond) return HK_ESTATE;
+    if (ctx->cut_mode != 0 && !is_uncut(cut_cm)) return HK_ESTATE;     // (width-relative cuts read counters back between passes)
+    if (make_layout(ctx, n_lines).total > (size_t)HK_STATIC_WS_BYTES) return HK_ENOSPC;
+    void* ws = nullptr;
+    const int rc_ws = static_ws_address(ctx, &ws);
+    if (rc_ws != HK_OK) return rc_ws;
+    // the caller's own workspace binding (if any) steps aside for this call.  The static array keeps what the last call on
+    // it -- of ANY context -- left there: everything compute_impl needs at zero it clears itself on the stream (counters,
+    // work-unit counts, node and extent-end sums, the sort's buckets), and the single-pass hint of the previous call is
+    // discarded (hint_ready = false: a list the previous call found sorted is no statement about this one's context)
+    void* const ws0 = ctx->ws;
+    const size_t bytes0 = ctx->ws_bytes;
+    const bool hint0 = ctx->hint_ready;
+    ctx->ws = ws; ctx->ws_bytes = (size_t)HK_STATIC_WS_BYTES; ctx->hint_ready = false;
+    const int rc = compute_any(ctx, lines, n_lines, cut_cm, out_k_dev, (cudaStream_t)stream_v, true);
+    ctx->ws = ws0; ctx->ws_bytes = bytes0; ctx->hint_ready = hint0;
+    return rc;
+}
+
 int hk_compute_batch(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, double cut_cm, int32_t n_cond, const double* T_K,
                      const double* P_atm, const double* Q, double* out_k_dev, void* stream_v)
 {
@@ -1230,7 +1285,7 @@ const char* hk_strerror(int status)
         case HK_OK: return "ok";
         case HK_EINVAL: return "invalid argument";
         case HK_ESTATE: return "call out of order (conditions / workspace / compute missing)";
-        case HK_ENOSPC: return "workspace too small";
+        case HK_ENOSPC: return "workspace too small (hk_compute_static: problem larger than HK_STATIC_WS_BYTES)";
         case HK_ECUDA: return "CUDA call failed (see hk_last_cuda_error)";
         case HK_ENOMEM: return "host allocation failed";
         default: return "unknown status";
