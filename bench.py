@@ -275,7 +275,7 @@ def _kernel_flops(st):
         # line centres, rows: two-term outside the core, Gauss-Hermite 4 / 6 rings, the 10-point class of wide lines
         "centre": (f"centre_row_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
                    + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * g10_row),
-        # line centres, innermost bins: trapezoid rule with pole term (y < 2), 10-point rule of narrow lines
+        # line centres, innermost bins: trapezoid rule with pole term (y < 1.8), 10-point rule of narrow lines
         "lane": (f"centre_lane_kernel<{kb}>", FLOP["gh10"] * g10_lane + FLOP["trap"] * n_trap),
     }
 

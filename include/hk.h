@@ -65,7 +65,7 @@ typedef struct {
     int64_t n_evals_mid;   /* HK_Z2 <= |z|^2 < HK_Z1 (2-term asymptotic) */
     int64_t n_evals_core;  /* |z|^2 < HK_Z2: 4-point Gauss-Hermite (outer ring), 6-point, trapezoid + pole term innermost */
     int64_t n_evals_gh6;   /* of n_evals_core: the 6-point ring (HK_Z3 <= |z|^2 < HK_Z4 at small y; see HK_Z4 for its dependence on y) */
-    int64_t n_evals_trap;  /* of n_evals_core: |z|^2 < HK_Z3 and y < 3 (trapezoid, or 10-point Gauss-Hermite when y >= 2) */
+    int64_t n_evals_trap;  /* of n_evals_core: |z|^2 < HK_Z3 (21 when y >= 1) and y < 3 (trapezoid, or 10-point Gauss-Hermite when y >= 1.8) */
     int64_t n_units_far;   /* (tile, line-chunk) work units run by the far kernel */
     int64_t n_units_mid;   /* ... by the mid kernel */
     int64_t n_units_near;  /* ... by the near/edge kernel */
@@ -79,7 +79,7 @@ typedef struct {
     int64_t n_pairs_centre; /* (line, bin) slots the centre kernel walked (two-term outside the core, core evaluators inside) */
     int64_t n_pairs_node;  /* (line, tile) pairs evaluated at the tile's HK_NODES Chebyshev nodes (two-term asymptotic) */
     int64_t n_bins_node;   /* (line, bin) pairs those node evaluations stand for */
-    int64_t n_evals_gh10;  /* of n_evals_trap: lines with y >= 2, evaluated by the 10-point Gauss-Hermite rule */
+    int64_t n_evals_gh10;  /* of n_evals_trap: lines with y >= 1.8, evaluated by the 10-point Gauss-Hermite rule */
     int64_t n_pairs_edge_node; /* (line, extent end) pairs evaluated at the nodes of their edge tile (per-bin accumulators) */
     int64_t n_launches;    /* kernels of this library launched by the last hk_compute (CUB passes excluded) */
     int64_t n_plinth_illcond; /* plinth removal: lines with V(cut) > V(0) / HK_PLINTH_RATIO, whose difference V - V(cut) is
@@ -108,7 +108,7 @@ enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, H
 #define HK_Z4 49.0f    /* 7 <= |z| < 25: 4-point Gauss-Hermite rational form, <= 3e-6; below: 6-point.  The rings shrink as y grows
                           (the pole moves away from the real axis): 4 points from |z|^2 >= 36 for y >= 1.5, >= 30.25 for y >= 3, and
                           on the whole core for y >= 4.5; 6 points on the whole core for y >= 3 (hk_device.cuh: z4_for, z3_for) */
-#define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3) and y < 3: trapezoid rule + pole term, <= 2e-6; 10-point Gauss-Hermite when y >= 2, <= 2.7e-6 */
+#define HK_Z3 30.25f   /* |z| < 5.5 (|z|^2 < 50 when y < 1e-3, < 21 when y >= 1) and y < 3: trapezoid rule + pole term, <= 2e-6; 10-point Gauss-Hermite when y >= 1.8, <= 9e-6 */
 #ifndef HK_NODES
 #define HK_NODES 12    /* Chebyshev nodes per tile of the separated-tile evaluation; 8, 10 or 12 */
 #endif
@@ -332,7 +332,7 @@ int hk_probe_fp32_peak(int packed, int iters, double* flops_out, float* ms_out, 
  * Fig. 4): out[i] = Re w(x[i] + i y[i]) exactly as the accumulation
  * kernels evaluate it (region chosen by |z|^2 with alpha_D = 1 bin).  DEVICE fp32
  * arrays of n.  region_out (optional, int32): 0 far, 1 mid, 2 Gauss-Hermite 4, 3 Gauss-Hermite 6, 4 trapezoid,
- * 5 Gauss-Hermite 10 (|z|^2 < HK_Z3 and y >= 2). */
+ * 5 Gauss-Hermite 10 (|z|^2 < HK_Z3 and y >= 1.8). */
 int hk_eval_voigt_f32(const float* x_dev, const float* y_dev, int64_t n, float* out_dev,
                       int32_t* region_out_dev, void* stream);
 

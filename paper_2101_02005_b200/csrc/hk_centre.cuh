@@ -10,13 +10,13 @@
 //            R2   two asymptotic terms                  (every bin of the tile has |z|^2 >= Z2)
 //            R4   4-point Gauss-Hermite, cubic/quartic  (every bin has |z|^2 >= Z4)
 //            R6m  6-point Gauss-Hermite, quintic/sextic (the tile holds bins with |z|^2 < Z4), zero where X < xl
-//            R10  10-point Gauss-Hermite, degree 9/10   (the tile holds bins with |z|^2 < Z3 of a line with y >= 2)
+//            R10  10-point Gauss-Hermite, degree 9/10   (the tile holds bins with |z|^2 < Z3 of a line with y >= 1.8)
 //            R2m  two terms, zero where X < xl          (lines narrower than a fifth of a bin: the whole core is lane work)
 //        A warp is a work unit of its own (no block-level synchronisation anywhere); its 32 KB bins reach k(nu) with one
 //        fp64 atomic per bin per unit.
 //   centre_lane_kernel<KB,W,kBinned>   the innermost bins, X < xl (|z| < 5.5, or the whole core of a narrow line):
 //        lane <-> line, 32 lines step through the same bins, each evaluating its own line there -- 10-point
-//        Gauss-Hermite (y >= 2), trapezoid rule with pole term (y < 2), the bare Gaussian (y = 0) or the bin-averaged
+//        Gauss-Hermite (y >= 1.8), trapezoid rule with pole term (y < 1.8), the bare Gaussian (y = 0) or the bin-averaged
 //        Gaussian.  A batch is counting-sorted by y = Gamma_L/alpha_D when it is staged, so the 32 lines of a group
 //        share evaluator and ring width.  Values go through a shared staging matrix and are summed per bin (a
 //        transpose, no atomics).
@@ -94,8 +94,8 @@ __device__ __forceinline__ CentreLine centre_setup(const float4 ra, const float4
     L.xl = z3 - L.y2;                                              // (<= 0 for y >= 3: the 6-point rows take the whole tile)
     L.row = has_gh ? kRowR6m : kRowNone;
     if (L.xl > 0.f && Xmin < L.xl) {
-        // innermost bins.  y >= 2: the 10-point rule converges on all of them -- as a row over the whole tile when X^10
-        // stays inside fp32 (a >= 0.85 bins per 64 bins of tile), else in the lane pass.  y < 2: trapezoid rule, lane pass
+        // innermost bins.  y >= 1.8 (HK_Y10): the 10-point rule converges on all of them -- as a row over the whole tile when X^10
+        // stays inside fp32 (a >= 0.85 bins per 64 bins of tile), else in the lane pass.  y < 1.8: trapezoid rule, lane pass
         constexpr float kWide = 1.0f / (0.85f * (float)(KB / 2));
         if (L.y2 >= HK_Y10 * HK_Y10 && has_gh && L.inva < kWide) { L.row = kRowR10; L.xl = -1.0f; }
         else L.lane = L.y2 == 0.f ? kLaneGauss : L.y2 >= HK_Y10 * HK_Y10 ? kLaneGH10 : kLaneTrap;
@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
                 }
             }
         };
-        // ---- R10: N(X)/D'(X), degree 9 over degree 10, the whole tile (y >= 2); records rw[0..5][0..n)
+        // ---- R10: N(X)/D'(X), degree 9 over degree 10, the whole tile (y >= 1.8); records rw[0..5][0..n)
         auto run_r10 = [&](int n) {
 #pragma unroll 1
             for (int l = 0; l < n; ++l) {

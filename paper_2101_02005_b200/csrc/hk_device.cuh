@@ -168,10 +168,10 @@ __device__ __forceinline__ float gh6_K(float x2, float s, float y)
     return y * num * rcp_approx(D12 * D3);
 }
 
-// 10-point rule for the innermost region when the pole is far enough from the real axis: for y >= 2 the quadrature
-// converges on all of |z|^2 < HK_Z3 (measured in fp32 against the oracle: <= 2.7e-6), at a quarter of the cost of
-// the trapezoid evaluator with its pole term.
-#define HK_Y10 2.0f
+// 10-point rule for the innermost region when the pole is far enough from the real axis: for y >= 1.8 the quadrature
+// converges on all of |z|^2 < HK_Z3 (in fp64 against w(z): <= 8.2e-6, worst at y = 1.8, x = 0; 2.6e-6 from y = 2 on), at
+// a quarter of the cost of the trapezoid evaluator with its pole term.
+#define HK_Y10 1.8f
 __device__ __forceinline__ float gh10_K(float x2, float s, float y)
 {
     constexpr float T1 = 0.11758132021177813f, T2 = 1.074562012436904f, T3 = 3.0859374437175497f,
@@ -191,8 +191,8 @@ __device__ __forceinline__ float gh10_K(float x2, float s, float y)
 // The Gauss-Hermite rules converge faster the farther the pole lies from the real axis: the region each one is good
 // for grows with y.  Measured in fp64 against the oracle's w(z) on a lattice (worst case always at the smallest |z|):
 //   4 points: <= 3.0e-6 for |z|^2 >= 49 (any y), >= 36 (y >= 1.5), >= 30.25 (y >= 3); on ALL of the core for y >= 4.5 (5.7e-6)
-//   6 points: <= 4.8e-7 for |z|^2 >= 30.25 (any y);                                   on ALL of the core for y >= 3 (3.6e-6)
-//  10 points: on all of the core for y >= 2 (2.6e-6)
+//   6 points: <= 4.8e-7 for |z|^2 >= 30.25 (any y), <= 1.05e-6 for |z|^2 >= 21 (y >= 1); on ALL of the core for y >= 3 (3.6e-6)
+//  10 points: on all of the core for y >= 1.8 (8.2e-6; y >= 2: 2.6e-6)
 // so a line with y >= 4.5 -- the majority at high pressure -- has no inner rings at all.
 #define HK_Y4 4.5f
 #define HK_Y6 3.0f
@@ -206,9 +206,10 @@ __device__ __forceinline__ float z4_for(float y2)
 //  its amplitude, gauss_term below, and followed down to x^2 = HK_ZG: with the launch scale putting the largest
 //  amplitude at 2^100 that is the end of the fp32 range, 2^-126 -- DESIGN.md R22)
 #define HK_ZG 157.0f
+#define HK_Z3Y1 21.0f        // inner edge of the 6-point ring for y >= 1
 __device__ __forceinline__ float z3_for(float y2)
 {
-    return y2 == 0.f ? HK_ZG : y2 >= HK_Y6 * HK_Y6 ? 0.f : y2 < 1e-6f ? 50.0f : HK_Z3;
+    return y2 == 0.f ? HK_ZG : y2 >= HK_Y6 * HK_Y6 ? 0.f : y2 < 1e-6f ? 50.0f : y2 >= 1.0f ? HK_Z3Y1 : HK_Z3;
 }
 
 // cK exp(-x^2) for a pure Gaussian, amplitude and exponent combined BEFORE the exponential so that the product is

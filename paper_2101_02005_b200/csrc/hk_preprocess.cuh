@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(256, 4) line_kernel(Params p, const double* __
 __global__ void __launch_bounds__(256) region_stats_kernel(const float4* __restrict__ recA, const float4* __restrict__ recB,
                                                            int64_t n, int profile, int kb, DevStats* __restrict__ st)
 {
-    unsigned long long c[6] = {0, 0, 0, 0, 0, 0};        // below Z1, Z2, Z4, Z3 (trapezoid region), of that with y >= 2, of that in rows
+    unsigned long long c[6] = {0, 0, 0, 0, 0, 0};        // below Z1, Z2, Z4, Z3 (trapezoid region), of that with y >= HK_Y10, of that in rows
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const float4 ra = recA[i], rb = recB[i];
         const int32_t ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);

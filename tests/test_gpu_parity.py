@@ -1115,10 +1115,16 @@ def test_evaluator_accuracy_map(B):
     ys = np.logspace(-2, 7, 576)
     X, Y = np.meshgrid(xs, ys, indexing="ij")
     # region boundaries +- a few ulp
-    for z2 in (B.HK_Z1, B.HK_Z2, B.HK_Z4, B.HK_Z3, 50.0, 88.0):
+    for z2 in (B.HK_Z1, B.HK_Z2, B.HK_Z4, 36.0, B.HK_Z3, 21.0, 50.0, 88.0):
         for yv in np.logspace(-2, math.log10(math.sqrt(z2)) - 1e-3, 64):
             xb = math.sqrt(z2 - yv * yv)
             xe = xb * (1 + np.array([-4, -2, -1, 0, 1, 2, 4]) * 6e-8)
+            X = np.concatenate([X.ravel(), xe])
+            Y = np.concatenate([Y.ravel(), np.full(xe.size, yv)])
+    # the values of y at which the rings change (z3_for, z4_for, HK_Y10: hk_device.cuh), from both sides, x dense across the core
+    for yb in (1.0, 1.5, 1.8, 3.0, 4.5):
+        for yv in (yb * (1 - 1e-6), yb, yb * (1 + 1e-6), yb * 1.03):
+            xe = np.linspace(0.0, 8.0, 801)
             X = np.concatenate([X.ravel(), xe])
             Y = np.concatenate([Y.ravel(), np.full(xe.size, yv)])
     x32 = X.ravel().astype(np.float32)
