@@ -39,7 +39,7 @@ UNIT = "lines/s"
 FP32_LANES_PER_SM = 128          # FP32 FMA lanes per SM (4 SMSPs x 32), DESIGN.md section 7
 # algorithmic FLOPs per Voigt evaluation by formula (FMA = 2, add/mul/reciprocal = 1):
 # far 1 term, mid 2 terms, 4/6/10-point Gauss-Hermite rational forms, trapezoid rule with pole term
-FLOP = {"far": 6.0, "mid": 12.0, "gh4": 24.0, "gh6": 36.0, "gh10": 52.0, "trap": 125.0}
+FLOP = {"far": 6.0, "mid": 12.0, "gh4": 23.0, "gh6": 36.0, "gh10": 52.0, "trap": 125.0}
 
 
 def _workload_name(cfg, n):

@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
     constexpr int kTB = 32 * KB;
     // per warp: the row records of the 32 staged lines, bucketed by class.  float4 x 4 per record:
     //   R2 / R2m: A = { ndl, nf, G2, c },       B = { 1.5 a^2, -2 a^2 G^2, inva, nfa },  C = { xl, ... }
-    //   R4      : A = { ndl, nfa, inva, 1/P },  B = { n0, n1, n2, d3/P },  C = { d0/P, d1/P, d2/P, - }
+    //   R4      : A = { -, u0 = ndl inva + nfa, inva, 1/P },  B = { n0, n1, n2, d3/P },  C = { d0/P, d1/P, d2/P, - }
     //   R6m     : A = { ndl, nfa, inva, xl },   B = { n0, n1, n2, n3 },  C = { n4, d0/P, d1/P, d2/P },  D = { d3/P, d4/P, d5/P, 1/P }
     //   R10     : A = { ndl, nfa, inva, 1/P },  B, C = { n0 .. n7 },  D = { n8, d0/P, d1/P, d2/P },  E = { d3/P .. d6/P },  F = { d7/P, d8/P, d9/P, - }
     //   (P = cK y, the amplitude of the Gauss-Hermite forms, divides the DENOMINATOR's coefficients: the leading 1 becomes
@@ -355,7 +355,9 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
                 if (rc == kRowR4) {
                     float n[3], d[4];
                     gh4_coeffs(L.y2, n, d);
-                    A = make_float4(L.ndl, L.nfa, L.inva, ip);
+                    // (u = b inva + u0 with u0 = ndl inva + nfa: no bin of an R4 visit is masked, so its u need not match the
+                    //  lane pass bit for bit, and |u0| <= 64 inva ulps are far inside the evaluator's budget)
+                    A = make_float4(0.f, __fmaf_rn(L.ndl, L.inva, L.nfa), L.inva, ip);
                     B = make_float4(n[0], n[1], n[2], d[3] * ip);
                     C = make_float4(d[0] * ip, d[1] * ip, d[2] * ip, 0.f);
                 } else if (rc == kRowR6m || rc == kRowR10) {
@@ -438,13 +440,12 @@ __global__ void __launch_bounds__(32 * kRowWarps, kRowCtas) centre_row_kernel(Ac
 #pragma unroll 4
             for (; l < e4; ++l) {
                 const float4 ea = rw[0][l], eb = rw[1][l], ec = rw[2][l];
-                const float2 ndl = bcast2(ea.x), nfa = bcast2(ea.y), ia = bcast2(ea.z), ip = bcast2(ea.w);
+                const float2 u0 = bcast2(ea.y), ia = bcast2(ea.z), ip = bcast2(ea.w);
                 const float2 n0 = bcast2(eb.x), n1 = bcast2(eb.y), n2c = bcast2(eb.z), d3 = bcast2(eb.w);
                 const float2 d0 = bcast2(ec.x), d1 = bcast2(ec.y), d2 = bcast2(ec.z), n3 = bcast2(kGhN);
 #pragma unroll
                 for (int m = 0; m < M; ++m) {
-                    const float2 d = __fadd2_rn(tb[m], ndl);          // exact: both are small integers
-                    const float2 un = __ffma2_rn(d, ia, nfa);
+                    const float2 un = __ffma2_rn(tb[m], ia, u0);
                     const float2 X = __fmul2_rn(un, un);
                     float2 N = __ffma2_rn(n3, X, n2c);
                     N = __ffma2_rn(N, X, n1);
