@@ -918,6 +918,7 @@ __device__ __forceinline__ void nl_candidates(const Params& p, const Levels& lv,
     }
 }
 
+constexpr int kNLDirect = 3;      // node pairs (of kP / 2) whose two reciprocals are taken directly instead of through their product
 __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params p, AccArgs a)
 {
     constexpr int M = kP / 2;
@@ -1033,6 +1034,10 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
                             for (int m = 0; m < M; ++m) {
                                 const float2 t = __fadd2_rn(xk[m], np2);
                                 const float2 q = __ffma2_rn(t, t, g2);
+                                if (m >= M - kNLDirect) {                          // (a share of the reciprocals taken one by one:
+                                    acc[m] = __ffma2_rn(c2, make_float2(rcp_approx(q.x), rcp_approx(q.y)), acc[m]);   //  two instructions
+                                    continue;                                      //  fewer, one more on the special-function unit)
+                                }
                                 const float R = rcp_approx(q.x * q.y);             // 1/q.x = R q.y, 1/q.y = R q.x
                                 acc[m] = __ffma2_rn(c2, make_float2(R * q.y, R * q.x), acc[m]);
                             }
@@ -1043,8 +1048,9 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
                             for (int m = 0; m < M; ++m) {
                                 const float2 t = __fadd2_rn(xk[m], np2);
                                 const float2 q = __ffma2_rn(t, t, g2);
-                                const float R = rcp_approx(q.x * q.y);
-                                const float2 rr = make_float2(R * q.y, R * q.x);
+                                float2 rr;
+                                if (m >= M - kNLDirect) rr = make_float2(rcp_approx(q.x), rcp_approx(q.y));
+                                else { const float R = rcp_approx(q.x * q.y); rr = make_float2(R * q.y, R * q.x); }
                                 const float2 uu = __ffma2_rn(nA2, rr, A1);
                                 const float2 vv = __ffma2_rn(uu, rr, one);
                                 const float2 ww = __fmul2_rn(rr, vv);
@@ -1145,8 +1151,10 @@ __global__ void __launch_bounds__(kThreads, 3) edge_node_kernel(Params p, AccArg
                         for (int mm = 0; mm < M; ++mm) {
                             const float2 t = __fadd2_rn(xk[mm], np2);
                             const float2 q = __ffma2_rn(t, t, g2);
-                            const float R = rcp_approx(q.x * q.y);
-                            const float2 ww = __fmul2_rn(c2, make_float2(R * q.y, R * q.x));
+                            float2 rr;                                       // (as node_lines_kernel: kNLDirect)
+                            if (mm >= M - kNLDirect) rr = make_float2(rcp_approx(q.x), rcp_approx(q.y));
+                            else { const float R = rcp_approx(q.x * q.y); rr = make_float2(R * q.y, R * q.x); }
+                            const float2 ww = __fmul2_rn(c2, rr);
                             v[2 * mm] = ww.x; v[2 * mm + 1] = ww.y;
                         }
                     } else {
@@ -1156,8 +1164,9 @@ __global__ void __launch_bounds__(kThreads, 3) edge_node_kernel(Params p, AccArg
                         for (int mm = 0; mm < M; ++mm) {
                             const float2 t = __fadd2_rn(xk[mm], np2);
                             const float2 q = __ffma2_rn(t, t, g2);
-                            const float R = rcp_approx(q.x * q.y);
-                            const float2 rr = make_float2(R * q.y, R * q.x);
+                            float2 rr;
+                            if (mm >= M - kNLDirect) rr = make_float2(rcp_approx(q.x), rcp_approx(q.y));
+                            else { const float R = rcp_approx(q.x * q.y); rr = make_float2(R * q.y, R * q.x); }
                             const float2 uu = __ffma2_rn(nA2, rr, A1);
                             const float2 vv = __ffma2_rn(uu, rr, one);
                             const float2 ww = __fmul2_rn(c2, __fmul2_rn(rr, vv));
