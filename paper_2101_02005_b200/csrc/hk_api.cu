@@ -603,7 +603,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     HK_CUDA(cudaMemsetAsync(counts, 0, (size_t)n_counts * 4, stream));
     range_kernel<<<(p.n_ct + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, cnt_far, cnt_mid, cnt_edge, cnt_centre,
                                                            cnt_near, cnt_lane, st);
-    ctx->last_launches = 5 + (try_single ? 2 : 0) + ((counting && !reuse_sort) ? 1 : 0);   // line, scale, gather / scatter, range (+ single pass and its decision, hint; node range below)
+    ctx->last_launches = 4 + (try_single ? 2 : 0) + ((counting && !reuse_sort) ? 1 : 0);   // line, scale, gather / scatter, range (+ single pass and its decision, hint; node range below)
     if (lv.n_entries > 0) {
         HK_CUDA(cudaMemsetAsync(node_acc, 0, (size_t)lv.n_entries * kP * sizeof(double), stream));
         node_range_kernel<<<(lv.n_entries + 255) / 256, 256, 0, stream>>>(p, lv, keys_out, n, tr, nr, cnt_node, st);
