@@ -143,6 +143,18 @@ __device__ __forceinline__ int64_t centre_bin(const Params& p, double ctr)
     return (int64_t)c;
 }
 
+// a / dnu, correctly rounded like the IEEE division the oracle performs, in three operations: with y = RN(1/dnu)
+// (p.inv_dnu, an IEEE division on the host) and q0 = RN(a y) -- within one ulp of the quotient -- the residual
+// r = a - dnu q0 is exact under FMA and RN(q0 + r y) is the correctly rounded quotient (Markstein's theorem).  A
+// quotient beyond 2^62 bins (where q0 may already be infinite) is used as it is: every caller clamps it to 4e18.
+__device__ __forceinline__ double div_by_dnu(const Params& p, double a)
+{
+    const double q0 = __dmul_rn(a, p.inv_dnu);
+    const double r = __fma_rn(-p.dnu, q0, a);
+    const double q1 = __fma_rn(r, p.inv_dnu, q0);
+    return fabs(q0) < 4.6e18 ? q1 : q0;
+}
+
 struct LineOut {
     bool valid;       // passes the R14 checks
     bool on_grid;     // extent non-empty and centre within 2^30 bins
@@ -195,7 +207,7 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
     if (!isfinite(o.gammaL) || !isfinite(o.S) || !isfinite(o.cK)) { o.valid = false; o.S = o.gammaL = o.alphaD = o.cK = 0.0; return o; }
     const double big = 4.0e18;
     nu0 = ctr;
-    double pos = __ddiv_rn(__dsub_rn(nu0, p.numin), p.dnu);
+    double pos = div_by_dnu(p, __dsub_rn(nu0, p.numin));
     double c = floor(pos);
     c = fmin(fmax(c, -big), big);
     o.jc = (int64_t)c;
@@ -207,8 +219,8 @@ __device__ __forceinline__ LineOut line_math(const Params& p, double nu0, double
             if (!(cutl > 0.0)) return o;                                        // zero width: no extent
             if (!(cutl >= p.cls_lo && cutl < p.cls_hi)) { o.foreign = true; return o; }
         }
-        double lo = ceil(__ddiv_rn(__dsub_rn(__dsub_rn(nu0, cutl), p.numin), p.dnu));
-        double hi = floor(__ddiv_rn(__dsub_rn(__dadd_rn(nu0, cutl), p.numin), p.dnu));
+        double lo = ceil(div_by_dnu(p, __dsub_rn(__dsub_rn(nu0, cutl), p.numin)));
+        double hi = floor(div_by_dnu(p, __dsub_rn(__dadd_rn(nu0, cutl), p.numin)));
         if (lo < 0.0) lo = 0.0;
         if (hi > (double)(p.N - 1)) hi = (double)(p.N - 1);
         lo = fmin(lo, big);
