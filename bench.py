@@ -267,7 +267,9 @@ def _kernel_flops(st):
     g10_lane = st["n_evals_gh10"] - g10_row
     kb = st["bins_per_lane"]
     return {
-        "node": ("node_kernel", (FLOP["mid"] * (st["n_pairs_node"] - st["n_pairs_node_far"]) + FLOP["far"] * st["n_pairs_node_far"]) * HK_NODES),
+        # separated (line, tile) pairs at the tile's nodes: one term (far), two terms, or -- the core at nodes -- the 4-point form
+        "node": ("node_lines_kernel", (FLOP["mid"] * (st["n_pairs_node"] - st["n_pairs_node_far"] - st["n_pairs_node_core"])
+                                       + FLOP["far"] * st["n_pairs_node_far"] + FLOP["gh4"] * st["n_pairs_node_core"]) * HK_NODES),
         "far": (f"interior_kernel<{kb},false>", FLOP["far"] * st["n_pairs_far"]),
         "mid": (f"interior_kernel<{kb},true>", FLOP["mid"] * st["n_pairs_mid"]),
         # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end
@@ -472,7 +474,7 @@ def run_ours(args):
            "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"],
                                "core_gh6": st["n_evals_gh6"], "core_trap": st["n_evals_trap"], "core_gh10": st["n_evals_gh10"],
                                "core_gh10_row": st["n_evals_gh10_row"]},
-           "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
+           "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "node_tiles_core": st["n_pairs_node_core"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
                                "edge": st["n_pairs_edge"], "edge_node_ends": st["n_pairs_edge_node"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
            "bins_per_lane": st["bins_per_lane"], "sorted_input": st["n_unsorted"] == 0,
            "single_pass_preprocess": bool(st["single_pass"]),

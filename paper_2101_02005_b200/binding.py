@@ -27,7 +27,7 @@ FIELDS = ("nu0", "A", "g_up", "E_low", "gamma_ref", "n_exp")
 EXPORTS = ("hk_create", "hk_destroy", "hk_grid_size", "hk_set_conditions", "hk_workspace_bytes",
            "hk_set_workspace", "hk_compute", "hk_accumulate", "hk_compute_static", "hk_compute_batch", "hk_workspace_bytes_host", "hk_compute_host",
            "hk_get_extents", "hk_get_line_params", "hk_get_stats", "hk_get_phase_ms", "hk_probe_fp32_peak", "hk_probe_fp32_ops",
-           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_node_kernel", "hk_set_single_pass", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode", "hk_compute_bands",
+           "hk_eval_voigt_f32", "hk_set_debug_mode", "hk_set_tile_bins", "hk_set_node_separation", "hk_set_edge_nodes", "hk_set_node_kernel", "hk_set_core_nodes", "hk_set_single_pass", "hk_set_plinth", "hk_set_profile", "hk_set_cut_mode", "hk_compute_bands",
            "hk_set_conditions_hitran", "hk_compute_hitran", "hk_get_line_params_hitran",
            "hk_last_cuda_error", "hk_strerror")
 PHASES = ("preprocess", "sort", "ranges", "node", "far", "mid", "edge", "centre", "lane", "near", "down")
@@ -50,7 +50,7 @@ class hk_stats(C.Structure):
                                          "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_units_edge",
                                          "n_units_centre", "n_pairs_edge", "n_pairs_centre", "n_pairs_node",
                                          "n_bins_node", "n_evals_gh10", "n_pairs_edge_node", "n_launches",
-                                         "n_plinth_illcond", "n_evals_gh10_row", "n_pairs_node_eval", "n_pairs_node_far", "n_unsorted")] + \
+                                         "n_plinth_illcond", "n_evals_gh10_row", "n_pairs_node_eval", "n_pairs_node_far", "n_unsorted", "n_pairs_node_core")] + \
                [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("n_levels", C.c_int32),
                 ("single_pass", C.c_int32), ("reserved0", C.c_int32)]
 
@@ -96,6 +96,8 @@ _lib.hk_set_edge_nodes.argtypes = [_vp, C.c_int]
 _lib.hk_set_edge_nodes.restype = C.c_int
 _lib.hk_set_node_kernel.argtypes = [_vp, C.c_int]
 _lib.hk_set_node_kernel.restype = C.c_int
+_lib.hk_set_core_nodes.argtypes = [_vp, C.c_int]
+_lib.hk_set_core_nodes.restype = C.c_int
 _lib.hk_set_single_pass.argtypes = [_vp, C.c_int]
 _lib.hk_set_single_pass.restype = C.c_int
 _lib.hk_set_plinth.argtypes = [_vp, C.c_int]
@@ -212,6 +214,9 @@ class Opacity:
 
     def set_node_kernel(self, entry_stationary: bool):
         self._check(_lib.hk_set_node_kernel(self._ctx, 1 if entry_stationary else 0), "hk_set_node_kernel")
+
+    def set_core_nodes(self, on: bool):
+        self._check(_lib.hk_set_core_nodes(self._ctx, 1 if on else 0), "hk_set_core_nodes")
 
     def set_single_pass(self, on: bool):
         self._check(_lib.hk_set_single_pass(self._ctx, 1 if on else 0), "hk_set_single_pass")

@@ -1010,6 +1010,7 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
                 }
                 const float4* __restrict__ wrec = sRec + warp * (32 * kNLPerLane);
                 const int fLr = r.fL - wl, fRr = r.fR - wl;        // far boundaries relative to the warp's first line
+                const int gLr = r.gL - wl, gRr = r.gR - wl;        // core boundaries (empty unless core_nodes)
                 // the members among this warp's lines: up to four runs [s, e) of offsets (one, in dense lists); every
                 // bound below is warp-uniform, the lanes only compare their own offset with it
                 auto run = [&](int x0, int x1) {
@@ -1026,9 +1027,34 @@ __global__ void __launch_bounds__(kNLThreads, kNLCtas) node_lines_kernel(Params 
                         const float4 rec = wrec[o];
                         const uint32_t pk = (uint32_t)__float_as_int(rec.y);
                         const float f = (float)(pk >> 19) * (1.0f / 8192.0f);
-                        const float2 np2 = bcast2(-((float)(__float_as_int(rec.x) + D) + f)), g2 = bcast2(rec.z),
-                                     c2 = bcast2(member ? rec.w : 0.f);
-                        const bool far = all_far || (!none_far && (!member || o < fLr || o >= fRr));
+                        const float2 np2 = bcast2(-((float)(__float_as_int(rec.x) + D) + f)), g2 = bcast2(rec.z);
+                        // the core at nodes: lines whose core may reach this tile take the 4-point Gauss-Hermite form
+                        // K = y N(X, Y) / D(X, Y), X = t^2 / a^2, Y = G^2 / a^2, amplitude cK y = c sqrt(pi) / a^2; the other
+                        // lanes of the batch (amplitude 0, X = 0) follow with the asymptotic forms below
+                        const bool core = member && o >= gLr && o < gRr;
+                        if (__any_sync(0xffffffffu, core)) {
+                            const float a2c = __int_as_float((int)((pk & 0x7FFFFu) << 12));
+                            const float ia = (core && a2c > 0.f) ? __fdividef(1.0f, a2c) : 0.f;
+                            float n4[3], d4[4];
+                            gh4_coeffs(rec.z * ia, n4, d4);
+                            const float2 ia2 = bcast2(ia), amp = bcast2(core ? rec.w * 1.7724538509f * ia : 0.f);
+#pragma unroll
+                            for (int m = 0; m < M; ++m) {
+                                const float2 t = __fadd2_rn(xk[m], np2);
+                                const float2 X = __fmul2_rn(__fmul2_rn(t, t), ia2);
+                                float2 N = __ffma2_rn(bcast2(kGhN), X, bcast2(n4[2]));
+                                N = __ffma2_rn(N, X, bcast2(n4[1]));
+                                N = __ffma2_rn(N, X, bcast2(n4[0]));
+                                float2 Dn = __fadd2_rn(X, bcast2(d4[3]));
+                                Dn = __ffma2_rn(Dn, X, bcast2(d4[2]));
+                                Dn = __ffma2_rn(Dn, X, bcast2(d4[1]));
+                                Dn = __ffma2_rn(Dn, X, bcast2(d4[0]));
+                                acc[m] = __ffma2_rn(__fmul2_rn(amp, N), make_float2(rcp_approx(Dn.x), rcp_approx(Dn.y)), acc[m]);
+                            }
+                            if (!__any_sync(0xffffffffu, member && !core)) continue;
+                        }
+                        const float2 c2 = bcast2((member && !core) ? rec.w : 0.f);
+                        const bool far = all_far || (!none_far && (!member || core || o < fLr || o >= fRr));
                         if (all_far || (!none_far && __all_sync(0xffffffffu, far))) {
 #pragma unroll
                             for (int m = 0; m < M; ++m) {

@@ -48,6 +48,7 @@ struct hk_ctx {
     // sorted records of the last pass (for the on-demand region counts and hk_get_extents) with the sort's permutation
     const float4 *last_recA, *last_recB, *last_recN;
     const int32_t* last_idx;
+    int core_nodes;              // 1 (default): separated tiles of the core outside the inner region go to the node hierarchy
     int single_pass;             // 1 (default): a list the previous compute found sorted is preprocessed in one pass
     bool hint_ready;             // the DevHint of the bound workspace has been initialised
     bool in_batch;               // inside hk_compute_batch: tile ranges may serve later conditions with other widths
@@ -224,6 +225,7 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     if (p.profile == HK_PROFILE_LORENTZ) p.kappa1 = p.kappa2 = 0.0;      // no core, no second term: every pair is "far"
     p.inv1p_k1 = 1.0 / (1.0 + p.kappa1); p.inv1m_k1 = 1.0 / (1.0 - p.kappa1);
     p.inv1p_k2 = 1.0 / (1.0 + p.kappa2); p.inv1m_k2 = 1.0 / (1.0 - p.kappa2);
+    p.kappaN = p.kappa2; p.inv1p_kN = p.inv1p_k2; p.inv1m_kN = p.inv1m_k2; p.core_nodes = 0;
     p.kappa3 = std::sqrt((double)HK_ZG) * p.beta * 1.005;
     p.inv1p_k3 = 1.0 / (1.0 + p.kappa3); p.inv1m_k3 = 1.0 / (1.0 - p.kappa3);
     p.numin_bins = c->numin / c->dnu;
@@ -348,6 +350,7 @@ int hk_create(double numin, double numax, double dnu, hk_ctx** out)
     c->node_sep = HK_NODE_SEP;
     c->edge_nodes = 1;
     c->single_pass = 1;
+    c->core_nodes = 1;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
@@ -402,6 +405,13 @@ int hk_set_workspace(hk_ctx* ctx, void* dev_ptr, size_t bytes)
     ctx->ws_bytes = bytes;
     ctx->have_run = false;
     ctx->hint_ready = false;
+    return HK_OK;
+}
+
+int hk_set_core_nodes(hk_ctx* ctx, int on)
+{
+    if (!ctx) return HK_EINVAL;
+    ctx->core_nodes = on ? 1 : 0;
     return HK_OK;
 }
 
@@ -489,6 +499,13 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     //  masked direct edge kernel takes those tiles)
     p.edge_nodes = (L.edge_acc_bytes > 0 && ctx->edge_nodes && p.cut_mode == 0) ? 1 : 0;
     p.lane_tight = ctx->in_batch ? 0 : 1;
+    // the core at nodes: plain Voigt profile, fixed cut or none, default kernels, and ranges that serve this condition only
+    if (p.profile == HK_PROFILE_VOIGT && p.mode == 0 && p.cut_mode == 0 && !ctx->in_batch && !ctx->node_entry_stationary &&
+        ctx->core_nodes) {
+        p.core_nodes = 1;
+        p.kappaN = std::fmin(std::sqrt((double)HK_ZN) * p.beta * 1.001, p.kappa2);
+        p.inv1p_kN = 1.0 / (1.0 + p.kappaN); p.inv1m_kN = 1.0 / (1.0 - p.kappaN);
+    }
 
     // reuse (batched conditions on one resident list): 0 nothing, 1 the order of the lines by centre bin (any change of
     // condition), 2 everything but the Lorentz widths (same T, Q, mass: only the pressure moved)
@@ -1188,6 +1205,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_unsorted = (int64_t)d.n_unsorted;
     host_out->single_pass = d.single_pass;
     host_out->n_pairs_node_far = (int64_t)d.pairs_node_far;
+    host_out->n_pairs_node_core = (int64_t)d.pairs_node_core;
     host_out->n_pairs_node_eval = (int64_t)d.pairs_node_eval;
     host_out->n_evals_gh10_row = (int64_t)d.n_cnt_gh10_row;
     if (ctx->host_totals) {

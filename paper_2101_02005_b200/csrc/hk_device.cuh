@@ -61,6 +61,7 @@ struct __align__(8) NodeRange {
     int32_t a0, a1, b0, b1, c0, c1, d0, d1;
     int32_t fL, fR;      // lines with index < fL (left ranges) or >= fR (right ranges) have |z|^2 >= Z1 on the whole tile:
                          // one asymptotic term is enough (the lists are sorted by centre, so far lines are a prefix / suffix)
+    int32_t gL, gR;      // lines with gL <= index < gR may have |z|^2 < Z2 on the tile (the core at nodes): 4-point form
 };
 
 // ---- Chebyshev nodes of the separated-tile evaluation ----------------
@@ -206,6 +207,7 @@ __device__ __forceinline__ float z4_for(float y2)
 //  its amplitude, gauss_term below, and followed down to x^2 = HK_ZG: with the launch scale putting the largest
 //  amplitude at 2^100 that is the end of the fp32 range, 2^-126 -- DESIGN.md R22)
 #define HK_ZG 157.0f
+#define HK_ZN 49.0f          // the node hierarchy takes separated tiles with |z|^2 >= HK_ZN on all of them (4-point form valid for any y)
 #define HK_Z3Y1 21.0f        // inner edge of the 6-point ring for y >= 1
 __device__ __forceinline__ float z3_for(float y2)
 {

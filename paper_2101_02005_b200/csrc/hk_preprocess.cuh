@@ -53,6 +53,11 @@ struct Params {
     int64_t cb_floor, cb_ceil;  // floor/ceil of cut/dnu (bins)
     double kappa1, kappa2;      // sqrt(Z1) * beta and sqrt(Z2) * beta, slightly inflated
     double kappa3;              // sqrt(ZG) * beta: beyond it no line has innermost (lane-pass) bins
+    double kappaN;              // the node hierarchy takes separated tiles that lie beyond kappaN of the line: kappa2, or
+                                // sqrt(HK_ZN) * beta with core_nodes (the tiles of the core outside the inner region too)
+    double inv1p_kN, inv1m_kN;
+    int core_nodes;             // 1: node-handled pairs may lie inside the core (|z|^2 < Z2): evaluated at the nodes with the
+                                //    4-point Gauss-Hermite form ("the core at nodes")
     double inv1p_k1, inv1m_k1, inv1p_k2, inv1m_k2, inv1p_k3, inv1m_k3;   // 1/(1 + kappa), 1/(1 - kappa)
     double numin_bins;          // numin / dnu
     int32_t kb;                 // bins per lane (2, 4, 8)
@@ -90,6 +95,7 @@ struct DevStats {
     unsigned long long bins_node;                          // (line, bin) pairs those node evaluations stand for
     unsigned long long pairs_node_eval;                    // (line, tile) pairs the node kernel evaluated: must equal pairs_node
     unsigned long long pairs_node_far;                     // of pairs_node: |z|^2 >= Z1 on the whole tile (one asymptotic term)
+    unsigned long long pairs_node_core;                    // of pairs_node: |z|^2 < Z2 possible on the tile (4-point form at the nodes)
     unsigned long long shift_bits;                         // max |delta P| over the lines (cm^-1) as double bits (pressure shift)
     unsigned long long n_plinth_illcond;                   // plinth removal: lines whose cutting length falls inside their core
     unsigned long long n_unsorted;                         // adjacent pairs of valid lines out of centre-bin order (input order)
@@ -127,6 +133,16 @@ __device__ __forceinline__ void apply_shift_bound(Params& p, const DevStats* __r
 {
     const double s = __longlong_as_double((long long)st->shift_bits);
     if (s > 0.0) p.numin_bins += s / p.dnu;
+    // The core at nodes (core_nodes): no node-handled tile may reach into the INNER region of any line, where the profile
+    // is not the smooth function the 12 nodes resolve (the Gaussian of a line with next to no Lorentz width is followed to
+    // |z|^2 = 50 or HK_ZG).  z3max is the largest z3_for(y^2) of this launch's lines (line_record).
+    if (p.core_nodes) {
+        const float z3m = __uint_as_float((unsigned)st->z3max_bits);
+        if (z3m * 1.02f > HK_ZN) {
+            p.kappaN = fmin(sqrt((double)(z3m * 1.02f)) * p.beta * 1.001, p.kappa2);
+            p.inv1p_kN = 1.0 / (1.0 + p.kappaN); p.inv1m_kN = 1.0 / (1.0 - p.kappaN);
+        }
+    }
 }
 
 __device__ __forceinline__ bool finite6(double a, double b, double c, double d, double e, double f)
@@ -286,7 +302,8 @@ __device__ __forceinline__ int32_t line_record(const Params& p, const LineOut& o
         c.shiftb = max(c.shiftb, (unsigned long long)__double_as_longlong(o.shift));
         // (y^2 exactly as write_sorted_records forms it)
         const float y2f = (gauss || !(r.a2 > 0.f)) ? 0.f : __fdiv_rn(r.G2, r.a2);
-        c.z3b = max(c.z3b, (unsigned long long)__float_as_uint(z3_for(y2f)));
+        // (a damping too small for the Lorentzian wing to outweigh the Gaussian at |x| = 7 counts as none: HK_ZG)
+        c.z3b = max(c.z3b, (unsigned long long)__float_as_uint(y2f < 1.0e-30f ? HK_ZG : z3_for(y2f)));
         // (the per-region evaluation counts are reporting only: region_stats_kernel derives them from the records when
         //  hk_get_stats asks, so the fp64 pipe of this kernel is spent on the physics alone)
     }
@@ -735,8 +752,8 @@ __device__ __forceinline__ NodeKeys node_keys(const Params& p, int64_t w0, int64
     k.hiR = p.uncut ? kBigKey : w0 + p.cb_floor - 2;
     const int64_t sepL = (int64_t)floor(m - p.sep * h) - 1;
     const int64_t sepR = (int64_t)ceil(m + p.sep * h);
-    k.upL = min(sepL, left_bound((double)w0, p.kappa2, p.inv1p_k2, p.numin_bins));
-    k.dnR = max(sepR, right_bound((double)(w1 - 1), p.kappa2, p.inv1m_k2, p.numin_bins));
+    k.upL = min(sepL, left_bound((double)w0, p.kappaN, p.inv1p_kN, p.numin_bins));
+    k.dnR = max(sepR, right_bound((double)(w1 - 1), p.kappaN, p.inv1m_kN, p.numin_bins));
     // empty sets are written as [lo, lo - 1] / [hi + 1, hi]
     k.upL = max(k.upL, k.loL - 1);
     k.dnR = min(k.dnR, k.hiR + 1);
@@ -837,6 +854,12 @@ __global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, co
     // where one asymptotic term suffices on the whole tile (|z|^2 >= Z1): the same bound range_kernel uses for "far"
     r.fL = idx_of(p, keys, n_act, left_bound((double)w0, p.kappa1, p.inv1p_k1, p.numin_bins) + 1);
     r.fR = idx_of(p, keys, n_act, right_bound((double)(min(p.N, w0 + W) - 1), p.kappa1, p.inv1m_k1, p.numin_bins));
+    // where the two asymptotic terms do not hold on the whole tile (the core at nodes): the bound range_kernel uses for "mid"
+    r.gL = r.gR = 0;
+    if (p.core_nodes) {
+        r.gL = idx_of(p, keys, n_act, left_bound((double)w0, p.kappa2, p.inv1p_k2, p.numin_bins) + 1);
+        r.gR = idx_of(p, keys, n_act, right_bound((double)(min(p.N, w0 + W) - 1), p.kappa2, p.inv1m_k2, p.numin_bins));
+    }
     nr[e] = r;
     const int64_t tot = (int64_t)(r.a1 - r.a0) + (r.b1 - r.b0) + (r.c1 - r.c0) + (r.d1 - r.d0);
     counts[e] = (int32_t)((tot + p.chunk_node - 1) / p.chunk_node);
@@ -844,6 +867,9 @@ __global__ void __launch_bounds__(256) node_range_kernel(Params p, Levels lv, co
         const int64_t nfar = (int64_t)max(0, min(r.a1, r.fL) - r.a0) + max(0, min(r.b1, r.fL) - r.b0)
                            + max(0, r.c1 - max(r.c0, r.fR)) + max(0, r.d1 - max(r.d0, r.fR));
         if (nfar) atomicAdd(&st->pairs_node_far, (unsigned long long)nfar);
+        auto within = [&](int32_t x0, int32_t x1) { return (int64_t)max(0, min(x1, r.gR) - max(x0, r.gL)); };
+        const int64_t ncore = within(r.a0, r.a1) + within(r.b0, r.b1) + within(r.c0, r.c1) + within(r.d0, r.d1);
+        if (ncore) atomicAdd(&st->pairs_node_core, (unsigned long long)ncore);
         atomicAdd(&st->pairs_node, (unsigned long long)tot);
         atomicAdd(&st->bins_node, (unsigned long long)tot * (unsigned long long)(min(p.N, w0 + W) - w0));
     }
@@ -897,17 +923,6 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
     fr1 = max(min(fr1, r.A1), ml1);
     fr0 = max(min(fr0, fr1), ml1);
     mr0 = max(min(mr0, fr0), ml1);
-    // node-handled lines (this tile's nodes or an ancestor's): a prefix of the left interior classes and a
-    // suffix of the right ones
-    int32_t nl = fl0, nrr = fr1;
-    if (lv.n_levels > 0) {
-        const NodeKeys k = node_keys(p, w0, wb);
-        nl = min(max(idx_of(p, keys, n_act, k.upL + 1), fl0), ml1);
-        nrr = max(min(idx_of(p, keys, n_act, k.dnR), fr1), mr0);
-    }
-    fl1 = max(fl1, nl);
-    fr0 = min(fr0, nrr);
-    r.FL0 = fl0; r.NL = nl; r.FL1 = fl1; r.ML1 = ml1; r.MR0 = mr0; r.FR0 = fr0; r.NR = nrr; r.FR1 = fr1;
     // formula-uniform parts of the edge and centre segments (the rest stays with the generic near kernel):
     //   edge, no core : the tile is only partly inside the extent, but |z|^2 >= Z2 on all of it
     //   centre, full  : the tile is inside the extent; bins with |z|^2 < Z2 exist
@@ -918,6 +933,21 @@ __global__ void __launch_bounds__(256) range_kernel(Params p, Levels lv, const i
         r.CL = min(max(idx_of(p, keys, n_act, jLmin), ml1), mr0);
         r.CR = min(max(idx_of(p, keys, n_act, jRmax + 1), r.CL), mr0);
     }
+    // node-handled lines (this tile's nodes or an ancestor's): a prefix of the left interior classes and a
+    // suffix of the right ones.  With core_nodes the prefix / suffix may reach into the centre class [CL, CR) (separated
+    // tiles of the core outside the inner region): every class in between gives way
+    int32_t nl = fl0, nrr = fr1;
+    if (lv.n_levels > 0) {
+        const NodeKeys k = node_keys(p, w0, wb);
+        const bool core = p.core_nodes && p.mode == 0;
+        nl = min(max(idx_of(p, keys, n_act, k.upL + 1), fl0), core ? r.CR : ml1);
+        nrr = max(min(idx_of(p, keys, n_act, k.dnR), fr1), core ? max(r.CL, nl) : mr0);
+    }
+    fl1 = max(fl1, nl);
+    fr0 = min(fr0, nrr);
+    ml1 = max(ml1, nl);  r.CL = max(r.CL, nl);       // (no-ops unless core_nodes)
+    mr0 = min(mr0, nrr); r.CR = max(min(r.CR, nrr), r.CL);
+    r.FL0 = fl0; r.NL = nl; r.FL1 = fl1; r.ML1 = ml1; r.MR0 = mr0; r.FR0 = fr0; r.NR = nrr; r.FR1 = fr1;
     // lane-pass candidates (centre_setup, hk_centre.cuh): innermost bins lie within sqrt(ZG) alpha_D of the centre
     // (z3_for <= HK_ZG; the binned Gaussian: 1/2 + 6 alpha_D), or within the whole core of a line narrower than
     // 0.224 kb/2 bins (25 alpha_D < 5.6 kb/2 bins); centre_setup's own test is 0.2 % generous, kappa3 0.5 %

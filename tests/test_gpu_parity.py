@@ -304,6 +304,7 @@ def test_node_kernels_agree(B, cfg, n):
         op = B.Opacity(*grid)
         op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
         op.set_node_kernel(entry_stationary)
+        op.set_core_nodes(False)             # (the core at nodes exists in the line-stationary kernel only)
         ks.append(op.compute(_to_cuda(lines), cut).cpu().numpy())
         torch.cuda.synchronize()
         sts.append(op.stats() if not entry_stationary else None)       # (only the line-stationary kernel counts its pairs)
@@ -314,6 +315,38 @@ def test_node_kernels_agree(B, cfg, n):
         assert (sts[0]["n_unsorted"] == 0) == bool((nu0[1:] >= nu0[:-1]).all())
     big = ks[1] >= 1e-8 * ks[1].max()
     assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 1e-6
+
+
+@pytest.mark.parametrize("cfg,n", [(2, 20_000), (3, 200_000), (4, 6_000), (1, None)])
+def test_core_at_nodes_on_vs_off(B, cfg, n):
+    """hk_set_core_nodes: separated tiles of the core (|z|^2 >= 49 on all of them) through the node hierarchy, their node
+    values from the 4-point Gauss-Hermite form, against direct evaluation of every core bin by the centre kernels.  Both
+    against the oracle on all bins; the pairs that moved are counted; the two spectra differ by the interpolation error
+    (tests/test_nodes.py: <= 1.3e-5) plus the node record's quantisation."""
+    lines, cond, grid, cut = _mini(cfg, n)
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    ks, sts = [], []
+    for on in (True, False):
+        op = B.Opacity(*grid)
+        op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+        op.set_core_nodes(on)
+        ks.append(op.compute(_to_cuda(lines), cut).cpu().numpy())
+        st = op.stats()
+        sts.append(st)
+        assert st["n_evals"] == evals
+        rel, ab, _ = check_parity(ks[-1], k_ref, what=f"config {cfg}, core at nodes {on}")
+        print(f"config {cfg} core at nodes {on}: rel={rel:.2e} abs={ab:.2e} node pairs {st['n_pairs_node']} (core {st['n_pairs_node_core']}) "
+              f"centre slots {st['n_pairs_centre']}")
+        op.close()
+    assert sts[1]["n_pairs_node_core"] == 0
+    if cfg in (2, 4):                        # 0.01 cm^-1 grids: the core spans several level-0 tiles
+        assert sts[0]["n_pairs_node_core"] > 0
+    if sts[0]["n_pairs_node_core"] > 0:
+        assert sts[0]["n_pairs_centre"] < sts[1]["n_pairs_centre"] and sts[0]["n_pairs_node"] > sts[1]["n_pairs_node"]
+    else:                                    # (cores narrower than the separation distance: nothing to move)
+        assert sts[0]["n_pairs_centre"] == sts[1]["n_pairs_centre"] and sts[0]["n_pairs_node"] == sts[1]["n_pairs_node"]
+    big = k_ref >= 1e-8 * k_ref.max()
+    assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 4e-5
 
 
 @pytest.mark.parametrize("sep", [B_SEP_MIN, 2.0, 3.0, 4.0, 6.0])
@@ -397,6 +430,7 @@ def test_batched_conditions(B):
         check_parity(kb[c].cpu().numpy(), k_ref, what=f"batch condition {c}")
         op1 = B.Opacity(*grid)
         op1.set_conditions(T[c], P[c], cond["mass_amu"], Q[c])
+        op1.set_core_nodes(False)            # (a batch keeps the core out of the node hierarchy: its ranges serve several conditions)
         k1 = op1.compute(dl, cut)
         torch.cuda.synchronize()
         big = k_ref >= 1e-8 * k_ref.max()

@@ -7,7 +7,11 @@ against the fp64 oracle's profile -- no CUDA code involved:
     budgets), and degrades as the separation shrinks (why the library refuses a separation below its default - 1/4);
  2. the restriction of a degree-(P-1) polynomial from a parent tile's nodes to its two children's nodes is exact,
     so the downward pass adds no error;
- 3. a sum of interpolants is the interpolant of the sum (linearity), which is what lets lines share node sums.
+ 3. a sum of interpolants is the interpolant of the sum (linearity), which is what lets lines share node sums;
+ 4. "the core at nodes" (hk_set_core_nodes): the same interpolant stays accurate INSIDE the core, as long as the tile is
+    separated and holds no bin with |z|^2 < 49 -- the Voigt profile is entire in x, and beyond |x| = 7 its Gaussian part
+    is 1e-21 of the Lorentzian wing, whose pole sets the convergence rate exactly as in the wings: <= 1.3e-5 for any
+    width and damping; and a tile that reaches into the inner region (|z| ~ 3) is NOT resolved (the threshold matters).
 """
 import numpy as np
 import pytest
@@ -74,6 +78,30 @@ def test_chebyshev_interpolant_of_a_separated_line(W, sep, tol):
     assert sep != SEP or worst <= 6.1e-6                                  # the default pair
     if sep < SEP:
         assert worst > 1.0e-5        # closer tiles really are worse: the separation threshold matters
+
+
+@pytest.mark.skipif(P != 12, reason="measured for the library's 12 nodes at 2 half-widths")
+@pytest.mark.parametrize("W", [64, 128, 1024])
+def test_chebyshev_interpolant_inside_the_core(W):
+    b, xi, xn = tile_coords(W)
+    hc, hw = 0.5 * (W - 1), 0.5 * W
+    worst, worst_inner = 0.0, 0.0
+    for side in (-1.0, 1.0):
+        for extra in (0.0, 0.05, 0.2, 0.5, 1.0, 2.0):
+            pos = hc + side * ((SEP + extra) * hw + 0.37)                 # separated: >= SEP half-widths from the tile centre
+            dmin = np.abs(b - pos).min()
+            for xmin in (7.0, 7.5, 9.0, 12.0, 18.0, 24.9):                # nearest bin at |x| = xmin Doppler widths: |z|^2 >= 49
+                a = dmin / xmin
+                for y in (1e-4, 1e-2, 0.1, 0.5, 1.0, 2.0, 4.0, 10.0):
+                    exact = voigt_bins(b - pos, y * a, a)
+                    interp = bary(voigt_bins(xn - pos, y * a, a), xi)
+                    worst = max(worst, np.abs(interp / exact - 1.0).max())
+            a = dmin / 3.0                                                # the tile reaches |x| = 3: inside the inner region
+            exact = voigt_bins(b - pos, 0.01 * a, a)
+            interp = bary(voigt_bins(xn - pos, 0.01 * a, a), xi)
+            worst_inner = max(worst_inner, np.abs(interp / exact - 1.0).max())
+    assert worst <= 1.3e-5, worst
+    assert worst_inner > 1.0e-4, worst_inner
 
 
 def test_parent_to_child_restriction_is_exact():
