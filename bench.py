@@ -261,7 +261,8 @@ def _kernel_flops(st):
     """Algorithmic FLOPs per accumulation kernel (FLOPs of the formula evaluated, per evaluation the
     definition or the node scheme requires; masked-out slots and idle lanes count nothing) -> {phase: (kernel, flops)}."""
     core = st["n_evals_core"]
-    n_gh4 = core - st["n_evals_gh6"] - st["n_evals_trap"]
+    # (core bins of node-handled tiles are covered by interpolation: the row kernel does not evaluate them)
+    n_gh4 = core - st["n_evals_gh6"] - st["n_evals_trap"] - st["n_evals_core_nodes"]
     n_trap = st["n_evals_trap"] - st["n_evals_gh10"]
     g10_row = st["n_evals_gh10_row"]
     g10_lane = st["n_evals_gh10"] - g10_row
@@ -275,7 +276,7 @@ def _kernel_flops(st):
         # half of a direct edge tile is inside the extent; separated edge tiles are evaluated at 8 nodes per extent end
         "edge": (f"edge_kernel<{kb}> + edge_node_kernel", FLOP["mid"] * (0.5 * st["n_pairs_edge"] + HK_NODES * st["n_pairs_edge_node"])),
         # line centres, rows: two-term outside the core, Gauss-Hermite 4 / 6 rings, the 10-point class of wide lines
-        "centre": (f"centre_row_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - core, 0) + FLOP["gh4"] * n_gh4
+        "centre": (f"centre_row_kernel<{kb}>", FLOP["mid"] * max(st["n_pairs_centre"] - (core - st["n_evals_core_nodes"]), 0) + FLOP["gh4"] * n_gh4
                    + FLOP["gh6"] * st["n_evals_gh6"] + FLOP["gh10"] * g10_row),
         # line centres, innermost bins: trapezoid rule with pole term (y < 1.8), 10-point rule of narrow lines
         "lane": (f"centre_lane_kernel<{kb}>", FLOP["gh10"] * g10_lane + FLOP["trap"] * n_trap),
@@ -473,7 +474,7 @@ def run_ours(args):
            "evals_per_step": st["n_evals"],
            "evals_by_region": {"far": st["n_evals_far"], "mid": st["n_evals_mid"], "core": st["n_evals_core"],
                                "core_gh6": st["n_evals_gh6"], "core_trap": st["n_evals_trap"], "core_gh10": st["n_evals_gh10"],
-                               "core_gh10_row": st["n_evals_gh10_row"]},
+                               "core_gh10_row": st["n_evals_gh10_row"], "core_at_nodes": st["n_evals_core_nodes"]},
            "pairs_by_kernel": {"node_tiles": st["n_pairs_node"], "node_tiles_core": st["n_pairs_node_core"], "far": st["n_pairs_far"], "mid": st["n_pairs_mid"],
                                "edge": st["n_pairs_edge"], "edge_node_ends": st["n_pairs_edge_node"], "centre": st["n_pairs_centre"], "near": st["n_pairs_near"]},
            "bins_per_lane": st["bins_per_lane"], "sorted_input": st["n_unsorted"] == 0,

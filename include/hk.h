@@ -89,6 +89,8 @@ typedef struct {
     int64_t n_pairs_node_far; /* of n_pairs_node: |z|^2 >= HK_Z1 on the whole tile, evaluated with one asymptotic term */
     int64_t n_unsorted;    /* adjacent pairs of the input list out of centre-bin order (0: the list arrived sorted and the
                               radix sort was skipped on the device) */
+    int64_t n_evals_core_nodes; /* of n_evals_core: bins of tiles the node hierarchy handles (hk_set_core_nodes): covered by the
+                                   interpolant of the tile's node values, not evaluated one by one */
     int64_t n_pairs_node_core; /* of n_pairs_node: the tile may hold bins with |z|^2 < HK_Z2 (a separated tile of the core, outside
                                   the inner region): evaluated at the nodes with the 4-point Gauss-Hermite form */
     int32_t scale_exp;     /* per-launch power-of-two scale applied to line strengths */

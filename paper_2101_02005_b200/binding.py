@@ -50,7 +50,7 @@ class hk_stats(C.Structure):
                                          "n_pairs_far", "n_pairs_mid", "n_pairs_near", "n_units_node", "n_units_edge",
                                          "n_units_centre", "n_pairs_edge", "n_pairs_centre", "n_pairs_node",
                                          "n_bins_node", "n_evals_gh10", "n_pairs_edge_node", "n_launches",
-                                         "n_plinth_illcond", "n_evals_gh10_row", "n_pairs_node_eval", "n_pairs_node_far", "n_unsorted", "n_pairs_node_core")] + \
+                                         "n_plinth_illcond", "n_evals_gh10_row", "n_pairs_node_eval", "n_pairs_node_far", "n_unsorted", "n_evals_core_nodes", "n_pairs_node_core")] + \
                [("scale_exp", C.c_int32), ("sort_bits", C.c_int32), ("bins_per_lane", C.c_int32), ("n_levels", C.c_int32),
                 ("single_pass", C.c_int32), ("reserved0", C.c_int32)]
 

@@ -53,6 +53,8 @@ struct hk_ctx {
     bool hint_ready;             // the DevHint of the bound workspace has been initialised
     bool in_batch;               // inside hk_compute_batch: tile ranges may serve later conditions with other widths
     int last_profile;
+    Params last_p;               // the launch constants and node levels of the last pass (for the on-demand counts)
+    Levels last_lv;
     bool regions_done;
     // totals over the blocks of the last hk_compute_host (0 after a plain hk_compute)
     bool host_totals;            // the counts of the last call are totals kept on the device (d_totals)
@@ -553,6 +555,7 @@ static int compute_impl(hk_ctx* ctx, const hk_lines* lines, int64_t n_lines, dou
     ctx->last_recA = recA; ctx->last_recB = recB; ctx->last_recN = recN; ctx->last_idx = idx_out;
     ctx->last_profile = p.profile;
     ctx->last_levels = lv.n_levels;
+    ctx->last_p = p; ctx->last_lv = lv;
 
     if (widths_only) {
         rewidth_kernel<<<grid_for(ctx, n), 256, 0, stream>>>(p, lines->A, lines->gamma_ref, lines->n_exp, idx_out, st, recA, recB,
@@ -1166,6 +1169,9 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
         if (nl > 0) {
             region_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_recA, ctx->last_recB, nl, ctx->last_profile,
                                                                                  ctx->last_kb, ctx->d_stats);
+            if (ctx->last_p.core_nodes && ctx->last_lv.n_levels > 0)
+                core_nodes_stats_kernel<<<grid_for(ctx, nl), 256, 0, ctx->last_stream>>>(ctx->last_p, ctx->last_lv, ctx->last_recA,
+                                                                                      ctx->last_recB, ctx->last_recN, nl, ctx->d_stats);
             HK_CUDA(cudaStreamSynchronize(ctx->last_stream));
         }
         ctx->regions_done = true;
@@ -1208,6 +1214,7 @@ int hk_get_stats(hk_ctx* ctx, hk_stats* host_out)
     host_out->n_pairs_node_core = (int64_t)d.pairs_node_core;
     host_out->n_pairs_node_eval = (int64_t)d.pairs_node_eval;
     host_out->n_evals_gh10_row = (int64_t)d.n_cnt_gh10_row;
+    host_out->n_evals_core_nodes = (int64_t)d.n_cnt_core_nodes;
     if (ctx->host_totals) {
         DevTotals t;
         std::memset(&t, 0, sizeof(t));

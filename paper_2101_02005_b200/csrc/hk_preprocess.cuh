@@ -81,6 +81,7 @@ struct DevStats {
     unsigned long long n_skipped, n_off_grid, n_evals, n_cnt_mid, n_cnt_core;  // cnt_*: evals with |z|^2 below Z1 / Z2
     unsigned long long n_cnt_gh6, n_cnt_trap;                                  // ... below Z4 / Z3
     unsigned long long n_cnt_gh10;                                             // of n_cnt_trap: lines with y >= HK_Y10
+    unsigned long long n_cnt_core_nodes;                                       // of n_cnt_core: bins of node-handled tiles (the core at nodes)
     unsigned long long n_cnt_gh10_row;                                         // of n_cnt_gh10: lines wide enough for the row kernel's 10-point class
     unsigned long long cmax_bits, cKmax_bits;                                  // max Lorentz amplitude / cK as double bits
     int32_t scale_exp;
@@ -797,6 +798,41 @@ __device__ __forceinline__ EdgeKeys edge_keys(const Params& p, int64_t w0, int64
     k.upL = edge_key_upL(p, w0, W);
     k.dnR = edge_key_dnR(p, w0, W);
     return k;
+}
+
+// The core at nodes, counted (on demand, for hk_get_stats): for each line, the bins with |z|^2 < Z2 that lie in tiles the
+// node hierarchy handles -- at level 0 or through an ancestor -- and are therefore covered by interpolation instead of
+// being evaluated one by one.  The same keys as range_kernel / node_range_kernel (node_keys), per line.
+__global__ void __launch_bounds__(256) core_nodes_stats_kernel(Params p, Levels lv, const float4* __restrict__ recA,
+                                                               const float4* __restrict__ recB, const float4* __restrict__ recN,
+                                                               int64_t n, DevStats* __restrict__ st)
+{
+    apply_shift_bound(p, st);
+    unsigned long long moved = 0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float4 ra = recA[i], rb = recB[i];
+        const int64_t ilo = __float_as_int(rb.y), ihi = __float_as_int(rb.z);
+        const double a2 = (double)rb.x, G2 = (double)ra.z;
+        const double t2 = (double)HK_Z2 * a2 - G2;
+        if (ihi < ilo || !(t2 > 0.0)) continue;
+        const double R = (double)sqrtf((float)t2);                        // (as region_stats_kernel counts the core)
+        const double pos = (double)__float_as_int(ra.x) + (double)ra.y;
+        const int64_t jc = __float_as_int(recN[i].x);
+        const int64_t b_lo = max(ilo, (int64_t)(floor(pos - R) + 1.0)), b_hi = min(ihi, (int64_t)(ceil(pos + R) - 1.0));
+        const int64_t wb = lv.w0;
+        for (int64_t t0 = (b_lo / wb) * wb; t0 <= b_hi; t0 += wb) {
+            bool handled = false;
+            for (int l = 0; l < lv.n_levels && !handled; ++l) {
+                const int64_t W = wb << l;
+                const NodeKeys k = node_keys(p, (t0 / W) * W, W);
+                handled = (jc >= k.loL && jc <= k.upL) || (jc >= k.dnR && jc <= k.hiR);
+            }
+            if (handled) moved += (unsigned long long)count_within(pos, R, max(ilo, t0), min(ihi, t0 + wb - 1));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) moved += __shfl_xor_sync(0xffffffffu, moved, o);
+    if ((threadIdx.x & 31) == 0 && moved) atomicAdd(&st->n_cnt_core_nodes, moved);
 }
 
 // index of the first sorted line with centre bin >= j (keys are jc - kmin)

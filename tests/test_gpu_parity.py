@@ -341,8 +341,13 @@ def test_core_at_nodes_on_vs_off(B, cfg, n):
     assert sts[1]["n_pairs_node_core"] == 0
     if cfg in (2, 4):                        # 0.01 cm^-1 grids: the core spans several level-0 tiles
         assert sts[0]["n_pairs_node_core"] > 0
+    assert sts[1]["n_evals_core_nodes"] == 0
     if sts[0]["n_pairs_node_core"] > 0:
         assert sts[0]["n_pairs_centre"] < sts[1]["n_pairs_centre"] and sts[0]["n_pairs_node"] > sts[1]["n_pairs_node"]
+        # the core bins now covered by interpolation lie in the (line, tile) slots that left the centre kernels
+        moved = sts[1]["n_pairs_centre"] - sts[0]["n_pairs_centre"]
+        assert 0 < sts[0]["n_evals_core_nodes"] <= moved
+        assert sts[0]["n_evals_core_nodes"] <= sts[0]["n_evals_core"] - sts[0]["n_evals_gh6"] - sts[0]["n_evals_trap"]
     else:                                    # (cores narrower than the separation distance: nothing to move)
         assert sts[0]["n_pairs_centre"] == sts[1]["n_pairs_centre"] and sts[0]["n_pairs_node"] == sts[1]["n_pairs_node"]
     big = k_ref >= 1e-8 * k_ref.max()
