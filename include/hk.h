@@ -117,6 +117,8 @@ enum { HK_PH_PREPROCESS = 0, HK_PH_SORT = 1, HK_PH_RANGES = 2, HK_PH_NODE = 3, H
 #define HK_NODES 12    /* Chebyshev nodes per tile of the separated-tile evaluation; 8, 10 or 12 */
 #endif
 #define HK_NODE_SEP (HK_NODES == 8 ? 4.0 : HK_NODES == 10 ? 2.5 : 2.0) /* default separation, tile half-widths: interpolation error <= 6e-6 */
+#define HK_NODE_SEP_PLINTH (HK_NODE_SEP + 1.0) /* smallest separation used with plinth removal (hk_set_plinth): ~3e-8 of the
+                                                  unsubtracted value, which the subtraction amplifies towards the extent ends */
 
 /* Grid: bin i is the POINT nu_i = numin + i*dnu (R8, R9).  HK_EINVAL if dnu <= 0,
  * numax <= numin, a non-finite argument, N < 1 or N too large. */
@@ -169,11 +171,16 @@ int hk_set_cut_mode(hk_ctx* ctx, int mode);
  * 1e-6 (inside the core) of ITSELF.  While every line's value at its cutting length is small against its peak,
  * V(cut) <= V(0) / HK_PLINTH_RATIO -- the normal use: a cut of many half-widths -- the SUBTRACTED opacity meets the
  * tolerance of the library (1e-4 per bin relative to the result, 1e-8 max(k) below that: the bins next to the extent's
- * ends, where the difference vanishes, fall under the absolute branch).  A line that does not is counted in
+ * ends, where the difference vanishes, fall under the absolute branch) up to the ROUNDING of its two terms, 2^-22
+ * (HK_PLINTH_ROUNDING) of the opacity before removal -- which shows only where an isolated line's subtracted value is
+ * below ~0.2 % of its unsubtracted one and still above 1e-8 max(k), the last bins before an extent end.  Separated tiles
+ * are evaluated at HK_NODE_SEP_PLINTH half-widths (interpolation error 3e-8 instead of 6e-6 of the unsubtracted value:
+ * it would not cancel against the directly evaluated plinth).  A line that does not is counted in
  * hk_stats.n_plinth_illcond (cut inside the line's core, or shorter than ~23 Lorentz half-widths); in the bins such
  * lines dominate the result is then good to 1e-4 of the opacity BEFORE removal only -- no fp32 evaluation can do better
  * -- and a caller who needs more must use a longer cut. */
 #define HK_PLINTH_RATIO 512.0
+#define HK_PLINTH_ROUNDING 2.384185791015625e-07 /* 2^-22 */
 int hk_set_plinth(hk_ctx* ctx, int on);
 
 /* Device scratch the caller must provide for hk_compute with up to n_lines lines. */

@@ -239,6 +239,11 @@ Params make_params(const hk_ctx* c, double cut, int32_t chunk, bool hitran = fal
     p.chunk_lane = 16384;
     p.sep = c->node_sep;
     p.plinth = (c->plinth && !p.uncut) ? 1 : 0;
+    // Plinth removal subtracts each line's value at its cutting length, evaluated directly: towards the extent ends
+    // V - V(cut) is a small fraction of V, and the interpolation error of the node scheme (6e-6 of V at 2 half-widths),
+    // which does not cancel against the plinth, would be a large one of the difference.  At 3 half-widths the
+    // interpolant is good to ~3e-8 (2.8e-7 at 2.5, 3e-9 at 4: tests/test_nodes.py), below the rounding of the two terms.
+    if (p.plinth) p.sep = std::fmax(p.sep, HK_NODE_SEP_PLINTH);
     p.cut_bins = cb;
     p.mode = c->debug_mode;
     return p;

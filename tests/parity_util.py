@@ -43,6 +43,23 @@ def check_parity_plinth(k_gpu, k_ref, k_raw, rel=REL_TOL, floor=FLOOR, what=""):
     return worst
 
 
+def check_parity_subtracted(k_gpu, k_ref, k_raw, rel=REL_TOL, floor=FLOOR, rounding=2.0 ** -22, what=""):
+    """The accuracy contract of hk_set_plinth for well-conditioned lines (include/hk.h, HK_PLINTH_ROUNDING): the north_star
+    pair on the SUBTRACTED opacity, plus the rounding of the two fp32 terms of the difference, 2^-22 of the opacity before
+    removal (one to two fp32 ulps of it: what no fp32 evaluation of V - V(cut) can avoid).  Returns the worst relative
+    error among the bins of the relative regime."""
+    k_gpu = np.asarray(k_gpu, dtype=np.float64)
+    assert np.all(np.isfinite(k_gpu)), f"{what}: non-finite GPU output"
+    kmax = float(k_ref.max()) if k_ref.size else 0.0
+    err = np.abs(k_gpu - k_ref)
+    big = k_ref >= floor * kmax
+    bad = err > rel * np.where(big, k_ref, 0.0) + floor * kmax * (~big) + rounding * k_raw
+    worst = float((err[big] / k_ref[big]).max()) if big.any() else 0.0
+    assert not bad.any(), (f"{what}: {int(bad.sum())} bins beyond {rel:g} x subtracted k + 2^-22 x unsubtracted k "
+                           f"(worst relative {worst:.3e} at bin {int(np.argmax(np.where(big, err / np.maximum(k_ref, 1e-300), 0)))})")
+    return worst
+
+
 def sample_windows(N, n_windows, width, rng):
     """Stratified windows of `width` contiguous bins incl. the first and last."""
     if N <= n_windows * width:

@@ -14,7 +14,7 @@ torch = pytest.importorskip("torch")
 from oracle import hk_oracle as O
 from workload import linelists as W
 
-from parity_util import check_parity, check_parity_plinth, sample_windows
+from parity_util import check_parity, check_parity_plinth, check_parity_subtracted, sample_windows
 
 _HK_NODES = int(re.search(r"#define HK_NODES (\d+)", open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "..", "include", "hk.h")).read()).group(1))
 B_SEP_MIN = {8: 4.0, 10: 2.5, 12: 2.0}[_HK_NODES] - 0.25     # smallest node separation hk_set_node_separation accepts
@@ -488,11 +488,13 @@ def _oracle_illcond(lines, cond, grid, cut, slack=1.0):
 
 def _check_plinth(op, k, k_ref, k_raw, what):
     """The accuracy contract of hk_set_plinth (include/hk.h): while every line's value at its cutting length is below 1/512
-    of its peak (hk_stats.n_plinth_illcond == 0) the SUBTRACTED opacity meets the north_star pair; otherwise the opacity
-    before removal is the reference magnitude (R27)."""
+    of its peak (hk_stats.n_plinth_illcond == 0) the SUBTRACTED opacity meets the north_star pair, up to the rounding of
+    the two fp32 terms (2^-22 of the opacity before removal: seen only in the last bins before the extent end of an
+    isolated line, found by the randomised test at 300 seeds); otherwise the opacity before removal is the reference
+    magnitude (R27)."""
     in_core = op.stats()["n_plinth_illcond"]
     if in_core == 0:
-        return check_parity(k, k_ref, what=what + " (subtracted reference)")[0], in_core
+        return check_parity_subtracted(k, k_ref, k_raw, what=what + " (subtracted reference)"), in_core
     return check_parity_plinth(k, k_ref, k_raw, what=what + f" ({in_core} ill-conditioned lines)"), in_core
 
 
@@ -904,6 +906,8 @@ def test_randomised_entry_points(B, seed):
         tag = f"entry points {seed} {what}: cut {cut:g} plinth {plinth} grid {grid} n {n}"
         if plinth and in_core > 0:       # the contract of hk_set_plinth (hk.h): cut inside a line's core
             check_parity_plinth(np.asarray(k), ref, raw, what=tag)
+        elif plinth and ref.max() > 0:   # ... and for well-conditioned lines: the subtracted value, up to the rounding of its terms
+            check_parity_subtracted(np.asarray(k), ref, raw, what=tag)
         elif ref.max() > 0:
             check_parity(np.asarray(k), ref, what=tag)
 
