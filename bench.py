@@ -143,9 +143,11 @@ class OracleSample:
         """-> (seconds, evaluations)"""
         t0 = time.perf_counter()
         evals = 0
+        self.values = []                         # (first bin, oracle k on the window) of the last run
         for b0, sub in self.subs:
             bins = np.arange(b0, b0 + self.width, dtype=np.int64)
-            _, ev = self.O.opacity_bins(sub, self.cond, self.grid, self.cut, bins)
+            kw, ev = self.O.opacity_bins(sub, self.cond, self.grid, self.cut, bins)
+            self.values.append((b0, kw))
             evals += ev
         return time.perf_counter() - t0, evals
 
@@ -182,14 +184,23 @@ def _evals_per_line(dl, cfg, O):
     return total / float(nu0.numel())
 
 
-def cpu_baseline(dl, cfg, n_lines, seconds=15.0):
+def cpu_baseline(dl, cfg, n_lines, seconds=15.0, k_timed=None):
     samp = OracleSample(dl, cfg)
     width = samp.size_for(seconds)
     t, ev = samp.run()
     epl = _evals_per_line(dl, cfg, samp.O)
     rate = ev / t
+    check = None
+    if k_timed is not None:
+        # the oracle's values on the sampled windows against the output of the TIMED run itself (north_star: relative error
+        # where the oracle is at least 1e-8 of its largest sampled value -- a lower bound of max(k), so the stricter regime)
+        ref = np.concatenate([kw for _, kw in samp.values])
+        got = np.concatenate([k_timed[b0:b0 + kw.size] for b0, kw in samp.values])
+        big = ref >= 1e-8 * ref.max()
+        check = {"bins": int(ref.size), "max_rel_err": float(np.abs(got[big] / ref[big] - 1.0).max()) if big.any() else 0.0,
+                 "tolerance": 1e-4}
     return {"value": rate / epl, "unit": UNIT, "cores": samp.O.num_threads(), "kind": "oracle",
-            "evals_per_s": rate, "seconds": t,
+            "evals_per_s": rate, "seconds": t, "timed_output_vs_oracle": check,
             "sample": (f"{len(samp.subs)} stratified windows x {width} bins, every bin summed over all lines within its cut "
                        f"({ev:.3e} Voigt evaluations); lines/s extrapolated = evals/s / ({epl:.1f} evals per line)")}
 
@@ -419,6 +430,7 @@ def run_ours(args):
     sampler = ClockSampler(gpu_id) if rank == 0 else None
     step_ms, phases, st, k = _timed(op, dl, cut, args.steps, 0, flush, barrier)
     clocks = sampler.stop() if sampler else None
+    k_timed_host = k.cpu().numpy()                     # the timed run's own output: checked against the oracle's sampled windows below
     total_ms = max_over_ranks(float(sum(step_ms)), dist, "cuda")
     value = replicas_value(n, args.steps, world, total_ms)
 
@@ -575,7 +587,7 @@ def run_ours(args):
     if not args.no_cpu_baseline and world == 1:
         if dl is None:
             dl = W.make_lines(cfg, n=n, seed=0, device="cuda")
-        out["cpu_baseline"] = cpu_baseline(dl, cfg, n)
+        out["cpu_baseline"] = cpu_baseline(dl, cfg, n, k_timed=k_timed_host)
 
     print(json.dumps(out))
     if dist is not None:
