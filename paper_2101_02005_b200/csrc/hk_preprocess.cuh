@@ -151,15 +151,6 @@ __device__ __forceinline__ bool finite6(double a, double b, double c, double d, 
     return isfinite(a) && isfinite(b) && isfinite(c) && isfinite(d) && isfinite(e) && isfinite(f);
 }
 
-// the bin a centre falls in, as line_math computes it (same operations, same order)
-__device__ __forceinline__ int64_t centre_bin(const Params& p, double ctr)
-{
-    const double big = 4.0e18;
-    double c = floor(__ddiv_rn(__dsub_rn(ctr, p.numin), p.dnu));
-    c = fmin(fmax(c, -big), big);
-    return (int64_t)c;
-}
-
 // a / dnu, correctly rounded like the IEEE division the oracle performs, in three operations: with y = RN(1/dnu)
 // (p.inv_dnu, an IEEE division on the host) and q0 = RN(a y) -- within one ulp of the quotient -- the residual
 // r = a - dnu q0 is exact under FMA and RN(q0 + r y) is the correctly rounded quotient (Markstein's theorem).  A
@@ -170,6 +161,15 @@ __device__ __forceinline__ double div_by_dnu(const Params& p, double a)
     const double r = __fma_rn(-p.dnu, q0, a);
     const double q1 = __fma_rn(r, p.inv_dnu, q0);
     return fabs(q0) < 4.6e18 ? q1 : q0;
+}
+
+// the bin a centre falls in, as line_math computes it (same operations, same order)
+__device__ __forceinline__ int64_t centre_bin(const Params& p, double ctr)
+{
+    const double big = 4.0e18;
+    double c = floor(div_by_dnu(p, __dsub_rn(ctr, p.numin)));
+    c = fmin(fmax(c, -big), big);
+    return (int64_t)c;
 }
 
 struct LineOut {
