@@ -354,6 +354,41 @@ def test_core_at_nodes_on_vs_off(B, cfg, n):
     assert np.abs(ks[0][big] / ks[1][big] - 1.0).max() <= 4e-5
 
 
+@pytest.mark.parametrize("aD_bins", [0.7, 3.0, 9.0, 25.0, 80.0])
+@pytest.mark.parametrize("y", [1e-3, 0.2, 1.2, 6.0])
+def test_core_at_nodes_across_widths(B, aD_bins, y):
+    """The core at nodes over the whole range of geometries: Doppler widths from under a bin to more than a level-0 tile
+    (so that the separated tiles of the core are found at level 0, or only at higher levels), damping from next to none
+    to Lorentz-dominated; isolated lines and a dense clump, all bins against the oracle."""
+    rng = np.random.default_rng(int(aD_bins * 10) + int(y * 1000))
+    dnu, nbins = 0.005, 60_000
+    grid = (20000.0, 20000.0 + nbins * dnu, dnu)
+    cut = 60.0                                                    # 12000 bins: several levels of the hierarchy
+    T, mass = 1000.0, 30.0
+    beta = math.sqrt(2 * 1.380649e-16 * T / (mass / 6.02214076e23)) / 2.99792458e10
+    # the mass that gives alpha_D = aD_bins * dnu at 20150 cm^-1
+    mass = mass * (beta * 20150.0 / (aD_bins * dnu)) ** 2
+    n = 300
+    nu0 = np.sort(np.concatenate([rng.uniform(grid[0] - 5.0, grid[1] + 5.0, n - 60), rng.normal(20150.0, 0.3, 60)]))
+    aD = aD_bins * dnu
+    lines = _simple_lines(nu0, A=10 ** rng.uniform(-1, 2, n), gamma_ref=np.full(n, y * aD), n_exp=np.zeros(n))
+    cond = dict(T=T, P_atm=1.0, mass_amu=mass, Q=50.0)
+    _, gL, aDs, _ = O.line_params(lines, cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    assert abs(np.median(aDs) / dnu / aD_bins - 1.0) < 0.02 and abs(np.median(gL / aDs) / y - 1.0) < 0.05
+    op = B.Opacity(*grid)
+    op.set_conditions(cond["T"], cond["P_atm"], cond["mass_amu"], cond["Q"])
+    k = op.compute(_to_cuda(lines), cut).cpu().numpy()
+    st = op.stats()
+    k_ref, evals = O.opacity_grid(lines, cond, grid, cut)
+    assert st["n_evals"] == evals
+    rel, ab, _ = check_parity(k, k_ref, what=f"core at nodes, alpha_D {aD_bins} bins, y {y}")
+    if aD_bins >= 3.0:                       # the core (25 alpha_D) reaches beyond the two tiles next to the line
+        assert st["n_pairs_node_core"] > 0 and st["n_evals_core_nodes"] > 0
+    print(f"alpha_D {aD_bins} bins, y {y}: rel={rel:.2e} abs={ab:.2e} core pairs {st['n_pairs_node_core']} "
+          f"core bins at nodes {st['n_evals_core_nodes']} of {st['n_evals_core']}")
+    op.close()
+
+
 @pytest.mark.parametrize("sep", [B_SEP_MIN, 2.0, 3.0, 4.0, 6.0])
 def test_node_separation_sweep(B, sep):
     """The node hierarchy at other separations (fewer / more pairs at nodes) against the oracle, down to the smallest
